@@ -1,0 +1,426 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself through the same formula: each uses a closed form,
+a library routine (numpy FFT, scipy spherical harmonics / B-splines / Chebyshev), brute force, a
+finite difference of the oracle's own ENERGY / CHARGES, or an exact invariant.
+"""
+import os
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import qnep_inputs as I
+
+K = 14.3996454784
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")) as _f:
+    for _line in _f:
+        if _line.strip() and not _line.startswith("#"):
+            _k, _v = _line.split()[:2]
+            GOLD[_k] = float(_v)
+
+
+def rel_rms(a, b):
+    return np.sqrt(((a - b) ** 2).sum() / (b ** 2).sum())
+
+
+# ---------------------------------------------------------------- P1 Madelung
+def test_madelung_converged(oracle):
+    pos, types, box = I.rocksalt_lattice(4, 2.82)
+    q = np.where(types == 0, 1.0, -1.0)
+    es = I.EsDesc(method=1, alpha=0.6, ewald_nmax2=144)
+    r = oracle.electrostatics(pos, q, box, 11.0, 1, es)
+    M = -r["U"].sum() * 2.82 / (K * 32)
+    assert abs(M - GOLD["madelung_nacl"]) < 2e-6
+    # perfect lattice: every force vanishes, phi_i = -/+ M K / r0
+    assert np.abs(r["F"]).max() < 1e-9
+    assert np.allclose(r["phi"] * q, -GOLD["madelung_nacl"] * K / 2.82, rtol=2e-6)
+
+
+def test_madelung_paper_defaults(oracle):
+    """alpha = pi/r_c (:91) and kmax = 2 pi alpha (:110) give 'approximately 1e-5'."""
+    pos, types, box = I.rocksalt_lattice(4, 2.82)
+    q = np.where(types == 0, 1.0, -1.0)
+    es = I.EsDesc(method=1, alpha=-1.0, ewald_nmax2=0)
+    r = oracle.electrostatics(pos, q, box, 6.0, 1, es)
+    M = -r["U"].sum() * 2.82 / (K * 32)
+    err = abs(M - GOLD["madelung_nacl"])
+    assert 1e-6 < err < 5 * GOLD["ewald_accuracy"]
+
+
+# ------------------------------------------- P2 Ewald vs brute-force image sum
+def _cubic_cluster(L):
+    """Neutral cell with full cubic point symmetry: dipole and quadrupole vanish, so the
+    shell-by-shell Coulomb sum converges fast and has no surface term."""
+    a, b = 0.21 * L, 0.13 * L
+    pts, q = [[0.0, 0.0, 0.0]], [-6.0 + 8 * 0.5]
+    for ax in range(3):
+        for s in (-1, 1):
+            v = [0.0, 0.0, 0.0]
+            v[ax] = s * a
+            pts.append(v)
+            q.append(1.0)
+    for sx in (-1, 1):
+        for sy in (-1, 1):
+            for sz in (-1, 1):
+                pts.append([sx * b, sy * b, sz * b])
+                q.append(-0.5)
+    pos = (np.array(pts) + L / 2).T.copy()
+    q = np.array(q)
+    assert abs(q.sum()) < 1e-14
+    return pos, q
+
+
+def test_ewald_vs_bruteforce_images(oracle):
+    L = 7.0
+    pos, q = _cubic_cluster(L)
+    n = pos.shape[1]
+    box = np.diag([L, L, L]).ravel()
+    es = I.EsDesc(method=1, alpha=0.75, ewald_nmax2=196)
+    r = oracle.electrostatics(pos, q, box, 13.9, 1, es)
+    # brute force: sum over image cells in growing cubes
+    M = 12
+    g = np.arange(-M, M + 1)
+    S = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3) * L
+    d = pos.T[:, None, None, :] - pos.T[None, :, None, :] - S[None, None, :, :]   # r_i - r_j - s
+    dist = np.linalg.norm(d, axis=-1)
+    qq = q[:, None, None] * q[None, :, None]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        inv = np.where(dist > 0, 1.0 / dist, 0.0)
+        U = 0.5 * K * (qq * inv).sum()
+        F = K * (qq[..., None] * d * inv[..., None] ** 3).sum(axis=(1, 2))
+    assert abs(U - r["U"].sum()) < 1e-7 * abs(U)
+    assert rel_rms(r["F"].T, F) < 1e-6
+    assert np.abs(F).max() > 0.1     # the test is not vacuous
+
+
+# ----------------------------------------------- P3 / P4 split consistency
+def _random_charges(n, L, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    pos = rng.uniform(0, L, size=(3, n))
+    q = rng.normal(size=n)
+    q -= q.mean()
+    return pos, q
+
+
+def test_ewald_alpha_independence_and_phi_identity(oracle):
+    L = 14.0
+    pos, q = _random_charges(40, L, 7)
+    box = np.diag([L, L, L]).ravel()
+    res = []
+    for alpha, nmax2 in ((0.55, 196), (0.75, 400)):
+        r = oracle.electrostatics(pos, q, box, 13.5, 1, I.EsDesc(method=1, alpha=alpha, ewald_nmax2=nmax2))
+        res.append(r)
+        # P4: U^ES = 1/2 sum q_i phi_i (phi includes phi^s, and 1/2 sum q phi^s = U^s)
+        assert abs(0.5 * (q * r["phi"]).sum() - r["U"].sum()) < 1e-10 * abs(r["U"].sum())
+        # Eq. 10 closed form
+        assert np.isclose(r["U"][2], -K * alpha / np.sqrt(np.pi) * (q ** 2).sum(), rtol=1e-13)
+    a, b = res
+    assert abs(a["U"].sum() - b["U"].sum()) < 1e-7 * abs(a["U"].sum())
+    assert rel_rms(a["F"], b["F"]) < 1e-7
+    assert np.abs(a["phi"] - b["phi"]).max() < 1e-6
+    assert np.abs(a["W"] - b["W"]).max() < 1e-6 * np.abs(a["W"]).max()
+    # the parts themselves differ (the test is not vacuous)
+    assert abs(a["U"][1] - b["U"][1]) > 1e-2
+
+
+def test_static_force_and_virial_are_derivatives_of_the_energy(oracle):
+    """Eq. 15/18 = -dU/dr and Eq. 12/22 = -dU/d(strain) for fixed charges (mode 1, converged)."""
+    L = 12.0
+    pos, q = _random_charges(24, L, 11)
+    box = np.diag([L, L, L]).ravel()
+    es = I.EsDesc(method=1, alpha=0.8, ewald_nmax2=225)
+    rc = 5.9      # alpha rc = 4.7: the truncation jump K erfc(4.7)/rc is ~1e-10 (S17)
+    r0 = oracle.electrostatics(pos, q, box, rc, 1, es)
+    h = 1e-5
+    for (a, i) in ((0, 3), (1, 7), (2, 20)):
+        p1, p2 = pos.copy(), pos.copy()
+        p1[a, i] += h
+        p2[a, i] -= h
+        fd = -(oracle.electrostatics(p1, q, box, rc, 1, es)["U"].sum()
+               - oracle.electrostatics(p2, q, box, rc, 1, es)["U"].sum()) / (2 * h)
+        assert abs(fd - r0["F"][a, i]) < 2e-7 * max(1.0, abs(fd))
+    # finite strain, integer k-set fixed (nmax2 criterion)
+    for (a, b) in ((0, 0), (1, 2), (2, 1), (0, 1)):
+        eps = np.zeros((3, 3))
+        eps[a, b] = h
+        def energy(sign):
+            Fm = np.eye(3) + sign * eps
+            return oracle.electrostatics(Fm @ pos, q, (box.reshape(3, 3) @ Fm.T).ravel(), rc, 1, es)["U"].sum()
+        fd = -(energy(1) - energy(-1)) / (2 * h)
+        assert abs(fd - r0["W"][a, b]) < 5e-7 * np.abs(r0["W"]).max()
+    assert np.allclose(r0["W"], r0["W"].T, atol=1e-10)
+
+
+# ------------------------------------------------------------- P12 FFT, W, d(z)
+def test_fft_vs_numpy(oracle):
+    rng = np.random.Generator(np.random.PCG64(3))
+    x = rng.normal(size=(8, 4, 16)) + 1j * rng.normal(size=(8, 4, 16))
+    assert np.allclose(oracle.fft3d(x, -1), np.fft.fftn(x), atol=1e-12)
+    assert np.allclose(oracle.fft3d(x, +1), np.fft.ifftn(x) * x.size, atol=1e-12)
+
+
+def test_bspline_vs_library_definition(oracle):
+    from scipy.interpolate import BSpline
+    b = BSpline.basis_element(np.arange(6) - 2.5)      # centred cardinal B-spline of order 5
+    for dx in (-0.5, -0.31, 0.0, 0.123, 0.4999):
+        w = oracle.bspline5(dx)
+        ref = np.array([b(dx - o) if abs(dx - o) < 2.5 else 0.0 for o in (-2, -1, 0, 1, 2)])
+        ref = np.nan_to_num(ref)
+        assert np.allclose(w, ref, atol=1e-14), (dx, w, ref)
+        assert abs(w.sum() - 1.0) < 1e-14
+
+
+def test_alias_denominator_vs_brute_sum(oracle):
+    """G2: d(z) = sum_m sinc^10(x + pi m), z = sin x -- fixes the sign of the 17/189 term."""
+    m = np.arange(-4000, 4001)
+    for x in (0.1, 0.7, 1.2, np.pi / 2):
+        brute = (np.sinc((x + np.pi * m) / np.pi) ** 10).sum()
+        assert abs(oracle.alias_denominator(np.sin(x)) - brute) < 1e-13
+
+
+# --------------------------------------------------------------- P6 / P7 PPPM
+def test_pppm_adjointness_identity(oracle):
+    """U^k_mesh = 1/2 sum_i q_i phi^k_i exactly (Eq. 34 vs Eq. 38): pins the FFT normalisation (S11)
+    and that spreading and back-interpolation use the same W."""
+    L = 13.0
+    pos, q = _random_charges(50, L, 5)
+    box = np.diag([L, L, L]).ravel()
+    r = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=2, alpha=0.3, grid=(16, 16, 16)), want_rho=True)
+    assert abs(0.5 * (q * r["phi"]).sum() - r["U"][1]) < 1e-12 * abs(r["U"][1])
+    assert abs(r["rho"].sum() - q.sum()) < 1e-12          # W sums to one
+    assert np.abs(r["F"].sum(axis=1)).max() < 1e-10         # P9: static mesh force sums to zero
+    # phi^k is the exact charge-derivative of the mesh energy
+    h = 1e-5
+    for i in (0, 17):
+        q1, q2 = q.copy(), q.copy()
+        q1[i] += h
+        q2[i] -= h
+        es = I.EsDesc(method=2, alpha=0.3, grid=(16, 16, 16))
+        fd = (oracle.electrostatics(pos, q1, box, 6.0, 2, es)["U"][1]
+              - oracle.electrostatics(pos, q2, box, 6.0, 2, es)["U"][1]) / (2 * h)
+        assert abs(fd - r["phi"][i]) < 1e-8
+
+
+def test_pppm_converges_to_ewald(oracle):
+    """P7 / G2: rel. force error falls as the mesh is refined and is ~1e-5..1e-4 at h ~ 1 A (:280)."""
+    L = 16.0
+    pos, q = _random_charges(120, L, 9)
+    box = np.diag([L, L, L]).ravel()
+    ew = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=1, alpha=0.3, ewald_nmax2=169))
+    errs = []
+    for g in (16, 32, 64):
+        pm = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=2, alpha=0.3, grid=(g, g, g)))
+        errs.append((rel_rms(pm["F"], ew["F"]), abs(pm["U"][1] - ew["U"][1]) / abs(ew["U"][1]),
+                     rel_rms(pm["phi"], ew["phi"]), np.abs(pm["W"] - ew["W"]).max() / np.abs(ew["W"]).max()))
+    assert errs[0][0] < GOLD["pppm_accuracy"] and errs[0][1] < 2e-5 and errs[0][2] < 1e-4 and errs[0][3] < 1e-4
+    assert errs[1][0] < 3e-6 and errs[2][0] < 1e-7
+    assert errs[2][1] < 1e-8 and errs[2][2] < 1e-7
+
+
+# ------------------------------------------------ neighbours (a1): closed form + bins
+def test_neighbor_counts_on_lattice(oracle):
+    pos, types, box = I.rocksalt_lattice(4, 2.82)
+    for rc in (4.0, 6.0):
+        counts, _, _ = oracle.neighbors(pos, box, rc)
+        g = np.arange(-4, 5)
+        v = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+        d2 = (v ** 2).sum(1) * 2.82 ** 2
+        expect = int(((d2 > 0) & (d2 < rc * rc)).sum())
+        assert (counts == expect).all()
+
+
+def test_binned_neighbors_equal_brute_force(oracle):
+    rng = np.random.Generator(np.random.PCG64(17))
+    box = np.array([13.0, 0, 0, 1.5, 14.0, 0, -1.0, 2.0, 15.0])     # triclinic
+    pos = rng.uniform(-5, 20, size=(3, 400))
+    rc = 4.0
+    c0, j0, d0 = oracle.neighbors(pos, box, rc, use_bins=False, cap=96)
+    c1, j1, d1 = oracle.neighbors(pos, box, rc, use_bins=True, cap=96)
+    assert (c0 == c1).all() and c0.max() <= 96 and c0.min() > 0
+    for i in range(400):
+        a = sorted(zip(j0[i, :c0[i]], np.round(d0[i, :c0[i], 3], 9)))
+        b = sorted(zip(j1[i, :c1[i]], np.round(d1[i, :c1[i], 3], 9)))
+        assert a == b
+
+
+# --------------------------------------------------- P10 descriptors vs library Y_lm
+def test_descriptors_vs_spherical_harmonics(oracle):
+    """Independent route (S1): D_nl = 4 pi/(2l+1) sum_m |sum_j g_n(r_ij) Y_lm(rhat_ij)|^2 with scipy's
+    Y_lm and numpy's Chebyshev series -- the addition theorem must reproduce the Legendre double sum."""
+    from numpy.polynomial import chebyshev as Ch
+    try:
+        from scipy.special import sph_harm_y
+        Y = lambda l, m, theta, phi: sph_harm_y(l, m, theta, phi)
+    except ImportError:       # older scipy
+        from scipy.special import sph_harm
+        Y = lambda l, m, theta, phi: sph_harm(m, l, phi, theta)
+    w = I.config0()
+    m = w.model
+    p = w.params.astype(np.float64)
+    off = I.param_offsets(m)
+    nR, nA, Kb = m.n_max_r + 1, m.n_max_a + 1, m.basis_r + 1
+    cR = p[off["c_r"]:off["c_a"]].reshape(2, 2, nR, Kb)
+    cA = p[off["c_a"]:off["scaler"]].reshape(2, 2, nA, Kb)
+    D = oracle.descriptors(m, p, w.pos, w.types, w.box)
+    counts, jj, dd = oracle.neighbors(w.pos, w.box, m.rc_r, cap=48)
+
+    def g(c, r, rc):
+        x = 2 * (r / rc - 1) ** 2 - 1
+        fc = 0.5 * (1 + np.cos(np.pi * r / rc))
+        # sum_k c_k 1/2 (T_k(x) + 1) f_c
+        return 0.5 * (Ch.chebval(x, c) + c.sum()) * fc
+
+    for i in (0, 13, 40):
+        ti = w.types[i]
+        nb = [(jj[i, s], dd[i, s]) for s in range(counts[i])]
+        Dn = np.zeros(m.n_desc)
+        for n in range(nR):
+            Dn[n] = sum(g(cR[ti, w.types[j], n], d[3], m.rc_r) for j, d in nb)
+        ang = [(j, d) for j, d in nb if d[3] < m.rc_a]
+        for n in range(nA):
+            for l in range(1, m.l_max + 1):
+                tot = 0.0
+                for mm in range(-l, l + 1):
+                    A = 0.0
+                    for j, d in ang:
+                        theta = np.arccos(d[2] / d[3])
+                        phi = np.arctan2(d[1], d[0])
+                        A += g(cA[ti, w.types[j], n], d[3], m.rc_a) * Y(l, mm, theta, phi)
+                    tot += abs(A) ** 2
+                Dn[nR + n * m.l_max + (l - 1)] = 4 * np.pi / (2 * l + 1) * tot
+        assert np.allclose(D[i], Dn, rtol=1e-10, atol=1e-12)
+
+
+# --------------------------------------------------- P5 / P8 full model derivatives
+def _small_workload(mode, alpha):
+    w = I.config0(mode=mode)
+    w.es = replace(w.es, alpha=alpha, ewald_nmax2=36 if alpha < 0.5 else 300)
+    return w
+
+
+@pytest.mark.parametrize("mode,alpha", [(2, 0.3), (1, 0.8)])
+def test_forces_are_minus_energy_gradient(oracle, mode, alpha):
+    """Eq. 11, 14-19, 23 with the folding (:140) and S6: F = -dE/dr by central differences.
+    Mode 1 uses alpha r_c = 4.8 so the real-space cutoff jump is negligible (S17)."""
+    w = _small_workload(mode, alpha)
+    out = oracle.compute_workload(w, use_bins=False)
+    h = 1e-5
+    for (a, i) in ((0, 0), (1, 21), (2, 63)):
+        p1, p2 = w.pos.copy(), w.pos.copy()
+        p1[a, i] += h
+        p2[a, i] -= h
+        e1 = oracle.compute(w.model, w.params, w.es, p1, w.types, w.box, use_bins=False)["energy"]
+        e2 = oracle.compute(w.model, w.params, w.es, p2, w.types, w.box, use_bins=False)["energy"]
+        fd = -(e1 - e2) / (2 * h)
+        assert abs(fd - out["forces"][a, i]) < 2e-7 * max(1.0, abs(fd)), (fd, out["forces"][a, i])
+    assert np.abs(out["forces"]).max() > 0.05
+    assert np.abs(out["forces"].sum(axis=1)).max() < 1e-10          # P9
+    assert abs(out["charges"].sum() - w.model.q_total) < 1e-12      # P9, Eq. 33 (G3)
+    assert abs(out["energy_parts"]["k"]) > 1e-3                     # the charge path is exercised
+
+
+@pytest.mark.parametrize("mode,alpha", [(2, 0.3), (1, 0.8)])
+def test_virial_is_minus_strain_derivative(oracle, mode, alpha):
+    """Eq. 12 + Eq. 21-22: W = -dE/d(eps) under r -> (1+eps) r, cell -> (1+eps) cell, k-set fixed in integers."""
+    w = _small_workload(mode, alpha)
+    out = oracle.compute_workload(w, use_bins=False)
+    h = 1e-5
+    for (a, b) in ((0, 0), (2, 2), (0, 1), (2, 1)):
+        eps = np.zeros((3, 3))
+        eps[a, b] = h
+        def energy(sign):
+            Fm = np.eye(3) + sign * eps
+            return oracle.compute(w.model, w.params, w.es, Fm @ w.pos, w.types,
+                                  (w.box.reshape(3, 3) @ Fm.T).ravel(), use_bins=False)["energy"]
+        fd = -(energy(1) - energy(-1)) / (2 * h)
+        assert abs(fd - out["virial"][a, b]) < 1e-6 * np.abs(out["virial"]).max(), (fd, out["virial"][a, b])
+    assert np.allclose(out["virial"], out["virial"].T, atol=1e-9 * np.abs(out["virial"]).max())
+
+
+def test_translation_and_permutation_invariance(oracle):
+    w = I.config0(mode=1)
+    a = oracle.compute_workload(w, use_bins=False, want_bec=True)
+    shift = np.array([[0.3712], [-5.17], [13.09]])
+    b = oracle.compute(w.model, w.params, w.es, w.pos + shift, w.types, w.box, use_bins=False, want_bec=True)
+    assert abs(a["energy"] - b["energy"]) < 1e-10
+    assert np.abs(a["forces"] - b["forces"]).max() < 1e-10
+    assert np.abs(a["charges"] - b["charges"]).max() < 1e-12
+    assert np.abs(a["bec"] - b["bec"]).max() < 1e-10
+    perm = np.random.Generator(np.random.PCG64(1)).permutation(w.n_atoms)
+    c = oracle.compute(w.model, w.params, w.es, w.pos[:, perm], w.types[perm], w.box, use_bins=False)
+    assert abs(a["energy"] - c["energy"]) < 1e-10
+    assert np.abs(a["forces"][:, perm] - c["forces"]).max() < 1e-10
+
+
+# ------------------------------------------------------------- P13 limits
+def test_static_charge_limits(oracle):
+    w = I.config0(mode=1)
+    off = I.param_offsets(w.model)
+    H, D = w.model.n_neurons, w.model.n_desc
+    # (a) w1q = 0 -> uniform charges -> neutralised to zero -> pure NEP
+    p = w.params.copy()
+    for t in range(2):
+        base = off["nn"] + t * off["per_type"] + H * D + 2 * H
+        p[base:base + H] = 0.0
+    a = oracle.compute(w.model, p, w.es, w.pos, w.types, w.box, use_bins=False)
+    assert np.abs(a["charges"]).max() < 1e-15
+    assert a["energy"] == a["energy_parts"]["nep"]
+    # (b) w0 = 0 -> charges depend on the species only -> textbook fixed-charge Ewald forces
+    p = w.params.copy()
+    for t in range(2):
+        base = off["nn"] + t * off["per_type"]
+        p[base:base + H * D] = 0.0
+    b = oracle.compute(w.model, p, w.es, w.pos, w.types, w.box, use_bins=False)
+    q = b["charges"]
+    assert np.ptp(q[w.types == 0]) < 1e-14 and abs(q[w.types == 0][0] + q[w.types == 1][0]) < 1e-14
+    assert abs(q[0]) > 1e-3
+    s = oracle.electrostatics(w.pos, q, w.box, w.model.rc_r, 1, w.es)
+    assert np.abs(b["forces"] - s["F"]).max() < 1e-12
+    assert np.abs(b["virial"] - s["W"]).max() < 1e-11
+    assert abs(b["energy"] - b["energy_parts"]["nep"] - s["U"].sum()) < 1e-11
+
+
+# ------------------------------------------------------------- P11 BEC
+def test_bec_sum_rule_and_finite_difference_assembly(oracle):
+    """Eq. 28 (S12): sum_i Z_i = Q I, and Z assembled in python from FINITE-DIFFERENCED dq_i/dr_j."""
+    pos, types, box = I.rocksalt_lattice(3, 2.82)
+    rng = np.random.Generator(np.random.PCG64(23))
+    L = 14.0                                   # > 2 r_c: every (i, j) pair is seen through one image only
+    pos = pos * (L / box[0]) * 0.55 + rng.normal(0, 0.1, pos.shape) + 1.0
+    types = types.copy()
+    box = np.diag([L, L, L]).ravel()
+    model = I.ModelDesc(n_types=2, n_neurons=10, mode=2)
+    params = I.random_params(model, 5)
+    es = I.EsDesc(method=0)
+    n = pos.shape[1]
+    out = oracle.compute(model, params, es, pos, types, box, use_bins=False, want_bec=True, debug=True)
+    Z = out["bec"].reshape(3, 3, n)
+    qt = model.sqrt_eps_inf * out["charges"]
+    assert np.abs(Z.sum(axis=2) - qt.sum() * np.eye(3)).max() < 1e-12
+    # c[i][j][beta] = sqrt(eps) d q_i^raw / d r_j,beta  (j != i)
+    h = 1e-5
+    c = np.zeros((n, n, 3))
+    for j in range(n):
+        for b in range(3):
+            p1, p2 = pos.copy(), pos.copy()
+            p1[b, j] += h
+            p2[b, j] -= h
+            q1 = oracle.compute(model, params, es, p1, types, box, use_bins=False, debug=True)["q_raw"]
+            q2 = oracle.compute(model, params, es, p2, types, box, use_bins=False, debug=True)["q_raw"]
+            c[:, j, b] = model.sqrt_eps_inf * (q1 - q2) / (2 * h)
+    _, jj, dd = oracle.neighbors(pos, box, model.rc_r, cap=n)
+    Zfd = np.zeros((3, 3, n))
+    for i in range(n):
+        Zfd[:, :, i] += qt[i] * np.eye(3)
+        for j in range(n):
+            if j == i:
+                continue
+            rij = pos[:, j] - pos[:, i]
+            rij -= L * np.round(rij / L)
+            if np.linalg.norm(rij) >= model.rc_r:
+                continue
+            Zfd[:, :, i] += 0.5 * (np.outer(rij, c[i, j]) - np.outer(-rij, c[j, i]))
+    assert np.abs(Z - Zfd).max() < 5e-8
+    assert np.abs(Z - qt[None, None, :] * np.eye(3)[:, :, None]).max() > 1e-3
