@@ -1,0 +1,192 @@
+/*
+ * qnep.h -- C ABI of the B200-native qNEP force evaluation (arXiv 2601.19034).
+ *
+ * One call, qnep_compute(), evaluates for given positions, species and a periodic box
+ * the total energy (Eq. 4), forces (Eq. 11), total virial (Eq. 12 + Eq. 22),
+ * the neutralised partial charges (Eq. 1 second output node, Eq. 33) and, on request,
+ * the per-ion Born effective charge tensor (Eq. 28).  Every step runs in hand-written
+ * CUDA kernels for sm_100a inside this library; there is no CPU fallback, no cuFFT and
+ * no other library on the path.
+ *
+ * Conventions
+ *   - every function returns QNEP_OK (0) or a negative QNEP_ERR_* code; no C++ exception
+ *     crosses this boundary; on error the outputs are unspecified but nothing is written
+ *     out of bounds;
+ *   - "_dev" pointers are DEVICE pointers owned by the caller (e.g. PyTorch tensors);
+ *     "_host" pointers are HOST pointers owned by the caller and copied during the call;
+ *   - the handle owns its workspace and its copy of the model; all work is enqueued on the
+ *     caller's stream; qnep_compute() does not synchronise -- neighbour-capacity overflow
+ *     and skin violation are detected on the device and reported by the NEXT call on the
+ *     handle or by qnep_check() (which synchronises the stream);
+ *   - units: Angstrom, eV, elementary charge; 1/(4 pi eps0) = 14.3996454784 eV A / e^2.
+ */
+#ifndef QNEP_H
+#define QNEP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qnep_handle qnep_handle; /* opaque */
+
+enum {
+    QNEP_OK = 0,
+    QNEP_ERR_INVALID_ARG = -1,
+    QNEP_ERR_UNSUPPORTED = -2,       /* triclinic box, order != 5, non-power-of-2 grid, > 4 species, box < r_c + skin */
+    QNEP_ERR_NEIGHBOR_OVERFLOW = -3, /* a neighbour list exceeded its capacity; capacity has been grown, call again */
+    QNEP_ERR_SKIN_VIOLATED = -4,     /* an atom moved more than skin/2 since the last neighbour build */
+    QNEP_ERR_CUDA = -5,
+    QNEP_ERR_OOM = -6
+};
+
+/* The qNEP model (PAPER.md :37-60, Eq. 1; descriptor form: DESIGN.md reading S1-S5). Plain data, copied at create. */
+typedef struct {
+    int32_t n_types;      /* number of species T (1..4)                                                      */
+    int32_t n_max_r;      /* radial descriptors  n = 0..n_max_r                                              */
+    int32_t n_max_a;      /* angular descriptors n = 0..n_max_a                                              */
+    int32_t l_max;        /* angular momentum l = 1..l_max (4 in this version)                               */
+    int32_t basis_r;      /* Chebyshev basis k = 0..basis_r (radial)                                         */
+    int32_t basis_a;      /* Chebyshev basis k = 0..basis_a (angular)                                        */
+    int32_t n_neurons;    /* hidden layer width N_neu (Eq. 1)                                                */
+    double rc_r, rc_a;    /* radial / angular cutoff, Angstrom; rc_a <= rc_r; rc_r is also the real-space
+                             Coulomb cutoff (:89-91)                                                         */
+    int32_t mode;         /* 1: U^ES = U^r + U^k + U^s (Eq. 3); 2: U^ES = U^k (Eq. 5)                        */
+    double sqrt_eps_inf;  /* Eq. 24, used only by the Born effective charges                                 */
+    double q_total;       /* target total charge Q of Eq. 33                                                 */
+} qnep_model_desc;
+
+/* Reciprocal-space method -- the Ewald / PPPM selector (PAPER.md II.B.2 and II.F). */
+typedef struct {
+    int32_t method;       /* 0: no electrostatics; 1: Ewald summation (Eq. 7-9); 2: PPPM (Eq. 34-38)         */
+    double alpha;         /* Ewald splitting parameter, 1/Angstrom; <= 0 selects pi / rc_r (:91)             */
+    int32_t ewald_nmax2;  /* Ewald: keep integer n.n <= nmax2 (k = 2 pi n / L); <= 0 selects |k| <= 2 pi alpha (:110) */
+    int32_t grid[3];      /* PPPM mesh N_x, N_y, N_z: powers of two, 8..512                                  */
+    int32_t order;        /* PPPM interpolation order P; 5 only (:280)                                       */
+} qnep_es_desc;
+
+/* bit flags of `want` */
+enum { QNEP_WANT_ENERGY = 1, QNEP_WANT_FORCES = 2, QNEP_WANT_VIRIAL = 4, QNEP_WANT_CHARGES = 8, QNEP_WANT_BEC = 16 };
+
+/* stages reported by qnep_get_timings (milliseconds of the last qnep_compute) */
+enum {
+    QNEP_T_NEIGHBOR = 0,   /* a1  cell list + neighbour lists (0 when not rebuilt)   */
+    QNEP_T_PREP,           /*     cell-relative fp32 coordinates, skin check         */
+    QNEP_T_DESC_RADIAL,    /* a2                                                     */
+    QNEP_T_DESC_ANGULAR,   /* a3                                                     */
+    QNEP_T_NN,             /* a4, a5, a10                                            */
+    QNEP_T_REALSPACE,      /* a6, a8                                                 */
+    QNEP_T_RECIPROCAL,     /* a7E or a7P-1..5                                        */
+    QNEP_T_FORCE_ANGULAR,  /* a11 (angular partial forces)                           */
+    QNEP_T_FORCE_RADIAL,   /* a11 (radial partial forces, assembly, outputs)         */
+    QNEP_T_BEC,            /* a12                                                    */
+    QNEP_T_TOTAL,
+    QNEP_T_COUNT
+};
+
+/* per-stage intermediates for the parity tests (qnep_debug_copy) */
+enum {
+    QNEP_DBG_DESCRIPTORS = 0, /* [N][n_desc] unscaled D^i, row per atom       */
+    QNEP_DBG_SITE_ENERGY,     /* [N] U_i                                        */
+    QNEP_DBG_Q_RAW,           /* [N] q_i before Eq. 33                          */
+    QNEP_DBG_PHI,             /* [N] dU^ES/dq_i before the mean subtraction     */
+    QNEP_DBG_FP,              /* [N][n_desc] dU_i/dD + phi_eff dq_i/dD          */
+    QNEP_DBG_MESH_RHO,        /* [Nx][Ny][Nz] PPPM charge mesh                  */
+    QNEP_DBG_F_STATIC,        /* [3][N] static electrostatic force              */
+    QNEP_DBG_ENERGY_PARTS     /* [4] U^NEP, U^r, U^k, U^s                       */
+};
+
+/*
+ * qnep_create: build a handle.
+ *   params_host [n_params] float32, order:
+ *     c_R[ti][tj][n][k], c_A[ti][tj][n][k], s[n_desc],
+ *     then per type: w0[H][n_desc], b0[H], w1U[H], w1q[H]; then b1U, b1q.
+ *   n_desc = (n_max_r + 1) + (n_max_a + 1) * l_max.  The vector is copied.
+ * Errors: INVALID_ARG (null pointer, wrong n_params, rc_a > rc_r), UNSUPPORTED, CUDA, OOM.
+ */
+int qnep_create(const qnep_model_desc *model, const float *params_host, size_t n_params,
+                const qnep_es_desc *es, qnep_handle **out);
+
+/* the Ewald / PPPM selector; may be called between computes.  Errors: INVALID_ARG, UNSUPPORTED. */
+int qnep_set_electrostatics(qnep_handle *h, const qnep_es_desc *es);
+
+/*
+ * Neighbour policy: lists hold every pair within r_c + skin and are rebuilt every `rebuild_every`
+ * calls (0 or 1: every call).  Entries beyond r_c contribute exactly zero (the cutoff function
+ * vanishes; the real-space Coulomb sum tests r < r_c explicitly), so results do not depend on skin.
+ * Default: skin = 0, rebuild every call.
+ */
+int qnep_set_neighbor_policy(qnep_handle *h, double skin, int32_t rebuild_every);
+
+/* Override the automatic neighbour-list capacities (entries per atom); <= 0 keeps the automatic value. */
+int qnep_set_neighbor_capacity(qnep_handle *h, int32_t cap_radial, int32_t cap_angular);
+
+/*
+ * qnep_compute: one force evaluation, enqueued on `cuda_stream`.
+ *   pos_dev     [3][N] float64, component-major, Angstrom, any periodic image (wrapped inside)
+ *   types_dev   [N] int32, 0..n_types-1
+ *   box         [9] float64 HOST, rows = cell vectors a, b, c; orthorhombic only in this version
+ *   want        QNEP_WANT_* flags; an output whose flag is clear may be NULL
+ *   energy_dev  [1]    eV,   U^tot = U^NEP + U^ES (Eq. 4)
+ *   forces_dev  [3][N] eV/A  (Eq. 11 + static electrostatic forces Eq. 15, 18 / 37)
+ *   virial_dev  [9]    eV,   W_ab row-major, W = sum_i sum_j r_ij (x) F_ji + W^k,static (Eq. 12, 22) = -dU/d(strain)
+ *   charges_dev [N]    e,    neutralised, unscaled q_i (Eq. 33)
+ *   bec_dev     [9][N] e,    Z_i,ab at [(3a+b)][i] (Eq. 28), or NULL
+ * Errors: INVALID_ARG, UNSUPPORTED, CUDA, OOM; NEIGHBOR_OVERFLOW / SKIN_VIOLATED of the PREVIOUS call.
+ */
+int qnep_compute(qnep_handle *h, int64_t n_atoms, const double *pos_dev, const int32_t *types_dev,
+                 const double box[9], uint32_t want, double *energy_dev, double *forces_dev,
+                 double *virial_dev, double *charges_dev, double *bec_dev, void *cuda_stream);
+
+/*
+ * qnep_compute_host: the same evaluation with HOST buffers: copies positions and types to the device,
+ * runs qnep_compute, copies the requested outputs back and synchronises the stream; device-side errors
+ * of THIS call are reported.  Layouts as above.
+ */
+int qnep_compute_host(qnep_handle *h, int64_t n_atoms, const double *pos_host, const int32_t *types_host,
+                      const double box[9], uint32_t want, double *energy_host, double *forces_host,
+                      double *virial_host, double *charges_host, double *bec_host, void *cuda_stream);
+
+/*
+ * qnep_md_run: n_steps of velocity-Verlet (kick-drift-kick) around qnep_compute, all on the device.
+ *   pos_dev, vel_dev [3][N] float64, updated in place; mass_host[n_types] in amu;
+ *   dt in natural units (Angstrom * sqrt(amu/eV); 1 fs = 1/10.180505);
+ *   energy_dev[2]: potential and kinetic energy after the last step.
+ * The first call computes the initial forces; forces are kept in the handle between calls.
+ * The neighbour policy set by qnep_set_neighbor_policy applies.  Synchronises at the end and reports
+ * device-side errors (SKIN_VIOLATED, NEIGHBOR_OVERFLOW) of the run.
+ */
+int qnep_md_run(qnep_handle *h, int64_t n_atoms, double *pos_dev, double *vel_dev, const int32_t *types_dev,
+                const double box[9], const double *mass_host, double dt, int32_t n_steps,
+                double *energy_dev, void *cuda_stream);
+
+/* Synchronise the stream of the last call and report its device-side error state (OK, NEIGHBOR_OVERFLOW, SKIN_VIOLATED, CUDA). */
+int qnep_check(qnep_handle *h);
+
+/* CUDA-event times in milliseconds of the last qnep_compute, ms[QNEP_T_*]; n = number of entries to write. Synchronises. */
+int qnep_get_timings(qnep_handle *h, float *ms_per_stage_host, int32_t n);
+
+/* number of kernels launched by this handle since creation (bench.py's gpu_launches claim) */
+int64_t qnep_kernel_launches(const qnep_handle *h);
+
+/* live neighbour statistics of the last build: out[0..3] = max radial, max angular, mean radial, mean angular (synchronises) */
+int qnep_neighbor_stats(qnep_handle *h, double out_host[4]);
+
+/*
+ * Copy a per-stage intermediate of the last qnep_compute into a caller-owned DEVICE float64 buffer
+ * (original atom order), for the per-stage parity tests.  `which` is a QNEP_DBG_* value; `n` is the
+ * number of float64 elements `dst_dev` can hold.  Errors: INVALID_ARG.
+ */
+int qnep_debug_copy(qnep_handle *h, int32_t which, double *dst_dev, int64_t n);
+
+void qnep_destroy(qnep_handle *h);
+
+/* Message of the last error on this handle (or of the last failed qnep_create if h == NULL); valid until the next call. */
+const char *qnep_last_error(const qnep_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QNEP_H */

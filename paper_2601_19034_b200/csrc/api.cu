@@ -1,0 +1,633 @@
+// api.cu -- the C ABI of include/qnep.h: handle management and the per-step pipeline
+// (SURVEY.md 8(a) steps a1-a12 in order).  Host code only orchestrates; every step runs in the
+// CUDA kernels of neighbor.cu, descriptor.cu, electro.cu and pppm.cu.
+#include "qnep_internal.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+namespace {
+
+std::string g_create_error;
+
+template <typename Tp>
+int dev_alloc(qnep_handle* h, Tp** p, size_t count)
+{
+    if (*p) { cudaFree(*p); *p = nullptr; }
+    QNEP_CUDA_OK(h, cudaMalloc((void**)p, sizeof(Tp) * std::max<size_t>(count, 1)));
+    return QNEP_OK;
+}
+
+void free_workspace(qnep_handle* h)
+{
+    void** ptrs[] = {(void**)&h->d_key, (void**)&h->d_cnt, (void**)&h->d_start, (void**)&h->d_fill, (void**)&h->d_tmpidx,
+                     (void**)&h->d_sidx, (void**)&h->d_cellc, (void**)&h->d_xyzt, (void**)&h->d_off0, (void**)&h->d_mfrac,
+                     (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_nlA, (void**)&h->d_nnA,
+                     (void**)&h->d_revA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
+                     (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_P,
+                     (void**)&h->d_phik, (void**)&h->d_phir, (void**)&h->d_phi, (void**)&h->d_Fs, (void**)&h->d_Fa,
+                     (void**)&h->d_f12, (void**)&h->d_Fmd};
+    for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
+    h->N = 0;
+    h->md_have_forces = false;
+}
+
+int validate_es(qnep_handle* h, const qnep_es_desc* es)
+{
+    if (es->method < 0 || es->method > 2) { h->err = "es.method must be 0, 1 or 2"; return QNEP_ERR_INVALID_ARG; }
+    if (es->method == 2) {
+        if (es->order != 5) { h->err = "PPPM order must be 5"; return QNEP_ERR_UNSUPPORTED; }
+        for (int a = 0; a < 3; ++a) {
+            const int n = es->grid[a];
+            if (n < 16 || n > 512 || (n & (n - 1))) { h->err = "PPPM grid must be a power of two in 16..512"; return QNEP_ERR_UNSUPPORTED; }
+        }
+    }
+    return QNEP_OK;
+}
+
+// geometry for a box; returns UNSUPPORTED for triclinic / too small boxes
+int make_geometry(qnep_handle* h, const double box[9], Geometry* g)
+{
+    if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) {
+        h->err = "only orthorhombic boxes are supported in this version";
+        return QNEP_ERR_UNSUPPORTED;
+    }
+    const double rcs = h->model.rc_r + h->skin;
+    g->ncells = 1;
+    for (int a = 0; a < 3; ++a) {
+        g->L[a] = box[4 * a];
+        if (!(g->L[a] > 0)) { h->err = "box edge must be positive"; return QNEP_ERR_INVALID_ARG; }
+        if (g->L[a] < rcs) { h->err = "box edge smaller than r_c + skin"; return QNEP_ERR_UNSUPPORTED; }
+        g->ncell[a] = std::min(1023, std::max(1, (int)floor(g->L[a] / rcs)));
+        g->hcell[a] = g->L[a] / g->ncell[a];
+        g->ncells *= g->ncell[a];
+        g->grid[a] = h->es.method == 2 ? h->es.grid[a] : 0;
+        g->hmesh_inv[a] = g->grid[a] > 0 ? g->grid[a] / g->L[a] : 0.0;
+    }
+    g->rc_r2 = (float)(h->model.rc_r * h->model.rc_r);
+    g->rc_a2 = (float)(h->model.rc_a * h->model.rc_a);
+    g->rcs_r2 = (float)(rcs * rcs);
+    g->rcs_a2 = (float)((h->model.rc_a + h->skin) * (h->model.rc_a + h->skin));
+    g->skin_half2 = (float)(0.25 * h->skin * h->skin);
+    return QNEP_OK;
+}
+
+int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
+{
+    Geometry g;
+    int rc = make_geometry(h, box, &g);
+    if (rc) return rc;
+    const bool box_changed = std::memcmp(box, h->box, sizeof(double) * 9) != 0;
+    const double vol = g.L[0] * g.L[1] * g.L[2];
+    const double rho = (double)N / vol;
+    auto cap_for = [&](double rc_, int user) {
+        if (user > 0) return user;
+        const double expect = 4.0 / 3.0 * M_PI * rc_ * rc_ * rc_ * rho;
+        return ((int)(expect * 1.5) + 24 + 3) / 4 * 4;
+    };
+    const int capR = cap_for(h->model.rc_r + h->skin, h->user_capR);
+    const int capA = cap_for(h->model.rc_a + h->skin, h->user_capA);
+    const int T = h->model.n_types;
+    const int nkeys = T * g.ncells;
+    const bool realloc_atoms = N != h->N || capR != h->capR || capA != h->capA;
+    if (realloc_atoms) {
+        free_workspace(h);
+        const size_t n = (size_t)N;
+        if ((rc = dev_alloc(h, &h->d_key, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_tmpidx, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_sidx, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_cellc, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_xyzt, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_off0, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_mfrac, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_mi0, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nlR, n * capR))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nnR, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nlA, n * capA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nnA, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_revA, n * capA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_D, n * QNEP_NDESC))) return rc;
+        if ((rc = dev_alloc(h, &h->d_A, n * QNEP_NRAD * QNEP_NLM))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Ui, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_qraw, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_q, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_FpU, n * QNEP_NDESC))) return rc;
+        if ((rc = dev_alloc(h, &h->d_FpQ, n * QNEP_NDESC))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Fp, n * QNEP_NDESC))) return rc;
+        if ((rc = dev_alloc(h, &h->d_P, n * T * QNEP_KPAD))) return rc;
+        if ((rc = dev_alloc(h, &h->d_phik, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_phir, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_phi, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Fs, n * 3))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Fa, n * 9))) return rc;
+        if ((rc = dev_alloc(h, &h->d_f12, n * capA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Fmd, n * 3))) return rc;
+        h->N = N; h->capR = capR; h->capA = capA;
+        h->force_rebuild = true;
+    }
+    if (nkeys != h->nkeys || !h->d_cnt) {
+        if ((rc = dev_alloc(h, &h->d_cnt, (size_t)nkeys + 1))) return rc;
+        if ((rc = dev_alloc(h, &h->d_start, (size_t)nkeys + 1))) return rc;
+        if ((rc = dev_alloc(h, &h->d_fill, (size_t)nkeys))) return rc;
+        h->nkeys = nkeys;
+        h->force_rebuild = true;
+    }
+    const bool geo_changed = box_changed || std::memcmp(&g, &h->geo, sizeof(Geometry)) != 0;
+    h->geo = g;
+    std::memcpy(h->box, box, sizeof(double) * 9);
+    if (geo_changed || realloc_atoms) {
+        h->force_rebuild = true;
+        if (h->es.method == 1) { if ((rc = qnep_setup_ewald(h))) return rc; }
+        if (h->es.method == 2) { if ((rc = qnep_setup_pppm(h))) return rc; }
+    }
+    return QNEP_OK;
+}
+
+// translate the flags copied back by the previous call
+int consume_flags(qnep_handle* h)
+{
+    h->flags_pending = false;
+    const int* f = h->h_flags;
+    if (f[FLAG_REV_MISS]) { h->err = "internal error: asymmetric angular neighbour list"; h->force_rebuild = true; return QNEP_ERR_CUDA; }
+    if (f[FLAG_MAX_NR] > h->capR || f[FLAG_MAX_NA] > h->capA) {
+        h->err = "neighbour list capacity exceeded (radial " + std::to_string(f[FLAG_MAX_NR]) + "/" + std::to_string(h->capR) +
+                 ", angular " + std::to_string(f[FLAG_MAX_NA]) + "/" + std::to_string(h->capA) + "); capacity grown, call again";
+        h->user_capR = std::max(h->capR, (f[FLAG_MAX_NR] * 5 / 4 + 8 + 3) / 4 * 4);
+        h->user_capA = std::max(h->capA, (f[FLAG_MAX_NA] * 5 / 4 + 8 + 3) / 4 * 4);
+        h->force_rebuild = true;
+        return QNEP_ERR_NEIGHBOR_OVERFLOW;
+    }
+    if (f[FLAG_SKIN]) {
+        h->err = "an atom moved more than skin/2 since the last neighbour build";
+        h->force_rebuild = true;
+        return QNEP_ERR_SKIN_VIOLATED;
+    }
+    return QNEP_OK;
+}
+
+__global__ void k_finalize(const double* __restrict__ sums, int mode, double* __restrict__ energy, double* __restrict__ virial)
+{
+    if (threadIdx.x == 0 && energy) {
+        double e = sums[SUM_E_NEP] + sums[SUM_U_K];
+        if (mode == 1) e += sums[SUM_U_R] + sums[SUM_U_S];
+        energy[0] = e;
+    }
+    if (threadIdx.x < 9 && virial) virial[threadIdx.x] = sums[SUM_W0 + threadIdx.x];
+}
+
+// ---- debug / parity helpers -----------------------------------------------------------------------
+__global__ void k_dbg_rows(int64_t N, int ncomp, const float* __restrict__ src, const int* __restrict__ sidx,
+                           int atom_major, double* __restrict__ dst)
+{
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const int64_t i = sidx[p];
+    for (int v = 0; v < ncomp; ++v) {
+        const double x = src[(int64_t)v * N + p];
+        if (atom_major) dst[i * ncomp + v] = x; else dst[(int64_t)v * N + i] = x;
+    }
+}
+
+__global__ void k_dbg_copy(int64_t n, const float* __restrict__ src, double* __restrict__ dst)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[i];
+}
+
+__global__ void k_dbg_energy(const double* __restrict__ sums, double* __restrict__ dst)
+{
+    dst[0] = sums[SUM_E_NEP]; dst[1] = sums[SUM_U_R]; dst[2] = sums[SUM_U_K]; dst[3] = sums[SUM_U_S];
+}
+
+// ---- velocity-Verlet kernels ----------------------------------------------------------------------
+struct Masses { double m[QNEP_MAX_TYPES]; };
+
+__global__ void k_vv_kick_drift(int64_t N, double* __restrict__ pos, double* __restrict__ vel, const double* __restrict__ F,
+                                const int32_t* __restrict__ types, Masses ms, double dt)
+{
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double im = 0.5 * dt / ms.m[types[i]];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double v = vel[a * N + i] + im * F[a * N + i];
+        vel[a * N + i] = v;
+        pos[a * N + i] += dt * v;
+    }
+}
+
+__global__ void k_vv_kick(int64_t N, double* __restrict__ vel, const double* __restrict__ F, const int32_t* __restrict__ types,
+                          Masses ms, double dt, double* __restrict__ sums)
+{
+    __shared__ double sh[32];
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    double ke = 0.0;
+    if (i < N) {
+        const double m = ms.m[types[i]];
+        const double im = 0.5 * dt / m;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double v = vel[a * N + i] + im * F[a * N + i];
+            vel[a * N + i] = v;
+            ke += 0.5 * m * v * v;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ke += __shfl_xor_sync(0xffffffffu, ke, o);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = ke;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double r = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+        if (threadIdx.x == 0) atomicAdd(&sums[SUM_KE], r);
+    }
+}
+
+__global__ void k_md_energy(const double* __restrict__ sums, int mode, double* __restrict__ out)
+{
+    double e = sums[SUM_E_NEP] + sums[SUM_U_K];
+    if (mode == 1) e += sums[SUM_U_R] + sums[SUM_U_S];
+    out[0] = e;
+    out[1] = sums[SUM_KE];
+}
+
+int upload_model(qnep_handle* h)
+{
+    const qnep_model_desc& m = h->model;
+    const int T = m.n_types, H = m.n_neurons, D = QNEP_NDESC;
+    const float* p = h->h_params.data();
+    const size_t ncoef = (size_t)T * T * QNEP_NRAD * QNEP_NB;
+    const float* cR = p;
+    const float* cA = cR + ncoef;
+    const float* scaler = cA + ncoef;
+    const float* nn = scaler + D;
+    const int per_type = H * D + 3 * H;
+    const float* b1 = nn + (size_t)T * per_type;
+    // padded coefficient tables [T*T][5][KPAD]
+    std::vector<float> pR((size_t)T * T * QNEP_NRAD * QNEP_KPAD, 0.f), pA(pR.size(), 0.f);
+    for (int tt = 0; tt < T * T; ++tt)
+        for (int n = 0; n < QNEP_NRAD; ++n)
+            for (int k = 0; k < QNEP_NB; ++k) {
+                pR[((size_t)tt * QNEP_NRAD + n) * QNEP_KPAD + k] = cR[((size_t)tt * QNEP_NRAD + n) * QNEP_NB + k];
+                pA[((size_t)tt * QNEP_NRAD + n) * QNEP_KPAD + k] = cA[((size_t)tt * QNEP_NRAD + n) * QNEP_NB + k];
+            }
+    // NN per type: w0 * scaler in rows padded to 28, then b0, w1U, w1q
+    const int W0P = 28;
+    h->nn_stride = H * W0P + 3 * H;
+    h->nn_stride = (h->nn_stride + 3) / 4 * 4;
+    std::vector<float> pn((size_t)T * h->nn_stride, 0.f);
+    for (int t = 0; t < T; ++t) {
+        const float* src = nn + (size_t)t * per_type;
+        float* dst = pn.data() + (size_t)t * h->nn_stride;
+        for (int mu = 0; mu < H; ++mu)
+            for (int v = 0; v < D; ++v) dst[mu * W0P + v] = src[mu * D + v] * scaler[v];
+        for (int i = 0; i < 3 * H; ++i) dst[H * W0P + i] = src[H * D + i];
+    }
+    h->b1U = b1[0];
+    h->b1q = b1[1];
+    int rc;
+    if ((rc = dev_alloc(h, &h->d_cR, pR.size()))) return rc;
+    if ((rc = dev_alloc(h, &h->d_cA, pA.size()))) return rc;
+    if ((rc = dev_alloc(h, &h->d_nn, pn.size()))) return rc;
+    QNEP_CUDA_OK(h, cudaMemcpy(h->d_cR, pR.data(), sizeof(float) * pR.size(), cudaMemcpyHostToDevice));
+    QNEP_CUDA_OK(h, cudaMemcpy(h->d_cA, pA.data(), sizeof(float) * pA.size(), cudaMemcpyHostToDevice));
+    QNEP_CUDA_OK(h, cudaMemcpy(h->d_nn, pn.data(), sizeof(float) * pn.size(), cudaMemcpyHostToDevice));
+    return QNEP_OK;
+}
+
+// the pipeline proper; `forces_out` may be NULL (then an internal buffer is used when the virial is wanted)
+int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* types, uint32_t want, double* energy,
+                 double* forces, double* virial, double* charges, double* bec, cudaStream_t s)
+{
+    int rc;
+    const bool rebuild = h->force_rebuild || h->rebuild_every <= 1 || h->calls_since_build < 0 ||
+                         h->calls_since_build >= h->rebuild_every;
+    cudaEvent_t* ev = h->ev;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[0], s));
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_sums, 0, sizeof(double) * SUM_COUNT, s));
+    if (rebuild) {
+        if ((rc = qnep_launch_build(h, pos, types, s))) return rc;
+        h->calls_since_build = 0;
+        h->force_rebuild = false;
+    }
+    h->rebuilt_last = rebuild;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[1], s));
+    if (!rebuild) { if ((rc = qnep_launch_prep(h, pos, false, s))) return rc; }
+    h->calls_since_build += 1;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[2], s));
+    if ((rc = qnep_launch_desc_radial(h, s))) return rc;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[3], s));
+    if ((rc = qnep_launch_desc_angular(h, s))) return rc;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[4], s));
+    if ((rc = qnep_launch_nn(h, (want & QNEP_WANT_CHARGES) ? charges : nullptr, s))) return rc;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[5], s));
+    if (h->es.method != 0 && h->model.mode == 1) { if ((rc = qnep_launch_realspace(h, s))) return rc; }
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[6], s));
+    if (h->es.method == 1) { if ((rc = qnep_launch_ewald(h, pos, s))) return rc; }
+    else if (h->es.method == 2) { if ((rc = qnep_launch_pppm(h, s))) return rc; }
+    else QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
+    if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[7], s));
+    const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
+    if (need_forces) {
+        if ((rc = qnep_launch_fp_combine(h, false, s))) return rc;
+        if ((rc = qnep_launch_force_angular(h, false, s))) return rc;
+        QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
+        double* fout = ((want & QNEP_WANT_FORCES) && forces) ? forces : h->d_Fmd;
+        if ((rc = qnep_launch_force_radial(h, false, fout, s))) return rc;
+    } else {
+        QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
+    }
+    k_finalize<<<1, 32, 0, s>>>(h->d_sums, h->model.mode, (want & QNEP_WANT_ENERGY) ? energy : nullptr,
+                                (want & QNEP_WANT_VIRIAL) ? virial : nullptr);
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[9], s));
+    if ((want & QNEP_WANT_BEC) && bec) {
+        if ((rc = qnep_launch_fp_combine(h, true, s))) return rc;
+        if ((rc = qnep_launch_force_angular(h, true, s))) return rc;
+        if ((rc = qnep_launch_force_radial(h, true, bec, s))) return rc;
+    }
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[10], s));
+    h->ev_valid = true;
+    QNEP_CUDA_OK(h, cudaMemcpyAsync(h->h_flags, h->d_flags, sizeof(int) * FLAG_COUNT, cudaMemcpyDeviceToHost, s));
+    QNEP_CUDA_OK(h, cudaEventRecord(h->ev_flags, s));
+    h->flags_pending = true;
+    h->last_stream = s;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int check_args(qnep_handle* h, int64_t n_atoms, const void* pos, const void* types, const double* box, uint32_t want,
+               const void* energy, const void* forces, const void* virial, const void* charges, const void* bec)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (n_atoms <= 0 || n_atoms > QNEP_NL_MASK) { h->err = "n_atoms out of range"; return QNEP_ERR_INVALID_ARG; }
+    if (!pos || !types || !box) { h->err = "null input pointer"; return QNEP_ERR_INVALID_ARG; }
+    if (((want & QNEP_WANT_ENERGY) && !energy) || ((want & QNEP_WANT_FORCES) && !forces) ||
+        ((want & QNEP_WANT_VIRIAL) && !virial) || ((want & QNEP_WANT_CHARGES) && !charges) ||
+        ((want & QNEP_WANT_BEC) && !bec)) {
+        h->err = "a requested output pointer is null";
+        return QNEP_ERR_INVALID_ARG;
+    }
+    return QNEP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int qnep_create(const qnep_model_desc* model, const float* params_host, size_t n_params, const qnep_es_desc* es,
+                qnep_handle** out)
+{
+    if (out) *out = nullptr;
+    if (!model || !params_host || !es || !out) { g_create_error = "null argument"; return QNEP_ERR_INVALID_ARG; }
+    qnep_handle* h = new (std::nothrow) qnep_handle();
+    if (!h) { g_create_error = "out of host memory"; return QNEP_ERR_OOM; }
+    auto fail = [&](int code) { g_create_error = h->err; qnep_destroy(h); return code; };
+    h->model = *model;
+    std::memset(h->box, 0, sizeof(h->box));
+    std::memset(&h->geo, 0, sizeof(h->geo));
+    const qnep_model_desc& m = h->model;
+    if (m.n_types < 1 || m.n_neurons < 1 || m.rc_r <= 0 || m.rc_a <= 0 || m.rc_a > m.rc_r || (m.mode != 1 && m.mode != 2)) {
+        h->err = "invalid model description";
+        return fail(QNEP_ERR_INVALID_ARG);
+    }
+    if (m.n_types > QNEP_MAX_TYPES || m.n_max_r != 4 || m.n_max_a != 4 || m.l_max != 4 || m.basis_r != 8 || m.basis_a != 8 ||
+        m.n_neurons > 256) {
+        h->err = "this version supports n_types <= 4, n_max = 4, l_max = 4, basis = 8, n_neurons <= 256";
+        return fail(QNEP_ERR_UNSUPPORTED);
+    }
+    const int T = m.n_types, H = m.n_neurons, D = QNEP_NDESC;
+    const size_t expect = 2 * (size_t)T * T * QNEP_NRAD * QNEP_NB + D + (size_t)T * (H * D + 3 * H) + 2;
+    if (n_params != expect) { h->err = "n_params does not match the model description"; return fail(QNEP_ERR_INVALID_ARG); }
+    int rc = validate_es(h, es);
+    if (rc) return fail(rc);
+    h->es = *es;
+    h->alpha = es->alpha > 0 ? es->alpha : M_PI / m.rc_r;
+    h->h_params.assign(params_host, params_host + n_params);
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) {
+        h->err = "no CUDA device: this library has no CPU fallback";
+        return fail(QNEP_ERR_CUDA);
+    }
+    if ((rc = upload_model(h))) return fail(rc);
+    if (cudaMalloc(&h->d_sums, sizeof(double) * SUM_COUNT) != cudaSuccess ||
+        cudaMalloc(&h->d_flags, sizeof(int) * FLAG_COUNT) != cudaSuccess ||
+        cudaMallocHost(&h->h_flags, sizeof(int) * FLAG_COUNT) != cudaSuccess) {
+        h->err = "allocation of accumulators failed";
+        return fail(QNEP_ERR_OOM);
+    }
+    cudaMemset(h->d_flags, 0, sizeof(int) * FLAG_COUNT);
+    std::memset(h->h_flags, 0, sizeof(int) * FLAG_COUNT);
+    cudaEventCreateWithFlags(&h->ev_flags, cudaEventDisableTiming);
+    for (auto& e : h->ev) cudaEventCreate(&e);
+    *out = h;
+    return QNEP_OK;
+}
+
+int qnep_set_electrostatics(qnep_handle* h, const qnep_es_desc* es)
+{
+    if (!h || !es) return QNEP_ERR_INVALID_ARG;
+    int rc = validate_es(h, es);
+    if (rc) return rc;
+    h->es = *es;
+    h->alpha = es->alpha > 0 ? es->alpha : M_PI / h->model.rc_r;
+    std::memset(h->box, 0, sizeof(h->box));   // forces the tables to be rebuilt at the next compute
+    h->force_rebuild = true;
+    return QNEP_OK;
+}
+
+int qnep_set_neighbor_policy(qnep_handle* h, double skin, int32_t rebuild_every)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (skin < 0 || rebuild_every < 0) { h->err = "skin and rebuild_every must be non-negative"; return QNEP_ERR_INVALID_ARG; }
+    h->skin = skin;
+    h->rebuild_every = rebuild_every;
+    h->force_rebuild = true;
+    std::memset(h->box, 0, sizeof(h->box));
+    return QNEP_OK;
+}
+
+int qnep_set_neighbor_capacity(qnep_handle* h, int32_t cap_radial, int32_t cap_angular)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    h->user_capR = cap_radial > 0 ? cap_radial : 0;
+    h->user_capA = cap_angular > 0 ? cap_angular : 0;
+    h->force_rebuild = true;
+    return QNEP_OK;
+}
+
+int qnep_compute(qnep_handle* h, int64_t n_atoms, const double* pos_dev, const int32_t* types_dev, const double box[9],
+                 uint32_t want, double* energy_dev, double* forces_dev, double* virial_dev, double* charges_dev,
+                 double* bec_dev, void* cuda_stream)
+{
+    int rc = check_args(h, n_atoms, pos_dev, types_dev, box, want, energy_dev, forces_dev, virial_dev, charges_dev, bec_dev);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (h->flags_pending && cudaEventQuery(h->ev_flags) == cudaSuccess) {
+        if ((rc = consume_flags(h))) return rc;
+    }
+    if ((rc = ensure_workspace(h, n_atoms, box))) return rc;
+    return run_pipeline(h, n_atoms, pos_dev, types_dev, want, energy_dev, forces_dev, virial_dev, charges_dev, bec_dev, s);
+}
+
+int qnep_check(qnep_handle* h)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    QNEP_CUDA_OK(h, cudaStreamSynchronize(h->last_stream));
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    if (h->flags_pending) return consume_flags(h);
+    return QNEP_OK;
+}
+
+int qnep_compute_host(qnep_handle* h, int64_t n_atoms, const double* pos_host, const int32_t* types_host,
+                      const double box[9], uint32_t want, double* energy_host, double* forces_host, double* virial_host,
+                      double* charges_host, double* bec_host, void* cuda_stream)
+{
+    int rc = check_args(h, n_atoms, pos_host, types_host, box, want, energy_host, forces_host, virial_host, charges_host, bec_host);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)n_atoms;
+    if (h->hostN != n_atoms) {
+        if ((rc = dev_alloc(h, &h->d_hpos, 3 * n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_htypes, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_hout, 1 + 3 * n + 9 + n + 9 * n))) return rc;
+        h->hostN = n_atoms;
+    }
+    double* d_e = h->d_hout;
+    double* d_f = d_e + 1;
+    double* d_w = d_f + 3 * n;
+    double* d_q = d_w + 9;
+    double* d_z = d_q + n;
+    QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, s));
+    QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_htypes, types_host, sizeof(int32_t) * n, cudaMemcpyHostToDevice, s));
+    rc = qnep_compute(h, n_atoms, h->d_hpos, h->d_htypes, box, want, d_e, d_f, d_w, d_q, d_z, s);
+    if (rc) return rc;
+    if (want & QNEP_WANT_ENERGY) QNEP_CUDA_OK(h, cudaMemcpyAsync(energy_host, d_e, sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (want & QNEP_WANT_FORCES) QNEP_CUDA_OK(h, cudaMemcpyAsync(forces_host, d_f, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, s));
+    if (want & QNEP_WANT_VIRIAL) QNEP_CUDA_OK(h, cudaMemcpyAsync(virial_host, d_w, sizeof(double) * 9, cudaMemcpyDeviceToHost, s));
+    if (want & QNEP_WANT_CHARGES) QNEP_CUDA_OK(h, cudaMemcpyAsync(charges_host, d_q, sizeof(double) * n, cudaMemcpyDeviceToHost, s));
+    if (want & QNEP_WANT_BEC) QNEP_CUDA_OK(h, cudaMemcpyAsync(bec_host, d_z, sizeof(double) * 9 * n, cudaMemcpyDeviceToHost, s));
+    return qnep_check(h);
+}
+
+int qnep_md_run(qnep_handle* h, int64_t n_atoms, double* pos_dev, double* vel_dev, const int32_t* types_dev,
+                const double box[9], const double* mass_host, double dt, int32_t n_steps, double* energy_dev,
+                void* cuda_stream)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (n_atoms <= 0 || !pos_dev || !vel_dev || !types_dev || !box || !mass_host || n_steps < 0) {
+        h->err = "invalid argument to qnep_md_run";
+        return QNEP_ERR_INVALID_ARG;
+    }
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int rc;
+    if (h->flags_pending) { if ((rc = qnep_check(h))) return rc; }
+    if ((rc = ensure_workspace(h, n_atoms, box))) return rc;
+    Masses ms;
+    for (int t = 0; t < QNEP_MAX_TYPES; ++t) ms.m[t] = t < h->model.n_types ? mass_host[t] : 1.0;
+    const int nb = (int)((n_atoms + 255) / 256);
+    const uint32_t want = QNEP_WANT_ENERGY | QNEP_WANT_FORCES;
+    if (!h->md_have_forces) {
+        if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
+        h->md_have_forces = true;
+    }
+    for (int step = 0; step < n_steps; ++step) {
+        k_vv_kick_drift<<<nb, 256, 0, s>>>(n_atoms, pos_dev, vel_dev, h->d_Fmd, types_dev, ms, dt);
+        if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
+        k_vv_kick<<<nb, 256, 0, s>>>(n_atoms, vel_dev, h->d_Fmd, types_dev, ms, dt, h->d_sums);
+        h->launches += 2;
+    }
+    if (energy_dev) { k_md_energy<<<1, 1, 0, s>>>(h->d_sums, h->model.mode, energy_dev); h->launches += 1; }
+    return qnep_check(h);
+}
+
+int qnep_get_timings(qnep_handle* h, float* ms, int32_t n)
+{
+    if (!h || !ms) return QNEP_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) ms[i] = 0.f;
+    if (!h->ev_valid) return QNEP_OK;
+    QNEP_CUDA_OK(h, cudaEventSynchronize(h->ev[10]));
+    // ev[i] .. ev[i+1] -> stage i
+    for (int i = 0; i < QNEP_T_TOTAL && i < n; ++i) {
+        float t = 0.f;
+        QNEP_CUDA_OK(h, cudaEventElapsedTime(&t, h->ev[i], h->ev[i + 1]));
+        ms[i] = t;
+    }
+    if (n > QNEP_T_TOTAL) {
+        float t = 0.f;
+        QNEP_CUDA_OK(h, cudaEventElapsedTime(&t, h->ev[0], h->ev[10]));
+        ms[QNEP_T_TOTAL] = t;
+    }
+    return QNEP_OK;
+}
+
+int64_t qnep_kernel_launches(const qnep_handle* h) { return h ? h->launches : 0; }
+
+int qnep_neighbor_stats(qnep_handle* h, double out[4])
+{
+    if (!h || !out) return QNEP_ERR_INVALID_ARG;
+    if (!h->d_flags || h->N == 0) { out[0] = out[1] = out[2] = out[3] = 0; return QNEP_OK; }
+    QNEP_CUDA_OK(h, cudaStreamSynchronize(h->last_stream));
+    int f[FLAG_COUNT];
+    QNEP_CUDA_OK(h, cudaMemcpy(f, h->d_flags, sizeof(f), cudaMemcpyDeviceToHost));
+    unsigned long long sr, sa;
+    std::memcpy(&sr, &f[FLAG_SUM_NR], 8);
+    std::memcpy(&sa, &f[FLAG_SUM_NA], 8);
+    out[0] = f[FLAG_MAX_NR]; out[1] = f[FLAG_MAX_NA];
+    out[2] = (double)sr / (double)h->N; out[3] = (double)sa / (double)h->N;
+    return QNEP_OK;
+}
+
+int qnep_debug_copy(qnep_handle* h, int32_t which, double* dst, int64_t n)
+{
+    if (!h || !dst || h->N == 0) return QNEP_ERR_INVALID_ARG;
+    const int64_t N = h->N;
+    cudaStream_t s = h->last_stream;
+    const int nb = (int)((N + 255) / 256);
+    auto need = [&](int64_t cnt) { if (n < cnt) { h->err = "debug buffer too small"; return false; } return true; };
+    switch (which) {
+        case QNEP_DBG_DESCRIPTORS: if (!need(N * QNEP_NDESC)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, QNEP_NDESC, h->d_D, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_SITE_ENERGY: if (!need(N)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, 1, h->d_Ui, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_Q_RAW: if (!need(N)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, 1, h->d_qraw, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_PHI: if (!need(N)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, 1, h->d_phi, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_FP: if (!need(N * QNEP_NDESC)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, QNEP_NDESC, h->d_Fp, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_F_STATIC: if (!need(3 * N)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, 3, h->d_Fs, h->d_sidx, 0, dst); break;
+        case QNEP_DBG_MESH_RHO:
+            if (h->es.method != 2 || !h->d_mesh || !need(h->ngrid)) { h->err = "no PPPM mesh"; return QNEP_ERR_INVALID_ARG; }
+            k_dbg_copy<<<(int)((h->ngrid + 255) / 256), 256, 0, s>>>(h->ngrid, h->d_mesh, dst); break;
+        case QNEP_DBG_ENERGY_PARTS: if (!need(4)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_energy<<<1, 1, 0, s>>>(h->d_sums, dst); break;
+        default: h->err = "unknown debug selector"; return QNEP_ERR_INVALID_ARG;
+    }
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    QNEP_CUDA_OK(h, cudaStreamSynchronize(s));
+    return QNEP_OK;
+}
+
+void qnep_destroy(qnep_handle* h)
+{
+    if (!h) return;
+    free_workspace(h);
+    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_sums, h->d_flags, h->d_kvec,
+                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_cm1, h->d_cm2, h->d_gtab, h->d_twiddle, h->d_hpos,
+                    h->d_htypes, h->d_hout};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    if (h->h_flags) cudaFreeHost(h->h_flags);
+    if (h->ev_flags) cudaEventDestroy(h->ev_flags);
+    for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+    delete h;
+}
+
+const char* qnep_last_error(const qnep_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,720 @@
+// descriptor.cu -- steps a2, a3, a4, a5, a10, a11, a12 of SURVEY.md 8(a):
+//   radial / angular NEP descriptors (PAPER.md :56; readings S1-S3),
+//   the per-atom network with the extra charge output (Eq. 1, :58-60),
+//   Eq. 33 neutralisation, the folded back-propagation  Fp = dU_i/dD + phi_eff dq_i/dD  (:140, Eq. 14, 17),
+//   partial forces, force / virial assembly (Eq. 11, 12) and the Born effective charges (Eq. 28).
+//
+// One thread owns one atom; atoms are (type, cell)-sorted so a warp is type-uniform and its
+// neighbour gathers hit the same cache lines.  All per-neighbour state lives in registers.
+//
+// Algebra used to keep the hot loops on the FP32 FMA pipe:
+//   * radial:  D_n = sum_j sum_k c^{ti tj}_{nk} f_k(r_ij) = sum_t sum_k c^{ti t}_{nk} S^t_k,
+//     S^t_k = sum_{j in t} f_k(r_ij): the per-neighbour work is the 9 basis values only; the
+//     coefficient contraction is done once per atom.  Backward likewise with
+//     P^{t}_k = sum_n Fp_n c^{ti t}_{nk}.
+//   * angular: A_nlm = sum_j g_n(r_ij) b_lm(rhat_ij) with 24 real harmonic polynomials b_lm;
+//     D_nl = sum_m C_lm A_nlm^2 equals the Legendre double sum of the definition by the addition
+//     theorem (weights C_lm are exact rationals, see harmonic weights below).
+//   * F_ji of the radial part is recomputed by atom i from P^{ti}_k of atom j (no atomics, no
+//     pair storage); the angular F_ij are stored once per pair and fetched through a reverse
+//     index built with the neighbour list (deterministic, no atomics).
+#include "qnep_internal.cuh"
+
+#include <type_traits>
+
+namespace {
+
+constexpr int NB = QNEP_NB;       // 9 basis functions
+constexpr int NR = QNEP_NRAD;     // 5 radial functions
+constexpr int KP = QNEP_KPAD;     // padded row
+constexpr int NLM = QNEP_NLM;
+constexpr int ND = QNEP_NDESC;
+
+// addition-theorem weights: P_l(u.v) = sum_m C_lm b_lm(u) b_lm(v)
+__constant__ float c_Clm[NLM] = {1.f, 1.f, 1.f,
+                                 0.25f, 3.f, 3.f, 0.75f, 0.75f,
+                                 0.25f, 0.375f, 0.375f, 3.75f, 3.75f, 0.625f, 0.625f,
+                                 1.f / 64.f, 0.625f, 0.625f, 0.3125f, 0.3125f, 4.375f, 4.375f, 35.f / 64.f, 35.f / 64.f};
+__host__ __device__ __forceinline__ constexpr int l_of_lm(int lm) { return lm < 3 ? 0 : (lm < 8 ? 1 : (lm < 15 ? 2 : 3)); }
+
+// f_k(r) = 1/2 [T_k(x) + 1] f_c(r), x = 2 (r/rc - 1)^2 - 1, f_c = 1/2 [1 + cos(pi r / rc)]   (S1)
+template <bool VAL, bool DERIV>
+__device__ __forceinline__ void cheb_basis(float r, float rcinv, float* __restrict__ f, float* __restrict__ df)
+{
+    const float t = r * rcinv;
+    const float fc = 0.5f + 0.5f * cospif(t);
+    const float tm1 = t - 1.f;
+    const float x = 2.f * tm1 * tm1 - 1.f;
+    const float hfc = 0.5f * fc;
+    float dfc = 0.f, dx = 0.f, hdxfc = 0.f, hdfc = 0.f;
+    if (DERIV) {
+        dfc = -1.5707963267948966f * rcinv * sinpif(t);
+        dx = 4.f * tm1 * rcinv;
+        hdxfc = 0.5f * dx * fc;
+        hdfc = 0.5f * dfc;
+    }
+    float Tm = 1.f, Tc = x, dTm = 0.f, dTc = 1.f;
+    if (VAL) { f[0] = fc; f[1] = hfc * (x + 1.f); }
+    if (DERIV) { df[0] = dfc; df[1] = hdxfc + hdfc * (x + 1.f); }
+#pragma unroll
+    for (int k = 2; k < NB; ++k) {
+        const float Tn = 2.f * x * Tc - Tm;
+        if (VAL) f[k] = hfc * (Tn + 1.f);
+        if (DERIV) {
+            const float dTn = 2.f * Tc + 2.f * x * dTc - dTm;
+            df[k] = hdxfc * dTn + hdfc * (Tn + 1.f);
+            dTm = dTc; dTc = dTn;
+        }
+        Tm = Tc; Tc = Tn;
+    }
+}
+
+__device__ __forceinline__ void load_shift_table(float4* sh, const Geometry& g)
+{
+    if (threadIdx.x < 27) {
+        const int code = threadIdx.x;
+        sh[code] = make_float4((code / 9 - 1) * (float)g.hcell[0], ((code / 3) % 3 - 1) * (float)g.hcell[1],
+                               (code % 3 - 1) * (float)g.hcell[2], 0.f);
+    }
+}
+
+__device__ __forceinline__ double block_sum(double v, double* sh)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (wid == 0) {
+        r = lane < (blockDim.x >> 5) ? sh[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+    }
+    return r;   // valid in thread 0
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: radial descriptors
+// ------------------------------------------------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(128)
+k_desc_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
+              const int* __restrict__ nn, const float* __restrict__ cR, float rcinv, float* __restrict__ D)
+{
+    __shared__ float4 sh_shift[27];
+    __shared__ float sh_c[T * T * NR * KP];
+    load_shift_table(sh_shift, g);
+    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
+    __syncthreads();
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const float4 xi = xyzt[p];
+    const int ti = __float_as_int(xi.w);
+    float S[T][NB];
+#pragma unroll
+    for (int t = 0; t < T; ++t)
+#pragma unroll
+        for (int k = 0; k < NB; ++k) S[t][k] = 0.f;
+    const int n = nn[p];
+    for (int s = 0; s < n; ++s) {
+        const int e = nl[(int64_t)s * N + p];
+        const float4 xj = xyzt[e & QNEP_NL_MASK];
+        const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+        const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 >= g.rc_r2) continue;
+        float f[NB];
+        cheb_basis<true, false>(sqrtf(r2), rcinv, f, nullptr);
+        const int tj = __float_as_int(xj.w);
+#pragma unroll
+        for (int t = 0; t < T; ++t) {
+            const float w = (tj == t) ? 1.f : 0.f;
+#pragma unroll
+            for (int k = 0; k < NB; ++k) S[t][k] = fmaf(w, f[k], S[t][k]);
+        }
+    }
+#pragma unroll
+    for (int nidx = 0; nidx < NR; ++nidx) {
+        float d = 0.f;
+#pragma unroll
+        for (int t = 0; t < T; ++t) {
+            const float* c = sh_c + ((ti * T + t) * NR + nidx) * KP;
+#pragma unroll
+            for (int k = 0; k < NB; ++k) d = fmaf(c[k], S[t][k], d);
+        }
+        D[(int64_t)nidx * N + p] = d;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// real harmonic polynomials b_lm(u), l = 1..4 (unit vector u = (x, y, z))
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void harmonics(float x, float y, float z, float* __restrict__ b)
+{
+    const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y;
+    const float x2my2 = x2 - y2;
+    b[0] = z; b[1] = x; b[2] = y;
+    b[3] = 3.f * z2 - 1.f; b[4] = x * z; b[5] = y * z; b[6] = x2my2; b[7] = 2.f * xy;
+    const float f5 = 5.f * z2 - 1.f;
+    b[8] = (5.f * z2 - 3.f) * z; b[9] = f5 * x; b[10] = f5 * y; b[11] = x2my2 * z; b[12] = 2.f * xy * z;
+    b[13] = (x2 - 3.f * y2) * x; b[14] = (3.f * x2 - y2) * y;
+    const float f7 = 7.f * z2 - 1.f, f73 = 7.f * z2 - 3.f;
+    b[15] = (35.f * z2 - 30.f) * z2 + 3.f; b[16] = f73 * x * z; b[17] = f73 * y * z; b[18] = f7 * x2my2;
+    b[19] = f7 * 2.f * xy; b[20] = (x2 - 3.f * y2) * x * z; b[21] = (3.f * x2 - y2) * y * z;
+    b[22] = x2my2 * x2my2 - 4.f * x2 * y2; b[23] = 4.f * x2my2 * xy;
+}
+
+// ------------------------------------------------------------------------------------------
+// a3: angular descriptors; A_nlm kept for the backward pass
+// ------------------------------------------------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(64)
+k_desc_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
+               const int* __restrict__ nn, const float* __restrict__ cA, float rcinv, float* __restrict__ D,
+               float* __restrict__ Aout)
+{
+    __shared__ float4 sh_shift[27];
+    __shared__ __align__(16) float sh_c[T * T * NR * KP];
+    load_shift_table(sh_shift, g);
+    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
+    __syncthreads();
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const float4 xi = xyzt[p];
+    const int ti = __float_as_int(xi.w);
+    float A[NR][NLM];
+#pragma unroll
+    for (int a = 0; a < NR; ++a)
+#pragma unroll
+        for (int lm = 0; lm < NLM; ++lm) A[a][lm] = 0.f;
+    const int n = nn[p];
+    for (int s = 0; s < n; ++s) {
+        const int e = nl[(int64_t)s * N + p];
+        const float4 xj = xyzt[e & QNEP_NL_MASK];
+        const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+        const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 >= g.rc_a2) continue;
+        const float r = sqrtf(r2), rinv = 1.f / r;
+        float f[NB];
+        cheb_basis<true, false>(r, rcinv, f, nullptr);
+        const float* c = sh_c + (ti * T + __float_as_int(xj.w)) * NR * KP;
+        float gn[NR];
+#pragma unroll
+        for (int a = 0; a < NR; ++a) {
+            float v = 0.f;
+#pragma unroll
+            for (int k = 0; k < NB; ++k) v = fmaf(c[a * KP + k], f[k], v);
+            gn[a] = v;
+        }
+        float b[NLM];
+        harmonics(dx * rinv, dy * rinv, dz * rinv, b);
+#pragma unroll
+        for (int a = 0; a < NR; ++a)
+#pragma unroll
+            for (int lm = 0; lm < NLM; ++lm) A[a][lm] = fmaf(gn[a], b[lm], A[a][lm]);
+    }
+#pragma unroll
+    for (int a = 0; a < NR; ++a) {
+        float d[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int lm = 0; lm < NLM; ++lm) {
+            d[l_of_lm(lm)] = fmaf(c_Clm[lm] * A[a][lm], A[a][lm], d[l_of_lm(lm)]);
+            Aout[(int64_t)(a * NLM + lm) * N + p] = A[a][lm];
+        }
+#pragma unroll
+        for (int l = 0; l < 4; ++l) D[(int64_t)(NR + a * 4 + l) * N + p] = d[l];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a4 (+a10 in two halves): NN forward, dU/dD and dq/dD.  Weights per type in shared memory:
+//   w0s[H][28] (= w0 * scaler, rows padded to 28), b0[H], w1U[H], w1q[H]
+// ------------------------------------------------------------------------------------------
+constexpr int W0P = 28;
+
+__device__ __forceinline__ float tanh_f32(float z)
+{
+    // tanh z = 1 - 2 / (exp(2z) + 1); exact limits at +-inf, abs error ~1e-7
+    const float e = expf(2.f * z);
+    return 1.f - __fdividef(2.f, e + 1.f);
+}
+
+__global__ void __launch_bounds__(128)
+k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, float b1U, float b1q,
+     const float4* __restrict__ xyzt, const float* __restrict__ D, float* __restrict__ Ui, float* __restrict__ qraw,
+     float* __restrict__ FpU, float* __restrict__ FpQ, double* __restrict__ sums)
+{
+    extern __shared__ __align__(16) float sh_w[];
+    __shared__ double sh_red[32];
+    for (int i = threadIdx.x; i < T * nn_stride; i += blockDim.x) sh_w[i] = nnw[i];
+    __syncthreads();
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float U = 0.f, q = 0.f;
+    if (p < N) {
+        const int ti = __float_as_int(xyzt[p].w);
+        const float* w = sh_w + ti * nn_stride;
+        const float* b0 = w + H * W0P;
+        const float* w1U = b0 + H;
+        const float* w1q = w1U + H;
+        float x[W0P], dU[W0P], dQ[W0P];
+#pragma unroll
+        for (int v = 0; v < W0P; ++v) { x[v] = v < ND ? D[(int64_t)v * N + p] : 0.f; dU[v] = 0.f; dQ[v] = 0.f; }
+        for (int mu = 0; mu < H; ++mu) {
+            const float4* row = reinterpret_cast<const float4*>(w + mu * W0P);
+            float wr[W0P];
+#pragma unroll
+            for (int v4 = 0; v4 < W0P / 4; ++v4) {
+                const float4 t = row[v4];
+                wr[4 * v4] = t.x; wr[4 * v4 + 1] = t.y; wr[4 * v4 + 2] = t.z; wr[4 * v4 + 3] = t.w;
+            }
+            float z0 = -b0[mu], z1 = 0.f;
+#pragma unroll
+            for (int v = 0; v < ND; v += 2) { z0 = fmaf(wr[v], x[v], z0); if (v + 1 < ND) z1 = fmaf(wr[v + 1], x[v + 1], z1); }
+            const float hmu = tanh_f32(z0 + z1);
+            const float a = w1U[mu], b = w1q[mu];
+            U = fmaf(a, hmu, U);
+            q = fmaf(b, hmu, q);
+            const float dh = 1.f - hmu * hmu;
+            const float au = a * dh, bq = b * dh;
+#pragma unroll
+            for (int v = 0; v < ND; ++v) { dU[v] = fmaf(au, wr[v], dU[v]); dQ[v] = fmaf(bq, wr[v], dQ[v]); }
+        }
+        U -= b1U;
+        q -= b1q;
+        Ui[p] = U;
+        qraw[p] = q;
+#pragma unroll
+        for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + p] = dU[v]; FpQ[(int64_t)v * N + p] = dQ[v]; }
+    }
+    const double su = block_sum((double)U, sh_red);
+    const double sq = block_sum((double)q, sh_red);
+    if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
+}
+
+// a5: Eq. 33 (reading G3): q_i = q_i^raw + (Q - sum_j q_j^raw) / N
+__global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const double* __restrict__ sums, double Qtot,
+                             const int* __restrict__ sidx, float* __restrict__ q, double* __restrict__ charges_out)
+{
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const double shift = (Qtot - sums[SUM_Q]) / (double)N;
+    const double v = (double)qraw[p] + shift;
+    q[p] = (float)v;
+    if (charges_out) charges_out[sidx[p]] = v;
+}
+
+// a10: Fp = dU/dD + phi_eff dq/dD (S6: phi_eff = phi - mean phi), and the radial vectors
+//      P^t_k = sum_n Fp_n c^{ti t}_{nk}.  BEC mode: Fp = sqrt(eps_inf) dq/dD (Eq. 24, 28; S12).
+template <int T>
+__global__ void __launch_bounds__(128)
+k_fp_combine(int64_t N, const float4* __restrict__ xyzt, const float* __restrict__ FpU, const float* __restrict__ FpQ,
+             const float* __restrict__ phi, const double* __restrict__ sums, int bec, float sqrt_eps,
+             const float* __restrict__ cR, float* __restrict__ Fp, float* __restrict__ P)
+{
+    __shared__ float sh_c[T * T * NR * KP];
+    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
+    __syncthreads();
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const int ti = __float_as_int(xyzt[p].w);
+    float cu, cq;
+    if (bec) { cu = 0.f; cq = sqrt_eps; }
+    else { cu = 1.f; cq = phi[p] - (float)(sums[SUM_PHI] / (double)N); }
+    float fr[NR];
+#pragma unroll
+    for (int v = 0; v < ND; ++v) {
+        const float val = cu * FpU[(int64_t)v * N + p] + cq * FpQ[(int64_t)v * N + p];
+        Fp[(int64_t)v * N + p] = val;
+        if (v < NR) fr[v] = val;
+    }
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        float4* out = reinterpret_cast<float4*>(P + ((int64_t)p * T + t) * KP);
+        float pk[KP];
+#pragma unroll
+        for (int k = 0; k < KP; ++k) {
+            float v = 0.f;
+            if (k < NB) {
+#pragma unroll
+                for (int a = 0; a < NR; ++a) v = fmaf(fr[a], sh_c[((ti * T + t) * NR + a) * KP + k], v);
+            }
+            pk[k] = v;
+        }
+        out[0] = make_float4(pk[0], pk[1], pk[2], pk[3]);
+        out[1] = make_float4(pk[4], pk[5], pk[6], pk[7]);
+        out[2] = make_float4(pk[8], pk[9], pk[10], pk[11]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a11 (angular part): F_ij = sum_{n,lm} Q_nlm d/dr_ij [ g_n(r_ij) b_lm(rhat_ij) ],
+//   Q_nlm = dE/dA_nlm = 2 C_lm Fp_{nl} A_nlm.  With G_lm = sum_n Q_nlm g_n, G'_lm = sum_n Q_nlm g_n':
+//   F_ij = rhat sum_lm G'_lm b_lm + [v - (rhat.v) rhat] / r,  v = sum_lm G_lm grad_u b_lm.
+// Own sums go to Fa (3 per atom; BEC: 9 per atom = 1/2 r_ij (x) c_ij), pair vectors to f12.
+// ------------------------------------------------------------------------------------------
+#define QNEP_HTERM(LM, B, GX, GY, GZ)                                        \
+    {                                                                        \
+        float G_ = 0.f, Gp_ = 0.f;                                           \
+        _Pragma("unroll") for (int a = 0; a < NR; ++a) {                     \
+            G_ = fmaf(Q[a][LM], gn[a], G_);                                  \
+            Gp_ = fmaf(Q[a][LM], dgn[a], Gp_);                               \
+        }                                                                    \
+        s0 = fmaf(Gp_, (B), s0);                                             \
+        vx = fmaf(G_, (GX), vx);                                             \
+        vy = fmaf(G_, (GY), vy);                                             \
+        vz = fmaf(G_, (GZ), vz);                                             \
+    }
+
+template <int T, bool BEC>
+__global__ void __launch_bounds__(64)
+k_force_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
+                const int* __restrict__ nn, const float* __restrict__ cA, float rcinv, const float* __restrict__ Fp,
+                const float* __restrict__ Ain, float4* __restrict__ f12, float* __restrict__ Fa,
+                double* __restrict__ sums)
+{
+    __shared__ float4 sh_shift[27];
+    __shared__ __align__(16) float sh_c[T * T * NR * KP];
+    __shared__ double sh_red[32];
+    load_shift_table(sh_shift, g);
+    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
+    __syncthreads();
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float W[9];
+#pragma unroll
+    for (int a = 0; a < 9; ++a) W[a] = 0.f;
+    if (p < N) {
+        const float4 xi = xyzt[p];
+        const int ti = __float_as_int(xi.w);
+        float Q[NR][NLM];
+#pragma unroll
+        for (int a = 0; a < NR; ++a) {
+            float fpl[4];
+#pragma unroll
+            for (int l = 0; l < 4; ++l) fpl[l] = 2.f * Fp[(int64_t)(NR + a * 4 + l) * N + p];
+#pragma unroll
+            for (int lm = 0; lm < NLM; ++lm)
+                Q[a][lm] = c_Clm[lm] * fpl[l_of_lm(lm)] * Ain[(int64_t)(a * NLM + lm) * N + p];
+        }
+        float Fx = 0.f, Fy = 0.f, Fz = 0.f;
+        const int n = nn[p];
+        for (int s = 0; s < n; ++s) {
+            const int e = nl[(int64_t)s * N + p];
+            const float4 xj = xyzt[e & QNEP_NL_MASK];
+            const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+            const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 >= g.rc_a2) { f12[(int64_t)s * N + p] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
+            const float r = sqrtf(r2), rinv = 1.f / r;
+            float f[NB], df[NB];
+            cheb_basis<true, true>(r, rcinv, f, df);
+            const float* c = sh_c + (ti * T + __float_as_int(xj.w)) * NR * KP;
+            float gn[NR], dgn[NR];
+#pragma unroll
+            for (int a = 0; a < NR; ++a) {
+                float v = 0.f, dv = 0.f;
+#pragma unroll
+                for (int k = 0; k < NB; ++k) { v = fmaf(c[a * KP + k], f[k], v); dv = fmaf(c[a * KP + k], df[k], dv); }
+                gn[a] = v; dgn[a] = dv;
+            }
+            const float x = dx * rinv, y = dy * rinv, z = dz * rinv;
+            const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z;
+            const float x2my2 = x2 - y2;
+            float s0 = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
+            // l = 1
+            QNEP_HTERM(0, z, 0.f, 0.f, 1.f)
+            QNEP_HTERM(1, x, 1.f, 0.f, 0.f)
+            QNEP_HTERM(2, y, 0.f, 1.f, 0.f)
+            // l = 2
+            QNEP_HTERM(3, 3.f * z2 - 1.f, 0.f, 0.f, 6.f * z)
+            QNEP_HTERM(4, xz, z, 0.f, x)
+            QNEP_HTERM(5, yz, 0.f, z, y)
+            QNEP_HTERM(6, x2my2, 2.f * x, -2.f * y, 0.f)
+            QNEP_HTERM(7, 2.f * xy, 2.f * y, 2.f * x, 0.f)
+            // l = 3
+            const float f5 = 5.f * z2 - 1.f;
+            const float t3 = 3.f * x2my2;            // 3x^2 - 3y^2
+            QNEP_HTERM(8, (5.f * z2 - 3.f) * z, 0.f, 0.f, 15.f * z2 - 3.f)
+            QNEP_HTERM(9, f5 * x, f5, 0.f, 10.f * xz)
+            QNEP_HTERM(10, f5 * y, 0.f, f5, 10.f * yz)
+            QNEP_HTERM(11, x2my2 * z, 2.f * xz, -2.f * yz, x2my2)
+            QNEP_HTERM(12, 2.f * xy * z, 2.f * yz, 2.f * xz, 2.f * xy)
+            QNEP_HTERM(13, (x2 - 3.f * y2) * x, t3, -6.f * xy, 0.f)
+            QNEP_HTERM(14, (3.f * x2 - y2) * y, 6.f * xy, t3, 0.f)
+            // l = 4
+            const float f7 = 7.f * z2 - 1.f, f73 = 7.f * z2 - 3.f;
+            const float cx = (x2 - 3.f * y2) * x, cy = (3.f * x2 - y2) * y;   // x^3 - 3xy^2, 3x^2 y - y^3
+            QNEP_HTERM(15, (35.f * z2 - 30.f) * z2 + 3.f, 0.f, 0.f, (140.f * z2 - 60.f) * z)
+            QNEP_HTERM(16, f73 * xz, f73 * z, 0.f, (21.f * z2 - 3.f) * x)
+            QNEP_HTERM(17, f73 * yz, 0.f, f73 * z, (21.f * z2 - 3.f) * y)
+            QNEP_HTERM(18, f7 * x2my2, 2.f * x * f7, -2.f * y * f7, 14.f * z * x2my2)
+            QNEP_HTERM(19, f7 * 2.f * xy, 2.f * y * f7, 2.f * x * f7, 28.f * xy * z)
+            QNEP_HTERM(20, cx * z, t3 * z, -6.f * xy * z, cx)
+            QNEP_HTERM(21, cy * z, 6.f * xy * z, t3 * z, cy)
+            QNEP_HTERM(22, x2my2 * x2my2 - 4.f * x2 * y2, 4.f * cx, -4.f * cy, 0.f)
+            QNEP_HTERM(23, 4.f * x2my2 * xy, 4.f * cy, 4.f * cx, 0.f)
+            const float uv = x * vx + y * vy + z * vz;
+            const float fx = s0 * x + (vx - uv * x) * rinv;
+            const float fy = s0 * y + (vy - uv * y) * rinv;
+            const float fz = s0 * z + (vz - uv * z) * rinv;
+            f12[(int64_t)s * N + p] = make_float4(fx, fy, fz, 0.f);
+            Fx += fx; Fy += fy; Fz += fz;
+            // -r_ij (x) F_ij : virial partial (Eq. 12);  BEC: +1/2 r_ij (x) c_ij (Eq. 28)
+            W[0] = fmaf(dx, fx, W[0]); W[1] = fmaf(dx, fy, W[1]); W[2] = fmaf(dx, fz, W[2]);
+            W[3] = fmaf(dy, fx, W[3]); W[4] = fmaf(dy, fy, W[4]); W[5] = fmaf(dy, fz, W[5]);
+            W[6] = fmaf(dz, fx, W[6]); W[7] = fmaf(dz, fy, W[7]); W[8] = fmaf(dz, fz, W[8]);
+        }
+        if (BEC) {
+#pragma unroll
+            for (int a = 0; a < 9; ++a) Fa[(int64_t)a * N + p] = 0.5f * W[a];
+        } else {
+            Fa[p] = Fx; Fa[N + p] = Fy; Fa[2 * N + p] = Fz;
+        }
+    }
+    if (!BEC) {
+#pragma unroll
+        for (int a = 0; a < 9; ++a) {
+            const double w = block_sum((double)W[a], sh_red);
+            if (threadIdx.x == 0) atomicAdd(&sums[SUM_W0 + a], -w);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a11 (radial part + assembly): F_i = sum_j (s_ij + s_ji) rhat_ij  +  angular own sum
+//   - sum_j f12[rev][j]  +  static electrostatic force;  s_ij = sum_k P^{i,tj}_k f_k'(r_ij).
+// BEC mode (a12): Z_i = qt_i I + 1/2 sum_j r_ij (x) (c_ij + c_ji).
+// Output in ORIGINAL atom order, float64.
+// ------------------------------------------------------------------------------------------
+template <int T, bool BEC>
+__global__ void __launch_bounds__(128)
+k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nlR,
+               const int* __restrict__ nnR, const int* __restrict__ nlA, const int* __restrict__ nnA,
+               const int* __restrict__ revA, float rcinv, const float* __restrict__ P, const float4* __restrict__ f12,
+               const float* __restrict__ Fa, const float* __restrict__ Fs, const float* __restrict__ q, float sqrt_eps,
+               const int* __restrict__ sidx, double* __restrict__ out, double* __restrict__ sums)
+{
+    __shared__ float4 sh_shift[27];
+    __shared__ double sh_red[32];
+    load_shift_table(sh_shift, g);
+    __syncthreads();
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float W[9];
+#pragma unroll
+    for (int a = 0; a < 9; ++a) W[a] = 0.f;
+    if (p < N) {
+        const float4 xi = xyzt[p];
+        const int ti = __float_as_int(xi.w);
+        float Pi[T][NB];
+#pragma unroll
+        for (int t = 0; t < T; ++t) {
+            const float4* src = reinterpret_cast<const float4*>(P + ((int64_t)p * T + t) * KP);
+            const float4 a = src[0], b = src[1], c = src[2];
+            Pi[t][0] = a.x; Pi[t][1] = a.y; Pi[t][2] = a.z; Pi[t][3] = a.w;
+            Pi[t][4] = b.x; Pi[t][5] = b.y; Pi[t][6] = b.z; Pi[t][7] = b.w; Pi[t][8] = c.x;
+        }
+        float Fx = 0.f, Fy = 0.f, Fz = 0.f;
+        float Z[9];
+#pragma unroll
+        for (int a = 0; a < 9; ++a) Z[a] = 0.f;
+        const int n = nnR[p];
+        for (int s = 0; s < n; ++s) {
+            const int e = nlR[(int64_t)s * N + p];
+            const int j = e & QNEP_NL_MASK;
+            const float4 xj = xyzt[j];
+            const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+            const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 >= g.rc_r2) continue;
+            const float r = sqrtf(r2), rinv = 1.f / r;
+            float df[NB];
+            cheb_basis<false, true>(r, rcinv, nullptr, df);
+            const int tj = __float_as_int(xj.w);
+            const float4* pj = reinterpret_cast<const float4*>(P + ((int64_t)j * T + ti) * KP);
+            const float4 a = pj[0], b = pj[1], c = pj[2];
+            float sji = a.x * df[0];
+            sji = fmaf(a.y, df[1], sji); sji = fmaf(a.z, df[2], sji); sji = fmaf(a.w, df[3], sji);
+            sji = fmaf(b.x, df[4], sji); sji = fmaf(b.y, df[5], sji); sji = fmaf(b.z, df[6], sji);
+            sji = fmaf(b.w, df[7], sji); sji = fmaf(c.x, df[8], sji);
+            float sij = 0.f;
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+                float v = 0.f;
+#pragma unroll
+                for (int k = 0; k < NB; ++k) v = fmaf(Pi[t][k], df[k], v);
+                sij = (tj == t) ? v : sij;
+            }
+            const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+            if (BEC) {
+                // 1/2 r_ij (x) (c_ij + c_ji), c_ij = s_ij rhat, c_ji = s_ji rhat_ji = -s_ji rhat
+                const float w = 0.5f * (sij - sji);
+                Z[0] = fmaf(dx, w * ux, Z[0]); Z[1] = fmaf(dx, w * uy, Z[1]); Z[2] = fmaf(dx, w * uz, Z[2]);
+                Z[3] = fmaf(dy, w * ux, Z[3]); Z[4] = fmaf(dy, w * uy, Z[4]); Z[5] = fmaf(dy, w * uz, Z[5]);
+                Z[6] = fmaf(dz, w * ux, Z[6]); Z[7] = fmaf(dz, w * uy, Z[7]); Z[8] = fmaf(dz, w * uz, Z[8]);
+            } else {
+                const float w = sij + sji;
+                Fx = fmaf(w, ux, Fx); Fy = fmaf(w, uy, Fy); Fz = fmaf(w, uz, Fz);
+                const float wx = sij * ux, wy = sij * uy, wz = sij * uz;     // F_ij
+                W[0] = fmaf(dx, wx, W[0]); W[1] = fmaf(dx, wy, W[1]); W[2] = fmaf(dx, wz, W[2]);
+                W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
+                W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
+            }
+        }
+        // angular partial forces of the neighbours on i
+        const int na = nnA[p];
+        for (int s = 0; s < na; ++s) {
+            const int e = nlA[(int64_t)s * N + p];
+            const int j = e & QNEP_NL_MASK;
+            const int rs = revA[(int64_t)s * N + p];
+            const float4 fji = f12[(int64_t)rs * N + j];
+            if (BEC) {
+                const float4 xj = xyzt[j];
+                const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+                const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+                Z[0] = fmaf(0.5f * dx, fji.x, Z[0]); Z[1] = fmaf(0.5f * dx, fji.y, Z[1]); Z[2] = fmaf(0.5f * dx, fji.z, Z[2]);
+                Z[3] = fmaf(0.5f * dy, fji.x, Z[3]); Z[4] = fmaf(0.5f * dy, fji.y, Z[4]); Z[5] = fmaf(0.5f * dy, fji.z, Z[5]);
+                Z[6] = fmaf(0.5f * dz, fji.x, Z[6]); Z[7] = fmaf(0.5f * dz, fji.y, Z[7]); Z[8] = fmaf(0.5f * dz, fji.z, Z[8]);
+            } else {
+                Fx -= fji.x; Fy -= fji.y; Fz -= fji.z;
+            }
+        }
+        const int io = sidx[p];
+        if (BEC) {
+            const float qt = sqrt_eps * q[p];
+#pragma unroll
+            for (int a = 0; a < 9; ++a) {
+                float v = Z[a] + Fa[(int64_t)a * N + p];
+                if (a == 0 || a == 4 || a == 8) v += qt;
+                out[(int64_t)a * N + io] = (double)v;
+            }
+        } else {
+            out[io] = (double)Fx + (double)Fa[p] + (double)Fs[p];
+            out[N + io] = (double)Fy + (double)Fa[N + p] + (double)Fs[N + p];
+            out[2 * N + io] = (double)Fz + (double)Fa[2 * N + p] + (double)Fs[2 * N + p];
+        }
+    }
+    if (!BEC) {
+#pragma unroll
+        for (int a = 0; a < 9; ++a) {
+            const double w = block_sum((double)W[a], sh_red);
+            if (threadIdx.x == 0) atomicAdd(&sums[SUM_W0 + a], -w);
+        }
+    }
+}
+
+template <typename F>
+int dispatch_T(int T, F&& f)
+{
+    switch (T) {
+        case 1: f(std::integral_constant<int, 1>()); return 0;
+        case 2: f(std::integral_constant<int, 2>()); return 0;
+        case 3: f(std::integral_constant<int, 3>()); return 0;
+        case 4: f(std::integral_constant<int, 4>()); return 0;
+    }
+    return -1;
+}
+
+}  // namespace
+
+int qnep_launch_desc_radial(qnep_handle* h, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 127) / 128);
+    const float rcinv = (float)(1.0 / h->model.rc_r);
+    dispatch_T(h->model.n_types, [&](auto t) {
+        constexpr int T = decltype(t)::value;
+        k_desc_radial<T><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->d_D);
+    });
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 63) / 64);
+    const float rcinv = (float)(1.0 / h->model.rc_a);
+    dispatch_T(h->model.n_types, [&](auto t) {
+        constexpr int T = decltype(t)::value;
+        k_desc_angular<T><<<nb, 64, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlA, h->d_nnA, h->d_cA, rcinv, h->d_D, h->d_A);
+    });
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 127) / 128);
+    const size_t smem = sizeof(float) * (size_t)h->model.n_types * h->nn_stride;
+    static bool attr_set = false;
+    if (!attr_set) {
+        QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_set = true;
+    }
+    k_nn<<<nb, 128, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
+                               h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
+    const int nb2 = (int)((N + 255) / 256);
+    k_neutralise<<<nb2, 256, 0, s>>>(N, h->d_qraw, h->d_sums, h->model.q_total, h->d_sidx, h->d_q, charges_out);
+    h->launches += 2;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int qnep_launch_fp_combine(qnep_handle* h, bool bec, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 127) / 128);
+    dispatch_T(h->model.n_types, [&](auto t) {
+        constexpr int T = decltype(t)::value;
+        k_fp_combine<T><<<nb, 128, 0, s>>>(N, h->d_xyzt, h->d_FpU, h->d_FpQ, h->d_phi, h->d_sums, bec ? 1 : 0,
+                                           (float)h->model.sqrt_eps_inf, h->d_cR, h->d_Fp, h->d_P);
+    });
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int qnep_launch_force_angular(qnep_handle* h, bool bec, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 63) / 64);
+    const float rcinv = (float)(1.0 / h->model.rc_a);
+    dispatch_T(h->model.n_types, [&](auto t) {
+        constexpr int T = decltype(t)::value;
+        if (bec)
+            k_force_angular<T, true><<<nb, 64, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlA, h->d_nnA, h->d_cA, rcinv, h->d_Fp,
+                                                       h->d_A, h->d_f12, h->d_Fa, h->d_sums);
+        else
+            k_force_angular<T, false><<<nb, 64, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlA, h->d_nnA, h->d_cA, rcinv, h->d_Fp,
+                                                        h->d_A, h->d_f12, h->d_Fa, h->d_sums);
+    });
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int qnep_launch_force_radial(qnep_handle* h, bool bec, double* out, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 127) / 128);
+    const float rcinv = (float)(1.0 / h->model.rc_r);
+    dispatch_T(h->model.n_types, [&](auto t) {
+        constexpr int T = decltype(t)::value;
+        if (bec)
+            k_force_radial<T, true><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlA, h->d_nnA,
+                                                       h->d_revA, rcinv, h->d_P, h->d_f12, h->d_Fa, h->d_Fs, h->d_q,
+                                                       (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums);
+        else
+            k_force_radial<T, false><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlA, h->d_nnA,
+                                                        h->d_revA, rcinv, h->d_P, h->d_f12, h->d_Fa, h->d_Fs, h->d_q,
+                                                        (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums);
+    });
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}

@@ -1,0 +1,279 @@
+// neighbor.cu -- step a1 of SURVEY.md 8(a): cell list, (type, cell)-sorted atom order and the
+// radial / angular neighbour lists with image codes (PAPER.md :91, Eq. 13), plus the per-step
+// "prep" pass that turns fp64 positions into cell-relative fp32 coordinates.
+//
+// Layout decisions:
+//  * atoms are reordered by key = type * ncells + cell, so a warp holds atoms of ONE species
+//    (weights / coefficients become warp-uniform) that are close in space (gathers hit L1/L2);
+//  * positions are stored as float4 (x, y, z relative to the atom's own cell origin, type bits):
+//    r_ij = off_j - off_i + delta_cell * hcell is formed from small numbers, so fp32 keeps
+//    ~1e-7 A resolution in a 217 A box;
+//  * a neighbour entry packs the sorted index of j (27 bits) and the image code
+//    (dx+1)*9 + (dy+1)*3 + (dz+1) of the cell offset (5 bits): the same atom may appear more than
+//    once through different images when the box is smaller than 2 (r_c + skin);
+//  * lists are column-major [slot][atom] so that a warp reads consecutive words.
+#include "qnep_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ int pack3(int a, int b, int c) { return a | (b << 10) | (c << 20); }
+
+// ---- binning -------------------------------------------------------------------------------
+__global__ void k_bin_count(int64_t N, const double* __restrict__ pos, const int32_t* __restrict__ types,
+                            Geometry g, int* __restrict__ key, int* __restrict__ cnt)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int c[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        double f = pos[a * N + i] / g.L[a];
+        f -= floor(f);
+        int ci = (int)(f * g.ncell[a]);
+        c[a] = min(max(ci, 0), g.ncell[a] - 1);
+    }
+    int cell = (c[0] * g.ncell[1] + c[1]) * g.ncell[2] + c[2];
+    int k = types[i] * g.ncells + cell;
+    key[i] = k;
+    atomicAdd(&cnt[k], 1);
+}
+
+// single-block exclusive scan over n ints (n up to a few million; runs once per rebuild)
+__global__ void k_exclusive_scan(int n, const int* __restrict__ in, int* __restrict__ out)
+{
+    __shared__ int warp_sums[32];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int base = 0; base < n; base += blockDim.x) {
+        int idx = base + threadIdx.x;
+        int v = idx < n ? in[idx] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_sums[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            int w = lane < (blockDim.x >> 5) ? warp_sums[lane] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += y;
+            }
+            warp_sums[lane] = w;
+        }
+        __syncthreads();
+        int prefix = carry + (wid > 0 ? warp_sums[wid - 1] : 0) + x - v;
+        if (idx < n) out[idx] = prefix;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = prefix + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[n] = carry;
+}
+
+__global__ void k_scatter(int64_t N, const int* __restrict__ key, const int* __restrict__ start,
+                          int* __restrict__ fill, int* __restrict__ tmpidx)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int k = key[i];
+    int slot = start[k] + atomicAdd(&fill[k], 1);
+    tmpidx[slot] = (int)i;
+}
+
+// deterministic order inside a bucket: rank by original index
+__global__ void k_rank(int64_t N, const int* __restrict__ key, const int* __restrict__ start,
+                       const int* __restrict__ tmpidx, int* __restrict__ sidx)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    int me = tmpidx[p];
+    int k = key[me];
+    int b = start[k], e = start[k + 1];
+    int rank = 0;
+    for (int q = b; q < e; ++q) rank += (tmpidx[q] < me);
+    sidx[b + rank] = me;
+}
+
+// ---- per-step prep: cell-relative fp32 coordinates, PPPM mesh coordinates, skin check --------
+__global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t* __restrict__ types_or_null,
+                       const int* __restrict__ sidx, const int* __restrict__ key, Geometry g, int at_build,
+                       int* __restrict__ cellc, float4* __restrict__ xyzt, float4* __restrict__ off0,
+                       float4* __restrict__ mfrac, int* __restrict__ mi0, int* __restrict__ flags)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    int i = sidx[p];
+    int c[3];
+    int type;
+    if (at_build) {
+        int k = key[i];
+        type = k / g.ncells;
+        int cell = k - type * g.ncells;
+        c[2] = cell % g.ncell[2];
+        c[1] = (cell / g.ncell[2]) % g.ncell[1];
+        c[0] = cell / (g.ncell[2] * g.ncell[1]);
+        cellc[p] = pack3(c[0], c[1], c[2]);
+    } else {
+        int pc = cellc[p];
+        c[0] = pc & 1023; c[1] = (pc >> 10) & 1023; c[2] = (pc >> 20) & 1023;
+        type = __float_as_int(xyzt[p].w);
+    }
+    float off[3], dx[3];
+    int m0[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        double origin = c[a] * g.hcell[a];
+        double d = pos[a * N + i] - origin;
+        d -= g.L[a] * rint(d / g.L[a]);            // nearest image of the atom to its cell origin
+        off[a] = (float)d;
+        if (g.grid[a] > 0) {
+            double u = (origin + d) * g.hmesh_inv[a];
+            double r = floor(u + 0.5);
+            dx[a] = (float)(u - r);
+            int ir = (int)r % g.grid[a];
+            m0[a] = ir < 0 ? ir + g.grid[a] : ir;
+        } else { dx[a] = 0.f; m0[a] = 0; }
+    }
+    float4 v = make_float4(off[0], off[1], off[2], __int_as_float(type));
+    xyzt[p] = v;
+    mfrac[p] = make_float4(dx[0], dx[1], dx[2], 0.f);
+    mi0[p] = pack3(m0[0], m0[1], m0[2]);
+    if (at_build) {
+        off0[p] = v;
+    } else {
+        float4 o = off0[p];
+        float ddx = off[0] - o.x, ddy = off[1] - o.y, ddz = off[2] - o.z;
+        if (ddx * ddx + ddy * ddy + ddz * ddz > g.skin_half2) atomicOr(&flags[FLAG_SKIN], 1);
+    }
+}
+
+// ---- neighbour lists -------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ cellc,
+              const int* __restrict__ start, int capR, int capA, int* __restrict__ nlR, int* __restrict__ nnR,
+              int* __restrict__ nlA, int* __restrict__ nnA, int* __restrict__ flags)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const float4 xi = xyzt[p];
+    const int pc = cellc[p];
+    const int c0 = pc & 1023, c1 = (pc >> 10) & 1023, c2 = (pc >> 20) & 1023;
+    int nR = 0, nA = 0;
+    for (int code = 0; code < 27; ++code) {
+        const int d0 = code / 9 - 1, d1 = (code / 3) % 3 - 1, d2 = code % 3 - 1;
+        int n0 = c0 + d0, n1 = c1 + d1, n2 = c2 + d2;
+        n0 = n0 < 0 ? n0 + g.ncell[0] : (n0 >= g.ncell[0] ? n0 - g.ncell[0] : n0);
+        n1 = n1 < 0 ? n1 + g.ncell[1] : (n1 >= g.ncell[1] ? n1 - g.ncell[1] : n1);
+        n2 = n2 < 0 ? n2 + g.ncell[2] : (n2 >= g.ncell[2] ? n2 - g.ncell[2] : n2);
+        const int cell = (n0 * g.ncell[1] + n1) * g.ncell[2] + n2;
+        const float sx = d0 * (float)g.hcell[0], sy = d1 * (float)g.hcell[1], sz = d2 * (float)g.hcell[2];
+        for (int t = 0; t < T; ++t) {
+            const int k = t * g.ncells + cell;
+            const int b = start[k], e = start[k + 1];
+            for (int q = b; q < e; ++q) {
+                const float4 xj = xyzt[q];
+                const float dx = (xj.x - xi.x) + sx, dy = (xj.y - xi.y) + sy, dz = (xj.z - xi.z) + sz;
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 < g.rcs_r2 && r2 > 1e-12f && !(q == p && code == 13)) {
+                    const int entry = q | (code << QNEP_NL_SHIFT);
+                    if (nR < capR) nlR[(int64_t)nR * N + p] = entry;
+                    ++nR;
+                    if (r2 < g.rcs_a2) {
+                        if (nA < capA) nlA[(int64_t)nA * N + p] = entry;
+                        ++nA;
+                    }
+                }
+            }
+        }
+    }
+    nnR[p] = min(nR, capR);
+    nnA[p] = min(nA, capA);
+    // statistics / overflow detection: warp-aggregated
+    int mR = nR, mA = nA, sR = nR, sA = nA;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mR = max(mR, __shfl_xor_sync(0xffffffffu, mR, o));
+        mA = max(mA, __shfl_xor_sync(0xffffffffu, mA, o));
+        sR += __shfl_xor_sync(0xffffffffu, sR, o);
+        sA += __shfl_xor_sync(0xffffffffu, sA, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(&flags[FLAG_MAX_NR], mR);
+        atomicMax(&flags[FLAG_MAX_NA], mA);
+        atomicAdd((unsigned long long*)&flags[FLAG_SUM_NR], (unsigned long long)sR);
+    }
+    (void)sA;
+}
+
+// separate 64-bit sums need aligned slots: FLAG_SUM_NR uses ints [4..5]; angular sum is taken here
+__global__ void k_sum_counts(int64_t N, const int* __restrict__ nnA, unsigned long long* __restrict__ out)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int v = p < N ? nnA[p] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, (unsigned long long)v);
+}
+
+// reverse slot of every angular entry: the entry (p | 26 - code) in the list of q
+__global__ void k_build_reverse(int64_t N, int capA, const int* __restrict__ nlA, const int* __restrict__ nnA,
+                                int* __restrict__ revA, int* __restrict__ flags)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const int n = nnA[p];
+    for (int s = 0; s < n; ++s) {
+        const int e = nlA[(int64_t)s * N + p];
+        const int q = e & QNEP_NL_MASK, code = (unsigned)e >> QNEP_NL_SHIFT;
+        const int want = (int)p | ((26 - code) << QNEP_NL_SHIFT);
+        const int nq = nnA[q];
+        int found = -1;
+        for (int s2 = 0; s2 < nq; ++s2)
+            if (nlA[(int64_t)s2 * N + q] == want) { found = s2; break; }
+        if (found < 0) { atomicOr(&flags[FLAG_REV_MISS], 1); found = 0; }
+        revA[(int64_t)s * N + p] = found;
+    }
+}
+
+}  // namespace
+
+int qnep_launch_prep(qnep_handle* h, const double* pos, bool at_build, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 255) / 256);
+    k_prep<<<nb, 256, 0, s>>>(N, pos, nullptr, h->d_sidx, h->d_key, h->geo, at_build ? 1 : 0, h->d_cellc, h->d_xyzt,
+                              h->d_off0, h->d_mfrac, h->d_mi0, h->d_flags);
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 255) / 256);
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_cnt, 0, sizeof(int) * (h->nkeys + 1), s));
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_fill, 0, sizeof(int) * h->nkeys, s));
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_flags, 0, sizeof(int) * FLAG_COUNT, s));
+    k_bin_count<<<nb, 256, 0, s>>>(N, pos, types, h->geo, h->d_key, h->d_cnt);
+    k_exclusive_scan<<<1, 1024, 0, s>>>(h->nkeys, h->d_cnt, h->d_start);
+    k_scatter<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_fill, h->d_tmpidx);
+    k_rank<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_tmpidx, h->d_sidx);
+    h->launches += 4;
+    int rc = qnep_launch_prep(h, pos, true, s);
+    if (rc) return rc;
+    const int nb2 = (int)((N + 127) / 128);
+    k_build_lists<<<nb2, 128, 0, s>>>(N, h->model.n_types, h->geo, h->d_xyzt, h->d_cellc, h->d_start, h->capR, h->capA,
+                                     h->d_nlR, h->d_nnR, h->d_nlA, h->d_nnA, h->d_flags);
+    k_sum_counts<<<nb, 256, 0, s>>>(N, h->d_nnA, (unsigned long long*)&h->d_flags[FLAG_SUM_NA]);
+    k_build_reverse<<<nb2, 128, 0, s>>>(N, h->capA, h->d_nlA, h->d_nnA, h->d_revA, h->d_flags);
+    h->launches += 3;
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}

@@ -1,0 +1,163 @@
+// qnep_internal.cuh -- handle layout and launcher prototypes shared by the .cu files of the
+// B200-native qNEP force evaluation (arXiv 2601.19034).  Not part of the public boundary
+// (include/qnep.h).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/qnep.h"
+
+#define QNEP_MAX_TYPES 4
+#define QNEP_NLM 24                 // real harmonics l = 1..4: 3 + 5 + 7 + 9
+#define QNEP_NL_MASK 0x07ffffff     // neighbour entry: low 27 bits = sorted atom index, high 5 bits = image code 0..26
+#define QNEP_NL_SHIFT 27
+#define QNEP_KPAD 12                // Chebyshev coefficient rows padded from 9 to 12 floats (3 x float4)
+#define QNEP_NB 9                   // basis functions k = 0..8 (basis_r = basis_a = 8 in this version)
+#define QNEP_NRAD 5                 // n = 0..4
+#define QNEP_NDESC 25
+
+constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (reading S9)
+
+// device-side double accumulators
+enum { SUM_E_NEP = 0, SUM_Q, SUM_PHI, SUM_U_R, SUM_U_K, SUM_U_S, SUM_W0 /* 9 entries */, SUM_KE = 15, SUM_COUNT = 16 };
+// device-side int flags
+// ints 0..3 are 32-bit flags; ints 4..5 and 6..7 are two 64-bit counters
+enum { FLAG_MAX_NR = 0, FLAG_MAX_NA, FLAG_SKIN, FLAG_REV_MISS, FLAG_SUM_NR = 4, FLAG_SUM_NA = 6, FLAG_COUNT = 8 };
+
+struct Geometry {            // orthorhombic cell and the cell grid of the neighbour search
+    double L[3];
+    double hcell[3];         // cell edge = L / ncell >= rc_r + skin
+    int ncell[3];
+    int ncells;
+    float rc_r2, rc_a2;      // cutoffs squared
+    float rcs_r2, rcs_a2;    // (cutoff + skin)^2, used at build time
+    float skin_half2;        // (skin/2)^2
+    // PPPM
+    int grid[3];
+    double hmesh_inv[3];     // N / L
+};
+
+struct qnep_handle {
+    qnep_model_desc model;
+    qnep_es_desc es;
+    double alpha;            // resolved alpha
+    std::string err;
+    int64_t launches = 0;
+
+    // model on device
+    float* d_params = nullptr;       // raw copy
+    float* d_cR = nullptr;           // [T*T][5][KPAD]
+    float* d_cA = nullptr;           // [T*T][5][KPAD]
+    float* d_nn = nullptr;           // per type: w0[H][28] (scaler folded in? no: raw), b0[H], w1U[H], w1q[H]
+    int nn_stride = 0;               // floats per type in d_nn
+    float b1U = 0.f, b1q = 0.f;
+    std::vector<float> h_params;
+
+    // policy
+    double skin = 0.0;
+    int rebuild_every = 0;
+    int calls_since_build = -1;      // -1: never built
+    int user_capR = 0, user_capA = 0;
+    bool force_rebuild = true;
+
+    // workspace (sorted atom order p unless noted)
+    int64_t N = 0;                   // atoms the workspace is sized for
+    int capR = 0, capA = 0;
+    Geometry geo;
+    double box[9];
+    int nkeys = 0;
+    int* d_key = nullptr;            // [N] original order
+    int* d_cnt = nullptr;            // [nkeys + 1]
+    int* d_start = nullptr;          // [nkeys + 1]
+    int* d_fill = nullptr;           // [nkeys]
+    int* d_tmpidx = nullptr;         // [N]
+    int* d_sidx = nullptr;           // [N] sorted -> original
+    int* d_cellc = nullptr;          // [N] packed cell coordinates (10 bits each)
+    float4* d_xyzt = nullptr;        // [N] cell-relative position, w = type bits
+    float4* d_off0 = nullptr;        // [N] the same at build time (skin check)
+    float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, -)
+    int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each
+    int* d_nlR = nullptr;            // [capR][N]
+    int* d_nnR = nullptr;            // [N]
+    int* d_nlA = nullptr;            // [capA][N]
+    int* d_nnA = nullptr;            // [N]
+    int* d_revA = nullptr;           // [capA][N] slot of the reverse entry
+    float* d_D = nullptr;            // [25][N]
+    float* d_A = nullptr;            // [5*24][N]
+    float* d_Ui = nullptr;           // [N]
+    float* d_qraw = nullptr;         // [N]
+    float* d_q = nullptr;            // [N]
+    float* d_FpU = nullptr;          // [25][N]
+    float* d_FpQ = nullptr;          // [25][N]
+    float* d_Fp = nullptr;           // [25][N]
+    float* d_P = nullptr;            // [N][T][KPAD]  radial back-prop vectors P^{t}_k
+    float* d_phik = nullptr;         // [N]
+    float* d_phir = nullptr;         // [N]
+    float* d_phi = nullptr;          // [N]
+    float* d_Fs = nullptr;           // [3][N] static electrostatic force
+    float* d_Fa = nullptr;           // [3][N] own angular partial-force sum (or [9][N] in BEC mode)
+    float4* d_f12 = nullptr;         // [capA][N]
+    double* d_sums = nullptr;        // [SUM_COUNT]
+    int* d_flags = nullptr;          // [FLAG_COUNT]
+    int* h_flags = nullptr;          // pinned
+    cudaEvent_t ev_flags = nullptr;
+    bool flags_pending = false;
+    double* d_Fmd = nullptr;         // [3][N] forces kept for qnep_md_run (original order)
+    bool md_have_forces = false;
+
+    // Ewald
+    int nk = 0;
+    float4* d_kvec = nullptr;        // [nk] (kx, ky, kz, G)
+    int* d_kint = nullptr;           // [nk] packed integers
+    int ew_nmax = 0;
+    float2* d_ephase = nullptr;      // [3][nmax+1][N]
+    double2* d_S = nullptr;          // [nk]
+    // PPPM
+    int64_t ngrid = 0;
+    float* d_mesh = nullptr;         // [Nx][Ny][Nz] real charge mesh
+    float2* d_cm1 = nullptr;         // complex meshes
+    float2* d_cm2 = nullptr;
+    float* d_gtab = nullptr;         // 1-D influence tables: per axis N entries of (A_alpha) then k_alpha
+    float2* d_twiddle = nullptr;     // per axis twiddles
+    int tw_n = 0;
+
+    // host staging (qnep_compute_host)
+    double* d_hpos = nullptr; int32_t* d_htypes = nullptr; double* d_hout = nullptr; int64_t hostN = 0;
+
+    // timing
+    cudaEvent_t ev[QNEP_T_COUNT + 2] = {};
+    bool ev_valid = false;
+    bool rebuilt_last = false;
+    cudaStream_t last_stream = nullptr;
+};
+
+#define QNEP_CUDA_OK(h, call)                                                              \
+    do {                                                                                   \
+        cudaError_t e__ = (call);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            (h)->err = std::string(#call) + ": " + cudaGetErrorString(e__);                \
+            return e__ == cudaErrorMemoryAllocation ? QNEP_ERR_OOM : QNEP_ERR_CUDA;        \
+        }                                                                                  \
+    } while (0)
+
+// ---- launchers (each enqueues kernels on `s` and bumps h->launches) ----
+// neighbor.cu
+int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, cudaStream_t s);
+int qnep_launch_prep(qnep_handle* h, const double* pos, bool at_build, cudaStream_t s);
+// descriptor.cu
+int qnep_launch_desc_radial(qnep_handle* h, cudaStream_t s);
+int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s);
+int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s);
+int qnep_launch_fp_combine(qnep_handle* h, bool bec, cudaStream_t s);
+int qnep_launch_force_angular(qnep_handle* h, bool bec, cudaStream_t s);
+int qnep_launch_force_radial(qnep_handle* h, bool bec, double* out, cudaStream_t s);
+// electro.cu
+int qnep_launch_realspace(qnep_handle* h, cudaStream_t s);
+int qnep_launch_phi_finalize(qnep_handle* h, cudaStream_t s);
+int qnep_setup_ewald(qnep_handle* h);
+int qnep_launch_ewald(qnep_handle* h, const double* pos, cudaStream_t s);
+// pppm.cu
+int qnep_setup_pppm(qnep_handle* h);
+int qnep_launch_pppm(qnep_handle* h, cudaStream_t s);

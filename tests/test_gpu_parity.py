@@ -1,0 +1,251 @@
+"""GPU-vs-oracle parity of the whole hot path and of its stages, through the C ABI (marked gpu).
+
+Tolerances are BASELINE.json north_star's: energy <= 1e-5 eV/atom, forces <= 1e-4 relative RMS,
+charges <= 1e-5 e.  PPPM runs are compared with the oracle's PPPM (same algorithm in fp64), never with
+Ewald, because PPPM's own discretisation error is of the order of the force tolerance."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import paper_2601_19034_b200 as Q
+import qnep_inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL_E_PER_ATOM = 1e-5
+TOL_F_RELRMS = 1e-4
+TOL_Q = 1e-5
+TOL_W_REL = 1e-4      # of max |W_ab|; DESIGN.md derives it from the force tolerance
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def rel_rms(a, b):
+    return float(np.sqrt(((a - b) ** 2).sum() / (b ** 2).sum()))
+
+
+def gpu_eval(torch, w, want=Q.WANT_ALL, handle=None, skin=0.0, rebuild_every=0):
+    h = handle or Q.from_workload(w)
+    if skin or rebuild_every:
+        h.set_neighbor_policy(skin, rebuild_every)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    out = h.compute(pos, types, w.box, want=want)
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    return h, res
+
+
+def assert_parity(w, res, ref, label=""):
+    n = w.n_atoms
+    de = abs(res["energy"][0] - ref["energy"]) / n
+    df = rel_rms(res["forces"], ref["forces"])
+    dq = np.abs(res["charges"] - ref["charges"]).max()
+    dw = np.abs(res["virial"].reshape(3, 3) - ref["virial"]).max() / np.abs(ref["virial"]).max()
+    print(f"[parity {label or w.name}] N={n} dE/N={de:.2e} dF={df:.2e} dq={dq:.2e} dW={dw:.2e}")
+    assert de <= TOL_E_PER_ATOM, de
+    assert df <= TOL_F_RELRMS, df
+    assert dq <= TOL_Q, dq
+    assert dw <= TOL_W_REL, dw
+    return de, df, dq, dw
+
+
+# ---------------------------------------------------------------- config 0: Ewald, both modes
+@pytest.mark.parametrize("mode", [2, 1])
+def test_config0_ewald(torch, oracle, mode):
+    w = I.config0(mode=mode)
+    ref = oracle.compute_workload(w, use_bins=False, debug=True)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, ref, f"config0 mode {mode}")
+    # stage parity (T1): descriptors, site energies, raw charges, phi, Fp, static force
+    n, D = w.n_atoms, w.model.n_desc
+    Dg = h.debug_copy(Q.DBG_DESCRIPTORS, (n, D)).cpu().numpy()
+    assert np.abs(Dg - ref["D"]).max() <= 2e-5 * np.abs(ref["D"]).max()
+    assert np.abs(h.debug_copy(Q.DBG_SITE_ENERGY, (n,)).cpu().numpy() - ref["U_i"]).max() < 1e-5
+    assert np.abs(h.debug_copy(Q.DBG_Q_RAW, (n,)).cpu().numpy() - ref["q_raw"]).max() < 1e-5
+    assert np.abs(h.debug_copy(Q.DBG_PHI, (n,)).cpu().numpy() - ref["phi"]).max() < 2e-5 * max(1.0, np.abs(ref["phi"]).max())
+    Fpg = h.debug_copy(Q.DBG_FP, (n, D)).cpu().numpy()
+    assert rel_rms(Fpg, ref["Fp"]) < 1e-4
+    Fsg = h.debug_copy(Q.DBG_F_STATIC, (3, n)).cpu().numpy()
+    assert rel_rms(Fsg, ref["F_es"]) < 1e-4
+    parts = h.debug_copy(Q.DBG_ENERGY_PARTS, (4,)).cpu().numpy()
+    ep = ref["energy_parts"]
+    assert np.allclose(parts, [ep["nep"], ep["r"], ep["k"], ep["s"]], atol=1e-5 * n)
+    # neighbour statistics equal the oracle's brute-force image-aware search (small box: images matter)
+    cr, _, _ = oracle.neighbors(w.pos, w.box, w.model.rc_r)
+    ca, _, _ = oracle.neighbors(w.pos, w.box, w.model.rc_a)
+    st = h.neighbor_stats()
+    assert st["max_radial"] == cr.max() and st["max_angular"] == ca.max()
+    assert abs(st["mean_radial"] - cr.mean()) < 1e-9 and abs(st["mean_angular"] - ca.mean()) < 1e-9
+
+
+def test_config0_no_electrostatics_and_default_alpha(torch, oracle):
+    w = I.config0(mode=1)
+    w.es = replace(w.es, method=0)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, oracle.compute_workload(w, use_bins=False), "config0 no ES")
+    w.es = replace(w.es, method=1, alpha=-1.0, ewald_nmax2=0)     # alpha = pi/rc, kmax = 2 pi alpha (:91, :110)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, oracle.compute_workload(w, use_bins=False), "config0 paper defaults")
+
+
+# ---------------------------------------------------------------- config 1: water, PPPM
+@pytest.mark.parametrize("mode", [2, 1])
+def test_config1_pppm(torch, oracle, mode):
+    w = I.config1(mode=mode)
+    ref = oracle.compute_workload(w, debug=True)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, ref, f"config1 mode {mode}")
+    rho = h.debug_copy(Q.DBG_MESH_RHO, tuple(w.es.grid)).cpu().numpy()
+    assert np.abs(rho - ref["rho"]).max() <= 2e-6 * np.abs(ref["rho"]).max() + 1e-7
+    assert abs(rho.sum()) < 1e-3                                    # neutral mesh
+    n = w.n_atoms
+    assert np.abs(h.debug_copy(Q.DBG_PHI, (n,)).cpu().numpy() - ref["phi"]).max() < 2e-5 * max(1.0, np.abs(ref["phi"]).max())
+    assert rel_rms(h.debug_copy(Q.DBG_F_STATIC, (3, n)).cpu().numpy(), ref["F_es"]) < 1e-4
+    # invariants on the GPU output (T3)
+    assert np.abs(res["forces"].sum(axis=1)).max() < 1e-3
+    assert abs(res["charges"].sum()) < 1e-4
+    W = res["virial"].reshape(3, 3)
+    assert np.abs(W - W.T).max() < 1e-4 * np.abs(W).max()
+
+
+def test_config1_ragged_subsets(torch, oracle):
+    """Sizes that are not multiples of the block / warp / tile sizes, including a single warp's tail."""
+    w = I.config1()
+    for n_mol in (333, 11):
+        n = 3 * n_mol
+        sub = replace(w, pos=np.ascontiguousarray(w.pos[:, :n]), types=w.types[:n].copy())
+        ref = oracle.compute_workload(sub)
+        h, res = gpu_eval(torch, sub)
+        assert_parity(sub, res, ref, f"config1 first {n} atoms")
+
+
+# ---------------------------------------------------------------- config 3 cross-check: 3 species, Ewald and PPPM
+@pytest.mark.parametrize("method", [1, 2])
+def test_config3_crosscheck(torch, oracle, method):
+    w = I.config3(n_cells=8, grid=32, method=method)
+    ref = oracle.compute_workload(w)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, ref, f"config3 8^3 cells method {method}")
+
+
+def test_pppm_vs_ewald_accuracy_on_gpu(torch):
+    """PAPER.md:280 / SURVEY P7: at h = 1 A, P = 5 the PPPM forces agree with Ewald to ~1e-4."""
+    a = gpu_eval(torch, I.config3(n_cells=8, grid=32, method=1))[1]
+    b = gpu_eval(torch, I.config3(n_cells=8, grid=32, method=2))[1]
+    assert rel_rms(b["forces"], a["forces"]) < 1e-4
+    assert abs(a["energy"][0] - b["energy"][0]) / 2560 < 1e-5
+
+
+# ---------------------------------------------------------------- config 2: 4 species
+def test_config2_garnet(torch, oracle):
+    w = I.config2()
+    ref = oracle.compute_workload(w)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, ref, "config2")
+
+
+# ---------------------------------------------------------------- BEC (a12)
+def test_bec_parity_and_sum_rule(torch, oracle):
+    w = I.config0(mode=2)
+    ref = oracle.compute_workload(w, use_bins=False, want_bec=True)
+    h, res = gpu_eval(torch, w, want=Q.WANT_ALL | Q.WANT_BEC)
+    assert_parity(w, res, ref, "config0 + BEC")
+    assert np.abs(res["bec"] - ref["bec"]).max() < 1e-4 * max(1.0, np.abs(ref["bec"]).max())
+    Z = res["bec"].reshape(3, 3, -1).sum(axis=2)
+    assert np.abs(Z - w.model.sqrt_eps_inf * w.model.q_total * np.eye(3)).max() < 1e-4
+    w1 = I.config1()
+    ref1 = oracle.compute_workload(w1, want_bec=True)
+    h, res1 = gpu_eval(torch, w1, want=Q.WANT_ALL | Q.WANT_BEC)
+    assert rel_rms(res1["bec"], ref1["bec"]) < 1e-4
+
+
+# ---------------------------------------------------------------- neighbour policy, errors
+def test_skin_and_rebuild_identity(torch, oracle):
+    """Lists built with a skin and reused after the atoms moved give the same result as a fresh build."""
+    w = I.config1()
+    rng = np.random.Generator(np.random.PCG64(5))
+    moved = replace(w, pos=w.pos + rng.uniform(-0.2, 0.2, size=w.pos.shape))
+    ref = oracle.compute_workload(moved)
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(1.0, 10)
+    gpu_eval(torch, w, handle=h)                 # builds the lists at the OLD positions
+    _, res = gpu_eval(torch, moved, handle=h)    # reuses them
+    assert h.get_timings()["neighbor"] < 0.05    # no rebuild happened
+    assert_parity(moved, res, ref, "config1 skin=1.0 reuse")
+    # moving an atom by more than skin/2 is detected
+    far = moved.pos.copy()
+    far[0, 0] += 0.9
+    with pytest.raises(Q.QnepError) as ei:
+        gpu_eval(torch, replace(moved, pos=far), handle=h)
+    assert ei.value.code == Q.QNEP_ERR_SKIN_VIOLATED
+
+
+def test_neighbor_overflow_is_reported_and_recovered(torch, oracle):
+    w = I.config0()
+    h = Q.from_workload(w)
+    h.set_neighbor_capacity(8, 4)
+    with pytest.raises(Q.QnepError) as ei:
+        gpu_eval(torch, w, handle=h)
+    assert ei.value.code == Q.QNEP_ERR_NEIGHBOR_OVERFLOW
+    _, res = gpu_eval(torch, w, handle=h)        # capacity was grown
+    assert_parity(w, res, oracle.compute_workload(w, use_bins=False), "config0 after overflow")
+
+
+def test_unsupported_inputs(torch):
+    w = I.config0()
+    h = Q.from_workload(w)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    tric = w.box.copy()
+    tric[3] = 1.0
+    with pytest.raises(Q.QnepError) as ei:
+        h.compute(pos, types, tric)
+    assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED
+    small = np.diag([5.0, 11.28, 11.28]).ravel()
+    with pytest.raises(Q.QnepError) as ei:
+        h.compute(pos, types, small)
+    assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED
+
+
+def test_host_buffer_entry_point(torch, oracle):
+    w = I.config1()
+    h = Q.from_workload(w)
+    res = h.compute_host(w.pos, w.types, w.box)
+    assert_parity(w, res, oracle.compute_workload(w), "config1 via qnep_compute_host")
+
+
+def test_translation_and_permutation_on_gpu(torch):
+    w = I.config1()
+    _, a = gpu_eval(torch, w)
+    shifted = replace(w, pos=w.pos + np.array([[0.3712], [-5.17], [13.09]]))
+    _, b = gpu_eval(torch, shifted)
+    # PPPM is translation invariant only to its own accuracy (P9)
+    assert rel_rms(b["forces"], a["forces"]) < 1e-4
+    assert abs(a["energy"][0] - b["energy"][0]) / w.n_atoms < 1e-5
+    perm = np.random.Generator(np.random.PCG64(2)).permutation(w.n_atoms)
+    _, c = gpu_eval(torch, replace(w, pos=np.ascontiguousarray(w.pos[:, perm]), types=w.types[perm].copy()))
+    assert rel_rms(c["forces"], a["forces"][:, perm]) < 2e-5
+    assert np.abs(c["charges"] - a["charges"][perm]).max() < 2e-6
+
+
+def test_md_run_conserves_energy(torch):
+    """Velocity-Verlet around the force call (config 4's driver) on the 3000-atom box: total energy drift is small."""
+    w = I.config1()
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(1.0, 10)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    vel = torch.tensor(I.maxwell_boltzmann(w), dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    dt = 0.1 / 10.180505
+    e0 = h.md_run(pos, vel, types, w.box, w.masses, dt, 0).cpu().numpy()
+    ke0 = float((0.5 * torch.tensor(w.masses[w.types], device="cuda") * (vel ** 2).sum(0)).sum())
+    e1 = h.md_run(pos, vel, types, w.box, w.masses, dt, 20).cpu().numpy()
+    tot0, tot1 = e0[0] + ke0, e1[0] + e1[1]
+    assert abs(tot1 - tot0) / w.n_atoms < 2e-4, (tot0, tot1)
+    assert abs(e1[0] - e0[0]) > 1e-6            # the atoms did move
