@@ -150,7 +150,6 @@ int consume_flags(qnep_handle* h)
 {
     h->flags_pending = false;
     const int* f = h->h_flags;
-    if (f[FLAG_REV_MISS]) { h->err = "internal error: asymmetric angular neighbour list"; h->force_rebuild = true; return QNEP_ERR_CUDA; }
     if (f[FLAG_MAX_NR] > h->capR || f[FLAG_MAX_NA] > h->capA) {
         h->err = "neighbour list capacity exceeded (radial " + std::to_string(f[FLAG_MAX_NR]) + "/" + std::to_string(h->capR) +
                  ", angular " + std::to_string(f[FLAG_MAX_NA]) + "/" + std::to_string(h->capA) + "); capacity grown, call again";
@@ -159,6 +158,8 @@ int consume_flags(qnep_handle* h)
         h->force_rebuild = true;
         return QNEP_ERR_NEIGHBOR_OVERFLOW;
     }
+    // (a truncated list also breaks the reverse index, so overflow is tested first)
+    if (f[FLAG_REV_MISS]) { h->err = "internal error: asymmetric angular neighbour list"; h->force_rebuild = true; return QNEP_ERR_CUDA; }
     if (f[FLAG_SKIN]) {
         h->err = "an atom moved more than skin/2 since the last neighbour build";
         h->force_rebuild = true;
@@ -471,6 +472,7 @@ int qnep_compute(qnep_handle* h, int64_t n_atoms, const double* pos_dev, const i
         if ((rc = consume_flags(h))) return rc;
     }
     if ((rc = ensure_workspace(h, n_atoms, box))) return rc;
+    h->md_have_forces = false;
     return run_pipeline(h, n_atoms, pos_dev, types_dev, want, energy_dev, forces_dev, virial_dev, charges_dev, bec_dev, s);
 }
 
