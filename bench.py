@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- atom-steps/s of the full qNEP+PPPM force evaluation (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (neighbour build amortised at the
+configured interval, descriptors, NN, PPPM, folded back-prop, force/virial assembly) inside the library's
+velocity-Verlet driver (qnep_md_run), i.e. BASELINE.json configs[4]: 1,029,000-atom water-like box,
+PPPM 256^3, neighbour rebuild every 10 steps, timed per force evaluation.
+
+Prints ONE JSON line (see the keys below).  N > 1 runs N independent replicas (the path is single-GPU by
+the north_star: "replicas only"), one process per GPU, timed as the max over ranks.
+
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import qnep_inputs as I  # noqa: E402
+
+METRIC = "atom-steps/s for full qNEP+PPPM force eval"
+FS = 1.0 / 10.180505          # 1 fs in natural units (Angstrom * sqrt(amu/eV))
+
+# ---- algorithmic work model, frozen before optimisation --------
+FLOPS_ANG_BWD_PER_NEIGHBOUR = 1500.0   # angular backward, per angular neighbour inside r_c^A
+FLOPS_ANG_FWD_PER_NEIGHBOUR = 450.0
+FLOPS_RAD_FWD_PER_NEIGHBOUR = 150.0
+FLOPS_RAD_BWD_PER_NEIGHBOUR = 250.0
+FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.4: 148 SMs x 128 lanes x 2 x 1.965 GHz
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+def make_workload(cfg: int, args):
+    if cfg == 4:
+        return I.config4(n_side=args.n_side) if args.n_side else I.config4()
+    if cfg == 3:
+        return I.config3()
+    return I.CONFIGS[cfg]()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smmax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.lines if t0 - 0.05 <= t <= t1 + 0.2] or [l for (_, l) in self.lines]
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smmax.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smmax) if smmax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(sample_side: int, steps: int, warmup: int):
+    from oracle import oracle as O
+    O.build()
+    grid = 32 if sample_side <= 10 else (64 if sample_side <= 20 else (128 if sample_side <= 40 else 256))
+    w = I.config4(n_side=sample_side, grid=grid)
+    for _ in range(warmup):
+        O.compute_workload(w)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        O.compute_workload(w)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    sample = (f"fp64 oracle, one force evaluation of the config-4 construction at {sample_side}^3 molecules = "
+              f"{w.n_atoms} atoms, PPPM {grid}^3, wall clock")
+    return w.n_atoms / dt, dt, O.num_threads(), sample, w.n_atoms
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps, warmup = max(args.steps, 1), args.warmup
+    # bounded: keep the whole run within a few minutes
+    steps = min(steps, 5)
+    warmup = min(warmup, 1)
+    v, dt, cores, sample, n = time_oracle(args.cpu_sample_side, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "atom-steps/s", "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config4 water-like box, bounded sample ({n} atoms)", "sample": sample},
+            "cpu_baseline": {"value": v, "unit": "atom-steps/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "atom-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--n-side", type=int, default=0, help="override molecules per side of config 4 (debug)")
+    ap.add_argument("--skin", type=float, default=1.0)
+    ap.add_argument("--rebuild-every", type=int, default=10)
+    ap.add_argument("--dt-fs", type=float, default=0.5)
+    ap.add_argument("--cpu-sample-side", type=int, default=40)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2601_19034_b200 as Q
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    K, Wm = max(args.steps, 1), max(args.warmup, 3)
+
+    w = make_workload(args.config, args)
+    n = w.n_atoms
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(args.skin, args.rebuild_every)
+    masses = w.masses if w.masses is not None else np.ones(w.model.n_types)
+    pos0 = torch.tensor(w.pos, dtype=torch.float64, device=dev)
+    types = torch.tensor(w.types, dtype=torch.int32, device=dev)
+    vel0 = torch.tensor(I.maxwell_boltzmann(replace_masses(w, masses)), dtype=torch.float64, device=dev)
+
+    def md(pos, vel, nsteps, dt_fs):
+        return h.md_run(pos, vel, types, w.box, masses, dt_fs * FS, nsteps)
+
+    # warm-up (also grows neighbour capacity / shrinks dt if the random-init model is too violent)
+    dt_fs = args.dt_fs
+    pos, vel = pos0.clone(), vel0.clone()
+    for attempt in range(8):
+        try:
+            md(pos, vel, Wm, dt_fs)
+            break
+        except Q.QnepError as err:
+            if err.code == Q.QNEP_ERR_SKIN_VIOLATED:
+                dt_fs *= 0.5
+            elif err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
+                raise
+            pos, vel = pos0.clone(), vel0.clone()
+    else:
+        raise RuntimeError("warm-up failed")
+
+    # ---- timed region: exactly K steps, inputs resident in HBM -------------------------------------------
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    h.profile_reset()
+    l0 = h.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tw0 = time.time()
+    e0.record()
+    md(pos, vel, K, dt_fs)                       # synchronises at the end (device-side error check)
+    e1.record()
+    torch.cuda.synchronize()
+    tw1 = time.time()
+    if dist is not None:
+        dist.barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = h.kernel_launches() - l0
+    stage_ms, n_evals = h.profile_sum()
+    clocks = sampler.stop(tw0, tw1)
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_per_step = ms_total / K
+    value = world * n * K / (ms_total * 1e-3)
+    stats = h.neighbor_stats()
+
+    # ---- roofline of the dominant kernel ------------------------------------------------------------------
+    per_eval = {k: v / max(n_evals, 1) for k, v in stage_ms.items()}
+    # live angular neighbours (inside r_c^A) ~ list entries scaled by the volume ratio of cutoff and cutoff + skin
+    rc_a, rc_r = w.model.rc_a, w.model.rc_r
+    live_a = stats["mean_angular"] * (rc_a / (rc_a + args.skin)) ** 3
+    live_r = stats["mean_radial"] * (rc_r / (rc_r + args.skin)) ** 3
+    kernels = {
+        "k_force_angular": (per_eval["force_angular"], FLOPS_ANG_BWD_PER_NEIGHBOUR * live_a * n),
+        "k_desc_angular": (per_eval["desc_angular"], FLOPS_ANG_FWD_PER_NEIGHBOUR * live_a * n),
+    }
+    dom = max(kernels, key=lambda k: kernels[k][0])
+    dom_ms, dom_flops = kernels[dom]
+    achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS, "traffic": None,
+                "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops}
+    peaks = load_peaks()
+    mesh_bytes = float(np.prod(w.es.grid)) * 8.0
+    fft_bytes = 3 * 3 * 2 * mesh_bytes - float(np.prod(w.es.grid)) * 4.0   # 3 transforms x 3 passes x (read + write)
+    pppm = {"stage": "reciprocal (spread + 3 FFTs + influence + gather)", "bound": "hbm", "ms": per_eval["reciprocal"],
+            "algorithmic_bytes": 2.4e9 * float(np.prod(w.es.grid)) / 256 ** 3,
+            "peak": peaks["hbm_gbs"], "unit": "GB/s", "peak_source": peaks["source"]}
+    pppm["achieved"] = pppm["algorithmic_bytes"] / (pppm["ms"] * 1e-3) / 1e9 if pppm["ms"] > 0 else 0.0
+    pppm["frac"] = pppm["achieved"] / pppm["peak"]
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----------
+    hp = torch.empty((3, n), dtype=torch.float64).pin_memory()
+    hp.copy_(torch.from_numpy(np.ascontiguousarray(w.pos)))
+    ht = torch.from_numpy(np.ascontiguousarray(w.types)).pin_memory()
+    he = torch.empty(1, dtype=torch.float64).pin_memory()
+    hf = torch.empty((3, n), dtype=torch.float64).pin_memory()
+    want = Q.WANT_ENERGY | Q.WANT_FORCES
+    box9 = Q._box(w.box)
+    h2 = Q.from_workload(w)
+    h2.set_neighbor_policy(args.skin, args.rebuild_every)
+    Ke = max(1, min(args.e2e_steps, K))
+
+    def e2e_step():
+        h2.compute_host_raw(n, hp.data_ptr(), ht.data_ptr(), box9, want, he.data_ptr(), hf.data_ptr(), 0, 0, 0)
+
+    for _ in range(3):
+        try:
+            e2e_step()
+        except Q.QnepError as err:
+            if err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
+                raise
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        e2e_step()
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_e2e = float(t.item())
+    e2e = {"value": world * n * Ke / t_e2e, "unit": "atom-steps/s", "steps": Ke,
+           "h2d_bytes_per_step": int(hp.numel() * 8 + ht.numel() * 4), "d2h_bytes_per_step": int(hf.numel() * 8 + 8),
+           "api": "qnep_compute_host (pinned host buffers; neighbour rebuild every %d calls)" % args.rebuild_every}
+
+    # ---- CPU baseline: the oracle as it stands, on rank 0 at N = 1 only -----------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, dt, cores, sample, _ = time_oracle(args.cpu_sample_side, 1, 0)
+        cpu = {"value": v, "unit": "atom-steps/s", "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "n_atoms": n, "species": w.model.n_types, "pppm_grid": list(w.es.grid),
+                       "mode": w.model.mode, "n_neurons": w.model.n_neurons, "md": "velocity-Verlet via qnep_md_run",
+                       "dt_fs": dt_fs, "skin_A": args.skin, "rebuild_every": args.rebuild_every,
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2_policy": "inputs larger than L2 (neighbour lists + meshes >> 126 MB); no flush needed",
+                       "mean_neighbours_radial_list": stats["mean_radial"], "mean_neighbours_angular_list": stats["mean_angular"]},
+            "roofline": roofline, "roofline_pppm": pppm,
+            "stage_ms_per_eval": per_eval, "evals_profiled": n_evals,
+            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def replace_masses(w, masses):
+    if w.masses is None:
+        from dataclasses import replace
+        return replace(w, masses=np.asarray(masses, dtype=np.float64))
+    return w
+
+
+if __name__ == "__main__":
+    main()

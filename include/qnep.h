@@ -168,6 +168,15 @@ int qnep_check(qnep_handle *h);
 /* CUDA-event times in milliseconds of the last qnep_compute, ms[QNEP_T_*]; n = number of entries to write. Synchronises. */
 int qnep_get_timings(qnep_handle *h, float *ms_per_stage_host, int32_t n);
 
+/*
+ * Accumulated stage times: qnep_profile_reset() starts a window; qnep_profile_sum() synchronises and adds up the
+ * CUDA-event stage times (ms[QNEP_T_*], as qnep_get_timings) of every evaluation since the reset, including those run
+ * inside qnep_md_run (at most the 512 most recent); *n_evals = number of evaluations summed.  QNEP_T_FORCE_ANGULAR
+ * brackets exactly one kernel launch per evaluation (the angular partial-force kernel).
+ */
+int qnep_profile_reset(qnep_handle *h);
+int qnep_profile_sum(qnep_handle *h, float *ms_sum_host, int32_t n, int64_t *n_evals_host);
+
 /* number of kernels launched by this handle since creation (bench.py's gpu_launches claim) */
 int64_t qnep_kernel_launches(const qnep_handle *h);
 

@@ -36,7 +36,7 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
                "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_check", "qnep_get_timings",
-               "qnep_kernel_launches", "qnep_neighbor_stats", "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
+               "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_neighbor_stats", "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
 
 
 class qnep_model_desc(C.Structure):
@@ -88,6 +88,10 @@ def load_library():
     lib.qnep_check.argtypes = [vp]
     lib.qnep_get_timings.restype = C.c_int
     lib.qnep_get_timings.argtypes = [vp, C.POINTER(C.c_float), i32]
+    lib.qnep_profile_reset.restype = C.c_int
+    lib.qnep_profile_reset.argtypes = [vp]
+    lib.qnep_profile_sum.restype = C.c_int
+    lib.qnep_profile_sum.argtypes = [vp, C.POINTER(C.c_float), i32, C.POINTER(i64)]
     lib.qnep_kernel_launches.restype = i64
     lib.qnep_kernel_launches.argtypes = [vp]
     lib.qnep_neighbor_stats.restype = C.c_int
@@ -238,6 +242,16 @@ class QNEP:
         ms = (C.c_float * len(TIMING_NAMES))()
         self._ok(self._lib.qnep_get_timings(self._h, ms, len(TIMING_NAMES)))
         return {k: float(v) for k, v in zip(TIMING_NAMES, ms)}
+
+    def profile_reset(self):
+        self._ok(self._lib.qnep_profile_reset(self._h))
+
+    def profile_sum(self):
+        """(dict of summed stage times in ms, number of evaluations summed)."""
+        ms = (C.c_float * len(TIMING_NAMES))()
+        n = C.c_int64(0)
+        self._ok(self._lib.qnep_profile_sum(self._h, ms, len(TIMING_NAMES), C.byref(n)))
+        return {k: float(v) for k, v in zip(TIMING_NAMES, ms)}, int(n.value)
 
     def kernel_launches(self) -> int:
         return int(self._lib.qnep_kernel_launches(self._h))

@@ -306,7 +306,9 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     int rc;
     const bool rebuild = h->force_rebuild || h->rebuild_every <= 1 || h->calls_since_build < 0 ||
                          h->calls_since_build >= h->rebuild_every;
-    cudaEvent_t* ev = h->ev;
+    cudaEvent_t* ev = h->ring.data() + (size_t)(h->prof_count % qnep_handle::RING) * qnep_handle::NEV;
+    h->ev = ev;
+    h->prof_count += 1;
     QNEP_CUDA_OK(h, cudaEventRecord(ev[0], s));
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_sums, 0, sizeof(double) * SUM_COUNT, s));
     if (rebuild) {
@@ -331,11 +333,11 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     else if (h->es.method == 2) { if ((rc = qnep_launch_pppm(h, s))) return rc; }
     else QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
     if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[7], s));
     const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
+    if (need_forces) { if ((rc = qnep_launch_fp_combine(h, false, s))) return rc; }
+    QNEP_CUDA_OK(h, cudaEventRecord(ev[7], s));
     if (need_forces) {
-        if ((rc = qnep_launch_fp_combine(h, false, s))) return rc;
-        if ((rc = qnep_launch_force_angular(h, false, s))) return rc;
+        if ((rc = qnep_launch_force_angular(h, false, s))) return rc;     // bracketed alone by ev[7], ev[8]
         QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
         double* fout = ((want & QNEP_WANT_FORCES) && forces) ? forces : h->d_Fmd;
         if ((rc = qnep_launch_force_radial(h, false, fout, s))) return rc;
@@ -424,7 +426,8 @@ int qnep_create(const qnep_model_desc* model, const float* params_host, size_t n
     cudaMemset(h->d_flags, 0, sizeof(int) * FLAG_COUNT);
     std::memset(h->h_flags, 0, sizeof(int) * FLAG_COUNT);
     cudaEventCreateWithFlags(&h->ev_flags, cudaEventDisableTiming);
-    for (auto& e : h->ev) cudaEventCreate(&e);
+    h->ring.resize((size_t)qnep_handle::RING * qnep_handle::NEV);
+    for (auto& e : h->ring) cudaEventCreate(&e);
     *out = h;
     return QNEP_OK;
 }
@@ -567,6 +570,38 @@ int qnep_get_timings(qnep_handle* h, float* ms, int32_t n)
     return QNEP_OK;
 }
 
+int qnep_profile_reset(qnep_handle* h)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    h->prof_count = 0;
+    return QNEP_OK;
+}
+
+int qnep_profile_sum(qnep_handle* h, float* ms, int32_t n, int64_t* n_evals)
+{
+    if (!h || !ms || !n_evals) return QNEP_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) ms[i] = 0.f;
+    const int64_t cnt = std::min<int64_t>(h->prof_count, qnep_handle::RING);
+    *n_evals = cnt;
+    if (cnt == 0) return QNEP_OK;
+    QNEP_CUDA_OK(h, cudaStreamSynchronize(h->last_stream));
+    for (int64_t c = 0; c < cnt; ++c) {
+        const int64_t slot = (h->prof_count - 1 - c) % qnep_handle::RING;
+        cudaEvent_t* ev = h->ring.data() + (size_t)slot * qnep_handle::NEV;
+        for (int i = 0; i < QNEP_T_TOTAL && i < n; ++i) {
+            float t = 0.f;
+            QNEP_CUDA_OK(h, cudaEventElapsedTime(&t, ev[i], ev[i + 1]));
+            ms[i] += t;
+        }
+        if (n > QNEP_T_TOTAL) {
+            float t = 0.f;
+            QNEP_CUDA_OK(h, cudaEventElapsedTime(&t, ev[0], ev[QNEP_T_TOTAL]));
+            ms[QNEP_T_TOTAL] += t;
+        }
+    }
+    return QNEP_OK;
+}
+
 int64_t qnep_kernel_launches(const qnep_handle* h) { return h ? h->launches : 0; }
 
 int qnep_neighbor_stats(qnep_handle* h, double out[4])
@@ -626,7 +661,7 @@ void qnep_destroy(qnep_handle* h)
     for (void* p : ptrs) if (p) cudaFree(p);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     if (h->ev_flags) cudaEventDestroy(h->ev_flags);
-    for (auto& e : h->ev) if (e) cudaEventDestroy(e);
+    for (auto& e : h->ring) if (e) cudaEventDestroy(e);
     delete h;
 }
 

@@ -127,7 +127,11 @@ struct qnep_handle {
     double* d_hpos = nullptr; int32_t* d_htypes = nullptr; double* d_hout = nullptr; int64_t hostN = 0;
 
     // timing
-    cudaEvent_t ev[QNEP_T_COUNT + 2] = {};
+    static constexpr int NEV = QNEP_T_COUNT;   // events per evaluation: QNEP_T_TOTAL stage boundaries + 1
+    static constexpr int RING = 512;           // evaluations kept for qnep_profile_sum
+    std::vector<cudaEvent_t> ring;             // [RING][NEV]
+    int64_t prof_count = 0;                    // evaluations since qnep_profile_reset
+    cudaEvent_t* ev = nullptr;                 // event set of the last evaluation
     bool ev_valid = false;
     bool rebuilt_last = false;
     cudaStream_t last_stream = nullptr;
