@@ -240,10 +240,9 @@ def main():
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------------
     per_eval = {k: v / max(n_evals, 1) for k, v in stage_ms.items()}
-    # live angular neighbours (inside r_c^A) ~ list entries scaled by the volume ratio of cutoff and cutoff + skin
-    rc_a, rc_r = w.model.rc_a, w.model.rc_r
-    live_a = stats["mean_angular"] * (rc_a / (rc_a + args.skin)) ** 3
-    live_r = stats["mean_radial"] * (rc_r / (rc_r + args.skin)) ** 3
+    # neighbours inside the cutoffs at the last step (the exact per-step lists)
+    live_a, live_r = stats["mean_angular"], stats["mean_radial"]
+    fma_measured = Q.fma_peak()
     kernels = {
         "k_force_angular": (per_eval["force_angular"], FLOPS_ANG_BWD_PER_NEIGHBOUR * live_a * n),
         "k_desc_angular": (per_eval["desc_angular"], FLOPS_ANG_FWD_PER_NEIGHBOUR * live_a * n),
@@ -254,6 +253,7 @@ def main():
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS, "traffic": None,
                 "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                "fma_loop_measured_tflops": fma_measured, "frac_of_measured_fma_loop": achieved / fma_measured if fma_measured else None,
                 "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops}
     peaks = load_peaks()
     mesh_bytes = float(np.prod(w.es.grid)) * 8.0
@@ -317,7 +317,8 @@ def main():
                        "dt_fs": dt_fs, "skin_A": args.skin, "rebuild_every": args.rebuild_every,
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2_policy": "inputs larger than L2 (neighbour lists + meshes >> 126 MB); no flush needed",
-                       "mean_neighbours_radial_list": stats["mean_radial"], "mean_neighbours_angular_list": stats["mean_angular"]},
+                       "mean_skin_list": stats["mean_list"], "mean_neighbours_radial": stats["mean_radial"],
+                       "mean_neighbours_angular": stats["mean_angular"]},
             "roofline": roofline, "roofline_pppm": pppm,
             "stage_ms_per_eval": per_eval, "evals_profiled": n_evals,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,

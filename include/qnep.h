@@ -113,14 +113,14 @@ int qnep_create(const qnep_model_desc *model, const float *params_host, size_t n
 int qnep_set_electrostatics(qnep_handle *h, const qnep_es_desc *es);
 
 /*
- * Neighbour policy: lists hold every pair within r_c + skin and are rebuilt every `rebuild_every`
- * calls (0 or 1: every call).  Entries beyond r_c contribute exactly zero (the cutoff function
- * vanishes; the real-space Coulomb sum tests r < r_c explicitly), so results do not depend on skin.
- * Default: skin = 0, rebuild every call.
+ * Neighbour policy: the cell list and the skin list (every pair within rc_r + skin) are rebuilt every
+ * `rebuild_every` calls (0 or 1: every call).  Every call derives the exact lists (r < rc_r, r < rc_a) of
+ * its own positions from the skin list, so results do not depend on skin.  Default: skin = 0, rebuild every call.
  */
 int qnep_set_neighbor_policy(qnep_handle *h, double skin, int32_t rebuild_every);
 
-/* Override the automatic neighbour-list capacities (entries per atom); <= 0 keeps the automatic value. */
+/* Override the automatic list capacities (entries per atom): cap_radial sizes the skin list and the live radial
+ * list, cap_angular the live angular list; <= 0 keeps the automatic value. */
 int qnep_set_neighbor_capacity(qnep_handle *h, int32_t cap_radial, int32_t cap_angular);
 
 /*
@@ -180,8 +180,18 @@ int qnep_profile_sum(qnep_handle *h, float *ms_sum_host, int32_t n, int64_t *n_e
 /* number of kernels launched by this handle since creation (bench.py's gpu_launches claim) */
 int64_t qnep_kernel_launches(const qnep_handle *h);
 
-/* live neighbour statistics of the last build: out[0..3] = max radial, max angular, mean radial, mean angular (synchronises) */
-int qnep_neighbor_stats(qnep_handle *h, double out_host[4]);
+/*
+ * Neighbour statistics of the last call (synchronises): out[0], out[1] = max / mean length of the skin list
+ * (r < rc_r + skin at build time); out[2], out[3] = max / mean number of radial neighbours inside rc_r;
+ * out[4], out[5] = max / mean number of angular neighbours inside rc_a (the exact per-step lists).
+ */
+int qnep_neighbor_stats(qnep_handle *h, double out_host[6]);
+
+/*
+ * FP32 FMA throughput of the current device in TFLOP/s: a dependent-free FFMA loop on every SM, best of 4 launches,
+ * CUDA-event timed on `cuda_stream`.  bench.py reports it beside the nominal FP32 peak.  Synchronises.
+ */
+int qnep_fma_peak(double *tflops_host, void *cuda_stream);
 
 /*
  * Copy a per-stage intermediate of the last qnep_compute into a caller-owned DEVICE float64 buffer

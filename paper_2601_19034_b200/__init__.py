@@ -36,7 +36,8 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
                "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_check", "qnep_get_timings",
-               "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_neighbor_stats", "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
+               "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_neighbor_stats", "qnep_fma_peak",
+               "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
 
 
 class qnep_model_desc(C.Structure):
@@ -96,6 +97,8 @@ def load_library():
     lib.qnep_kernel_launches.argtypes = [vp]
     lib.qnep_neighbor_stats.restype = C.c_int
     lib.qnep_neighbor_stats.argtypes = [vp, C.POINTER(dbl)]
+    lib.qnep_fma_peak.restype = C.c_int
+    lib.qnep_fma_peak.argtypes = [C.POINTER(dbl), vp]
     lib.qnep_debug_copy.restype = C.c_int
     lib.qnep_debug_copy.argtypes = [vp, i32, vp, i64]
     lib.qnep_destroy.restype = None
@@ -257,15 +260,25 @@ class QNEP:
         return int(self._lib.qnep_kernel_launches(self._h))
 
     def neighbor_stats(self) -> dict:
-        out = (C.c_double * 4)()
+        out = (C.c_double * 6)()
         self._ok(self._lib.qnep_neighbor_stats(self._h, out))
-        return dict(max_radial=out[0], max_angular=out[1], mean_radial=out[2], mean_angular=out[3])
+        return dict(max_list=out[0], mean_list=out[1], max_radial=out[2], mean_radial=out[3],
+                    max_angular=out[4], mean_angular=out[5])
 
     def debug_copy(self, which: int, shape):
         import torch
         t = torch.zeros(shape, dtype=torch.float64, device="cuda")
         self._ok(self._lib.qnep_debug_copy(self._h, which, C.c_void_p(t.data_ptr()), t.numel()))
         return t
+
+
+def fma_peak(stream=None) -> float:
+    """Measured FP32 FMA throughput of the current device, TFLOP/s (qnep_fma_peak)."""
+    out = C.c_double(0.0)
+    rc = load_library().qnep_fma_peak(C.byref(out), QNEP._stream(stream))
+    if rc != QNEP_OK:
+        raise QnepError(rc, "qnep_fma_peak failed")
+    return float(out.value)
 
 
 def from_workload(w) -> QNEP:

@@ -24,11 +24,11 @@ void free_workspace(qnep_handle* h)
 {
     void** ptrs[] = {(void**)&h->d_key, (void**)&h->d_cnt, (void**)&h->d_start, (void**)&h->d_fill, (void**)&h->d_tmpidx,
                      (void**)&h->d_sidx, (void**)&h->d_cellc, (void**)&h->d_xyzt, (void**)&h->d_off0, (void**)&h->d_mfrac,
-                     (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_nlA, (void**)&h->d_nnA,
-                     (void**)&h->d_revA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
+                     (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_lvR, (void**)&h->d_nlvR,
+                     (void**)&h->d_lvA, (void**)&h->d_nlvA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
                      (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_P,
-                     (void**)&h->d_phik, (void**)&h->d_phir, (void**)&h->d_phi, (void**)&h->d_Fs, (void**)&h->d_Fa,
-                     (void**)&h->d_f12, (void**)&h->d_Fmd};
+                     (void**)&h->d_phik, (void**)&h->d_phir, (void**)&h->d_phi, (void**)&h->d_Fs, (void**)&h->d_Facc,
+                     (void**)&h->d_Fmd};
     for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
     h->N = 0;
     h->md_have_forces = false;
@@ -87,11 +87,12 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         const double expect = 4.0 / 3.0 * M_PI * rc_ * rc_ * rc_ * rho;
         return ((int)(expect * 1.5) + 24 + 3) / 4 * 4;
     };
-    const int capR = cap_for(h->model.rc_r + h->skin, h->user_capR);
-    const int capA = cap_for(h->model.rc_a + h->skin, h->user_capA);
+    const int capR = cap_for(h->model.rc_r + h->skin, h->user_capR);     // skin list
+    const int capLR = cap_for(h->model.rc_r, h->user_capLR);             // live radial list
+    const int capLA = cap_for(h->model.rc_a, h->user_capA);              // live angular pairs
     const int T = h->model.n_types;
     const int nkeys = T * g.ncells;
-    const bool realloc_atoms = N != h->N || capR != h->capR || capA != h->capA;
+    const bool realloc_atoms = N != h->N || capR != h->capR || capLR != h->capLR || capLA != h->capLA;
     if (realloc_atoms) {
         free_workspace(h);
         const size_t n = (size_t)N;
@@ -105,9 +106,10 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_mi0, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_nlR, n * capR))) return rc;
         if ((rc = dev_alloc(h, &h->d_nnR, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_nlA, n * capA))) return rc;
-        if ((rc = dev_alloc(h, &h->d_nnA, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_revA, n * capA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_lvR, n * capLR))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nlvR, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_lvA, n * capLA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nlvA, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_D, n * QNEP_NDESC))) return rc;
         if ((rc = dev_alloc(h, &h->d_A, n * QNEP_NRAD * QNEP_NLM))) return rc;
         if ((rc = dev_alloc(h, &h->d_Ui, n))) return rc;
@@ -121,10 +123,11 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_phir, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_phi, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_Fs, n * 3))) return rc;
-        if ((rc = dev_alloc(h, &h->d_Fa, n * 9))) return rc;
-        if ((rc = dev_alloc(h, &h->d_f12, n * capA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Facc, n * 9))) return rc;
         if ((rc = dev_alloc(h, &h->d_Fmd, n * 3))) return rc;
-        h->N = N; h->capR = capR; h->capA = capA;
+        h->N = N; h->capR = capR; h->capLR = capLR; h->capLA = capLA;
+        QNEP_CUDA_OK(h, cudaMemset(h->d_nlvR, 0, sizeof(int) * n));
+        QNEP_CUDA_OK(h, cudaMemset(h->d_nlvA, 0, sizeof(int) * n));
         h->force_rebuild = true;
     }
     if (nkeys != h->nkeys || !h->d_cnt) {
@@ -150,16 +153,24 @@ int consume_flags(qnep_handle* h)
 {
     h->flags_pending = false;
     const int* f = h->h_flags;
-    if (f[FLAG_MAX_NR] > h->capR || f[FLAG_MAX_NA] > h->capA) {
-        h->err = "neighbour list capacity exceeded (radial " + std::to_string(f[FLAG_MAX_NR]) + "/" + std::to_string(h->capR) +
-                 ", angular " + std::to_string(f[FLAG_MAX_NA]) + "/" + std::to_string(h->capA) + "); capacity grown, call again";
-        h->user_capR = std::max(h->capR, (f[FLAG_MAX_NR] * 5 / 4 + 8 + 3) / 4 * 4);
-        h->user_capA = std::max(h->capA, (f[FLAG_MAX_NA] * 5 / 4 + 8 + 3) / 4 * 4);
+    if (f[FLAG_MAX_NR] > h->capR || f[FLAG_MAX_LR] > h->capLR || f[FLAG_MAX_LA] > h->capLA) {
+        h->err = "neighbour list capacity exceeded (skin list " + std::to_string(f[FLAG_MAX_NR]) + "/" + std::to_string(h->capR) +
+                 ", live radial " + std::to_string(f[FLAG_MAX_LR]) + "/" + std::to_string(h->capLR) + ", live angular " +
+                 std::to_string(f[FLAG_MAX_LA]) + "/" + std::to_string(h->capLA) + "); capacity grown, call again";
+        auto grow = [](int cap, int seen) { return std::max(cap, (seen * 5 / 4 + 8 + 3) / 4 * 4); };
+        if (f[FLAG_MAX_NR] > h->capR) {
+            // the truncated skin list hid the true live counts: scale them from the skin-list count by the volume ratios
+            h->user_capR = grow(h->capR, f[FLAG_MAX_NR]);
+            const double rcs = h->model.rc_r + h->skin;
+            const double fr = std::pow(h->model.rc_r / rcs, 3.0), fa = std::pow(h->model.rc_a / rcs, 3.0);
+            h->user_capLR = grow(h->capLR, (int)(f[FLAG_MAX_NR] * fr * 1.1) + 1);
+            h->user_capA = grow(h->capLA, (int)(f[FLAG_MAX_NR] * fa * 1.3) + 1);
+        }
+        if (f[FLAG_MAX_LR] > h->capLR) h->user_capLR = grow(h->capLR, f[FLAG_MAX_LR]);
+        if (f[FLAG_MAX_LA] > h->capLA) h->user_capA = grow(h->capLA, f[FLAG_MAX_LA]);
         h->force_rebuild = true;
         return QNEP_ERR_NEIGHBOR_OVERFLOW;
     }
-    // (a truncated list also breaks the reverse index, so overflow is tested first)
-    if (f[FLAG_REV_MISS]) { h->err = "internal error: asymmetric angular neighbour list"; h->force_rebuild = true; return QNEP_ERR_CUDA; }
     if (f[FLAG_SKIN]) {
         h->err = "an atom moved more than skin/2 since the last neighbour build";
         h->force_rebuild = true;
@@ -321,7 +332,7 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     if (!rebuild) { if ((rc = qnep_launch_prep(h, pos, false, s))) return rc; }
     h->calls_since_build += 1;
     QNEP_CUDA_OK(h, cudaEventRecord(ev[2], s));
-    if ((rc = qnep_launch_desc_radial(h, s))) return rc;
+    if ((rc = qnep_launch_pairs(h, s))) return rc;
     QNEP_CUDA_OK(h, cudaEventRecord(ev[3], s));
     if ((rc = qnep_launch_desc_angular(h, s))) return rc;
     QNEP_CUDA_OK(h, cudaEventRecord(ev[4], s));
@@ -334,13 +345,14 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     else QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
     if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
     const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
+    const bool need_virial = (want & QNEP_WANT_VIRIAL) != 0;
     if (need_forces) { if ((rc = qnep_launch_fp_combine(h, false, s))) return rc; }
     QNEP_CUDA_OK(h, cudaEventRecord(ev[7], s));
     if (need_forces) {
-        if ((rc = qnep_launch_force_angular(h, false, s))) return rc;     // bracketed alone by ev[7], ev[8]
+        if ((rc = qnep_launch_force_angular(h, false, need_virial, s))) return rc;     // bracketed alone by ev[7], ev[8]
         QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
         double* fout = ((want & QNEP_WANT_FORCES) && forces) ? forces : h->d_Fmd;
-        if ((rc = qnep_launch_force_radial(h, false, fout, s))) return rc;
+        if ((rc = qnep_launch_force_radial(h, false, need_virial, fout, s))) return rc;
     } else {
         QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
     }
@@ -350,8 +362,8 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     QNEP_CUDA_OK(h, cudaEventRecord(ev[9], s));
     if ((want & QNEP_WANT_BEC) && bec) {
         if ((rc = qnep_launch_fp_combine(h, true, s))) return rc;
-        if ((rc = qnep_launch_force_angular(h, true, s))) return rc;
-        if ((rc = qnep_launch_force_radial(h, true, bec, s))) return rc;
+        if ((rc = qnep_launch_force_angular(h, true, false, s))) return rc;
+        if ((rc = qnep_launch_force_radial(h, true, false, bec, s))) return rc;
     }
     QNEP_CUDA_OK(h, cudaEventRecord(ev[10], s));
     h->ev_valid = true;
@@ -459,6 +471,7 @@ int qnep_set_neighbor_capacity(qnep_handle* h, int32_t cap_radial, int32_t cap_a
 {
     if (!h) return QNEP_ERR_INVALID_ARG;
     h->user_capR = cap_radial > 0 ? cap_radial : 0;
+    h->user_capLR = h->user_capR;
     h->user_capA = cap_angular > 0 ? cap_angular : 0;
     h->force_rebuild = true;
     return QNEP_OK;
@@ -604,19 +617,18 @@ int qnep_profile_sum(qnep_handle* h, float* ms, int32_t n, int64_t* n_evals)
 
 int64_t qnep_kernel_launches(const qnep_handle* h) { return h ? h->launches : 0; }
 
-int qnep_neighbor_stats(qnep_handle* h, double out[4])
+int qnep_neighbor_stats(qnep_handle* h, double out[6])
 {
     if (!h || !out) return QNEP_ERR_INVALID_ARG;
-    if (!h->d_flags || h->N == 0) { out[0] = out[1] = out[2] = out[3] = 0; return QNEP_OK; }
-    QNEP_CUDA_OK(h, cudaStreamSynchronize(h->last_stream));
-    int f[FLAG_COUNT];
-    QNEP_CUDA_OK(h, cudaMemcpy(f, h->d_flags, sizeof(f), cudaMemcpyDeviceToHost));
-    unsigned long long sr, sa;
-    std::memcpy(&sr, &f[FLAG_SUM_NR], 8);
-    std::memcpy(&sa, &f[FLAG_SUM_NA], 8);
-    out[0] = f[FLAG_MAX_NR]; out[1] = f[FLAG_MAX_NA];
-    out[2] = (double)sr / (double)h->N; out[3] = (double)sa / (double)h->N;
-    return QNEP_OK;
+    for (int i = 0; i < 6; ++i) out[i] = 0;
+    if (!h->d_flags || h->N == 0) return QNEP_OK;
+    return qnep_launch_list_stats(h, out, h->last_stream);
+}
+
+int qnep_fma_peak(double* tflops_host, void* cuda_stream)
+{
+    if (!tflops_host) return QNEP_ERR_INVALID_ARG;
+    return qnep_launch_fma_peak(tflops_host, (cudaStream_t)cuda_stream);
 }
 
 int qnep_debug_copy(qnep_handle* h, int32_t which, double* dst, int64_t n)

@@ -7,6 +7,11 @@
 // One thread owns one atom; atoms are (type, cell)-sorted so a warp is type-uniform and its
 // neighbour gathers hit the same cache lines.  All per-neighbour state lives in registers.
 //
+// Per step the skin list is walked ONCE (k_pairs): it accumulates the radial descriptors and emits the
+// exact lists of this step -- the live radial list (packed indices) and the live angular pairs
+// (dx, dy, dz, j | tj), which the angular kernels then stream coalesced, with no gather and no skin-shell
+// divergence.
+//
 // Algebra used to keep the hot loops on the FP32 FMA pipe:
 //   * radial:  D_n = sum_j sum_k c^{ti tj}_{nk} f_k(r_ij) = sum_t sum_k c^{ti t}_{nk} S^t_k,
 //     S^t_k = sum_{j in t} f_k(r_ij): the per-neighbour work is the 9 basis values only; the
@@ -16,10 +21,11 @@
 //     D_nl = sum_m C_lm A_nlm^2 equals the Legendre double sum of the definition by the addition
 //     theorem (weights C_lm are exact rationals, see harmonic weights below).
 //   * F_ji of the radial part is recomputed by atom i from P^{ti}_k of atom j (no atomics, no
-//     pair storage); the angular F_ij are stored once per pair and fetched through a reverse
-//     index built with the neighbour list (deterministic, no atomics).
+//     pair storage); the angular F_ij is added to atom i's own sum and scattered to atom j with
+//     fp32 atomic adds (RED) into a zeroed accumulator.
 #include "qnep_internal.cuh"
 
+#include <algorithm>
 #include <type_traits>
 
 namespace {
@@ -42,13 +48,16 @@ template <bool VAL, bool DERIV>
 __device__ __forceinline__ void cheb_basis(float r, float rcinv, float* __restrict__ f, float* __restrict__ df)
 {
     const float t = r * rcinv;
-    const float fc = 0.5f + 0.5f * cospif(t);
+    float sn, cs;                                   // MUFU sin / cos of pi t, t in [0, 1]: abs error < 5e-7
+    if (DERIV) __sincosf(3.14159265358979f * t, &sn, &cs);
+    else cs = __cosf(3.14159265358979f * t);
+    const float fc = 0.5f + 0.5f * cs;
     const float tm1 = t - 1.f;
     const float x = 2.f * tm1 * tm1 - 1.f;
     const float hfc = 0.5f * fc;
     float dfc = 0.f, dx = 0.f, hdxfc = 0.f, hdfc = 0.f;
     if (DERIV) {
-        dfc = -1.5707963267948966f * rcinv * sinpif(t);
+        dfc = -1.5707963267948966f * rcinv * sn;
         dx = 4.f * tm1 * rcinv;
         hdxfc = 0.5f * dx * fc;
         hdfc = 0.5f * dfc;
@@ -96,12 +105,16 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: radial descriptors
+// a2: one walk over the skin list: radial descriptors + the exact lists of this step
+//   live radial entry : the skin-list word (sorted index | image code << 27)
+//   live angular pair : (dx, dy, dz, bits(sorted index | type << 27))
 // ------------------------------------------------------------------------------------------
 template <int T>
 __global__ void __launch_bounds__(128)
-k_desc_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
-              const int* __restrict__ nn, const float* __restrict__ cR, float rcinv, float* __restrict__ D)
+k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
+        const int* __restrict__ nn, const float* __restrict__ cR, float rcinv, int capLR, int capLA,
+        int* __restrict__ lvR, int* __restrict__ nlvR, float4* __restrict__ lvA, int* __restrict__ nlvA,
+        float* __restrict__ D, int* __restrict__ flags)
 {
     __shared__ float4 sh_shift[27];
     __shared__ float sh_c[T * T * NR * KP];
@@ -118,16 +131,26 @@ k_desc_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int*
 #pragma unroll
         for (int k = 0; k < NB; ++k) S[t][k] = 0.f;
     const int n = nn[p];
+    int cR_ = 0, cA_ = 0;
+    int e_next = n > 0 ? nl[p] : 0;
     for (int s = 0; s < n; ++s) {
-        const int e = nl[(int64_t)s * N + p];
-        const float4 xj = xyzt[e & QNEP_NL_MASK];
+        const int e = e_next;
+        if (s + 1 < n) e_next = nl[(int64_t)(s + 1) * N + p];
+        const int j = e & QNEP_NL_MASK;
+        const float4 xj = xyzt[j];
         const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
         const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
         const float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 >= g.rc_r2) continue;
-        float f[NB];
-        cheb_basis<true, false>(sqrtf(r2), rcinv, f, nullptr);
+        if (r2 >= g.rc_r2 || r2 < 1e-12f) continue;
         const int tj = __float_as_int(xj.w);
+        if (cR_ < capLR) lvR[(int64_t)cR_ * N + p] = e;
+        ++cR_;
+        if (r2 < g.rc_a2) {
+            if (cA_ < capLA) lvA[(int64_t)cA_ * N + p] = make_float4(dx, dy, dz, __int_as_float(j | (tj << QNEP_NL_SHIFT)));
+            ++cA_;
+        }
+        float f[NB];
+        cheb_basis<true, false>(r2 * rsqrtf(r2), rcinv, f, nullptr);
 #pragma unroll
         for (int t = 0; t < T; ++t) {
             const float w = (tj == t) ? 1.f : 0.f;
@@ -135,6 +158,10 @@ k_desc_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int*
             for (int k = 0; k < NB; ++k) S[t][k] = fmaf(w, f[k], S[t][k]);
         }
     }
+    nlvR[p] = min(cR_, capLR);
+    nlvA[p] = min(cA_, capLA);
+    if (cR_ > capLR) atomicMax(&flags[FLAG_MAX_LR], cR_);
+    if (cA_ > capLA) atomicMax(&flags[FLAG_MAX_LA], cA_);
 #pragma unroll
     for (int nidx = 0; nidx < NR; ++nidx) {
         float d = 0.f;
@@ -171,36 +198,31 @@ __device__ __forceinline__ void harmonics(float x, float y, float z, float* __re
 // ------------------------------------------------------------------------------------------
 template <int T>
 __global__ void __launch_bounds__(64)
-k_desc_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
-               const int* __restrict__ nn, const float* __restrict__ cA, float rcinv, float* __restrict__ D,
-               float* __restrict__ Aout)
+k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, const int* __restrict__ nlvA,
+               const float* __restrict__ cA, float rcinv, float* __restrict__ D, float* __restrict__ Aout)
 {
-    __shared__ float4 sh_shift[27];
     __shared__ __align__(16) float sh_c[T * T * NR * KP];
-    load_shift_table(sh_shift, g);
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
     __syncthreads();
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
-    const float4 xi = xyzt[p];
-    const int ti = __float_as_int(xi.w);
+    const int ti = __float_as_int(xyzt[p].w);
     float A[NR][NLM];
 #pragma unroll
     for (int a = 0; a < NR; ++a)
 #pragma unroll
         for (int lm = 0; lm < NLM; ++lm) A[a][lm] = 0.f;
-    const int n = nn[p];
+    const int n = nlvA[p];
+    float4 pr_next = n > 0 ? lvA[p] : make_float4(0.f, 0.f, 0.f, 0.f);
     for (int s = 0; s < n; ++s) {
-        const int e = nl[(int64_t)s * N + p];
-        const float4 xj = xyzt[e & QNEP_NL_MASK];
-        const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-        const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 >= g.rc_a2) continue;
-        const float r = sqrtf(r2), rinv = 1.f / r;
+        const float4 pr = pr_next;
+        if (s + 1 < n) pr_next = lvA[(int64_t)(s + 1) * N + p];
+        const float r2 = pr.x * pr.x + pr.y * pr.y + pr.z * pr.z;
+        const float rinv = rsqrtf(r2), r = r2 * rinv;
         float f[NB];
         cheb_basis<true, false>(r, rcinv, f, nullptr);
-        const float* c = sh_c + (ti * T + __float_as_int(xj.w)) * NR * KP;
+        const int tj = (unsigned)__float_as_int(pr.w) >> QNEP_NL_SHIFT;
+        const float* c = sh_c + (ti * T + tj) * NR * KP;
         float gn[NR];
 #pragma unroll
         for (int a = 0; a < NR; ++a) {
@@ -210,7 +232,7 @@ k_desc_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int
             gn[a] = v;
         }
         float b[NLM];
-        harmonics(dx * rinv, dy * rinv, dz * rinv, b);
+        harmonics(pr.x * rinv, pr.y * rinv, pr.z * rinv, b);
 #pragma unroll
         for (int a = 0; a < NR; ++a)
 #pragma unroll
@@ -368,17 +390,14 @@ k_fp_combine(int64_t N, const float4* __restrict__ xyzt, const float* __restrict
         vz = fmaf(G_, (GZ), vz);                                             \
     }
 
-template <int T, bool BEC>
+template <int T, bool BEC, bool VIRIAL>
 __global__ void __launch_bounds__(64)
-k_force_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
-                const int* __restrict__ nn, const float* __restrict__ cA, float rcinv, const float* __restrict__ Fp,
-                const float* __restrict__ Ain, float4* __restrict__ f12, float* __restrict__ Fa,
-                double* __restrict__ sums)
+k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, const int* __restrict__ nlvA,
+                const float* __restrict__ cA, float rcinv, const float* __restrict__ Fp, const float* __restrict__ Ain,
+                float* __restrict__ Facc, double* __restrict__ sums)
 {
-    __shared__ float4 sh_shift[27];
     __shared__ __align__(16) float sh_c[T * T * NR * KP];
     __shared__ double sh_red[32];
-    load_shift_table(sh_shift, g);
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
     __syncthreads();
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -386,8 +405,7 @@ k_force_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const in
 #pragma unroll
     for (int a = 0; a < 9; ++a) W[a] = 0.f;
     if (p < N) {
-        const float4 xi = xyzt[p];
-        const int ti = __float_as_int(xi.w);
+        const int ti = __float_as_int(xyzt[p].w);
         float Q[NR][NLM];
 #pragma unroll
         for (int a = 0; a < NR; ++a) {
@@ -399,18 +417,19 @@ k_force_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const in
                 Q[a][lm] = c_Clm[lm] * fpl[l_of_lm(lm)] * Ain[(int64_t)(a * NLM + lm) * N + p];
         }
         float Fx = 0.f, Fy = 0.f, Fz = 0.f;
-        const int n = nn[p];
+        const int n = nlvA[p];
+        float4 pr_next = n > 0 ? lvA[p] : make_float4(0.f, 0.f, 0.f, 0.f);
         for (int s = 0; s < n; ++s) {
-            const int e = nl[(int64_t)s * N + p];
-            const float4 xj = xyzt[e & QNEP_NL_MASK];
-            const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-            const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+            const float4 pr = pr_next;
+            if (s + 1 < n) pr_next = lvA[(int64_t)(s + 1) * N + p];
+            const float dx = pr.x, dy = pr.y, dz = pr.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 >= g.rc_a2) { f12[(int64_t)s * N + p] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
-            const float r = sqrtf(r2), rinv = 1.f / r;
+            const float rinv = rsqrtf(r2), r = r2 * rinv;
             float f[NB], df[NB];
             cheb_basis<true, true>(r, rcinv, f, df);
-            const float* c = sh_c + (ti * T + __float_as_int(xj.w)) * NR * KP;
+            const int jw = __float_as_int(pr.w);
+            const int j = jw & QNEP_NL_MASK;
+            const float* c = sh_c + (ti * T + (int)((unsigned)jw >> QNEP_NL_SHIFT)) * NR * KP;
             float gn[NR], dgn[NR];
 #pragma unroll
             for (int a = 0; a < NR; ++a) {
@@ -459,21 +478,31 @@ k_force_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const in
             const float fx = s0 * x + (vx - uv * x) * rinv;
             const float fy = s0 * y + (vy - uv * y) * rinv;
             const float fz = s0 * z + (vz - uv * z) * rinv;
-            f12[(int64_t)s * N + p] = make_float4(fx, fy, fz, 0.f);
-            Fx += fx; Fy += fy; Fz += fz;
-            // -r_ij (x) F_ij : virial partial (Eq. 12);  BEC: +1/2 r_ij (x) c_ij (Eq. 28)
-            W[0] = fmaf(dx, fx, W[0]); W[1] = fmaf(dx, fy, W[1]); W[2] = fmaf(dx, fz, W[2]);
-            W[3] = fmaf(dy, fx, W[3]); W[4] = fmaf(dy, fy, W[4]); W[5] = fmaf(dy, fz, W[5]);
-            W[6] = fmaf(dz, fx, W[6]); W[7] = fmaf(dz, fy, W[7]); W[8] = fmaf(dz, fz, W[8]);
+            if (BEC) {
+                // Z_i += 1/2 r_ij (x) c_ij ;  Z_j += 1/2 r_ji (x) c_ij = -1/2 r_ij (x) c_ij   (Eq. 28)
+                const float hx = 0.5f * dx, hy = 0.5f * dy, hz = 0.5f * dz;
+                const float z9[9] = {hx * fx, hx * fy, hx * fz, hy * fx, hy * fy, hy * fz, hz * fx, hz * fy, hz * fz};
+#pragma unroll
+                for (int a = 0; a < 9; ++a) { W[a] += z9[a]; atomicAdd(&Facc[(int64_t)a * N + j], -z9[a]); }
+            } else {
+                // F_i += F_ij, F_j -= F_ij (Eq. 11)
+                Fx += fx; Fy += fy; Fz += fz;
+                atomicAdd(&Facc[j], -fx); atomicAdd(&Facc[N + j], -fy); atomicAdd(&Facc[2 * N + j], -fz);
+                if (VIRIAL) {   // -r_ij (x) F_ij (Eq. 12)
+                    W[0] = fmaf(dx, fx, W[0]); W[1] = fmaf(dx, fy, W[1]); W[2] = fmaf(dx, fz, W[2]);
+                    W[3] = fmaf(dy, fx, W[3]); W[4] = fmaf(dy, fy, W[4]); W[5] = fmaf(dy, fz, W[5]);
+                    W[6] = fmaf(dz, fx, W[6]); W[7] = fmaf(dz, fy, W[7]); W[8] = fmaf(dz, fz, W[8]);
+                }
+            }
         }
         if (BEC) {
 #pragma unroll
-            for (int a = 0; a < 9; ++a) Fa[(int64_t)a * N + p] = 0.5f * W[a];
+            for (int a = 0; a < 9; ++a) atomicAdd(&Facc[(int64_t)a * N + p], W[a]);
         } else {
-            Fa[p] = Fx; Fa[N + p] = Fy; Fa[2 * N + p] = Fz;
+            atomicAdd(&Facc[p], Fx); atomicAdd(&Facc[N + p], Fy); atomicAdd(&Facc[2 * N + p], Fz);
         }
     }
-    if (!BEC) {
+    if (!BEC && VIRIAL) {
 #pragma unroll
         for (int a = 0; a < 9; ++a) {
             const double w = block_sum((double)W[a], sh_red);
@@ -483,17 +512,16 @@ k_force_angular(int64_t N, Geometry g, const float4* __restrict__ xyzt, const in
 }
 
 // ------------------------------------------------------------------------------------------
-// a11 (radial part + assembly): F_i = sum_j (s_ij + s_ji) rhat_ij  +  angular own sum
-//   - sum_j f12[rev][j]  +  static electrostatic force;  s_ij = sum_k P^{i,tj}_k f_k'(r_ij).
+// a11 (radial part + assembly): F_i = sum_j (s_ij + s_ji) rhat_ij  +  angular accumulator
+//   +  static electrostatic force;  s_ij = sum_k P^{i,tj}_k f_k'(r_ij).
 // BEC mode (a12): Z_i = qt_i I + 1/2 sum_j r_ij (x) (c_ij + c_ji).
 // Output in ORIGINAL atom order, float64.
 // ------------------------------------------------------------------------------------------
-template <int T, bool BEC>
+template <int T, bool BEC, bool VIRIAL>
 __global__ void __launch_bounds__(128)
-k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nlR,
-               const int* __restrict__ nnR, const int* __restrict__ nlA, const int* __restrict__ nnA,
-               const int* __restrict__ revA, float rcinv, const float* __restrict__ P, const float4* __restrict__ f12,
-               const float* __restrict__ Fa, const float* __restrict__ Fs, const float* __restrict__ q, float sqrt_eps,
+k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ lvR,
+               const int* __restrict__ nlvR, float rcinv, const float* __restrict__ P, const float* __restrict__ Facc,
+               const float* __restrict__ Fs, const float* __restrict__ q, float sqrt_eps,
                const int* __restrict__ sidx, double* __restrict__ out, double* __restrict__ sums)
 {
     __shared__ float4 sh_shift[27];
@@ -516,24 +544,31 @@ k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int
             Pi[t][4] = b.x; Pi[t][5] = b.y; Pi[t][6] = b.z; Pi[t][7] = b.w; Pi[t][8] = c.x;
         }
         float Fx = 0.f, Fy = 0.f, Fz = 0.f;
-        float Z[9];
-#pragma unroll
-        for (int a = 0; a < 9; ++a) Z[a] = 0.f;
-        const int n = nnR[p];
+        const int n = nlvR[p];
+        // software pipeline: list word two ahead, gathered records one ahead
+        int e_nn = n > 1 ? lvR[N + p] : 0;
+        int e_n = n > 0 ? lvR[p] : 0;
+        float4 xj_n = xyzt[e_n & QNEP_NL_MASK];
+        const float4* pj_n = reinterpret_cast<const float4*>(P + ((int64_t)(e_n & QNEP_NL_MASK) * T + ti) * KP);
+        float4 pa_n = pj_n[0], pb_n = pj_n[1], pc_n = pj_n[2];
         for (int s = 0; s < n; ++s) {
-            const int e = nlR[(int64_t)s * N + p];
-            const int j = e & QNEP_NL_MASK;
-            const float4 xj = xyzt[j];
+            const int e = e_n;
+            const float4 xj = xj_n, a = pa_n, b = pb_n, c = pc_n;
+            e_n = e_nn;
+            if (s + 2 < n) e_nn = lvR[(int64_t)(s + 2) * N + p];
+            if (s + 1 < n) {
+                const int jn = e_n & QNEP_NL_MASK;
+                xj_n = xyzt[jn];
+                pj_n = reinterpret_cast<const float4*>(P + ((int64_t)jn * T + ti) * KP);
+                pa_n = pj_n[0]; pb_n = pj_n[1]; pc_n = pj_n[2];
+            }
             const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
             const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 >= g.rc_r2) continue;
-            const float r = sqrtf(r2), rinv = 1.f / r;
+            const float rinv = rsqrtf(r2), r = r2 * rinv;
             float df[NB];
             cheb_basis<false, true>(r, rcinv, nullptr, df);
             const int tj = __float_as_int(xj.w);
-            const float4* pj = reinterpret_cast<const float4*>(P + ((int64_t)j * T + ti) * KP);
-            const float4 a = pj[0], b = pj[1], c = pj[2];
             float sji = a.x * df[0];
             sji = fmaf(a.y, df[1], sji); sji = fmaf(a.z, df[2], sji); sji = fmaf(a.w, df[3], sji);
             sji = fmaf(b.x, df[4], sji); sji = fmaf(b.y, df[5], sji); sji = fmaf(b.z, df[6], sji);
@@ -550,34 +585,18 @@ k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int
             if (BEC) {
                 // 1/2 r_ij (x) (c_ij + c_ji), c_ij = s_ij rhat, c_ji = s_ji rhat_ji = -s_ji rhat
                 const float w = 0.5f * (sij - sji);
-                Z[0] = fmaf(dx, w * ux, Z[0]); Z[1] = fmaf(dx, w * uy, Z[1]); Z[2] = fmaf(dx, w * uz, Z[2]);
-                Z[3] = fmaf(dy, w * ux, Z[3]); Z[4] = fmaf(dy, w * uy, Z[4]); Z[5] = fmaf(dy, w * uz, Z[5]);
-                Z[6] = fmaf(dz, w * ux, Z[6]); Z[7] = fmaf(dz, w * uy, Z[7]); Z[8] = fmaf(dz, w * uz, Z[8]);
+                W[0] = fmaf(dx, w * ux, W[0]); W[1] = fmaf(dx, w * uy, W[1]); W[2] = fmaf(dx, w * uz, W[2]);
+                W[3] = fmaf(dy, w * ux, W[3]); W[4] = fmaf(dy, w * uy, W[4]); W[5] = fmaf(dy, w * uz, W[5]);
+                W[6] = fmaf(dz, w * ux, W[6]); W[7] = fmaf(dz, w * uy, W[7]); W[8] = fmaf(dz, w * uz, W[8]);
             } else {
                 const float w = sij + sji;
                 Fx = fmaf(w, ux, Fx); Fy = fmaf(w, uy, Fy); Fz = fmaf(w, uz, Fz);
-                const float wx = sij * ux, wy = sij * uy, wz = sij * uz;     // F_ij
-                W[0] = fmaf(dx, wx, W[0]); W[1] = fmaf(dx, wy, W[1]); W[2] = fmaf(dx, wz, W[2]);
-                W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
-                W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
-            }
-        }
-        // angular partial forces of the neighbours on i
-        const int na = nnA[p];
-        for (int s = 0; s < na; ++s) {
-            const int e = nlA[(int64_t)s * N + p];
-            const int j = e & QNEP_NL_MASK;
-            const int rs = revA[(int64_t)s * N + p];
-            const float4 fji = f12[(int64_t)rs * N + j];
-            if (BEC) {
-                const float4 xj = xyzt[j];
-                const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-                const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
-                Z[0] = fmaf(0.5f * dx, fji.x, Z[0]); Z[1] = fmaf(0.5f * dx, fji.y, Z[1]); Z[2] = fmaf(0.5f * dx, fji.z, Z[2]);
-                Z[3] = fmaf(0.5f * dy, fji.x, Z[3]); Z[4] = fmaf(0.5f * dy, fji.y, Z[4]); Z[5] = fmaf(0.5f * dy, fji.z, Z[5]);
-                Z[6] = fmaf(0.5f * dz, fji.x, Z[6]); Z[7] = fmaf(0.5f * dz, fji.y, Z[7]); Z[8] = fmaf(0.5f * dz, fji.z, Z[8]);
-            } else {
-                Fx -= fji.x; Fy -= fji.y; Fz -= fji.z;
+                if (VIRIAL) {
+                    const float wx = sij * ux, wy = sij * uy, wz = sij * uz;     // F_ij
+                    W[0] = fmaf(dx, wx, W[0]); W[1] = fmaf(dx, wy, W[1]); W[2] = fmaf(dx, wz, W[2]);
+                    W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
+                    W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
+                }
             }
         }
         const int io = sidx[p];
@@ -585,23 +604,43 @@ k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int
             const float qt = sqrt_eps * q[p];
 #pragma unroll
             for (int a = 0; a < 9; ++a) {
-                float v = Z[a] + Fa[(int64_t)a * N + p];
+                float v = W[a] + Facc[(int64_t)a * N + p];
                 if (a == 0 || a == 4 || a == 8) v += qt;
                 out[(int64_t)a * N + io] = (double)v;
             }
         } else {
-            out[io] = (double)Fx + (double)Fa[p] + (double)Fs[p];
-            out[N + io] = (double)Fy + (double)Fa[N + p] + (double)Fs[N + p];
-            out[2 * N + io] = (double)Fz + (double)Fa[2 * N + p] + (double)Fs[2 * N + p];
+            out[io] = (double)Fx + (double)Facc[p] + (double)Fs[p];
+            out[N + io] = (double)Fy + (double)Facc[N + p] + (double)Fs[N + p];
+            out[2 * N + io] = (double)Fz + (double)Facc[2 * N + p] + (double)Fs[2 * N + p];
         }
     }
-    if (!BEC) {
+    if (!BEC && VIRIAL) {
 #pragma unroll
         for (int a = 0; a < 9; ++a) {
             const double w = block_sum((double)W[a], sh_red);
             if (threadIdx.x == 0) atomicAdd(&sums[SUM_W0 + a], -w);
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// dependent-free FFMA loop: the FP32 roofline denominator measured in the same run
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_fma_peak(int iters, float seed, float* __restrict__ out)
+{
+    float a[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = seed + (float)(threadIdx.x + i);
+    const float m = 0.999999f, c = 1e-7f * seed;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = fmaf(a[i], m, c);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+    if (s == 123.456f) out[0] = s;     // never true; keeps the loop alive
 }
 
 template <typename F>
@@ -618,14 +657,15 @@ int dispatch_T(int T, F&& f)
 
 }  // namespace
 
-int qnep_launch_desc_radial(qnep_handle* h, cudaStream_t s)
+int qnep_launch_pairs(qnep_handle* h, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
     const float rcinv = (float)(1.0 / h->model.rc_r);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_desc_radial<T><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->d_D);
+        k_pairs<T><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->capLR, h->capLA, h->d_lvR,
+                                      h->d_nlvR, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -639,7 +679,7 @@ int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s)
     const float rcinv = (float)(1.0 / h->model.rc_a);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_desc_angular<T><<<nb, 64, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlA, h->d_nnA, h->d_cA, rcinv, h->d_D, h->d_A);
+        k_desc_angular<T><<<nb, 64, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A);
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -679,42 +719,70 @@ int qnep_launch_fp_combine(qnep_handle* h, bool bec, cudaStream_t s)
     return QNEP_OK;
 }
 
-int qnep_launch_force_angular(qnep_handle* h, bool bec, cudaStream_t s)
+int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 63) / 64);
     const float rcinv = (float)(1.0 / h->model.rc_a);
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Facc, 0, sizeof(float) * (bec ? 9 : 3) * N, s));
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        if (bec)
-            k_force_angular<T, true><<<nb, 64, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlA, h->d_nnA, h->d_cA, rcinv, h->d_Fp,
-                                                       h->d_A, h->d_f12, h->d_Fa, h->d_sums);
-        else
-            k_force_angular<T, false><<<nb, 64, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlA, h->d_nnA, h->d_cA, rcinv, h->d_Fp,
-                                                        h->d_A, h->d_f12, h->d_Fa, h->d_sums);
+#define QNEP_FA(B, V) k_force_angular<T, B, V><<<nb, 64, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->d_nlvA, h->d_cA, rcinv, h->d_Fp, \
+                                                                  h->d_A, h->d_Facc, h->d_sums)
+        if (bec) QNEP_FA(true, false);
+        else if (virial) QNEP_FA(false, true);
+        else QNEP_FA(false, false);
+#undef QNEP_FA
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;
 }
 
-int qnep_launch_force_radial(qnep_handle* h, bool bec, double* out, cudaStream_t s)
+int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
     const float rcinv = (float)(1.0 / h->model.rc_r);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        if (bec)
-            k_force_radial<T, true><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlA, h->d_nnA,
-                                                       h->d_revA, rcinv, h->d_P, h->d_f12, h->d_Fa, h->d_Fs, h->d_q,
-                                                       (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums);
-        else
-            k_force_radial<T, false><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlA, h->d_nnA,
-                                                        h->d_revA, rcinv, h->d_P, h->d_f12, h->d_Fa, h->d_Fs, h->d_q,
-                                                        (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums);
+#define QNEP_FR(B, V) k_force_radial<T, B, V><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_lvR, h->d_nlvR, rcinv, h->d_P, \
+                                                                  h->d_Facc, h->d_Fs, h->d_q, (float)h->model.sqrt_eps_inf,  \
+                                                                  h->d_sidx, out, h->d_sums)
+        if (bec) QNEP_FR(true, false);
+        else if (virial) QNEP_FR(false, true);
+        else QNEP_FR(false, false);
+#undef QNEP_FR
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+// FP32 FMA throughput of this device (TFLOP/s), timed with CUDA events on `s`
+int qnep_launch_fma_peak(double* tflops_host, cudaStream_t s)
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return QNEP_ERR_CUDA;
+    float* d = nullptr;
+    if (cudaMalloc(&d, sizeof(float)) != cudaSuccess) return QNEP_ERR_OOM;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = sms * 8, iters = 4096;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, s);
+        k_fma_peak<<<blocks, 256, 0, s>>>(iters, 1.f + rep, d);
+        cudaEventRecord(e1, s);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return QNEP_ERR_CUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * 16.0 * iters * 256.0 * blocks;
+        if (rep > 0 && ms > 0.f) best = std::max(best, flops / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    *tflops_host = best;
     return QNEP_OK;
 }

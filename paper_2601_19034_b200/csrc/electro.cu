@@ -30,7 +30,7 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
     return r;
 }
 
-// ---- a6: real-space term over the radial neighbour list (mode 1) -----------------------------
+// ---- a6: real-space term over the live radial list of this step (mode 1) ---------------------
 __global__ void __launch_bounds__(128)
 k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
             const int* __restrict__ nn, const float* __restrict__ q, float alpha, float* __restrict__ phir,
@@ -238,7 +238,7 @@ int qnep_launch_realspace(qnep_handle* h, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
-    k_realspace<<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_q, (float)h->alpha, h->d_phir, h->d_Fs,
+    k_realspace<<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_lvR, h->d_nlvR, h->d_q, (float)h->alpha, h->d_phir, h->d_Fs,
                                    h->d_sums);
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());

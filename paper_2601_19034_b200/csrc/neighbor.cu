@@ -1,5 +1,5 @@
 // neighbor.cu -- step a1 of SURVEY.md 8(a): cell list, (type, cell)-sorted atom order and the
-// radial / angular neighbour lists with image codes (PAPER.md :91, Eq. 13), plus the per-step
+// skin neighbour list with image codes (PAPER.md :91, Eq. 13), plus the per-step
 // "prep" pass that turns fp64 positions into cell-relative fp32 coordinates.
 //
 // Layout decisions:
@@ -153,18 +153,19 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
     }
 }
 
-// ---- neighbour lists -------------------------------------------------------------------------
+// ---- skin neighbour list -----------------------------------------------------------------------
+// every (j, image) with r < rc_r + skin; the exact per-step lists are derived from it by k_pairs
 __global__ void __launch_bounds__(128)
 k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ cellc,
-              const int* __restrict__ start, int capR, int capA, int* __restrict__ nlR, int* __restrict__ nnR,
-              int* __restrict__ nlA, int* __restrict__ nnA, int* __restrict__ flags)
+              const int* __restrict__ start, int capR, int* __restrict__ nlR, int* __restrict__ nnR,
+              int* __restrict__ flags)
 {
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
     const float4 xi = xyzt[p];
     const int pc = cellc[p];
     const int c0 = pc & 1023, c1 = (pc >> 10) & 1023, c2 = (pc >> 20) & 1023;
-    int nR = 0, nA = 0;
+    int nR = 0;
     for (int code = 0; code < 27; ++code) {
         const int d0 = code / 9 - 1, d1 = (code / 3) % 3 - 1, d2 = code % 3 - 1;
         int n0 = c0 + d0, n1 = c1 + d1, n2 = c2 + d2;
@@ -180,65 +181,29 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
                 const float4 xj = xyzt[q];
                 const float dx = (xj.x - xi.x) + sx, dy = (xj.y - xi.y) + sy, dz = (xj.z - xi.z) + sz;
                 const float r2 = dx * dx + dy * dy + dz * dz;
-                if (r2 < g.rcs_r2 && r2 > 1e-12f && !(q == p && code == 13)) {
-                    const int entry = q | (code << QNEP_NL_SHIFT);
-                    if (nR < capR) nlR[(int64_t)nR * N + p] = entry;
+                if (r2 < g.rcs_r2 && !(q == p && code == 13)) {
+                    if (nR < capR) nlR[(int64_t)nR * N + p] = q | (code << QNEP_NL_SHIFT);
                     ++nR;
-                    if (r2 < g.rcs_a2) {
-                        if (nA < capA) nlA[(int64_t)nA * N + p] = entry;
-                        ++nA;
-                    }
                 }
             }
         }
     }
     nnR[p] = min(nR, capR);
-    nnA[p] = min(nA, capA);
-    // statistics / overflow detection: warp-aggregated
-    int mR = nR, mA = nA, sR = nR, sA = nA;
+    if (nR > capR) atomicMax(&flags[FLAG_MAX_NR], nR);
+}
+
+// max and sum of a per-atom count array (statistics on request only)
+__global__ void k_count_stats(int64_t N, const int* __restrict__ cnt, int* __restrict__ out_max,
+                              unsigned long long* __restrict__ out_sum)
+{
+    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int v = p < N ? cnt[p] : 0, m = v;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        mR = max(mR, __shfl_xor_sync(0xffffffffu, mR, o));
-        mA = max(mA, __shfl_xor_sync(0xffffffffu, mA, o));
-        sR += __shfl_xor_sync(0xffffffffu, sR, o);
-        sA += __shfl_xor_sync(0xffffffffu, sA, o);
+        v += __shfl_xor_sync(0xffffffffu, v, o);
+        m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
     }
-    if ((threadIdx.x & 31) == 0) {
-        atomicMax(&flags[FLAG_MAX_NR], mR);
-        atomicMax(&flags[FLAG_MAX_NA], mA);
-        atomicAdd((unsigned long long*)&flags[FLAG_SUM_NR], (unsigned long long)sR);
-    }
-    (void)sA;
-}
-
-// separate 64-bit sums need aligned slots: FLAG_SUM_NR uses ints [4..5]; angular sum is taken here
-__global__ void k_sum_counts(int64_t N, const int* __restrict__ nnA, unsigned long long* __restrict__ out)
-{
-    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    int v = p < N ? nnA[p] : 0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if ((threadIdx.x & 31) == 0 && v) atomicAdd(out, (unsigned long long)v);
-}
-
-// reverse slot of every angular entry: the entry (p | 26 - code) in the list of q
-__global__ void k_build_reverse(int64_t N, int capA, const int* __restrict__ nlA, const int* __restrict__ nnA,
-                                int* __restrict__ revA, int* __restrict__ flags)
-{
-    int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (p >= N) return;
-    const int n = nnA[p];
-    for (int s = 0; s < n; ++s) {
-        const int e = nlA[(int64_t)s * N + p];
-        const int q = e & QNEP_NL_MASK, code = (unsigned)e >> QNEP_NL_SHIFT;
-        const int want = (int)p | ((26 - code) << QNEP_NL_SHIFT);
-        const int nq = nnA[q];
-        int found = -1;
-        for (int s2 = 0; s2 < nq; ++s2)
-            if (nlA[(int64_t)s2 * N + q] == want) { found = s2; break; }
-        if (found < 0) { atomicOr(&flags[FLAG_REV_MISS], 1); found = 0; }
-        revA[(int64_t)s * N + p] = found;
-    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(out_sum, (unsigned long long)v); atomicMax(out_max, m); }
 }
 
 }  // namespace
@@ -269,11 +234,30 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
     int rc = qnep_launch_prep(h, pos, true, s);
     if (rc) return rc;
     const int nb2 = (int)((N + 127) / 128);
-    k_build_lists<<<nb2, 128, 0, s>>>(N, h->model.n_types, h->geo, h->d_xyzt, h->d_cellc, h->d_start, h->capR, h->capA,
-                                     h->d_nlR, h->d_nnR, h->d_nlA, h->d_nnA, h->d_flags);
-    k_sum_counts<<<nb, 256, 0, s>>>(N, h->d_nnA, (unsigned long long*)&h->d_flags[FLAG_SUM_NA]);
-    k_build_reverse<<<nb2, 128, 0, s>>>(N, h->capA, h->d_nlA, h->d_nnA, h->d_revA, h->d_flags);
-    h->launches += 3;
+    k_build_lists<<<nb2, 128, 0, s>>>(N, h->model.n_types, h->geo, h->d_xyzt, h->d_cellc, h->d_start, h->capR,
+                                     h->d_nlR, h->d_nnR, h->d_flags);
+    h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+// out[0..5] = max / mean of the skin list, of the live radial list and of the live angular list (last call)
+int qnep_launch_list_stats(qnep_handle* h, double out[6], cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const int nb = (int)((N + 255) / 256);
+    struct Acc { unsigned long long sum[3]; int mx[3]; int pad; };
+    Acc* d = nullptr;
+    QNEP_CUDA_OK(h, cudaMalloc(&d, sizeof(Acc)));
+    QNEP_CUDA_OK(h, cudaMemsetAsync(d, 0, sizeof(Acc), s));
+    const int* arrays[3] = {h->d_nnR, h->d_nlvR, h->d_nlvA};
+    for (int a = 0; a < 3; ++a) k_count_stats<<<nb, 256, 0, s>>>(N, arrays[a], &d->mx[a], &d->sum[a]);
+    h->launches += 3;
+    Acc r;
+    cudaError_t e = cudaMemcpyAsync(&r, d, sizeof(Acc), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d);
+    QNEP_CUDA_OK(h, e);
+    for (int a = 0; a < 3; ++a) { out[2 * a] = r.mx[a]; out[2 * a + 1] = (double)r.sum[a] / (double)N; }
     return QNEP_OK;
 }

@@ -23,8 +23,8 @@ constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (DESIGN.md read
 // device-side double accumulators
 enum { SUM_E_NEP = 0, SUM_Q, SUM_PHI, SUM_U_R, SUM_U_K, SUM_U_S, SUM_W0 /* 9 entries */, SUM_KE = 15, SUM_COUNT = 16 };
 // device-side int flags
-// ints 0..3 are 32-bit flags; ints 4..5 and 6..7 are two 64-bit counters
-enum { FLAG_MAX_NR = 0, FLAG_MAX_NA, FLAG_SKIN, FLAG_REV_MISS, FLAG_SUM_NR = 4, FLAG_SUM_NA = 6, FLAG_COUNT = 8 };
+// overflow flags hold the largest count seen when a list exceeded its capacity (0 otherwise)
+enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_COUNT = 8 };
 
 struct Geometry {            // orthorhombic cell and the cell grid of the neighbour search
     double L[3];
@@ -59,12 +59,13 @@ struct qnep_handle {
     double skin = 0.0;
     int rebuild_every = 0;
     int calls_since_build = -1;      // -1: never built
-    int user_capR = 0, user_capA = 0;
+    int user_capR = 0, user_capLR = 0, user_capA = 0;   // capacity overrides: skin list, live radial, live angular (0: automatic)
     bool force_rebuild = true;
 
     // workspace (sorted atom order p unless noted)
     int64_t N = 0;                   // atoms the workspace is sized for
-    int capR = 0, capA = 0;
+    int capR = 0;                    // skin-list capacity (entries per atom)
+    int capLR = 0, capLA = 0;        // live-list capacities
     Geometry geo;
     double box[9];
     int nkeys = 0;
@@ -79,11 +80,12 @@ struct qnep_handle {
     float4* d_off0 = nullptr;        // [N] the same at build time (skin check)
     float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, -)
     int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each
-    int* d_nlR = nullptr;            // [capR][N]
+    int* d_nlR = nullptr;            // [capR][N]  skin list (r < rc_r + skin at build time)
     int* d_nnR = nullptr;            // [N]
-    int* d_nlA = nullptr;            // [capA][N]
-    int* d_nnA = nullptr;            // [N]
-    int* d_revA = nullptr;           // [capA][N] slot of the reverse entry
+    int* d_lvR = nullptr;            // [capLR][N] live radial list of this step (r < rc_r)
+    int* d_nlvR = nullptr;           // [N]
+    float4* d_lvA = nullptr;         // [capLA][N] live angular pairs of this step: (dx, dy, dz, bits(j | tj << 27))
+    int* d_nlvA = nullptr;           // [N]
     float* d_D = nullptr;            // [25][N]
     float* d_A = nullptr;            // [5*24][N]
     float* d_Ui = nullptr;           // [N]
@@ -97,8 +99,7 @@ struct qnep_handle {
     float* d_phir = nullptr;         // [N]
     float* d_phi = nullptr;          // [N]
     float* d_Fs = nullptr;           // [3][N] static electrostatic force
-    float* d_Fa = nullptr;           // [3][N] own angular partial-force sum (or [9][N] in BEC mode)
-    float4* d_f12 = nullptr;         // [capA][N]
+    float* d_Facc = nullptr;         // [3][N] fp32 force accumulator of the angular pass (atomics); [9][N] in BEC mode
     double* d_sums = nullptr;        // [SUM_COUNT]
     int* d_flags = nullptr;          // [FLAG_COUNT]
     int* h_flags = nullptr;          // pinned
@@ -150,13 +151,15 @@ struct qnep_handle {
 // neighbor.cu
 int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, cudaStream_t s);
 int qnep_launch_prep(qnep_handle* h, const double* pos, bool at_build, cudaStream_t s);
+int qnep_launch_list_stats(qnep_handle* h, double out[6], cudaStream_t s);
 // descriptor.cu
-int qnep_launch_desc_radial(qnep_handle* h, cudaStream_t s);
+int qnep_launch_pairs(qnep_handle* h, cudaStream_t s);
 int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s);
 int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s);
 int qnep_launch_fp_combine(qnep_handle* h, bool bec, cudaStream_t s);
-int qnep_launch_force_angular(qnep_handle* h, bool bec, cudaStream_t s);
-int qnep_launch_force_radial(qnep_handle* h, bool bec, double* out, cudaStream_t s);
+int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_t s);
+int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, cudaStream_t s);
+int qnep_launch_fma_peak(double* tflops_host, cudaStream_t s);
 // electro.cu
 int qnep_launch_realspace(qnep_handle* h, cudaStream_t s);
 int qnep_launch_phi_finalize(qnep_handle* h, cudaStream_t s);
