@@ -341,7 +341,7 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     if (h->es.method != 0 && h->model.mode == 1) { if ((rc = qnep_launch_realspace(h, s))) return rc; }
     QNEP_CUDA_OK(h, cudaEventRecord(ev[6], s));
     if (h->es.method == 1) { if ((rc = qnep_launch_ewald(h, pos, s))) return rc; }
-    else if (h->es.method == 2) { if ((rc = qnep_launch_pppm(h, s))) return rc; }
+    else if (h->es.method == 2) { if ((rc = qnep_launch_pppm(h, (want & QNEP_WANT_VIRIAL) != 0, s))) return rc; }
     else QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
     if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
     const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
@@ -668,7 +668,7 @@ void qnep_destroy(qnep_handle* h)
     if (!h) return;
     free_workspace(h);
     void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_sums, h->d_flags, h->d_kvec,
-                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_cm1, h->d_cm2, h->d_gtab, h->d_twiddle, h->d_hpos,
+                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
                     h->d_htypes, h->d_hout};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (h->h_flags) cudaFreeHost(h->h_flags);

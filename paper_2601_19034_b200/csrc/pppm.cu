@@ -1,25 +1,30 @@
 // pppm.cu -- steps a7P-1..5 of SURVEY.md 8(a): PPPM evaluation of the reciprocal-space part
 // (PAPER.md II.F, Eq. 34-38; readings G2, S10, S11):
 //   1. charge assignment with the order-5 cardinal B-spline (Eq. 35)
-//   2. forward 3-D FFT of the charge mesh (hand-written, shared memory, no cuFFT; :302)
+//   2. forward 3-D FFT of the charge mesh (hand-written, no cuFFT; :302)
 //   3. multiply by the optimised influence function G^opt (Eq. 36), energy (Eq. 34) and virial (Eq. 22)
 //   4. inverse 3-D FFTs.  The four real fields F^-1[S G], F^-1[i k_a S G] (Eq. 37, 38; "3 + 1 backward
 //      FFTs", :302) are packed pairwise into TWO complex transforms: M1 = Phi + i E_x, M2 = E_y + i E_z.
 //   5. back-interpolation of phi^k_i and F^{k,static}_i with the same B-spline.
 //
-// FFT: one block transforms a tile of B = 16 lines held in shared memory as sm[k][b] (b fastest, so
-// every butterfly access is a contiguous 128-byte row segment: conflict-free for any stride).  In-place
-// decimation-in-frequency, radix 4 (+ one radix-2 stage when log2 n is odd); the digit-reversed order
-// is undone for free when the rows are written back.  Strided axes move 128-byte row segments, the
-// contiguous axis moves whole lines, so global traffic is coalesced in all three passes.
+// FFT design: a line of N = R1 R2 points is held in the REGISTERS of N / 16 (or fewer) threads; two
+// small register DFTs (fft_reg.cuh) with one shared-memory exchange in between transform it, so a pass is one
+// coalesced global read and one coalesced global write of the mesh.  16 lines form a tile; strided axes move
+// 128-byte row segments.  The pass along x is FUSED with step 3 and with the first inverse pass: forward x-FFT ->
+// influence multiply (+ energy / virial sums) -> two inverse x-FFTs, all on registers: the spectrum S(k) and the
+// four field spectra never exist in HBM.  The last inverse pass (z) transforms M1 and M2 together and writes the
+// four real fields interleaved as float4 (Phi, E_x, E_y, E_z), which step 5 reads with one 16-byte load per point.
+// Passes per evaluation: z, y, x-fused, y (x2 meshes), z (x2 meshes) = 5 kernels, 7 mesh read+write sweeps
+// instead of 9 transforms x 3 passes.
 #include "qnep_internal.cuh"
 
 #include <cmath>
+#include <type_traits>
+
+#include "fft_reg.cuh"
 
 namespace {
 
-constexpr int FFT_B = 16;          // lines per tile
-constexpr int FFT_BP = FFT_B + 1;  // padded row
 constexpr int FFT_MAXN = 512;
 
 __device__ __forceinline__ void bspline5(float dx, float* __restrict__ w)
@@ -72,168 +77,230 @@ k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
     }
 }
 
-// ---- 2./4. FFT along one axis -----------------------------------------------------------------
-struct FftPlan {
-    int n, log2n;
-    int axis;                 // 0, 1, 2 of an [n0][n1][n2] array (n2 fastest)
-    int n0, n1, n2;
-    int sign;                 // -1 forward, +1 inverse (both unnormalised; reading S11)
+// ---- 2./4. FFT building blocks ------------------------------------------------------------------
+using fftreg::dft;
+
+constexpr int LINES = 16;          // lines per tile
+
+template <int R1, int R2>
+struct Split {
+    static constexpr int N = R1 * R2;
+    static constexpr int TPL = R1 < R2 ? R1 : R2;      // threads per line
+    static constexpr int E = N / TPL;                  // elements per thread
+    static constexpr int D1 = R2 / TPL;                // stage-1 DFTs (length R1) per thread
+    static constexpr int D2 = R1 / TPL;                // stage-2 DFTs (length R2) per thread
+    static constexpr int LP = (R2 * (R1 + 1)) | 1;     // exchange pitch of one line (float2), odd: conflict-free across lines
+    static constexpr int THREADS = TPL * LINES;
 };
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
-template <bool IN_REAL>
-__global__ void __launch_bounds__(256)
-k_fft_axis(FftPlan pl, const float* __restrict__ in_real, const float2* in, float2* out,   // in may alias out (in place)
-           const float2* __restrict__ twiddle /* [n] e^{-2 pi i t / n} */, const int* __restrict__ perm /* pos -> freq */)
+// One line transform on registers.
+//   in : v[d * R1 + m]  = x[(u + TPL d) + R2 m],   d < D1, m < R1     ("stage-1 layout" of <R1, R2>)
+//   out: v[d * R2 + k1] = X[(u + TPL d) + R1 k1],  d < D2, k1 < R2    ("stage-2 layout" of <R1, R2>,
+//                                                                       = the stage-1 layout of <R2, R1>)
+// sm: this line's exchange area (Split::LP float2); tw: omega_N^j = e^{-2 pi i j / N}, j < N (shared memory).
+// All threads of the block must call it (two block barriers).
+template <int R1, int R2, int SIGN>
+__device__ __forceinline__ void line_fft(float2* v, float2* sm, int u, const float2* tw)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* sm = reinterpret_cast<float2*>(smem_raw);                 // [n][FFT_BP]
-    float2* tw = sm + (size_t)pl.n * FFT_BP;                          // [n]
-    int* pm = reinterpret_cast<int*>(tw + pl.n);                      // [n]
-    const int n = pl.n;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    for (int t = tid; t < n; t += nt) {
-        float2 w = twiddle[t];
-        if (pl.sign > 0) w.y = -w.y;
-        tw[t] = w;
-        pm[t] = perm[t];
-    }
-    // tile addressing
-    int64_t base;          // element offset of (k = 0, b = 0)
-    int64_t stride_k;      // between consecutive k of one line
-    const int64_t tile = blockIdx.x;
-    if (pl.axis == 2) { base = tile * FFT_B * (int64_t)n; stride_k = 1; }
-    else if (pl.axis == 1) {
-        const int tiles_per_plane = pl.n2 / FFT_B;
-        base = (tile / tiles_per_plane) * (int64_t)pl.n1 * pl.n2 + (tile % tiles_per_plane) * FFT_B;
-        stride_k = pl.n2;
-    } else { base = tile * FFT_B; stride_k = (int64_t)pl.n1 * pl.n2; }
-    // load
-    if (pl.axis == 2) {
-        for (int e = tid; e < n * FFT_B; e += nt) {
-            const int b = e / n, k = e - b * n;
-            float2 v;
-            if (IN_REAL) v = make_float2(in_real[base + e], 0.f);
-            else v = in[base + e];
-            sm[k * FFT_BP + b] = v;
-        }
-    } else {
-        for (int e = tid; e < n * FFT_B; e += nt) {
-            const int k = e / FFT_B, b = e - k * FFT_B;
-            sm[k * FFT_BP + b] = in[base + k * stride_k + b];
+    using S = Split<R1, R2>;
+#pragma unroll
+    for (int d = 0; d < S::D1; ++d) {
+        dft<R1, SIGN>(v + d * R1);
+        const int t = u + S::TPL * d;
+#pragma unroll
+        for (int k2 = 0; k2 < R1; ++k2) {
+            float2 x = v[d * R1 + k2];
+            if (k2 > 0) {
+                float2 w = tw[t * k2];
+                if (SIGN > 0) w.y = -w.y;
+                x = cmul(x, w);
+            }
+            sm[t * (R1 + 1) + k2] = x;
         }
     }
     __syncthreads();
-    // DIF stages
-    int m = n;                                  // current sub-transform length
-    while (m >= 4) {
-        const int qn = m >> 2;                  // quarter
-        const int tstep = n / m;                // twiddle index step
-        for (int e = tid; e < (n >> 2) * FFT_B; e += nt) {
-            const int b = e % FFT_B;
-            const int bf = e / FFT_B;           // butterfly id 0..n/4-1
-            const int j = bf % qn;
-            const int blk = bf / qn;
-            const int i0 = blk * m + j;
-            float2* p0 = sm + (i0)*FFT_BP + b;
-            float2* p1 = p0 + qn * FFT_BP;
-            float2* p2 = p1 + qn * FFT_BP;
-            float2* p3 = p2 + qn * FFT_BP;
-            const float2 a0 = *p0, a1 = *p1, a2 = *p2, a3 = *p3;
-            const float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), d13 = csub(a1, a3);
-            // omega * d13, omega = -i (forward) or +i (inverse)
-            const float2 t3 = pl.sign < 0 ? make_float2(d13.y, -d13.x) : make_float2(-d13.y, d13.x);
-            const float2 y0 = cadd(t0, t2), y1 = cadd(t1, t3), y2 = csub(t0, t2), y3 = csub(t1, t3);
-            const int ti = j * tstep;
-            *p0 = y0;
-            *p1 = cmul(y1, tw[ti]);
-            *p2 = cmul(y2, tw[2 * ti]);
-            *p3 = cmul(y3, tw[3 * ti]);
-        }
-        __syncthreads();
-        m >>= 2;
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d) {
+        const int k2 = u + S::TPL * d;
+#pragma unroll
+        for (int t = 0; t < R2; ++t) v[d * R2 + t] = sm[t * (R1 + 1) + k2];
+        dft<R2, SIGN>(v + d * R2);
     }
-    if (m == 2) {
-        for (int e = tid; e < (n >> 1) * FFT_B; e += nt) {
-            const int b = e % FFT_B;
-            const int blk = e / FFT_B;
-            float2* p0 = sm + (2 * blk) * FFT_BP + b;
-            float2* p1 = p0 + FFT_BP;
-            const float2 a0 = *p0, a1 = *p1;
-            *p0 = cadd(a0, a1);
-            *p1 = csub(a0, a1);
-        }
-        __syncthreads();
-    }
-    // store: row `pos` holds frequency pm[pos]
-    if (pl.axis == 2) {
-        for (int e = tid; e < n * FFT_B; e += nt) {
-            const int b = e / n, pos = e - b * n;
-            out[base + (int64_t)b * n + pm[pos]] = sm[pos * FFT_BP + b];
-        }
-    } else {
-        for (int e = tid; e < n * FFT_B; e += nt) {
-            const int pos = e / FFT_B, b = e - pos * FFT_B;
-            out[base + pm[pos] * stride_k + b] = sm[pos * FFT_BP + b];
-        }
-    }
+    __syncthreads();
 }
 
-// ---- 3. influence function ----------------------------------------------------------------------
+struct TileAddr { int64_t base, stride; };
+
+// tile -> (base, stride) of a strided-axis tile: 16 consecutive z (b), all points of `axis`
+__device__ __forceinline__ TileAddr strided_tile(int axis, int n0, int n1, int n2, int64_t tile)
+{
+    const int zc = n2 / LINES;
+    TileAddr a;
+    if (axis == 1) { a.base = (tile / zc) * (int64_t)n1 * n2 + (tile % zc) * LINES; a.stride = n2; }
+    else { a.base = (tile / zc) * (int64_t)n2 + (tile % zc) * LINES; a.stride = (int64_t)n1 * n2; }
+    (void)n0;
+    return a;
+}
+
+__device__ __forceinline__ void load_twiddles(float2* tw, const float2* __restrict__ g, int n)
+{
+    for (int i = threadIdx.x; i < n; i += blockDim.x) tw[i] = g[i];
+}
+
+// ---- forward pass along z: real mesh -> complex ---------------------------------------------------
+template <int R1, int R2>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+k_fft_z_fwd(const float* __restrict__ rho, float2* __restrict__ out, const float2* __restrict__ twg)
+{
+    using S = Split<R1, R2>;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * S::LP;
+    load_twiddles(tw, twg, S::N);
+    __syncthreads();
+    const int u = threadIdx.x % S::TPL, b = threadIdx.x / S::TPL;
+    const int64_t base = ((int64_t)blockIdx.x * LINES + b) * S::N;
+    float2 v[S::E];
+#pragma unroll
+    for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+        for (int m = 0; m < R1; ++m) v[d * R1 + m] = make_float2(rho[base + (u + S::TPL * d) + R2 * m], 0.f);
+    line_fft<R1, R2, -1>(v, smem + b * S::LP, u, tw);
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) out[base + (u + S::TPL * d) + R1 * k1] = v[d * R2 + k1];
+}
+
+// ---- in-place pass along a strided axis (y): grid.y selects the mesh --------------------------------
+template <int R1, int R2, int SIGN>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+k_fft_strided(int axis, int n0, int n1, int n2, float2* __restrict__ mesh_a, float2* __restrict__ mesh_b,
+              const float2* __restrict__ twg)
+{
+    using S = Split<R1, R2>;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * S::LP;
+    load_twiddles(tw, twg, S::N);
+    __syncthreads();
+    float2* mesh = blockIdx.y == 0 ? mesh_a : mesh_b;
+    const int b = threadIdx.x % LINES, u = threadIdx.x / LINES;
+    const TileAddr ta = strided_tile(axis, n0, n1, n2, blockIdx.x);
+    float2* p = mesh + ta.base + b;
+    float2 v[S::E];
+#pragma unroll
+    for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+        for (int m = 0; m < R1; ++m) v[d * R1 + m] = p[((u + S::TPL * d) + R2 * m) * ta.stride];
+    line_fft<R1, R2, SIGN>(v, smem + b * S::LP, u, tw);
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) p[((u + S::TPL * d) + R1 * k1) * ta.stride] = v[d * R2 + k1];
+}
+
+// ---- 3. fused pass along x: forward FFT, influence function, two inverse FFTs ------------------------
 // tables per axis a (offset a * FFT_MAXN): A[m] = exp(-k^2/4 alpha^2) sinc^10(pi n/N) / d(z)^2, kk[m] = k (true, for
 // k^2), kd[m] = k with the Nyquist entry zeroed (for the i k multiplier, S11).
-__global__ void __launch_bounds__(256)
-k_influence(Geometry g, const float* __restrict__ tabA, const float* __restrict__ tabK, const float* __restrict__ tabKd,
-            double c0 /* 2 pi / Omega */, double inv4a2, const float2* S, float2* M1,   // S may alias M1
-            float2* __restrict__ M2, double* __restrict__ sums)
+//   M1 = Phi + i (i kx Phi) = (1 - kx) Phi ;  M2 = i ky Phi + i (i kz Phi) = (-kz + i ky) Phi
+template <int R1, int R2, bool VIRIAL>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+k_fft_x_fused(int n0, int n1, int n2, float2* __restrict__ M1 /* in: S after the z and y passes; out: M1 */,
+              float2* __restrict__ M2, const float2* __restrict__ twg, const float* __restrict__ tabA,
+              const float* __restrict__ tabK, const float* __restrict__ tabKd, float c0 /* 2 pi / Omega */, float inv4a2,
+              double* __restrict__ sums)
 {
+    using S = Split<R1, R2>;
+    using SI = Split<R2, R1>;
+    constexpr int LPMAX = S::LP > SI::LP ? S::LP : SI::LP;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * LPMAX;
+    float* tA = reinterpret_cast<float*>(tw + S::N);
+    float* tK = tA + S::N;
+    float* tKd = tK + S::N;
     __shared__ double sh_red[32];
-    const int64_t ng = (int64_t)g.grid[0] * g.grid[1] * g.grid[2];
-    double acc[7] = {0, 0, 0, 0, 0, 0, 0};
-    for (int64_t m = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; m < ng; m += (int64_t)gridDim.x * blockDim.x) {
-        const int m2 = (int)(m % g.grid[2]);
-        const int m1 = (int)((m / g.grid[2]) % g.grid[1]);
-        const int m0 = (int)(m / ((int64_t)g.grid[2] * g.grid[1]));
-        const float kx = tabK[m0], ky = tabK[FFT_MAXN + m1], kz = tabK[2 * FFT_MAXN + m2];
-        const float k2 = kx * kx + ky * ky + kz * kz;
-        float2 phi = make_float2(0.f, 0.f);
-        const float2 s = S[m];
-        if (k2 > 0.f) {
-            const float G = (float)c0 * tabA[m0] * tabA[FFT_MAXN + m1] * tabA[2 * FFT_MAXN + m2] / k2;
-            phi = make_float2(G * s.x, G * s.y);
-            const double e = QNEP_K_COULOMB * (double)G * ((double)s.x * s.x + (double)s.y * s.y);
-            const double bf = 2.0 * inv4a2 + 2.0 / (double)k2;
-            acc[0] += e;
-            acc[1] += e * (1.0 - bf * kx * kx);
-            acc[2] += e * (-bf * kx * ky);
-            acc[3] += e * (-bf * kx * kz);
-            acc[4] += e * (1.0 - bf * ky * ky);
-            acc[5] += e * (-bf * ky * kz);
-            acc[6] += e * (1.0 - bf * kz * kz);
-        }
-        const float kdx = tabKd[m0], kdy = tabKd[FFT_MAXN + m1], kdz = tabKd[2 * FFT_MAXN + m2];
-        // M1 = Phi + i (i kx Phi) = (1 - kx) Phi ;  M2 = i ky Phi + i (i kz Phi) = (-kz + i ky) Phi
-        M1[m] = make_float2((1.f - kdx) * phi.x, (1.f - kdx) * phi.y);
-        M2[m] = make_float2(-kdz * phi.x - kdy * phi.y, -kdz * phi.y + kdy * phi.x);
+    load_twiddles(tw, twg, S::N);
+    for (int i = threadIdx.x; i < S::N; i += blockDim.x) { tA[i] = tabA[i]; tK[i] = tabK[i]; tKd[i] = tabKd[i]; }
+    __syncthreads();
+    const int b = threadIdx.x % LINES, u = threadIdx.x / LINES;
+    const TileAddr ta = strided_tile(0, n0, n1, n2, blockIdx.x);
+    const int zc = n2 / LINES;
+    const int iy = (int)(blockIdx.x / zc), iz = (int)(blockIdx.x % zc) * LINES + b;
+    float2 v[S::E], w[S::E];
+    {
+        const float2* p = M1 + ta.base + b;
+#pragma unroll
+        for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+            for (int m = 0; m < R1; ++m) v[d * R1 + m] = p[((u + S::TPL * d) + R2 * m) * ta.stride];
     }
+    line_fft<R1, R2, -1>(v, smem + b * S::LP, u, tw);
+    // v[d * R2 + k1] = S(kx = (u + TPL d) + R1 k1, ky, kz)
+    const float ky = tabK[FFT_MAXN + iy], kz = tabK[2 * FFT_MAXN + iz];
+    const float kdy = tabKd[FFT_MAXN + iy], kdz = tabKd[2 * FFT_MAXN + iz];
+    const float Ayz = c0 * tabA[FFT_MAXN + iy] * tabA[2 * FFT_MAXN + iz];
+    const float kyz2 = ky * ky + kz * kz;
+    float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) {
+            const int ix = (u + S::TPL * d) + R1 * k1;
+            const float kx = tK[ix], kdx = tKd[ix];
+            const float k2 = kx * kx + kyz2;
+            const float2 s = v[d * R2 + k1];
+            float G = 0.f;
+            if (k2 > 0.f) G = __fdividef(Ayz * tA[ix], k2);
+            const float2 phi = make_float2(G * s.x, G * s.y);
+            const float e = G * (s.x * s.x + s.y * s.y);
+            acc[0] += e;
+            if (VIRIAL && k2 > 0.f) {
+                const float bf = 2.f * inv4a2 + __fdividef(2.f, k2);
+                acc[1] += e * (1.f - bf * kx * kx);
+                acc[2] += e * (-bf * kx * ky);
+                acc[3] += e * (-bf * kx * kz);
+                acc[4] += e * (1.f - bf * ky * ky);
+                acc[5] += e * (-bf * ky * kz);
+                acc[6] += e * (1.f - bf * kz * kz);
+            }
+            v[d * R2 + k1] = make_float2((1.f - kdx) * phi.x, (1.f - kdx) * phi.y);
+            w[d * R2 + k1] = make_float2(-kdz * phi.x - kdy * phi.y, -kdz * phi.y + kdy * phi.x);
+        }
+    // inverse along x with the swapped split <R2, R1>: its stage-1 layout is the layout we hold
+    line_fft<R2, R1, +1>(v, smem + b * SI::LP, u, tw);
+    {
+        float2* p = M1 + ta.base + b;
+#pragma unroll
+        for (int d = 0; d < SI::D2; ++d)
+#pragma unroll
+            for (int k1 = 0; k1 < R1; ++k1) p[((u + SI::TPL * d) + R2 * k1) * ta.stride] = v[d * R1 + k1];
+    }
+    line_fft<R2, R1, +1>(w, smem + b * SI::LP, u, tw);
+    {
+        float2* p = M2 + ta.base + b;
+#pragma unroll
+        for (int d = 0; d < SI::D2; ++d)
+#pragma unroll
+            for (int k1 = 0; k1 < R1; ++k1) p[((u + SI::TPL * d) + R2 * k1) * ta.stride] = w[d * R1 + k1];
+    }
+    // U^k = K sum G |S|^2 (Eq. 34), W^k = K sum G |S|^2 B (Eq. 22): fp32 per thread, fp64 across threads
     const int slot[7] = {SUM_U_K, SUM_W0 + 0, SUM_W0 + 1, SUM_W0 + 2, SUM_W0 + 4, SUM_W0 + 5, SUM_W0 + 8};
     const int mirror[7] = {-1, -1, SUM_W0 + 3, SUM_W0 + 6, -1, SUM_W0 + 7, -1};
 #pragma unroll
-    for (int a = 0; a < 7; ++a) {
-        double v = acc[a];
+    for (int a = 0; a < (VIRIAL ? 7 : 1); ++a) {
+        double x = (double)acc[a];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
         __syncthreads();
-        if ((threadIdx.x & 31) == 0) sh_red[threadIdx.x >> 5] = v;
+        if ((threadIdx.x & 31) == 0) sh_red[threadIdx.x >> 5] = x;
         __syncthreads();
         if (threadIdx.x < 32) {
             double r = threadIdx.x < (blockDim.x >> 5) ? sh_red[threadIdx.x] : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
             if (threadIdx.x == 0) {
+                r *= QNEP_K_COULOMB;
                 atomicAdd(&sums[slot[a]], r);
                 if (mirror[a] >= 0) atomicAdd(&sums[mirror[a]], r);
             }
@@ -241,10 +308,42 @@ k_influence(Geometry g, const float* __restrict__ tabA, const float* __restrict_
     }
 }
 
+// ---- last inverse pass along z: M1, M2 -> interleaved real fields (Phi, E_x, E_y, E_z) -------------------
+template <int R1, int R2>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+k_fft_z_fields(const float2* __restrict__ M1, const float2* __restrict__ M2, float4* __restrict__ field,
+               const float2* __restrict__ twg)
+{
+    using S = Split<R1, R2>;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * S::LP;
+    load_twiddles(tw, twg, S::N);
+    __syncthreads();
+    const int u = threadIdx.x % S::TPL, b = threadIdx.x / S::TPL;
+    const int64_t base = ((int64_t)blockIdx.x * LINES + b) * S::N;
+    float2 v[S::E], w[S::E];
+#pragma unroll
+    for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+        for (int m = 0; m < R1; ++m) {
+            v[d * R1 + m] = M1[base + (u + S::TPL * d) + R2 * m];
+            w[d * R1 + m] = M2[base + (u + S::TPL * d) + R2 * m];
+        }
+    line_fft<R1, R2, +1>(v, smem + b * S::LP, u, tw);
+    line_fft<R1, R2, +1>(w, smem + b * S::LP, u, tw);
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) {
+            const float2 a = v[d * R2 + k1], c = w[d * R2 + k1];
+            field[base + (u + S::TPL * d) + R1 * k1] = make_float4(a.x, a.y, c.x, c.y);
+        }
+}
+
 // ---- 5. back-interpolation ------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0,
-         const float* __restrict__ q, const float2* __restrict__ M1, const float2* __restrict__ M2, int add_to_Fs,
+         const float* __restrict__ q, const float4* __restrict__ field, int add_to_Fs,
          float* __restrict__ phik, float* __restrict__ Fs)
 {
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -264,10 +363,9 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
 #pragma unroll
             for (int c = 0; c < 5; ++c) {
                 const float w = wab * wz[c];
-                const float2 u = M1[row + idx[2][c]];
-                const float2 v = M2[row + idx[2][c]];
-                ph = fmaf(w, u.x, ph); ex = fmaf(w, u.y, ex);
-                ey = fmaf(w, v.x, ey); ez = fmaf(w, v.y, ez);
+                const float4 f = field[row + idx[2][c]];
+                ph = fmaf(w, f.x, ph); ex = fmaf(w, f.y, ex);
+                ey = fmaf(w, f.z, ey); ez = fmaf(w, f.w, ez);
             }
         }
     }
@@ -278,31 +376,25 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
     else { Fs[p] = cq * ex; Fs[N + p] = cq * ey; Fs[2 * N + p] = cq * ez; }
 }
 
-int launch_fft3d(qnep_handle* h, const float* in_real, float2* data, int sign, cudaStream_t s)
+// ---- dispatch on the axis length ---------------------------------------------------------------------
+template <typename F>
+bool with_split(int n, F&& f)
 {
-    const int n0 = h->geo.grid[0], n1 = h->geo.grid[1], n2 = h->geo.grid[2];
-    const int order_fwd[3] = {2, 1, 0}, order_inv[3] = {0, 1, 2};
-    for (int step = 0; step < 3; ++step) {
-        const int axis = sign < 0 ? order_fwd[step] : order_inv[step];
-        const int n = axis == 0 ? n0 : (axis == 1 ? n1 : n2);
-        FftPlan pl;
-        pl.n = n; pl.log2n = 0; while ((1 << pl.log2n) < n) ++pl.log2n;
-        pl.axis = axis; pl.n0 = n0; pl.n1 = n1; pl.n2 = n2; pl.sign = sign;
-        const int64_t lines = (int64_t)n0 * n1 * n2 / n;
-        const int tiles = (int)(lines / FFT_B);
-        const size_t smem = sizeof(float2) * ((size_t)n * FFT_BP + n) + sizeof(int) * n;
-        const int threads = std::min(256, std::max(32, n * FFT_B / 4));
-        const bool real_in = (in_real != nullptr) && step == 0 && sign < 0;
-        if (real_in)
-            k_fft_axis<true><<<tiles, threads, smem, s>>>(pl, in_real, nullptr, data, h->d_twiddle + axis * FFT_MAXN,
-                                                          reinterpret_cast<const int*>(h->d_twiddle + 3 * FFT_MAXN) + axis * FFT_MAXN);
-        else
-            k_fft_axis<false><<<tiles, threads, smem, s>>>(pl, nullptr, data, data, h->d_twiddle + axis * FFT_MAXN,
-                                                           reinterpret_cast<const int*>(h->d_twiddle + 3 * FFT_MAXN) + axis * FFT_MAXN);
-        h->launches += 1;
+    switch (n) {
+        case 16: f(std::integral_constant<int, 4>(), std::integral_constant<int, 4>()); return true;
+        case 32: f(std::integral_constant<int, 8>(), std::integral_constant<int, 4>()); return true;
+        case 64: f(std::integral_constant<int, 8>(), std::integral_constant<int, 8>()); return true;
+        case 128: f(std::integral_constant<int, 16>(), std::integral_constant<int, 8>()); return true;
+        case 256: f(std::integral_constant<int, 16>(), std::integral_constant<int, 16>()); return true;
+        case 512: f(std::integral_constant<int, 32>(), std::integral_constant<int, 16>()); return true;
     }
-    QNEP_CUDA_OK(h, cudaGetLastError());
-    return QNEP_OK;
+    return false;
+}
+
+template <typename K>
+cudaError_t allow_smem(K kernel, size_t bytes)
+{
+    return bytes > 48 * 1024 ? cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) : cudaSuccess;
 }
 
 double alias_den(double z)
@@ -313,28 +405,28 @@ double alias_den(double z)
 
 }  // namespace
 
-// tables: twiddles, digit-reversal permutations and the separable factors of G^opt (Eq. 36)
+// tables: twiddles and the separable factors of G^opt (Eq. 36)
 int qnep_setup_pppm(qnep_handle* h)
 {
     const int* grid = h->es.grid;
     for (int a = 0; a < 3; ++a) {
         const int n = grid[a];
-        if (n < FFT_B || n > FFT_MAXN || (n & (n - 1))) { h->err = "PPPM grid must be a power of two in 16..512"; return QNEP_ERR_UNSUPPORTED; }
+        if (n < LINES || n > FFT_MAXN || (n & (n - 1))) { h->err = "PPPM grid must be a power of two in 16..512"; return QNEP_ERR_UNSUPPORTED; }
     }
     if (h->es.order != 5) { h->err = "PPPM order must be 5"; return QNEP_ERR_UNSUPPORTED; }
     const int64_t ng = (int64_t)grid[0] * grid[1] * grid[2];
     if (ng != h->ngrid) {
-        cudaFree(h->d_mesh); cudaFree(h->d_cm1); cudaFree(h->d_cm2);
-        h->d_mesh = nullptr; h->d_cm1 = nullptr; h->d_cm2 = nullptr;
+        cudaFree(h->d_mesh); cudaFree(h->d_cm1); cudaFree(h->d_cm2); cudaFree(h->d_field);
+        h->d_mesh = nullptr; h->d_cm1 = nullptr; h->d_cm2 = nullptr; h->d_field = nullptr;
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_mesh, sizeof(float) * ng));
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm1, sizeof(float2) * ng));
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm2, sizeof(float2) * ng));
+        QNEP_CUDA_OK(h, cudaMalloc(&h->d_field, sizeof(float4) * ng));
         h->ngrid = ng;
     }
-    if (!h->d_twiddle) QNEP_CUDA_OK(h, cudaMalloc(&h->d_twiddle, sizeof(float2) * 3 * FFT_MAXN + sizeof(int) * 3 * FFT_MAXN));
+    if (!h->d_twiddle) QNEP_CUDA_OK(h, cudaMalloc(&h->d_twiddle, sizeof(float2) * 3 * FFT_MAXN));
     if (!h->d_gtab) QNEP_CUDA_OK(h, cudaMalloc(&h->d_gtab, sizeof(float) * 9 * FFT_MAXN));
     std::vector<float2> tw(3 * FFT_MAXN, make_float2(0.f, 0.f));
-    std::vector<int> pm(3 * FFT_MAXN, 0);
     std::vector<float> tab(9 * FFT_MAXN, 0.f);
     const double L[3] = {h->box[0], h->box[4], h->box[8]};
     for (int a = 0; a < 3; ++a) {
@@ -342,13 +434,6 @@ int qnep_setup_pppm(qnep_handle* h)
         for (int t = 0; t < n; ++t) {
             const double ang = -2.0 * M_PI * t / n;
             tw[a * FFT_MAXN + t] = make_float2((float)cos(ang), (float)sin(ang));
-        }
-        // position -> frequency after the DIF stages: pos = sum_i c_i q_i, freq = c_1 + r_1 (c_2 + r_2 (...))
-        for (int pos = 0; pos < n; ++pos) {
-            int rem = pos, m = n, freq = 0, weight = 1;
-            while (m >= 4) { const int q = m / 4; const int c = rem / q; rem -= c * q; freq += c * weight; weight *= 4; m = q; }
-            if (m == 2) { const int c = rem; freq += c * weight; }
-            pm[a * FFT_MAXN + pos] = freq;
         }
         for (int m = 0; m < n; ++m) {
             const int nn = m < n / 2 ? m : m - n;                 // -N/2 <= n < N/2 (:285)
@@ -362,39 +447,77 @@ int qnep_setup_pppm(qnep_handle* h)
         }
     }
     QNEP_CUDA_OK(h, cudaMemcpy(h->d_twiddle, tw.data(), sizeof(float2) * 3 * FFT_MAXN, cudaMemcpyHostToDevice));
-    QNEP_CUDA_OK(h, cudaMemcpy(h->d_twiddle + 3 * FFT_MAXN, pm.data(), sizeof(int) * 3 * FFT_MAXN, cudaMemcpyHostToDevice));
     QNEP_CUDA_OK(h, cudaMemcpy(h->d_gtab, tab.data(), sizeof(float) * 9 * FFT_MAXN, cudaMemcpyHostToDevice));
-    static bool attr = false;
-    if (!attr) {
-        QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_fft_axis<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-        QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_fft_axis<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-        attr = true;
-    }
     return QNEP_OK;
 }
 
-int qnep_launch_pppm(qnep_handle* h, cudaStream_t s)
+int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
     const double L[3] = {h->box[0], h->box[4], h->box[8]};
+    const int n0 = h->geo.grid[0], n1 = h->geo.grid[1], n2 = h->geo.grid[2];
+    const float2* tw0 = h->d_twiddle;
+    const float2* tw1 = h->d_twiddle + FFT_MAXN;
+    const float2* tw2 = h->d_twiddle + 2 * FFT_MAXN;
+    cudaError_t ce = cudaSuccess;
+    auto note = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
+
+    // 1. spread
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mesh, 0, sizeof(float) * h->ngrid, s));
     k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_q, h->d_mesh);
-    h->launches += 1;
-    int rc = launch_fft3d(h, h->d_mesh, h->d_cm1, -1, s);
-    if (rc) return rc;
-    const int nblk = (int)std::min<int64_t>((h->ngrid + 255) / 256, 148 * 8);
-    k_influence<<<nblk, 256, 0, s>>>(h->geo, h->d_gtab, h->d_gtab + 3 * FFT_MAXN, h->d_gtab + 6 * FFT_MAXN,
-                                     2.0 * M_PI / (L[0] * L[1] * L[2]), 1.0 / (4.0 * h->alpha * h->alpha), h->d_cm1,
-                                     h->d_cm1, h->d_cm2, h->d_sums);
-    h->launches += 1;
-    rc = launch_fft3d(h, nullptr, h->d_cm1, +1, s);
-    if (rc) return rc;
-    rc = launch_fft3d(h, nullptr, h->d_cm2, +1, s);
-    if (rc) return rc;
-    k_gather<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_q, h->d_cm1, h->d_cm2, h->model.mode == 1 ? 1 : 0,
-                                h->d_phik, h->d_Fs);
-    h->launches += 1;
+    // 2. forward z (real -> complex), forward y
+    with_split(n2, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_z_fwd<R1, R2>, smem));
+        k_fft_z_fwd<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_mesh, h->d_cm1, tw2);
+    });
+    with_split(n1, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_strided<R1, R2, -1>, smem));
+        k_fft_strided<R1, R2, -1><<<dim3((unsigned)((int64_t)n0 * n2 / LINES), 1), S::THREADS, smem, s>>>(1, n0, n1, n2, h->d_cm1, h->d_cm1, tw1);
+    });
+    // 3. + first inverse pass: x
+    with_split(n0, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        using SI = Split<R2, R1>;
+        const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 3 * S::N;
+        const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+        const unsigned nt = (unsigned)((int64_t)n1 * n2 / LINES);
+        if (virial) {
+            note(allow_smem(k_fft_x_fused<R1, R2, true>, smem));
+            k_fft_x_fused<R1, R2, true><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, tw0, h->d_gtab, h->d_gtab + 3 * FFT_MAXN,
+                                                                    h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
+        } else {
+            note(allow_smem(k_fft_x_fused<R1, R2, false>, smem));
+            k_fft_x_fused<R1, R2, false><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, tw0, h->d_gtab, h->d_gtab + 3 * FFT_MAXN,
+                                                                     h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
+        }
+    });
+    // 4. inverse y on both meshes, inverse z -> interleaved real fields
+    with_split(n1, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_strided<R1, R2, +1>, smem));
+        k_fft_strided<R1, R2, +1><<<dim3((unsigned)((int64_t)n0 * n2 / LINES), 2), S::THREADS, smem, s>>>(1, n0, n1, n2, h->d_cm1, h->d_cm2, tw1);
+    });
+    with_split(n2, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_z_fields<R1, R2>, smem));
+        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm1, h->d_cm2, h->d_field, tw2);
+    });
+    // 5. gather
+    k_gather<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_q, h->d_field, h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs);
+    h->launches += 7;
+    QNEP_CUDA_OK(h, ce);
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;
 }

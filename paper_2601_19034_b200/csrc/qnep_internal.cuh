@@ -120,6 +120,7 @@ struct qnep_handle {
     float* d_mesh = nullptr;         // [Nx][Ny][Nz] real charge mesh
     float2* d_cm1 = nullptr;         // complex meshes
     float2* d_cm2 = nullptr;
+    float4* d_field = nullptr;       // [Nx][Ny][Nz] (Phi, E_x, E_y, E_z)
     float* d_gtab = nullptr;         // 1-D influence tables: per axis N entries of (A_alpha) then k_alpha
     float2* d_twiddle = nullptr;     // per axis twiddles
     int tw_n = 0;
@@ -167,4 +168,4 @@ int qnep_setup_ewald(qnep_handle* h);
 int qnep_launch_ewald(qnep_handle* h, const double* pos, cudaStream_t s);
 // pppm.cu
 int qnep_setup_pppm(qnep_handle* h);
-int qnep_launch_pppm(qnep_handle* h, cudaStream_t s);
+int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s);
