@@ -39,6 +39,8 @@ FLOPS_ANG_BWD_PER_NEIGHBOUR = 1500.0   # angular backward, per angular neighbour
 FLOPS_ANG_FWD_PER_NEIGHBOUR = 450.0
 FLOPS_RAD_FWD_PER_NEIGHBOUR = 150.0
 FLOPS_RAD_BWD_PER_NEIGHBOUR = 250.0
+FLOPS_NN_FWD_H80 = 5100.0               # per atom, H = 80 (scaled linearly with H)
+FLOPS_NN_BWD_H80 = 4400.0
 FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.4: 148 SMs x 128 lanes x 2 x 1.965 GHz
 
 
@@ -195,9 +197,10 @@ def main():
     # warm-up (also grows neighbour capacity / shrinks dt if the random-init model is too violent)
     dt_fs = args.dt_fs
     pos, vel = pos0.clone(), vel0.clone()
+    e_start = None
     for attempt in range(8):
         try:
-            md(pos, vel, Wm, dt_fs)
+            e_start = md(pos, vel, Wm, dt_fs).cpu().numpy()
             break
         except Q.QnepError as err:
             if err.code == Q.QNEP_ERR_SKIN_VIOLATED:
@@ -220,7 +223,7 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     tw0 = time.time()
     e0.record()
-    md(pos, vel, K, dt_fs)                       # synchronises at the end (device-side error check)
+    e_end = md(pos, vel, K, dt_fs)               # synchronises at the end (device-side error check: skin, capacity)
     e1.record()
     torch.cuda.synchronize()
     tw1 = time.time()
@@ -235,6 +238,13 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
     ms_per_step = ms_total / K
+    # the MD must have stayed an MD: (E_pot + E_kin) conserved between the end of the warm-up and the end of the
+    # timed run, no skin violation (md_run raises), kinetic temperature reported
+    e_end = e_end.cpu().numpy()
+    kB = 8.617333262e-5
+    md_sanity = {"etot_start_eV": float(e_start[0] + e_start[1]), "etot_end_eV": float(e_end[0] + e_end[1]),
+                 "drift_eV_per_atom": float((e_end[0] + e_end[1] - e_start[0] - e_start[1]) / n),
+                 "T_start_K": float(e_start[1] / (1.5 * n * kB)), "T_end_K": float(e_end[1] / (1.5 * n * kB))}
     value = world * n * K / (ms_total * 1e-3)
     stats = h.neighbor_stats()
 
@@ -243,18 +253,30 @@ def main():
     # neighbours inside the cutoffs at the last step (the exact per-step lists)
     live_a, live_r = stats["mean_angular"], stats["mean_radial"]
     fma_measured = Q.fma_peak()
-    kernels = {
-        "k_force_angular": (per_eval["force_angular"], FLOPS_ANG_BWD_PER_NEIGHBOUR * live_a * n),
+    H = w.model.n_neurons
+    kernels = {   # stage time (the kernel is bracketed alone, or with O(N) helpers), algorithmic flops per launch
+        "k_pairs": (per_eval["desc_radial"], FLOPS_RAD_FWD_PER_NEIGHBOUR * live_r * n),
         "k_desc_angular": (per_eval["desc_angular"], FLOPS_ANG_FWD_PER_NEIGHBOUR * live_a * n),
+        "k_nn": (per_eval["nn"], (FLOPS_NN_FWD_H80 + FLOPS_NN_BWD_H80) * (H / 80.0) * n),
+        "k_force_angular": (per_eval["force_angular"], FLOPS_ANG_BWD_PER_NEIGHBOUR * live_a * n),
+        "k_force_radial": (per_eval["force_radial"], FLOPS_RAD_BWD_PER_NEIGHBOUR * live_r * n),
     }
     dom = max(kernels, key=lambda k: kernels[k][0])
     dom_ms, dom_flops = kernels[dom]
+    fp32_ms = sum(v[0] for v in kernels.values())
+    fp32_flops = sum(v[1] for v in kernels.values())
     achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS, "traffic": None,
                 "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "fma_loop_measured_tflops": fma_measured, "frac_of_measured_fma_loop": achieved / fma_measured if fma_measured else None,
-                "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops}
+                "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops,
+                "per_kernel": {k: {"ms": v[0], "tflops": v[1] / (v[0] * 1e-3) / 1e12 if v[0] > 0 else 0.0,
+                                   "frac": v[1] / (v[0] * 1e-3) / 1e12 / FP32_PEAK_NOMINAL_TFLOPS if v[0] > 0 else 0.0}
+                               for k, v in kernels.items()},
+                "all_fp32_stages": {"ms": fp32_ms, "algorithmic_flops": fp32_flops,
+                                    "tflops": fp32_flops / (fp32_ms * 1e-3) / 1e12,
+                                    "frac": fp32_flops / (fp32_ms * 1e-3) / 1e12 / FP32_PEAK_NOMINAL_TFLOPS}}
     peaks = load_peaks()
     mesh_bytes = float(np.prod(w.es.grid)) * 8.0
     fft_bytes = 3 * 3 * 2 * mesh_bytes - float(np.prod(w.es.grid)) * 4.0   # 3 transforms x 3 passes x (read + write)
@@ -321,6 +343,7 @@ def main():
                        "mean_neighbours_angular": stats["mean_angular"]},
             "roofline": roofline, "roofline_pppm": pppm,
             "stage_ms_per_eval": per_eval, "evals_profiled": n_evals,
+            "md_sanity": md_sanity,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line))

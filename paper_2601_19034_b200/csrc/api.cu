@@ -153,6 +153,12 @@ int consume_flags(qnep_handle* h)
 {
     h->flags_pending = false;
     const int* f = h->h_flags;
+    // the device flags are sticky (a rebuild inside qnep_md_run must not erase a violation seen earlier in the
+    // run): they are cleared here, on the error path only, once the host has read them
+    if (f[FLAG_MAX_NR] || f[FLAG_MAX_LR] || f[FLAG_MAX_LA] || f[FLAG_SKIN]) {
+        cudaMemsetAsync(h->d_flags, 0, sizeof(int) * FLAG_COUNT, h->last_stream);
+        cudaStreamSynchronize(h->last_stream);
+    }
     if (f[FLAG_MAX_NR] > h->capR || f[FLAG_MAX_LR] > h->capLR || f[FLAG_MAX_LA] > h->capLA) {
         h->err = "neighbour list capacity exceeded (skin list " + std::to_string(f[FLAG_MAX_NR]) + "/" + std::to_string(h->capR) +
                  ", live radial " + std::to_string(f[FLAG_MAX_LR]) + "/" + std::to_string(h->capLR) + ", live angular " +

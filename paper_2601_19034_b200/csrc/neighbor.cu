@@ -225,7 +225,6 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
     const int nb = (int)((N + 255) / 256);
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_cnt, 0, sizeof(int) * (h->nkeys + 1), s));
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_fill, 0, sizeof(int) * h->nkeys, s));
-    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_flags, 0, sizeof(int) * FLAG_COUNT, s));
     k_bin_count<<<nb, 256, 0, s>>>(N, pos, types, h->geo, h->d_key, h->d_cnt);
     k_exclusive_scan<<<1, 1024, 0, s>>>(h->nkeys, h->d_cnt, h->d_start);
     k_scatter<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_fill, h->d_tmpidx);

@@ -256,3 +256,50 @@ def test_md_run_conserves_energy(torch):
     tot0, tot1 = e0[0] + ke0, e1[0] + e1[1]
     assert abs(tot1 - tot0) / w.n_atoms < 2e-4, (tot0, tot1)
     assert abs(e1[0] - e0[0]) > 1e-6            # the atoms did move
+
+
+# ---------------------------------------------------------------- full BASELINE sizes (configs 3 and 4)
+def test_config3_full_size(torch, oracle):
+    """BASELINE configs[3] at its full size: 320 000 atoms, 3 species, PPPM 128^3."""
+    w = I.config3()
+    ref = oracle.compute_workload(w)
+    h, res = gpu_eval(torch, w)
+    assert_parity(w, res, ref, "config3 full (320k atoms, 128^3)")
+    assert np.abs(res["forces"].sum(axis=1)).max() < 0.3        # sum F = 0 to fp32 atomics / PPPM accuracy over 320k atoms
+    assert abs(res["charges"].sum()) < 1e-3
+
+
+def test_config4_full_size_in_the_bench_configuration(torch, oracle):
+    """BASELINE configs[4] (1 029 000 atoms, PPPM 256^3) in the launch configuration bench.py times: skin 1 A, rebuild
+    every 10 calls, lists REUSED after the velocity-Verlet driver has moved the atoms.  Parity is checked at fixed
+    positions (SURVEY 8(c) protocol): step 0, and the driver's own positions after 15 steps fed back to the oracle."""
+    w = I.config4()
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(1.0, 10)
+    ref = oracle.compute_workload(w)
+    _, res = gpu_eval(torch, w, handle=h)
+    assert_parity(w, res, ref, "config4 full, step 0")
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    vel = torch.tensor(I.maxwell_boltzmann(w), dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    dt = 0.1 / 10.180505
+    h.md_run(pos, vel, types, w.box, w.masses, dt, 15)          # ends 5 steps after a rebuild
+    moved = replace(w, pos=pos.cpu().numpy())
+    assert np.abs(moved.pos - w.pos).max() > 1e-3                # the atoms did move
+    out = h.compute(pos, types, w.box, want=Q.WANT_ALL)          # 6th call since the rebuild: lists reused
+    assert h.get_timings()["neighbor"] < 0.05
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    assert_parity(moved, res, oracle.compute_workload(moved), "config4 full, after 15 MD steps, lists reused")
+
+
+def test_md_skin_violation_survives_a_rebuild(torch):
+    """A violation in an early block of steps must still be reported after later rebuilds (the flags are sticky)."""
+    w = I.config1()
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(0.05, 10)                              # a skin the thermal motion exceeds within 10 steps
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    vel = torch.tensor(I.maxwell_boltzmann(w), dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    with pytest.raises(Q.QnepError) as ei:
+        h.md_run(pos, vel, types, w.box, w.masses, 0.5 / 10.180505, 31)   # ends right after a rebuild
+    assert ei.value.code == Q.QNEP_ERR_SKIN_VIOLATED
