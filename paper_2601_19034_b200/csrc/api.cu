@@ -26,7 +26,7 @@ void free_workspace(qnep_handle* h)
                      (void**)&h->d_sidx, (void**)&h->d_cellc, (void**)&h->d_xyzt, (void**)&h->d_off0, (void**)&h->d_mfrac,
                      (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_lvR, (void**)&h->d_nlvR,
                      (void**)&h->d_lvA, (void**)&h->d_nlvA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
-                     (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_P,
+                     (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_recA, (void**)&h->d_recB, (void**)&h->d_lvRend,
                      (void**)&h->d_phik, (void**)&h->d_phir, (void**)&h->d_phi, (void**)&h->d_Fs, (void**)&h->d_Facc,
                      (void**)&h->d_Fmd};
     for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
@@ -83,7 +83,7 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
     const double vol = g.L[0] * g.L[1] * g.L[2];
     const double rho = (double)N / vol;
     auto cap_for = [&](double rc_, int user) {
-        if (user > 0) return user;
+        if (user > 0) return (user + 3) / 4 * 4;          // packed-word lists hold four slots per int4
         const double expect = 4.0 / 3.0 * M_PI * rc_ * rc_ * rc_ * rho;
         return ((int)(expect * 1.5) + 24 + 3) / 4 * 4;
     };
@@ -104,11 +104,12 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_off0, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_mfrac, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_mi0, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_nlR, n * capR))) return rc;
+        const size_t npad = (n + QNEP_TILE - 1) / QNEP_TILE * QNEP_TILE;
+        if ((rc = dev_alloc(h, &h->d_nlR, npad * (capR / 4)))) return rc;
         if ((rc = dev_alloc(h, &h->d_nnR, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_lvR, n * capLR))) return rc;
+        if ((rc = dev_alloc(h, &h->d_lvR, npad * (capLR / 4)))) return rc;
         if ((rc = dev_alloc(h, &h->d_nlvR, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_lvA, n * capLA))) return rc;
+        if ((rc = dev_alloc(h, &h->d_lvA, npad * capLA))) return rc;
         if ((rc = dev_alloc(h, &h->d_nlvA, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_D, n * QNEP_NDESC))) return rc;
         if ((rc = dev_alloc(h, &h->d_A, n * QNEP_NRAD * QNEP_NLM))) return rc;
@@ -118,7 +119,9 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_FpU, n * QNEP_NDESC))) return rc;
         if ((rc = dev_alloc(h, &h->d_FpQ, n * QNEP_NDESC))) return rc;
         if ((rc = dev_alloc(h, &h->d_Fp, n * QNEP_NDESC))) return rc;
-        if ((rc = dev_alloc(h, &h->d_P, n * T * QNEP_KPAD))) return rc;
+        if ((rc = dev_alloc(h, &h->d_recA, n * T * 8))) return rc;
+        if ((rc = dev_alloc(h, &h->d_recB, n * T))) return rc;
+        if ((rc = dev_alloc(h, &h->d_lvRend, n * T))) return rc;
         if ((rc = dev_alloc(h, &h->d_phik, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_phir, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_phi, n))) return rc;
@@ -352,7 +355,6 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
     const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
     const bool need_virial = (want & QNEP_WANT_VIRIAL) != 0;
-    if (need_forces) { if ((rc = qnep_launch_fp_combine(h, false, s))) return rc; }
     QNEP_CUDA_OK(h, cudaEventRecord(ev[7], s));
     if (need_forces) {
         if ((rc = qnep_launch_force_angular(h, false, need_virial, s))) return rc;     // bracketed alone by ev[7], ev[8]
@@ -367,7 +369,6 @@ int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* ty
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaEventRecord(ev[9], s));
     if ((want & QNEP_WANT_BEC) && bec) {
-        if ((rc = qnep_launch_fp_combine(h, true, s))) return rc;
         if ((rc = qnep_launch_force_angular(h, true, false, s))) return rc;
         if ((rc = qnep_launch_force_radial(h, true, false, bec, s))) return rc;
     }

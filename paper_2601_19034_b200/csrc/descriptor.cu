@@ -78,6 +78,14 @@ __device__ __forceinline__ void cheb_basis(float r, float rcinv, float* __restri
     }
 }
 
+// MUFU.RSQ without the denormal range fix-up of rsqrtf (arguments here are squared distances >= 1e-12)
+__device__ __forceinline__ float fast_rsqrt(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ void load_shift_table(float4* sh, const Geometry& g)
 {
     if (threadIdx.x < 27) {
@@ -105,62 +113,185 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: one walk over the skin list: radial descriptors + the exact lists of this step
-//   live radial entry : the skin-list word (sorted index | image code << 27)
-//   live angular pair : (dx, dy, dz, bits(sorted index | type << 27))
+// asynchronous global -> shared copies (LDGSTS): a thread streams its own list rows through a small ring in
+// shared memory, so many loads are in flight per thread at no register cost.  A thread only ever reads what it
+// copied itself, so cp.async.wait_group is the only synchronisation needed.
 // ------------------------------------------------------------------------------------------
-template <int T>
-__global__ void __launch_bounds__(128)
-k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
-        const int* __restrict__ nn, const float* __restrict__ cR, float rcinv, int capLR, int capLA,
-        int* __restrict__ lvR, int* __restrict__ nlvR, float4* __restrict__ lvA, int* __restrict__ nlvA,
-        float* __restrict__ D, int* __restrict__ flags)
+__device__ __forceinline__ void cp_async4(void* sm, const void* g)
 {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async16_ca(void* sm, const void* g)      // gathers: keep the line in L1
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async16_cg(void* sm, const void* g)      // streams: bypass L1
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
+
+// ------------------------------------------------------------------------------------------
+// a2: one walk over the skin list: the exact lists of this step and the radial descriptors
+//   live radial entry : the skin-list word (sorted index | image code << 27), type-major like the skin list
+//                       (warp-tiled int4 layout); lvRend[t][p] = end of the species-t segment
+//   live angular pair : (dx, dy, dz, bits(sorted index | type << 27))
+// The skin list is processed in chunks of PAIRS_CH slots, each in two phases:
+//   phase 1, per SKIN entry (all lanes busy): list word -> position gather -> distance test; accepted entries are
+//     pushed to a per-thread queue in shared memory (word, r^2) and, inside the angular cutoff, appended to the
+//     angular pair list.  List vectors arrive through a double-buffered cp.async stage (one chunk ahead), gathered
+//     positions through a register ring PAIRS_DX entries ahead (plain loads, so that they hit L1).
+//   phase 2, per ACCEPTED entry: basis functions f_k(r) and S^t_k += f_k for t = t_j, append to the live radial
+//     list.  The expensive part runs for accepted entries only, with no skin-shell divergence.
+// ------------------------------------------------------------------------------------------
+constexpr int PAIRS_BLOCK = 128, PAIRS_CH = 32, PAIRS_DX = 8;
+
+template <int T>
+__global__ void __launch_bounds__(PAIRS_BLOCK)
+k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __restrict__ nl,
+        const int* __restrict__ nn, const float* __restrict__ cR, float rcinv, int capR, int capLR, int capLA,
+        int4* __restrict__ lvR, int* __restrict__ nlvR, int* __restrict__ lvRend,
+        float4* __restrict__ lvA, int* __restrict__ nlvA, float* __restrict__ D, int* __restrict__ flags)
+{
+    constexpr int NV = PAIRS_CH / 4;                         // int4 vectors per chunk
     __shared__ float4 sh_shift[27];
     __shared__ float sh_c[T * T * NR * KP];
+    extern __shared__ __align__(16) unsigned char pairs_smem[];
+    int4 (*sh_l)[NV][PAIRS_BLOCK] = reinterpret_cast<int4 (*)[NV][PAIRS_BLOCK]>(pairs_smem);              // list stage x 2
+    int (*sh_qe)[PAIRS_BLOCK] = reinterpret_cast<int (*)[PAIRS_BLOCK]>(pairs_smem + sizeof(int4) * 2 * NV * PAIRS_BLOCK);   // queue: words
+    float (*sh_qr)[PAIRS_BLOCK] = reinterpret_cast<float (*)[PAIRS_BLOCK]>(sh_qe + PAIRS_CH);              // queue: r^2
     load_shift_table(sh_shift, g);
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
     __syncthreads();
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int tid = threadIdx.x;
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
     if (p >= N) return;
     const float4 xi = xyzt[p];
     const int ti = __float_as_int(xi.w);
-    float S[T][NB];
+    const int n = nn[p];
+    const int n4 = (n + 3) >> 2;
+    const int4* lbase = nl + qnep_tiled_base(p, capR / 4);
+    auto issue_stage = [&](int c) {
 #pragma unroll
-    for (int t = 0; t < T; ++t)
+        for (int v = 0; v < NV; ++v) {
+            const int gv = c * NV + v;
+            if (gv < n4) cp_async16_cg(&sh_l[c & 1][v][tid], lbase + (int64_t)gv * QNEP_TILE);
+        }
+        cp_async_commit();
+    };
+    issue_stage(0);
+    issue_stage(1);
+    cp_async_wait<1>();
+    float4 ring[PAIRS_DX];
+#pragma unroll
+    for (int k = 0; k < PAIRS_DX; ++k) {
+        const int w = reinterpret_cast<const int*>(&sh_l[0][k >> 2][tid])[k & 3];
+        ring[k] = k < n ? xyzt[w & QNEP_NL_MASK] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    float S[T][NB];
+    int cnt[T];
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        cnt[t] = 0;
 #pragma unroll
         for (int k = 0; k < NB; ++k) S[t][k] = 0.f;
-    const int n = nn[p];
-    int cR_ = 0, cA_ = 0;
-    int e_next = n > 0 ? nl[p] : 0;
-    for (int s = 0; s < n; ++s) {
-        const int e = e_next;
-        if (s + 1 < n) e_next = nl[(int64_t)(s + 1) * N + p];
-        const int j = e & QNEP_NL_MASK;
-        const float4 xj = xyzt[j];
-        const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-        const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 >= g.rc_r2 || r2 < 1e-12f) continue;
-        const int tj = __float_as_int(xj.w);
-        if (cR_ < capLR) lvR[(int64_t)cR_ * N + p] = e;
-        ++cR_;
-        if (r2 < g.rc_a2) {
-            if (cA_ < capLA) lvA[(int64_t)cA_ * N + p] = make_float4(dx, dy, dz, __int_as_float(j | (tj << QNEP_NL_SHIFT)));
-            ++cA_;
-        }
-        float f[NB];
-        cheb_basis<true, false>(r2 * rsqrtf(r2), rcinv, f, nullptr);
-#pragma unroll
-        for (int t = 0; t < T; ++t) {
-            const float w = (tj == t) ? 1.f : 0.f;
-#pragma unroll
-            for (int k = 0; k < NB; ++k) S[t][k] = fmaf(w, f[k], S[t][k]);
-        }
     }
-    nlvR[p] = min(cR_, capLR);
+    int cA_ = 0, cRtot = 0;
+    int4* outR = lvR + qnep_tiled_base(p, capLR / 4);
+    float4* outA = lvA + qnep_tiled_base(p, capLA);
+    int4 rbuf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
+    const int nchunk = (n + PAIRS_CH - 1) / PAIRS_CH;
+    for (int c = 0; c < nchunk; ++c) {
+        const int sbase = c * PAIRS_CH;
+        int qn = 0;
+        int cc[T];
+#pragma unroll
+        for (int t = 0; t < T; ++t) cc[t] = 0;
+        // ---- phase 1 ----
+        int4 wv = make_int4(0, 0, 0, 0);
+#pragma unroll
+        for (int i = 0; i < PAIRS_CH; ++i) {
+            if ((i & 3) == 0) wv = sh_l[c & 1][i >> 2][tid];
+            const int e = (i & 3) == 0 ? wv.x : ((i & 3) == 1 ? wv.y : ((i & 3) == 2 ? wv.z : wv.w));
+            const float4 xj = ring[i % PAIRS_DX];
+            // prefetch the position of entry i + DX (same chunk, or the head of the next one)
+            {
+                const int i2 = i + PAIRS_DX;
+                if (i2 == PAIRS_CH) cp_async_wait<0>();            // the next stage has landed (issued a chunk ago)
+                const int buf2 = i2 < PAIRS_CH ? (c & 1) : ((c + 1) & 1);
+                const int k2 = i2 < PAIRS_CH ? i2 : i2 - PAIRS_CH;
+                if (sbase + i2 < n) {
+                    const int w2 = reinterpret_cast<const int*>(&sh_l[buf2][k2 >> 2][tid])[k2 & 3];
+                    ring[i % PAIRS_DX] = xyzt[w2 & QNEP_NL_MASK];
+                }
+            }
+            if (sbase + i < n) {
+                const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+                const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 < g.rc_r2 && r2 >= 1e-12f) {
+                    const int tj = __float_as_int(xj.w);
+                    sh_qe[qn][tid] = e;
+                    sh_qr[qn][tid] = r2;
+                    ++qn;
+#pragma unroll
+                    for (int t = 0; t < T; ++t) cc[t] += (tj == t) ? 1 : 0;
+                    if (r2 < g.rc_a2) {
+                        if (cA_ < capLA) {
+                            *outA = make_float4(dx, dy, dz, __int_as_float((e & QNEP_NL_MASK) | (tj << QNEP_NL_SHIFT)));
+                            outA += QNEP_TILE;
+                        }
+                        ++cA_;
+                    }
+                }
+            }
+        }
+        // stage c has been consumed: refill its buffer with chunk c + 2
+        issue_stage(c + 2);
+        // ---- phase 2 ----
+        int bnd[T];                                          // the queue is type-major: species t ends at bnd[t]
+        {
+            int e_ = 0;
+#pragma unroll
+            for (int t = 0; t < T; ++t) { e_ += cc[t]; bnd[t] = e_; }
+        }
+        for (int k = 0; k < qn; ++k) {
+            const int e = sh_qe[k][tid];
+            const float r2 = sh_qr[k][tid];
+            float f[NB];
+            cheb_basis<true, false>(r2 * fast_rsqrt(r2), rcinv, f, nullptr);
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+                const float w = (T == 1 || ((t == 0 || k >= bnd[t - 1]) && k < bnd[t])) ? 1.f : 0.f;
+#pragma unroll
+                for (int kk = 0; kk < NB; ++kk) S[t][kk] = fmaf(w, f[kk], S[t][kk]);
+            }
+            if (cRtot < capLR) {
+                const int pos = cRtot & 3;
+                if (pos == 0) rbuf.x = e; else if (pos == 1) rbuf.y = e; else if (pos == 2) rbuf.z = e; else rbuf.w = e;
+                if (pos == 3) {
+                    outR[(int64_t)(cRtot >> 2) * QNEP_TILE] = rbuf;
+                    rbuf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
+                }
+            }
+            ++cRtot;
+        }
+#pragma unroll
+        for (int t = 0; t < T; ++t) cnt[t] += cc[t];
+    }
+    cp_async_wait<0>();
+    const int nlive = min(cRtot, capLR);
+    if (nlive & 3) outR[(int64_t)(nlive >> 2) * QNEP_TILE] = rbuf;
+    nlvR[p] = nlive;
     nlvA[p] = min(cA_, capLA);
-    if (cR_ > capLR) atomicMax(&flags[FLAG_MAX_LR], cR_);
+    {
+        int end = 0;
+#pragma unroll
+        for (int t = 0; t < T; ++t) { end += cnt[t]; lvRend[(int64_t)t * N + p] = min(end, capLR); }
+    }
+    if (cRtot > capLR) atomicMax(&flags[FLAG_MAX_LR], cRtot);
     if (cA_ > capLA) atomicMax(&flags[FLAG_MAX_LA], cA_);
 #pragma unroll
     for (int nidx = 0; nidx < NR; ++nidx) {
@@ -196,12 +327,17 @@ __device__ __forceinline__ void harmonics(float x, float y, float z, float* __re
 // ------------------------------------------------------------------------------------------
 // a3: angular descriptors; A_nlm kept for the backward pass
 // ------------------------------------------------------------------------------------------
+// The live angular pairs are streamed through a cp.async ring ANG_DEPTH rows deep (the kernels hold 120+ accumulators
+// in registers, so occupancy is low and the loads must be issued far ahead).
+constexpr int ANG_BLOCK = 64, ANG_DEPTH = 8;
+
 template <int T>
-__global__ void __launch_bounds__(64)
-k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, const int* __restrict__ nlvA,
+__global__ void __launch_bounds__(ANG_BLOCK)
+k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
                const float* __restrict__ cA, float rcinv, float* __restrict__ D, float* __restrict__ Aout)
 {
     __shared__ __align__(16) float sh_c[T * T * NR * KP];
+    __shared__ float4 sh_ring[ANG_DEPTH][ANG_BLOCK];
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
     __syncthreads();
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -213,12 +349,20 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
 #pragma unroll
         for (int lm = 0; lm < NLM; ++lm) A[a][lm] = 0.f;
     const int n = nlvA[p];
-    float4 pr_next = n > 0 ? lvA[p] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4* rows = lvA + qnep_tiled_base(p, capLA);
+    const int tid = threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < ANG_DEPTH; ++k) {
+        if (k < n) cp_async16_cg(&sh_ring[k][tid], rows + (int64_t)k * QNEP_TILE);
+        cp_async_commit();
+    }
     for (int s = 0; s < n; ++s) {
-        const float4 pr = pr_next;
-        if (s + 1 < n) pr_next = lvA[(int64_t)(s + 1) * N + p];
+        cp_async_wait<ANG_DEPTH - 1>();
+        const float4 pr = sh_ring[s & (ANG_DEPTH - 1)][tid];
+        if (s + ANG_DEPTH < n) cp_async16_cg(&sh_ring[s & (ANG_DEPTH - 1)][tid], rows + (int64_t)(s + ANG_DEPTH) * QNEP_TILE);
+        cp_async_commit();
         const float r2 = pr.x * pr.x + pr.y * pr.y + pr.z * pr.z;
-        const float rinv = rsqrtf(r2), r = r2 * rinv;
+        const float rinv = fast_rsqrt(r2), r = r2 * rinv;
         float f[NB];
         cheb_basis<true, false>(r, rcinv, f, nullptr);
         const int tj = (unsigned)__float_as_int(pr.w) >> QNEP_NL_SHIFT;
@@ -328,49 +472,6 @@ __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const do
     if (charges_out) charges_out[sidx[p]] = v;
 }
 
-// a10: Fp = dU/dD + phi_eff dq/dD (S6: phi_eff = phi - mean phi), and the radial vectors
-//      P^t_k = sum_n Fp_n c^{ti t}_{nk}.  BEC mode: Fp = sqrt(eps_inf) dq/dD (Eq. 24, 28; S12).
-template <int T>
-__global__ void __launch_bounds__(128)
-k_fp_combine(int64_t N, const float4* __restrict__ xyzt, const float* __restrict__ FpU, const float* __restrict__ FpQ,
-             const float* __restrict__ phi, const double* __restrict__ sums, int bec, float sqrt_eps,
-             const float* __restrict__ cR, float* __restrict__ Fp, float* __restrict__ P)
-{
-    __shared__ float sh_c[T * T * NR * KP];
-    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
-    __syncthreads();
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (p >= N) return;
-    const int ti = __float_as_int(xyzt[p].w);
-    float cu, cq;
-    if (bec) { cu = 0.f; cq = sqrt_eps; }
-    else { cu = 1.f; cq = phi[p] - (float)(sums[SUM_PHI] / (double)N); }
-    float fr[NR];
-#pragma unroll
-    for (int v = 0; v < ND; ++v) {
-        const float val = cu * FpU[(int64_t)v * N + p] + cq * FpQ[(int64_t)v * N + p];
-        Fp[(int64_t)v * N + p] = val;
-        if (v < NR) fr[v] = val;
-    }
-#pragma unroll
-    for (int t = 0; t < T; ++t) {
-        float4* out = reinterpret_cast<float4*>(P + ((int64_t)p * T + t) * KP);
-        float pk[KP];
-#pragma unroll
-        for (int k = 0; k < KP; ++k) {
-            float v = 0.f;
-            if (k < NB) {
-#pragma unroll
-                for (int a = 0; a < NR; ++a) v = fmaf(fr[a], sh_c[((ti * T + t) * NR + a) * KP + k], v);
-            }
-            pk[k] = v;
-        }
-        out[0] = make_float4(pk[0], pk[1], pk[2], pk[3]);
-        out[1] = make_float4(pk[4], pk[5], pk[6], pk[7]);
-        out[2] = make_float4(pk[8], pk[9], pk[10], pk[11]);
-    }
-}
-
 // ------------------------------------------------------------------------------------------
 // a11 (angular part): F_ij = sum_{n,lm} Q_nlm d/dr_ij [ g_n(r_ij) b_lm(rhat_ij) ],
 //   Q_nlm = dE/dA_nlm = 2 C_lm Fp_{nl} A_nlm.  With G_lm = sum_n Q_nlm g_n, G'_lm = sum_n Q_nlm g_n':
@@ -391,40 +492,87 @@ k_fp_combine(int64_t N, const float4* __restrict__ xyzt, const float* __restrict
     }
 
 template <int T, bool BEC, bool VIRIAL>
-__global__ void __launch_bounds__(64)
-k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, const int* __restrict__ nlvA,
-                const float* __restrict__ cA, float rcinv, const float* __restrict__ Fp, const float* __restrict__ Ain,
-                float* __restrict__ Facc, double* __restrict__ sums)
+__global__ void __launch_bounds__(ANG_BLOCK)
+k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
+                const float* __restrict__ cA, const float* __restrict__ cR, float rcinv, const float* __restrict__ FpU,
+                const float* __restrict__ FpQ, const float* __restrict__ phi, float sqrt_eps, const float* __restrict__ Ain,
+                float* __restrict__ Fp, float* __restrict__ recA, float4* __restrict__ recB, float* __restrict__ Facc,
+                double* __restrict__ sums)
 {
     __shared__ __align__(16) float sh_c[T * T * NR * KP];
+    __shared__ __align__(16) float sh_cR[T * T * NR * KP];
+    __shared__ float4 sh_ring[ANG_DEPTH][ANG_BLOCK];
     __shared__ double sh_red[32];
-    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
+    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) { sh_c[i] = cA[i]; sh_cR[i] = cR[i]; }
     __syncthreads();
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int tid = threadIdx.x;
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
     float W[9];
 #pragma unroll
     for (int a = 0; a < 9; ++a) W[a] = 0.f;
     if (p < N) {
-        const int ti = __float_as_int(xyzt[p].w);
+        const int n = nlvA[p];
+        const float4* rows = lvA + qnep_tiled_base(p, capLA);
+#pragma unroll
+        for (int k = 0; k < ANG_DEPTH; ++k) {
+            if (k < n) cp_async16_cg(&sh_ring[k][tid], rows + (int64_t)k * QNEP_TILE);
+            cp_async_commit();
+        }
+        const float4 xi = xyzt[p];
+        const int ti = __float_as_int(xi.w);
+        // a10: Fp = dU/dD + phi_eff dq/dD (S6: phi_eff = phi - mean phi); BEC mode: Fp = sqrt(eps_inf) dq/dD (Eq. 24, 28; S12).
+        // The radial part goes into the gather records of the radial force kernel, one per species t of the atom
+        // that will read it: recA[t][p] = (x, y, z, P^t_0..P^t_4), recB[t][p] = (P^t_5..P^t_8), P^t_k = sum_n Fp_n c^{ti t}_{nk}.
+        float cu, cq;
+        if (BEC) { cu = 0.f; cq = sqrt_eps; }
+        else { cu = 1.f; cq = phi[p] - (float)(sums[SUM_PHI] / (double)N); }
+        {
+            float fr[NR];
+#pragma unroll
+            for (int v = 0; v < NR; ++v) {
+                fr[v] = cu * FpU[(int64_t)v * N + p] + cq * FpQ[(int64_t)v * N + p];
+                Fp[(int64_t)v * N + p] = fr[v];
+            }
+#pragma unroll
+            for (int t = 0; t < T; ++t) {
+                float pk[NB];
+#pragma unroll
+                for (int k = 0; k < NB; ++k) {
+                    float v = 0.f;
+#pragma unroll
+                    for (int a = 0; a < NR; ++a) v = fmaf(fr[a], sh_cR[((ti * T + t) * NR + a) * KP + k], v);
+                    pk[k] = v;
+                }
+                float4* r4 = reinterpret_cast<float4*>(recA + 8 * ((int64_t)t * N + p));
+                r4[0] = make_float4(xi.x, xi.y, xi.z, pk[0]);
+                r4[1] = make_float4(pk[1], pk[2], pk[3], pk[4]);
+                recB[(int64_t)t * N + p] = make_float4(pk[5], pk[6], pk[7], pk[8]);
+            }
+        }
         float Q[NR][NLM];
 #pragma unroll
         for (int a = 0; a < NR; ++a) {
             float fpl[4];
 #pragma unroll
-            for (int l = 0; l < 4; ++l) fpl[l] = 2.f * Fp[(int64_t)(NR + a * 4 + l) * N + p];
+            for (int l = 0; l < 4; ++l) {
+                const int64_t v = NR + a * 4 + l;
+                const float val = cu * FpU[v * N + p] + cq * FpQ[v * N + p];
+                Fp[v * N + p] = val;
+                fpl[l] = 2.f * val;
+            }
 #pragma unroll
             for (int lm = 0; lm < NLM; ++lm)
                 Q[a][lm] = c_Clm[lm] * fpl[l_of_lm(lm)] * Ain[(int64_t)(a * NLM + lm) * N + p];
         }
         float Fx = 0.f, Fy = 0.f, Fz = 0.f;
-        const int n = nlvA[p];
-        float4 pr_next = n > 0 ? lvA[p] : make_float4(0.f, 0.f, 0.f, 0.f);
         for (int s = 0; s < n; ++s) {
-            const float4 pr = pr_next;
-            if (s + 1 < n) pr_next = lvA[(int64_t)(s + 1) * N + p];
+            cp_async_wait<ANG_DEPTH - 1>();
+            const float4 pr = sh_ring[s & (ANG_DEPTH - 1)][tid];
+            if (s + ANG_DEPTH < n) cp_async16_cg(&sh_ring[s & (ANG_DEPTH - 1)][tid], rows + (int64_t)(s + ANG_DEPTH) * QNEP_TILE);
+            cp_async_commit();
             const float dx = pr.x, dy = pr.y, dz = pr.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
-            const float rinv = rsqrtf(r2), r = r2 * rinv;
+            const float rinv = fast_rsqrt(r2), r = r2 * rinv;
             float f[NB], df[NB];
             cheb_basis<true, true>(r, rcinv, f, df);
             const int jw = __float_as_int(pr.w);
@@ -512,93 +660,141 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
 }
 
 // ------------------------------------------------------------------------------------------
-// a11 (radial part + assembly): F_i = sum_j (s_ij + s_ji) rhat_ij  +  angular accumulator
-//   +  static electrostatic force;  s_ij = sum_k P^{i,tj}_k f_k'(r_ij).
+// a11 (radial part + assembly): F_i = sum_j (s_ij + s_ji) rhat_ij  +  angular accumulator  +  static electrostatic
+//   force;  s_ij = sum_k P^{i,tj}_k f_k'(r_ij),  s_ji = sum_k P^{j,ti}_k f_k'(r_ij),  P^{i,t}_k = sum_n Fp^i_n c^{ti t}_{nk}.
 // BEC mode (a12): Z_i = qt_i I + 1/2 sum_j r_ij (x) (c_ij + c_ji).
+// Per neighbour two gathers from the records the angular kernel wrote for readers of species ti: recA[ti][j] =
+// (x, y, z, P_0..P_4) (one 32-byte sector, LDG.256) and recB[ti][j] = (P_5..P_8).  The list is type-major, so the
+// thread's own vector P^{i,tj} changes T - 1 times along the list (it is the thread's own record for species tj).
+// List words run through a cp.async ring RAD_DW rows ahead, records through a register ring RAD_DX deep.
 // Output in ORIGINAL atom order, float64.
 // ------------------------------------------------------------------------------------------
+constexpr int RAD_BLOCK = 128, RAD_LV = 4;      // list vectors (4 slots each) in flight; records are requested 4 slots ahead
+
+__device__ __forceinline__ void ldg256(const float* p, float (&v)[8])
+{
+    asm volatile("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                 : "l"(p));
+}
+
 template <int T, bool BEC, bool VIRIAL>
-__global__ void __launch_bounds__(128)
-k_force_radial(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ lvR,
-               const int* __restrict__ nlvR, float rcinv, const float* __restrict__ P, const float* __restrict__ Facc,
-               const float* __restrict__ Fs, const float* __restrict__ q, float sqrt_eps,
-               const int* __restrict__ sidx, double* __restrict__ out, double* __restrict__ sums)
+__global__ void __launch_bounds__(RAD_BLOCK)
+k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const float4* __restrict__ recB,
+               const float4* __restrict__ xyzt, const int4* __restrict__ lvR, int capLR, const int* __restrict__ nlvR,
+               const int* __restrict__ lvRend, float rcinv, const float* __restrict__ Facc, const float* __restrict__ Fs,
+               const float* __restrict__ q, float sqrt_eps, const int* __restrict__ sidx, double* __restrict__ out,
+               double* __restrict__ sums)
 {
     __shared__ float4 sh_shift[27];
+    __shared__ int4 sh_w[RAD_LV][RAD_BLOCK];
     __shared__ double sh_red[32];
     load_shift_table(sh_shift, g);
     __syncthreads();
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int tid = threadIdx.x;
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
     float W[9];
 #pragma unroll
     for (int a = 0; a < 9; ++a) W[a] = 0.f;
     if (p < N) {
+        const int n = nlvR[p];
+        const int n4 = (n + 3) >> 2;
+        const int4* vbase = lvR + qnep_tiled_base(p, capLR / 4);
         const float4 xi = xyzt[p];
         const int ti = __float_as_int(xi.w);
-        float Pi[T][NB];
+        const float* gA = recA + 8 * (int64_t)ti * N;       // records for readers of my species
+        const float4* gB = recB + (int64_t)ti * N;
+        // prologue: vector 0 by a plain load (its records are requested at once), vectors 1..LV through the ring.
+        // cp.async groups: LV in the prologue, one per iteration; at the top of iteration v the group of vector v + 1
+        // is number v + 1 of LV + v, so LV - 1 may stay pending.
+        int4 cur = n > 0 ? vbase[0] : make_int4((int)p, (int)p, (int)p, (int)p);
 #pragma unroll
-        for (int t = 0; t < T; ++t) {
-            const float4* src = reinterpret_cast<const float4*>(P + ((int64_t)p * T + t) * KP);
-            const float4 a = src[0], b = src[1], c = src[2];
-            Pi[t][0] = a.x; Pi[t][1] = a.y; Pi[t][2] = a.z; Pi[t][3] = a.w;
-            Pi[t][4] = b.x; Pi[t][5] = b.y; Pi[t][6] = b.z; Pi[t][7] = b.w; Pi[t][8] = c.x;
+        for (int k = 1; k <= RAD_LV; ++k) {
+            if (k < n4) cp_async16_cg(&sh_w[k & (RAD_LV - 1)][tid], vbase + (int64_t)k * QNEP_TILE);
+            cp_async_commit();
         }
+        float ra[4][8];
+        float4 rb[4];
+        {
+            const int e0[4] = {cur.x, cur.y, cur.z, cur.w};
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int j = u < n ? (e0[u] & QNEP_NL_MASK) : (int)p;
+                ldg256(gA + 8 * (int64_t)j, ra[u]);
+                rb[u] = __ldg(gB + j);
+            }
+        }
+        int tj = -1, seg_end = 0;
+        float Pi[NB];
+#pragma unroll
+        for (int k = 0; k < NB; ++k) Pi[k] = 0.f;
         float Fx = 0.f, Fy = 0.f, Fz = 0.f;
-        const int n = nlvR[p];
-        // software pipeline: list word two ahead, gathered records one ahead
-        int e_nn = n > 1 ? lvR[N + p] : 0;
-        int e_n = n > 0 ? lvR[p] : 0;
-        float4 xj_n = xyzt[e_n & QNEP_NL_MASK];
-        const float4* pj_n = reinterpret_cast<const float4*>(P + ((int64_t)(e_n & QNEP_NL_MASK) * T + ti) * KP);
-        float4 pa_n = pj_n[0], pb_n = pj_n[1], pc_n = pj_n[2];
-        for (int s = 0; s < n; ++s) {
-            const int e = e_n;
-            const float4 xj = xj_n, a = pa_n, b = pb_n, c = pc_n;
-            e_n = e_nn;
-            if (s + 2 < n) e_nn = lvR[(int64_t)(s + 2) * N + p];
-            if (s + 1 < n) {
-                const int jn = e_n & QNEP_NL_MASK;
-                xj_n = xyzt[jn];
-                pj_n = reinterpret_cast<const float4*>(P + ((int64_t)jn * T + ti) * KP);
-                pa_n = pj_n[0]; pb_n = pj_n[1]; pc_n = pj_n[2];
-            }
-            const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-            const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
-            const float r2 = dx * dx + dy * dy + dz * dz;
-            const float rinv = rsqrtf(r2), r = r2 * rinv;
-            float df[NB];
-            cheb_basis<false, true>(r, rcinv, nullptr, df);
-            const int tj = __float_as_int(xj.w);
-            float sji = a.x * df[0];
-            sji = fmaf(a.y, df[1], sji); sji = fmaf(a.z, df[2], sji); sji = fmaf(a.w, df[3], sji);
-            sji = fmaf(b.x, df[4], sji); sji = fmaf(b.y, df[5], sji); sji = fmaf(b.z, df[6], sji);
-            sji = fmaf(b.w, df[7], sji); sji = fmaf(c.x, df[8], sji);
-            float sij = 0.f;
+        for (int v = 0; v < n4; ++v) {
+            cp_async_wait<RAD_LV - 1>();
+            int4 nxt = cur;
+            if (v + 1 < n4) nxt = sh_w[(v + 1) & (RAD_LV - 1)][tid];
+            if (v + 1 + RAD_LV < n4) cp_async16_cg(&sh_w[(v + 1) & (RAD_LV - 1)][tid], vbase + (int64_t)(v + 1 + RAD_LV) * QNEP_TILE);
+            cp_async_commit();
+            const int ec[4] = {cur.x, cur.y, cur.z, cur.w};
+            const int en[4] = {nxt.x, nxt.y, nxt.z, nxt.w};
 #pragma unroll
-            for (int t = 0; t < T; ++t) {
-                float v = 0.f;
+            for (int u = 0; u < 4; ++u) {
+                const int s = 4 * v + u;
+                if (s < n) {
+                    const int e = ec[u];
+                    float a8[8];
 #pragma unroll
-                for (int k = 0; k < NB; ++k) v = fmaf(Pi[t][k], df[k], v);
-                sij = (tj == t) ? v : sij;
-            }
-            const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
-            if (BEC) {
-                // 1/2 r_ij (x) (c_ij + c_ji), c_ij = s_ij rhat, c_ji = s_ji rhat_ji = -s_ji rhat
-                const float w = 0.5f * (sij - sji);
-                W[0] = fmaf(dx, w * ux, W[0]); W[1] = fmaf(dx, w * uy, W[1]); W[2] = fmaf(dx, w * uz, W[2]);
-                W[3] = fmaf(dy, w * ux, W[3]); W[4] = fmaf(dy, w * uy, W[4]); W[5] = fmaf(dy, w * uz, W[5]);
-                W[6] = fmaf(dz, w * ux, W[6]); W[7] = fmaf(dz, w * uy, W[7]); W[8] = fmaf(dz, w * uz, W[8]);
-            } else {
-                const float w = sij + sji;
-                Fx = fmaf(w, ux, Fx); Fy = fmaf(w, uy, Fy); Fz = fmaf(w, uz, Fz);
-                if (VIRIAL) {
-                    const float wx = sij * ux, wy = sij * uy, wz = sij * uz;     // F_ij
-                    W[0] = fmaf(dx, wx, W[0]); W[1] = fmaf(dx, wy, W[1]); W[2] = fmaf(dx, wz, W[2]);
-                    W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
-                    W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
+                    for (int a = 0; a < 8; ++a) a8[a] = ra[u][a];
+                    const float4 b4 = rb[u];
+                    if (s + 4 < n) {
+                        const int j2 = en[u] & QNEP_NL_MASK;
+                        ldg256(gA + 8 * (int64_t)j2, ra[u]);
+                        rb[u] = __ldg(gB + j2);
+                    }
+                    if (s >= seg_end) {
+                        // next non-empty species segment: my own vector for neighbours of species tj is my record for tj
+                        do { ++tj; seg_end = lvRend[(int64_t)tj * N + p]; } while (s >= seg_end && tj < T - 1);
+                        float o8[8];
+                        ldg256(recA + 8 * ((int64_t)tj * N + p), o8);
+                        const float4 o4 = __ldg(recB + (int64_t)tj * N + p);
+                        Pi[0] = o8[3]; Pi[1] = o8[4]; Pi[2] = o8[5]; Pi[3] = o8[6]; Pi[4] = o8[7];
+                        Pi[5] = o4.x; Pi[6] = o4.y; Pi[7] = o4.z; Pi[8] = o4.w;
+                    }
+                    const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+                    const float dx = (a8[0] - xi.x) + sh.x, dy = (a8[1] - xi.y) + sh.y, dz = (a8[2] - xi.z) + sh.z;
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    const float rinv = fast_rsqrt(r2), r = r2 * rinv;
+                    float df[NB];
+                    cheb_basis<false, true>(r, rcinv, nullptr, df);
+                    float sij = Pi[0] * df[0], sji = a8[3] * df[0];
+#pragma unroll
+                    for (int k = 1; k < 5; ++k) { sij = fmaf(Pi[k], df[k], sij); sji = fmaf(a8[3 + k], df[k], sji); }
+                    sij = fmaf(Pi[5], df[5], sij); sji = fmaf(b4.x, df[5], sji);
+                    sij = fmaf(Pi[6], df[6], sij); sji = fmaf(b4.y, df[6], sji);
+                    sij = fmaf(Pi[7], df[7], sij); sji = fmaf(b4.z, df[7], sji);
+                    sij = fmaf(Pi[8], df[8], sij); sji = fmaf(b4.w, df[8], sji);
+                    const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+                    if (BEC) {
+                        // 1/2 r_ij (x) (c_ij + c_ji), c_ij = s_ij rhat, c_ji = s_ji rhat_ji = -s_ji rhat
+                        const float w = 0.5f * (sij - sji);
+                        W[0] = fmaf(dx, w * ux, W[0]); W[1] = fmaf(dx, w * uy, W[1]); W[2] = fmaf(dx, w * uz, W[2]);
+                        W[3] = fmaf(dy, w * ux, W[3]); W[4] = fmaf(dy, w * uy, W[4]); W[5] = fmaf(dy, w * uz, W[5]);
+                        W[6] = fmaf(dz, w * ux, W[6]); W[7] = fmaf(dz, w * uy, W[7]); W[8] = fmaf(dz, w * uz, W[8]);
+                    } else {
+                        const float w = sij + sji;
+                        Fx = fmaf(w, ux, Fx); Fy = fmaf(w, uy, Fy); Fz = fmaf(w, uz, Fz);
+                        if (VIRIAL) {
+                            const float wx = sij * ux, wy = sij * uy, wz = sij * uz;     // F_ij
+                            W[0] = fmaf(dx, wx, W[0]); W[1] = fmaf(dx, wy, W[1]); W[2] = fmaf(dx, wz, W[2]);
+                            W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
+                            W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
+                        }
+                    }
                 }
             }
+            cur = nxt;
         }
+        cp_async_wait<0>();
         const int io = sidx[p];
         if (BEC) {
             const float qt = sqrt_eps * q[p];
@@ -660,12 +856,15 @@ int dispatch_T(int T, F&& f)
 int qnep_launch_pairs(qnep_handle* h, cudaStream_t s)
 {
     const int64_t N = h->N;
-    const int nb = (int)((N + 127) / 128);
+    const int nb = (int)((N + PAIRS_BLOCK - 1) / PAIRS_BLOCK);
     const float rcinv = (float)(1.0 / h->model.rc_r);
+    const size_t smem = sizeof(int4) * 2 * (PAIRS_CH / 4) * PAIRS_BLOCK + 2 * sizeof(int) * PAIRS_CH * PAIRS_BLOCK;
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_pairs<T><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->capLR, h->capLA, h->d_lvR,
-                                      h->d_nlvR, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
+        static bool attr_set = false;
+        if (!attr_set) { cudaFuncSetAttribute(k_pairs<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+        k_pairs<T><<<nb, PAIRS_BLOCK, smem, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
+                                              h->d_lvR, h->d_nlvR, h->d_lvRend, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -679,7 +878,7 @@ int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s)
     const float rcinv = (float)(1.0 / h->model.rc_a);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_desc_angular<T><<<nb, 64, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A);
+        k_desc_angular<T><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A);
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -705,30 +904,17 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
     return QNEP_OK;
 }
 
-int qnep_launch_fp_combine(qnep_handle* h, bool bec, cudaStream_t s)
-{
-    const int64_t N = h->N;
-    const int nb = (int)((N + 127) / 128);
-    dispatch_T(h->model.n_types, [&](auto t) {
-        constexpr int T = decltype(t)::value;
-        k_fp_combine<T><<<nb, 128, 0, s>>>(N, h->d_xyzt, h->d_FpU, h->d_FpQ, h->d_phi, h->d_sums, bec ? 1 : 0,
-                                           (float)h->model.sqrt_eps_inf, h->d_cR, h->d_Fp, h->d_P);
-    });
-    h->launches += 1;
-    QNEP_CUDA_OK(h, cudaGetLastError());
-    return QNEP_OK;
-}
-
 int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_t s)
 {
     const int64_t N = h->N;
-    const int nb = (int)((N + 63) / 64);
+    const int nb = (int)((N + ANG_BLOCK - 1) / ANG_BLOCK);
     const float rcinv = (float)(1.0 / h->model.rc_a);
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Facc, 0, sizeof(float) * (bec ? 9 : 3) * N, s));
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-#define QNEP_FA(B, V) k_force_angular<T, B, V><<<nb, 64, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->d_nlvA, h->d_cA, rcinv, h->d_Fp, \
-                                                                  h->d_A, h->d_Facc, h->d_sums)
+#define QNEP_FA(B, V) k_force_angular<T, B, V><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv, \
+                                                                         h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf, \
+                                                                         h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums)
         if (bec) QNEP_FA(true, false);
         else if (virial) QNEP_FA(false, true);
         else QNEP_FA(false, false);
@@ -739,16 +925,17 @@ int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_
     return QNEP_OK;
 }
 
+// must follow qnep_launch_force_angular of the same mode (it writes the gather records and the angular accumulator)
 int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, cudaStream_t s)
 {
     const int64_t N = h->N;
-    const int nb = (int)((N + 127) / 128);
+    const int nb = (int)((N + RAD_BLOCK - 1) / RAD_BLOCK);
     const float rcinv = (float)(1.0 / h->model.rc_r);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-#define QNEP_FR(B, V) k_force_radial<T, B, V><<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_lvR, h->d_nlvR, rcinv, h->d_P, \
-                                                                  h->d_Facc, h->d_Fs, h->d_q, (float)h->model.sqrt_eps_inf,  \
-                                                                  h->d_sidx, out, h->d_sums)
+#define QNEP_FR(B, V) k_force_radial<T, B, V><<<nb, RAD_BLOCK, 0, s>>>(N, h->geo, h->d_recA, h->d_recB, h->d_xyzt, h->d_lvR, h->capLR, h->d_nlvR, \
+                                                                        h->d_lvRend, rcinv, h->d_Facc, h->d_Fs, h->d_q,                  \
+                                                                        (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums)
         if (bec) QNEP_FR(true, false);
         else if (virial) QNEP_FR(false, true);
         else QNEP_FR(false, false);

@@ -32,7 +32,7 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
 
 // ---- a6: real-space term over the live radial list of this step (mode 1) ---------------------
 __global__ void __launch_bounds__(128)
-k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ nl,
+k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __restrict__ nl, int cap,
             const int* __restrict__ nn, const float* __restrict__ q, float alpha, float* __restrict__ phir,
             float* __restrict__ Fs, double* __restrict__ sums)
 {
@@ -54,8 +54,9 @@ k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int* _
         const float qi = q[p];
         float phi = 0.f, Fx = 0.f, Fy = 0.f, Fz = 0.f;
         const int n = nn[p];
+        const int* words = reinterpret_cast<const int*>(nl + qnep_tiled_base(p, cap / 4));   // slot s: int4 s / 4, lane s % 4
         for (int s = 0; s < n; ++s) {
-            const int e = nl[(int64_t)s * N + p];
+            const int e = words[(int64_t)(s >> 2) * (4 * QNEP_TILE) + (s & 3)];
             const int j = e & QNEP_NL_MASK;
             const float4 xj = xyzt[j];
             const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
@@ -238,7 +239,7 @@ int qnep_launch_realspace(qnep_handle* h, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
-    k_realspace<<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_lvR, h->d_nlvR, h->d_q, (float)h->alpha, h->d_phir, h->d_Fs,
+    k_realspace<<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_lvR, h->capLR, h->d_nlvR, h->d_q, (float)h->alpha, h->d_phir, h->d_Fs,
                                    h->d_sums);
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());

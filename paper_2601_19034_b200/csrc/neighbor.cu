@@ -154,10 +154,11 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
 }
 
 // ---- skin neighbour list -----------------------------------------------------------------------
-// every (j, image) with r < rc_r + skin; the exact per-step lists are derived from it by k_pairs
+// every (j, image) with r < rc_r + skin; the exact per-step lists are derived from it by k_pairs.
+// Warp-tiled int4 layout (qnep_internal.cuh): four consecutive slots are collected in registers and stored at once.
 __global__ void __launch_bounds__(128)
 k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ cellc,
-              const int* __restrict__ start, int capR, int* __restrict__ nlR, int* __restrict__ nnR,
+              const int* __restrict__ start, int capR, int4* __restrict__ nlR, int* __restrict__ nnR,
               int* __restrict__ flags)
 {
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -165,16 +166,20 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
     const float4 xi = xyzt[p];
     const int pc = cellc[p];
     const int c0 = pc & 1023, c1 = (pc >> 10) & 1023, c2 = (pc >> 20) & 1023;
+    int4* out = nlR + qnep_tiled_base(p, capR / 4);
+    int4 buf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
     int nR = 0;
-    for (int code = 0; code < 27; ++code) {
-        const int d0 = code / 9 - 1, d1 = (code / 3) % 3 - 1, d2 = code % 3 - 1;
-        int n0 = c0 + d0, n1 = c1 + d1, n2 = c2 + d2;
-        n0 = n0 < 0 ? n0 + g.ncell[0] : (n0 >= g.ncell[0] ? n0 - g.ncell[0] : n0);
-        n1 = n1 < 0 ? n1 + g.ncell[1] : (n1 >= g.ncell[1] ? n1 - g.ncell[1] : n1);
-        n2 = n2 < 0 ? n2 + g.ncell[2] : (n2 >= g.ncell[2] ? n2 - g.ncell[2] : n2);
-        const int cell = (n0 * g.ncell[1] + n1) * g.ncell[2] + n2;
-        const float sx = d0 * (float)g.hcell[0], sy = d1 * (float)g.hcell[1], sz = d2 * (float)g.hcell[2];
-        for (int t = 0; t < T; ++t) {
+    // type-major order: all neighbours of species 0 first, then species 1, ...  The per-step lists derived from
+    // this one inherit the order, so the radial force kernel switches its own coefficient vector T - 1 times per atom.
+    for (int t = 0; t < T; ++t) {
+        for (int code = 0; code < 27; ++code) {
+            const int d0 = code / 9 - 1, d1 = (code / 3) % 3 - 1, d2 = code % 3 - 1;
+            int n0 = c0 + d0, n1 = c1 + d1, n2 = c2 + d2;
+            n0 = n0 < 0 ? n0 + g.ncell[0] : (n0 >= g.ncell[0] ? n0 - g.ncell[0] : n0);
+            n1 = n1 < 0 ? n1 + g.ncell[1] : (n1 >= g.ncell[1] ? n1 - g.ncell[1] : n1);
+            n2 = n2 < 0 ? n2 + g.ncell[2] : (n2 >= g.ncell[2] ? n2 - g.ncell[2] : n2);
+            const int cell = (n0 * g.ncell[1] + n1) * g.ncell[2] + n2;
+            const float sx = d0 * (float)g.hcell[0], sy = d1 * (float)g.hcell[1], sz = d2 * (float)g.hcell[2];
             const int k = t * g.ncells + cell;
             const int b = start[k], e = start[k + 1];
             for (int q = b; q < e; ++q) {
@@ -182,13 +187,23 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
                 const float dx = (xj.x - xi.x) + sx, dy = (xj.y - xi.y) + sy, dz = (xj.z - xi.z) + sz;
                 const float r2 = dx * dx + dy * dy + dz * dz;
                 if (r2 < g.rcs_r2 && !(q == p && code == 13)) {
-                    if (nR < capR) nlR[(int64_t)nR * N + p] = q | (code << QNEP_NL_SHIFT);
+                    if (nR < capR) {
+                        const int w = q | (code << QNEP_NL_SHIFT);
+                        const int pos = nR & 3;
+                        if (pos == 0) buf.x = w; else if (pos == 1) buf.y = w; else if (pos == 2) buf.z = w; else buf.w = w;
+                        if (pos == 3) {
+                            out[(int64_t)(nR >> 2) * QNEP_TILE] = buf;
+                            buf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
+                        }
+                    }
                     ++nR;
                 }
             }
         }
     }
-    nnR[p] = min(nR, capR);
+    const int kept = min(nR, capR);
+    if (kept & 3) out[(int64_t)(kept >> 2) * QNEP_TILE] = buf;
+    nnR[p] = kept;
     if (nR > capR) atomicMax(&flags[FLAG_MAX_NR], nR);
 }
 

@@ -18,6 +18,20 @@
 #define QNEP_NRAD 5                 // n = 0..4
 #define QNEP_NDESC 25
 
+// Neighbour lists are WARP-TILED: the rows of the 32 atoms p = 32 w .. 32 w + 31 are interleaved in one contiguous
+// block, so a warp streams its lists sequentially (one DRAM page after the other) and every thread loads 16 bytes
+// per request.  Packed-word lists (skin list, live radial list) keep four consecutive slots of an atom in one int4:
+//     vector (g, p) at  ((p >> 5) * (cap / 4) + g) * 32 + (p & 31)          [int4 units], slots 4g .. 4g+3
+// and the live angular pairs one float4 per slot:
+//     entry (s, p)  at  ((p >> 5) * cap + s) * 32 + (p & 31)                [float4 units].
+// Unused slots of the last int4 of an atom hold QNEP_NL_EMPTY.
+#define QNEP_TILE 32
+#define QNEP_NL_EMPTY (-1)
+__host__ __device__ __forceinline__ int64_t qnep_tiled_base(int64_t p, int rows_per_atom)
+{
+    return ((p >> 5) * (int64_t)rows_per_atom) * QNEP_TILE + (p & 31);
+}
+
 constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (reading S9)
 
 // device-side double accumulators
@@ -80,11 +94,12 @@ struct qnep_handle {
     float4* d_off0 = nullptr;        // [N] the same at build time (skin check)
     float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, -)
     int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each
-    int* d_nlR = nullptr;            // [capR][N]  skin list (r < rc_r + skin at build time)
+    int4* d_nlR = nullptr;           // warp-tiled [capR / 4] int4 per atom: skin list (r < rc_r + skin at build time)
     int* d_nnR = nullptr;            // [N]
-    int* d_lvR = nullptr;            // [capLR][N] live radial list of this step (r < rc_r)
+    int4* d_lvR = nullptr;           // warp-tiled [capLR / 4] int4 per atom: live radial list of this step (r < rc_r)
     int* d_nlvR = nullptr;           // [N]
-    float4* d_lvA = nullptr;         // [capLA][N] live angular pairs of this step: (dx, dy, dz, bits(j | tj << 27))
+    int* d_lvRend = nullptr;         // [T][N] end of the species-t segment of the (type-major) live radial list
+    float4* d_lvA = nullptr;         // warp-tiled [capLA] float4 per atom: live angular pairs (dx, dy, dz, bits(j | tj << 27))
     int* d_nlvA = nullptr;           // [N]
     float* d_D = nullptr;            // [25][N]
     float* d_A = nullptr;            // [5*24][N]
@@ -94,7 +109,8 @@ struct qnep_handle {
     float* d_FpU = nullptr;          // [25][N]
     float* d_FpQ = nullptr;          // [25][N]
     float* d_Fp = nullptr;           // [25][N]
-    float* d_P = nullptr;            // [N][T][KPAD]  radial back-prop vectors P^{t}_k
+    float* d_recA = nullptr;         // [T][N][8] gather records of the radial force kernel: (x, y, z, P^t_0..P^t_4)
+    float4* d_recB = nullptr;        // [T][N]    (P^t_5..P^t_8),  P^t_k = sum_n Fp_n c^{ti t}_{nk}
     float* d_phik = nullptr;         // [N]
     float* d_phir = nullptr;         // [N]
     float* d_phi = nullptr;          // [N]
@@ -157,7 +173,6 @@ int qnep_launch_list_stats(qnep_handle* h, double out[6], cudaStream_t s);
 int qnep_launch_pairs(qnep_handle* h, cudaStream_t s);
 int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s);
 int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s);
-int qnep_launch_fp_combine(qnep_handle* h, bool bec, cudaStream_t s);
 int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_t s);
 int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, cudaStream_t s);
 int qnep_launch_fma_peak(double* tflops_host, cudaStream_t s);
