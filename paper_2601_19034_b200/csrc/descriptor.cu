@@ -146,7 +146,15 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 //   phase 2, per ACCEPTED entry: basis functions f_k(r) and S^t_k += f_k for t = t_j, append to the live radial
 //     list.  The expensive part runs for accepted entries only, with no skin-shell divergence.
 // ------------------------------------------------------------------------------------------
-constexpr int PAIRS_BLOCK = 128, PAIRS_CH = 32, PAIRS_DX = 8;
+constexpr int PAIRS_BLOCK = 128, PAIRS_CH = 32, PAIRS_DX = 4;
+
+__device__ __forceinline__ int4 ldg_stream(const int4* p)        // streamed once: do not allocate in L1
+{
+    int4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int word_of(const int4& v, int u) { return u == 0 ? v.x : (u == 1 ? v.y : (u == 2 ? v.z : v.w)); }
 
 template <int T>
 __global__ void __launch_bounds__(PAIRS_BLOCK)
@@ -156,12 +164,11 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
         float4* __restrict__ lvA, int* __restrict__ nlvA, float* __restrict__ D, int* __restrict__ flags)
 {
     constexpr int NV = PAIRS_CH / 4;                         // int4 vectors per chunk
+    static_assert(NV % 4 == 0 && PAIRS_DX == 4, "the register rotation below assumes 4 list vectors and 4 positions in flight");
     __shared__ float4 sh_shift[27];
     __shared__ float sh_c[T * T * NR * KP];
-    extern __shared__ __align__(16) unsigned char pairs_smem[];
-    int4 (*sh_l)[NV][PAIRS_BLOCK] = reinterpret_cast<int4 (*)[NV][PAIRS_BLOCK]>(pairs_smem);              // list stage x 2
-    int (*sh_qe)[PAIRS_BLOCK] = reinterpret_cast<int (*)[PAIRS_BLOCK]>(pairs_smem + sizeof(int4) * 2 * NV * PAIRS_BLOCK);   // queue: words
-    float (*sh_qr)[PAIRS_BLOCK] = reinterpret_cast<float (*)[PAIRS_BLOCK]>(sh_qe + PAIRS_CH);              // queue: r^2
+    __shared__ int sh_qe[PAIRS_CH][PAIRS_BLOCK];             // queue: words
+    __shared__ float sh_qr[PAIRS_CH][PAIRS_BLOCK];           // queue: r^2
     load_shift_table(sh_shift, g);
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
     __syncthreads();
@@ -173,28 +180,22 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
     const int n = nn[p];
     const int n4 = (n + 3) >> 2;
     const int4* lbase = nl + qnep_tiled_base(p, capR / 4);
-    auto issue_stage = [&](int c) {
+    // list vectors: lv[gv & 3] holds vector gv; while gv is processed, gv + 1 feeds the position gathers (PAIRS_DX = 4
+    // slots ahead) and gv + 2, gv + 3 are in flight
+    int4 lv[4];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) {
-            const int gv = c * NV + v;
-            if (gv < n4) cp_async16_cg(&sh_l[c & 1][v][tid], lbase + (int64_t)gv * QNEP_TILE);
-        }
-        cp_async_commit();
-    };
-    issue_stage(0);
-    issue_stage(1);
-    cp_async_wait<1>();
-    float4 ring[PAIRS_DX];
+    for (int k = 0; k < 3; ++k) lv[k] = k < n4 ? ldg_stream(lbase + (int64_t)k * QNEP_TILE) : make_int4(0, 0, 0, 0);
+    lv[3] = make_int4(0, 0, 0, 0);
+    float4 ring[PAIRS_DX];                                   // ring[s & 3] holds the position of the atom of slot s
 #pragma unroll
-    for (int k = 0; k < PAIRS_DX; ++k) {
-        const int w = reinterpret_cast<const int*>(&sh_l[0][k >> 2][tid])[k & 3];
-        ring[k] = k < n ? xyzt[w & QNEP_NL_MASK] : make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    float S[T][NB];
+    for (int k = 0; k < PAIRS_DX; ++k)
+        ring[k] = k < n ? xyzt[word_of(lv[k >> 2], k & 3) & QNEP_NL_MASK] : make_float4(0.f, 0.f, 0.f, 0.f);
+    float S[T][NB];                                          // S^t_k without the "+1" part: sum_j 1/2 fc T_k
+    float S1[T];                                             // sum_j 1/2 fc
     int cnt[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        cnt[t] = 0;
+        cnt[t] = 0; S1[t] = 0.f;
 #pragma unroll
         for (int k = 0; k < NB; ++k) S[t][k] = 0.f;
     }
@@ -203,6 +204,8 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
     float4* outA = lvA + qnep_tiled_base(p, capLA);
     int4 rbuf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
     const int nchunk = (n + PAIRS_CH - 1) / PAIRS_CH;
+    int* qe = &sh_qe[0][tid];
+    float* qr = &sh_qr[0][tid];
     for (int c = 0; c < nchunk; ++c) {
         const int sbase = c * PAIRS_CH;
         int qn = 0;
@@ -210,80 +213,83 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
 #pragma unroll
         for (int t = 0; t < T; ++t) cc[t] = 0;
         // ---- phase 1 ----
-        int4 wv = make_int4(0, 0, 0, 0);
 #pragma unroll
-        for (int i = 0; i < PAIRS_CH; ++i) {
-            if ((i & 3) == 0) wv = sh_l[c & 1][i >> 2][tid];
-            const int e = (i & 3) == 0 ? wv.x : ((i & 3) == 1 ? wv.y : ((i & 3) == 2 ? wv.z : wv.w));
-            const float4 xj = ring[i % PAIRS_DX];
-            // prefetch the position of entry i + DX (same chunk, or the head of the next one)
+        for (int v = 0; v < NV; ++v) {
             {
-                const int i2 = i + PAIRS_DX;
-                if (i2 == PAIRS_CH) cp_async_wait<0>();            // the next stage has landed (issued a chunk ago)
-                const int buf2 = i2 < PAIRS_CH ? (c & 1) : ((c + 1) & 1);
-                const int k2 = i2 < PAIRS_CH ? i2 : i2 - PAIRS_CH;
-                if (sbase + i2 < n) {
-                    const int w2 = reinterpret_cast<const int*>(&sh_l[buf2][k2 >> 2][tid])[k2 & 3];
-                    ring[i % PAIRS_DX] = xyzt[w2 & QNEP_NL_MASK];
-                }
+                const int gv = c * NV + v + 3;
+                if (gv < n4) lv[(v + 3) & 3] = ldg_stream(lbase + (int64_t)gv * QNEP_TILE);
             }
-            if (sbase + i < n) {
-                const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-                const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                if (r2 < g.rc_r2 && r2 >= 1e-12f) {
-                    const int tj = __float_as_int(xj.w);
-                    sh_qe[qn][tid] = e;
-                    sh_qr[qn][tid] = r2;
-                    ++qn;
 #pragma unroll
-                    for (int t = 0; t < T; ++t) cc[t] += (tj == t) ? 1 : 0;
-                    if (r2 < g.rc_a2) {
-                        if (cA_ < capLA) {
-                            *outA = make_float4(dx, dy, dz, __int_as_float((e & QNEP_NL_MASK) | (tj << QNEP_NL_SHIFT)));
-                            outA += QNEP_TILE;
+            for (int u = 0; u < 4; ++u) {
+                const int i = 4 * v + u;
+                const int e = word_of(lv[v & 3], u);
+                const float4 xj = ring[u];
+                if (sbase + i + PAIRS_DX < n) ring[u] = xyzt[word_of(lv[(v + 1) & 3], u) & QNEP_NL_MASK];
+                if (sbase + i < n) {
+                    const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+                    const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 < g.rc_r2 && r2 >= 1e-12f) {
+                        const int tj = __float_as_int(xj.w);
+                        qe[qn * PAIRS_BLOCK] = e;
+                        qr[qn * PAIRS_BLOCK] = r2;
+                        ++qn;
+#pragma unroll
+                        for (int t = 0; t < T - 1; ++t) cc[t] += (tj == t) ? 1 : 0;
+                        if (r2 < g.rc_a2) {
+                            if (cA_ < capLA) {
+                                *outA = make_float4(dx, dy, dz, __int_as_float((e & QNEP_NL_MASK) | (tj << QNEP_NL_SHIFT)));
+                                outA += QNEP_TILE;
+                            }
+                            ++cA_;
                         }
-                        ++cA_;
                     }
                 }
             }
         }
-        // stage c has been consumed: refill its buffer with chunk c + 2
-        issue_stage(c + 2);
-        // ---- phase 2 ----
-        int bnd[T];                                          // the queue is type-major: species t ends at bnd[t]
+        // ---- phase 2: the queue is type-major, species t ends at bnd[t] ----
+        int bnd[T];
         {
             int e_ = 0;
 #pragma unroll
-            for (int t = 0; t < T; ++t) { e_ += cc[t]; bnd[t] = e_; }
+            for (int t = 0; t < T - 1; ++t) { e_ += cc[t]; bnd[t] = e_; cnt[t] += cc[t]; }
+            bnd[T - 1] = qn;
+            cnt[T - 1] += qn - e_;
         }
         for (int k = 0; k < qn; ++k) {
-            const int e = sh_qe[k][tid];
-            const float r2 = sh_qr[k][tid];
-            float f[NB];
-            cheb_basis<true, false>(r2 * fast_rsqrt(r2), rcinv, f, nullptr);
+            const int e = qe[k * PAIRS_BLOCK];
+            const float r2 = qr[k * PAIRS_BLOCK];
+            // 1/2 fc(r) T_k(x), k = 0..8   (f_k = 1/2 fc (T_k + 1): the "+1" part is accumulated once in S1)
+            const float tt = r2 * fast_rsqrt(r2) * rcinv;
+            const float hfc = 0.25f + 0.25f * __cosf(3.14159265358979f * tt);
+            const float tm1 = tt - 1.f;
+            const float x = 2.f * tm1 * tm1 - 1.f, x2 = x + x;
+            float a[T];
 #pragma unroll
-            for (int t = 0; t < T; ++t) {
-                const float w = (T == 1 || ((t == 0 || k >= bnd[t - 1]) && k < bnd[t])) ? 1.f : 0.f;
+            for (int t = 0; t < T; ++t) a[t] = (T == 1 || ((t == 0 || k >= bnd[t - 1]) && k < bnd[t])) ? hfc : 0.f;
+            float Tm = 1.f, Tc = x;
 #pragma unroll
-                for (int kk = 0; kk < NB; ++kk) S[t][kk] = fmaf(w, f[kk], S[t][kk]);
+            for (int t = 0; t < T; ++t) { S1[t] += a[t]; S[t][1] = fmaf(a[t], Tc, S[t][1]); }
+#pragma unroll
+            for (int kk = 2; kk < NB; ++kk) {
+                const float Tn = fmaf(x2, Tc, -Tm);
+#pragma unroll
+                for (int t = 0; t < T; ++t) S[t][kk] = fmaf(a[t], Tn, S[t][kk]);
+                Tm = Tc; Tc = Tn;
             }
-            if (cRtot < capLR) {
-                const int pos = cRtot & 3;
-                if (pos == 0) rbuf.x = e; else if (pos == 1) rbuf.y = e; else if (pos == 2) rbuf.z = e; else rbuf.w = e;
-                if (pos == 3) {
-                    outR[(int64_t)(cRtot >> 2) * QNEP_TILE] = rbuf;
-                    rbuf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
-                }
-            }
+            // append to the live radial list (four slots per int4)
+            const int pos = cRtot & 3;
+            rbuf.x = pos == 0 ? e : rbuf.x; rbuf.y = pos == 1 ? e : rbuf.y; rbuf.z = pos == 2 ? e : rbuf.z; rbuf.w = pos == 3 ? e : rbuf.w;
+            if (pos == 3 && cRtot < capLR) outR[(int64_t)(cRtot >> 2) * QNEP_TILE] = rbuf;
             ++cRtot;
         }
-#pragma unroll
-        for (int t = 0; t < T; ++t) cnt[t] += cc[t];
     }
-    cp_async_wait<0>();
     const int nlive = min(cRtot, capLR);
-    if (nlive & 3) outR[(int64_t)(nlive >> 2) * QNEP_TILE] = rbuf;
+    if (nlive & 3) {
+        const int m = nlive & 3;
+        rbuf.y = m > 1 ? rbuf.y : QNEP_NL_EMPTY; rbuf.z = m > 2 ? rbuf.z : QNEP_NL_EMPTY; rbuf.w = QNEP_NL_EMPTY;
+        outR[(int64_t)(nlive >> 2) * QNEP_TILE] = rbuf;
+    }
     nlvR[p] = nlive;
     nlvA[p] = min(cA_, capLA);
     {
@@ -293,14 +299,16 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
     }
     if (cRtot > capLR) atomicMax(&flags[FLAG_MAX_LR], cRtot);
     if (cA_ > capLA) atomicMax(&flags[FLAG_MAX_LA], cA_);
+    // f_0 = fc = 2 (1/2 fc): S^t_0 = 2 S1;  f_k = 1/2 fc T_k + 1/2 fc: S^t_k = S[t][k] + S1
 #pragma unroll
     for (int nidx = 0; nidx < NR; ++nidx) {
         float d = 0.f;
 #pragma unroll
         for (int t = 0; t < T; ++t) {
             const float* c = sh_c + ((ti * T + t) * NR + nidx) * KP;
+            d = fmaf(c[0], 2.f * S1[t], d);
 #pragma unroll
-            for (int k = 0; k < NB; ++k) d = fmaf(c[k], S[t][k], d);
+            for (int k = 1; k < NB; ++k) d = fmaf(c[k], S[t][k] + S1[t], d);
         }
         D[(int64_t)nidx * N + p] = d;
     }
@@ -858,12 +866,9 @@ int qnep_launch_pairs(qnep_handle* h, cudaStream_t s)
     const int64_t N = h->N;
     const int nb = (int)((N + PAIRS_BLOCK - 1) / PAIRS_BLOCK);
     const float rcinv = (float)(1.0 / h->model.rc_r);
-    const size_t smem = sizeof(int4) * 2 * (PAIRS_CH / 4) * PAIRS_BLOCK + 2 * sizeof(int) * PAIRS_CH * PAIRS_BLOCK;
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        static bool attr_set = false;
-        if (!attr_set) { cudaFuncSetAttribute(k_pairs<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
-        k_pairs<T><<<nb, PAIRS_BLOCK, smem, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
+        k_pairs<T><<<nb, PAIRS_BLOCK, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
                                               h->d_lvR, h->d_nlvR, h->d_lvRend, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
     });
     h->launches += 1;
