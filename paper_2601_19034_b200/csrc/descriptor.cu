@@ -750,15 +750,8 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                 const int s = 4 * v + u;
                 if (s < n) {
                     const int e = ec[u];
-                    float a8[8];
-#pragma unroll
-                    for (int a = 0; a < 8; ++a) a8[a] = ra[u][a];
-                    const float4 b4 = rb[u];
-                    if (s + 4 < n) {
-                        const int j2 = en[u] & QNEP_NL_MASK;
-                        ldg256(gA + 8 * (int64_t)j2, ra[u]);
-                        rb[u] = __ldg(gB + j2);
-                    }
+                    const float (&a8)[8] = ra[u];
+                    const float4& b4 = rb[u];
                     if (s >= seg_end) {
                         // next non-empty species segment: my own vector for neighbours of species tj is my record for tj
                         do { ++tj; seg_end = lvRend[(int64_t)tj * N + p]; } while (s >= seg_end && tj < T - 1);
@@ -797,6 +790,12 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                             W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
                             W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
                         }
+                    }
+                    // the record registers are free again: request the record of slot s + 4 into them
+                    if (s + 4 < n) {
+                        const int j2 = en[u] & QNEP_NL_MASK;
+                        ldg256(gA + 8 * (int64_t)j2, ra[u]);
+                        rb[u] = __ldg(gB + j2);
                     }
                 }
             }
