@@ -23,7 +23,7 @@ int dev_alloc(qnep_handle* h, Tp** p, size_t count)
 void free_workspace(qnep_handle* h)
 {
     void** ptrs[] = {(void**)&h->d_key, (void**)&h->d_cnt, (void**)&h->d_start, (void**)&h->d_fill, (void**)&h->d_tmpidx,
-                     (void**)&h->d_sidx, (void**)&h->d_cellc, (void**)&h->d_xyzt, (void**)&h->d_off0, (void**)&h->d_mfrac,
+                     (void**)&h->d_sidx, (void**)&h->d_cm, (void**)&h->d_cmi, (void**)&h->d_cellc, (void**)&h->d_xyzt, (void**)&h->d_off0, (void**)&h->d_mfrac,
                      (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_lvR, (void**)&h->d_nlvR,
                      (void**)&h->d_lvA, (void**)&h->d_nlvA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
                      (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_recA, (void**)&h->d_recB, (void**)&h->d_lvRend,
@@ -99,6 +99,8 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_key, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_tmpidx, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_sidx, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_cm, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_cmi, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_cellc, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_xyzt, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_off0, n))) return rc;
@@ -137,6 +139,8 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_cnt, (size_t)nkeys + 1))) return rc;
         if ((rc = dev_alloc(h, &h->d_start, (size_t)nkeys + 1))) return rc;
         if ((rc = dev_alloc(h, &h->d_fill, (size_t)nkeys))) return rc;
+        if ((rc = dev_alloc(h, &h->d_ctot, (size_t)g.ncells + 1))) return rc;
+        if ((rc = dev_alloc(h, &h->d_cstart, (size_t)g.ncells + 1))) return rc;
         h->nkeys = nkeys;
         h->force_rebuild = true;
     }
@@ -674,7 +678,7 @@ void qnep_destroy(qnep_handle* h)
 {
     if (!h) return;
     free_workspace(h);
-    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_sums, h->d_flags, h->d_kvec,
+    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_sums, h->d_flags, h->d_kvec,
                     h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
                     h->d_htypes, h->d_hout};
     for (void* p : ptrs) if (p) cudaFree(p);

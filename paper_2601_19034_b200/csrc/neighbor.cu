@@ -100,9 +100,36 @@ __global__ void k_rank(int64_t N, const int* __restrict__ key, const int* __rest
     sidx[b + rank] = me;
 }
 
+// ---- cell-major order for the PPPM kernels ---------------------------------------------------------
+// The neighbour kernels want a warp to hold ONE species, hence the (type, cell) order.  Spreading and back-
+// interpolation want atoms that are close in space to be close in the launch order whatever their species, so that
+// the mesh is swept once: rank q = cstart[cell] + (atoms of lower species in the cell) + (rank inside the bucket).
+__global__ void k_cell_totals(int ncells, int T, const int* __restrict__ cnt, int* __restrict__ ctot)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncells) return;
+    int v = 0;
+    for (int t = 0; t < T; ++t) v += cnt[t * ncells + c];
+    ctot[c] = v;
+}
+
+__global__ void k_cm_rank(int64_t N, int ncells, const int* __restrict__ key, const int* __restrict__ sidx,
+                          const int* __restrict__ start, const int* __restrict__ cnt, const int* __restrict__ cstart,
+                          int* __restrict__ cm, int* __restrict__ cmi)
+{
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const int k = key[sidx[p]];
+    const int t = k / ncells, c = k - t * ncells;
+    int q = cstart[c] + ((int)p - start[k]);
+    for (int u = 0; u < t; ++u) q += cnt[u * ncells + c];
+    cm[p] = q;
+    cmi[q] = (int)p;
+}
+
 // ---- per-step prep: cell-relative fp32 coordinates, PPPM mesh coordinates, skin check --------
 __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t* __restrict__ types_or_null,
-                       const int* __restrict__ sidx, const int* __restrict__ key, Geometry g, int at_build,
+                       const int* __restrict__ sidx, const int* __restrict__ key, const int* __restrict__ cm, Geometry g, int at_build,
                        int* __restrict__ cellc, float4* __restrict__ xyzt, float4* __restrict__ off0,
                        float4* __restrict__ mfrac, int* __restrict__ mi0, int* __restrict__ flags)
 {
@@ -142,8 +169,11 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
     }
     float4 v = make_float4(off[0], off[1], off[2], __int_as_float(type));
     xyzt[p] = v;
-    mfrac[p] = make_float4(dx[0], dx[1], dx[2], 0.f);
-    mi0[p] = pack3(m0[0], m0[1], m0[2]);
+    {
+        const int q = cm[p];                       // PPPM arrays are kept in cell-major order
+        mfrac[q] = make_float4(dx[0], dx[1], dx[2], 0.f);
+        mi0[q] = pack3(m0[0], m0[1], m0[2]);
+    }
     if (at_build) {
         off0[p] = v;
     } else {
@@ -227,7 +257,7 @@ int qnep_launch_prep(qnep_handle* h, const double* pos, bool at_build, cudaStrea
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 255) / 256);
-    k_prep<<<nb, 256, 0, s>>>(N, pos, nullptr, h->d_sidx, h->d_key, h->geo, at_build ? 1 : 0, h->d_cellc, h->d_xyzt,
+    k_prep<<<nb, 256, 0, s>>>(N, pos, nullptr, h->d_sidx, h->d_key, h->d_cm, h->geo, at_build ? 1 : 0, h->d_cellc, h->d_xyzt,
                               h->d_off0, h->d_mfrac, h->d_mi0, h->d_flags);
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -244,7 +274,13 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
     k_exclusive_scan<<<1, 1024, 0, s>>>(h->nkeys, h->d_cnt, h->d_start);
     k_scatter<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_fill, h->d_tmpidx);
     k_rank<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_tmpidx, h->d_sidx);
-    h->launches += 4;
+    {
+        const int nc = h->geo.ncells;
+        k_cell_totals<<<(nc + 255) / 256, 256, 0, s>>>(nc, h->model.n_types, h->d_cnt, h->d_ctot);
+        k_exclusive_scan<<<1, 1024, 0, s>>>(nc, h->d_ctot, h->d_cstart);
+        k_cm_rank<<<nb, 256, 0, s>>>(N, nc, h->d_key, h->d_sidx, h->d_start, h->d_cnt, h->d_cstart, h->d_cm, h->d_cmi);
+    }
+    h->launches += 7;
     int rc = qnep_launch_prep(h, pos, true, s);
     if (rc) return rc;
     const int nb2 = (int)((N + 127) / 128);

@@ -61,10 +61,10 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, 
 }
 
 __global__ void __launch_bounds__(128)
-k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0,
+k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0, const int* __restrict__ cmi,
          const float* __restrict__ q, float* __restrict__ mesh)
 {
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;      // cell-major rank
     if (p >= N) return;
     const float4 fr = mfrac[p];
     float wx[5], wy[5], wz[5];
@@ -84,7 +84,7 @@ k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
             if (i - c >= 0 && i - c <= 3) v = (o == i - c) ? wz[c] : v;
         w8[i] = v;
     }
-    const float qi = q[p];
+    const float qi = q[cmi[p]];
 #pragma unroll
     for (int a = 0; a < 5; ++a) {
         const float qa = qi * wx[a];
@@ -370,7 +370,7 @@ constexpr int GATHER_GROUP = 8;
 constexpr int GATHER_BLOCK = 128;
 
 __global__ void __launch_bounds__(GATHER_BLOCK)
-k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0,
+k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0, const int* __restrict__ cmi,
          const float* __restrict__ q, const float4* __restrict__ field, int add_to_Fs,
          float* __restrict__ phik, float* __restrict__ Fs)
 {
@@ -432,8 +432,8 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
         if (c == 0) { s_out[0][al] = ph; s_out[1][al] = ex; s_out[2][al] = ey; s_out[3][al] = ez; }
     }
     __syncthreads();
-    const int64_t p = p0 + t;
-    if (p >= N) return;
+    if (p0 + t >= N) return;
+    const int64_t p = cmi[p0 + t];                         // the block walked cell-major ranks; outputs in sorted order
     const float c2k = 2.f * (float)QNEP_K_COULOMB;
     phik[p] = c2k * s_out[0][t];                          // bracket of Eq. 38
     const float cq = -c2k * q[p];                         // Eq. 37
@@ -531,7 +531,7 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
 
     // 1. spread
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mesh, 0, sizeof(float) * h->ngrid, s));
-    k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_q, h->d_mesh);
+    k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_mesh);
     // 2. forward z (real -> complex), forward y
     with_split(n2, [&](auto r1, auto r2) {
         constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
@@ -582,7 +582,7 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
     });
     // 5. gather
     const int nbg = (int)((N + GATHER_BLOCK - 1) / GATHER_BLOCK);
-    k_gather<<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_q, h->d_field, h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs);
+    k_gather<<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs);
     h->launches += 7;
     QNEP_CUDA_OK(h, ce);
     QNEP_CUDA_OK(h, cudaGetLastError());

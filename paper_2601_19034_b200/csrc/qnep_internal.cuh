@@ -89,11 +89,15 @@ struct qnep_handle {
     int* d_fill = nullptr;           // [nkeys]
     int* d_tmpidx = nullptr;         // [N]
     int* d_sidx = nullptr;           // [N] sorted -> original
+    int* d_ctot = nullptr;           // [ncells + 1] atoms per cell (all species)
+    int* d_cstart = nullptr;         // [ncells + 1] its exclusive scan
+    int* d_cm = nullptr;             // [N] sorted index p -> cell-major rank q (order of the PPPM kernels)
+    int* d_cmi = nullptr;            // [N] q -> p
     int* d_cellc = nullptr;          // [N] packed cell coordinates (10 bits each)
     float4* d_xyzt = nullptr;        // [N] cell-relative position, w = type bits
     float4* d_off0 = nullptr;        // [N] the same at build time (skin check)
-    float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, -)
-    int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each
+    float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, -), cell-major order
+    int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each, cell-major order
     int4* d_nlR = nullptr;           // warp-tiled [capR / 4] int4 per atom: skin list (r < rc_r + skin at build time)
     int* d_nnR = nullptr;            // [N]
     int4* d_lvR = nullptr;           // warp-tiled [capLR / 4] int4 per atom: live radial list of this step (r < rc_r)
