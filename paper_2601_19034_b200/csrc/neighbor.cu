@@ -185,7 +185,9 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
 
 // ---- skin neighbour list -----------------------------------------------------------------------
 // every (j, image) with r < rc_r + skin; the exact per-step lists are derived from it by k_pairs.
-// Warp-tiled int4 layout (qnep_internal.cuh): four consecutive slots are collected in registers and stored at once.
+// Warp-tiled int4 layout (qnep_internal.cuh); entries are appended one 4-byte word at a time (the partial vectors
+// merge in L2), readers never look beyond the count.  The candidate loop is the whole cost of a rebuild
+// (~920 candidates per atom), so it is kept to a dozen instructions per candidate.
 __global__ void __launch_bounds__(128)
 k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ cellc,
               const int* __restrict__ start, int capR, int4* __restrict__ nlR, int* __restrict__ nnR,
@@ -194,46 +196,55 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
     const float4 xi = xyzt[p];
+    const int ti = __float_as_int(xi.w);
     const int pc = cellc[p];
     const int c0 = pc & 1023, c1 = (pc >> 10) & 1023, c2 = (pc >> 20) & 1023;
-    int4* out = nlR + qnep_tiled_base(p, capR / 4);
-    int4 buf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
+    int* out = reinterpret_cast<int*>(nlR + qnep_tiled_base(p, capR / 4));    // slot s at out[(s >> 2) * 128 + (s & 3)]
     int nR = 0;
+    const float rcs2 = g.rcs_r2;
+    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
     // type-major order: all neighbours of species 0 first, then species 1, ...  The per-step lists derived from
     // this one inherit the order, so the radial force kernel switches its own coefficient vector T - 1 times per atom.
     for (int t = 0; t < T; ++t) {
         for (int code = 0; code < 27; ++code) {
             const int d0 = code / 9 - 1, d1 = (code / 3) % 3 - 1, d2 = code % 3 - 1;
+            // the whole cell is out of reach of this atom?  (positions are relative to the atom's own cell, in [0, hcell);
+            // with a single cell along an axis the coordinate is the nearest image to the origin instead: no pruning there)
+            {
+                const float ex = g.ncell[0] < 2 ? 0.f : (d0 < 0 ? xi.x : (d0 > 0 ? h0 - xi.x : 0.f));
+                const float ey = g.ncell[1] < 2 ? 0.f : (d1 < 0 ? xi.y : (d1 > 0 ? h1 - xi.y : 0.f));
+                const float ez = g.ncell[2] < 2 ? 0.f : (d2 < 0 ? xi.z : (d2 > 0 ? h2 - xi.z : 0.f));
+                const float em = fmaxf(ex, 0.f) * fmaxf(ex, 0.f) + fmaxf(ey, 0.f) * fmaxf(ey, 0.f) + fmaxf(ez, 0.f) * fmaxf(ez, 0.f);
+                if (em > rcs2 * 1.0001f) continue;
+            }
             int n0 = c0 + d0, n1 = c1 + d1, n2 = c2 + d2;
             n0 = n0 < 0 ? n0 + g.ncell[0] : (n0 >= g.ncell[0] ? n0 - g.ncell[0] : n0);
             n1 = n1 < 0 ? n1 + g.ncell[1] : (n1 >= g.ncell[1] ? n1 - g.ncell[1] : n1);
             n2 = n2 < 0 ? n2 + g.ncell[2] : (n2 >= g.ncell[2] ? n2 - g.ncell[2] : n2);
             const int cell = (n0 * g.ncell[1] + n1) * g.ncell[2] + n2;
-            const float sx = d0 * (float)g.hcell[0], sy = d1 * (float)g.hcell[1], sz = d2 * (float)g.hcell[2];
+            // r_ij = x_j - (x_i - shift)
+            const float ox = xi.x - d0 * h0, oy = xi.y - d1 * h1, oz = xi.z - d2 * h2;
             const int k = t * g.ncells + cell;
             const int b = start[k], e = start[k + 1];
-            for (int q = b; q < e; ++q) {
-                const float4 xj = xyzt[q];
-                const float dx = (xj.x - xi.x) + sx, dy = (xj.y - xi.y) + sy, dz = (xj.z - xi.z) + sz;
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                if (r2 < g.rcs_r2 && !(q == p && code == 13)) {
-                    if (nR < capR) {
-                        const int w = q | (code << QNEP_NL_SHIFT);
-                        const int pos = nR & 3;
-                        if (pos == 0) buf.x = w; else if (pos == 1) buf.y = w; else if (pos == 2) buf.z = w; else buf.w = w;
-                        if (pos == 3) {
-                            out[(int64_t)(nR >> 2) * QNEP_TILE] = buf;
-                            buf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
-                        }
-                    }
+            const int self = (code == 13 && t == ti) ? (int)p : -1;
+            const int cbits = code << QNEP_NL_SHIFT;
+            auto test = [&](int q, const float4& xj) {
+                const float dx = xj.x - ox, dy = xj.y - oy, dz = xj.z - oz;
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                if (r2 < rcs2 && q != self) {
+                    if (nR < capR) out[((nR >> 2) << 7) | (nR & 3)] = q | cbits;
                     ++nR;
                 }
+            };
+            int q = b;
+            for (; q + 4 <= e; q += 4) {
+                const float4 x0 = xyzt[q], x1 = xyzt[q + 1], x2 = xyzt[q + 2], x3 = xyzt[q + 3];
+                test(q, x0); test(q + 1, x1); test(q + 2, x2); test(q + 3, x3);
             }
+            for (; q < e; ++q) test(q, xyzt[q]);
         }
     }
-    const int kept = min(nR, capR);
-    if (kept & 3) out[(int64_t)(kept >> 2) * QNEP_TILE] = buf;
-    nnR[p] = kept;
+    nnR[p] = min(nR, capR);
     if (nR > capR) atomicMax(&flags[FLAG_MAX_NR], nR);
 }
 

@@ -24,9 +24,9 @@
 //     vector (g, p) at  ((p >> 5) * (cap / 4) + g) * 32 + (p & 31)          [int4 units], slots 4g .. 4g+3
 // and the live angular pairs one float4 per slot:
 //     entry (s, p)  at  ((p >> 5) * cap + s) * 32 + (p & 31)                [float4 units].
-// Unused slots of the last int4 of an atom hold QNEP_NL_EMPTY.
+// Slots at and beyond an atom's count are undefined: readers never look at them.
 #define QNEP_TILE 32
-#define QNEP_NL_EMPTY (-1)
+#define QNEP_NL_EMPTY (-1)           // filler of the last int4 of a live list (never read: readers stop at the count)
 __host__ __device__ __forceinline__ int64_t qnep_tiled_base(int64_t p, int rows_per_atom)
 {
     return ((p >> 5) * (int64_t)rows_per_atom) * QNEP_TILE + (p & 31);
