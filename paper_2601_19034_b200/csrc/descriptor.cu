@@ -411,11 +411,16 @@ constexpr int W0P = 28;
 
 __device__ __forceinline__ float tanh_f32(float z)
 {
-    // tanh z = 1 - 2 / (exp(2z) + 1); exact limits at +-inf, abs error ~1e-7
-    const float e = expf(2.f * z);
-    return 1.f - __fdividef(2.f, e + 1.f);
+    // tanh z = 1 - 2 / (exp(2z) + 1) on the MUFU pipe (EX2, RCP); exact limits at +-inf.  Where the exponent is
+    // large the result is insensitive to it, so the fp32 rounding of 2 z log2(e) costs < 1e-7 absolute.
+    float e, r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * 2.885390081777927f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.f));
+    return fmaf(-2.f, r, 1.f);
 }
 
+// Persistent blocks: the weights of all species are staged in shared memory once per block, then the block walks
+// chunks of 128 atoms.
 __global__ void __launch_bounds__(128)
 k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, float b1U, float b1q,
      const float4* __restrict__ xyzt, const float* __restrict__ D, float* __restrict__ Ui, float* __restrict__ qraw,
@@ -423,11 +428,14 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
 {
     extern __shared__ __align__(16) float sh_w[];
     __shared__ double sh_red[32];
-    for (int i = threadIdx.x; i < T * nn_stride; i += blockDim.x) sh_w[i] = nnw[i];
+    {
+        const float4* src = reinterpret_cast<const float4*>(nnw);
+        float4* dst = reinterpret_cast<float4*>(sh_w);
+        for (int i = threadIdx.x; i < T * nn_stride / 4; i += blockDim.x) dst[i] = src[i];
+    }
     __syncthreads();
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    float U = 0.f, q = 0.f;
-    if (p < N) {
+    double accU = 0.0, accQ = 0.0;
+    for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < N; p += (int64_t)gridDim.x * blockDim.x) {
         const int ti = __float_as_int(xyzt[p].w);
         const float* w = sh_w + ti * nn_stride;
         const float* b0 = w + H * W0P;
@@ -436,6 +444,7 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
         float x[W0P], dU[W0P], dQ[W0P];
 #pragma unroll
         for (int v = 0; v < W0P; ++v) { x[v] = v < ND ? D[(int64_t)v * N + p] : 0.f; dU[v] = 0.f; dQ[v] = 0.f; }
+        float U = 0.f, q = 0.f;
         for (int mu = 0; mu < H; ++mu) {
             const float4* row = reinterpret_cast<const float4*>(w + mu * W0P);
             float wr[W0P];
@@ -451,7 +460,7 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
             const float a = w1U[mu], b = w1q[mu];
             U = fmaf(a, hmu, U);
             q = fmaf(b, hmu, q);
-            const float dh = 1.f - hmu * hmu;
+            const float dh = fmaf(-hmu, hmu, 1.f);
             const float au = a * dh, bq = b * dh;
 #pragma unroll
             for (int v = 0; v < ND; ++v) { dU[v] = fmaf(au, wr[v], dU[v]); dQ[v] = fmaf(bq, wr[v], dQ[v]); }
@@ -462,9 +471,11 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
         qraw[p] = q;
 #pragma unroll
         for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + p] = dU[v]; FpQ[(int64_t)v * N + p] = dQ[v]; }
+        accU += (double)U;
+        accQ += (double)q;
     }
-    const double su = block_sum((double)U, sh_red);
-    const double sq = block_sum((double)q, sh_red);
+    const double su = block_sum(accU, sh_red);
+    const double sq = block_sum(accQ, sh_red);
     if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
 }
 
@@ -892,9 +903,11 @@ int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s)
 int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
 {
     const int64_t N = h->N;
-    const int nb = (int)((N + 127) / 128);
     const size_t smem = sizeof(float) * (size_t)h->model.n_types * h->nn_stride;
     static bool attr_set = false;
+    static int sms = 0;
+    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
+    const int nb = (int)std::min<int64_t>((N + 127) / 128, (int64_t)sms * 4);      // persistent: 4 blocks of 128 threads per SM
     if (!attr_set) {
         QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
