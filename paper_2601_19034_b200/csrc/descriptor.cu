@@ -78,6 +78,48 @@ __device__ __forceinline__ void cheb_basis(float r, float rcinv, float* __restri
     }
 }
 
+// Derivative basis in the form used by the radial force kernel:  f_k'(r) = A k U_{k-1}(x) + B (T_k(x) + 1)  with
+// A = 1/2 fc dx/dr, B = 1/2 dfc/dr (T_k' = k U_{k-1}; f_0 = fc = 1/2 fc (T_0 + 1) fits the same formula), so
+//   sum_k a_k f_k'(r) = A sum_{k>=1} a_k kU_k + B sum_k a_k Tp_k,   kU_k = k U_{k-1},  Tp_k = T_k + 1.
+struct ChebDeriv {
+    float A, B;
+    float kU[NB];     // kU[0] = 0 (unused)
+    float Tp[NB];
+    __device__ __forceinline__ void eval(float r, float rcinv)
+    {
+        const float t = r * rcinv;
+        float sn, cs;
+        __sincosf(3.14159265358979f * t, &sn, &cs);
+        const float tm1 = t - 1.f;
+        const float x = 2.f * tm1 * tm1 - 1.f, x2 = x + x;
+        A = (0.5f + 0.5f * cs) * (2.f * tm1 * rcinv);            // 1/2 fc * 4 (t - 1) / rc
+        B = -0.7853981633974483f * rcinv * sn;                   // 1/2 * (-pi / (2 rc)) sin(pi t)
+        float Tm = 1.f, Tc = x, Um = 1.f, Uc = x2;               // T_0, T_1, U_0, U_1
+        Tp[0] = 2.f; Tp[1] = x + 1.f;
+        kU[0] = 0.f; kU[1] = 1.f; kU[2] = 2.f * Uc;
+#pragma unroll
+        for (int k = 2; k < NB; ++k) {
+            const float Tn = fmaf(x2, Tc, -Tm);
+            Tp[k] = Tn + 1.f;
+            Tm = Tc; Tc = Tn;
+            if (k + 1 < NB) {
+                const float Un = fmaf(x2, Uc, -Um);              // U_k
+                kU[k + 1] = (float)(k + 1) * Un;
+                Um = Uc; Uc = Un;
+            }
+        }
+    }
+    __device__ __forceinline__ float dot(const float (&a)[NB]) const
+    {
+        float du = a[1], dt = a[0] * Tp[0];
+#pragma unroll
+        for (int k = 1; k < NB; ++k) dt = fmaf(a[k], Tp[k], dt);
+#pragma unroll
+        for (int k = 2; k < NB; ++k) du = fmaf(a[k], kU[k], du);
+        return fmaf(A, du, B * dt);
+    }
+};
+
 // MUFU.RSQ without the denormal range fix-up of rsqrtf (arguments here are squared distances >= 1e-12)
 __device__ __forceinline__ float fast_rsqrt(float x)
 {
@@ -776,15 +818,21 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                     const float dx = (a8[0] - xi.x) + sh.x, dy = (a8[1] - xi.y) + sh.y, dz = (a8[2] - xi.z) + sh.z;
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     const float rinv = fast_rsqrt(r2), r = r2 * rinv;
-                    float df[NB];
-                    cheb_basis<false, true>(r, rcinv, nullptr, df);
-                    float sij = Pi[0] * df[0], sji = a8[3] * df[0];
+                    ChebDeriv cd;
+                    cd.eval(r, rcinv);
+                    const float Pj[NB] = {a8[3], a8[4], a8[5], a8[6], a8[7], b4.x, b4.y, b4.z, b4.w};
+                    float sij, sji;
+                    if (BEC || VIRIAL) {
+                        sij = cd.dot(Pi);
+                        sji = cd.dot(Pj);
+                    } else {
+                        // only s_ij + s_ji is needed: one contraction with P^{i,tj} + P^{j,ti}
+                        float Ps[NB];
 #pragma unroll
-                    for (int k = 1; k < 5; ++k) { sij = fmaf(Pi[k], df[k], sij); sji = fmaf(a8[3 + k], df[k], sji); }
-                    sij = fmaf(Pi[5], df[5], sij); sji = fmaf(b4.x, df[5], sji);
-                    sij = fmaf(Pi[6], df[6], sij); sji = fmaf(b4.y, df[6], sji);
-                    sij = fmaf(Pi[7], df[7], sij); sji = fmaf(b4.z, df[7], sji);
-                    sij = fmaf(Pi[8], df[8], sij); sji = fmaf(b4.w, df[8], sji);
+                        for (int k = 0; k < NB; ++k) Ps[k] = Pi[k] + Pj[k];
+                        sij = cd.dot(Ps);
+                        sji = 0.f;
+                    }
                     const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
                     if (BEC) {
                         // 1/2 r_ij (x) (c_ij + c_ji), c_ij = s_ij rhat, c_ji = s_ji rhat_ji = -s_ji rhat
