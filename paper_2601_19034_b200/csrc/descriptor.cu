@@ -82,7 +82,7 @@ __device__ __forceinline__ void cheb_basis(float r, float rcinv, float* __restri
 // A = 1/2 fc dx/dr, B = 1/2 dfc/dr (T_k' = k U_{k-1}; f_0 = fc = 1/2 fc (T_0 + 1) fits the same formula), so
 //   sum_k a_k f_k'(r) = A sum_{k>=1} a_k kU_k + B sum_k a_k Tp_k,   kU_k = k U_{k-1},  Tp_k = T_k + 1.
 struct ChebDeriv {
-    float A, B;
+    float A, B, hfc;  // hfc = 1/2 fc(r)
     float kU[NB];     // kU[0] = 0 (unused)
     float Tp[NB];
     __device__ __forceinline__ void eval(float r, float rcinv)
@@ -92,7 +92,8 @@ struct ChebDeriv {
         __sincosf(3.14159265358979f * t, &sn, &cs);
         const float tm1 = t - 1.f;
         const float x = 2.f * tm1 * tm1 - 1.f, x2 = x + x;
-        A = (0.5f + 0.5f * cs) * (2.f * tm1 * rcinv);            // 1/2 fc * 4 (t - 1) / rc
+        hfc = 0.25f + 0.25f * cs;
+        A = hfc * (4.f * tm1 * rcinv);                           // 1/2 fc dx/dr, x = 2 (t - 1)^2 - 1
         B = -0.7853981633974483f * rcinv * sn;                   // 1/2 * (-pi / (2 rc)) sin(pi t)
         float Tm = 1.f, Tc = x, Um = 1.f, Uc = x2;               // T_0, T_1, U_0, U_1
         Tp[0] = 2.f; Tp[1] = x + 1.f;
@@ -553,7 +554,7 @@ __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const do
     }
 
 template <int T, bool BEC, bool VIRIAL>
-__global__ void __launch_bounds__(ANG_BLOCK)
+__global__ void __launch_bounds__(ANG_BLOCK, BEC || VIRIAL ? 4 : 6)
 k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
                 const float* __restrict__ cA, const float* __restrict__ cR, float rcinv, const float* __restrict__ FpU,
                 const float* __restrict__ FpQ, const float* __restrict__ phi, float sqrt_eps, const float* __restrict__ Ain,
@@ -634,18 +635,22 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
             const float dx = pr.x, dy = pr.y, dz = pr.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float rinv = fast_rsqrt(r2), r = r2 * rinv;
-            float f[NB], df[NB];
-            cheb_basis<true, true>(r, rcinv, f, df);
+            // g_n = 1/2 fc sum_k c_nk Tp_k,  g_n' = A sum_k c_nk kU_k + B sum_k c_nk Tp_k   (ChebDeriv)
+            ChebDeriv cd;
+            cd.eval(r, rcinv);
             const int jw = __float_as_int(pr.w);
             const int j = jw & QNEP_NL_MASK;
             const float* c = sh_c + (ti * T + (int)((unsigned)jw >> QNEP_NL_SHIFT)) * NR * KP;
             float gn[NR], dgn[NR];
 #pragma unroll
             for (int a = 0; a < NR; ++a) {
-                float v = 0.f, dv = 0.f;
+                float dt = c[a * KP] * cd.Tp[0], du = c[a * KP + 1];
 #pragma unroll
-                for (int k = 0; k < NB; ++k) { v = fmaf(c[a * KP + k], f[k], v); dv = fmaf(c[a * KP + k], df[k], dv); }
-                gn[a] = v; dgn[a] = dv;
+                for (int k = 1; k < NB; ++k) dt = fmaf(c[a * KP + k], cd.Tp[k], dt);
+#pragma unroll
+                for (int k = 2; k < NB; ++k) du = fmaf(c[a * KP + k], cd.kU[k], du);
+                gn[a] = cd.hfc * dt;
+                dgn[a] = fmaf(cd.A, du, cd.B * dt);
             }
             const float x = dx * rinv, y = dy * rinv, z = dz * rinv;
             const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z;
