@@ -44,6 +44,28 @@ FLOPS_NN_BWD_H80 = 4400.0
 FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.4: 148 SMs x 128 lanes x 2 x 1.965 GHz
 
 
+def max_over_ranks(x, dist=None, device="cpu"):
+    """Job time of a multi-rank run: every rank contributes its own device time, the job took the longest."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_atoms, steps, world, ms_total):
+    """Replicas only: every rank evaluates its own copy of the workload, so the whole job processed
+    world * n_atoms * steps atom-steps in the time of the slowest rank."""
+    return world * n_atoms * steps / (ms_total * 1e-3)
+
+
+# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the five FP32 kernels on config 4, from the
+# ncu --set full capture summarised in profiles/r01_ncu_full_tiled_lists.txt (reported only for that workload)
+NCU_TRAFFIC_CONFIG4 = {"k_pairs": 1.72e9, "k_desc_angular": 1.03e9, "k_nn": 0.28e9, "k_force_angular": 1.45e9,
+                       "k_force_radial": 0.68e9}
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -233,10 +255,7 @@ def main():
     launches = h.kernel_launches() - l0
     stage_ms, n_evals = h.profile_sum()
     clocks = sampler.stop(tw0, tw1)
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, dev)
     ms_per_step = ms_total / K
     # the MD must have stayed an MD: (E_pot + E_kin) conserved between the end of the warm-up and the end of the
     # timed run, no skin violation (md_run raises), kinetic temperature reported
@@ -245,7 +264,7 @@ def main():
     md_sanity = {"etot_start_eV": float(e_start[0] + e_start[1]), "etot_end_eV": float(e_end[0] + e_end[1]),
                  "drift_eV_per_atom": float((e_end[0] + e_end[1] - e_start[0] - e_start[1]) / n),
                  "T_start_K": float(e_start[1] / (1.5 * n * kB)), "T_end_K": float(e_end[1] / (1.5 * n * kB))}
-    value = world * n * K / (ms_total * 1e-3)
+    value = whole_job_value(n, K, world, ms_total)
     stats = h.neighbor_stats()
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------------
@@ -267,7 +286,9 @@ def main():
     fp32_flops = sum(v[1] for v in kernels.values())
     achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS, "traffic": None,
+                "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
+                "traffic": NCU_TRAFFIC_CONFIG4.get(dom) if (args.config == 4 and not args.n_side) else None,
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_ncu_full_tiled_lists.txt",
                 "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "fma_loop_measured_tflops": fma_measured, "frac_of_measured_fma_loop": achieved / fma_measured if fma_measured else None,
                 "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops,
@@ -315,11 +336,8 @@ def main():
         e2e_step()
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_e2e = float(t.item())
-    e2e = {"value": world * n * Ke / t_e2e, "unit": "atom-steps/s", "steps": Ke,
+    t_e2e = max_over_ranks(t_e2e, dist, dev)
+    e2e = {"value": whole_job_value(n, Ke, world, t_e2e * 1e3), "unit": "atom-steps/s", "steps": Ke,
            "h2d_bytes_per_step": int(hp.numel() * 8 + ht.numel() * 4), "d2h_bytes_per_step": int(hf.numel() * 8 + 8),
            "api": "qnep_compute_host (pinned host buffers; neighbour rebuild every %d calls)" % args.rebuild_every}
 
