@@ -181,6 +181,21 @@ int qnep_profile_sum(qnep_handle *h, float *ms_sum_host, int32_t n, int64_t *n_e
 int64_t qnep_kernel_launches(const qnep_handle *h);
 
 /*
+ * Response of the ions to a homogeneous external electric field and ionic polarization current (PAPER.md II.D,
+ * Eq. 29-30, :229-237), from the Born effective charges Z written by qnep_compute (QNEP_WANT_BEC):
+ *     F^ext_{i,b} = sum_a E_a Z_{i,ab}            (Eq. 29)        -> fext_dev [3][N], eV/A for E in V/A
+ *     Pdot_a      = sum_i sum_b Z_{i,ab} v_{i,b}  (Eq. 30)        -> pdot_dev [3], e A / (time unit of v)
+ * bec_dev : DEVICE, [9][N] component-major, entry (3 a + b) * N + i = Z_{i,ab} (a: polarization component,
+ *           b: displacement component), the layout qnep_compute writes; owned by the caller.
+ * efield  : HOST, 3 doubles, or NULL to skip Eq. 29 (fext_dev is then ignored).
+ * vel_dev : DEVICE, [3][N] component-major, or NULL to skip Eq. 30 (pdot_dev is then ignored).
+ * Enqueued on `cuda_stream`, no synchronisation.  Returns QNEP_ERR_INVALID_ARG for a null handle / bec pointer,
+ * n_atoms <= 0, or a requested output whose pointer is null.
+ */
+int qnep_response(qnep_handle *h, int64_t n_atoms, const double *bec_dev, const double *efield_host,
+                  const double *vel_dev, double *fext_dev, double *pdot_dev, void *cuda_stream);
+
+/*
  * Neighbour statistics of the last call (synchronises): out[0], out[1] = max / mean length of the skin list
  * (r < rc_r + skin at build time); out[2], out[3] = max / mean number of radial neighbours inside rc_r;
  * out[4], out[5] = max / mean number of angular neighbours inside rc_a (the exact per-step lists).

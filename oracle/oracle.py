@@ -149,6 +149,21 @@ def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, d
     return out
 
 
+def response(bec, efield=None, vel=None):
+    """Eq. 29-30: (fext [3][N] or None, pdot [3] or None) from the BEC tensor [9][N]."""
+    bec = _f64(bec)
+    n = bec.shape[1]
+    fext = np.zeros((3, n)) if efield is not None else None
+    pdot = np.zeros(3) if vel is not None else None
+    e = _f64(np.asarray(efield, dtype=np.float64)) if efield is not None else None
+    v = _f64(vel) if vel is not None else None
+    f = lib().orc_response
+    f.restype = None
+    f(C.c_int64(n), _p(bec), _p(e) if e is not None else None, _p(v) if v is not None else None,
+      _p(fext) if fext is not None else None, _p(pdot) if pdot is not None else None)
+    return fext, pdot
+
+
 def compute_workload(w, **kw):
     return compute(w.model, w.params, w.es, w.pos, w.types, w.box, **kw)
 

@@ -21,6 +21,7 @@
  *   U^r, U^k, U^s     :85-118 Eq. 6-10        reading G1 (erfc(alpha r), k != 0)
  *   forces / virial   :124-199 Eq. 11-23      dynamic-charge terms folded (:140), reading S6
  *   BEC               :205-227 Eq. 24-28      reading S12
+ *   field response    :229-237 Eq. 29-30      F^ext = E.Z, Pdot = sum_i Z_i v_i (orc_response)
  *   PPPM              :266-304 Eq. 34-38      readings G2 (Eq. 36), S10 (W, P = 5), S11 (FFT)
  *
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): NaCl Madelung constant,
@@ -28,7 +29,8 @@
  * finite-difference forces and finite-strain virials, PPPM adjointness identity,
  * PPPM -> Ewald convergence, invariants, Legendre double sum vs spherical
  * harmonics (scipy), FFT vs numpy, B-spline vs its convolution definition,
- * alias-sum denominator vs brute force, BEC vs finite differences of q.
+ * alias-sum denominator vs brute force, BEC vs finite differences of q,
+ * Eq. 29-30 vs the point-charge limit (F = q E, Pdot = sum q v) and the power identity.
  * No function here is "parity unpinned".
  *
  * Units: Angstrom, eV, elementary charge.  K = 1/(4 pi eps0) (reading S9).
@@ -976,4 +978,29 @@ int orc_compute(const orc_model *m, const double *params, const orc_es *es, int6
     nlist_free(&nl);
     free(w); free(D); free(dU); free(dq); free(Ui); free(q); free(phi); free(Fes);
     return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Eq. 29-30 (PAPER.md :229-237): response to a homogeneous external field    */
+/* ------------------------------------------------------------------------- */
+/* bec[9][N] with entry (3 a + b) N + i = Z_{i,ab} (a: polarization component, b: displacement component, Eq. 27-28).
+ * efield[3] or NULL -> fext[3][N];  vel[3][N] or NULL -> pdot[3]. */
+void orc_response(int64_t n, const double *bec, const double *efield, const double *vel, double *fext, double *pdot)
+{
+    if (efield) {
+        for (int64_t i = 0; i < n; ++i)
+            for (int b = 0; b < 3; ++b) {
+                double f = 0.0;
+                for (int a = 0; a < 3; ++a) f += efield[a] * bec[(3 * a + b) * n + i];   /* Eq. 29 */
+                fext[b * n + i] = f;
+            }
+    }
+    if (vel) {
+        for (int a = 0; a < 3; ++a) {
+            double p = 0.0;
+            for (int64_t i = 0; i < n; ++i)
+                for (int b = 0; b < 3; ++b) p += bec[(3 * a + b) * n + i] * vel[b * n + i];   /* Eq. 30 */
+            pdot[a] = p;
+        }
+    }
 }

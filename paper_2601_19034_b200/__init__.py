@@ -36,7 +36,8 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
                "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_check", "qnep_get_timings",
-               "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_neighbor_stats", "qnep_fma_peak",
+               "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
+               "qnep_fma_peak",
                "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
 
 
@@ -95,6 +96,8 @@ def load_library():
     lib.qnep_profile_sum.argtypes = [vp, C.POINTER(C.c_float), i32, C.POINTER(i64)]
     lib.qnep_kernel_launches.restype = i64
     lib.qnep_kernel_launches.argtypes = [vp]
+    lib.qnep_response.restype = C.c_int
+    lib.qnep_response.argtypes = [vp, i64, vp, C.POINTER(dbl), vp, vp, vp, vp]
     lib.qnep_neighbor_stats.restype = C.c_int
     lib.qnep_neighbor_stats.argtypes = [vp, C.POINTER(dbl)]
     lib.qnep_fma_peak.restype = C.c_int
@@ -258,6 +261,20 @@ class QNEP:
 
     def kernel_launches(self) -> int:
         return int(self._lib.qnep_kernel_launches(self._h))
+
+    def response(self, bec, efield=None, vel=None, stream=None):
+        """Eq. 29-30 from the BEC tensor [9][N] (cuda float64): returns (fext [3][N] or None, pdot [3] or None)."""
+        import torch
+        assert bec.is_cuda and bec.dtype == torch.float64 and bec.is_contiguous() and bec.shape[0] == 9
+        n = bec.shape[1]
+        fext = torch.empty((3, n), dtype=torch.float64, device=bec.device) if efield is not None else None
+        pdot = torch.empty(3, dtype=torch.float64, device=bec.device) if vel is not None else None
+        if vel is not None:
+            assert vel.is_cuda and vel.dtype == torch.float64 and vel.is_contiguous() and tuple(vel.shape) == (3, n)
+        e3 = (C.c_double * 3)(*[float(x) for x in efield]) if efield is not None else None
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        self._ok(self._lib.qnep_response(self._h, n, ptr(bec), e3, ptr(vel), ptr(fext), ptr(pdot), self._stream(stream)))
+        return fext, pdot
 
     def neighbor_stats(self) -> dict:
         out = (C.c_double * 6)()

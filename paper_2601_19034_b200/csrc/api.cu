@@ -279,6 +279,47 @@ __global__ void k_md_energy(const double* __restrict__ sums, int mode, double* _
     out[1] = sums[SUM_KE];
 }
 
+// ---- Eq. 29-30: external-field force and polarization current from the Born effective charges -------------
+struct Vec3d { double v[3]; };
+
+__global__ void __launch_bounds__(256)
+k_response(int64_t N, const double* __restrict__ Z, Vec3d E, int want_f, const double* __restrict__ vel,
+           double* __restrict__ fext, double* __restrict__ pdot)
+{
+    __shared__ double sh[3][8];
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    double pd[3] = {0.0, 0.0, 0.0};
+    if (i < N) {
+        double z[9];
+#pragma unroll
+        for (int c = 0; c < 9; ++c) z[c] = Z[(int64_t)c * N + i];
+        if (want_f) {
+#pragma unroll
+            for (int b = 0; b < 3; ++b) fext[(int64_t)b * N + i] = E.v[0] * z[b] + E.v[1] * z[3 + b] + E.v[2] * z[6 + b];   // Eq. 29
+        }
+        if (vel) {
+            const double v0 = vel[i], v1 = vel[N + i], v2 = vel[2 * N + i];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) pd[a] = z[3 * a] * v0 + z[3 * a + 1] * v1 + z[3 * a + 2] * v2;                      // Eq. 30
+        }
+    }
+    if (vel) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            double x = pd[a];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+            if ((threadIdx.x & 31) == 0) sh[a][threadIdx.x >> 5] = x;
+        }
+        __syncthreads();
+        if (threadIdx.x < 3) {
+            double r = 0.0;
+            for (int w = 0; w < (int)(blockDim.x >> 5); ++w) r += sh[threadIdx.x][w];
+            atomicAdd(&pdot[threadIdx.x], r);
+        }
+    }
+}
+
 int upload_model(qnep_handle* h)
 {
     const qnep_model_desc& m = h->model;
@@ -623,6 +664,24 @@ int qnep_profile_sum(qnep_handle* h, float* ms, int32_t n, int64_t* n_evals)
             ms[QNEP_T_TOTAL] += t;
         }
     }
+    return QNEP_OK;
+}
+
+int qnep_response(qnep_handle* h, int64_t n_atoms, const double* bec_dev, const double* efield_host, const double* vel_dev,
+                  double* fext_dev, double* pdot_dev, void* cuda_stream)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (n_atoms <= 0 || !bec_dev) { h->err = "qnep_response: n_atoms <= 0 or null BEC pointer"; return QNEP_ERR_INVALID_ARG; }
+    if ((efield_host && !fext_dev) || (vel_dev && !pdot_dev)) { h->err = "qnep_response: a requested output pointer is null"; return QNEP_ERR_INVALID_ARG; }
+    if (!efield_host && !vel_dev) return QNEP_OK;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    Vec3d E = {{0.0, 0.0, 0.0}};
+    if (efield_host) for (int a = 0; a < 3; ++a) E.v[a] = efield_host[a];
+    if (vel_dev) QNEP_CUDA_OK(h, cudaMemsetAsync(pdot_dev, 0, sizeof(double) * 3, s));
+    const int nb = (int)((n_atoms + 255) / 256);
+    k_response<<<nb, 256, 0, s>>>(n_atoms, bec_dev, E, efield_host ? 1 : 0, vel_dev, fext_dev, pdot_dev);
+    h->launches += 1;
+    QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;
 }
 

@@ -303,3 +303,29 @@ def test_md_skin_violation_survives_a_rebuild(torch):
     with pytest.raises(Q.QnepError) as ei:
         h.md_run(pos, vel, types, w.box, w.masses, 0.5 / 10.180505, 31)   # ends right after a rebuild
     assert ei.value.code == Q.QNEP_ERR_SKIN_VIOLATED
+
+
+def test_field_response_parity(torch, oracle):
+    """Eq. 29-30 on the GPU (qnep_response) against the oracle, on the GPU's own BEC of config 1 (3000 atoms: several
+    blocks and a ragged tail) and on a 33-atom subset; fp64 contractions, so the bar is rounding."""
+    w = I.config1(mode=2)
+    rng = np.random.Generator(np.random.PCG64(5))
+    for n in (w.n_atoms, 33):
+        sub = replace(w, pos=np.ascontiguousarray(w.pos[:, :n]), types=np.ascontiguousarray(w.types[:n]))
+        h, res = gpu_eval(torch, sub, want=Q.WANT_ALL | Q.WANT_BEC)
+        E = np.array([0.02, -0.05, 0.01])
+        vel = rng.normal(0, 0.03, (3, n))
+        bec = torch.tensor(res["bec"], dtype=torch.float64, device="cuda")
+        f_gpu, p_gpu = h.response(bec, E, torch.tensor(vel, dtype=torch.float64, device="cuda"))
+        h.check()
+        f_ref, p_ref = oracle.response(res["bec"], E, vel)
+        assert np.abs(f_gpu.cpu().numpy() - f_ref).max() <= 1e-14 * max(1.0, np.abs(f_ref).max())
+        assert np.abs(p_gpu.cpu().numpy() - p_ref).max() <= 1e-12 * max(1.0, np.abs(p_ref).max())
+        # and end to end against the oracle's own BEC, at the force tolerance
+        ref = oracle.compute_workload(sub, want_bec=True)
+        f_o, p_o = oracle.response(ref["bec"], E, vel)
+        assert rel_rms(f_gpu.cpu().numpy(), f_o) <= TOL_F_RELRMS
+        assert np.abs(p_gpu.cpu().numpy() - p_o).max() <= TOL_F_RELRMS * np.abs(ref["bec"]).max() * np.abs(vel).sum()
+        f_only, none = h.response(bec, E, None)
+        assert none is None and torch.equal(f_only, f_gpu)
+        h.destroy()

@@ -424,3 +424,43 @@ def test_bec_sum_rule_and_finite_difference_assembly(oracle):
             Zfd[:, :, i] += 0.5 * (np.outer(rij, c[i, j]) - np.outer(-rij, c[j, i]))
     assert np.abs(Z - Zfd).max() < 5e-8
     assert np.abs(Z - qt[None, None, :] * np.eye(3)[:, :, None]).max() > 1e-3
+
+
+# ------------------------------------------------------------- Eq. 29-30: field response
+def test_field_response_point_charge_limit_and_power_identity(oracle):
+    """Pins for orc_response (PAPER.md :229-237).
+    (a) Point-charge limit: with the descriptor scaler set to zero the network sees x = 0, the charges depend on the
+        species only and the BEC is q~_i I, so Eq. 29 must give the textbook force q~_i E and Eq. 30 the textbook
+        current sum_i q~_i v_i.
+    (b) Power identity for position-dependent charges (Z_i not symmetric): sum_i F_i^ext . v_i = E . Pdot -- fails if
+        the two equations contract different indices of Z.
+    (c) Acoustic sum rule: sum_i F_i^ext = (sum_i Z_i)^T E = Q~ E = 0 and a rigid translation carries no current."""
+    w = I.config0(mode=2)
+    rng = np.random.Generator(np.random.PCG64(77))
+    n = w.n_atoms
+    E = np.array([0.3, -0.7, 0.45])
+    vel = rng.normal(0, 0.05, (3, n))
+    # (a)
+    m = w.model
+    params = w.params.copy()
+    nco = 2 * m.n_types ** 2 * (m.n_max_r + 1) * (m.basis_r + 1)
+    D = (m.n_max_r + 1) + (m.n_max_a + 1) * m.l_max
+    params[nco:nco + D] = 0.0                                     # scaler s = 0
+    out = oracle.compute(m, params, I.EsDesc(method=0), w.pos, w.types, w.box, use_bins=False, want_bec=True)
+    qt = m.sqrt_eps_inf * out["charges"]
+    assert np.abs(qt).max() > 1e-3 and len(np.unique(np.round(qt, 12))) == m.n_types
+    fext, pdot = oracle.response(out["bec"], E, vel)
+    assert np.abs(fext - E[:, None] * qt[None, :]).max() < 1e-13
+    assert np.abs(pdot - (vel * qt[None, :]).sum(axis=1)).max() < 1e-12
+    # (b), (c)
+    out = oracle.compute(m, w.params, I.EsDesc(method=0), w.pos, w.types, w.box, use_bins=False, want_bec=True)
+    Z = out["bec"].reshape(3, 3, n)
+    assert np.abs(Z - np.transpose(Z, (1, 0, 2))).max() > 1e-3    # the test is blind to transposition otherwise
+    fext, pdot = oracle.response(out["bec"], E, vel)
+    assert abs((fext * vel).sum() - E @ pdot) < 1e-12 * max(1.0, abs(E @ pdot))
+    assert np.abs(fext.sum(axis=1)).max() < 1e-12
+    _, p_rigid = oracle.response(out["bec"], None, np.repeat(np.array([[0.1], [0.2], [-0.3]]), n, axis=1))
+    assert np.abs(p_rigid).max() < 1e-12
+    # only one of the two outputs requested
+    f_only, none = oracle.response(out["bec"], E, None)
+    assert none is None and np.array_equal(f_only, fext)
