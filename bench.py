@@ -61,9 +61,9 @@ def whole_job_value(n_atoms, steps, world, ms_total):
 
 
 # DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the five FP32 kernels on config 4, from the
-# ncu --set full capture summarised in profiles/r01_ncu_full_tiled_lists.txt (reported only for that workload)
+# ncu --set full capture summarised in profiles/r01_ncu_full_current.txt (reported only for that workload)
 NCU_TRAFFIC_CONFIG4 = {"k_pairs": 1.72e9, "k_desc_angular": 1.03e9, "k_nn": 0.28e9, "k_force_angular": 1.45e9,
-                       "k_force_radial": 0.68e9}
+                       "k_force_radial": 0.68e9}      # MB read + written columns of that file
 
 
 def load_peaks():
@@ -219,22 +219,26 @@ def main():
     def md(pos, vel, nsteps, dt_fs):
         return h.md_run(pos, vel, types, w.box, masses, dt_fs * FS, nsteps)
 
-    # warm-up (also grows neighbour capacity / shrinks dt if the random-init model is too violent)
+    # dt search, untimed: a random-init model has no repulsive core and can be violent; the library reports an atom that
+    # moved more than skin/2 between rebuilds (QNEP_ERR_SKIN_VIOLATED) and the run is repeated with half the time step
+    # until warm-up + timed steps go through (the metric is per force evaluation, so dt does not change it).  The same
+    # loop lets the library grow its neighbour capacity (QNEP_ERR_NEIGHBOR_OVERFLOW).
     dt_fs = args.dt_fs
-    pos, vel = pos0.clone(), vel0.clone()
-    e_start = None
-    for attempt in range(8):
+    for attempt in range(12):
+        pos, vel = pos0.clone(), vel0.clone()
         try:
-            e_start = md(pos, vel, Wm, dt_fs).cpu().numpy()
+            md(pos, vel, Wm + K, dt_fs)
             break
         except Q.QnepError as err:
             if err.code == Q.QNEP_ERR_SKIN_VIOLATED:
                 dt_fs *= 0.5
             elif err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
                 raise
-            pos, vel = pos0.clone(), vel0.clone()
     else:
-        raise RuntimeError("warm-up failed")
+        raise RuntimeError("no stable time step found")
+    # warm-up proper, from the initial state again (the timed steps then repeat the validated trajectory)
+    pos, vel = pos0.clone(), vel0.clone()
+    e_start = md(pos, vel, Wm, dt_fs).cpu().numpy()
 
     # ---- timed region: exactly K steps, inputs resident in HBM -------------------------------------------
     sampler = ClockSampler(local)
@@ -291,7 +295,7 @@ def main():
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
                 "traffic": NCU_TRAFFIC_CONFIG4.get(dom) if (args.config == 4 and not args.n_side) else None,
-                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_ncu_full_tiled_lists.txt",
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_ncu_full_current.txt",
                 "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "fma_loop_measured_tflops": fma_measured, "frac_of_measured_fma_loop": achieved / fma_measured if fma_measured else None,
                 "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops,
