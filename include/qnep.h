@@ -162,6 +162,14 @@ int qnep_md_run(qnep_handle *h, int64_t n_atoms, double *pos_dev, double *vel_de
                 const double box[9], const double *mass_host, double dt, int32_t n_steps,
                 double *energy_dev, void *cuda_stream);
 
+/*
+ * CUDA graphs inside qnep_md_run: a step is ~25 kernel launches, which bounds small systems (a 3000-atom step is
+ * ~0.1 ms of GPU work), so the step is captured once per kind (lists reused / rebuild) and replayed.
+ * mode 0: never; 1 (default): when n_atoms <= 100000; 2: always.  Replayed steps carry no per-stage events
+ * (qnep_profile_sum counts no evaluations for them).
+ */
+int qnep_set_md_graphs(qnep_handle *h, int32_t mode);
+
 /* Synchronise the stream of the last call and report its device-side error state (OK, NEIGHBOR_OVERFLOW, SKIN_VIOLATED, CUDA). */
 int qnep_check(qnep_handle *h);
 

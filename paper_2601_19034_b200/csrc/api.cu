@@ -142,12 +142,14 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_ctot, (size_t)g.ncells + 1))) return rc;
         if ((rc = dev_alloc(h, &h->d_cstart, (size_t)g.ncells + 1))) return rc;
         h->nkeys = nkeys;
+        h->ws_generation += 1;
         h->force_rebuild = true;
     }
     const bool geo_changed = box_changed || std::memcmp(&g, &h->geo, sizeof(Geometry)) != 0;
     h->geo = g;
     std::memcpy(h->box, box, sizeof(double) * 9);
     if (geo_changed || realloc_atoms) {
+        h->ws_generation += 1;
         h->force_rebuild = true;
         if (h->es.method == 1) { if ((rc = qnep_setup_ewald(h))) return rc; }
         if (h->es.method == 2) { if ((rc = qnep_setup_pppm(h))) return rc; }
@@ -320,6 +322,14 @@ k_response(int64_t N, const double* __restrict__ Z, Vec3d E, int want_f, const d
     }
 }
 
+void drop_md_graphs(qnep_handle* h)
+{
+    for (int k = 0; k < 2; ++k) {
+        if (h->md_exec[k]) cudaGraphExecDestroy(h->md_exec[k]);
+        h->md_exec[k] = nullptr;
+    }
+}
+
 int upload_model(qnep_handle* h)
 {
     const qnep_model_desc& m = h->model;
@@ -364,67 +374,85 @@ int upload_model(qnep_handle* h)
     return QNEP_OK;
 }
 
-// the pipeline proper; `forces_out` may be NULL (then an internal buffer is used when the virial is wanted)
-int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* types, uint32_t want, double* energy,
-                 double* forces, double* virial, double* charges, double* bec, cudaStream_t s)
+// host-side decision of a pipeline run: does this evaluation rebuild the neighbour list?  (updates the counters)
+bool plan_pipeline(qnep_handle* h)
 {
-    int rc;
     const bool rebuild = h->force_rebuild || h->rebuild_every <= 1 || h->calls_since_build < 0 ||
                          h->calls_since_build >= h->rebuild_every;
-    cudaEvent_t* ev = h->ring.data() + (size_t)(h->prof_count % qnep_handle::RING) * qnep_handle::NEV;
-    h->ev = ev;
-    h->prof_count += 1;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[0], s));
-    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_sums, 0, sizeof(double) * SUM_COUNT, s));
     if (rebuild) {
-        if ((rc = qnep_launch_build(h, pos, types, s))) return rc;
         h->calls_since_build = 0;
         h->force_rebuild = false;
     }
     h->rebuilt_last = rebuild;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[1], s));
-    if (!rebuild) { if ((rc = qnep_launch_prep(h, pos, false, s))) return rc; }
     h->calls_since_build += 1;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[2], s));
+    return rebuild;
+}
+
+// the pipeline proper (enqueue only); `timed` = false leaves out the stage events (stream capture: qnep_md_run's graphs)
+int enqueue_pipeline(qnep_handle* h, bool rebuild, bool timed, int64_t N, const double* pos, const int32_t* types, uint32_t want,
+                     double* energy, double* forces, double* virial, double* charges, double* bec, cudaStream_t s)
+{
+    int rc;
+    cudaEvent_t* ev = nullptr;
+    if (timed) {
+        ev = h->ring.data() + (size_t)(h->prof_count % qnep_handle::RING) * qnep_handle::NEV;
+        h->ev = ev;
+        h->prof_count += 1;
+    }
+#define QNEP_STAGE(i) do { if (timed) QNEP_CUDA_OK(h, cudaEventRecord(ev[i], s)); } while (0)
+    QNEP_STAGE(0);
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_sums, 0, sizeof(double) * SUM_COUNT, s));
+    if (rebuild) { if ((rc = qnep_launch_build(h, pos, types, s))) return rc; }
+    QNEP_STAGE(1);
+    if (!rebuild) { if ((rc = qnep_launch_prep(h, pos, false, s))) return rc; }
+    QNEP_STAGE(2);
     if ((rc = qnep_launch_pairs(h, s))) return rc;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[3], s));
+    QNEP_STAGE(3);
     if ((rc = qnep_launch_desc_angular(h, s))) return rc;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[4], s));
+    QNEP_STAGE(4);
     if ((rc = qnep_launch_nn(h, (want & QNEP_WANT_CHARGES) ? charges : nullptr, s))) return rc;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[5], s));
+    QNEP_STAGE(5);
     if (h->es.method != 0 && h->model.mode == 1) { if ((rc = qnep_launch_realspace(h, s))) return rc; }
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[6], s));
+    QNEP_STAGE(6);
     if (h->es.method == 1) { if ((rc = qnep_launch_ewald(h, pos, s))) return rc; }
     else if (h->es.method == 2) { if ((rc = qnep_launch_pppm(h, (want & QNEP_WANT_VIRIAL) != 0, s))) return rc; }
     else QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
     if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
     const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
     const bool need_virial = (want & QNEP_WANT_VIRIAL) != 0;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[7], s));
+    QNEP_STAGE(7);
     if (need_forces) {
         if ((rc = qnep_launch_force_angular(h, false, need_virial, s))) return rc;     // bracketed alone by ev[7], ev[8]
-        QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
+        QNEP_STAGE(8);
         double* fout = ((want & QNEP_WANT_FORCES) && forces) ? forces : h->d_Fmd;
         if ((rc = qnep_launch_force_radial(h, false, need_virial, fout, s))) return rc;
     } else {
-        QNEP_CUDA_OK(h, cudaEventRecord(ev[8], s));
+        QNEP_STAGE(8);
     }
     k_finalize<<<1, 32, 0, s>>>(h->d_sums, h->model.mode, (want & QNEP_WANT_ENERGY) ? energy : nullptr,
                                 (want & QNEP_WANT_VIRIAL) ? virial : nullptr);
     h->launches += 1;
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[9], s));
+    QNEP_STAGE(9);
     if ((want & QNEP_WANT_BEC) && bec) {
         if ((rc = qnep_launch_force_angular(h, true, false, s))) return rc;
         if ((rc = qnep_launch_force_radial(h, true, false, bec, s))) return rc;
     }
-    QNEP_CUDA_OK(h, cudaEventRecord(ev[10], s));
-    h->ev_valid = true;
+    QNEP_STAGE(10);
+#undef QNEP_STAGE
+    h->ev_valid = timed;
     QNEP_CUDA_OK(h, cudaMemcpyAsync(h->h_flags, h->d_flags, sizeof(int) * FLAG_COUNT, cudaMemcpyDeviceToHost, s));
-    QNEP_CUDA_OK(h, cudaEventRecord(h->ev_flags, s));
+    if (timed) QNEP_CUDA_OK(h, cudaEventRecord(h->ev_flags, s));
     h->flags_pending = true;
     h->last_stream = s;
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;
+}
+
+int run_pipeline(qnep_handle* h, int64_t N, const double* pos, const int32_t* types, uint32_t want, double* energy,
+                 double* forces, double* virial, double* charges, double* bec, cudaStream_t s)
+{
+    const bool rebuild = plan_pipeline(h);
+    return enqueue_pipeline(h, rebuild, true, N, pos, types, want, energy, forces, virial, charges, bec, s);
 }
 
 int check_args(qnep_handle* h, int64_t n_atoms, const void* pos, const void* types, const double* box, uint32_t want,
@@ -544,6 +572,14 @@ int qnep_compute(qnep_handle* h, int64_t n_atoms, const double* pos_dev, const i
     return run_pipeline(h, n_atoms, pos_dev, types_dev, want, energy_dev, forces_dev, virial_dev, charges_dev, bec_dev, s);
 }
 
+int qnep_set_md_graphs(qnep_handle* h, int32_t mode)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (mode < 0 || mode > 2) { h->err = "qnep_set_md_graphs: mode must be 0, 1 or 2"; return QNEP_ERR_INVALID_ARG; }
+    h->md_graph_mode = mode;
+    return QNEP_OK;
+}
+
 int qnep_check(qnep_handle* h)
 {
     if (!h) return QNEP_ERR_INVALID_ARG;
@@ -605,11 +641,66 @@ int qnep_md_run(qnep_handle* h, int64_t n_atoms, double* pos_dev, double* vel_de
         if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
         h->md_have_forces = true;
     }
+    const bool graphs = h->md_graph_mode == 2 || (h->md_graph_mode == 1 && n_atoms <= QNEP_GRAPH_MAX_ATOMS);
+    cudaStream_t caller = s;
+    if (graphs && n_steps > 0) {
+        // the steps run on the handle's own stream, after everything the caller has enqueued so far
+        if (!h->md_stream) {
+            QNEP_CUDA_OK(h, cudaStreamCreateWithFlags(&h->md_stream, cudaStreamNonBlocking));
+            QNEP_CUDA_OK(h, cudaEventCreateWithFlags(&h->md_fence, cudaEventDisableTiming));
+        }
+        QNEP_CUDA_OK(h, cudaEventRecord(h->md_fence, caller));
+        QNEP_CUDA_OK(h, cudaStreamWaitEvent(h->md_stream, h->md_fence, 0));
+        s = h->md_stream;
+    }
+    if (graphs && n_steps > 0) {
+        qnep_handle::MdKey key = {};
+        key.pos = pos_dev; key.vel = vel_dev; key.types = types_dev; key.N = n_atoms; key.dt = dt; key.s = nullptr;     // replay always happens on md_stream
+        key.gen = h->ws_generation;
+        for (int t = 0; t < QNEP_MAX_TYPES; ++t) key.m[t] = ms.m[t];
+        if (std::memcmp(&key, &h->md_key, sizeof(key)) != 0) {
+            drop_md_graphs(h);
+            h->md_key = key;
+        }
+    }
     for (int step = 0; step < n_steps; ++step) {
-        k_vv_kick_drift<<<nb, 256, 0, s>>>(n_atoms, pos_dev, vel_dev, h->d_Fmd, types_dev, ms, dt);
-        if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
-        k_vv_kick<<<nb, 256, 0, s>>>(n_atoms, vel_dev, h->d_Fmd, types_dev, ms, dt, h->d_sums);
-        h->launches += 2;
+        if (!graphs) {
+            k_vv_kick_drift<<<nb, 256, 0, s>>>(n_atoms, pos_dev, vel_dev, h->d_Fmd, types_dev, ms, dt);
+            if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
+            k_vv_kick<<<nb, 256, 0, s>>>(n_atoms, vel_dev, h->d_Fmd, types_dev, ms, dt, h->d_sums);
+            h->launches += 2;
+            continue;
+        }
+        const int kind = plan_pipeline(h) ? 1 : 0;
+        if (!h->md_exec[kind]) {
+            // capture one step of this kind; nothing runs until the graph is launched below
+            const int64_t l0 = h->launches;
+            cudaGraph_t graph = nullptr;
+            QNEP_CUDA_OK(h, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+            k_vv_kick_drift<<<nb, 256, 0, s>>>(n_atoms, pos_dev, vel_dev, h->d_Fmd, types_dev, ms, dt);
+            rc = enqueue_pipeline(h, kind == 1, false, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s);
+            k_vv_kick<<<nb, 256, 0, s>>>(n_atoms, vel_dev, h->d_Fmd, types_dev, ms, dt, h->d_sums);
+            const cudaError_t ce = cudaStreamEndCapture(s, &graph);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            QNEP_CUDA_OK(h, ce);
+            const cudaError_t ci = cudaGraphInstantiate(&h->md_exec[kind], graph, 0);
+            cudaGraphDestroy(graph);
+            QNEP_CUDA_OK(h, ci);
+            h->md_exec_launches[kind] = h->launches - l0 + 2;
+            h->launches = l0;
+        }
+        QNEP_CUDA_OK(h, cudaGraphLaunch(h->md_exec[kind], s));
+        h->launches += h->md_exec_launches[kind];
+        h->ev_valid = false;
+        h->flags_pending = true;
+        h->last_stream = s;
+    }
+    if (s != caller) {
+        // hand back to the caller's stream
+        QNEP_CUDA_OK(h, cudaEventRecord(h->md_fence, s));
+        QNEP_CUDA_OK(h, cudaStreamWaitEvent(caller, h->md_fence, 0));
+        s = caller;
+        h->last_stream = caller;
     }
     if (energy_dev) { k_md_energy<<<1, 1, 0, s>>>(h->d_sums, h->model.mode, energy_dev); h->launches += 1; }
     return qnep_check(h);
@@ -736,6 +827,9 @@ int qnep_debug_copy(qnep_handle* h, int32_t which, double* dst, int64_t n)
 void qnep_destroy(qnep_handle* h)
 {
     if (!h) return;
+    drop_md_graphs(h);
+    if (h->md_stream) cudaStreamDestroy(h->md_stream);
+    if (h->md_fence) cudaEventDestroy(h->md_fence);
     free_workspace(h);
     void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_sums, h->d_flags, h->d_kvec,
                     h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,

@@ -17,6 +17,7 @@
 #define QNEP_NB 9                   // basis functions k = 0..8 (basis_r = basis_a = 8 in this version)
 #define QNEP_NRAD 5                 // n = 0..4
 #define QNEP_NDESC 25
+#define QNEP_GRAPH_MAX_ATOMS 100000   // above this the step is not launch-bound and keeps its per-stage events
 
 // Neighbour lists are WARP-TILED: the rows of the 32 atoms p = 32 w .. 32 w + 31 are interleaved in one contiguous
 // block, so a warp streams its lists sequentially (one DRAM page after the other) and every thread loads 16 bytes
@@ -144,6 +145,15 @@ struct qnep_handle {
     float* d_gtab = nullptr;         // 1-D influence tables: per axis N entries of (A_alpha) then k_alpha
     float2* d_twiddle = nullptr;     // per axis twiddles
     int tw_n = 0;
+
+    // qnep_md_run: one CUDA graph per step kind (0: lists reused, 1: rebuild), replayed while the key is unchanged
+    int md_graph_mode = 1;                 // 0 never, 1 when N <= QNEP_GRAPH_MAX_ATOMS (launch-bound sizes), 2 always
+    cudaGraphExec_t md_exec[2] = {nullptr, nullptr};
+    int64_t md_exec_launches[2] = {0, 0};
+    struct MdKey { const void *pos, *vel, *types; int64_t N; double dt; double m[QNEP_MAX_TYPES]; cudaStream_t s; uint64_t gen; } md_key = {};
+    cudaStream_t md_stream = nullptr;      // graphs run on an own stream (the legacy default stream cannot be captured), fenced by events
+    cudaEvent_t md_fence = nullptr;
+    uint64_t ws_generation = 0;            // bumped whenever workspace pointers, capacities or the geometry change
 
     // host staging (qnep_compute_host)
     double* d_hpos = nullptr; int32_t* d_htypes = nullptr; double* d_hout = nullptr; int64_t hostN = 0;

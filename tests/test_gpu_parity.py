@@ -258,6 +258,41 @@ def test_md_run_conserves_energy(torch):
     assert abs(e1[0] - e0[0]) > 1e-6            # the atoms did move
 
 
+def test_md_run_graph_replay_matches_plain_launches(torch):
+    """qnep_md_run replays one CUDA graph per step kind (lists reused / rebuild) for launch-bound sizes: the trajectory
+    must be the one the plain launches give (up to the order of fp32 atomics), device-side errors must still surface,
+    and a changed time step must not replay the old graph."""
+    w = I.config1()
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    dt = 0.1 / 10.180505
+    res = {}
+    for mode in (0, 2):
+        h = Q.from_workload(w)
+        h.set_neighbor_policy(1.0, 10)
+        h.set_md_graphs(mode)
+        pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+        vel = torch.tensor(I.maxwell_boltzmann(w), dtype=torch.float64, device="cuda")
+        l0 = h.kernel_launches()
+        e = h.md_run(pos, vel, types, w.box, w.masses, dt, 25).cpu().numpy()      # 25 steps: both step kinds, twice
+        launches = h.kernel_launches() - l0
+        e2 = h.md_run(pos, vel, types, w.box, w.masses, 0.5 * dt, 5).cpu().numpy()  # new dt: graphs must be re-captured
+        res[mode] = (pos.cpu().numpy(), e, e2, launches)
+        if mode == 2:
+            stage, n_evals = h.profile_sum()
+            assert n_evals <= 1                      # replayed steps carry no stage events (only the initial force call)
+            big = pos.clone()
+            big[0, 0] += 0.9                         # a jump beyond skin/2 must be reported from inside a replayed step
+            with pytest.raises(Q.QnepError) as ei:
+                h.md_run(big, vel, types, w.box, w.masses, dt, 3)
+            assert ei.value.code == Q.QNEP_ERR_SKIN_VIOLATED
+        h.destroy()
+    (p0, e0, e0b, l0), (p2, e2, e2b, l2) = res[0], res[2]
+    assert l0 == l2                                  # the launch claim counts replayed kernels too
+    assert np.abs(p0 - p2).max() < 1e-6
+    assert abs(e0[0] - e2[0]) / w.n_atoms < 1e-6 and abs(e0[1] - e2[1]) / w.n_atoms < 1e-6
+    assert abs(e0b[0] - e2b[0]) / w.n_atoms < 1e-6 and abs(e0b[1] - e2b[1]) / w.n_atoms < 1e-6
+
+
 # ---------------------------------------------------------------- full BASELINE sizes (configs 3 and 4)
 def test_config3_full_size(torch, oracle):
     """BASELINE configs[3] at its full size: 320 000 atoms, 3 species, PPPM 128^3."""
