@@ -158,16 +158,9 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
 // ------------------------------------------------------------------------------------------
 // asynchronous global -> shared copies (LDGSTS): a thread streams its own list rows through a small ring in
 // shared memory, so many loads are in flight per thread at no register cost.  A thread only ever reads what it
-// copied itself, so cp.async.wait_group is the only synchronisation needed.
+// copied itself, so cp.async.wait_group is the only synchronisation needed.  (Used for streams only: LDGSTS does
+// not allocate in L1, so gathers that profit from L1 hits use plain loads into register rotations instead.)
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ void cp_async4(void* sm, const void* g)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
-}
-__device__ __forceinline__ void cp_async16_ca(void* sm, const void* g)      // gathers: keep the line in L1
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");
-}
 __device__ __forceinline__ void cp_async16_cg(void* sm, const void* g)      // streams: bypass L1
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(sm)), "l"(g) : "memory");

@@ -258,6 +258,38 @@ def test_md_run_conserves_energy(torch):
     assert abs(e1[0] - e0[0]) > 1e-6            # the atoms did move
 
 
+def test_degenerate_inputs(torch, oracle):
+    """Degenerate cases of the method: a single species (T = 1), atoms with no neighbour at all inside r_c (the
+    descriptors vanish, only the network biases and the mesh electrostatics remain), a single atom, and an atom count
+    that leaves every tile ragged.  PPPM with mode 1 so that every stage runs on them."""
+    rng = np.random.Generator(np.random.PCG64(314))
+    # (a) one species, 101 atoms of the config-1 box (oxygens only)
+    w1 = I.config1(mode=1)
+    ox = np.where(w1.types == 0)[0][:101]
+    m1 = I.ModelDesc(n_types=1, n_neurons=80, mode=1)
+    wa = I.Workload("one species", np.ascontiguousarray(w1.pos[:, ox]), np.zeros(101, dtype=np.int32), w1.box, m1,
+                    I.random_params(m1, 11), w1.es)
+    _, res = gpu_eval(torch, wa)
+    assert_parity(wa, res, oracle.compute_workload(wa, use_bins=False), "T = 1, 101 atoms")
+    # (b) a dilute gas: 40 atoms in a 40 A box, nearest pair further apart than r_c = 6 A -> every list is empty
+    L = 40.0
+    grid = np.stack(np.meshgrid(*[np.arange(4)] * 3, indexing="ij")).reshape(3, -1)[:, :40] * 9.0 + 2.0
+    pos = grid + rng.uniform(-1.0, 1.0, grid.shape)
+    m2 = I.ModelDesc(n_types=2, n_neurons=30, mode=1)
+    wb = I.Workload("dilute gas", pos, (np.arange(40) % 2).astype(np.int32), np.diag([L, L, L]).ravel(), m2,
+                    I.random_params(m2, 12), I.EsDesc(method=2, alpha=0.3, grid=(32, 32, 32), order=5))
+    h, res = gpu_eval(torch, wb)
+    st = h.neighbor_stats()
+    assert st["max_list"] == 0 and st["max_radial"] == 0 and st["max_angular"] == 0
+    assert_parity(wb, res, oracle.compute_workload(wb, use_bins=False), "no neighbours")
+    # (c) a single atom: the neutralised charge is 0, so is the force; the energy is the network's bias response
+    wc = replace(wb, name="one atom", pos=np.ascontiguousarray(pos[:, :1]), types=np.zeros(1, dtype=np.int32))
+    _, res = gpu_eval(torch, wc)
+    ref = oracle.compute_workload(wc, use_bins=False)
+    assert abs(res["charges"][0]) < 1e-12 and np.abs(res["forces"]).max() < 1e-6
+    assert abs(res["energy"][0] - ref["energy"]) < 1e-5
+
+
 def test_md_run_graph_replay_matches_plain_launches(torch):
     """qnep_md_run replays one CUDA graph per step kind (lists reused / rebuild) for launch-bound sizes: the trajectory
     must be the one the plain launches give (up to the order of fp32 atomics), device-side errors must still surface,
