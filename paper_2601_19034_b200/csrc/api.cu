@@ -832,7 +832,7 @@ void qnep_destroy(qnep_handle* h)
     if (h->md_fence) cudaEventDestroy(h->md_fence);
     free_workspace(h);
     void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_sums, h->d_flags, h->d_kvec,
-                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
+                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_half, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
                     h->d_htypes, h->d_hout};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (h->h_flags) cudaFreeHost(h->h_flags);

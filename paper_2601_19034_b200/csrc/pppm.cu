@@ -194,6 +194,35 @@ k_fft_z_fwd(const float* __restrict__ rho, float2* __restrict__ out, const float
         for (int k1 = 0; k1 < R2; ++k1) out[base + (u + S::TPL * d) + R1 * k1] = v[d * R2 + k1];
 }
 
+// ---- forward pass along z, half spectrum: the mesh is real, so S(-k) = conj S(k) and only kz = 0 .. N/2 is kept.
+// Half arrays are [x][y][NH] with NH = N/2 + LINES: slots 0 .. N/2 hold kz, the rest of the last tile stays zero.
+template <int R1, int R2>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+k_fft_z_fwd_half(const float* __restrict__ rho, float2* __restrict__ out, const float2* __restrict__ twg)
+{
+    using S = Split<R1, R2>;
+    constexpr int NH = S::N / 2 + LINES;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * S::LP;
+    load_twiddles(tw, twg, S::N);
+    __syncthreads();
+    const int u = threadIdx.x % S::TPL, b = threadIdx.x / S::TPL;
+    const int64_t line = (int64_t)blockIdx.x * LINES + b;
+    float2 v[S::E];
+#pragma unroll
+    for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+        for (int m = 0; m < R1; ++m) v[d * R1 + m] = make_float2(rho[line * S::N + (u + S::TPL * d) + R2 * m], 0.f);
+    line_fft<R1, R2, -1>(v, smem + b * S::LP, u, tw);
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) {
+            const int kz = (u + S::TPL * d) + R1 * k1;
+            if (kz <= S::N / 2) out[line * NH + kz] = v[d * R2 + k1];
+        }
+}
+
 // ---- in-place pass along a strided axis (y): grid.y selects the mesh --------------------------------
 template <int R1, int R2, int SIGN>
 __global__ void __launch_bounds__(Split<R1, R2>::THREADS)
@@ -327,6 +356,137 @@ k_fft_x_fused(int n0, int n1, int n2, float2* __restrict__ M1 /* in: S after the
             }
         }
     }
+}
+
+// ---- 3'. fused pass along x on the half spectrum ----------------------------------------------------
+// Input: half array H (kz = 0 .. N2/2) after the z and y passes.  For every stored line (ky, kz) the kernel writes the
+// inverse-x transforms of M1 and M2 at (ky, kz) and, for 0 < kz < N2/2, at the mirror line (-ky, -kz), which is not
+// stored: with phi(-k) = conj phi(k), k_d odd and the identity  IDFT[conj a(-k)] = conj IDFT[a(k)]  the mirror lines are
+//     M1(x; -ky, -kz) = conj IDFT_x[(1 + kd_x) phi],     M2(x; -ky, -kz) = conj IDFT_x[(kd_z + i kd_y) phi],
+// with kd_y, kd_z of the STORED line.  Energy and virial sums weigh these lines twice.  One forward and four inverse
+// line transforms per stored line instead of one and two per line of the full spectrum.
+template <int R1, int R2, bool VIRIAL>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS, Split<R1, R2>::THREADS >= 256 ? 3 : 1)
+k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2* __restrict__ M1, float2* __restrict__ M2,
+                   const float2* __restrict__ twg, const float* __restrict__ tabA, const float* __restrict__ tabK,
+                   const float* __restrict__ tabKd, float c0 /* 2 pi / Omega */, float inv4a2, double* __restrict__ sums)
+{
+    using S = Split<R1, R2>;
+    using SI = Split<R2, R1>;
+    constexpr int LPMAX = S::LP > SI::LP ? S::LP : SI::LP;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * LPMAX;
+    float* tA = reinterpret_cast<float*>(tw + S::N);
+    float* tK = tA + S::N;
+    float* tKd = tK + S::N;
+    float2* sphi = reinterpret_cast<float2*>(tKd + S::N) + threadIdx.x;     // phi(kx) of this thread: sphi[e * THREADS]
+    __shared__ double sh_red[32];
+    load_twiddles(tw, twg, S::N);
+    for (int i = threadIdx.x; i < S::N; i += blockDim.x) { tA[i] = tabA[i]; tK[i] = tabK[i]; tKd[i] = tabKd[i]; }
+    __syncthreads();
+    const int NH = n2 / 2 + LINES;
+    const int b = threadIdx.x % LINES, u = threadIdx.x / LINES;
+    const int zc = NH / LINES;
+    const int iy = (int)(blockIdx.x / zc), kz = (int)(blockIdx.x % zc) * LINES + b;
+    const bool valid = kz <= n2 / 2;
+    const bool mirrored = kz > 0 && kz < n2 / 2;
+    const int64_t hstride = (int64_t)n1 * NH, fstride = (int64_t)n1 * n2;
+    float2 v[S::E];
+    {
+        const float2* p = H + (int64_t)iy * NH + kz;
+#pragma unroll
+        for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+            for (int m = 0; m < R1; ++m) v[d * R1 + m] = p[((u + S::TPL * d) + R2 * m) * hstride];
+    }
+    line_fft<R1, R2, -1>(v, smem + b * S::LP, u, tw);
+    // v[d * R2 + k1] = S(kx = (u + TPL d) + R1 k1, ky, kz)
+    const int kzc = valid ? kz : 0;
+    const float ky = tabK[FFT_MAXN + iy], kzv = tabK[2 * FFT_MAXN + kzc];
+    const float kdy = tabKd[FFT_MAXN + iy], kdz = tabKd[2 * FFT_MAXN + kzc];
+    const float Ayz = c0 * tabA[FFT_MAXN + iy] * tabA[2 * FFT_MAXN + kzc];
+    const float kyz2 = ky * ky + kzv * kzv;
+    const float wgt = !valid ? 0.f : (mirrored ? 2.f : 1.f);
+    float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) {
+            const int ix = (u + S::TPL * d) + R1 * k1;
+            const float kx = tK[ix];
+            const float k2 = kx * kx + kyz2;
+            const float2 sv = v[d * R2 + k1];
+            float G = 0.f;
+            if (k2 > 0.f) G = __fdividef(Ayz * tA[ix], k2);
+            sphi[(d * R2 + k1) * S::THREADS] = make_float2(G * sv.x, G * sv.y);
+            const float e = wgt * G * (sv.x * sv.x + sv.y * sv.y);
+            acc[0] += e;
+            if (VIRIAL && k2 > 0.f) {
+                const float bf = 2.f * inv4a2 + __fdividef(2.f, k2);
+                acc[1] += e * (1.f - bf * kx * kx);
+                acc[2] += e * (-bf * kx * ky);
+                acc[3] += e * (-bf * kx * kzv);
+                acc[4] += e * (1.f - bf * ky * ky);
+                acc[5] += e * (-bf * ky * kzv);
+                acc[6] += e * (1.f - bf * kzv * kzv);
+            }
+        }
+    // the four inverse transforms along x (swapped split <R2, R1>: its stage-1 layout is the layout we hold)
+    const int iym = (n1 - iy) % n1, kzm = n2 - kz;
+#pragma unroll 1
+    for (int which = 0; which < 4; ++which) {
+#pragma unroll
+        for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+            for (int k1 = 0; k1 < R2; ++k1) {
+                const int ix = (u + S::TPL * d) + R1 * k1;
+                const float kdx = tKd[ix];
+                const float2 ph = sphi[(d * R2 + k1) * S::THREADS];
+                float2 o;
+                if (which == 0) o = make_float2((1.f - kdx) * ph.x, (1.f - kdx) * ph.y);                     // M1 at (ky, kz)
+                else if (which == 1) o = make_float2(-kdz * ph.x - kdy * ph.y, -kdz * ph.y + kdy * ph.x);    // M2 at (ky, kz)
+                else if (which == 2) o = make_float2((1.f + kdx) * ph.x, (1.f + kdx) * ph.y);                // conj M1 at (-ky, -kz)
+                else o = make_float2(kdz * ph.x - kdy * ph.y, kdz * ph.y + kdy * ph.x);                      // conj M2 at (-ky, -kz)
+                v[d * R2 + k1] = o;
+            }
+        line_fft<R2, R1, +1>(v, smem + b * SI::LP, u, tw);
+        float2* dst = (which & 1) ? M2 : M1;
+        const bool own = which < 2;
+        if (own ? valid : mirrored) {
+            float2* p = dst + (own ? (int64_t)iy * n2 + kz : (int64_t)iym * n2 + kzm);
+            const float sgn = own ? 1.f : -1.f;
+#pragma unroll
+            for (int d = 0; d < SI::D2; ++d)
+#pragma unroll
+                for (int k1 = 0; k1 < R1; ++k1) {
+                    const float2 o = v[d * R1 + k1];
+                    p[((u + SI::TPL * d) + R2 * k1) * fstride] = make_float2(o.x, sgn * o.y);
+                }
+        }
+    }
+    // U^k = K sum G |S|^2 (Eq. 34), W^k = K sum G |S|^2 B (Eq. 22): fp32 per thread, fp64 across threads
+    const int slot[7] = {SUM_U_K, SUM_W0 + 0, SUM_W0 + 1, SUM_W0 + 2, SUM_W0 + 4, SUM_W0 + 5, SUM_W0 + 8};
+    const int mirror[7] = {-1, -1, SUM_W0 + 3, SUM_W0 + 6, -1, SUM_W0 + 7, -1};
+#pragma unroll
+    for (int a = 0; a < (VIRIAL ? 7 : 1); ++a) {
+        double x = (double)acc[a];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) sh_red[threadIdx.x >> 5] = x;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            double r = threadIdx.x < (blockDim.x >> 5) ? sh_red[threadIdx.x] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+            if (threadIdx.x == 0) {
+                r *= QNEP_K_COULOMB;
+                atomicAdd(&sums[slot[a]], r);
+                if (mirror[a] >= 0) atomicAdd(&sums[mirror[a]], r);
+            }
+        }
+    }
+    (void)n0;
 }
 
 // ---- last inverse pass along z: M1, M2 -> interleaved real fields (Phi, E_x, E_y, E_z) -------------------
@@ -490,6 +650,16 @@ int qnep_setup_pppm(qnep_handle* h)
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_field, sizeof(float4) * ng));
         h->ngrid = ng;
     }
+    {
+        // half-spectrum array of the forward transform, [x][y][N2/2 + LINES]; the padding of the last tile stays zero
+        const int64_t nh = grid[2] >= 2 * LINES ? (int64_t)grid[0] * grid[1] * (grid[2] / 2 + LINES) : 0;
+        if (nh != h->nhalf) {
+            cudaFree(h->d_half); h->d_half = nullptr;
+            if (nh) QNEP_CUDA_OK(h, cudaMalloc(&h->d_half, sizeof(float2) * nh));
+            h->nhalf = nh;
+        }
+        if (nh) QNEP_CUDA_OK(h, cudaMemset(h->d_half, 0, sizeof(float2) * nh));
+    }
     if (!h->d_twiddle) QNEP_CUDA_OK(h, cudaMalloc(&h->d_twiddle, sizeof(float2) * 3 * FFT_MAXN));
     if (!h->d_gtab) QNEP_CUDA_OK(h, cudaMalloc(&h->d_gtab, sizeof(float) * 9 * FFT_MAXN));
     std::vector<float2> tw(3 * FFT_MAXN, make_float2(0.f, 0.f));
@@ -532,6 +702,43 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
     // 1. spread
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mesh, 0, sizeof(float) * h->ngrid, s));
     k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_mesh);
+    const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    if (h->d_half) {
+        // 2.-3. forward transform on the half spectrum (the mesh is real): z and y passes on [x][y][N2/2 + LINES],
+        //       the fused x pass restores the full spectrum of M1, M2 on the way out
+        const int NH = n2 / 2 + LINES;
+        with_split(n2, [&](auto r1, auto r2) {
+            constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+            using S = Split<R1, R2>;
+            const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+            note(allow_smem(k_fft_z_fwd_half<R1, R2>, smem));
+            k_fft_z_fwd_half<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_mesh, h->d_half, tw2);
+        });
+        with_split(n1, [&](auto r1, auto r2) {
+            constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+            using S = Split<R1, R2>;
+            const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+            note(allow_smem(k_fft_strided<R1, R2, -1>, smem));
+            k_fft_strided<R1, R2, -1><<<dim3((unsigned)((int64_t)n0 * NH / LINES), 1), S::THREADS, smem, s>>>(1, n0, n1, NH, h->d_half, h->d_half, tw1);
+        });
+        with_split(n0, [&](auto r1, auto r2) {
+            constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+            using S = Split<R1, R2>;
+            using SI = Split<R2, R1>;
+            const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 3 * S::N +
+                                sizeof(float2) * S::E * S::THREADS;
+            const unsigned nt = (unsigned)((int64_t)n1 * NH / LINES);
+            if (virial) {
+                note(allow_smem(k_fft_x_fused_half<R1, R2, true>, smem));
+                k_fft_x_fused_half<R1, R2, true><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_half, h->d_cm1, h->d_cm2, tw0, h->d_gtab,
+                                                                             h->d_gtab + 3 * FFT_MAXN, h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
+            } else {
+                note(allow_smem(k_fft_x_fused_half<R1, R2, false>, smem));
+                k_fft_x_fused_half<R1, R2, false><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_half, h->d_cm1, h->d_cm2, tw0, h->d_gtab,
+                                                                              h->d_gtab + 3 * FFT_MAXN, h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
+            }
+        });
+    } else {
     // 2. forward z (real -> complex), forward y
     with_split(n2, [&](auto r1, auto r2) {
         constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
@@ -553,7 +760,6 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
         using S = Split<R1, R2>;
         using SI = Split<R2, R1>;
         const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 3 * S::N;
-        const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
         const unsigned nt = (unsigned)((int64_t)n1 * n2 / LINES);
         if (virial) {
             note(allow_smem(k_fft_x_fused<R1, R2, true>, smem));
@@ -565,6 +771,7 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
                                                                      h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
         }
     });
+    }
     // 4. inverse y on both meshes, inverse z -> interleaved real fields
     with_split(n1, [&](auto r1, auto r2) {
         constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;

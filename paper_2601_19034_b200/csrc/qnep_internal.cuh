@@ -138,7 +138,9 @@ struct qnep_handle {
     double2* d_S = nullptr;          // [nk]
     // PPPM
     int64_t ngrid = 0;
+    int64_t nhalf = 0;               // elements of d_half
     float* d_mesh = nullptr;         // [Nx][Ny][Nz] real charge mesh
+    float2* d_half = nullptr;        // half-spectrum array of the forward transform [x][y][N2/2 + 16] (N2 >= 32)
     float2* d_cm1 = nullptr;         // complex meshes
     float2* d_cm2 = nullptr;
     float4* d_field = nullptr;       // [Nx][Ny][Nz] (Phi, E_x, E_y, E_z)
