@@ -418,7 +418,11 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
             const float2 sv = v[d * R2 + k1];
             float G = 0.f;
             if (k2 > 0.f) G = __fdividef(Ayz * tA[ix], k2);
-            sphi[(d * R2 + k1) * S::THREADS] = make_float2(G * sv.x, G * sv.y);
+            // phi = G S stays in the registers, kd_x phi is parked in shared memory for the second inverse transform
+            const float2 ph = make_float2(G * sv.x, G * sv.y);
+            const float kdx = tKd[ix];
+            v[d * R2 + k1] = ph;
+            sphi[(d * R2 + k1) * S::THREADS] = make_float2(kdx * ph.x, kdx * ph.y);
             const float e = wgt * G * (sv.x * sv.x + sv.y * sv.y);
             acc[0] += e;
             if (VIRIAL && k2 > 0.f) {
@@ -431,39 +435,41 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
                 acc[6] += e * (1.f - bf * kzv * kzv);
             }
         }
-    // the four inverse transforms along x (swapped split <R2, R1>: its stage-1 layout is the layout we hold)
+    // Two inverse transforms along x give all four output lines, because kd_y and kd_z are constants of the line:
+    //   A = IDFT_x[phi], B = IDFT_x[kd_x phi]:   M1 = A - B,  M2 = (-kd_z + i kd_y) A   at (ky, kz),
+    //   conj(A + B)  and  conj((kd_z + i kd_y) A)                                         at (-ky, -kz).
+    // (swapped split <R2, R1>: its stage-1 layout is the layout we hold)
     const int iym = (n1 - iy) % n1, kzm = n2 - kz;
-#pragma unroll 1
-    for (int which = 0; which < 4; ++which) {
+    float2* own1 = M1 + (int64_t)iy * n2 + kz;
+    float2* own2 = M2 + (int64_t)iy * n2 + kz;
+    float2* mir1 = M1 + (int64_t)iym * n2 + kzm;
+    float2* mir2 = M2 + (int64_t)iym * n2 + kzm;
+    line_fft<R2, R1, +1>(v, smem + b * SI::LP, u, tw);          // v = A
 #pragma unroll
-        for (int d = 0; d < S::D2; ++d)
+    for (int d = 0; d < SI::D2; ++d)
 #pragma unroll
-            for (int k1 = 0; k1 < R2; ++k1) {
-                const int ix = (u + S::TPL * d) + R1 * k1;
-                const float kdx = tKd[ix];
-                const float2 ph = sphi[(d * R2 + k1) * S::THREADS];
-                float2 o;
-                if (which == 0) o = make_float2((1.f - kdx) * ph.x, (1.f - kdx) * ph.y);                     // M1 at (ky, kz)
-                else if (which == 1) o = make_float2(-kdz * ph.x - kdy * ph.y, -kdz * ph.y + kdy * ph.x);    // M2 at (ky, kz)
-                else if (which == 2) o = make_float2((1.f + kdx) * ph.x, (1.f + kdx) * ph.y);                // conj M1 at (-ky, -kz)
-                else o = make_float2(kdz * ph.x - kdy * ph.y, kdz * ph.y + kdy * ph.x);                      // conj M2 at (-ky, -kz)
-                v[d * R2 + k1] = o;
-            }
-        line_fft<R2, R1, +1>(v, smem + b * SI::LP, u, tw);
-        float2* dst = (which & 1) ? M2 : M1;
-        const bool own = which < 2;
-        if (own ? valid : mirrored) {
-            float2* p = dst + (own ? (int64_t)iy * n2 + kz : (int64_t)iym * n2 + kzm);
-            const float sgn = own ? 1.f : -1.f;
-#pragma unroll
-            for (int d = 0; d < SI::D2; ++d)
-#pragma unroll
-                for (int k1 = 0; k1 < R1; ++k1) {
-                    const float2 o = v[d * R1 + k1];
-                    p[((u + SI::TPL * d) + R2 * k1) * fstride] = make_float2(o.x, sgn * o.y);
-                }
+        for (int k1 = 0; k1 < R1; ++k1) {
+            const int64_t off = (int64_t)((u + SI::TPL * d) + R2 * k1) * fstride;
+            const float2 A = v[d * R1 + k1];
+            if (valid) own2[off] = make_float2(-kdz * A.x - kdy * A.y, -kdz * A.y + kdy * A.x);
+            if (mirrored) mir2[off] = make_float2(kdz * A.x - kdy * A.y, -(kdz * A.y + kdy * A.x));
+            // swap: A goes to shared memory, kd_x phi comes back for the second transform.  The element index differs
+            // between the two layouts, but a slot is only a parking place of this thread: any one-to-one order works.
+            float2* slot = sphi + (d * R1 + k1) * S::THREADS;
+            const float2 t = *slot;
+            *slot = A;
+            v[d * R1 + k1] = t;
         }
-    }
+    line_fft<R2, R1, +1>(v, smem + b * SI::LP, u, tw);          // v = B
+#pragma unroll
+    for (int d = 0; d < SI::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R1; ++k1) {
+            const int64_t off = (int64_t)((u + SI::TPL * d) + R2 * k1) * fstride;
+            const float2 A = sphi[(d * R1 + k1) * S::THREADS], B = v[d * R1 + k1];
+            if (valid) own1[off] = make_float2(A.x - B.x, A.y - B.y);
+            if (mirrored) mir1[off] = make_float2(A.x + B.x, -(A.y + B.y));
+        }
     // U^k = K sum G |S|^2 (Eq. 34), W^k = K sum G |S|^2 B (Eq. 22): fp32 per thread, fp64 across threads
     const int slot[7] = {SUM_U_K, SUM_W0 + 0, SUM_W0 + 1, SUM_W0 + 2, SUM_W0 + 4, SUM_W0 + 5, SUM_W0 + 8};
     const int mirror[7] = {-1, -1, SUM_W0 + 3, SUM_W0 + 6, -1, SUM_W0 + 7, -1};
