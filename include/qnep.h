@@ -154,13 +154,20 @@ int qnep_compute_host(qnep_handle *h, int64_t n_atoms, const double *pos_host, c
  *   pos_dev, vel_dev [3][N] float64, updated in place; mass_host[n_types] in amu;
  *   dt in natural units (Angstrom * sqrt(amu/eV); 1 fs = 1/10.180505);
  *   energy_dev[2]: potential and kinetic energy after the last step.
- * The first call computes the initial forces; forces are kept in the handle between calls.
+ * The first call computes the initial forces; forces are kept in the handle between calls, so consecutive calls
+ * continue one trajectory (call qnep_md_reset before starting another one from different positions).
  * The neighbour policy set by qnep_set_neighbor_policy applies.  Synchronises at the end and reports
  * device-side errors (SKIN_VIOLATED, NEIGHBOR_OVERFLOW) of the run.
  */
 int qnep_md_run(qnep_handle *h, int64_t n_atoms, double *pos_dev, double *vel_dev, const int32_t *types_dev,
                 const double box[9], const double *mass_host, double dt, int32_t n_steps,
                 double *energy_dev, void *cuda_stream);
+
+/*
+ * Tell the handle that the caller changed positions or velocities behind qnep_md_run's back (a restart from a stored
+ * state): the forces kept from the previous call are dropped and the next evaluation rebuilds the neighbour list.
+ */
+int qnep_md_reset(qnep_handle *h);
 
 /*
  * CUDA graphs inside qnep_md_run: a step is ~25 kernel launches, which bounds small systems (a 3000-atom step is

@@ -35,7 +35,7 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
-               "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_set_md_graphs", "qnep_check", "qnep_get_timings",
+               "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_md_reset", "qnep_set_md_graphs", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
                "qnep_fma_peak",
                "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
@@ -87,6 +87,8 @@ def load_library():
     lib.qnep_md_run.restype = C.c_int
     lib.qnep_md_run.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i32, vp, vp]
     lib.qnep_check.restype = C.c_int
+    lib.qnep_md_reset.restype = C.c_int
+    lib.qnep_md_reset.argtypes = [vp]
     lib.qnep_set_md_graphs.restype = C.c_int
     lib.qnep_set_md_graphs.argtypes = [vp, i32]
     lib.qnep_check.argtypes = [vp]
@@ -263,6 +265,10 @@ class QNEP:
 
     def kernel_launches(self) -> int:
         return int(self._lib.qnep_kernel_launches(self._h))
+
+    def md_reset(self):
+        """Positions / velocities were changed outside md_run: drop the kept forces, rebuild the lists next time."""
+        self._ok(self._lib.qnep_md_reset(self._h))
 
     def set_md_graphs(self, mode: int):
         """0 never, 1 (default) for n_atoms <= 100000, 2 always: CUDA graphs for the steps of md_run."""

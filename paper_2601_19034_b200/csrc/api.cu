@@ -572,6 +572,14 @@ int qnep_compute(qnep_handle* h, int64_t n_atoms, const double* pos_dev, const i
     return run_pipeline(h, n_atoms, pos_dev, types_dev, want, energy_dev, forces_dev, virial_dev, charges_dev, bec_dev, s);
 }
 
+int qnep_md_reset(qnep_handle* h)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    h->md_have_forces = false;
+    h->force_rebuild = true;
+    return QNEP_OK;
+}
+
 int qnep_set_md_graphs(qnep_handle* h, int32_t mode)
 {
     if (!h) return QNEP_ERR_INVALID_ARG;

@@ -290,6 +290,26 @@ def test_degenerate_inputs(torch, oracle):
     assert abs(res["energy"][0] - ref["energy"]) < 1e-5
 
 
+def test_md_reset_starts_a_new_trajectory(torch):
+    """Consecutive md_run calls continue one trajectory (kept forces, list age); after qnep_md_reset a run from the
+    initial state must reproduce the first one, and without it the stale state is detected (the atoms 'jumped')."""
+    w = I.config1()
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(1.0, 10)
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    pos0 = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    vel0 = torch.tensor(I.maxwell_boltzmann(w), dtype=torch.float64, device="cuda")
+    dt = 0.1 / 10.180505
+    p1, v1 = pos0.clone(), vel0.clone()
+    e1 = h.md_run(p1, v1, types, w.box, w.masses, dt, 13).cpu().numpy()
+    assert float((p1 - pos0).abs().max()) > 0.01
+    h.md_reset()
+    p2, v2 = pos0.clone(), vel0.clone()
+    e2 = h.md_run(p2, v2, types, w.box, w.masses, dt, 13).cpu().numpy()
+    assert float((p1 - p2).abs().max()) < 1e-6 and abs(e1[0] - e2[0]) / w.n_atoms < 1e-6
+    h.destroy()
+
+
 def test_md_run_graph_replay_matches_plain_launches(torch):
     """qnep_md_run replays one CUDA graph per step kind (lists reused / rebuild) for launch-bound sizes: the trajectory
     must be the one the plain launches give (up to the order of fp32 atomics), device-side errors must still surface,
