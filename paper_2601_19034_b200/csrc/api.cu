@@ -82,14 +82,14 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
     const bool box_changed = std::memcmp(box, h->box, sizeof(double) * 9) != 0;
     const double vol = g.L[0] * g.L[1] * g.L[2];
     const double rho = (double)N / vol;
-    auto cap_for = [&](double rc_, int user) {
+    auto cap_for = [&](double rc_, int user, int grown) {
         if (user > 0) return (user + 3) / 4 * 4;          // packed-word lists hold four slots per int4
         const double expect = 4.0 / 3.0 * M_PI * rc_ * rc_ * rc_ * rho;
-        return ((int)(expect * 1.5) + 24 + 3) / 4 * 4;
+        return std::max(((int)(expect * 1.5) + 24 + 3) / 4 * 4, grown);
     };
-    const int capR = cap_for(h->model.rc_r + h->skin, h->user_capR);     // skin list
-    const int capLR = cap_for(h->model.rc_r, h->user_capLR);             // live radial list
-    const int capLA = cap_for(h->model.rc_a, h->user_capA);              // live angular pairs
+    const int capR = cap_for(h->model.rc_r + h->skin, h->user_capR, h->grown_capR);     // skin list
+    const int capLR = cap_for(h->model.rc_r, h->user_capLR, h->grown_capLR);            // live radial list
+    const int capLA = cap_for(h->model.rc_a, h->user_capA, h->grown_capA);              // live angular pairs
     const int T = h->model.n_types;
     const int nkeys = T * g.ncells;
     const bool realloc_atoms = N != h->N || capR != h->capR || capLR != h->capLR || capLA != h->capLA;
@@ -173,16 +173,19 @@ int consume_flags(qnep_handle* h)
                  ", live radial " + std::to_string(f[FLAG_MAX_LR]) + "/" + std::to_string(h->capLR) + ", live angular " +
                  std::to_string(f[FLAG_MAX_LA]) + "/" + std::to_string(h->capLA) + "); capacity grown, call again";
         auto grow = [](int cap, int seen) { return std::max(cap, (seen * 5 / 4 + 8 + 3) / 4 * 4); };
+        // the grown values are lower bounds on top of the automatic estimate (a stale one can only be too generous);
+        // an explicit capacity that proved too small is dropped
         if (f[FLAG_MAX_NR] > h->capR) {
             // the truncated skin list hid the true live counts: scale them from the skin-list count by the volume ratios
-            h->user_capR = grow(h->capR, f[FLAG_MAX_NR]);
+            h->grown_capR = grow(h->capR, f[FLAG_MAX_NR]);
             const double rcs = h->model.rc_r + h->skin;
             const double fr = std::pow(h->model.rc_r / rcs, 3.0), fa = std::pow(h->model.rc_a / rcs, 3.0);
-            h->user_capLR = grow(h->capLR, (int)(f[FLAG_MAX_NR] * fr * 1.1) + 1);
-            h->user_capA = grow(h->capLA, (int)(f[FLAG_MAX_NR] * fa * 1.3) + 1);
+            h->grown_capLR = grow(h->capLR, (int)(f[FLAG_MAX_NR] * fr * 1.1) + 1);
+            h->grown_capA = grow(h->capLA, (int)(f[FLAG_MAX_NR] * fa * 1.3) + 1);
+            h->user_capR = h->user_capLR = h->user_capA = 0;
         }
-        if (f[FLAG_MAX_LR] > h->capLR) h->user_capLR = grow(h->capLR, f[FLAG_MAX_LR]);
-        if (f[FLAG_MAX_LA] > h->capLA) h->user_capA = grow(h->capLA, f[FLAG_MAX_LA]);
+        if (f[FLAG_MAX_LR] > h->capLR) { h->grown_capLR = grow(h->capLR, f[FLAG_MAX_LR]); h->user_capLR = 0; }
+        if (f[FLAG_MAX_LA] > h->capLA) { h->grown_capA = grow(h->capLA, f[FLAG_MAX_LA]); h->user_capA = 0; }
         h->force_rebuild = true;
         return QNEP_ERR_NEIGHBOR_OVERFLOW;
     }

@@ -74,7 +74,8 @@ struct qnep_handle {
     double skin = 0.0;
     int rebuild_every = 0;
     int calls_since_build = -1;      // -1: never built
-    int user_capR = 0, user_capLR = 0, user_capA = 0;   // capacity overrides: skin list, live radial, live angular (0: automatic)
+    int user_capR = 0, user_capLR = 0, user_capA = 0;   // explicit capacities (qnep_set_neighbor_capacity): skin list, live radial, live angular (0: automatic)
+    int grown_capR = 0, grown_capLR = 0, grown_capA = 0;   // lower bounds learnt from an overflow; the automatic estimate still applies on top
     bool force_rebuild = true;
 
     // workspace (sorted atom order p unless noted)

@@ -290,6 +290,44 @@ def test_degenerate_inputs(torch, oracle):
     assert abs(res["energy"][0] - ref["energy"]) < 1e-5
 
 
+def test_one_handle_many_shapes(torch, oracle):
+    """One handle is reused while the atom count, the box and the electrostatics selector change between calls: the
+    workspace, the PPPM tables and the captured MD graphs must follow (no stale pointer, no stale geometry)."""
+    w = I.config1(mode=2)
+    h = Q.from_workload(w)
+    for n in (3000, 1200, 3000):
+        sub = replace(w, pos=np.ascontiguousarray(w.pos[:, :n]), types=np.ascontiguousarray(w.types[:n]))
+        _, res = gpu_eval(torch, sub, handle=h)
+        assert_parity(sub, res, oracle.compute_workload(sub), f"reused handle, N = {n}")
+    # a uniformly scaled box (positions scale with it): new cell grid, new influence function
+    big = replace(w, pos=w.pos * 1.1, box=w.box * 1.1)
+    _, res = gpu_eval(torch, big, handle=h)
+    assert_parity(big, res, oracle.compute_workload(big), "reused handle, box x 1.1")
+    # an MD run (graphs captured), then another atom count through the same handle, then MD again
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    vel = torch.tensor(I.maxwell_boltzmann(w), dtype=torch.float64, device="cuda")
+    h.set_neighbor_policy(1.0, 10)
+    h.md_reset()
+    h.md_run(pos, vel, types, w.box, w.masses, 0.1 / 10.180505, 12)
+    sub = replace(w, pos=np.ascontiguousarray(w.pos[:, :999]), types=np.ascontiguousarray(w.types[:999]))
+    _, res = gpu_eval(torch, sub, handle=h)
+    assert_parity(sub, res, oracle.compute_workload(sub), "reused handle after MD, N = 999")
+    h.md_reset()
+    e = h.md_run(pos, vel, types, w.box, w.masses, 0.1 / 10.180505, 12).cpu().numpy()
+    assert np.isfinite(e).all()
+    # the selector: PPPM -> Ewald on the same handle
+    w0 = I.config3(n_cells=8, grid=32, method=2)
+    h2 = Q.from_workload(w0)
+    _, r_p = gpu_eval(torch, w0, handle=h2)
+    w0e = I.config3(n_cells=8, grid=32, method=1)
+    h2.set_electrostatics(w0e.es)
+    _, r_e = gpu_eval(torch, w0e, handle=h2)
+    assert_parity(w0e, r_e, oracle.compute_workload(w0e), "selector switched to Ewald")
+    assert rel_rms(r_p["forces"], r_e["forces"]) < 2e-4          # PPPM and Ewald agree to PPPM's own accuracy
+    h.destroy(); h2.destroy()
+
+
 def test_md_reset_starts_a_new_trajectory(torch):
     """Consecutive md_run calls continue one trajectory (kept forces, list age); after qnep_md_reset a run from the
     initial state must reproduce the first one, and without it the stale state is detected (the atoms 'jumped')."""
