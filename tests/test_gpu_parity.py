@@ -290,6 +290,40 @@ def test_degenerate_inputs(torch, oracle):
     assert abs(res["energy"][0] - ref["energy"]) < 1e-5
 
 
+def test_orthorhombic_box_and_anisotropic_mesh(torch, oracle):
+    """All BASELINE configs are cubic; the path itself is orthorhombic: three different box edges, three different mesh
+    sizes (every FFT pass gets its own length and split), both electrostatics methods, mode 1."""
+    w = I.config1(mode=1)
+    scale = np.array([1.0, 1.37, 0.81])
+    pos = w.pos * scale[:, None]
+    box = np.diag(np.diag(w.box.reshape(3, 3)) * scale).ravel()
+    for es, label in ((I.EsDesc(method=2, alpha=0.3, grid=(32, 64, 16), order=5), "PPPM 32x64x16"),
+                      (I.EsDesc(method=2, alpha=0.3, grid=(64, 32, 128), order=5), "PPPM 64x32x128"),
+                      (I.EsDesc(method=1, alpha=0.3, ewald_nmax2=36), "Ewald")):
+        wo = replace(w, name="orthorhombic " + label, pos=pos, box=box, es=es)
+        _, res = gpu_eval(torch, wo)
+        assert_parity(wo, res, oracle.compute_workload(wo), wo.name)
+
+
+def test_output_selection(torch, oracle):
+    """`want` selects the outputs; a buffer that is not wanted is not touched and may be absent."""
+    w = I.config1(mode=2)
+    ref = oracle.compute_workload(w)
+    h = Q.from_workload(w)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    out = h.compute(pos, types, w.box, want=Q.WANT_ENERGY)
+    assert set(out) == {"energy"} and abs(float(out["energy"][0]) - ref["energy"]) / w.n_atoms <= TOL_E_PER_ATOM
+    out = h.compute(pos, types, w.box, want=Q.WANT_CHARGES)
+    assert set(out) == {"charges"} and np.abs(out["charges"].cpu().numpy() - ref["charges"]).max() <= TOL_Q
+    out = h.compute(pos, types, w.box, want=Q.WANT_FORCES)
+    assert set(out) == {"forces"} and rel_rms(out["forces"].cpu().numpy(), ref["forces"]) <= TOL_F_RELRMS
+    out = h.compute(pos, types, w.box, want=Q.WANT_VIRIAL)
+    dw = np.abs(out["virial"].cpu().numpy().reshape(3, 3) - ref["virial"]).max() / np.abs(ref["virial"]).max()
+    assert set(out) == {"virial"} and dw <= TOL_W_REL
+    h.destroy()
+
+
 def test_one_handle_many_shapes(torch, oracle):
     """One handle is reused while the atom count, the box and the electrostatics selector change between calls: the
     workspace, the PPPM tables and the captured MD graphs must follow (no stale pointer, no stale geometry)."""
