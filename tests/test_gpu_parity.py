@@ -235,6 +235,13 @@ def test_translation_and_permutation_on_gpu(torch):
     # PPPM is translation invariant only to its own accuracy (P9)
     assert rel_rms(b["forces"], a["forces"]) < 1e-4
     assert abs(a["energy"][0] - b["energy"][0]) / w.n_atoms < 1e-5
+    # unwrapped coordinates: every atom moved by its own lattice vector (up to +-9 box lengths) is the same structure
+    rng = np.random.Generator(np.random.PCG64(3))
+    L = np.diag(w.box.reshape(3, 3))
+    images = replace(w, pos=w.pos + rng.integers(-9, 10, size=w.pos.shape) * L[:, None])
+    _, d = gpu_eval(torch, images)
+    assert rel_rms(d["forces"], a["forces"]) < 2e-5 and np.abs(d["charges"] - a["charges"]).max() < 2e-6
+    assert abs(a["energy"][0] - d["energy"][0]) / w.n_atoms < 1e-6
     perm = np.random.Generator(np.random.PCG64(2)).permutation(w.n_atoms)
     _, c = gpu_eval(torch, replace(w, pos=np.ascontiguousarray(w.pos[:, perm]), types=w.types[perm].copy()))
     assert rel_rms(c["forces"], a["forces"][:, perm]) < 2e-5
