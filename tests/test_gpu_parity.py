@@ -170,6 +170,12 @@ def test_bec_parity_and_sum_rule(torch, oracle):
     ref1 = oracle.compute_workload(w1, want_bec=True)
     h, res1 = gpu_eval(torch, w1, want=Q.WANT_ALL | Q.WANT_BEC)
     assert rel_rms(res1["bec"], ref1["bec"]) < 1e-4
+    # four species, 26 112 atoms (several hundred blocks, type boundaries inside warps), lists reused with a skin
+    w2 = I.config2()
+    ref2 = oracle.compute_workload(w2, want_bec=True)
+    h, res2 = gpu_eval(torch, w2, want=Q.WANT_ALL | Q.WANT_BEC, skin=0.5, rebuild_every=5)
+    assert rel_rms(res2["bec"], ref2["bec"]) < 1e-4
+    assert np.abs(res2["bec"].reshape(3, 3, -1).sum(axis=2)).max() < 1e-4 * w2.n_atoms ** 0.5
 
 
 # ---------------------------------------------------------------- neighbour policy, errors
