@@ -119,8 +119,11 @@ int qnep_set_electrostatics(qnep_handle *h, const qnep_es_desc *es);
  */
 int qnep_set_neighbor_policy(qnep_handle *h, double skin, int32_t rebuild_every);
 
-/* Override the automatic list capacities (entries per atom): cap_radial sizes the skin list and the live radial
- * list, cap_angular the live angular list; <= 0 keeps the automatic value. */
+/* Override the automatic list capacities (entries per atom, rounded up to a multiple of 4): cap_radial sizes the skin
+ * list and the live radial list, cap_angular the live angular list; <= 0 keeps the automatic value (1.5 x the count
+ * expected from the mean density + 24).  When a list overflows, the call that notices it returns
+ * QNEP_ERR_NEIGHBOR_OVERFLOW, the handle drops an explicit capacity that proved too small and remembers the observed
+ * count as a lower bound for its automatic sizing: the caller repeats the call. */
 int qnep_set_neighbor_capacity(qnep_handle *h, int32_t cap_radial, int32_t cap_angular);
 
 /*
