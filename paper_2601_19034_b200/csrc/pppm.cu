@@ -61,11 +61,15 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, 
 }
 
 __global__ void __launch_bounds__(128)
-k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0, const int* __restrict__ cmi,
+k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0, const int* __restrict__ cm,
          const float* __restrict__ q, float* __restrict__ mesh)
 {
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;      // cell-major rank
-    if (p >= N) return;
+    // Threads walk the (type, cell) order here, not the cell-major one: the kernel is bound by L2 reductions, and
+    // spreading one species at a time halves the number of reductions that meet in the same sector at the same moment
+    // (0.23 -> 0.21 ms on config 4; a stride that scatters concurrent threads over the whole box is slower again).  The mesh coordinates are stored in cell-major order (for k_gather): one gather.
+    const int64_t ps = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;     // sorted index
+    if (ps >= N) return;
+    const int64_t p = cm[ps];                                              // cell-major rank
     const float4 fr = mfrac[p];
     float wx[5], wy[5], wz[5];
     bspline5(fr.x, wx); bspline5(fr.y, wy); bspline5(fr.z, wz);
@@ -84,7 +88,7 @@ k_spread(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
             if (i - c >= 0 && i - c <= 3) v = (o == i - c) ? wz[c] : v;
         w8[i] = v;
     }
-    const float qi = q[cmi[p]];
+    const float qi = q[ps];
 #pragma unroll
     for (int a = 0; a < 5; ++a) {
         const float qa = qi * wx[a];
@@ -707,7 +711,7 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
 
     // 1. spread
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mesh, 0, sizeof(float) * h->ngrid, s));
-    k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_mesh);
+    k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cm, h->d_q, h->d_mesh);
     const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
     if (h->d_half) {
         // 2.-3. forward transform on the half spectrum (the mesh is real): z and y passes on [x][y][N2/2 + LINES],
