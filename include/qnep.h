@@ -74,12 +74,12 @@ enum { QNEP_WANT_ENERGY = 1, QNEP_WANT_FORCES = 2, QNEP_WANT_VIRIAL = 4, QNEP_WA
 enum {
     QNEP_T_NEIGHBOR = 0,   /* a1  cell list + neighbour lists (0 when not rebuilt)   */
     QNEP_T_PREP,           /*     cell-relative fp32 coordinates, skin check         */
-    QNEP_T_DESC_RADIAL,    /* a2                                                     */
+    QNEP_T_DESC_RADIAL,    /* a2  skin-list walk: exact lists of the step + radial   */
     QNEP_T_DESC_ANGULAR,   /* a3                                                     */
-    QNEP_T_NN,             /* a4, a5, a10                                            */
+    QNEP_T_NN,             /* a4, a5 (+ dU/dD, dq/dD of a10)                         */
     QNEP_T_REALSPACE,      /* a6, a8                                                 */
-    QNEP_T_RECIPROCAL,     /* a7E or a7P-1..5                                        */
-    QNEP_T_FORCE_ANGULAR,  /* a11 (angular partial forces)                           */
+    QNEP_T_RECIPROCAL,     /* a7E or a7P-1..5, a9 (potential assembly)               */
+    QNEP_T_FORCE_ANGULAR,  /* a10 (Fp combine) + a11 (angular partial forces)        */
     QNEP_T_FORCE_RADIAL,   /* a11 (radial partial forces, assembly, outputs)         */
     QNEP_T_BEC,            /* a12                                                    */
     QNEP_T_TOTAL,
