@@ -20,7 +20,17 @@ K_COULOMB = 14.3996454784  # eV*A/e^2 (reading S9); repeated here only for the t
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (plain C99 + OpenMP)."""
+    """Compile the oracle with gcc (plain C99 + OpenMP).
+
+    QNEP_ORACLE_SANITIZE=1 builds a second library with -fsanitize=address,undefined instead; run the
+    CPU tests on it with  LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0."""
+    if os.environ.get("QNEP_ORACLE_SANITIZE") == "1":
+        lib_ = os.path.join(_HERE, "libqnep_oracle_san.so")
+        if force or not os.path.exists(lib_) or os.path.getmtime(lib_) < os.path.getmtime(_SRC):
+            cmd = ["gcc", "-O1", "-g", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-fsanitize=address,undefined",
+                   "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-o", lib_, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+        return lib_
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"]
         subprocess.run(cmd, check=True)

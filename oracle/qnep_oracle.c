@@ -29,8 +29,10 @@
  * finite-difference forces and finite-strain virials, PPPM adjointness identity,
  * PPPM -> Ewald convergence, invariants, Legendre double sum vs spherical
  * harmonics (scipy), FFT vs numpy, B-spline vs its convolution definition,
- * alias-sum denominator vs brute force, BEC vs finite differences of q,
- * Eq. 29-30 vs the point-charge limit (F = q E, Pdot = sum q v) and the power identity.
+ * alias-sum denominator vs brute force, BEC vs finite differences of q and of the cluster
+ * polarization P = sum q~_i r_i (Eq. 26-28), Eq. 1 evaluated by hand (bias signs, per-type blocks),
+ * Eq. 29-30 vs the point-charge limit (F = q E, Pdot = sum q v), the power identity, a case evaluated by
+ * hand and finite differences of E.P and of P(t) (index order of Z).
  * No function here is "parity unpinned".
  *
  * Units: Angstrom, eV, elementary charge.  K = 1/(4 pi eps0) (reading S9).

@@ -433,7 +433,8 @@ def test_field_response_point_charge_limit_and_power_identity(oracle):
         species only and the BEC is q~_i I, so Eq. 29 must give the textbook force q~_i E and Eq. 30 the textbook
         current sum_i q~_i v_i.
     (b) Power identity for position-dependent charges (Z_i not symmetric): sum_i F_i^ext . v_i = E . Pdot -- fails if
-        the two equations contract different indices of Z.
+        the two equations contract DIFFERENT indices of Z (it is blind to transposing Z in both at once; that case is
+        pinned by test_field_response_vs_polarization_finite_differences).
     (c) Acoustic sum rule: sum_i F_i^ext = (sum_i Z_i)^T E = Q~ E = 0 and a rigid translation carries no current."""
     w = I.config0(mode=2)
     rng = np.random.Generator(np.random.PCG64(77))
@@ -464,3 +465,190 @@ def test_field_response_point_charge_limit_and_power_identity(oracle):
     # only one of the two outputs requested
     f_only, none = oracle.response(out["bec"], E, None)
     assert none is None and np.array_equal(f_only, fext)
+
+
+# ------------------------------------------------------------- Eq. 1: hand-evaluated network
+def _pin_model(H=2):
+    m = I.ModelDesc(n_types=2, n_neurons=H, mode=2)
+    p = np.zeros(m.n_params())
+    off = I.param_offsets(m)
+    return m, p, off
+
+
+def test_nn_forward_hand_evaluated(oracle):
+    """Eq. 1 (PAPER.md :41-45) and the charge node (:58-60) with every number typed by hand: pins the MINUS signs of
+    b0 and b1 and the per-type weight blocks (S4).
+    (a) scaler = 0: the network sees x = 0, so h = tanh(-b0).
+        type 0: b0 = (-atanh 1/2, +atanh 1/4) -> h = (1/2, -1/4); w1U = (3, 8), w1q = (4, 4); b1U = 3/4, b1q = 1/8
+                -> U = 3/2 - 2 - 3/4 = -5/4,  q = 2 - 1 - 1/8 = 7/8;
+        type 1: b0 = (+atanh 1/2, 0) -> h = (-1/2, 0); w1U = (2, 5), w1q = (-2, 7)
+                -> U = -1 - 3/4 = -7/4,  q = 1 - 1/8 = 7/8.
+    (b) an isolated pair at r = r_c^R / 2 with c^R_{n k} = 2 delta_{n0} delta_{k0}, c^A = 0: f_0 = f_c = 1/2[1 + cos(pi/2)]
+        = 1/2, so D_0 = 1 exactly and all other descriptors vanish.  With s_0 = 1, w0[mu][0] = (2 atanh 1/2, 0),
+        b0 = (atanh 1/2, -atanh 1/4): z = (atanh 1/2, atanh 1/4), h = (1/2, 1/4) -> the w0 . D term enters with PLUS,
+        the bias with MINUS (with +b0, h_0 would be tanh(3 atanh 1/2) = 13/14)."""
+    a2, a4 = np.arctanh(0.5), np.arctanh(0.25)
+    # ---- (a)
+    m, p, off = _pin_model()
+    H, D = 2, m.n_desc
+    t0, t1 = off["nn"], off["nn"] + off["per_type"]
+    p[t0 + H * D: t0 + H * D + 2] = [-a2, a4]          # b0, type 0
+    p[t0 + H * D + 2: t0 + H * D + 4] = [3.0, 8.0]     # w1U
+    p[t0 + H * D + 4: t0 + H * D + 6] = [4.0, 4.0]     # w1q
+    p[t1 + H * D: t1 + H * D + 2] = [a2, 0.0]          # b0, type 1
+    p[t1 + H * D + 2: t1 + H * D + 4] = [2.0, 5.0]
+    p[t1 + H * D + 4: t1 + H * D + 6] = [-2.0, 7.0]
+    p[off["b1"]], p[off["b1"] + 1] = 0.75, 0.125
+    p[off["c_r"]:off["scaler"]] = 0.37                 # descriptors are non-zero but the scaler (= 0) hides them
+    w = I.config0(mode=2)
+    out = oracle.compute(m, p, I.EsDesc(method=0), w.pos, w.types, w.box, use_bins=False, debug=True)
+    assert np.abs(out["D"]).max() > 0.1
+    U0, q0, U1, q1 = -1.25, 0.875, -1.75, 0.875         # typed from Eq. 1, see the docstring
+    assert np.abs(out["U_i"][w.types == 0] - U0).max() < 1e-14
+    assert np.abs(out["q_raw"][w.types == 0] - q0).max() < 1e-14
+    assert np.abs(out["U_i"][w.types == 1] - U1).max() < 1e-14
+    assert np.abs(out["q_raw"][w.types == 1] - q1).max() < 1e-14
+    assert abs(out["energy"] - (32 * U0 + 32 * U1)) < 1e-12                      # Eq. 2
+    # ---- (b)
+    m, p, off = _pin_model()
+    nb = m.basis_r + 1
+    nR = m.n_max_r + 1
+    for ti in range(2):
+        for tj in range(2):
+            p[off["c_r"] + ((ti * 2 + tj) * nR + 0) * nb + 0] = 2.0
+    p[off["scaler"]] = 1.0
+    for t in (0, 1):
+        b = off["nn"] + t * off["per_type"]
+        p[b + 0 * D + 0] = 2.0 * a2                     # w0[0][0]
+        p[b + H * D: b + H * D + 2] = [a2, -a4]         # b0
+        p[b + H * D + 2: b + H * D + 4] = [4.0, 8.0]    # w1U
+        p[b + H * D + 4: b + H * D + 6] = [2.0, -4.0]   # w1q
+    p[off["b1"]], p[off["b1"] + 1] = -0.5, 0.25
+    L = 40.0
+    pos = np.array([[10.0, 10.0 + 3.0 / np.sqrt(3)], [12.0, 12.0 + 3.0 / np.sqrt(3)], [9.0, 9.0 + 3.0 / np.sqrt(3)]])
+    out = oracle.compute(m, p, I.EsDesc(method=0), pos, np.array([0, 1], dtype=np.int32),
+                         np.diag([L, L, L]).ravel(), use_bins=False, debug=True)
+    expect_D = np.zeros(m.n_desc)
+    expect_D[0] = 1.0
+    assert np.abs(out["D"] - expect_D[None, :]).max() < 1e-14
+    # h = (1/2, 1/4): U = 4/2 + 8/4 - (-1/2) = 9/2, q = 2/2 - 4/4 - 1/4 = -1/4
+    assert np.abs(out["U_i"] - 4.5).max() < 1e-13
+    assert np.abs(out["q_raw"] + 0.25).max() < 1e-13
+
+
+# ------------------------------------------------------------- Eq. 26-30: cluster polarization
+def _cluster():
+    rng = np.random.Generator(np.random.PCG64(101))
+    m = I.ModelDesc(n_types=2, n_neurons=8, mode=2)
+    p = I.random_params(m, 9).astype(np.float64)
+    L = 40.0
+    pos = (np.array([[0.0, 2.1, -0.4, 1.3, -1.9], [0.0, 0.3, 2.2, -1.7, -0.8], [0.0, -0.6, 0.9, 1.6, 2.0]])
+           + rng.normal(0, 0.05, (3, 5)) + 20.0)
+    types = np.array([0, 1, 1, 0, 1], dtype=np.int32)
+    return m, p, pos, types, np.diag([L, L, L]).ravel()
+
+
+def test_cluster_polarization_derivative_vs_bec(oracle):
+    """P11, second half, and the index order of Z (PAPER.md :216-227, Eq. 26-28).
+    For an isolated cluster P_a = sum_i q~_i r_ia (Eq. 26) is well defined and Z_{i,ab} = dP_a / dr_ib (Eq. 27).
+    Finite differences of P (from the oracle's CHARGES only) are compared with the oracle's BEC output (Eq. 28):
+      * dimer: Eq. 28 equals dP/dr exactly (r_i + r_j = 2 rbar);
+      * general cluster: Eq. 28 is a different per-atom partition of the same total; with c_ij = d q~_i / d r_ij
+        (finite differences of q_raw, S12)   Z^(28)_i,ab - dP_a/dr_ib = 1/2 sum_j (r_i + r_j - 2 rbar)_a (c_ij - c_ji)_b
+        (rbar enters through the Eq. 33 shift, whose derivative Eq. 28 drops).  DESIGN.md reading S12b.
+    Both are asymmetric in (a, b): a transposed BEC layout fails."""
+    m, p, pos, types, box = _cluster()
+    es = I.EsDesc(method=0)
+    h = 1e-5
+
+    def run(x, ty):
+        return oracle.compute(m, p, es, x, ty, box, use_bins=False, want_bec=True, debug=True)
+
+    def P(x, ty):
+        return m.sqrt_eps_inf * (run(x, ty)["charges"][None, :] * x).sum(axis=1)
+
+    def dP(x, ty):
+        n = x.shape[1]
+        Z = np.zeros((3, 3, n))
+        for i in range(n):
+            for b in range(3):
+                x1, x2 = x.copy(), x.copy()
+                x1[b, i] += h
+                x2[b, i] -= h
+                Z[:, b, i] = (P(x1, ty) - P(x2, ty)) / (2 * h)
+        return Z
+
+    # dimer
+    xd, td = pos[:, :2].copy(), types[:2].copy()
+    Zd = run(xd, td)["bec"].reshape(3, 3, 2)
+    assert np.abs(Zd - dP(xd, td)).max() < 2e-9
+    assert np.abs(Zd - m.sqrt_eps_inf * run(xd, td)["charges"][None, None, :] * np.eye(3)[:, :, None]).max() > 1e-3
+    # five atoms
+    n = pos.shape[1]
+    Z28 = run(pos, types)["bec"].reshape(3, 3, n)
+    Zfd = dP(pos, types)
+    c = np.zeros((n, n, 3))                         # c[i][j][b] = sqrt(eps) d q_raw_i / d r_jb = c_ij (j != i)
+    for j in range(n):
+        for b in range(3):
+            x1, x2 = pos.copy(), pos.copy()
+            x1[b, j] += h
+            x2[b, j] -= h
+            c[:, j, b] = m.sqrt_eps_inf * (run(x1, types)["q_raw"] - run(x2, types)["q_raw"]) / (2 * h)
+    rbar = pos.mean(axis=1)
+    corr = np.zeros((3, 3, n))
+    for i in range(n):
+        for j in range(n):
+            if j != i:
+                corr[:, :, i] += 0.5 * np.outer(pos[:, i] + pos[:, j] - 2 * rbar, c[i, j] - c[j, i])
+    assert np.abs(corr).max() > 1e-3 and np.abs(Zfd - np.transpose(Zfd, (1, 0, 2))).max() > 1e-3
+    assert np.abs(Z28 - corr - Zfd).max() < 5e-9
+    assert np.abs(np.transpose(Z28, (1, 0, 2)) - corr - Zfd).max() > 1e-3      # the transposed layout is rejected
+
+
+def test_field_response_vs_polarization_finite_differences(oracle):
+    """Eq. 29-30 (PAPER.md :229-237) as the chain rule they are: with Z_{i,ab} = dP_a/dr_ib (here taken by finite
+    differences of the cluster polarization, asymmetric),  F^ext_ib = d(E.P)/dr_ib  and  Pdot_a = dP_a/dt along the
+    velocities.  Transposing Z in BOTH equations (which the power identity cannot see) fails here.  Plus one case
+    evaluated by hand."""
+    # by hand: one ion, Z_ab = 3a + b + 1, E = (1, 0, 0) -> F_b = Z_0b; v = (0, 0, 1) -> Pdot_a = Z_a2
+    Z1 = np.arange(1.0, 10.0).reshape(9, 1)
+    f, pd = oracle.response(Z1, np.array([1.0, 0.0, 0.0]), np.array([[0.0], [0.0], [1.0]]))
+    assert np.array_equal(f[:, 0], [1.0, 2.0, 3.0]) and np.array_equal(pd, [3.0, 6.0, 9.0])
+    f, pd = oracle.response(Z1, np.array([0.0, 2.0, -1.0]), np.array([[1.0], [-1.0], [0.5]]))
+    assert np.array_equal(f[:, 0], [2 * 4.0 - 7.0, 2 * 5.0 - 8.0, 2 * 6.0 - 9.0])
+    assert np.array_equal(pd, [1.0 - 2.0 + 1.5, 4.0 - 5.0 + 3.0, 7.0 - 8.0 + 4.5])
+    # cluster
+    m, p, pos, types, box = _cluster()
+    es = I.EsDesc(method=0)
+    n = pos.shape[1]
+    h = 1e-5
+
+    def P(x):
+        q = oracle.compute(m, p, es, x, types, box, use_bins=False)["charges"]
+        return m.sqrt_eps_inf * (q[None, :] * x).sum(axis=1)
+
+    Z = np.zeros((9, n))
+    for i in range(n):
+        for b in range(3):
+            x1, x2 = pos.copy(), pos.copy()
+            x1[b, i] += h
+            x2[b, i] -= h
+            Z[[b, 3 + b, 6 + b], i] = (P(x1) - P(x2)) / (2 * h)      # entry (3 a + b): dP_a / dr_ib
+    rng = np.random.Generator(np.random.PCG64(5))
+    E = np.array([0.4, -0.9, 0.25])
+    vel = rng.normal(0, 1.0, (3, n))
+    fext, pdot = oracle.response(Z, E, vel)
+    dt = 1e-5
+    pdot_fd = (P(pos + dt * vel) - P(pos - dt * vel)) / (2 * dt)
+    assert np.abs(pdot - pdot_fd).max() < 1e-8 * max(1.0, np.abs(pdot_fd).max())
+    fext_fd = np.zeros((3, n))
+    for i in range(n):
+        for b in range(3):
+            x1, x2 = pos.copy(), pos.copy()
+            x1[b, i] += h
+            x2[b, i] -= h
+            fext_fd[b, i] = (E @ P(x1) - E @ P(x2)) / (2 * h)
+    assert np.abs(fext - fext_fd).max() < 1e-9
+    Zt = Z.reshape(3, 3, n).transpose(1, 0, 2).reshape(9, n)
+    ft, pt = oracle.response(Zt, E, vel)
+    assert np.abs(ft - fext_fd).max() > 1e-3 and np.abs(pt - pdot_fd).max() > 1e-3
