@@ -188,6 +188,7 @@ def main():
     ap.add_argument("--cpu-sample-side", type=int, default=70, help="molecules per side of the oracle's sample (70 = full config 4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--pppm-kernels", type=int, default=0, help="qnep_set_pppm_kernels: 0 automatic, 1 per-atom spread, 2 sweep spread")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -211,6 +212,7 @@ def main():
     n = w.n_atoms
     h = Q.from_workload(w)
     h.set_neighbor_policy(args.skin, args.rebuild_every)
+    h.set_pppm_kernels(args.pppm_kernels)
     masses = w.masses if w.masses is not None else np.ones(w.model.n_types)
     pos0 = torch.tensor(w.pos, dtype=torch.float64, device=dev)
     types = torch.tensor(w.types, dtype=torch.int32, device=dev)

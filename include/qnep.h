@@ -45,9 +45,12 @@ enum {
 /* The qNEP model (PAPER.md :37-60, Eq. 1; descriptor form: DESIGN.md reading S1-S5). Plain data, copied at create. */
 typedef struct {
     int32_t n_types;      /* number of species T (1..4)                                                      */
+    /* The next five describe the parameter vector; THIS VERSION accepts exactly n_max_r = n_max_a = 4, l_max = 4,
+     * basis_r = basis_a = 8 (the shape of every BASELINE.json config; the kernels are specialised for it) and
+     * qnep_create returns QNEP_ERR_UNSUPPORTED for anything else. */
     int32_t n_max_r;      /* radial descriptors  n = 0..n_max_r                                              */
     int32_t n_max_a;      /* angular descriptors n = 0..n_max_a                                              */
-    int32_t l_max;        /* angular momentum l = 1..l_max (4 in this version)                               */
+    int32_t l_max;        /* angular momentum l = 1..l_max                                                   */
     int32_t basis_r;      /* Chebyshev basis k = 0..basis_r (radial)                                         */
     int32_t basis_a;      /* Chebyshev basis k = 0..basis_a (angular)                                        */
     int32_t n_neurons;    /* hidden layer width N_neu (Eq. 1)                                                */
@@ -63,7 +66,7 @@ typedef struct {
     int32_t method;       /* 0: no electrostatics; 1: Ewald summation (Eq. 7-9); 2: PPPM (Eq. 34-38)         */
     double alpha;         /* Ewald splitting parameter, 1/Angstrom; <= 0 selects pi / rc_r (:91)             */
     int32_t ewald_nmax2;  /* Ewald: keep integer n.n <= nmax2 (k = 2 pi n / L); <= 0 selects |k| <= 2 pi alpha (:110) */
-    int32_t grid[3];      /* PPPM mesh N_x, N_y, N_z: powers of two, 8..512                                  */
+    int32_t grid[3];      /* PPPM mesh N_x, N_y, N_z: powers of two, 16..512                                 */
     int32_t order;        /* PPPM interpolation order P; 5 only (:280)                                       */
 } qnep_es_desc;
 
@@ -137,7 +140,8 @@ int qnep_set_neighbor_capacity(qnep_handle *h, int32_t cap_radial, int32_t cap_a
  *   virial_dev  [9]    eV,   W_ab row-major, W = sum_i sum_j r_ij (x) F_ji + W^k,static (Eq. 12, 22) = -dU/d(strain)
  *   charges_dev [N]    e,    neutralised, unscaled q_i (Eq. 33)
  *   bec_dev     [9][N] e,    Z_i,ab at [(3a+b)][i] (Eq. 28), or NULL
- * Errors: INVALID_ARG, UNSUPPORTED, CUDA, OOM; NEIGHBOR_OVERFLOW / SKIN_VIOLATED of the PREVIOUS call.
+ * Errors: INVALID_ARG, UNSUPPORTED, CUDA, OOM; NEIGHBOR_OVERFLOW / SKIN_VIOLATED / INVALID_ARG (a species index
+ *         outside 0..n_types-1, detected on the device) of the PREVIOUS call.
  */
 int qnep_compute(qnep_handle *h, int64_t n_atoms, const double *pos_dev, const int32_t *types_dev,
                  const double box[9], uint32_t want, double *energy_dev, double *forces_dev,
@@ -179,6 +183,14 @@ int qnep_md_reset(qnep_handle *h);
  * (qnep_profile_sum counts no evaluations for them).
  */
 int qnep_set_md_graphs(qnep_handle *h, int32_t mode);
+
+/*
+ * Choice of the PPPM charge-assignment kernel (Eq. 35).  mode 0 (default): the shared-memory sweep kernel
+ * when n_atoms >= 20000 and skin / 2 <= mesh spacing, else one thread per atom; 1: always one thread per atom;
+ * 2: the sweep kernel whenever skin / 2 <= mesh spacing (small systems too: used by the parity tests).  Both give the
+ * same mesh up to the order of fp32 additions.  Errors: INVALID_ARG.
+ */
+int qnep_set_pppm_kernels(qnep_handle *h, int32_t mode);
 
 /* Synchronise the stream of the last call and report its device-side error state (OK, NEIGHBOR_OVERFLOW, SKIN_VIOLATED, CUDA). */
 int qnep_check(qnep_handle *h);

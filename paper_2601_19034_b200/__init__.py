@@ -35,7 +35,7 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
-               "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_md_reset", "qnep_set_md_graphs", "qnep_check", "qnep_get_timings",
+               "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
                "qnep_fma_peak",
                "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
@@ -92,6 +92,8 @@ def load_library():
     lib.qnep_set_md_graphs.restype = C.c_int
     lib.qnep_set_md_graphs.argtypes = [vp, i32]
     lib.qnep_check.argtypes = [vp]
+    lib.qnep_set_pppm_kernels.restype = C.c_int
+    lib.qnep_set_pppm_kernels.argtypes = [vp, i32]
     lib.qnep_get_timings.restype = C.c_int
     lib.qnep_get_timings.argtypes = [vp, C.POINTER(C.c_float), i32]
     lib.qnep_profile_reset.restype = C.c_int
@@ -273,6 +275,10 @@ class QNEP:
     def set_md_graphs(self, mode: int):
         """0 never, 1 (default) for n_atoms <= 100000, 2 always: CUDA graphs for the steps of md_run."""
         self._ok(self._lib.qnep_set_md_graphs(self._h, int(mode)))
+
+    def set_pppm_kernels(self, mode: int):
+        """0 automatic, 1 one thread per atom, 2 shared-memory sweep kernel: PPPM charge assignment."""
+        self._ok(self._lib.qnep_set_pppm_kernels(self._h, int(mode)))
 
     def response(self, bec, efield=None, vel=None, stream=None):
         """Eq. 29-30 from the BEC tensor [9][N] (cuda float64): returns (fext [3][N] or None, pdot [3] or None)."""

@@ -12,8 +12,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqnep_b200.so")
-SOURCES = ["api.cu", "neighbor.cu", "descriptor.cu", "electro.cu", "pppm.cu"]
-HEADERS = [os.path.join(CSRC, "qnep_internal.cuh"), os.path.join(CSRC, "fft_reg.cuh"),
+SOURCES = ["api.cu", "neighbor.cu", "descriptor.cu", "electro.cu", "pppm.cu", "pppm_sweep.cu"]
+HEADERS = [os.path.join(CSRC, "qnep_internal.cuh"), os.path.join(CSRC, "fft_reg.cuh"), os.path.join(CSRC, "pppm_common.cuh"),
            os.path.join(HERE, "..", "include", "qnep.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]
@@ -51,7 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if r.returncode:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
 
-    with ThreadPoolExecutor(max_workers=5) as ex:
+    with ThreadPoolExecutor(max_workers=6) as ex:
         list(ex.map(run, jobs))
     objs = [os.path.join(objdir, s.replace(".cu", ".o")) for s in SOURCES]
     if force or jobs or _stale(LIB, objs):

@@ -28,7 +28,7 @@ void free_workspace(qnep_handle* h)
                      (void**)&h->d_lvA, (void**)&h->d_nlvA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
                      (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_recA, (void**)&h->d_recB, (void**)&h->d_lvRend,
                      (void**)&h->d_phik, (void**)&h->d_phir, (void**)&h->d_phi, (void**)&h->d_Fs, (void**)&h->d_Facc,
-                     (void**)&h->d_Fmd};
+                     (void**)&h->d_Fmd, (void**)&h->d_mbkey, (void**)&h->d_qcm};
     for (void** p : ptrs) { if (*p) cudaFree(*p); *p = nullptr; }
     h->N = 0;
     h->md_have_forces = false;
@@ -101,6 +101,8 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_sidx, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_cm, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_cmi, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_mbkey, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_qcm, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_cellc, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_xyzt, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_off0, n))) return rc;
@@ -145,12 +147,32 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         h->ws_generation += 1;
         h->force_rebuild = true;
     }
+    {
+        // PPPM mesh bins (pppm_sweep.cu, k_mbin_key)
+        int nmb[3] = {0, 0, 0}, nmbins = 0;
+        if (h->es.method == 2) {
+            nmb[0] = g.grid[0] / QNEP_MB_X; nmb[1] = g.grid[1] / QNEP_MB_Y; nmb[2] = g.grid[2] / QNEP_MB_Z;
+            nmbins = nmb[0] * nmb[1] * nmb[2];
+        }
+        if (nmbins != h->nmbins || (nmbins > 0 && !h->d_mbcnt)) {
+            if ((rc = dev_alloc(h, &h->d_mbcnt, (size_t)nmbins + 1))) return rc;
+            if ((rc = dev_alloc(h, &h->d_mbstart, (size_t)nmbins + 1))) return rc;
+            if ((rc = dev_alloc(h, &h->d_mbfill, (size_t)nmbins + 1))) return rc;
+            h->nmbins = nmbins;
+            h->ws_generation += 1;
+            h->force_rebuild = true;
+        }
+        for (int a = 0; a < 3; ++a) h->nmb[a] = nmb[a];
+    }
     const bool geo_changed = box_changed || std::memcmp(&g, &h->geo, sizeof(Geometry)) != 0;
     h->geo = g;
     std::memcpy(h->box, box, sizeof(double) * 9);
     if (geo_changed || realloc_atoms) {
         h->ws_generation += 1;
         h->force_rebuild = true;
+        // the table uploads below are synchronous copies on the legacy stream: kernels of the previous (asynchronous)
+        // call on a non-blocking caller stream may still be reading the old tables
+        if (h->flags_pending) QNEP_CUDA_OK(h, cudaStreamSynchronize(h->last_stream));
         if (h->es.method == 1) { if ((rc = qnep_setup_ewald(h))) return rc; }
         if (h->es.method == 2) { if ((rc = qnep_setup_pppm(h))) return rc; }
     }
@@ -164,9 +186,14 @@ int consume_flags(qnep_handle* h)
     const int* f = h->h_flags;
     // the device flags are sticky (a rebuild inside qnep_md_run must not erase a violation seen earlier in the
     // run): they are cleared here, on the error path only, once the host has read them
-    if (f[FLAG_MAX_NR] || f[FLAG_MAX_LR] || f[FLAG_MAX_LA] || f[FLAG_SKIN]) {
+    if (f[FLAG_MAX_NR] || f[FLAG_MAX_LR] || f[FLAG_MAX_LA] || f[FLAG_SKIN] || f[FLAG_BAD_TYPE]) {
         cudaMemsetAsync(h->d_flags, 0, sizeof(int) * FLAG_COUNT, h->last_stream);
         cudaStreamSynchronize(h->last_stream);
+    }
+    if (f[FLAG_BAD_TYPE]) {
+        h->err = "types_dev holds a species index outside 0..n_types-1";
+        h->force_rebuild = true;
+        return QNEP_ERR_INVALID_ARG;
     }
     if (f[FLAG_MAX_NR] > h->capR || f[FLAG_MAX_LR] > h->capLR || f[FLAG_MAX_LA] > h->capLA) {
         h->err = "neighbour list capacity exceeded (skin list " + std::to_string(f[FLAG_MAX_NR]) + "/" + std::to_string(h->capR) +
@@ -591,6 +618,15 @@ int qnep_set_md_graphs(qnep_handle* h, int32_t mode)
     return QNEP_OK;
 }
 
+int qnep_set_pppm_kernels(qnep_handle* h, int32_t mode)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (mode < 0 || mode > 2) { h->err = "qnep_set_pppm_kernels: mode must be 0, 1 or 2"; return QNEP_ERR_INVALID_ARG; }
+    h->pppm_kernels = mode;
+    h->ws_generation += 1;      // captured MD graphs hold the old kernels
+    return QNEP_OK;
+}
+
 int qnep_check(qnep_handle* h)
 {
     if (!h) return QNEP_ERR_INVALID_ARG;
@@ -842,7 +878,7 @@ void qnep_destroy(qnep_handle* h)
     if (h->md_stream) cudaStreamDestroy(h->md_stream);
     if (h->md_fence) cudaEventDestroy(h->md_fence);
     free_workspace(h);
-    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_sums, h->d_flags, h->d_kvec,
+    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_mbcnt, h->d_mbstart, h->d_mbfill, h->d_sums, h->d_flags, h->d_kvec,
                     h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_half, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
                     h->d_htypes, h->d_hout};
     for (void* p : ptrs) if (p) cudaFree(p);

@@ -517,13 +517,15 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
 
 // a5: Eq. 33 (reading G3): q_i = q_i^raw + (Q - sum_j q_j^raw) / N
 __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const double* __restrict__ sums, double Qtot,
-                             const int* __restrict__ sidx, float* __restrict__ q, double* __restrict__ charges_out)
+                             const int* __restrict__ sidx, const int* __restrict__ cm, float* __restrict__ q,
+                             int2* __restrict__ qcm, double* __restrict__ charges_out)
 {
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
     const double shift = (Qtot - sums[SUM_Q]) / (double)N;
     const double v = (double)qraw[p] + shift;
     q[p] = (float)v;
+    qcm[cm[p]] = make_int2((int)p, __float_as_int((float)v));      // the same charge in the order of the PPPM kernels
     if (charges_out) charges_out[sidx[p]] = v;
 }
 
@@ -961,7 +963,7 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
     k_nn<<<nb, 128, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
                                h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
     const int nb2 = (int)((N + 255) / 256);
-    k_neutralise<<<nb2, 256, 0, s>>>(N, h->d_qraw, h->d_sums, h->model.q_total, h->d_sidx, h->d_q, charges_out);
+    k_neutralise<<<nb2, 256, 0, s>>>(N, h->d_qraw, h->d_sums, h->model.q_total, h->d_sidx, h->d_cm, h->d_q, h->d_qcm, charges_out);
     h->launches += 2;
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;

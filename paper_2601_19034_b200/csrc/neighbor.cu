@@ -18,9 +18,28 @@ namespace {
 
 __device__ __forceinline__ int pack3(int a, int b, int c) { return a | (b << 10) | (c << 20); }
 
+// offset of an atom from its cell origin: the periodic image nearest to `ref` (0 at build time: nearest to the origin;
+// the build-time offset on list-reuse steps)
+__device__ __forceinline__ double cell_offset(double x, double origin, double L, double ref)
+{
+    double d = x - origin;
+    d -= L * rint((d - ref) / L);
+    return d;
+}
+
+// PPPM mesh coordinate of x (reading S10): nearest mesh point i0 (wrapped into 0..n-1) and the fractional offset
+__device__ __forceinline__ void mesh_coord(double x, double hinv, int n, float* frac, int* i0)
+{
+    const double u = x * hinv;
+    const double r = floor(u + 0.5);
+    *frac = (float)(u - r);
+    const int ir = (int)r % n;
+    *i0 = ir < 0 ? ir + n : ir;
+}
+
 // ---- binning -------------------------------------------------------------------------------
-__global__ void k_bin_count(int64_t N, const double* __restrict__ pos, const int32_t* __restrict__ types,
-                            Geometry g, int* __restrict__ key, int* __restrict__ cnt)
+__global__ void k_bin_count(int64_t N, int T, const double* __restrict__ pos, const int32_t* __restrict__ types,
+                            Geometry g, int* __restrict__ key, int* __restrict__ cnt, int* __restrict__ flags)
 {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -33,7 +52,9 @@ __global__ void k_bin_count(int64_t N, const double* __restrict__ pos, const int
         c[a] = min(max(ci, 0), g.ncell[a] - 1);
     }
     int cell = (c[0] * g.ncell[1] + c[1]) * g.ncell[2] + c[2];
-    int k = types[i] * g.ncells + cell;
+    int t = types[i];
+    if (t < 0 || t >= T) { atomicOr(&flags[FLAG_BAD_TYPE], 1); t = 0; }      // reported as INVALID_ARG; nothing is written out of bounds
+    int k = t * g.ncells + cell;
     key[i] = k;
     atomicAdd(&cnt[k], 1);
 }
@@ -127,6 +148,39 @@ __global__ void k_cm_rank(int64_t N, int ncells, const int* __restrict__ key, co
     cmi[q] = (int)p;
 }
 
+// ---- mesh-bin order for the PPPM kernels (PPPM runs) -------------------------------------------------
+// The spreading and back-interpolation kernels (pppm_sweep.cu) work on bins of QNEP_MB_X x QNEP_MB_Y x QNEP_MB_Z mesh
+// points: an atom belongs to the bin of its nearest mesh point at BUILD time.  Bins are numbered column by column,
+// key = (by * nbz + bz) * nbx + bx, so the atoms a block meets while it sweeps a (y, z) column along x are contiguous.
+// q = mbstart[key] + (rank of the sorted index inside the bin) replaces the cell-major rank: cm[p] = q, cmi[q] = p.
+__global__ void k_mbin_key(int64_t N, const double* __restrict__ pos, const int* __restrict__ sidx, const int* __restrict__ key,
+                           Geometry g, int nbx, int nbz, int* __restrict__ mbkey, int* __restrict__ mbcnt)
+{
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const int i = sidx[p];
+    const int k = key[i];
+    const int cell = k % g.ncells;
+    const int c[3] = {cell / (g.ncell[2] * g.ncell[1]), (cell / g.ncell[2]) % g.ncell[1], cell % g.ncell[2]};
+    int m0[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double origin = c[a] * g.hcell[a];
+        const double d = cell_offset(pos[a * N + i], origin, g.L[a], 0.0);       // exactly what k_prep does at build time
+        float fr;
+        mesh_coord(origin + d, g.hmesh_inv[a], g.grid[a], &fr, &m0[a]);
+    }
+    const int kb = ((m0[1] / QNEP_MB_Y) * nbz + m0[2] / QNEP_MB_Z) * nbx + m0[0] / QNEP_MB_X;
+    mbkey[p] = kb;
+    atomicAdd(&mbcnt[kb], 1);
+}
+
+__global__ void k_invert_perm(int64_t N, const int* __restrict__ cmi, int* __restrict__ cm)
+{
+    const int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (q < N) cm[cmi[q]] = (int)q;
+}
+
 // ---- per-step prep: cell-relative fp32 coordinates, PPPM mesh coordinates, skin check --------
 __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t* __restrict__ types_or_null,
                        const int* __restrict__ sidx, const int* __restrict__ key, const int* __restrict__ cm, Geometry g, int at_build,
@@ -153,32 +207,30 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
     }
     float off[3], dx[3];
     int m0[3];
+    // On list-reuse steps the image is the one nearest to the build-time offset, not to the cell origin: with fewer
+    // than three cells along an axis an atom near the +-L/2 plane would otherwise flip by a whole L between two steps
+    // (a spurious skin violation, and a wrong r_ij for the list built from the other image).
+    float o0[3] = {0.f, 0.f, 0.f};
+    if (!at_build) { const float4 o = off0[p]; o0[0] = o.x; o0[1] = o.y; o0[2] = o.z; }
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        double origin = c[a] * g.hcell[a];
-        double d = pos[a * N + i] - origin;
-        d -= g.L[a] * rint(d / g.L[a]);            // nearest image of the atom to its cell origin
+        const double origin = c[a] * g.hcell[a];
+        const double d = cell_offset(pos[a * N + i], origin, g.L[a], (double)o0[a]);     // at build time o0 = 0
         off[a] = (float)d;
-        if (g.grid[a] > 0) {
-            double u = (origin + d) * g.hmesh_inv[a];
-            double r = floor(u + 0.5);
-            dx[a] = (float)(u - r);
-            int ir = (int)r % g.grid[a];
-            m0[a] = ir < 0 ? ir + g.grid[a] : ir;
-        } else { dx[a] = 0.f; m0[a] = 0; }
+        if (g.grid[a] > 0) mesh_coord(origin + d, g.hmesh_inv[a], g.grid[a], &dx[a], &m0[a]);
+        else { dx[a] = 0.f; m0[a] = 0; }
     }
     float4 v = make_float4(off[0], off[1], off[2], __int_as_float(type));
     xyzt[p] = v;
     {
         const int q = cm[p];                       // PPPM arrays are kept in cell-major order
-        mfrac[q] = make_float4(dx[0], dx[1], dx[2], 0.f);
+        mfrac[q] = make_float4(dx[0], dx[1], dx[2], __int_as_float(pack3(m0[0], m0[1], m0[2])));    // w: the packed nearest mesh point (= mi0[q])
         mi0[q] = pack3(m0[0], m0[1], m0[2]);
     }
     if (at_build) {
         off0[p] = v;
     } else {
-        float4 o = off0[p];
-        float ddx = off[0] - o.x, ddy = off[1] - o.y, ddz = off[2] - o.z;
+        float ddx = off[0] - o0[0], ddy = off[1] - o0[1], ddz = off[2] - o0[2];
         if (ddx * ddx + ddy * ddy + ddz * ddz > g.skin_half2) atomicOr(&flags[FLAG_SKIN], 1);
     }
 }
@@ -281,17 +333,28 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
     const int nb = (int)((N + 255) / 256);
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_cnt, 0, sizeof(int) * (h->nkeys + 1), s));
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_fill, 0, sizeof(int) * h->nkeys, s));
-    k_bin_count<<<nb, 256, 0, s>>>(N, pos, types, h->geo, h->d_key, h->d_cnt);
+    k_bin_count<<<nb, 256, 0, s>>>(N, h->model.n_types, pos, types, h->geo, h->d_key, h->d_cnt, h->d_flags);
     k_exclusive_scan<<<1, 1024, 0, s>>>(h->nkeys, h->d_cnt, h->d_start);
     k_scatter<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_fill, h->d_tmpidx);
     k_rank<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_tmpidx, h->d_sidx);
-    {
+    if (h->nmbins > 0) {
+        // PPPM: mesh-bin order (the sorted index p plays the role of the atom index in k_scatter / k_rank)
+        QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mbcnt, 0, sizeof(int) * (h->nmbins + 1), s));
+        QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mbfill, 0, sizeof(int) * h->nmbins, s));
+        k_mbin_key<<<nb, 256, 0, s>>>(N, pos, h->d_sidx, h->d_key, h->geo, h->nmb[0], h->nmb[2], h->d_mbkey, h->d_mbcnt);
+        k_exclusive_scan<<<1, 1024, 0, s>>>(h->nmbins, h->d_mbcnt, h->d_mbstart);
+        k_scatter<<<nb, 256, 0, s>>>(N, h->d_mbkey, h->d_mbstart, h->d_mbfill, h->d_tmpidx);
+        k_rank<<<nb, 256, 0, s>>>(N, h->d_mbkey, h->d_mbstart, h->d_tmpidx, h->d_cmi);
+        k_invert_perm<<<nb, 256, 0, s>>>(N, h->d_cmi, h->d_cm);
+        h->launches += 5;
+    } else {
         const int nc = h->geo.ncells;
         k_cell_totals<<<(nc + 255) / 256, 256, 0, s>>>(nc, h->model.n_types, h->d_cnt, h->d_ctot);
         k_exclusive_scan<<<1, 1024, 0, s>>>(nc, h->d_ctot, h->d_cstart);
         k_cm_rank<<<nb, 256, 0, s>>>(N, nc, h->d_key, h->d_sidx, h->d_start, h->d_cnt, h->d_cstart, h->d_cm, h->d_cmi);
+        h->launches += 3;
     }
-    h->launches += 7;
+    h->launches += 4;
     int rc = qnep_launch_prep(h, pos, true, s);
     if (rc) return rc;
     const int nb2 = (int)((N + 127) / 128);

@@ -22,21 +22,11 @@
 #include <type_traits>
 
 #include "fft_reg.cuh"
+#include "pppm_common.cuh"
 
 namespace {
 
 constexpr int FFT_MAXN = 512;
-
-__device__ __forceinline__ void bspline5(float dx, float* __restrict__ w)
-{
-    // centred cardinal B-spline of order 5 on mesh offsets -2..2 (reading S10)
-    const float d2 = dx * dx, d3 = d2 * dx, d4 = d2 * d2;
-    w[0] = (1.f - 8.f * dx + 24.f * d2 - 32.f * d3 + 16.f * d4) * (1.f / 384.f);
-    w[1] = (19.f - 44.f * dx + 24.f * d2 + 16.f * d3 - 16.f * d4) * (1.f / 96.f);
-    w[2] = (115.f - 120.f * d2 + 48.f * d4) * (1.f / 192.f);
-    w[3] = (19.f + 44.f * dx + 24.f * d2 - 16.f * d3 - 16.f * d4) * (1.f / 96.f);
-    w[4] = (1.f + 8.f * dx + 24.f * d2 + 32.f * d3 + 16.f * d4) * (1.f / 384.f);
-}
 
 __device__ __forceinline__ void stencil_indices(int packed, const int* grid, int (*idx)[5])
 {
@@ -694,7 +684,7 @@ int qnep_setup_pppm(qnep_handle* h)
     }
     QNEP_CUDA_OK(h, cudaMemcpy(h->d_twiddle, tw.data(), sizeof(float2) * 3 * FFT_MAXN, cudaMemcpyHostToDevice));
     QNEP_CUDA_OK(h, cudaMemcpy(h->d_gtab, tab.data(), sizeof(float) * 9 * FFT_MAXN, cudaMemcpyHostToDevice));
-    return QNEP_OK;
+    return qnep_setup_sweep(h);
 }
 
 int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
@@ -709,9 +699,16 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
     cudaError_t ce = cudaSuccess;
     auto note = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
 
-    // 1. spread
-    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mesh, 0, sizeof(float) * h->ngrid, s));
-    k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cm, h->d_q, h->d_mesh);
+    // 1. spread: a shared-memory tile swept along x (pppm_sweep.cu), or one thread per atom for small systems
+    const bool sweep = qnep_sweep_usable(h);
+    if (sweep) {
+        int rc = qnep_launch_spread_sweep(h, s);
+        if (rc) return rc;
+    } else {
+        QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mesh, 0, sizeof(float) * h->ngrid, s));
+        k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cm, h->d_q, h->d_mesh);
+        h->launches += 1;
+    }
     const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
     if (h->d_half) {
         // 2.-3. forward transform on the half spectrum (the mesh is real): z and y passes on [x][y][N2/2 + LINES],
@@ -800,7 +797,7 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
     // 5. gather
     const int nbg = (int)((N + GATHER_BLOCK - 1) / GATHER_BLOCK);
     k_gather<<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs);
-    h->launches += 7;
+    h->launches += 6;
     QNEP_CUDA_OK(h, ce);
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;

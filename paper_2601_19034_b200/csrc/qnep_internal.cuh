@@ -2,6 +2,7 @@
 // B200-native qNEP force evaluation (arXiv 2601.19034).  Not part of the public boundary
 // (include/qnep.h).  Shares nothing with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
@@ -18,6 +19,11 @@
 #define QNEP_NRAD 5                 // n = 0..4
 #define QNEP_NDESC 25
 #define QNEP_GRAPH_MAX_ATOMS 100000   // above this the step is not launch-bound and keeps its per-stage events
+// PPPM mesh bins of the sweep kernel (pppm_sweep.cu): bin edge in mesh points along x, y, z
+#define QNEP_MB_X 4
+#define QNEP_MB_Y 8
+#define QNEP_MB_Z 8
+#define QNEP_SWEEP_MIN_ATOMS 20000    // below this the per-atom spread kernel is used (too few columns to fill the GPU)
 
 // Neighbour lists are WARP-TILED: the rows of the 32 atoms p = 32 w .. 32 w + 31 are interleaved in one contiguous
 // block, so a warp streams its lists sequentially (one DRAM page after the other) and every thread loads 16 bytes
@@ -39,7 +45,7 @@ constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (DESIGN.md read
 enum { SUM_E_NEP = 0, SUM_Q, SUM_PHI, SUM_U_R, SUM_U_K, SUM_U_S, SUM_W0 /* 9 entries */, SUM_KE = 15, SUM_COUNT = 16 };
 // device-side int flags
 // overflow flags hold the largest count seen when a list exceeded its capacity (0 otherwise)
-enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_COUNT = 8 };
+enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_BAD_TYPE /* a species index outside 0..T-1 */, FLAG_COUNT = 8 };
 
 struct Geometry {            // orthorhombic cell and the cell grid of the neighbour search
     double L[3];
@@ -93,12 +99,22 @@ struct qnep_handle {
     int* d_sidx = nullptr;           // [N] sorted -> original
     int* d_ctot = nullptr;           // [ncells + 1] atoms per cell (all species)
     int* d_cstart = nullptr;         // [ncells + 1] its exclusive scan
-    int* d_cm = nullptr;             // [N] sorted index p -> cell-major rank q (order of the PPPM kernels)
+    int* d_cm = nullptr;             // [N] sorted index p -> rank q in the order of the PPPM kernels (mesh-bin order; cell-major without PPPM)
     int* d_cmi = nullptr;            // [N] q -> p
+    int nmb[3] = {0, 0, 0};          // PPPM mesh bins per axis (grid / QNEP_MB_*); nmbins = 0 when PPPM is off
+    int nmbins = 0;
+    int* d_mbkey = nullptr;          // [N] mesh-bin key of sorted atom p (build time)
+    int* d_mbcnt = nullptr;          // [nmbins + 1]
+    int* d_mbstart = nullptr;        // [nmbins + 1] first mesh-bin-order rank q of every bin
+    int* d_mbfill = nullptr;         // [nmbins]
+    int pppm_kernels = 0;            // 0 automatic, 1 per-atom spread / gather, 2 sweep kernels (qnep_set_pppm_kernels)
+    int2* d_qcm = nullptr;           // [N] mesh-bin order: (sorted index p, bits of the neutralised charge q_p) for the PPPM sweep kernels
+    alignas(64) CUtensorMap tm_mesh;  // TMA descriptor of the charge mesh (box 4 x 14 x 16 floats) for k_spread_sweep; valid when tm_ok
+    bool tm_ok = false;
     int* d_cellc = nullptr;          // [N] packed cell coordinates (10 bits each)
     float4* d_xyzt = nullptr;        // [N] cell-relative position, w = type bits
     float4* d_off0 = nullptr;        // [N] the same at build time (skin check)
-    float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, -), cell-major order
+    float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, bits of the packed nearest mesh point), mesh-bin order
     int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each, cell-major order
     int4* d_nlR = nullptr;           // warp-tiled [capR / 4] int4 per atom: skin list (r < rc_r + skin at build time)
     int* d_nnR = nullptr;            // [N]
@@ -201,3 +217,7 @@ int qnep_launch_ewald(qnep_handle* h, const double* pos, cudaStream_t s);
 // pppm.cu
 int qnep_setup_pppm(qnep_handle* h);
 int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s);
+// pppm_sweep.cu
+bool qnep_sweep_usable(const qnep_handle* h);
+int qnep_setup_sweep(qnep_handle* h);
+int qnep_launch_spread_sweep(qnep_handle* h, cudaStream_t s);

@@ -121,6 +121,55 @@ def test_config1_pppm(torch, oracle, mode):
     assert np.abs(W - W.T).max() < 1e-4 * np.abs(W).max()
 
 
+@pytest.mark.parametrize("case", ["config1", "config1_mode1", "config2", "aniso", "mesh16", "reuse"])
+def test_pppm_sweep_kernels(torch, oracle, case):
+    """The shared-memory sweep kernel of the charge assignment (pppm_sweep.cu), forced on small systems:
+    mesh, phi, static force and the final outputs against the oracle.  'aniso': 32 x 64 x 16 mesh (one bin column wraps
+    onto itself along z); 'mesh16': every axis is a single ring of 16 planes; 'reuse': atoms moved by up to 0.45 A
+    (skin 1.0) since they were binned -- the drift margin of the tiles."""
+    skin, rebuild = 0.0, 0
+    if case == "config1":
+        w = I.config1()
+    elif case == "config1_mode1":
+        w = I.config1(mode=1)
+    elif case == "config2":
+        w = I.config2()
+    elif case == "aniso":
+        w = I.config1()
+        w.es = replace(w.es, grid=(32, 64, 16))
+    elif case == "mesh16":
+        w = I.config1()
+        w.es = replace(w.es, grid=(16, 16, 16))
+    else:
+        w = I.config1()
+        skin, rebuild = 1.0, 10
+    h = Q.from_workload(w)
+    h.set_pppm_kernels(2)
+    if skin:
+        h.set_neighbor_policy(skin, rebuild)
+        gpu_eval(torch, w, handle=h)                                   # bins and lists built at the OLD positions
+        rng = np.random.Generator(np.random.PCG64(15))
+        d = rng.normal(size=w.pos.shape)
+        d *= rng.uniform(0.0, 0.45, size=(1, w.n_atoms)) / np.linalg.norm(d, axis=0, keepdims=True)
+        w = replace(w, pos=w.pos + d)
+    ref = oracle.compute_workload(w, debug=True)
+    _, res = gpu_eval(torch, w, handle=h)
+    if skin:
+        assert h.get_timings()["neighbor"] < 0.05                      # no rebuild: the build-time bins were used
+    assert_parity(w, res, ref, f"sweep kernels, {case}")
+    rho = h.debug_copy(Q.DBG_MESH_RHO, tuple(w.es.grid)).cpu().numpy()
+    assert np.abs(rho - ref["rho"]).max() <= 2e-6 * np.abs(ref["rho"]).max() + 1e-7
+    n = w.n_atoms
+    assert np.abs(h.debug_copy(Q.DBG_PHI, (n,)).cpu().numpy() - ref["phi"]).max() < 2e-5 * max(1.0, np.abs(ref["phi"]).max())
+    assert rel_rms(h.debug_copy(Q.DBG_F_STATIC, (3, n)).cpu().numpy(), ref["F_es"]) < 1e-4
+    # the per-atom kernels give the same mesh
+    h1 = Q.from_workload(w)
+    h1.set_pppm_kernels(1)
+    gpu_eval(torch, w, handle=h1)
+    rho1 = h1.debug_copy(Q.DBG_MESH_RHO, tuple(w.es.grid)).cpu().numpy()
+    assert np.abs(rho - rho1).max() <= 2e-6 * np.abs(ref["rho"]).max() + 1e-7
+
+
 def test_config1_ragged_subsets(torch, oracle):
     """Sizes that are not multiples of the block / warp / tile sizes, including a single warp's tail."""
     w = I.config1()
@@ -197,6 +246,49 @@ def test_skin_and_rebuild_identity(torch, oracle):
     with pytest.raises(Q.QnepError) as ei:
         gpu_eval(torch, replace(moved, pos=far), handle=h)
     assert ei.value.code == Q.QNEP_ERR_SKIN_VIOLATED
+
+
+@pytest.mark.parametrize("ncell", [1, 2])
+def test_list_reuse_on_small_boxes(torch, oracle, ncell):
+    """Fewer than three cells per axis: an atom that drifts across the +-L/2 plane of its cell-relative coordinate must
+    keep the image it had at build time (no spurious SKIN_VIOLATED, same result as a fresh build).
+    ncell = 1: config 0 (L = 11.28 A, rock-salt sites sit exactly on L/2); ncell = 2: the same lattice with 6 sites per
+    edge (L = 16.92 A >= 2 (r_c + skin))."""
+    if ncell == 1:
+        w = I.config0(mode=1)
+    else:
+        base = I.config0(mode=1)
+        pos, types, box = I.rocksalt_lattice(6, 2.82)
+        rng = np.random.Generator(np.random.PCG64(77))
+        w = replace(base, pos=pos + rng.normal(0, 0.1, pos.shape), types=types, box=box)
+    rng = np.random.Generator(np.random.PCG64(8))
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(1.0, 50)
+    gpu_eval(torch, w, handle=h)                                    # build
+    cur = w
+    for step in range(4):                                           # a small random walk, 0.02-0.05 A rms per step
+        cur = replace(cur, pos=cur.pos + rng.normal(0, 0.03, cur.pos.shape))
+        _, res = gpu_eval(torch, cur, handle=h)
+        assert h.get_timings()["neighbor"] < 0.02                   # lists reused
+    assert_parity(cur, res, oracle.compute_workload(cur, use_bins=False), f"reuse, {ncell} cell(s) per axis")
+    # and through the MD driver
+    vel = torch.tensor(rng.normal(0, 0.02, w.pos.shape), dtype=torch.float64, device="cuda")
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    h.md_reset()
+    h.md_run(pos, vel, types, w.box, np.array([22.99, 35.45]), 0.02, 40)     # raises on SKIN_VIOLATED
+
+
+def test_species_index_out_of_range_is_reported(torch):
+    w = I.config0()
+    h = Q.from_workload(w)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    bad = w.types.copy()
+    bad[5] = 7
+    types = torch.tensor(bad, dtype=torch.int32, device="cuda")
+    with pytest.raises(Q.QnepError) as ei:
+        h.compute(pos, types, w.box)                 # the binding checks the device-side flags after the call
+    assert ei.value.code == Q.QNEP_ERR_INVALID_ARG
 
 
 def test_neighbor_overflow_is_reported_and_recovered(torch, oracle):
