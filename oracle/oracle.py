@@ -110,8 +110,8 @@ def descriptors(model, params, pos, types, box, use_bins=False):
     return D
 
 
-def electrostatics(pos, q, box, rc, mode, es, want_rho=False):
-    """Fixed charges -> dict(U=[U^r, U^k, U^s], phi, F[3][N], W[3][3], rho)."""
+def electrostatics(pos, q, box, rc, mode, es, want_rho=False, want_atom_virial=False):
+    """Fixed charges -> dict(U=[U^r, U^k, U^s], phi, F[3][N], W[3][3], rho, W_atom[9][N])."""
     pos = _f64(pos)
     n = pos.shape[1]
     U = np.zeros(3)
@@ -120,13 +120,14 @@ def electrostatics(pos, q, box, rc, mode, es, want_rho=False):
     W = np.zeros(9)
     rho = np.zeros(tuple(es.grid)) if (want_rho and es.method == 2) else None
     ee = _es(es)
+    Wat = np.zeros((9, n)) if want_atom_virial else None
     rc_ = lib().orc_electrostatics(C.c_int64(n), _p(pos), _p(_f64(q)), _p(_f64(box)), C.c_double(rc),
-                                   C.c_int(mode), C.byref(ee), _p(U), _p(phi), _p(F), _p(W), _p(rho))
+                                   C.c_int(mode), C.byref(ee), _p(U), _p(phi), _p(F), _p(W), _p(rho), _p(Wat))
     assert rc_ == 0, rc_
-    return dict(U=U, phi=phi, F=F, W=W.reshape(3, 3), rho=rho)
+    return dict(U=U, phi=phi, F=F, W=W.reshape(3, 3), rho=rho, W_atom=Wat)
 
 
-def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, debug=False):
+def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, debug=False, want_atom_virial=False):
     """The whole force evaluation.  Returns a dict of fp64 arrays."""
     pos = _f64(pos)
     n = pos.shape[1]
@@ -136,6 +137,7 @@ def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, d
     virial = np.zeros(9)
     charges = np.zeros(n)
     bec = np.zeros((9, n)) if want_bec else None
+    wat = np.zeros((9, n)) if want_atom_virial else None
     out = {}
     dbg = None
     if debug:
@@ -151,11 +153,11 @@ def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, d
     rc_ = lib().orc_compute(C.byref(mm), _p(_f64(params)), C.byref(ee), C.c_int64(n), _p(pos),
                             _p(np.ascontiguousarray(types, dtype=np.int32)), _p(_f64(box)),
                             C.c_int(int(use_bins)), _p(energy), _p(forces), _p(virial), _p(charges), _p(bec),
-                            C.byref(dbg) if dbg is not None else None)
+                            C.byref(dbg) if dbg is not None else None, _p(wat))
     if rc_ != 0:
         raise RuntimeError(f"orc_compute failed with code {rc_}")
     out.update(energy=energy[0], energy_parts=dict(nep=energy[1], r=energy[2], k=energy[3], s=energy[4]),
-               forces=forces, virial=virial.reshape(3, 3), charges=charges, bec=bec)
+               forces=forces, virial=virial.reshape(3, 3), charges=charges, bec=bec, virial_atom=wat)
     return out
 
 

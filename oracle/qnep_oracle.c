@@ -19,7 +19,8 @@
  *   NN                :41-45 Eq. 1, :58-60    minus biases; second output node = q_i; S4, S5
  *   neutralisation    :255-262 Eq. 33         reading G3
  *   U^r, U^k, U^s     :85-118 Eq. 6-10        reading G1 (erfc(alpha r), k != 0)
- *   forces / virial   :124-199 Eq. 11-23      dynamic-charge terms folded (:140), reading S6
+ *   forces / virial   :124-199 Eq. 11-23      dynamic-charge terms folded (:140), reading S6;
+ *                                             per-atom virial: Eq. 12, Eq. 20 (real part, G4), Eq. 39
  *   BEC               :205-227 Eq. 24-28      reading S12
  *   field response    :229-237 Eq. 29-30      F^ext = E.Z, Pdot = sum_i Z_i v_i (orc_response)
  *   PPPM              :266-304 Eq. 34-38      readings G2 (Eq. 36), S10 (W, P = 5), S11 (FFT)
@@ -630,7 +631,7 @@ static double sinc(double x) { return x == 0.0 ? 1.0 : sin(x) / x; }
  * w = wrapped positions.  nl = radial neighbour list (rc = rc_r) or NULL when mode == 2. */
 static int electrostatics(int64_t n, const double *w, const double *q, const double *box, double rc, int mode,
                           const orc_es *es, const orc_nlist *nl, double *U, double *phi, double *F, double *W,
-                          double *rho_out)
+                          double *rho_out, double *Wat)
 {
     const double K = ORC_K_COULOMB;
     double alpha = es->alpha > 0.0 ? es->alpha : ORC_PI / rc;
@@ -639,6 +640,7 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
     for (int64_t i = 0; i < n; ++i) phi[i] = 0.0;
     for (int64_t i = 0; i < 3 * n; ++i) F[i] = 0.0;
     for (int a = 0; a < 9; ++a) W[a] = 0.0;
+    if (Wat) for (int64_t i = 0; i < 9 * n; ++i) Wat[i] = 0.0;
     if (es->method == 0) return 0;
 
     if (mode == 1) {
@@ -655,7 +657,11 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                 double br = (2.0 * alpha / sqrt(ORC_PI) * r * exp(-alpha * alpha * r * r) + erfc(alpha * r)) / (r * r * r);
                 for (int a = 0; a < 3; ++a) {
                     F[a * n + i] += -K * q[i] * q[j] * br * d[a];
-                    for (int c = 0; c < 3; ++c) Wr[3 * a + c] += 0.5 * K * q[i] * q[j] * br * d[a] * d[c];
+                    for (int c = 0; c < 3; ++c) {
+                        Wr[3 * a + c] += 0.5 * K * q[i] * q[j] * br * d[a] * d[c];
+                        /* Eq. 12 with Eq. 15: W_i = sum_j r_ij (x) F_ji^{r,static}, F_ji = +1/2 K q_i q_j [..] r_ij / r^3 */
+                        if (Wat) Wat[(3 * a + c) * n + i] += 0.5 * K * q[i] * q[j] * br * d[a] * d[c];
+                    }
                 }
             }
         }
@@ -687,6 +693,7 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
         {
             double *phi_l = (double *)calloc(n > 0 ? n : 1, sizeof(double));
             double *F_l = (double *)calloc(n > 0 ? 3 * n : 1, sizeof(double));
+            double *Wat_l = Wat ? (double *)calloc(n > 0 ? 9 * n : 1, sizeof(double)) : 0;
             double Uk_l = 0.0, Wk_l[9] = {0};
 #pragma omp for schedule(dynamic, 8)
             for (int64_t t = 0; t < nk_box; ++t) {
@@ -720,6 +727,10 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                     double im = Sr * s + Si * c;  /* Im[S e^{ik.r}] */
                     phi_l[i] += 2.0 * K * G * re;                                       /* bracket of Eq. 19 */
                     for (int a = 0; a < 3; ++a) F_l[a * n + i] += 2.0 * K * q[i] * G * k[a] * im; /* Eq. 18 */
+                    if (Wat_l)                                                          /* Eq. 20, real part (reading G4) */
+                        for (int a = 0; a < 3; ++a)
+                            for (int cc = 0; cc < 3; ++cc)
+                                Wat_l[(3 * a + cc) * n + i] += K * G * q[i] * re * ((a == cc ? 1.0 : 0.0) - bfac * k[a] * k[cc]);
                 }
             }
 #pragma omp critical
@@ -728,9 +739,11 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                 for (int a = 0; a < 9; ++a) Wk[a] += Wk_l[a];
                 for (int64_t i = 0; i < n; ++i) phi[i] += phi_l[i];
                 for (int64_t i = 0; i < 3 * n; ++i) F[i] += F_l[i];
+                if (Wat_l) for (int64_t i = 0; i < 9 * n; ++i) Wat[i] += Wat_l[i];
             }
             free(phi_l);
             free(F_l);
+            free(Wat_l);
         }
         U[1] = Uk;
         for (int a = 0; a < 9; ++a) W[a] += Wk[a];
@@ -838,6 +851,51 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
             phi[i] += 2.0 * K * acc[0];                                       /* bracket of Eq. 38 */
             for (int a = 0; a < 3; ++a) F[a * n + i] += -2.0 * K * q[i] * acc[1 + a]; /* Eq. 37 */
         }
+        if (Wat) {
+            /* Eq. 39: W_i^{k,static} = K q_i sum_s W(r_i - r_s) F^-1[S G^opt B]_s -- six inverse FFTs (:302), one per
+             * independent component of B (Eq. 21; true k in B, all mesh k != 0 as in Eq. 34) */
+            static const int comp_ab[6][2] = {{0, 0}, {1, 1}, {2, 2}, {0, 1}, {0, 2}, {1, 2}};
+            for (int comp = 0; comp < 6; ++comp) {
+                int a = comp_ab[comp][0], b = comp_ab[comp][1];
+                for (int64_t m0 = 0; m0 < N[0]; ++m0)
+                    for (int64_t m1 = 0; m1 < N[1]; ++m1)
+                        for (int64_t m2 = 0; m2 < N[2]; ++m2) {
+                            int64_t s = (m0 * N[1] + m1) * N[2] + m2;
+                            int64_t mm[3] = {m0, m1, m2};
+                            double k[3];
+                            for (int c = 0; c < 3; ++c) {
+                                int64_t nc = mm[c] < N[c] / 2 ? mm[c] : mm[c] - N[c];
+                                k[c] = 2.0 * ORC_PI * nc / L[c];
+                            }
+                            double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+                            double Bab = 0.0;
+                            if (k2 > 0.0) Bab = (a == b ? 1.0 : 0.0) - (2.0 / (4.0 * alpha * alpha) + 2.0 / k2) * k[a] * k[b];
+                            fld[2 * s] = rho[2 * s] * Gopt[s] * Bab;
+                            fld[2 * s + 1] = rho[2 * s + 1] * Gopt[s] * Bab;
+                        }
+                orc_fft3d(fld, N[0], N[1], N[2], +1);
+                for (int64_t i = 0; i < n; ++i) {
+                    int i0[3];
+                    double wt[3][5];
+                    for (int c = 0; c < 3; ++c) {
+                        double u = w[c * n + i] / L[c] * N[c];
+                        i0[c] = (int)floor(u + 0.5);
+                        orc_bspline5(u - i0[c], wt[c]);
+                    }
+                    double acc = 0.0;
+                    for (int aa = 0; aa < 5; ++aa)
+                        for (int bb = 0; bb < 5; ++bb)
+                            for (int cc = 0; cc < 5; ++cc) {
+                                int64_t s0 = ((i0[0] + aa - 2) % N[0] + N[0]) % N[0];
+                                int64_t s1 = ((i0[1] + bb - 2) % N[1] + N[1]) % N[1];
+                                int64_t s2 = ((i0[2] + cc - 2) % N[2] + N[2]) % N[2];
+                                acc += wt[0][aa] * wt[1][bb] * wt[2][cc] * fld[2 * ((s0 * N[1] + s1) * N[2] + s2)];
+                            }
+                    Wat[(3 * a + b) * n + i] += K * q[i] * acc;
+                    if (a != b) Wat[(3 * b + a) * n + i] += K * q[i] * acc;
+                }
+            }
+        }
         free(rho); free(fld); free(Gopt);
         for (int c = 0; c < 4; ++c) free(mesh[c]);
     } else {
@@ -848,14 +906,14 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
 
 /* exported: electrostatics of FIXED charges (the static-charge pins: Madelung, brute-force image sum...) */
 int orc_electrostatics(int64_t n, const double *pos, const double *q, const double *box, double rc, int mode,
-                       const orc_es *es, double *U3, double *phi, double *F, double *W, double *rho)
+                       const orc_es *es, double *U3, double *phi, double *F, double *W, double *rho, double *Wat)
 {
     double *w = (double *)malloc(sizeof(double) * 3 * (n > 0 ? n : 1));
     wrap_positions(n, pos, box, w);
     orc_nlist nl;
     memset(&nl, 0, sizeof(nl));
     if (mode == 1 && build_nlist(n, w, box, rc, 1, &nl)) { free(w); return -1; }
-    int rcode = electrostatics(n, w, q, box, rc, mode, es, mode == 1 ? &nl : 0, U3, phi, F, W, rho);
+    int rcode = electrostatics(n, w, q, box, rc, mode, es, mode == 1 ? &nl : 0, U3, phi, F, W, rho, Wat);
     if (mode == 1) nlist_free(&nl);
     free(w);
     return rcode;
@@ -864,10 +922,11 @@ int orc_electrostatics(int64_t n, const double *pos, const double *q, const doub
 /* ------------------------------------------------------------------------- */
 /* the whole force evaluation                        */
 /* ------------------------------------------------------------------------- */
-/* energy[5] = {U^tot, U^NEP, U^r, U^k, U^s};  forces[3][N];  virial[9];  charges[N];  bec[9][N] or NULL */
+/* energy[5] = {U^tot, U^NEP, U^r, U^k, U^s};  forces[3][N];  virial[9];  charges[N];  bec[9][N] or NULL;
+ * virial_atom[9][N] or NULL: per-atom virial, W_i = sum_j r_ij (x) F_ji (Eq. 12) + W_i^{k,static} (Eq. 20 / Eq. 39) */
 int orc_compute(const orc_model *m, const double *params, const orc_es *es, int64_t n, const double *pos,
                 const int32_t *types, const double *box, int use_bins, double *energy, double *forces,
-                double *virial, double *charges, double *bec, const orc_debug *dbg)
+                double *virial, double *charges, double *bec, const orc_debug *dbg, double *virial_atom)
 {
     orc_params P;
     split_params(m, params, &P);
@@ -903,7 +962,7 @@ int orc_compute(const orc_model *m, const double *params, const orc_es *es, int6
     for (int64_t i = 0; i < n; ++i) q[i] += (m->q_total - qsum) / (double)n;
     /* 5.-6. electrostatics with the unscaled neutralised charges */
     double U3[3], Wes[9];
-    int rcode = electrostatics(n, w, q, box, m->rc_r, m->mode, es, &nl, U3, phi, Fes, Wes, dbg ? dbg->rho : 0);
+    int rcode = electrostatics(n, w, q, box, m->rc_r, m->mode, es, &nl, U3, phi, Fes, Wes, dbg ? dbg->rho : 0, virial_atom);
     if (rcode) return rcode;
     if (dbg && dbg->phi) memcpy(dbg->phi, phi, sizeof(double) * n);
     if (dbg && dbg->F_es) memcpy(dbg->F_es, Fes, sizeof(double) * 3 * n);
@@ -937,7 +996,13 @@ int orc_compute(const orc_model *m, const double *params, const orc_es *es, int6
 #pragma omp atomic
                     forces[a * n + j] -= Fij[3 * p + a];      /* - F_ij on j (= -F_ji term of atom j) */
                     /* this F_ij is the "F_ji" of atom j's sum in Eq. 12 with r_ji = -r_ij */
-                    for (int c = 0; c < 3; ++c) Wl[3 * a + c] -= nl.d[4 * (b + p) + a] * Fij[3 * p + c];
+                    for (int c = 0; c < 3; ++c) {
+                        Wl[3 * a + c] -= nl.d[4 * (b + p) + a] * Fij[3 * p + c];
+                        if (virial_atom) {       /* W_j += r_ji (x) F_ij: the term belongs to atom j (Eq. 12) */
+#pragma omp atomic
+                            virial_atom[(3 * a + c) * n + j] -= nl.d[4 * (b + p) + a] * Fij[3 * p + c];
+                        }
+                    }
                 }
             }
             if (bec) {

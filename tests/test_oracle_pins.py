@@ -652,3 +652,104 @@ def test_field_response_vs_polarization_finite_differences(oracle):
     Zt = Z.reshape(3, 3, n).transpose(1, 0, 2).reshape(9, n)
     ft, pt = oracle.response(Zt, E, vel)
     assert np.abs(ft - fext_fd).max() > 1e-3 and np.abs(pt - pdot_fd).max() > 1e-3
+
+
+# ------------------------------------------------------------- per-atom virial (Eq. 12, 20, 39)
+def test_atom_virial_static_coulomb_vs_bruteforce_and_trace(oracle):
+    """Eq. 12 + Eq. 15 (real space) and Eq. 20 (reciprocal space, real part: reading G4) for FIXED charges, converged:
+    (a) against the pairwise definition W_i = 1/2 sum_j sum_images K q_i q_j r (x) r / r^3 summed by brute force over
+        image cubes of a neutral cell with cubic point symmetry (no dipole, isotropic second moment);
+    (b) Tr W_i = 1/2 q_i phi_i for every atom (the Coulomb virial theorem per atom; phi includes the self term);
+    (c) sum_i W_i = W (Eq. 22 + Eq. 12), W_i symmetric."""
+    L = 7.0
+    pos, q = _cubic_cluster(L)
+    n = pos.shape[1]
+    box = np.diag([L, L, L]).ravel()
+    es = I.EsDesc(method=1, alpha=0.75, ewald_nmax2=196)
+    r = oracle.electrostatics(pos, q, box, 13.9, 1, es, want_atom_virial=True)
+    Wat = r["W_atom"].reshape(3, 3, n)
+    M = 12
+    g = np.arange(-M, M + 1)
+    S = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3) * L
+    d = pos.T[:, None, None, :] - pos.T[None, :, None, :] - S[None, None, :, :]
+    dist = np.linalg.norm(d, axis=-1)
+    qq = q[:, None, None] * q[None, :, None]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        inv3 = np.where(dist > 0, 1.0 / dist ** 3, 0.0)
+    brute = 0.5 * K * np.einsum("ijs,ijsa,ijsb->abi", qq * inv3, d, d)
+    # Summed over cubes of images, the potential of a neutral cell without dipole still differs from the Ewald
+    # (tin-foil) one by the constant c = -2 pi K / (3 V) sum_j q_j |r_j|^2 (the trace of the second moment); the
+    # energy does not see it (sum q = 0), Tr W_i = 1/2 q_i phi_i does: W_i^brute = W_i^Ewald + (q_i c / 6) 1.
+    c = -(2 * np.pi / (3 * L ** 3)) * K * (q * ((pos - L / 2) ** 2).sum(axis=0)).sum()
+    shifted = brute - (q * c / 6.0)[None, None, :] * np.eye(3)[:, :, None]
+    assert abs(c) > 0.1
+    assert np.abs(Wat - shifted).max() < 1e-5 * np.abs(brute).max()
+    assert np.abs(np.einsum("aai->i", Wat) - 0.5 * q * r["phi"]).max() < 1e-9 * np.abs(q * r["phi"]).max()
+    assert np.abs(Wat.sum(axis=2) - r["W"]).max() < 1e-11 * np.abs(r["W"]).max()
+    assert np.abs(Wat - np.transpose(Wat, (1, 0, 2))).max() < 1e-12
+    assert np.abs(Wat[0, 1]).max() > 1e-3 * np.abs(Wat).max()          # off-diagonal elements are exercised
+
+
+def test_atom_virial_pppm_converges_to_ewald_and_sums_to_total(oracle):
+    """Eq. 39 (six inverse FFTs) against Eq. 20: same limit as the mesh is refined; sum_i W_i = W^k exactly (the
+    adjointness of spreading and back-interpolation)."""
+    L = 16.0
+    pos, q = _random_charges(120, L, 9)
+    box = np.diag([L, L, L]).ravel()
+    ew = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=1, alpha=0.3, ewald_nmax2=169), want_atom_virial=True)
+    errs = []
+    for g in (16, 32, 64):
+        pm = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=2, alpha=0.3, grid=(g, g, g)), want_atom_virial=True)
+        assert np.abs(pm["W_atom"].reshape(3, 3, -1).sum(axis=2) - pm["W"]).max() < 1e-11 * np.abs(pm["W"]).max()
+        errs.append(rel_rms(pm["W_atom"], ew["W_atom"]))
+    assert errs[0] < 2e-4 and errs[1] < 1e-5 and errs[2] < 1e-6 and errs[2] < errs[1] < errs[0]
+
+
+def test_atom_virial_pair_part_vs_site_energy_derivatives(oracle):
+    """Eq. 12, W_i = sum_j r_ij (x) F_ji, with the partial force F_ji = dU_j / dr_ji = dU_j / dr_i (Eq. 14; the site
+    energy of j depends on r_i only through r_ji): finite differences of the oracle's SITE ENERGIES fix which atom a
+    pair term belongs to.  Cluster without electrostatics (the descriptor part of the path)."""
+    m, p, pos, types, box = _cluster()
+    n = pos.shape[1]
+    es = I.EsDesc(method=0)
+    out = oracle.compute(m, p, es, pos, types, box, use_bins=False, want_atom_virial=True)
+    Wat = out["virial_atom"].reshape(3, 3, n)
+    h = 1e-5
+    ref = np.zeros((3, 3, n))
+    for i in range(n):
+        for b in range(3):
+            x1, x2 = pos.copy(), pos.copy()
+            x1[b, i] += h
+            x2[b, i] -= h
+            dU = (oracle.compute(m, p, es, x1, types, box, use_bins=False, debug=True)["U_i"]
+                  - oracle.compute(m, p, es, x2, types, box, use_bins=False, debug=True)["U_i"]) / (2 * h)
+            for j in range(n):
+                if j != i:
+                    ref[:, b, i] += (pos[:, j] - pos[:, i]) * dU[j]          # r_ij,a * dU_j/dr_i,b
+    assert np.abs(Wat - ref).max() < 2e-8 * max(1.0, np.abs(ref).max())
+    assert np.abs(Wat.sum(axis=2) - out["virial"]).max() < 1e-12 * max(1.0, np.abs(out["virial"]).max())
+    # the partition differs from "every atom keeps its own -r_ij (x) F_ij": the test would see that assignment
+    alt = np.zeros((3, 3, n))
+    for j in range(n):
+        for b in range(3):
+            x1, x2 = pos.copy(), pos.copy()
+            x1[b, j] += h
+            x2[b, j] -= h
+            dU = (oracle.compute(m, p, es, x1, types, box, use_bins=False, debug=True)["U_i"]
+                  - oracle.compute(m, p, es, x2, types, box, use_bins=False, debug=True)["U_i"]) / (2 * h)
+            for i in range(n):
+                if i != j:
+                    alt[:, b, i] += -(pos[:, j] - pos[:, i]) * dU[i]         # -r_ij,a * F_ij,b kept by atom i
+    assert np.abs(alt - ref).max() > 1e-3
+
+
+@pytest.mark.parametrize("mode,method", [(1, 1), (2, 1), (2, 2)])
+def test_atom_virial_full_model_sums_to_total(oracle, mode, method):
+    """All parts together (descriptor + dynamic-charge partial forces, Eq. 15 / 20 / 39 static parts)."""
+    w = I.config0(mode=mode)
+    if method == 2:
+        w.es = replace(w.es, method=2, grid=(16, 16, 16))
+    out = oracle.compute_workload(w, use_bins=False, want_atom_virial=True)
+    Wat = out["virial_atom"].reshape(3, 3, -1)
+    assert np.abs(Wat.sum(axis=2) - out["virial"]).max() < 1e-11 * np.abs(out["virial"]).max()
+    assert np.abs(Wat).max() > 1e-2
