@@ -71,7 +71,8 @@ typedef struct {
 } qnep_es_desc;
 
 /* bit flags of `want` */
-enum { QNEP_WANT_ENERGY = 1, QNEP_WANT_FORCES = 2, QNEP_WANT_VIRIAL = 4, QNEP_WANT_CHARGES = 8, QNEP_WANT_BEC = 16 };
+enum { QNEP_WANT_ENERGY = 1, QNEP_WANT_FORCES = 2, QNEP_WANT_VIRIAL = 4, QNEP_WANT_CHARGES = 8, QNEP_WANT_BEC = 16,
+       QNEP_WANT_ATOM_VIRIAL = 32 /* qnep_compute_atom_virial only */ };
 
 /* stages reported by qnep_get_timings (milliseconds of the last qnep_compute) */
 enum {
@@ -146,6 +147,23 @@ int qnep_set_neighbor_capacity(qnep_handle *h, int32_t cap_radial, int32_t cap_a
 int qnep_compute(qnep_handle *h, int64_t n_atoms, const double *pos_dev, const int32_t *types_dev,
                  const double box[9], uint32_t want, double *energy_dev, double *forces_dev,
                  double *virial_dev, double *charges_dev, double *bec_dev, void *cuda_stream);
+
+/*
+ * qnep_compute_atom_virial: qnep_compute with the per-atom virial as an additional output:
+ *   W_i = sum_j r_ij (x) F_ji                      for all partial forces: descriptor part (Eq. 14), dynamic-charge parts
+ *                                                  (Eq. 16, 19 / 38, 23, folded) and the real-space static part (Eq. 15)
+ *                                                  -- PAPER.md :130-132 Eq. 12, :149;
+ *       + W_i^{k,static}                           Ewald: Re[ sum_k G q_i e^{ik.r_i} S(k) B ] / (4 pi eps0), PAPER.md
+ *                                                  :179-185 Eq. 20-21 (real part: DESIGN.md reading G4);
+ *                                                  PPPM: q_i / (4 pi eps0) sum_s W(r_i - r_s) F^-1[S G^opt B]_s,
+ *                                                  :297-302 Eq. 39, six more inverse transforms.
+ *   atom_virial_dev [9][N] float64 DEVICE, component-major, entry (3 a + b) * N + i = W_{i,ab}, eV; owned by the caller.
+ *   sum_i W_i equals virial_dev up to rounding (Eq. 22).  `want` selects the other outputs as in qnep_compute
+ *   (QNEP_WANT_BEC is not available here); forces are always evaluated.  Errors as qnep_compute.
+ */
+int qnep_compute_atom_virial(qnep_handle *h, int64_t n_atoms, const double *pos_dev, const int32_t *types_dev,
+                             const double box[9], uint32_t want, double *energy_dev, double *forces_dev,
+                             double *virial_dev, double *charges_dev, double *atom_virial_dev, void *cuda_stream);
 
 /*
  * qnep_compute_host: the same evaluation with HOST buffers: copies positions and types to the device,

@@ -26,7 +26,7 @@ QNEP_ERR_OOM = -6
 ERROR_NAMES = {0: "OK", -1: "INVALID_ARG", -2: "UNSUPPORTED", -3: "NEIGHBOR_OVERFLOW", -4: "SKIN_VIOLATED",
                -5: "CUDA", -6: "OOM"}
 
-WANT_ENERGY, WANT_FORCES, WANT_VIRIAL, WANT_CHARGES, WANT_BEC = 1, 2, 4, 8, 16
+WANT_ENERGY, WANT_FORCES, WANT_VIRIAL, WANT_CHARGES, WANT_BEC, WANT_ATOM_VIRIAL = 1, 2, 4, 8, 16, 32
 WANT_ALL = WANT_ENERGY | WANT_FORCES | WANT_VIRIAL | WANT_CHARGES
 
 TIMING_NAMES = ["neighbor", "prep", "desc_radial", "desc_angular", "nn", "realspace", "reciprocal",
@@ -35,7 +35,7 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
-               "qnep_compute", "qnep_compute_host", "qnep_md_run", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
+               "qnep_compute", "qnep_compute_atom_virial", "qnep_compute_host", "qnep_md_run", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
                "qnep_fma_peak",
                "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
@@ -84,6 +84,8 @@ def load_library():
         f = getattr(lib, name)
         f.restype = C.c_int
         f.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), u32, vp, vp, vp, vp, vp, vp]
+    lib.qnep_compute_atom_virial.restype = C.c_int
+    lib.qnep_compute_atom_virial.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), u32, vp, vp, vp, vp, vp, vp]
     lib.qnep_md_run.restype = C.c_int
     lib.qnep_md_run.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i32, vp, vp]
     lib.qnep_check.restype = C.c_int
@@ -205,6 +207,29 @@ class QNEP:
         self._ok(rc)
         if check:
             self.check()
+        return out
+
+    def compute_atom_virial(self, pos, types, box, want=WANT_ALL, stream=None):
+        """qnep_compute_atom_virial: the outputs of compute() plus "virial_atom" [9][N] (Eq. 12, 20, 39)."""
+        import torch
+        assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous() and pos.shape[0] == 3
+        assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
+        n = pos.shape[1]
+        out = {"virial_atom": torch.empty((9, n), dtype=torch.float64, device=pos.device)}
+        def buf(key, flag, shape):
+            if not (want & flag):
+                return None
+            out[key] = torch.empty(shape, dtype=torch.float64, device=pos.device)
+            return out[key]
+        e = buf("energy", WANT_ENERGY, (1,))
+        f = buf("forces", WANT_FORCES, (3, n))
+        w = buf("virial", WANT_VIRIAL, (9,))
+        q = buf("charges", WANT_CHARGES, (n,))
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        rc = self._lib.qnep_compute_atom_virial(self._h, n, ptr(pos), ptr(types), _box(box), want, ptr(e), ptr(f), ptr(w),
+                                                ptr(q), ptr(out["virial_atom"]), self._stream(stream))
+        self._ok(rc)
+        self.check()
         return out
 
     def compute_host(self, pos, types, box, want=WANT_ALL, stream=None):

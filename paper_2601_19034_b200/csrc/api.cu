@@ -130,7 +130,8 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_phir, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_phi, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_Fs, n * 3))) return rc;
-        if ((rc = dev_alloc(h, &h->d_Facc, n * 9))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Facc, n * 12))) return rc;
+        if (h->d_Wat) { cudaFree(h->d_Wat); h->d_Wat = nullptr; }
         if ((rc = dev_alloc(h, &h->d_Fmd, n * 3))) return rc;
         h->N = N; h->capR = capR; h->capLR = capLR; h->capLA = capLA;
         QNEP_CUDA_OK(h, cudaMemset(h->d_nlvR, 0, sizeof(int) * n));
@@ -420,9 +421,12 @@ bool plan_pipeline(qnep_handle* h)
 
 // the pipeline proper (enqueue only); `timed` = false leaves out the stage events (stream capture: qnep_md_run's graphs)
 int enqueue_pipeline(qnep_handle* h, bool rebuild, bool timed, int64_t N, const double* pos, const int32_t* types, uint32_t want,
-                     double* energy, double* forces, double* virial, double* charges, double* bec, cudaStream_t s)
+                     double* energy, double* forces, double* virial, double* charges, double* bec, cudaStream_t s,
+                     double* atom_virial = nullptr)
 {
     int rc;
+    const bool atomv = (want & QNEP_WANT_ATOM_VIRIAL) && atom_virial;
+    if (atomv && !h->d_Wat) QNEP_CUDA_OK(h, cudaMalloc(&h->d_Wat, sizeof(float) * 9 * (size_t)N));
     cudaEvent_t* ev = nullptr;
     if (timed) {
         ev = h->ring.data() + (size_t)(h->prof_count % qnep_handle::RING) * qnep_handle::NEV;
@@ -442,20 +446,25 @@ int enqueue_pipeline(qnep_handle* h, bool rebuild, bool timed, int64_t N, const 
     QNEP_STAGE(4);
     if ((rc = qnep_launch_nn(h, (want & QNEP_WANT_CHARGES) ? charges : nullptr, s))) return rc;
     QNEP_STAGE(5);
-    if (h->es.method != 0 && h->model.mode == 1) { if ((rc = qnep_launch_realspace(h, s))) return rc; }
+    if (h->es.method != 0 && h->model.mode == 1) { if ((rc = qnep_launch_realspace(h, atomv, s))) return rc; }
     QNEP_STAGE(6);
-    if (h->es.method == 1) { if ((rc = qnep_launch_ewald(h, pos, s))) return rc; }
-    else if (h->es.method == 2) { if ((rc = qnep_launch_pppm(h, (want & QNEP_WANT_VIRIAL) != 0, s))) return rc; }
-    else QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
+    if (h->es.method == 1) { if ((rc = qnep_launch_ewald(h, pos, atomv, s))) return rc; }
+    else if (h->es.method == 2) {
+        if ((rc = qnep_launch_pppm(h, (want & QNEP_WANT_VIRIAL) != 0, s))) return rc;
+        if (atomv) { if ((rc = qnep_launch_pppm_atom_virial(h, s))) return rc; }
+    } else {
+        QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
+        if (atomv) QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Wat, 0, sizeof(float) * 9 * N, s));
+    }
     if ((rc = qnep_launch_phi_finalize(h, s))) return rc;
-    const bool need_forces = (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
-    const bool need_virial = (want & QNEP_WANT_VIRIAL) != 0;
+    const bool need_forces = atomv || (want & (QNEP_WANT_FORCES | QNEP_WANT_VIRIAL)) != 0;
+    const bool need_virial = atomv || (want & QNEP_WANT_VIRIAL) != 0;
     QNEP_STAGE(7);
     if (need_forces) {
-        if ((rc = qnep_launch_force_angular(h, false, need_virial, s))) return rc;     // bracketed alone by ev[7], ev[8]
+        if ((rc = qnep_launch_force_angular(h, false, need_virial, atomv, s))) return rc;     // bracketed alone by ev[7], ev[8]
         QNEP_STAGE(8);
         double* fout = ((want & QNEP_WANT_FORCES) && forces) ? forces : h->d_Fmd;
-        if ((rc = qnep_launch_force_radial(h, false, need_virial, fout, s))) return rc;
+        if ((rc = qnep_launch_force_radial(h, false, need_virial, fout, atomv ? atom_virial : nullptr, s))) return rc;
     } else {
         QNEP_STAGE(8);
     }
@@ -464,8 +473,8 @@ int enqueue_pipeline(qnep_handle* h, bool rebuild, bool timed, int64_t N, const 
     h->launches += 1;
     QNEP_STAGE(9);
     if ((want & QNEP_WANT_BEC) && bec) {
-        if ((rc = qnep_launch_force_angular(h, true, false, s))) return rc;
-        if ((rc = qnep_launch_force_radial(h, true, false, bec, s))) return rc;
+        if ((rc = qnep_launch_force_angular(h, true, false, false, s))) return rc;
+        if ((rc = qnep_launch_force_radial(h, true, false, bec, nullptr, s))) return rc;
     }
     QNEP_STAGE(10);
 #undef QNEP_STAGE
@@ -600,6 +609,26 @@ int qnep_compute(qnep_handle* h, int64_t n_atoms, const double* pos_dev, const i
     if ((rc = ensure_workspace(h, n_atoms, box))) return rc;
     h->md_have_forces = false;
     return run_pipeline(h, n_atoms, pos_dev, types_dev, want, energy_dev, forces_dev, virial_dev, charges_dev, bec_dev, s);
+}
+
+int qnep_compute_atom_virial(qnep_handle* h, int64_t n_atoms, const double* pos_dev, const int32_t* types_dev, const double box[9],
+                             uint32_t want, double* energy_dev, double* forces_dev, double* virial_dev, double* charges_dev,
+                             double* atom_virial_dev, void* cuda_stream)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (!atom_virial_dev) { h->err = "qnep_compute_atom_virial: null output pointer"; return QNEP_ERR_INVALID_ARG; }
+    if (want & QNEP_WANT_BEC) { h->err = "qnep_compute_atom_virial: QNEP_WANT_BEC is not available in this call"; return QNEP_ERR_INVALID_ARG; }
+    int rc = check_args(h, n_atoms, pos_dev, types_dev, box, want, energy_dev, forces_dev, virial_dev, charges_dev, nullptr);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (h->flags_pending && cudaEventQuery(h->ev_flags) == cudaSuccess) {
+        if ((rc = consume_flags(h))) return rc;
+    }
+    if ((rc = ensure_workspace(h, n_atoms, box))) return rc;
+    h->md_have_forces = false;
+    const bool rebuild = plan_pipeline(h);
+    return enqueue_pipeline(h, rebuild, true, n_atoms, pos_dev, types_dev, want | QNEP_WANT_ATOM_VIRIAL, energy_dev, forces_dev, virial_dev,
+                            charges_dev, nullptr, s, atom_virial_dev);
 }
 
 int qnep_md_reset(qnep_handle* h)
@@ -879,7 +908,7 @@ void qnep_destroy(qnep_handle* h)
     if (h->md_fence) cudaEventDestroy(h->md_fence);
     free_workspace(h);
     void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_mbcnt, h->d_mbstart, h->d_mbfill, h->d_sums, h->d_flags, h->d_kvec,
-                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_half, h->d_cm1, h->d_cm2, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
+                    h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_half, h->d_cm1, h->d_cm2, h->d_cm3, h->d_Wat, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
                     h->d_htypes, h->d_hout};
     for (void* p : ptrs) if (p) cudaFree(p);
     if (h->h_flags) cudaFreeHost(h->h_flags);

@@ -548,7 +548,9 @@ __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const do
         vz = fmaf(G_, (GZ), vz);                                             \
     }
 
-template <int T, bool BEC, bool VIRIAL>
+// ATOMV (with VIRIAL, not BEC): the pair term -r_ij (x) F_ij belongs to the per-atom virial of atom j (Eq. 12:
+// W_j = sum_i r_ji (x) F_ij) and is scattered to rows 3..11 of Facc.
+template <int T, bool BEC, bool VIRIAL, bool ATOMV = false>
 __global__ void __launch_bounds__(ANG_BLOCK, BEC || VIRIAL ? 4 : 6)
 k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
                 const float* __restrict__ cA, const float* __restrict__ cR, float rcinv, const float* __restrict__ FpU,
@@ -702,6 +704,11 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                     W[3] = fmaf(dy, fx, W[3]); W[4] = fmaf(dy, fy, W[4]); W[5] = fmaf(dy, fz, W[5]);
                     W[6] = fmaf(dz, fx, W[6]); W[7] = fmaf(dz, fy, W[7]); W[8] = fmaf(dz, fz, W[8]);
                 }
+                if (ATOMV) {
+                    const float w9[9] = {dx * fx, dx * fy, dx * fz, dy * fx, dy * fy, dy * fz, dz * fx, dz * fy, dz * fz};
+#pragma unroll
+                    for (int a = 0; a < 9; ++a) atomicAdd(&Facc[(int64_t)(3 + a) * N + j], -w9[a]);
+                }
             }
         }
         if (BEC) {
@@ -739,13 +746,15 @@ __device__ __forceinline__ void ldg256(const float* p, float (&v)[8])
                  : "l"(p));
 }
 
-template <int T, bool BEC, bool VIRIAL>
+// ATOMV (with VIRIAL): per-atom virial W_i = sum_j r_ij (x) F_ji with the radial F_ji = -s_ji rhat_ij, plus the angular
+// terms scattered by k_force_angular (Facc rows 3..11) and the static electrostatic parts (Wat), to atomv_out [9][N].
+template <int T, bool BEC, bool VIRIAL, bool ATOMV = false>
 __global__ void __launch_bounds__(RAD_BLOCK)
 k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const float4* __restrict__ recB,
                const float4* __restrict__ xyzt, const int4* __restrict__ lvR, int capLR, const int* __restrict__ nlvR,
                const int* __restrict__ lvRend, float rcinv, const float* __restrict__ Facc, const float* __restrict__ Fs,
                const float* __restrict__ q, float sqrt_eps, const int* __restrict__ sidx, double* __restrict__ out,
-               double* __restrict__ sums)
+               double* __restrict__ sums, const float* __restrict__ Wat, double* __restrict__ atomv_out)
 {
     __shared__ float4 sh_shift[27];
     __shared__ int4 sh_w[RAD_LV][RAD_BLOCK];
@@ -755,8 +764,11 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
     const int tid = threadIdx.x;
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
     float W[9];
+    float Wa[ATOMV ? 9 : 1];
 #pragma unroll
     for (int a = 0; a < 9; ++a) W[a] = 0.f;
+#pragma unroll
+    for (int a = 0; a < (ATOMV ? 9 : 1); ++a) Wa[a] = 0.f;
     if (p < N) {
         const int n = nlvR[p];
         const int n4 = (n + 3) >> 2;
@@ -849,6 +861,12 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                             W[3] = fmaf(dy, wx, W[3]); W[4] = fmaf(dy, wy, W[4]); W[5] = fmaf(dy, wz, W[5]);
                             W[6] = fmaf(dz, wx, W[6]); W[7] = fmaf(dz, wy, W[7]); W[8] = fmaf(dz, wz, W[8]);
                         }
+                        if (ATOMV) {
+                            const float ax = -sji * ux, ay = -sji * uy, az = -sji * uz;  // F_ji = s_ji rhat_ji
+                            Wa[0] = fmaf(dx, ax, Wa[0]); Wa[1] = fmaf(dx, ay, Wa[1]); Wa[2] = fmaf(dx, az, Wa[2]);
+                            Wa[3] = fmaf(dy, ax, Wa[3]); Wa[4] = fmaf(dy, ay, Wa[4]); Wa[5] = fmaf(dy, az, Wa[5]);
+                            Wa[6] = fmaf(dz, ax, Wa[6]); Wa[7] = fmaf(dz, ay, Wa[7]); Wa[8] = fmaf(dz, az, Wa[8]);
+                        }
                     }
                     // the record registers are free again: request the record of slot s + 4 into them
                     if (s + 4 < n) {
@@ -874,6 +892,11 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
             out[io] = (double)Fx + (double)Facc[p] + (double)Fs[p];
             out[N + io] = (double)Fy + (double)Facc[N + p] + (double)Fs[N + p];
             out[2 * N + io] = (double)Fz + (double)Facc[2 * N + p] + (double)Fs[2 * N + p];
+            if (ATOMV) {
+#pragma unroll
+                for (int a = 0; a < 9; ++a)
+                    atomv_out[(int64_t)a * N + io] = (double)Wa[a] + (double)Facc[(int64_t)(3 + a) * N + p] + (double)Wat[(int64_t)a * N + p];
+            }
         }
     }
     if (!BEC && VIRIAL) {
@@ -969,18 +992,21 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
     return QNEP_OK;
 }
 
-int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_t s)
+int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, bool atomv, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + ANG_BLOCK - 1) / ANG_BLOCK);
     const float rcinv = (float)(1.0 / h->model.rc_a);
-    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Facc, 0, sizeof(float) * (bec ? 9 : 3) * N, s));
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Facc, 0, sizeof(float) * (bec ? 9 : (atomv ? 12 : 3)) * N, s));
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
 #define QNEP_FA(B, V) k_force_angular<T, B, V><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv, \
                                                                          h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf, \
                                                                          h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums)
         if (bec) QNEP_FA(true, false);
+        else if (atomv) k_force_angular<T, false, true, true><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv,
+                                                                                       h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf,
+                                                                                       h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums);
         else if (virial) QNEP_FA(false, true);
         else QNEP_FA(false, false);
 #undef QNEP_FA
@@ -991,7 +1017,7 @@ int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_
 }
 
 // must follow qnep_launch_force_angular of the same mode (it writes the gather records and the angular accumulator)
-int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, cudaStream_t s)
+int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, double* atomv_out, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + RAD_BLOCK - 1) / RAD_BLOCK);
@@ -1000,8 +1026,11 @@ int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out,
         constexpr int T = decltype(t)::value;
 #define QNEP_FR(B, V) k_force_radial<T, B, V><<<nb, RAD_BLOCK, 0, s>>>(N, h->geo, h->d_recA, h->d_recB, h->d_xyzt, h->d_lvR, h->capLR, h->d_nlvR, \
                                                                         h->d_lvRend, rcinv, h->d_Facc, h->d_Fs, h->d_q,                  \
-                                                                        (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums)
+                                                                        (float)h->model.sqrt_eps_inf, h->d_sidx, out, h->d_sums, nullptr, nullptr)
         if (bec) QNEP_FR(true, false);
+        else if (atomv_out) k_force_radial<T, false, true, true><<<nb, RAD_BLOCK, 0, s>>>(N, h->geo, h->d_recA, h->d_recB, h->d_xyzt, h->d_lvR, h->capLR, h->d_nlvR,
+                                                                                          h->d_lvRend, rcinv, h->d_Facc, h->d_Fs, h->d_q, (float)h->model.sqrt_eps_inf,
+                                                                                          h->d_sidx, out, h->d_sums, h->d_Wat, atomv_out);
         else if (virial) QNEP_FR(false, true);
         else QNEP_FR(false, false);
 #undef QNEP_FR

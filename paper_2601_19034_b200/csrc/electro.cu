@@ -34,7 +34,7 @@ __device__ __forceinline__ double block_sum(double v, double* sh)
 __global__ void __launch_bounds__(128)
 k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __restrict__ nl, int cap,
             const int* __restrict__ nn, const float* __restrict__ q, float alpha, float* __restrict__ phir,
-            float* __restrict__ Fs, double* __restrict__ sums)
+            float* __restrict__ Fs, double* __restrict__ sums, float* __restrict__ Wat /* [9][N] or null */)
 {
     __shared__ float4 sh_shift[27];
     __shared__ double sh_red[32];
@@ -79,6 +79,13 @@ k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* 
         phir[p] = Kc * phi;
         Fs[p] = Kc * Fx; Fs[N + p] = Kc * Fy; Fs[2 * N + p] = Kc * Fz;
         Ur = 0.5f * Kc * qi * phi;
+        if (Wat) {
+            // per-atom virial of the real-space static part: W_i = sum_j r_ij (x) F_ji (Eq. 12 with Eq. 15)
+            const float h = 0.5f * Kc;
+            Wat[p] = h * W[0]; Wat[N + p] = h * W[1]; Wat[2 * N + p] = h * W[2];
+            Wat[3 * N + p] = h * W[1]; Wat[4 * N + p] = h * W[3]; Wat[5 * N + p] = h * W[4];
+            Wat[6 * N + p] = h * W[2]; Wat[7 * N + p] = h * W[4]; Wat[8 * N + p] = h * W[5];
+        }
     }
     const double u = block_sum((double)Ur, sh_red);
     if (threadIdx.x == 0) atomicAdd(&sums[SUM_U_R], u);
@@ -207,14 +214,16 @@ k_ewald_energy(int nk, const float4* __restrict__ kvec, const double2* __restric
 }
 
 // phi^k_i = 2K sum_k G Re[S e^{ik.r_i}] (Eq. 19 bracket), F^k_i = 2K q_i sum_k k G Im[S e^{ik.r_i}] (Eq. 18)
+template <bool ATOMV>
 __global__ void __launch_bounds__(128)
 k_ewald_atoms(int64_t N, int nk, int nmax, const float2* __restrict__ eph, const int* __restrict__ kint,
               const float4* __restrict__ kvec, const double2* __restrict__ S, const float* __restrict__ q, int add_to_Fs,
-              float* __restrict__ phik, float* __restrict__ Fs)
+              float* __restrict__ phik, float* __restrict__ Fs, float inv4a2, int add_to_Wat, float* __restrict__ Wat)
 {
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
     float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+    float wv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};           // xx, xy, xz, yy, yz, zz of sum_k G Re[S e^{ik.r}] B (Eq. 20-21)
     for (int k = 0; k < nk; ++k) {
         const float2 e = phase_of(eph, N, nmax, p, kint[k]);
         const float4 kv = kvec[k];
@@ -225,22 +234,39 @@ k_ewald_atoms(int64_t N, int nk, int nmax, const float2* __restrict__ eph, const
         phi = fmaf(kv.w, re, phi);
         const float gi = kv.w * im;
         fx = fmaf(gi, kv.x, fx); fy = fmaf(gi, kv.y, fy); fz = fmaf(gi, kv.z, fz);
+        if (ATOMV) {
+            const float gr = kv.w * re;
+            const float k2 = kv.x * kv.x + kv.y * kv.y + kv.z * kv.z;
+            const float bf = gr * (2.f * inv4a2 + 2.f / k2);
+            wv[0] += gr - bf * kv.x * kv.x; wv[1] -= bf * kv.x * kv.y; wv[2] -= bf * kv.x * kv.z;
+            wv[3] += gr - bf * kv.y * kv.y; wv[4] -= bf * kv.y * kv.z; wv[5] += gr - bf * kv.z * kv.z;
+        }
     }
     const float c = 4.f * (float)QNEP_K_COULOMB;              // 2K, times 2 for the -k half
     phik[p] = c * phi;
     const float cq = c * q[p];
     if (add_to_Fs) { Fs[p] += cq * fx; Fs[N + p] += cq * fy; Fs[2 * N + p] += cq * fz; }
     else { Fs[p] = cq * fx; Fs[N + p] = cq * fy; Fs[2 * N + p] = cq * fz; }
+    if (ATOMV) {
+        // K q_i sum over the FULL sphere = 2 K q_i sum over the stored half
+        const float cw = 2.f * (float)QNEP_K_COULOMB * q[p];
+        const int row[9] = {0, 1, 2, 1, 3, 4, 2, 4, 5};
+#pragma unroll
+        for (int a = 0; a < 9; ++a) {
+            const float v = cw * wv[row[a]];
+            if (add_to_Wat) Wat[(int64_t)a * N + p] += v; else Wat[(int64_t)a * N + p] = v;
+        }
+    }
 }
 
 }  // namespace
 
-int qnep_launch_realspace(qnep_handle* h, cudaStream_t s)
+int qnep_launch_realspace(qnep_handle* h, bool atomv, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
     k_realspace<<<nb, 128, 0, s>>>(N, h->geo, h->d_xyzt, h->d_lvR, h->capLR, h->d_nlvR, h->d_q, (float)h->alpha, h->d_phir, h->d_Fs,
-                                   h->d_sums);
+                                   h->d_sums, atomv ? h->d_Wat : nullptr);
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;
@@ -299,10 +325,12 @@ int qnep_setup_ewald(qnep_handle* h)
     return QNEP_OK;
 }
 
-int qnep_launch_ewald(qnep_handle* h, const double* pos, cudaStream_t s)
+int qnep_launch_ewald(qnep_handle* h, const double* pos, bool atomv, cudaStream_t s)
 {
     const int64_t N = h->N;
+    const int addw = h->model.mode == 1 ? 1 : 0;       // mode 1: k_realspace has written the rows of d_Wat
     if (h->nk == 0) {
+        if (atomv && !addw) QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Wat, 0, sizeof(float) * 9 * N, s));
         QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_phik, 0, sizeof(float) * N, s));
         if (h->model.mode != 1) QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Fs, 0, sizeof(float) * 3 * N, s));
         return QNEP_OK;
@@ -312,8 +340,13 @@ int qnep_launch_ewald(qnep_handle* h, const double* pos, cudaStream_t s)
     k_ewald_sfac<<<h->nk, 256, 0, s>>>(N, h->ew_nmax, h->d_ephase, h->d_kint, h->d_q, h->d_S);
     k_ewald_energy<<<std::min(64, (h->nk + 255) / 256), 256, 0, s>>>(h->nk, h->d_kvec, h->d_S, 1.0 / (4.0 * h->alpha * h->alpha),
                                                                     h->d_sums);
-    k_ewald_atoms<<<nb, 128, 0, s>>>(N, h->nk, h->ew_nmax, h->d_ephase, h->d_kint, h->d_kvec, h->d_S, h->d_q,
-                                     h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs);
+    const float inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    if (atomv)
+        k_ewald_atoms<true><<<nb, 128, 0, s>>>(N, h->nk, h->ew_nmax, h->d_ephase, h->d_kint, h->d_kvec, h->d_S, h->d_q,
+                                               h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs, inv4a2, addw, h->d_Wat);
+    else
+        k_ewald_atoms<false><<<nb, 128, 0, s>>>(N, h->nk, h->ew_nmax, h->d_ephase, h->d_kint, h->d_kvec, h->d_S, h->d_q,
+                                                h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs, inv4a2, 0, nullptr);
     h->launches += 4;
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;

@@ -489,6 +489,82 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
     (void)n0;
 }
 
+// ---- 3''. per-atom virial pass along x (Eq. 39): forward FFT, phi = G^opt S, three inverse FFTs ---------------
+// The six real fields F^-1[S G^opt B_ab] ("six backward FFTs", :302) are packed pairwise into three complex transforms,
+//   M1 = W_xx + i W_yy,   M2 = W_zz + i W_xy,   M3 = W_xz + i W_yz,      B_ab = delta_ab - (2 / 4 alpha^2 + 2 / k^2) k_a k_b
+// (B is real and even in k, so each product phi B_ab is the spectrum of a real field).  Full spectrum in M3 (after the
+// forward z and y passes), in-place line by line for M3.
+template <int R1, int R2>
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+k_fft_x_virial(int n0, int n1, int n2, float2* __restrict__ M1, float2* __restrict__ M2, float2* __restrict__ M3,
+               const float2* __restrict__ twg, const float* __restrict__ tabA, const float* __restrict__ tabK,
+               float c0 /* 2 pi / Omega */, float inv4a2)
+{
+    using S = Split<R1, R2>;
+    using SI = Split<R2, R1>;
+    constexpr int LPMAX = S::LP > SI::LP ? S::LP : SI::LP;
+    extern __shared__ __align__(16) float2 smem[];
+    float2* tw = smem + LINES * LPMAX;
+    float* tA = reinterpret_cast<float*>(tw + S::N);
+    float* tK = tA + S::N;
+    load_twiddles(tw, twg, S::N);
+    for (int i = threadIdx.x; i < S::N; i += blockDim.x) { tA[i] = tabA[i]; tK[i] = tabK[i]; }
+    __syncthreads();
+    const int b = threadIdx.x % LINES, u = threadIdx.x / LINES;
+    const TileAddr ta = strided_tile(0, n0, n1, n2, blockIdx.x);
+    const int zc = n2 / LINES;
+    const int iy = (int)(blockIdx.x / zc), iz = (int)(blockIdx.x % zc) * LINES + b;
+    float2 ph[S::E], v[S::E];
+    {
+        const float2* p = M3 + ta.base + b;
+#pragma unroll
+        for (int d = 0; d < S::D1; ++d)
+#pragma unroll
+            for (int m = 0; m < R1; ++m) ph[d * R1 + m] = p[((u + S::TPL * d) + R2 * m) * ta.stride];
+    }
+    line_fft<R1, R2, -1>(ph, smem + b * S::LP, u, tw);
+    const float ky = tabK[FFT_MAXN + iy], kz = tabK[2 * FFT_MAXN + iz];
+    const float Ayz = c0 * tabA[FFT_MAXN + iy] * tabA[2 * FFT_MAXN + iz];
+    const float kyz2 = ky * ky + kz * kz;
+#pragma unroll
+    for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+        for (int k1 = 0; k1 < R2; ++k1) {
+            const int ix = (u + S::TPL * d) + R1 * k1;
+            const float kx = tK[ix];
+            const float k2 = kx * kx + kyz2;
+            const float G = k2 > 0.f ? __fdividef(Ayz * tA[ix], k2) : 0.f;
+            ph[d * R2 + k1].x *= G; ph[d * R2 + k1].y *= G;
+        }
+    float2* const Ms[3] = {M1, M2, M3};
+#pragma unroll
+    for (int pair = 0; pair < 3; ++pair) {
+#pragma unroll
+        for (int d = 0; d < S::D2; ++d)
+#pragma unroll
+            for (int k1 = 0; k1 < R2; ++k1) {
+                const int ix = (u + S::TPL * d) + R1 * k1;
+                const float kx = tK[ix];
+                const float k2 = kx * kx + kyz2;
+                const float bf = k2 > 0.f ? 2.f * inv4a2 + __fdividef(2.f, k2) : 0.f;
+                const float one = k2 > 0.f ? 1.f : 0.f;
+                float B1, B2;
+                if (pair == 0) { B1 = one - bf * kx * kx; B2 = one - bf * ky * ky; }
+                else if (pair == 1) { B1 = one - bf * kz * kz; B2 = -bf * kx * ky; }
+                else { B1 = -bf * kx * kz; B2 = -bf * ky * kz; }
+                const float2 f = ph[d * R2 + k1];
+                v[d * R2 + k1] = make_float2(f.x * B1 - f.y * B2, f.x * B2 + f.y * B1);
+            }
+        // inverse along x with the swapped split <R2, R1>: its stage-1 layout is the layout we hold
+        line_fft<R2, R1, +1>(v, smem + b * SI::LP, u, tw);
+        float2* p = Ms[pair] + ta.base + b;
+#pragma unroll
+        for (int d = 0; d < SI::D2; ++d)
+#pragma unroll
+            for (int k1 = 0; k1 < R1; ++k1) p[((u + SI::TPL * d) + R2 * k1) * ta.stride] = v[d * R1 + k1];
+    }
+}
+
 // ---- last inverse pass along z: M1, M2 -> interleaved real fields (Phi, E_x, E_y, E_z) -------------------
 template <int R1, int R2>
 __global__ void __launch_bounds__(Split<R1, R2>::THREADS)
@@ -529,10 +605,15 @@ k_fft_z_fields(const float2* __restrict__ M1, const float2* __restrict__ M2, flo
 constexpr int GATHER_GROUP = 8;
 constexpr int GATHER_BLOCK = 128;
 
+// VMODE (per-atom virial pass, Eq. 39): the four interpolated values are K q_i times four virial components; rows.x..w /
+// mirror.x..w name the rows of Wat [9][N] they are added to (-1: none).
+struct GatherRows { int row[4], mirror[4]; };
+
+template <bool VMODE>
 __global__ void __launch_bounds__(GATHER_BLOCK)
 k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __restrict__ mi0, const int* __restrict__ cmi,
          const float* __restrict__ q, const float4* __restrict__ field, int add_to_Fs,
-         float* __restrict__ phik, float* __restrict__ Fs)
+         float* __restrict__ phik, float* __restrict__ Fs, GatherRows vr, float* __restrict__ Wat)
 {
     __shared__ float s_w[3][5][GATHER_BLOCK];
     __shared__ int s_i[3][5][GATHER_BLOCK];       // x: index * n1 * n2, y: index * n2, z: index
@@ -593,7 +674,17 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
     }
     __syncthreads();
     if (p0 + t >= N) return;
-    const int64_t p = cmi[p0 + t];                         // the block walked cell-major ranks; outputs in sorted order
+    const int64_t p = cmi[p0 + t];                         // the block walked mesh-bin ranks; outputs in sorted order
+    if (VMODE) {
+        const float cw = (float)QNEP_K_COULOMB * q[p];     // Eq. 39
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const float v = cw * s_out[k][t];
+            if (vr.row[k] >= 0) Wat[(int64_t)vr.row[k] * N + p] += v;
+            if (vr.mirror[k] >= 0) Wat[(int64_t)vr.mirror[k] * N + p] += v;
+        }
+        return;
+    }
     const float c2k = 2.f * (float)QNEP_K_COULOMB;
     phik[p] = c2k * s_out[0][t];                          // bracket of Eq. 38
     const float cq = -c2k * q[p];                         // Eq. 37
@@ -796,8 +887,76 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
     });
     // 5. gather
     const int nbg = (int)((N + GATHER_BLOCK - 1) / GATHER_BLOCK);
-    k_gather<<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, h->model.mode == 1 ? 1 : 0, h->d_phik, h->d_Fs);
+    k_gather<false><<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, h->model.mode == 1 ? 1 : 0, h->d_phik,
+                                                 h->d_Fs, GatherRows(), nullptr);
     h->launches += 6;
+    QNEP_CUDA_OK(h, ce);
+    QNEP_CUDA_OK(h, cudaGetLastError());
+    return QNEP_OK;
+}
+
+// Per-atom virial of the reciprocal part (Eq. 39) into d_Wat [9][N], after qnep_launch_pppm of the same evaluation (the
+// charge mesh is still in d_mesh; d_cm1, d_cm2 and d_field are free again).  A second forward transform on the FULL
+// spectrum feeds the virial pass along x; the inverse y / z passes and the back-interpolation kernel are the ones of the
+// main path, run on the three packed meshes.
+int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s)
+{
+    const int64_t N = h->N;
+    const double L[3] = {h->box[0], h->box[4], h->box[8]};
+    const int n0 = h->geo.grid[0], n1 = h->geo.grid[1], n2 = h->geo.grid[2];
+    const float2* tw0 = h->d_twiddle;
+    const float2* tw1 = h->d_twiddle + FFT_MAXN;
+    const float2* tw2 = h->d_twiddle + 2 * FFT_MAXN;
+    if (!h->d_cm3) QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm3, sizeof(float2) * h->ngrid));
+    cudaError_t ce = cudaSuccess;
+    auto note = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
+    const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    with_split(n2, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_z_fwd<R1, R2>, smem));
+        k_fft_z_fwd<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_mesh, h->d_cm3, tw2);
+    });
+    with_split(n1, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_strided<R1, R2, -1>, smem));
+        k_fft_strided<R1, R2, -1><<<dim3((unsigned)((int64_t)n0 * n2 / LINES), 1), S::THREADS, smem, s>>>(1, n0, n1, n2, h->d_cm3, h->d_cm3, tw1);
+    });
+    with_split(n0, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        using SI = Split<R2, R1>;
+        const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 2 * S::N;
+        note(allow_smem(k_fft_x_virial<R1, R2>, smem));
+        k_fft_x_virial<R1, R2><<<(unsigned)((int64_t)n1 * n2 / LINES), S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, h->d_cm3, tw0, h->d_gtab,
+                                                                                             h->d_gtab + 3 * FFT_MAXN, c0, inv4a2);
+    });
+    with_split(n1, [&](auto r1, auto r2) {
+        constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_strided<R1, R2, +1>, smem));
+        k_fft_strided<R1, R2, +1><<<dim3((unsigned)((int64_t)n0 * n2 / LINES), 2), S::THREADS, smem, s>>>(1, n0, n1, n2, h->d_cm1, h->d_cm2, tw1);
+        k_fft_strided<R1, R2, +1><<<dim3((unsigned)((int64_t)n0 * n2 / LINES), 1), S::THREADS, smem, s>>>(1, n0, n1, n2, h->d_cm3, h->d_cm3, tw1);
+    });
+    const int nbg = (int)((N + GATHER_BLOCK - 1) / GATHER_BLOCK);
+    if (h->model.mode != 1) QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Wat, 0, sizeof(float) * 9 * N, s));     // mode 1: k_realspace wrote d_Wat
+    GatherRows r1 = {{0, 4, 8, 1}, {-1, -1, -1, 3}};      // (W_xx, W_yy, W_zz, W_xy)
+    GatherRows r2 = {{2, 5, -1, -1}, {6, 7, -1, -1}};     // (W_xz, W_yz, W_xz, W_yz): the second copy is not used
+    with_split(n2, [&](auto q1, auto q2) {
+        constexpr int R1 = decltype(q1)::value, R2 = decltype(q2)::value;
+        using S = Split<R1, R2>;
+        const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
+        note(allow_smem(k_fft_z_fields<R1, R2>, smem));
+        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm1, h->d_cm2, h->d_field, tw2);
+        k_gather<true><<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, 0, nullptr, nullptr, r1, h->d_Wat);
+        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm3, h->d_cm3, h->d_field, tw2);
+        k_gather<true><<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, 0, nullptr, nullptr, r2, h->d_Wat);
+    });
+    h->launches += 9;
     QNEP_CUDA_OK(h, ce);
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;

@@ -137,7 +137,9 @@ struct qnep_handle {
     float* d_phir = nullptr;         // [N]
     float* d_phi = nullptr;          // [N]
     float* d_Fs = nullptr;           // [3][N] static electrostatic force
-    float* d_Facc = nullptr;         // [3][N] fp32 force accumulator of the angular pass (atomics); [9][N] in BEC mode
+    float* d_Facc = nullptr;         // [12][N] fp32 accumulators of the angular pass (atomics): rows 0-2 force (rows 0-8 Z in BEC
+                                     // mode), rows 3-11 per-atom virial (qnep_compute_atom_virial)
+    float* d_Wat = nullptr;          // [9][N] per-atom virial, static electrostatic parts (allocated on first use)
     double* d_sums = nullptr;        // [SUM_COUNT]
     int* d_flags = nullptr;          // [FLAG_COUNT]
     int* h_flags = nullptr;          // pinned
@@ -160,6 +162,7 @@ struct qnep_handle {
     float2* d_half = nullptr;        // half-spectrum array of the forward transform [x][y][N2/2 + 16] (N2 >= 32)
     float2* d_cm1 = nullptr;         // complex meshes
     float2* d_cm2 = nullptr;
+    float2* d_cm3 = nullptr;         // third complex mesh: per-atom virial pass only (allocated on first use)
     float4* d_field = nullptr;       // [Nx][Ny][Nz] (Phi, E_x, E_y, E_z)
     float* d_gtab = nullptr;         // 1-D influence tables: per axis N entries of (A_alpha) then k_alpha
     float2* d_twiddle = nullptr;     // per axis twiddles
@@ -206,17 +209,18 @@ int qnep_launch_list_stats(qnep_handle* h, double out[6], cudaStream_t s);
 int qnep_launch_pairs(qnep_handle* h, cudaStream_t s);
 int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s);
 int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s);
-int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, cudaStream_t s);
-int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, cudaStream_t s);
+int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, bool atomv, cudaStream_t s);
+int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, double* atomv_out, cudaStream_t s);
 int qnep_launch_fma_peak(double* tflops_host, cudaStream_t s);
 // electro.cu
-int qnep_launch_realspace(qnep_handle* h, cudaStream_t s);
+int qnep_launch_realspace(qnep_handle* h, bool atomv, cudaStream_t s);
 int qnep_launch_phi_finalize(qnep_handle* h, cudaStream_t s);
 int qnep_setup_ewald(qnep_handle* h);
-int qnep_launch_ewald(qnep_handle* h, const double* pos, cudaStream_t s);
+int qnep_launch_ewald(qnep_handle* h, const double* pos, bool atomv, cudaStream_t s);
 // pppm.cu
 int qnep_setup_pppm(qnep_handle* h);
 int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s);
+int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s);
 // pppm_sweep.cu
 bool qnep_sweep_usable(const qnep_handle* h);
 int qnep_setup_sweep(qnep_handle* h);
