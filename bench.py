@@ -11,7 +11,11 @@ PPPM 256^3, neighbour rebuild every 10 steps, timed per force evaluation.
 Prints ONE JSON line (see the keys below).  N > 1 runs N independent replicas (the path is single-GPU by
 the north_star: "replicas only"), one process per GPU, timed as the max over ranks.
 
---impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+The contract value is the step that produces the FULL output set of the north_star call (energy, forces, virial,
+charges); the cheaper energy + forces step an NVE run needs is timed in a second leg and reported beside it.
+
+--impl reference times the fp64 CPU oracle (oracle/) on the same workload (the whole config 4: ~11 s per evaluation on
+16 cores, at most 3 evaluations; --cpu-sample-side bounds it further).
 """
 from __future__ import annotations
 
@@ -60,10 +64,19 @@ def whole_job_value(n_atoms, steps, world, ms_total):
     return world * n_atoms * steps / (ms_total * 1e-3)
 
 
-# DRAM traffic per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the five FP32 kernels on config 4, from the
-# ncu --set full capture summarised in profiles/r01_ncu_full_current.txt (reported only for that workload)
-NCU_TRAFFIC_CONFIG4 = {"k_pairs": 1.72e9, "k_desc_angular": 1.03e9, "k_nn": 0.28e9, "k_force_angular": 1.45e9,
-                       "k_force_radial": 0.68e9}      # MB read + written columns of that file
+# ncu counters per launch on config 4 in the launch configuration timed here (all outputs), from the ncu --set full capture
+# summarised in profiles/r02_ncu_full.txt: DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) and EXECUTED FP32
+# flops (smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}_pred_on, FMA = 2).  Reported only for that workload; the
+# algorithmic work model above them is what the contract's `frac` uses, the executed figure is the north_star's evidence.
+NCU_COUNTERS_CONFIG4 = {
+    "k_pairs": {"dram_bytes": 1.68e9, "executed_flops": 5.695e9},
+    "k_desc_angular": {"dram_bytes": 0.975e9, "executed_flops": 9.423e9},
+    "k_nn": {"dram_bytes": 0.283e9, "executed_flops": 1.353e10},
+    "k_force_angular": {"dram_bytes": 1.43e9, "executed_flops": 2.552e10},
+    "k_force_radial": {"dram_bytes": 0.652e9, "executed_flops": 9.453e9},
+}
+NCU_COUNTERS_SOURCE = "profiles/r02_ncu_full.txt"
+NCU_PPPM_DRAM_BYTES_CONFIG4 = 1.92e9        # spread + five FFT kernels + gather, same capture
 
 
 def load_peaks():
@@ -245,30 +258,38 @@ def main():
     # safety margin: the order of fp32 atomics makes trajectories differ in the last bits from run to run, so the real
     # run uses half the first time step that went through
     dt_fs *= 0.5
-    # warm-up proper, from the initial state again
-    pos, vel = restart()
-    e_start = md(pos, vel, Wm, dt_fs).cpu().numpy()
+    # ---- secondary leg: energy + forces only (what an NVE run needs), exactly K steps after Wm warm-up steps ---------
+    def timed_leg():
+        pos, vel = restart()
+        e_a = md(pos, vel, Wm, dt_fs).cpu().numpy()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        h.profile_reset()
+        la = h.kernel_launches()
+        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ta = time.time()
+        ea.record()
+        e_b = md(pos, vel, K, dt_fs)             # synchronises at the end (device-side error check: skin, capacity)
+        eb.record()
+        torch.cuda.synchronize()
+        tb = time.time()
+        if dist is not None:
+            dist.barrier()
+        return e_a, e_b, ea.elapsed_time(eb), h.kernel_launches() - la, ta, tb
 
-    # ---- timed region: exactly K steps, inputs resident in HBM -------------------------------------------
+    h.md_set_outputs()
+    _, _, ms_ef, _, _, _ = timed_leg()
+    ms_ef = max_over_ranks(ms_ef, dist, dev)
+
+    # ---- timed region (contract): the full output set -- energy, forces, virial, charges -- every step ---------------
+    vir_t = torch.zeros(9, dtype=torch.float64, device=dev)
+    chg_t = torch.zeros(n, dtype=torch.float64, device=dev)
+    h.md_set_outputs(virial=vir_t, charges=chg_t)
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.25)
-    if dist is not None:
-        dist.barrier()
-    torch.cuda.synchronize()
-    h.profile_reset()
-    l0 = h.kernel_launches()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    tw0 = time.time()
-    e0.record()
-    e_end = md(pos, vel, K, dt_fs)               # synchronises at the end (device-side error check: skin, capacity)
-    e1.record()
-    torch.cuda.synchronize()
-    tw1 = time.time()
-    if dist is not None:
-        dist.barrier()
-    ms_total = e0.elapsed_time(e1)
-    launches = h.kernel_launches() - l0
+    e_start, e_end, ms_total, launches, tw0, tw1 = timed_leg()
     stage_ms, n_evals = h.profile_sum()
     md_graphs = n_evals == 0
     if md_graphs:
@@ -290,6 +311,8 @@ def main():
                  "drift_eV_per_atom": float((e_end[0] + e_end[1] - e_start[0] - e_start[1]) / n),
                  "T_start_K": float(e_start[1] / (1.5 * n * kB)), "T_end_K": float(e_end[1] / (1.5 * n * kB))}
     value = whole_job_value(n, K, world, ms_total)
+    value_ef = whole_job_value(n, K, world, ms_ef)
+    outputs_sanity = {"sum_charges_e": float(chg_t.sum().item()), "virial_trace_eV": float((vir_t[0] + vir_t[4] + vir_t[8]).item())}
     stats = h.neighbor_stats()
 
     # ---- roofline of the dominant kernel ------------------------------------------------------------------
@@ -310,19 +333,36 @@ def main():
     fp32_ms = sum(v[0] for v in kernels.values())
     fp32_flops = sum(v[1] for v in kernels.values())
     achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    full4 = args.config == 4 and not args.n_side       # the workload the ncu counters were taken on
+    ctr = NCU_COUNTERS_CONFIG4 if full4 else {}
+
+    def frac_of_peak(flops, ms):
+        return flops / (ms * 1e-3) / 1e12 / FP32_PEAK_NOMINAL_TFLOPS if ms > 0 else 0.0
+
+    exe_flops = sum(c["executed_flops"] for c in ctr.values()) if ctr else None
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
-                "traffic": NCU_TRAFFIC_CONFIG4.get(dom) if (args.config == 4 and not args.n_side) else None,
-                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_ncu_full_current.txt",
+                "frac_is": "frac_model: algorithmic flops of the frozen work model / live time / nominal peak; "
+                           "executed_frac (ncu-counted FP32 flops / live time / nominal peak) is the north_star's evidence",
+                "frac_model": achieved / FP32_PEAK_NOMINAL_TFLOPS,
+                "executed_flops_per_launch": ctr[dom]["executed_flops"] if ctr else None,
+                "executed_frac": frac_of_peak(ctr[dom]["executed_flops"], dom_ms) if ctr else None,
+                "traffic": ctr[dom]["dram_bytes"] if ctr else None,
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, " + NCU_COUNTERS_SOURCE,
                 "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "fma_loop_measured_tflops": fma_measured, "frac_of_measured_fma_loop": achieved / fma_measured if fma_measured else None,
                 "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops,
                 "per_kernel": {k: {"ms": v[0], "tflops": v[1] / (v[0] * 1e-3) / 1e12 if v[0] > 0 else 0.0,
-                                   "frac": v[1] / (v[0] * 1e-3) / 1e12 / FP32_PEAK_NOMINAL_TFLOPS if v[0] > 0 else 0.0}
+                                   "frac": frac_of_peak(v[1], v[0]), "frac_model": frac_of_peak(v[1], v[0]),
+                                   "executed_flops_per_launch": ctr[k]["executed_flops"] if ctr else None,
+                                   "executed_frac": frac_of_peak(ctr[k]["executed_flops"], v[0]) if ctr else None,
+                                   "dram_bytes_per_launch": ctr[k]["dram_bytes"] if ctr else None}
                                for k, v in kernels.items()},
                 "all_fp32_stages": {"ms": fp32_ms, "algorithmic_flops": fp32_flops,
                                     "tflops": fp32_flops / (fp32_ms * 1e-3) / 1e12,
-                                    "frac": fp32_flops / (fp32_ms * 1e-3) / 1e12 / FP32_PEAK_NOMINAL_TFLOPS}}
+                                    "frac": frac_of_peak(fp32_flops, fp32_ms), "frac_model": frac_of_peak(fp32_flops, fp32_ms),
+                                    "executed_flops": exe_flops,
+                                    "executed_frac": frac_of_peak(exe_flops, fp32_ms) if exe_flops else None}}
     peaks = load_peaks()
     mesh_bytes = float(np.prod(w.es.grid)) * 8.0
     fft_bytes = 3 * 3 * 2 * mesh_bytes - float(np.prod(w.es.grid)) * 4.0   # 3 transforms x 3 passes x (read + write)
@@ -331,40 +371,60 @@ def main():
             "peak": peaks["hbm_gbs"], "unit": "GB/s", "peak_source": peaks["source"]}
     pppm["achieved"] = pppm["algorithmic_bytes"] / (pppm["ms"] * 1e-3) / 1e9 if pppm["ms"] > 0 else 0.0
     pppm["frac"] = pppm["achieved"] / pppm["peak"]
+    pppm["frac_is"] = "frac_model: the survey's 3-pass byte model (2.4 GB at 256^3) / live stage time / measured copy peak"
+    pppm["frac_model"] = pppm["frac"]
+    pppm["dram_bytes_measured"] = NCU_PPPM_DRAM_BYTES_CONFIG4 if full4 else None
+    pppm["frac_measured_bytes"] = (NCU_PPPM_DRAM_BYTES_CONFIG4 / (pppm["ms"] * 1e-3) / 1e9 / pppm["peak"]
+                                   if (full4 and pppm["ms"] > 0) else None)
+    pppm["traffic_source"] = "ncu dram__bytes_read.sum + dram__bytes_write.sum over the stage's kernels, " + NCU_COUNTERS_SOURCE
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----------
-    hp = torch.empty((3, n), dtype=torch.float64).pin_memory()
-    hp.copy_(torch.from_numpy(np.ascontiguousarray(w.pos)))
+    # Every call gets its own positions: the start structure displaced along the initial velocities (0.5 fs per call), so
+    # lists are reused on atoms that did move; all four outputs come back to the host.
+    Ke = max(1, min(args.e2e_steps, K))
+    n_frames = min(Ke + 3, args.rebuild_every if args.rebuild_every > 1 else 2)
+    vel_host = vel0.cpu().numpy()
+    frames = []
+    for k in range(n_frames):
+        hp = torch.empty((3, n), dtype=torch.float64).pin_memory()
+        hp.copy_(torch.from_numpy(np.ascontiguousarray(w.pos + k * 0.5 * FS * vel_host)))
+        frames.append(hp)
     ht = torch.from_numpy(np.ascontiguousarray(w.types)).pin_memory()
     he = torch.empty(1, dtype=torch.float64).pin_memory()
     hf = torch.empty((3, n), dtype=torch.float64).pin_memory()
-    want = Q.WANT_ENERGY | Q.WANT_FORCES
+    hw = torch.empty(9, dtype=torch.float64).pin_memory()
+    hq = torch.empty(n, dtype=torch.float64).pin_memory()
+    want = Q.WANT_ALL
     box9 = Q._box(w.box)
     h2 = Q.from_workload(w)
-    h2.set_neighbor_policy(args.skin, args.rebuild_every)
-    Ke = max(1, min(args.e2e_steps, K))
+    h2.set_neighbor_policy(args.skin, n_frames)      # the frames repeat after n_frames calls: rebuild there
+    h2.set_pppm_kernels(args.pppm_kernels)
 
-    def e2e_step():
-        h2.compute_host_raw(n, hp.data_ptr(), ht.data_ptr(), box9, want, he.data_ptr(), hf.data_ptr(), 0, 0, 0)
+    def e2e_step(k):
+        h2.compute_host_raw(n, frames[k % n_frames].data_ptr(), ht.data_ptr(), box9, want, he.data_ptr(), hf.data_ptr(),
+                            hw.data_ptr(), hq.data_ptr(), 0)
 
-    for _ in range(3):
+    for k in range(n_frames):                        # warm-up: one full cycle of frames (ends before a rebuild call)
         try:
-            e2e_step()
+            e2e_step(k)
         except Q.QnepError as err:
             if err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
                 raise
+            e2e_step(k)
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    for _ in range(Ke):
-        e2e_step()
+    for k in range(Ke):
+        e2e_step(k)
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e, dist, dev)
     e2e = {"value": whole_job_value(n, Ke, world, t_e2e * 1e3), "unit": "atom-steps/s", "steps": Ke,
-           "h2d_bytes_per_step": int(hp.numel() * 8 + ht.numel() * 4), "d2h_bytes_per_step": int(hf.numel() * 8 + 8),
-           "api": "qnep_compute_host (pinned host buffers; neighbour rebuild every %d calls)" % args.rebuild_every}
+           "h2d_bytes_per_step": int(frames[0].numel() * 8 + ht.numel() * 4),
+           "d2h_bytes_per_step": int(hf.numel() * 8 + hq.numel() * 8 + 9 * 8 + 8),
+           "outputs": "energy, forces, virial, charges",
+           "api": "qnep_compute_host (pinned host buffers, a different frame per call; neighbour rebuild every %d calls)" % n_frames}
 
     # ---- CPU baseline: the oracle as it stands, on rank 0 at N = 1 only -----------------------------------
     cpu = None
@@ -385,6 +445,9 @@ def main():
                        "l2_policy": "inputs larger than L2 (neighbour lists + meshes >> 126 MB); no flush needed",
                        "mean_skin_list": stats["mean_list"], "mean_neighbours_radial": stats["mean_radial"],
                        "mean_neighbours_angular": stats["mean_angular"]},
+            "outputs_per_step": "energy, forces, virial, charges (qnep_md_set_outputs)",
+            "value_energy_forces_only": value_ef, "ms_per_step_energy_forces_only": ms_ef / K,
+            "outputs_sanity": outputs_sanity,
             "roofline": roofline, "roofline_pppm": pppm,
             "stage_ms_per_eval": per_eval, "evals_profiled": n_evals,
             "md_sanity": md_sanity,

@@ -189,6 +189,15 @@ int qnep_md_run(qnep_handle *h, int64_t n_atoms, double *pos_dev, double *vel_de
                 double *energy_dev, void *cuda_stream);
 
 /*
+ * Outputs of the evaluations inside qnep_md_run.  By default a step evaluates energy and forces only (all an NVE run
+ * needs).  With want = QNEP_WANT_VIRIAL and / or QNEP_WANT_CHARGES every step also evaluates the total virial / writes
+ * the charges: virial_dev [9] and charges_dev [N] (DEVICE, owned by the caller, must stay valid for the following
+ * qnep_md_run calls) hold the values of the LAST step when qnep_md_run returns.  want = 0 restores the default.
+ * Errors: INVALID_ARG (a requested output pointer is null, or a flag other than VIRIAL / CHARGES).
+ */
+int qnep_md_set_outputs(qnep_handle *h, uint32_t want, double *virial_dev, double *charges_dev);
+
+/*
  * Tell the handle that the caller changed positions or velocities behind qnep_md_run's back (a restart from a stored
  * state): the forces kept from the previous call are dropped and the next evaluation rebuilds the neighbour list.
  */

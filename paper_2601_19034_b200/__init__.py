@@ -35,7 +35,7 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 
 # every symbol include/qnep.h declares
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
-               "qnep_compute", "qnep_compute_atom_virial", "qnep_compute_host", "qnep_md_run", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
+               "qnep_compute", "qnep_compute_atom_virial", "qnep_compute_host", "qnep_md_run", "qnep_md_set_outputs", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
                "qnep_fma_peak",
                "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
@@ -89,6 +89,8 @@ def load_library():
     lib.qnep_md_run.restype = C.c_int
     lib.qnep_md_run.argtypes = [vp, i64, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), dbl, i32, vp, vp]
     lib.qnep_check.restype = C.c_int
+    lib.qnep_md_set_outputs.restype = C.c_int
+    lib.qnep_md_set_outputs.argtypes = [vp, u32, vp, vp]
     lib.qnep_md_reset.restype = C.c_int
     lib.qnep_md_reset.argtypes = [vp]
     lib.qnep_set_md_graphs.restype = C.c_int
@@ -292,6 +294,14 @@ class QNEP:
 
     def kernel_launches(self) -> int:
         return int(self._lib.qnep_kernel_launches(self._h))
+
+    def md_set_outputs(self, virial=None, charges=None):
+        """Extra outputs of the steps of md_run: cuda float64 tensors virial [9] and / or charges [N] (kept alive by the
+        caller), or neither to restore the default (energy and forces only)."""
+        want = (WANT_VIRIAL if virial is not None else 0) | (WANT_CHARGES if charges is not None else 0)
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        self._ok(self._lib.qnep_md_set_outputs(self._h, want, ptr(virial), ptr(charges)))
+        self._md_outputs = (virial, charges)
 
     def md_reset(self):
         """Positions / velocities were changed outside md_run: drop the kept forces, rebuild the lists next time."""

@@ -631,6 +631,20 @@ int qnep_compute_atom_virial(qnep_handle* h, int64_t n_atoms, const double* pos_
                             charges_dev, nullptr, s, atom_virial_dev);
 }
 
+int qnep_md_set_outputs(qnep_handle* h, uint32_t want, double* virial_dev, double* charges_dev)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if ((want & ~(uint32_t)(QNEP_WANT_VIRIAL | QNEP_WANT_CHARGES)) || ((want & QNEP_WANT_VIRIAL) && !virial_dev) ||
+        ((want & QNEP_WANT_CHARGES) && !charges_dev)) {
+        h->err = "qnep_md_set_outputs: only QNEP_WANT_VIRIAL / QNEP_WANT_CHARGES, each with its output pointer";
+        return QNEP_ERR_INVALID_ARG;
+    }
+    h->md_want = want;
+    h->md_virial = (want & QNEP_WANT_VIRIAL) ? virial_dev : nullptr;
+    h->md_charges = (want & QNEP_WANT_CHARGES) ? charges_dev : nullptr;
+    return QNEP_OK;
+}
+
 int qnep_md_reset(qnep_handle* h)
 {
     if (!h) return QNEP_ERR_INVALID_ARG;
@@ -712,9 +726,11 @@ int qnep_md_run(qnep_handle* h, int64_t n_atoms, double* pos_dev, double* vel_de
     Masses ms;
     for (int t = 0; t < QNEP_MAX_TYPES; ++t) ms.m[t] = t < h->model.n_types ? mass_host[t] : 1.0;
     const int nb = (int)((n_atoms + 255) / 256);
-    const uint32_t want = QNEP_WANT_ENERGY | QNEP_WANT_FORCES;
+    const uint32_t want = QNEP_WANT_ENERGY | QNEP_WANT_FORCES | h->md_want;
+    double* const mdW = h->md_virial;
+    double* const mdQ = h->md_charges;
     if (!h->md_have_forces) {
-        if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
+        if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, mdW, mdQ, nullptr, s))) return rc;
         h->md_have_forces = true;
     }
     const bool graphs = h->md_graph_mode == 2 || (h->md_graph_mode == 1 && n_atoms <= QNEP_GRAPH_MAX_ATOMS);
@@ -732,6 +748,7 @@ int qnep_md_run(qnep_handle* h, int64_t n_atoms, double* pos_dev, double* vel_de
     if (graphs && n_steps > 0) {
         qnep_handle::MdKey key = {};
         key.pos = pos_dev; key.vel = vel_dev; key.types = types_dev; key.N = n_atoms; key.dt = dt; key.s = nullptr;     // replay always happens on md_stream
+        key.virial = mdW; key.charges = mdQ; key.want = want;
         key.gen = h->ws_generation;
         for (int t = 0; t < QNEP_MAX_TYPES; ++t) key.m[t] = ms.m[t];
         if (std::memcmp(&key, &h->md_key, sizeof(key)) != 0) {
@@ -742,7 +759,7 @@ int qnep_md_run(qnep_handle* h, int64_t n_atoms, double* pos_dev, double* vel_de
     for (int step = 0; step < n_steps; ++step) {
         if (!graphs) {
             k_vv_kick_drift<<<nb, 256, 0, s>>>(n_atoms, pos_dev, vel_dev, h->d_Fmd, types_dev, ms, dt);
-            if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s))) return rc;
+            if ((rc = run_pipeline(h, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, mdW, mdQ, nullptr, s))) return rc;
             k_vv_kick<<<nb, 256, 0, s>>>(n_atoms, vel_dev, h->d_Fmd, types_dev, ms, dt, h->d_sums);
             h->launches += 2;
             continue;
@@ -754,7 +771,7 @@ int qnep_md_run(qnep_handle* h, int64_t n_atoms, double* pos_dev, double* vel_de
             cudaGraph_t graph = nullptr;
             QNEP_CUDA_OK(h, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
             k_vv_kick_drift<<<nb, 256, 0, s>>>(n_atoms, pos_dev, vel_dev, h->d_Fmd, types_dev, ms, dt);
-            rc = enqueue_pipeline(h, kind == 1, false, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, nullptr, nullptr, nullptr, s);
+            rc = enqueue_pipeline(h, kind == 1, false, n_atoms, pos_dev, types_dev, want, nullptr, h->d_Fmd, mdW, mdQ, nullptr, s);
             k_vv_kick<<<nb, 256, 0, s>>>(n_atoms, vel_dev, h->d_Fmd, types_dev, ms, dt, h->d_sums);
             const cudaError_t ce = cudaStreamEndCapture(s, &graph);
             if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }

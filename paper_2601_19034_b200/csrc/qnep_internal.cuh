@@ -147,6 +147,9 @@ struct qnep_handle {
     bool flags_pending = false;
     double* d_Fmd = nullptr;         // [3][N] forces kept for qnep_md_run (original order)
     bool md_have_forces = false;
+    uint32_t md_want = 0;            // extra outputs of the evaluations inside qnep_md_run (qnep_md_set_outputs)
+    double* md_virial = nullptr;
+    double* md_charges = nullptr;
 
     // Ewald
     int nk = 0;
@@ -172,7 +175,7 @@ struct qnep_handle {
     int md_graph_mode = 1;                 // 0 never, 1 when N <= QNEP_GRAPH_MAX_ATOMS (launch-bound sizes), 2 always
     cudaGraphExec_t md_exec[2] = {nullptr, nullptr};
     int64_t md_exec_launches[2] = {0, 0};
-    struct MdKey { const void *pos, *vel, *types; int64_t N; double dt; double m[QNEP_MAX_TYPES]; cudaStream_t s; uint64_t gen; } md_key = {};
+    struct MdKey { const void *pos, *vel, *types, *virial, *charges; int64_t N; double dt; double m[QNEP_MAX_TYPES]; cudaStream_t s; uint64_t gen; uint64_t want; } md_key = {};
     cudaStream_t md_stream = nullptr;      // graphs run on an own stream (the legacy default stream cannot be captured), fenced by events
     cudaEvent_t md_fence = nullptr;
     uint64_t ws_generation = 0;            // bumped whenever workspace pointers, capacities or the geometry change
