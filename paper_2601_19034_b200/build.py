@@ -37,6 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("QNEP_NVCC_EXTRA", "").split()      # e.g. -DNAME=value switches of an experiment
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)

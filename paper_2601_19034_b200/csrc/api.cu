@@ -232,7 +232,11 @@ __global__ void k_finalize(const double* __restrict__ sums, int mode, double* __
         if (mode == 1) e += sums[SUM_U_R] + sums[SUM_U_S];
         energy[0] = e;
     }
-    if (threadIdx.x < 9 && virial) virial[threadIdx.x] = sums[SUM_W0 + threadIdx.x];
+    if (threadIdx.x < 9 && virial) {
+        double w = sums[SUM_W0 + threadIdx.x];
+        for (int st = 0; st < QNEP_WSTRIPES; ++st) w += sums[SUM_COUNT + st * 9 + threadIdx.x];
+        virial[threadIdx.x] = w;
+    }
 }
 
 // ---- debug / parity helpers -----------------------------------------------------------------------
@@ -435,7 +439,7 @@ int enqueue_pipeline(qnep_handle* h, bool rebuild, bool timed, int64_t N, const 
     }
 #define QNEP_STAGE(i) do { if (timed) QNEP_CUDA_OK(h, cudaEventRecord(ev[i], s)); } while (0)
     QNEP_STAGE(0);
-    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_sums, 0, sizeof(double) * SUM_COUNT, s));
+    QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_sums, 0, sizeof(double) * QNEP_SUM_ALLOC, s));
     if (rebuild) { if ((rc = qnep_launch_build(h, pos, types, s))) return rc; }
     QNEP_STAGE(1);
     if (!rebuild) { if ((rc = qnep_launch_prep(h, pos, false, s))) return rc; }
@@ -548,7 +552,7 @@ int qnep_create(const qnep_model_desc* model, const float* params_host, size_t n
         return fail(QNEP_ERR_CUDA);
     }
     if ((rc = upload_model(h))) return fail(rc);
-    if (cudaMalloc(&h->d_sums, sizeof(double) * SUM_COUNT) != cudaSuccess ||
+    if (cudaMalloc(&h->d_sums, sizeof(double) * QNEP_SUM_ALLOC) != cudaSuccess ||
         cudaMalloc(&h->d_flags, sizeof(int) * FLAG_COUNT) != cudaSuccess ||
         cudaMallocHost(&h->h_flags, sizeof(int) * FLAG_COUNT) != cudaSuccess) {
         h->err = "allocation of accumulators failed";

@@ -182,7 +182,13 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 //   phase 2, per ACCEPTED entry: basis functions f_k(r) and S^t_k += f_k for t = t_j, append to the live radial
 //     list.  The expensive part runs for accepted entries only, with no skin-shell divergence.
 // ------------------------------------------------------------------------------------------
-constexpr int PAIRS_BLOCK = 128, PAIRS_CH = 32, PAIRS_DX = 4;
+#ifndef QNEP_PAIRS_BLOCK
+#define QNEP_PAIRS_BLOCK 128
+#endif
+#ifndef QNEP_PAIRS_CH
+#define QNEP_PAIRS_CH 32
+#endif
+constexpr int PAIRS_BLOCK = QNEP_PAIRS_BLOCK, PAIRS_CH = QNEP_PAIRS_CH, PAIRS_DX = 4;
 
 __device__ __forceinline__ int4 ldg_stream(const int4* p)        // streamed once: do not allocate in L1
 {
@@ -374,6 +380,7 @@ __device__ __forceinline__ void harmonics(float x, float y, float z, float* __re
 // The live angular pairs are streamed through a cp.async ring ANG_DEPTH rows deep (the kernels hold 120+ accumulators
 // in registers, so occupancy is low and the loads must be issued far ahead).
 constexpr int ANG_BLOCK = 64, ANG_DEPTH = 8;
+constexpr int FA_KP2 = 10;     // float2 per row of the packed coefficient table of k_force_angular
 
 template <int T>
 __global__ void __launch_bounds__(ANG_BLOCK)
@@ -387,11 +394,13 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
     const int ti = __float_as_int(xyzt[p].w);
-    float A[NR][NLM];
+    // accumulators as register pairs: the 120 updates A_nlm += g_n b_lm of a neighbour are 60 packed FMAs (FFMA2:
+    // two FP32 FMAs per issued instruction; this kernel is bound by issue slots, not by latency)
+    float2 A2[NR][NLM / 2];
 #pragma unroll
     for (int a = 0; a < NR; ++a)
 #pragma unroll
-        for (int lm = 0; lm < NLM; ++lm) A[a][lm] = 0.f;
+        for (int m = 0; m < NLM / 2; ++m) A2[a][m] = make_float2(0.f, 0.f);
     const int n = nlvA[p];
     const float4* rows = lvA + qnep_tiled_base(p, capLA);
     const int tid = threadIdx.x;
@@ -407,32 +416,38 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
         cp_async_commit();
         const float r2 = pr.x * pr.x + pr.y * pr.y + pr.z * pr.z;
         const float rinv = fast_rsqrt(r2), r = r2 * rinv;
-        float f[NB];
+        float f[KP];
         cheb_basis<true, false>(r, rcinv, f, nullptr);
+        f[9] = 0.f; f[10] = 0.f; f[11] = 0.f;
         const int tj = (unsigned)__float_as_int(pr.w) >> QNEP_NL_SHIFT;
-        const float* c = sh_c + (ti * T + tj) * NR * KP;
-        float gn[NR];
+        const float4* c4 = reinterpret_cast<const float4*>(sh_c + (ti * T + tj) * NR * KP);
+        float2 g2[NR];
 #pragma unroll
         for (int a = 0; a < NR; ++a) {
-            float v = 0.f;
-#pragma unroll
-            for (int k = 0; k < NB; ++k) v = fmaf(c[a * KP + k], f[k], v);
-            gn[a] = v;
+            // g_n = sum_k c_nk f_k over k pairs (rows are padded to 12 floats with zeros)
+            const float4 ca = c4[a * 3], cb = c4[a * 3 + 1], cc = c4[a * 3 + 2];
+            float2 v = __fmul2_rn(make_float2(ca.x, ca.y), make_float2(f[0], f[1]));
+            v = __ffma2_rn(make_float2(ca.z, ca.w), make_float2(f[2], f[3]), v);
+            v = __ffma2_rn(make_float2(cb.x, cb.y), make_float2(f[4], f[5]), v);
+            v = __ffma2_rn(make_float2(cb.z, cb.w), make_float2(f[6], f[7]), v);
+            const float g = fmaf(cc.x, f[8], v.x + v.y);
+            g2[a] = make_float2(g, g);
         }
         float b[NLM];
         harmonics(pr.x * rinv, pr.y * rinv, pr.z * rinv, b);
 #pragma unroll
         for (int a = 0; a < NR; ++a)
 #pragma unroll
-            for (int lm = 0; lm < NLM; ++lm) A[a][lm] = fmaf(gn[a], b[lm], A[a][lm]);
+            for (int m = 0; m < NLM / 2; ++m) A2[a][m] = __ffma2_rn(g2[a], make_float2(b[2 * m], b[2 * m + 1]), A2[a][m]);
     }
 #pragma unroll
     for (int a = 0; a < NR; ++a) {
         float d[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int lm = 0; lm < NLM; ++lm) {
-            d[l_of_lm(lm)] = fmaf(c_Clm[lm] * A[a][lm], A[a][lm], d[l_of_lm(lm)]);
-            Aout[(int64_t)(a * NLM + lm) * N + p] = A[a][lm];
+            const float Av = (lm & 1) ? A2[a][lm >> 1].y : A2[a][lm >> 1].x;
+            d[l_of_lm(lm)] = fmaf(c_Clm[lm] * Av, Av, d[l_of_lm(lm)]);
+            Aout[(int64_t)(a * NLM + lm) * N + p] = Av;
         }
 #pragma unroll
         for (int l = 0; l < 4; ++l) D[(int64_t)(NR + a * 4 + l) * N + p] = d[l];
@@ -477,6 +492,10 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
         const float* b0 = w + H * W0P;
         const float* w1U = b0 + H;
         const float* w1q = w1U + H;
+#ifndef QNEP_NN_PACK
+#define QNEP_NN_PACK 0
+#endif
+#if QNEP_NN_PACK == 0
         float x[W0P], dU[W0P], dQ[W0P];
 #pragma unroll
         for (int v = 0; v < W0P; ++v) { x[v] = v < ND ? D[(int64_t)v * N + p] : 0.f; dU[v] = 0.f; dQ[v] = 0.f; }
@@ -507,6 +526,48 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
         qraw[p] = q;
 #pragma unroll
         for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + p] = dU[v]; FpQ[(int64_t)v * N + p] = dQ[v]; }
+#else
+        // experiment: the forward dot product scalar, the two backward updates packed (QNEP_NN_PACK = 1)
+        constexpr int NP = W0P / 2;
+        float2 x2[NP], dU2[NP], dQ2[NP];
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+            x2[i] = make_float2(2 * i < ND ? D[(int64_t)(2 * i) * N + p] : 0.f, 2 * i + 1 < ND ? D[(int64_t)(2 * i + 1) * N + p] : 0.f);
+            dU2[i] = make_float2(0.f, 0.f);
+            dQ2[i] = make_float2(0.f, 0.f);
+        }
+        float U = 0.f, q = 0.f;
+        for (int mu = 0; mu < H; ++mu) {
+            const float4* row = reinterpret_cast<const float4*>(w + mu * W0P);
+            float2 wr[NP];
+#pragma unroll
+            for (int v4 = 0; v4 < W0P / 4; ++v4) {
+                const float4 t = row[v4];
+                wr[2 * v4] = make_float2(t.x, t.y); wr[2 * v4 + 1] = make_float2(t.z, t.w);
+            }
+            float z0 = -b0[mu], z1 = 0.f;
+#pragma unroll
+            for (int i = 0; i < (ND + 1) / 2; ++i) { z0 = fmaf(wr[i].x, x2[i].x, z0); if (2 * i + 1 < ND) z1 = fmaf(wr[i].y, x2[i].y, z1); }
+            const float hmu = tanh_f32(z0 + z1);
+            const float a = w1U[mu], b = w1q[mu];
+            U = fmaf(a, hmu, U);
+            q = fmaf(b, hmu, q);
+            const float dh = fmaf(-hmu, hmu, 1.f);
+            const float au = a * dh, bq = b * dh;
+            const float2 au2 = make_float2(au, au), bq2 = make_float2(bq, bq);
+#pragma unroll
+            for (int i = 0; i < (ND + 1) / 2; ++i) { dU2[i] = __ffma2_rn(au2, wr[i], dU2[i]); dQ2[i] = __ffma2_rn(bq2, wr[i], dQ2[i]); }
+        }
+        U -= b1U;
+        q -= b1q;
+        Ui[p] = U;
+        qraw[p] = q;
+#pragma unroll
+        for (int v = 0; v < ND; ++v) {
+            FpU[(int64_t)v * N + p] = (v & 1) ? dU2[v >> 1].y : dU2[v >> 1].x;
+            FpQ[(int64_t)v * N + p] = (v & 1) ? dQ2[v >> 1].y : dQ2[v >> 1].x;
+        }
+#endif
         accU += (double)U;
         accQ += (double)q;
     }
@@ -535,34 +596,38 @@ __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const do
 //   F_ij = rhat sum_lm G'_lm b_lm + [v - (rhat.v) rhat] / r,  v = sum_lm G_lm grad_u b_lm.
 // Own sums go to Fa (3 per atom; BEC: 9 per atom = 1/2 r_ij (x) c_ij), pair vectors to f12.
 // ------------------------------------------------------------------------------------------
-#define QNEP_HTERM(LM, B, GX, GY, GZ)                                        \
-    {                                                                        \
-        float G_ = 0.f, Gp_ = 0.f;                                           \
-        _Pragma("unroll") for (int a = 0; a < NR; ++a) {                     \
-            G_ = fmaf(Q[a][LM], gn[a], G_);                                  \
-            Gp_ = fmaf(Q[a][LM], dgn[a], Gp_);                               \
-        }                                                                    \
-        s0 = fmaf(Gp_, (B), s0);                                             \
-        vx = fmaf(G_, (GX), vx);                                             \
-        vy = fmaf(G_, (GY), vy);                                             \
-        vz = fmaf(G_, (GZ), vz);                                             \
-    }
-
 // ATOMV (with VIRIAL, not BEC): the pair term -r_ij (x) F_ij belongs to the per-atom virial of atom j (Eq. 12:
 // W_j = sum_i r_ji (x) F_ij) and is scattered to rows 3..11 of Facc.
 template <int T, bool BEC, bool VIRIAL, bool ATOMV = false>
-__global__ void __launch_bounds__(ANG_BLOCK, BEC || VIRIAL ? 4 : 6)
+#ifndef QNEP_FA_VIR_BLOCKS
+#define QNEP_FA_VIR_BLOCKS 4
+#endif
+#ifndef QNEP_FA_BLOCKS
+#define QNEP_FA_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(ANG_BLOCK, BEC || ATOMV ? 4 : (VIRIAL ? QNEP_FA_VIR_BLOCKS : QNEP_FA_BLOCKS))
 k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
                 const float* __restrict__ cA, const float* __restrict__ cR, float rcinv, const float* __restrict__ FpU,
                 const float* __restrict__ FpQ, const float* __restrict__ phi, float sqrt_eps, const float* __restrict__ Ain,
                 float* __restrict__ Fp, float* __restrict__ recA, float4* __restrict__ recB, float* __restrict__ Facc,
                 double* __restrict__ sums)
 {
-    __shared__ __align__(16) float sh_c[T * T * NR * KP];
+    // Packed angular coefficient table for the loop below: row (ti, tj, n) holds ten float2,
+    //   [0] = (2 c_0 + sum_{k>=1} c_k, 0)  and  [k] = (c_k, k c_k), k = 1..8   ([9] is padding),
+    // so that  (sum_k c_k (T_k + 1), sum_k c_k k U_{k-1}) = [0] + sum_{k>=1} [k] * (T_k, U_{k-1})  in eight packed FMAs.
+    __shared__ __align__(16) float2 sh_c2[T * T * NR * FA_KP2];
     __shared__ __align__(16) float sh_cR[T * T * NR * KP];
     __shared__ float4 sh_ring[ANG_DEPTH][ANG_BLOCK];
     __shared__ double sh_red[32];
-    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) { sh_c[i] = cA[i]; sh_cR[i] = cR[i]; }
+    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_cR[i] = cR[i];
+    for (int i = threadIdx.x; i < T * T * NR; i += blockDim.x) {
+        const float* c = cA + i * KP;
+        float c0 = 2.f * c[0];
+#pragma unroll
+        for (int k = 1; k < NB; ++k) { c0 += c[k]; sh_c2[i * FA_KP2 + k] = make_float2(c[k], (float)k * c[k]); }
+        sh_c2[i * FA_KP2] = make_float2(c0, 0.f);
+        sh_c2[i * FA_KP2 + 9] = make_float2(0.f, 0.f);
+    }
     __syncthreads();
     const int tid = threadIdx.x;
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
@@ -608,7 +673,10 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                 recB[(int64_t)t * N + p] = make_float4(pk[5], pk[6], pk[7], pk[8]);
             }
         }
-        float Q[NR][NLM];
+        // Q_nlm = dE/dA_nlm = 2 C_lm Fp_nl A_nlm, held as register PAIRS in the order of c_fa_pair (two harmonics with
+        // the same zero pattern of their gradient share a pair): the loop below is bound by issue slots, and a packed
+        // FMA (FFMA2) does two FP32 FMAs per issued instruction.
+        float2 Q2[NR][NLM / 2];
 #pragma unroll
         for (int a = 0; a < NR; ++a) {
             float fpl[4];
@@ -620,8 +688,12 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                 fpl[l] = 2.f * val;
             }
 #pragma unroll
-            for (int lm = 0; lm < NLM; ++lm)
-                Q[a][lm] = c_Clm[lm] * fpl[l_of_lm(lm)] * Ain[(int64_t)(a * NLM + lm) * N + p];
+            for (int m = 0; m < NLM / 2; ++m) {
+                constexpr int pa[NLM / 2] = {0, 8, 1, 6, 13, 22, 4, 9, 11, 16, 18, 20};
+                constexpr int pb[NLM / 2] = {3, 15, 2, 7, 14, 23, 5, 10, 12, 17, 19, 21};
+                Q2[a][m] = make_float2(c_Clm[pa[m]] * fpl[l_of_lm(pa[m])] * Ain[(int64_t)(a * NLM + pa[m]) * N + p],
+                                       c_Clm[pb[m]] * fpl[l_of_lm(pb[m])] * Ain[(int64_t)(a * NLM + pb[m]) * N + p]);
+            }
         }
         float Fx = 0.f, Fy = 0.f, Fz = 0.f;
         for (int s = 0; s < n; ++s) {
@@ -632,59 +704,138 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
             const float dx = pr.x, dy = pr.y, dz = pr.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float rinv = fast_rsqrt(r2), r = r2 * rinv;
-            // g_n = 1/2 fc sum_k c_nk Tp_k,  g_n' = A sum_k c_nk kU_k + B sum_k c_nk Tp_k   (ChebDeriv)
-            ChebDeriv cd;
-            cd.eval(r, rcinv);
             const int jw = __float_as_int(pr.w);
             const int j = jw & QNEP_NL_MASK;
-            const float* c = sh_c + (ti * T + (int)((unsigned)jw >> QNEP_NL_SHIFT)) * NR * KP;
-            float gn[NR], dgn[NR];
+            // g_n = 1/2 fc sum_k c_nk (T_k + 1),  g_n' = A sum_k c_nk k U_{k-1} + B sum_k c_nk (T_k + 1)   (see ChebDeriv);
+            // V_k = (T_k, U_{k-1}) obeys V_{k+1} = 2x V_k - V_{k-1} in both components
+            float2 g2[NR], dg2[NR];
+            {
+                const float t = r * rcinv;
+                float sn, cs;
+                __sincosf(3.14159265358979f * t, &sn, &cs);
+                const float tm1 = t - 1.f;
+                const float xx = 2.f * tm1 * tm1 - 1.f;
+                const float hfc = 0.25f + 0.25f * cs;
+                const float cA_ = hfc * (4.f * tm1 * rcinv);
+                const float cB_ = -0.7853981633974483f * rcinv * sn;
+                const float2 x22 = make_float2(xx + xx, xx + xx);
+                float2 V[NB];
+                V[0] = make_float2(1.f, 0.f);
+                V[1] = make_float2(xx, 1.f);
 #pragma unroll
-            for (int a = 0; a < NR; ++a) {
-                float dt = c[a * KP] * cd.Tp[0], du = c[a * KP + 1];
+                for (int k = 2; k < NB; ++k) V[k] = __ffma2_rn(x22, V[k - 1], make_float2(-V[k - 2].x, -V[k - 2].y));
+                const float4* c4 = reinterpret_cast<const float4*>(sh_c2 + (ti * T + (int)((unsigned)jw >> QNEP_NL_SHIFT)) * NR * FA_KP2);
 #pragma unroll
-                for (int k = 1; k < NB; ++k) dt = fmaf(c[a * KP + k], cd.Tp[k], dt);
-#pragma unroll
-                for (int k = 2; k < NB; ++k) du = fmaf(c[a * KP + k], cd.kU[k], du);
-                gn[a] = cd.hfc * dt;
-                dgn[a] = fmaf(cd.A, du, cd.B * dt);
+                for (int a = 0; a < NR; ++a) {
+                    const float4 q0 = c4[a * 5], q1 = c4[a * 5 + 1], q2 = c4[a * 5 + 2], q3 = c4[a * 5 + 3], q4 = c4[a * 5 + 4];
+                    float2 acc = make_float2(q0.x, q0.y);
+                    acc = __ffma2_rn(make_float2(q0.z, q0.w), V[1], acc);
+                    acc = __ffma2_rn(make_float2(q1.x, q1.y), V[2], acc);
+                    acc = __ffma2_rn(make_float2(q1.z, q1.w), V[3], acc);
+                    acc = __ffma2_rn(make_float2(q2.x, q2.y), V[4], acc);
+                    acc = __ffma2_rn(make_float2(q2.z, q2.w), V[5], acc);
+                    acc = __ffma2_rn(make_float2(q3.x, q3.y), V[6], acc);
+                    acc = __ffma2_rn(make_float2(q3.z, q3.w), V[7], acc);
+                    acc = __ffma2_rn(make_float2(q4.x, q4.y), V[8], acc);
+                    const float gv = hfc * acc.x, dgv = fmaf(cA_, acc.y, cB_ * acc.x);
+                    g2[a] = make_float2(gv, gv);
+                    dg2[a] = make_float2(dgv, dgv);
+                }
             }
             const float x = dx * rinv, y = dy * rinv, z = dz * rinv;
             const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z;
             const float x2my2 = x2 - y2;
-            float s0 = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
-            // l = 1
-            QNEP_HTERM(0, z, 0.f, 0.f, 1.f)
-            QNEP_HTERM(1, x, 1.f, 0.f, 0.f)
-            QNEP_HTERM(2, y, 0.f, 1.f, 0.f)
-            // l = 2
-            QNEP_HTERM(3, 3.f * z2 - 1.f, 0.f, 0.f, 6.f * z)
-            QNEP_HTERM(4, xz, z, 0.f, x)
-            QNEP_HTERM(5, yz, 0.f, z, y)
-            QNEP_HTERM(6, x2my2, 2.f * x, -2.f * y, 0.f)
-            QNEP_HTERM(7, 2.f * xy, 2.f * y, 2.f * x, 0.f)
-            // l = 3
+            float2 s02 = make_float2(0.f, 0.f), vx2 = s02, vy2 = s02, vz2 = s02;
+            float vxs = 0.f, vys = 0.f;
+            // G_lm = sum_n Q_nlm g_n, G'_lm = sum_n Q_nlm g_n' for the pair m; then s0 += G' b, v += G grad b
+#define QNEP_HPAIR(M)                                                                   \
+            float2 G_ = __fmul2_rn(Q2[0][M], g2[0]), Gp_ = __fmul2_rn(Q2[0][M], dg2[0]);  \
+            _Pragma("unroll") for (int a = 1; a < NR; ++a) {                             \
+                G_ = __ffma2_rn(Q2[a][M], g2[a], G_);                                    \
+                Gp_ = __ffma2_rn(Q2[a][M], dg2[a], Gp_);                                 \
+            }
             const float f5 = 5.f * z2 - 1.f;
             const float t3 = 3.f * x2my2;            // 3x^2 - 3y^2
-            QNEP_HTERM(8, (5.f * z2 - 3.f) * z, 0.f, 0.f, 15.f * z2 - 3.f)
-            QNEP_HTERM(9, f5 * x, f5, 0.f, 10.f * xz)
-            QNEP_HTERM(10, f5 * y, 0.f, f5, 10.f * yz)
-            QNEP_HTERM(11, x2my2 * z, 2.f * xz, -2.f * yz, x2my2)
-            QNEP_HTERM(12, 2.f * xy * z, 2.f * yz, 2.f * xz, 2.f * xy)
-            QNEP_HTERM(13, (x2 - 3.f * y2) * x, t3, -6.f * xy, 0.f)
-            QNEP_HTERM(14, (3.f * x2 - y2) * y, 6.f * xy, t3, 0.f)
-            // l = 4
             const float f7 = 7.f * z2 - 1.f, f73 = 7.f * z2 - 3.f;
             const float cx = (x2 - 3.f * y2) * x, cy = (3.f * x2 - y2) * y;   // x^3 - 3xy^2, 3x^2 y - y^3
-            QNEP_HTERM(15, (35.f * z2 - 30.f) * z2 + 3.f, 0.f, 0.f, (140.f * z2 - 60.f) * z)
-            QNEP_HTERM(16, f73 * xz, f73 * z, 0.f, (21.f * z2 - 3.f) * x)
-            QNEP_HTERM(17, f73 * yz, 0.f, f73 * z, (21.f * z2 - 3.f) * y)
-            QNEP_HTERM(18, f7 * x2my2, 2.f * x * f7, -2.f * y * f7, 14.f * z * x2my2)
-            QNEP_HTERM(19, f7 * 2.f * xy, 2.f * y * f7, 2.f * x * f7, 28.f * xy * z)
-            QNEP_HTERM(20, cx * z, t3 * z, -6.f * xy * z, cx)
-            QNEP_HTERM(21, cy * z, 6.f * xy * z, t3 * z, cy)
-            QNEP_HTERM(22, x2my2 * x2my2 - 4.f * x2 * y2, 4.f * cx, -4.f * cy, 0.f)
-            QNEP_HTERM(23, 4.f * x2my2 * xy, 4.f * cy, 4.f * cx, 0.f)
+            {   // (0, 3): z | 3z^2 - 1; gradients along z only
+                QNEP_HPAIR(0)
+                s02 = __ffma2_rn(Gp_, make_float2(z, 3.f * z2 - 1.f), s02);
+                vz2 = __ffma2_rn(G_, make_float2(1.f, 6.f * z), vz2);
+            }
+            {   // (8, 15): (5z^2 - 3) z | (35z^2 - 30) z^2 + 3; gradients along z only
+                QNEP_HPAIR(1)
+                s02 = __ffma2_rn(Gp_, make_float2((5.f * z2 - 3.f) * z, (35.f * z2 - 30.f) * z2 + 3.f), s02);
+                vz2 = __ffma2_rn(G_, make_float2(15.f * z2 - 3.f, (140.f * z2 - 60.f) * z), vz2);
+            }
+            {   // (1, 2): x | y
+                QNEP_HPAIR(2)
+                s02 = __ffma2_rn(Gp_, make_float2(x, y), s02);
+                vxs += G_.x; vys += G_.y;
+            }
+            {   // (6, 7): x^2 - y^2 | 2xy
+                QNEP_HPAIR(3)
+                s02 = __ffma2_rn(Gp_, make_float2(x2my2, 2.f * xy), s02);
+                vx2 = __ffma2_rn(G_, make_float2(2.f * x, 2.f * y), vx2);
+                vy2 = __ffma2_rn(G_, make_float2(-2.f * y, 2.f * x), vy2);
+            }
+            {   // (13, 14): x^3 - 3xy^2 | 3x^2 y - y^3
+                QNEP_HPAIR(4)
+                s02 = __ffma2_rn(Gp_, make_float2(cx, cy), s02);
+                vx2 = __ffma2_rn(G_, make_float2(t3, 6.f * xy), vx2);
+                vy2 = __ffma2_rn(G_, make_float2(-6.f * xy, t3), vy2);
+            }
+            {   // (22, 23): (x^2 - y^2)^2 - 4x^2 y^2 | 4 (x^2 - y^2) xy
+                QNEP_HPAIR(5)
+                s02 = __ffma2_rn(Gp_, make_float2(x2my2 * x2my2 - 4.f * x2 * y2, 4.f * x2my2 * xy), s02);
+                vx2 = __ffma2_rn(G_, make_float2(4.f * cx, 4.f * cy), vx2);
+                vy2 = __ffma2_rn(G_, make_float2(-4.f * cy, 4.f * cx), vy2);
+            }
+            {   // (4, 5): xz | yz
+                QNEP_HPAIR(6)
+                s02 = __ffma2_rn(Gp_, make_float2(xz, yz), s02);
+                vxs = fmaf(G_.x, z, vxs); vys = fmaf(G_.y, z, vys);
+                vz2 = __ffma2_rn(G_, make_float2(x, y), vz2);
+            }
+            {   // (9, 10): (5z^2 - 1) x | (5z^2 - 1) y
+                QNEP_HPAIR(7)
+                s02 = __ffma2_rn(Gp_, make_float2(f5 * x, f5 * y), s02);
+                vxs = fmaf(G_.x, f5, vxs); vys = fmaf(G_.y, f5, vys);
+                vz2 = __ffma2_rn(G_, make_float2(10.f * xz, 10.f * yz), vz2);
+            }
+            {   // (11, 12): (x^2 - y^2) z | 2xyz
+                QNEP_HPAIR(8)
+                s02 = __ffma2_rn(Gp_, make_float2(x2my2 * z, 2.f * xy * z), s02);
+                vx2 = __ffma2_rn(G_, make_float2(2.f * xz, 2.f * yz), vx2);
+                vy2 = __ffma2_rn(G_, make_float2(-2.f * yz, 2.f * xz), vy2);
+                vz2 = __ffma2_rn(G_, make_float2(x2my2, 2.f * xy), vz2);
+            }
+            {   // (16, 17): (7z^2 - 3) xz | (7z^2 - 3) yz
+                QNEP_HPAIR(9)
+                const float f73z = f73 * z, g21 = 21.f * z2 - 3.f;
+                s02 = __ffma2_rn(Gp_, make_float2(f73 * xz, f73 * yz), s02);
+                vxs = fmaf(G_.x, f73z, vxs); vys = fmaf(G_.y, f73z, vys);
+                vz2 = __ffma2_rn(G_, make_float2(g21 * x, g21 * y), vz2);
+            }
+            {   // (18, 19): (7z^2 - 1)(x^2 - y^2) | (7z^2 - 1) 2xy
+                QNEP_HPAIR(10)
+                const float xf7 = 2.f * x * f7, yf7 = 2.f * y * f7;
+                s02 = __ffma2_rn(Gp_, make_float2(f7 * x2my2, f7 * 2.f * xy), s02);
+                vx2 = __ffma2_rn(G_, make_float2(xf7, yf7), vx2);
+                vy2 = __ffma2_rn(G_, make_float2(-yf7, xf7), vy2);
+                vz2 = __ffma2_rn(G_, make_float2(14.f * z * x2my2, 28.f * xy * z), vz2);
+            }
+            {   // (20, 21): (x^3 - 3xy^2) z | (3x^2 y - y^3) z
+                QNEP_HPAIR(11)
+                const float t3z = t3 * z, xyz6 = 6.f * xy * z;
+                s02 = __ffma2_rn(Gp_, make_float2(cx * z, cy * z), s02);
+                vx2 = __ffma2_rn(G_, make_float2(t3z, xyz6), vx2);
+                vy2 = __ffma2_rn(G_, make_float2(-xyz6, t3z), vy2);
+                vz2 = __ffma2_rn(G_, make_float2(cx, cy), vz2);
+            }
+#undef QNEP_HPAIR
+            const float s0 = s02.x + s02.y;
+            const float vx = vxs + (vx2.x + vx2.y), vy = vys + (vy2.x + vy2.y), vz = vz2.x + vz2.y;
             const float uv = x * vx + y * vy + z * vz;
             const float fx = s0 * x + (vx - uv * x) * rinv;
             const float fy = s0 * y + (vy - uv * y) * rinv;
@@ -722,7 +873,7 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
 #pragma unroll
         for (int a = 0; a < 9; ++a) {
             const double w = block_sum((double)W[a], sh_red);
-            if (threadIdx.x == 0) atomicAdd(&sums[SUM_W0 + a], -w);
+            if (threadIdx.x == 0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * 9 + a], -w);
         }
     }
 }
@@ -834,16 +985,18 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                     cd.eval(r, rcinv);
                     const float Pj[NB] = {a8[3], a8[4], a8[5], a8[6], a8[7], b4.x, b4.y, b4.z, b4.w};
                     float sij, sji;
-                    if (BEC || VIRIAL) {
+                    if (BEC || ATOMV) {
                         sij = cd.dot(Pi);
                         sji = cd.dot(Pj);
                     } else {
-                        // only s_ij + s_ji is needed: one contraction with P^{i,tj} + P^{j,ti}
+                        // only s_ij + s_ji is needed: one contraction with P^{i,tj} + P^{j,ti}.  That holds for the TOTAL
+                        // virial too: sum_i sum_j r_ij (x) rhat_ij s_ij runs over ordered pairs, and the terms (i, j) and
+                        // (j, i) have the same dyad r_ij (x) rhat_ij, so every atom may book 1/2 (s_ij + s_ji) instead of s_ij.
                         float Ps[NB];
 #pragma unroll
                         for (int k = 0; k < NB; ++k) Ps[k] = Pi[k] + Pj[k];
-                        sij = cd.dot(Ps);
-                        sji = 0.f;
+                        sij = 0.5f * cd.dot(Ps);
+                        sji = sij;
                     }
                     const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
                     if (BEC) {
@@ -903,7 +1056,7 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
 #pragma unroll
         for (int a = 0; a < 9; ++a) {
             const double w = block_sum((double)W[a], sh_red);
-            if (threadIdx.x == 0) atomicAdd(&sums[SUM_W0 + a], -w);
+            if (threadIdx.x == 0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * 9 + a], -w);
         }
     }
 }

@@ -43,6 +43,11 @@ constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (DESIGN.md read
 
 // device-side double accumulators
 enum { SUM_E_NEP = 0, SUM_Q, SUM_PHI, SUM_U_R, SUM_U_K, SUM_U_S, SUM_W0 /* 9 entries */, SUM_KE = 15, SUM_COUNT = 16 };
+// The force kernels add one 3 x 3 partial virial per BLOCK: 16 000 blocks on nine addresses serialise in L2, so they
+// are spread over QNEP_WSTRIPES copies behind the named slots (stripe = block index mod QNEP_WSTRIPES); k_finalize adds
+// the stripes to SUM_W0.
+#define QNEP_WSTRIPES 64
+#define QNEP_SUM_ALLOC (SUM_COUNT + QNEP_WSTRIPES * 9)
 // device-side int flags
 // overflow flags hold the largest count seen when a list exceeded its capacity (0 otherwise)
 enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_BAD_TYPE /* a species index outside 0..T-1 */, FLAG_COUNT = 8 };
