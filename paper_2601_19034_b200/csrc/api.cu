@@ -24,7 +24,7 @@ void free_workspace(qnep_handle* h)
 {
     void** ptrs[] = {(void**)&h->d_key, (void**)&h->d_cnt, (void**)&h->d_start, (void**)&h->d_fill, (void**)&h->d_tmpidx,
                      (void**)&h->d_sidx, (void**)&h->d_cm, (void**)&h->d_cmi, (void**)&h->d_cellc, (void**)&h->d_xyzt, (void**)&h->d_off0, (void**)&h->d_mfrac,
-                     (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_lvR, (void**)&h->d_nlvR,
+                     (void**)&h->d_mi0, (void**)&h->d_nlR, (void**)&h->d_nnR, (void**)&h->d_nnR0, (void**)&h->d_nlRend, (void**)&h->d_lvR, (void**)&h->d_nlvR,
                      (void**)&h->d_lvA, (void**)&h->d_nlvA, (void**)&h->d_D, (void**)&h->d_A, (void**)&h->d_Ui, (void**)&h->d_qraw,
                      (void**)&h->d_q, (void**)&h->d_FpU, (void**)&h->d_FpQ, (void**)&h->d_Fp, (void**)&h->d_recA, (void**)&h->d_recB, (void**)&h->d_lvRend,
                      (void**)&h->d_phik, (void**)&h->d_phir, (void**)&h->d_phi, (void**)&h->d_Fs, (void**)&h->d_Facc,
@@ -111,6 +111,8 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         const size_t npad = (n + QNEP_TILE - 1) / QNEP_TILE * QNEP_TILE;
         if ((rc = dev_alloc(h, &h->d_nlR, npad * (capR / 4)))) return rc;
         if ((rc = dev_alloc(h, &h->d_nnR, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nnR0, n))) return rc;
+        if ((rc = dev_alloc(h, &h->d_nlRend, n * T))) return rc;
         if ((rc = dev_alloc(h, &h->d_lvR, npad * (capLR / 4)))) return rc;
         if ((rc = dev_alloc(h, &h->d_nlvR, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_lvA, npad * capLA))) return rc;

@@ -174,21 +174,21 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 //   live radial entry : the skin-list word (sorted index | image code << 27), type-major like the skin list
 //                       (warp-tiled int4 layout); lvRend[t][p] = end of the species-t segment
 //   live angular pair : (dx, dy, dz, bits(sorted index | type << 27))
-// The skin list is processed in chunks of PAIRS_CH slots, each in two phases:
+// The kernel is bound by L1 wavefronts (gathers of 16 bytes from ~15 lines per warp instruction, the queue and the
+// shift table in shared memory) and by issue slots, so both phases are kept to the instructions they need:
 //   phase 1, per SKIN entry (all lanes busy): list word -> position gather -> distance test; accepted entries are
-//     pushed to a per-thread queue in shared memory (word, r^2) and, inside the angular cutoff, appended to the
-//     angular pair list.  List vectors arrive through a double-buffered cp.async stage (one chunk ahead), gathered
-//     positions through a register ring PAIRS_DX entries ahead (plain loads, so that they hit L1).
-//   phase 2, per ACCEPTED entry: basis functions f_k(r) and S^t_k += f_k for t = t_j, append to the live radial
-//     list.  The expensive part runs for accepted entries only, with no skin-shell divergence.
+//     pushed to a per-thread RING in shared memory (word, r^2) and, inside the angular cutoff, appended to the
+//     angular pair list.  Bounds, prefetch and species are decided once per list vector: the build pads every species
+//     segment to a multiple of four slots (k_build_lists), nlRend[t][p] holds the segment ends.
+//   phase 2, per ACCEPTED entry, four at a time (one int4 of the live radial list): basis functions f_k(r) and
+//     S^t_k += f_k.  After every round of PAIRS_CH slots a warp pops the SAME number of entries from all its rings
+//     (what the emptiest lane has, but at least what the fullest lane must give up to leave room for the next
+//     round), so the binomial scatter of the acceptance count over a round does not idle lanes; what stays in a
+//     ring waits for the next round, the last round drains.
 // ------------------------------------------------------------------------------------------
-#ifndef QNEP_PAIRS_BLOCK
-#define QNEP_PAIRS_BLOCK 128
-#endif
-#ifndef QNEP_PAIRS_CH
-#define QNEP_PAIRS_CH 32
-#endif
-constexpr int PAIRS_BLOCK = QNEP_PAIRS_BLOCK, PAIRS_CH = QNEP_PAIRS_CH, PAIRS_DX = 4;
+constexpr int PAIRS_BLOCK = 128;
+constexpr int PAIRS_CH = 16;                 // skin slots per round (four list vectors)
+constexpr int PAIRS_QCAP = 2 * PAIRS_CH;     // ring capacity per thread
 
 __device__ __forceinline__ int4 ldg_stream(const int4* p)        // streamed once: do not allocate in L1
 {
@@ -201,145 +201,137 @@ __device__ __forceinline__ int word_of(const int4& v, int u) { return u == 0 ? v
 template <int T>
 __global__ void __launch_bounds__(PAIRS_BLOCK)
 k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __restrict__ nl,
-        const int* __restrict__ nn, const float* __restrict__ cR, float rcinv, int capR, int capLR, int capLA,
+        const int* __restrict__ nn, const int* __restrict__ nlRend, const float* __restrict__ cR, float rcinv, int capR, int capLR, int capLA,
         int4* __restrict__ lvR, int* __restrict__ nlvR, int* __restrict__ lvRend,
         float4* __restrict__ lvA, int* __restrict__ nlvA, float* __restrict__ D, int* __restrict__ flags)
 {
-    constexpr int NV = PAIRS_CH / 4;                         // int4 vectors per chunk
-    static_assert(NV % 4 == 0 && PAIRS_DX == 4, "the register rotation below assumes 4 list vectors and 4 positions in flight");
+    static_assert(PAIRS_CH == 16 && (PAIRS_QCAP & (PAIRS_QCAP - 1)) == 0, "four list vectors per round, power-of-two ring");
     __shared__ float4 sh_shift[27];
     __shared__ float sh_c[T * T * NR * KP];
-    __shared__ int sh_qe[PAIRS_CH][PAIRS_BLOCK];             // queue: words
-    __shared__ float sh_qr[PAIRS_CH][PAIRS_BLOCK];           // queue: r^2
+    __shared__ int sh_qe[PAIRS_QCAP][PAIRS_BLOCK];           // ring: words
+    __shared__ float sh_qr[PAIRS_QCAP][PAIRS_BLOCK];         // ring: r^2
     load_shift_table(sh_shift, g);
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
     __syncthreads();
     const int tid = threadIdx.x;
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
-    if (p >= N) return;
+    const int64_t p0 = blockIdx.x * (int64_t)blockDim.x + tid;
+    const bool live = p0 < N;                                // threads beyond N stay for the warp votes, with an empty list
+    const int64_t p = live ? p0 : N - 1;
     const float4 xi = xyzt[p];
     const int ti = __float_as_int(xi.w);
-    const int n = nn[p];
-    const int n4 = (n + 3) >> 2;
+    const int n4 = live ? (nn[p] >> 2) : 0;                  // list vectors (the count is a multiple of four)
+    int segend[T], acc_end[T];                               // skin slot / accepted count at which species t ends
+#pragma unroll
+    for (int t = 0; t < T; ++t) { segend[t] = (t < T - 1 && live) ? nlRend[(int64_t)t * N + p] : 0x7fffffff; acc_end[t] = 0x7fffffff; }
     const int4* lbase = nl + qnep_tiled_base(p, capR / 4);
-    // list vectors: lv[gv & 3] holds vector gv; while gv is processed, gv + 1 feeds the position gathers (PAIRS_DX = 4
-    // slots ahead) and gv + 2, gv + 3 are in flight
+    // list vectors: lv[gv & 3] holds vector gv; while gv is processed, gv + 1 feeds the position gathers (four slots
+    // ahead) and gv + 2, gv + 3 are in flight.  Beyond the end the registers hold the atom itself, so the gathers need no
+    // bound check.
+    const int4 filler = make_int4((int)p, (int)p, (int)p, (int)p);
     int4 lv[4];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) lv[k] = k < n4 ? ldg_stream(lbase + (int64_t)k * QNEP_TILE) : make_int4(0, 0, 0, 0);
-    lv[3] = make_int4(0, 0, 0, 0);
-    float4 ring[PAIRS_DX];                                   // ring[s & 3] holds the position of the atom of slot s
+    for (int k = 0; k < 4; ++k) lv[k] = (k < 3 && k < n4) ? ldg_stream(lbase + (int64_t)k * QNEP_TILE) : filler;
+    float4 ring[4];                                          // ring[u] holds the position of the atom of slot 4 gv + u
 #pragma unroll
-    for (int k = 0; k < PAIRS_DX; ++k)
-        ring[k] = k < n ? xyzt[word_of(lv[k >> 2], k & 3) & QNEP_NL_MASK] : make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int u = 0; u < 4; ++u) ring[u] = xyzt[word_of(lv[0], u) & QNEP_NL_MASK];
     float S[T][NB];                                          // S^t_k without the "+1" part: sum_j 1/2 fc T_k
     float S1[T];                                             // sum_j 1/2 fc
-    int cnt[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        cnt[t] = 0; S1[t] = 0.f;
+        S1[t] = 0.f;
 #pragma unroll
         for (int k = 0; k < NB; ++k) S[t][k] = 0.f;
     }
-    int cA_ = 0, cRtot = 0;
+    int cA_ = 0, head = 0, tail = 0;                         // angular pairs; accepted entries consumed / produced
     int4* outR = lvR + qnep_tiled_base(p, capLR / 4);
     float4* outA = lvA + qnep_tiled_base(p, capLA);
-    int4 rbuf = make_int4(QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY, QNEP_NL_EMPTY);
-    const int nchunk = (n + PAIRS_CH - 1) / PAIRS_CH;
     int* qe = &sh_qe[0][tid];
     float* qr = &sh_qr[0][tid];
-    for (int c = 0; c < nchunk; ++c) {
-        const int sbase = c * PAIRS_CH;
-        int qn = 0;
-        int cc[T];
-#pragma unroll
-        for (int t = 0; t < T; ++t) cc[t] = 0;
+    const int nround = __reduce_max_sync(0xffffffffu, (n4 + 3) >> 2);
+    for (int c = 0; c < nround; ++c) {
         // ---- phase 1 ----
 #pragma unroll
-        for (int v = 0; v < NV; ++v) {
-            {
-                const int gv = c * NV + v + 3;
-                if (gv < n4) lv[(v + 3) & 3] = ldg_stream(lbase + (int64_t)gv * QNEP_TILE);
+        for (int v = 0; v < 4; ++v) {
+            const int gv = 4 * c + v;
+            lv[(v + 3) & 3] = filler;                        // beyond the end the gathers below read the atom itself
+            if (gv + 3 < n4) lv[(v + 3) & 3] = ldg_stream(lbase + (int64_t)(gv + 3) * QNEP_TILE);
+            int tjv = 0;
+#pragma unroll
+            for (int t = 0; t < T - 1; ++t) {
+                if (4 * gv == segend[t]) acc_end[t] = tail;
+                tjv += (4 * gv >= segend[t]) ? 1 : 0;
             }
+            const int tjbits = tjv << QNEP_NL_SHIFT;
+            const bool act = gv < n4;
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const int i = 4 * v + u;
                 const int e = word_of(lv[v & 3], u);
                 const float4 xj = ring[u];
-                if (sbase + i + PAIRS_DX < n) ring[u] = xyzt[word_of(lv[(v + 1) & 3], u) & QNEP_NL_MASK];
-                if (sbase + i < n) {
-                    const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-                    const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 < g.rc_r2 && r2 >= 1e-12f) {
-                        const int tj = __float_as_int(xj.w);
-                        qe[qn * PAIRS_BLOCK] = e;
-                        qr[qn * PAIRS_BLOCK] = r2;
-                        ++qn;
-#pragma unroll
-                        for (int t = 0; t < T - 1; ++t) cc[t] += (tj == t) ? 1 : 0;
-                        if (r2 < g.rc_a2) {
-                            if (cA_ < capLA) {
-                                *outA = make_float4(dx, dy, dz, __int_as_float((e & QNEP_NL_MASK) | (tj << QNEP_NL_SHIFT)));
-                                outA += QNEP_TILE;
-                            }
-                            ++cA_;
+                ring[u] = xyzt[word_of(lv[(v + 1) & 3], u) & QNEP_NL_MASK];
+                const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
+                const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                if (act && r2 < g.rc_r2 && r2 >= 1e-12f) {
+                    const int slot = (tail & (PAIRS_QCAP - 1)) * PAIRS_BLOCK;
+                    qe[slot] = e;
+                    qr[slot] = r2;
+                    ++tail;
+                    if (r2 < g.rc_a2) {
+                        if (cA_ < capLA) {
+                            *outA = make_float4(dx, dy, dz, __int_as_float((e & QNEP_NL_MASK) | tjbits));
+                            outA += QNEP_TILE;
                         }
+                        ++cA_;
                     }
                 }
             }
         }
-        // ---- phase 2: the queue is type-major, species t ends at bnd[t] ----
-        int bnd[T];
-        {
-            int e_ = 0;
+        // ---- phase 2 ----
+        const int fill = tail - head;
+        const bool last = c == nround - 1;
+        const int mn = __reduce_min_sync(0xffffffffu, fill), mx = __reduce_max_sync(0xffffffffu, fill);
+        const int npop = last ? ((mx + 3) & ~3) : max(mn & ~3, (mx - PAIRS_CH + 3) & ~3);
+        const int mine = last ? fill : (min(npop, fill) & ~3);
+        for (int k = 0; k < npop; k += 4) {
+            if (k < mine) {
+                int w4[4];
 #pragma unroll
-            for (int t = 0; t < T - 1; ++t) { e_ += cc[t]; bnd[t] = e_; cnt[t] += cc[t]; }
-            bnd[T - 1] = qn;
-            cnt[T - 1] += qn - e_;
-        }
-        for (int k = 0; k < qn; ++k) {
-            const int e = qe[k * PAIRS_BLOCK];
-            const float r2 = qr[k * PAIRS_BLOCK];
-            // 1/2 fc(r) T_k(x), k = 0..8   (f_k = 1/2 fc (T_k + 1): the "+1" part is accumulated once in S1)
-            const float tt = r2 * fast_rsqrt(r2) * rcinv;
-            const float hfc = 0.25f + 0.25f * __cosf(3.14159265358979f * tt);
-            const float tm1 = tt - 1.f;
-            const float x = 2.f * tm1 * tm1 - 1.f, x2 = x + x;
-            float a[T];
+                for (int u = 0; u < 4; ++u) {
+                    const int gidx = head + k + u;                                   // accepted entry number gidx of this atom
+                    const int slot = (gidx & (PAIRS_QCAP - 1)) * PAIRS_BLOCK;
+                    const bool valid = k + u < mine;                                 // false only in the tail of the last round
+                    const float r2 = valid ? qr[slot] : 1.f;
+                    w4[u] = valid ? qe[slot] : QNEP_NL_EMPTY;
+                    // 1/2 fc(r) T_k(x), k = 0..8   (f_k = 1/2 fc (T_k + 1): the "+1" part is accumulated once in S1)
+                    const float tt = r2 * fast_rsqrt(r2) * rcinv;
+                    const float hfc = valid ? 0.25f + 0.25f * __cosf(3.14159265358979f * tt) : 0.f;
+                    const float tm1 = tt - 1.f;
+                    const float x = 2.f * tm1 * tm1 - 1.f, x2 = x + x;
+                    float a[T];
 #pragma unroll
-            for (int t = 0; t < T; ++t) a[t] = (T == 1 || ((t == 0 || k >= bnd[t - 1]) && k < bnd[t])) ? hfc : 0.f;
-            float Tm = 1.f, Tc = x;
+                    for (int t = 0; t < T; ++t) a[t] = (T == 1 || ((t == 0 || gidx >= acc_end[t - 1]) && (t == T - 1 || gidx < acc_end[t]))) ? hfc : 0.f;
+                    float Tm = 1.f, Tc = x;
 #pragma unroll
-            for (int t = 0; t < T; ++t) { S1[t] += a[t]; S[t][1] = fmaf(a[t], Tc, S[t][1]); }
+                    for (int t = 0; t < T; ++t) { S1[t] += a[t]; S[t][1] = fmaf(a[t], Tc, S[t][1]); }
 #pragma unroll
-            for (int kk = 2; kk < NB; ++kk) {
-                const float Tn = fmaf(x2, Tc, -Tm);
+                    for (int kk = 2; kk < NB; ++kk) {
+                        const float Tn = fmaf(x2, Tc, -Tm);
 #pragma unroll
-                for (int t = 0; t < T; ++t) S[t][kk] = fmaf(a[t], Tn, S[t][kk]);
-                Tm = Tc; Tc = Tn;
+                        for (int t = 0; t < T; ++t) S[t][kk] = fmaf(a[t], Tn, S[t][kk]);
+                        Tm = Tc; Tc = Tn;
+                    }
+                }
+                if (head + k < capLR) outR[(int64_t)((head + k) >> 2) * QNEP_TILE] = make_int4(w4[0], w4[1], w4[2], w4[3]);
             }
-            // append to the live radial list (four slots per int4)
-            const int pos = cRtot & 3;
-            rbuf.x = pos == 0 ? e : rbuf.x; rbuf.y = pos == 1 ? e : rbuf.y; rbuf.z = pos == 2 ? e : rbuf.z; rbuf.w = pos == 3 ? e : rbuf.w;
-            if (pos == 3 && cRtot < capLR) outR[(int64_t)(cRtot >> 2) * QNEP_TILE] = rbuf;
-            ++cRtot;
         }
+        head += mine;
     }
-    const int nlive = min(cRtot, capLR);
-    if (nlive & 3) {
-        const int m = nlive & 3;
-        rbuf.y = m > 1 ? rbuf.y : QNEP_NL_EMPTY; rbuf.z = m > 2 ? rbuf.z : QNEP_NL_EMPTY; rbuf.w = QNEP_NL_EMPTY;
-        outR[(int64_t)(nlive >> 2) * QNEP_TILE] = rbuf;
-    }
-    nlvR[p] = nlive;
+    if (!live) return;
+    nlvR[p] = min(tail, capLR);
     nlvA[p] = min(cA_, capLA);
-    {
-        int end = 0;
 #pragma unroll
-        for (int t = 0; t < T; ++t) { end += cnt[t]; lvRend[(int64_t)t * N + p] = min(end, capLR); }
-    }
-    if (cRtot > capLR) atomicMax(&flags[FLAG_MAX_LR], cRtot);
+    for (int t = 0; t < T; ++t) lvRend[(int64_t)t * N + p] = min(t < T - 1 ? min(acc_end[t], tail) : tail, capLR);
+    if (tail > capLR) atomicMax(&flags[FLAG_MAX_LR], tail);
     if (cA_ > capLA) atomicMax(&flags[FLAG_MAX_LA], cA_);
     // f_0 = fc = 2 (1/2 fc): S^t_0 = 2 S1;  f_k = 1/2 fc T_k + 1/2 fc: S^t_k = S[t][k] + S1
 #pragma unroll
@@ -1102,7 +1094,7 @@ int qnep_launch_pairs(qnep_handle* h, cudaStream_t s)
     const float rcinv = (float)(1.0 / h->model.rc_r);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_pairs<T><<<nb, PAIRS_BLOCK, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
+        k_pairs<T><<<nb, PAIRS_BLOCK, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlRend, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
                                               h->d_lvR, h->d_nlvR, h->d_lvRend, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
     });
     h->launches += 1;

@@ -243,7 +243,7 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
 __global__ void __launch_bounds__(128)
 k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, const int* __restrict__ cellc,
               const int* __restrict__ start, int capR, int4* __restrict__ nlR, int* __restrict__ nnR,
-              int* __restrict__ flags)
+              int* __restrict__ nnR0, int* __restrict__ nlRend, int* __restrict__ flags)
 {
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
@@ -252,7 +252,7 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
     const int pc = cellc[p];
     const int c0 = pc & 1023, c1 = (pc >> 10) & 1023, c2 = (pc >> 20) & 1023;
     int* out = reinterpret_cast<int*>(nlR + qnep_tiled_base(p, capR / 4));    // slot s at out[(s >> 2) * 128 + (s & 3)]
-    int nR = 0;
+    int nR = 0, nPad = 0;                // slots written, filler slots among them
     const float rcs2 = g.rcs_r2;
     const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
     // type-major order: all neighbours of species 0 first, then species 1, ...  The per-step lists derived from
@@ -295,8 +295,17 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
             }
             for (; q < e; ++q) test(q, xyzt[q]);
         }
+        // Every species segment is padded to a multiple of four slots (one int4) with the atom itself in its own cell
+        // (r = 0: the per-step filter drops it), so that the four slots of a list vector belong to ONE species and
+        // the walkers decide species, bounds and prefetch once per vector.
+        while (nR & 3) {
+            if (nR < capR) out[((nR >> 2) << 7) | (nR & 3)] = (int)p | (13 << QNEP_NL_SHIFT);
+            ++nR; ++nPad;
+        }
+        nlRend[(int64_t)t * N + p] = min(nR, capR);
     }
     nnR[p] = min(nR, capR);
+    nnR0[p] = min(nR, capR) - nPad;
     if (nR > capR) atomicMax(&flags[FLAG_MAX_NR], nR);
 }
 
@@ -359,7 +368,7 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
     if (rc) return rc;
     const int nb2 = (int)((N + 127) / 128);
     k_build_lists<<<nb2, 128, 0, s>>>(N, h->model.n_types, h->geo, h->d_xyzt, h->d_cellc, h->d_start, h->capR,
-                                     h->d_nlR, h->d_nnR, h->d_flags);
+                                     h->d_nlR, h->d_nnR, h->d_nnR0, h->d_nlRend, h->d_flags);
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
     return QNEP_OK;
@@ -374,7 +383,7 @@ int qnep_launch_list_stats(qnep_handle* h, double out[6], cudaStream_t s)
     Acc* d = nullptr;
     QNEP_CUDA_OK(h, cudaMalloc(&d, sizeof(Acc)));
     QNEP_CUDA_OK(h, cudaMemsetAsync(d, 0, sizeof(Acc), s));
-    const int* arrays[3] = {h->d_nnR, h->d_nlvR, h->d_nlvA};
+    const int* arrays[3] = {h->d_nnR0, h->d_nlvR, h->d_nlvA};
     for (int a = 0; a < 3; ++a) k_count_stats<<<nb, 256, 0, s>>>(N, arrays[a], &d->mx[a], &d->sum[a]);
     h->launches += 3;
     Acc r;

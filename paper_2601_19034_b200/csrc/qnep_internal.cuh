@@ -122,7 +122,9 @@ struct qnep_handle {
     float4* d_mfrac = nullptr;       // [N] PPPM: fractional mesh offsets (dx, dy, dz, bits of the packed nearest mesh point), mesh-bin order
     int* d_mi0 = nullptr;            // [N] PPPM: nearest mesh point, packed 10 bits each, cell-major order
     int4* d_nlR = nullptr;           // warp-tiled [capR / 4] int4 per atom: skin list (r < rc_r + skin at build time)
-    int* d_nnR = nullptr;            // [N]
+    int* d_nnR = nullptr;            // [N] slots of the skin list (every species segment padded to a multiple of 4)
+    int* d_nnR0 = nullptr;           // [N] neighbours in the skin list (statistics)
+    int* d_nlRend = nullptr;         // [T][N] end slot of the species-t segment of the skin list
     int4* d_lvR = nullptr;           // warp-tiled [capLR / 4] int4 per atom: live radial list of this step (r < rc_r)
     int* d_nlvR = nullptr;           // [N]
     int* d_lvRend = nullptr;         // [T][N] end of the species-t segment of the (type-major) live radial list
