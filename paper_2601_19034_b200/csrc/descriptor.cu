@@ -129,15 +129,6 @@ __device__ __forceinline__ float fast_rsqrt(float x)
     return y;
 }
 
-__device__ __forceinline__ void load_shift_table(float4* sh, const Geometry& g)
-{
-    if (threadIdx.x < 27) {
-        const int code = threadIdx.x;
-        sh[code] = make_float4((code / 9 - 1) * (float)g.hcell[0], ((code / 3) % 3 - 1) * (float)g.hcell[1],
-                               (code % 3 - 1) * (float)g.hcell[2], 0.f);
-    }
-}
-
 __device__ __forceinline__ double block_sum(double v, double* sh)
 {
 #pragma unroll
@@ -171,7 +162,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 // ------------------------------------------------------------------------------------------
 // a2: one walk over the skin list: the exact lists of this step and the radial descriptors
-//   live radial entry : the skin-list word (sorted index | image code << 27), type-major like the skin list
+//   live radial entry : the skin-list word (sorted index | cell offset of the image << 26), type-major like the skin list
 //                       (warp-tiled int4 layout); lvRend[t][p] = end of the species-t segment
 //   live angular pair : (dx, dy, dz, bits(sorted index | type << 27))
 // The kernel is bound by L1 wavefronts (gathers of 16 bytes from ~15 lines per warp instruction, the queue and the
@@ -189,6 +180,8 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 constexpr int PAIRS_BLOCK = 128;
 constexpr int PAIRS_CH = 16;                 // skin slots per round (four list vectors)
 constexpr int PAIRS_QCAP = 2 * PAIRS_CH;     // ring capacity per thread
+constexpr int PAIRS_LD = 8;                  // list vectors in flight per thread (power of two)
+constexpr size_t PAIRS_SMEM = sizeof(int4) * PAIRS_LD * PAIRS_BLOCK + sizeof(int) * 2 * PAIRS_QCAP * PAIRS_BLOCK;
 
 __device__ __forceinline__ int4 ldg_stream(const int4* p)        // streamed once: do not allocate in L1
 {
@@ -197,6 +190,31 @@ __device__ __forceinline__ int4 ldg_stream(const int4* p)        // streamed onc
     return v;
 }
 __device__ __forceinline__ int word_of(const int4& v, int u) { return u == 0 ? v.x : (u == 1 ? v.y : (u == 2 ? v.z : v.w)); }
+// position gather: one LOP3 + one IMAD.WIDE for the address (the compiler's own sequence re-reads the base pointer from
+// the constant bank and adds with carry: five instructions per gather)
+__device__ __forceinline__ float4 gather_pos(const float4* __restrict__ base, int word)
+{
+    const unsigned idx = (unsigned)word & QNEP_NL_MASK;
+    unsigned long long a;
+    asm("mad.wide.u32 %0, %1, 16, %2;" : "=l"(a) : "r"(idx), "l"(base));
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_pair(unsigned addr, int w, float r2, int second_offset_bytes)
+{
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(w) : "memory");
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr + second_offset_bytes), "f"(r2) : "memory");
+}
+// store of row `row` of a warp-tiled float4 list (rows are QNEP_TILE float4 = 512 bytes apart): one IMAD.WIDE + STG
+__device__ __forceinline__ void stg_tiled_row(float4* base, int row, float x, float y, float z, int w)
+{
+    unsigned long long a;
+    asm("mad.wide.u32 %0, %1, 512, %2;" : "=l"(a) : "r"((unsigned)row), "l"(base));
+    asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(a), "f"(x), "f"(y), "f"(z), "f"(__int_as_float(w)) : "memory");
+}
+__device__ __forceinline__ int lds_b32(unsigned addr) { int v; asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v; }
+__device__ __forceinline__ float lds_f32(unsigned addr) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory"); return v; }
 
 template <int T>
 __global__ void __launch_bounds__(PAIRS_BLOCK)
@@ -206,13 +224,14 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
         float4* __restrict__ lvA, int* __restrict__ nlvA, float* __restrict__ D, int* __restrict__ flags)
 {
     static_assert(PAIRS_CH == 16 && (PAIRS_QCAP & (PAIRS_QCAP - 1)) == 0, "four list vectors per round, power-of-two ring");
-    __shared__ float4 sh_shift[27];
     __shared__ float sh_c[T * T * NR * KP];
-    __shared__ int sh_qe[PAIRS_QCAP][PAIRS_BLOCK];           // ring: words
-    __shared__ float sh_qr[PAIRS_QCAP][PAIRS_BLOCK];         // ring: r^2
-    load_shift_table(sh_shift, g);
+    extern __shared__ __align__(16) unsigned char sh_dyn[];  // PAIRS_SMEM bytes (beyond the 48 KB of static shared memory)
+    int4 (*sh_l)[PAIRS_BLOCK] = reinterpret_cast<int4 (*)[PAIRS_BLOCK]>(sh_dyn);                                      // [PAIRS_LD]: list vectors in flight
+    int (*sh_q)[PAIRS_QCAP][PAIRS_BLOCK] = reinterpret_cast<int (*)[PAIRS_QCAP][PAIRS_BLOCK]>(sh_dyn + sizeof(int4) * PAIRS_LD * PAIRS_BLOCK);   // [2]: ring of words, then r^2 (as bits)
+    constexpr int QROW = PAIRS_BLOCK * 4, QR2 = PAIRS_QCAP * QROW, QMASK = QR2 - 1;   // bytes per slot, offset of the r^2 half, ring wrap
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
     __syncthreads();
+    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
     const int tid = threadIdx.x;
     const int64_t p0 = blockIdx.x * (int64_t)blockDim.x + tid;
     const bool live = p0 < N;                                // threads beyond N stay for the warp votes, with an empty list
@@ -224,16 +243,29 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
 #pragma unroll
     for (int t = 0; t < T; ++t) { segend[t] = (t < T - 1 && live) ? nlRend[(int64_t)t * N + p] : 0x7fffffff; acc_end[t] = 0x7fffffff; }
     const int4* lbase = nl + qnep_tiled_base(p, capR / 4);
-    // list vectors: lv[gv & 3] holds vector gv; while gv is processed, gv + 1 feeds the position gathers (four slots
-    // ahead) and gv + 2, gv + 3 are in flight.  Beyond the end the registers hold the atom itself, so the gathers need no
-    // bound check.
+    // List vectors come through a cp.async ring PAIRS_LD vectors deep in shared memory (they stream from DRAM); vector
+    // gv + 2 is taken from the ring into registers at the top of iteration gv and feeds the position gathers at once
+    // (eight slots ahead: the gathers mostly come from L2), lv[gv & 3] holds the vector being processed.  Beyond the
+    // end the registers hold the atom itself, so the gathers need no bound check.
     const int4 filler = make_int4((int)p, (int)p, (int)p, (int)p);
+#pragma unroll
+    for (int k = 0; k < PAIRS_LD; ++k) {
+        if (k < n4) cp_async16_cg(&sh_l[k][tid], lbase + (int64_t)k * QNEP_TILE);
+        cp_async_commit();
+    }
+    cp_async_wait<PAIRS_LD - 2>();
     int4 lv[4];
+    lv[0] = 0 < n4 ? sh_l[0][tid] : filler;
+    lv[1] = 1 < n4 ? sh_l[1][tid] : filler;
+    lv[2] = filler; lv[3] = filler;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) lv[k] = (k < 3 && k < n4) ? ldg_stream(lbase + (int64_t)k * QNEP_TILE) : filler;
-    float4 ring[4];                                          // ring[u] holds the position of the atom of slot 4 gv + u
+    for (int k = 0; k < 2; ++k) {                            // slots 0 and 1 are free again: vectors PAIRS_LD, PAIRS_LD + 1
+        if (PAIRS_LD + k < n4) cp_async16_cg(&sh_l[k][tid], lbase + (int64_t)(PAIRS_LD + k) * QNEP_TILE);
+        cp_async_commit();
+    }
+    float4 ring[8];                                          // ring[4 (gv & 1) + u] holds the position of the atom of slot 4 gv + u
 #pragma unroll
-    for (int u = 0; u < 4; ++u) ring[u] = xyzt[word_of(lv[0], u) & QNEP_NL_MASK];
+    for (int u = 0; u < 8; ++u) ring[u] = gather_pos(xyzt, word_of(lv[u >> 2], u & 3));
     float S[T][NB];                                          // S^t_k without the "+1" part: sum_j 1/2 fc T_k
     float S1[T];                                             // sum_j 1/2 fc
 #pragma unroll
@@ -245,16 +277,25 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
     int cA_ = 0, head = 0, tail = 0;                         // angular pairs; accepted entries consumed / produced
     int4* outR = lvR + qnep_tiled_base(p, capLR / 4);
     float4* outA = lvA + qnep_tiled_base(p, capLA);
-    int* qe = &sh_qe[0][tid];
-    float* qr = &sh_qr[0][tid];
+    const unsigned qbase = (unsigned)__cvta_generic_to_shared(&sh_q[0][0][tid]);
+    unsigned qoff = 0;                                       // byte offset of the ring slot of accepted entry `tail`
     const int nround = __reduce_max_sync(0xffffffffu, (n4 + 3) >> 2);
     for (int c = 0; c < nround; ++c) {
         // ---- phase 1 ----
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
             const int gv = 4 * c + v;
-            lv[(v + 3) & 3] = filler;                        // beyond the end the gathers below read the atom itself
-            if (gv + 3 < n4) lv[(v + 3) & 3] = ldg_stream(lbase + (int64_t)(gv + 3) * QNEP_TILE);
+            // vector gv + 2 from the ring; its slot is refilled with vector gv + 2 + PAIRS_LD
+            cp_async_wait<PAIRS_LD - 1>();                   // groups issued so far: PAIRS_LD + 2 + gv, one per vector; vector gv + 2 has landed
+            lv[(v + 2) & 3] = gv + 2 < n4 ? sh_l[(gv + 2) & (PAIRS_LD - 1)][tid] : filler;
+            if (gv + 2 + PAIRS_LD < n4) cp_async16_cg(&sh_l[(gv + 2) & (PAIRS_LD - 1)][tid], lbase + (int64_t)(gv + 2 + PAIRS_LD) * QNEP_TILE);
+            cp_async_commit();
+            float4 xjv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                xjv[u] = ring[4 * (v & 1) + u];
+                ring[4 * (v & 1) + u] = gather_pos(xyzt, word_of(lv[(v + 2) & 3], u));
+            }
             int tjv = 0;
 #pragma unroll
             for (int t = 0; t < T - 1; ++t) {
@@ -266,21 +307,16 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int e = word_of(lv[v & 3], u);
-                const float4 xj = ring[u];
-                ring[u] = xyzt[word_of(lv[(v + 1) & 3], u) & QNEP_NL_MASK];
-                const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-                const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+                const float4 xj = xjv[u];
+                float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
+                qnep_add_image_shift(e, h0, h1, h2, dx, dy, dz);
                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                 if (act && r2 < g.rc_r2 && r2 >= 1e-12f) {
-                    const int slot = (tail & (PAIRS_QCAP - 1)) * PAIRS_BLOCK;
-                    qe[slot] = e;
-                    qr[slot] = r2;
+                    sts_pair(qbase + qoff, e, r2, QR2);
+                    qoff = (qoff + QROW) & QMASK;
                     ++tail;
                     if (r2 < g.rc_a2) {
-                        if (cA_ < capLA) {
-                            *outA = make_float4(dx, dy, dz, __int_as_float((e & QNEP_NL_MASK) | tjbits));
-                            outA += QNEP_TILE;
-                        }
+                        if (cA_ < capLA) stg_tiled_row(outA, cA_, dx, dy, dz, (e & QNEP_NL_MASK) | tjbits);
                         ++cA_;
                     }
                 }
@@ -295,13 +331,13 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
         for (int k = 0; k < npop; k += 4) {
             if (k < mine) {
                 int w4[4];
+                const unsigned qa = qbase + (unsigned)((head + k) & (PAIRS_QCAP - 1)) * QROW;   // head + k is a multiple of four: no wrap inside the group
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     const int gidx = head + k + u;                                   // accepted entry number gidx of this atom
-                    const int slot = (gidx & (PAIRS_QCAP - 1)) * PAIRS_BLOCK;
                     const bool valid = k + u < mine;                                 // false only in the tail of the last round
-                    const float r2 = valid ? qr[slot] : 1.f;
-                    w4[u] = valid ? qe[slot] : QNEP_NL_EMPTY;
+                    const float r2 = valid ? lds_f32(qa + u * QROW + QR2) : 1.f;
+                    w4[u] = valid ? lds_b32(qa + u * QROW) : QNEP_NL_EMPTY;
                     // 1/2 fc(r) T_k(x), k = 0..8   (f_k = 1/2 fc (T_k + 1): the "+1" part is accumulated once in S1)
                     const float tt = r2 * fast_rsqrt(r2) * rcinv;
                     const float hfc = valid ? 0.25f + 0.25f * __cosf(3.14159265358979f * tt) : 0.f;
@@ -899,11 +935,9 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                const float* __restrict__ q, float sqrt_eps, const int* __restrict__ sidx, double* __restrict__ out,
                double* __restrict__ sums, const float* __restrict__ Wat, double* __restrict__ atomv_out)
 {
-    __shared__ float4 sh_shift[27];
     __shared__ int4 sh_w[RAD_LV][RAD_BLOCK];
     __shared__ double sh_red[32];
-    load_shift_table(sh_shift, g);
-    __syncthreads();
+    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
     const int tid = threadIdx.x;
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
     float W[9];
@@ -969,8 +1003,8 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                         Pi[0] = o8[3]; Pi[1] = o8[4]; Pi[2] = o8[5]; Pi[3] = o8[6]; Pi[4] = o8[7];
                         Pi[5] = o4.x; Pi[6] = o4.y; Pi[7] = o4.z; Pi[8] = o4.w;
                     }
-                    const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-                    const float dx = (a8[0] - xi.x) + sh.x, dy = (a8[1] - xi.y) + sh.y, dz = (a8[2] - xi.z) + sh.z;
+                    float dx = a8[0] - xi.x, dy = a8[1] - xi.y, dz = a8[2] - xi.z;
+                    qnep_add_image_shift(e, h0, h1, h2, dx, dy, dz);
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     const float rinv = fast_rsqrt(r2), r = r2 * rinv;
                     ChebDeriv cd;
@@ -1094,7 +1128,9 @@ int qnep_launch_pairs(qnep_handle* h, cudaStream_t s)
     const float rcinv = (float)(1.0 / h->model.rc_r);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_pairs<T><<<nb, PAIRS_BLOCK, 0, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlRend, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
+        static bool attr_set = false;                        // one flag per instantiation (the lambda is generic)
+        if (!attr_set) { cudaFuncSetAttribute(k_pairs<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PAIRS_SMEM); attr_set = true; }
+        k_pairs<T><<<nb, PAIRS_BLOCK, PAIRS_SMEM, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlRend, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
                                               h->d_lvR, h->d_nlvR, h->d_lvRend, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
     });
     h->launches += 1;

@@ -36,14 +36,8 @@ k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* 
             const int* __restrict__ nn, const float* __restrict__ q, float alpha, float* __restrict__ phir,
             float* __restrict__ Fs, double* __restrict__ sums, float* __restrict__ Wat /* [9][N] or null */)
 {
-    __shared__ float4 sh_shift[27];
     __shared__ double sh_red[32];
-    if (threadIdx.x < 27) {
-        const int code = threadIdx.x;
-        sh_shift[code] = make_float4((code / 9 - 1) * (float)g.hcell[0], ((code / 3) % 3 - 1) * (float)g.hcell[1],
-                                     (code % 3 - 1) * (float)g.hcell[2], 0.f);
-    }
-    __syncthreads();
+    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     const float Kc = (float)QNEP_K_COULOMB;
     const float two_a_sqrtpi = 2.f * alpha * 0.5641895835477563f;
@@ -59,8 +53,8 @@ k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* 
             const int e = words[(int64_t)(s >> 2) * (4 * QNEP_TILE) + (s & 3)];
             const int j = e & QNEP_NL_MASK;
             const float4 xj = xyzt[j];
-            const float4 sh = sh_shift[(unsigned)e >> QNEP_NL_SHIFT];
-            const float dx = (xj.x - xi.x) + sh.x, dy = (xj.y - xi.y) + sh.y, dz = (xj.z - xi.z) + sh.z;
+            float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
+            qnep_add_image_shift(e, h0, h1, h2, dx, dy, dz);
             const float r2 = dx * dx + dy * dy + dz * dz;
             if (r2 >= g.rc_r2) continue;
             const float r = sqrtf(r2), rinv = 1.f / r;

@@ -8,9 +8,9 @@
 //  * positions are stored as float4 (x, y, z relative to the atom's own cell origin, type bits):
 //    r_ij = off_j - off_i + delta_cell * hcell is formed from small numbers, so fp32 keeps
 //    ~1e-7 A resolution in a 217 A box;
-//  * a neighbour entry packs the sorted index of j (27 bits) and the image code
-//    (dx+1)*9 + (dy+1)*3 + (dz+1) of the cell offset (5 bits): the same atom may appear more than
-//    once through different images when the box is smaller than 2 (r_c + skin);
+//  * a neighbour entry packs the sorted index of j (26 bits) and the cell offset of the image (three signed
+//    2-bit fields): the same atom may appear more than once through different images when the box is smaller
+//    than 2 (r_c + skin);
 //  * lists are column-major [slot][atom] so that a warp reads consecutive words.
 #include "qnep_internal.cuh"
 
@@ -279,7 +279,7 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
             const int k = t * g.ncells + cell;
             const int b = start[k], e = start[k + 1];
             const int self = (code == 13 && t == ti) ? (int)p : -1;
-            const int cbits = code << QNEP_NL_SHIFT;
+            const int cbits = qnep_image_bits(d0, d1, d2);
             auto test = [&](int q, const float4& xj) {
                 const float dx = xj.x - ox, dy = xj.y - oy, dz = xj.z - oz;
                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
@@ -299,7 +299,7 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
         // (r = 0: the per-step filter drops it), so that the four slots of a list vector belong to ONE species and
         // the walkers decide species, bounds and prefetch once per vector.
         while (nR & 3) {
-            if (nR < capR) out[((nR >> 2) << 7) | (nR & 3)] = (int)p | (13 << QNEP_NL_SHIFT);
+            if (nR < capR) out[((nR >> 2) << 7) | (nR & 3)] = (int)p;      // zero cell offset
             ++nR; ++nPad;
         }
         nlRend[(int64_t)t * N + p] = min(nR, capR);

@@ -12,8 +12,8 @@
 
 #define QNEP_MAX_TYPES 4
 #define QNEP_NLM 24                 // real harmonics l = 1..4: 3 + 5 + 7 + 9
-#define QNEP_NL_MASK 0x07ffffff     // neighbour entry: low 27 bits = sorted atom index, high 5 bits = image code 0..26
-#define QNEP_NL_SHIFT 27
+#define QNEP_NL_MASK 0x03ffffff     // neighbour entry: low 26 bits = sorted atom index, high 6 bits = cell offset of the image
+#define QNEP_NL_SHIFT 26            // (three signed 2-bit fields d0, d1, d2 in {-1, 0, 1}, d0 in the top bits); pair lists: species
 #define QNEP_KPAD 12                // Chebyshev coefficient rows padded from 9 to 12 floats (3 x float4)
 #define QNEP_NB 9                   // basis functions k = 0..8 (basis_r = basis_a = 8 in this version)
 #define QNEP_NRAD 5                 // n = 0..4
@@ -37,6 +37,19 @@
 __host__ __device__ __forceinline__ int64_t qnep_tiled_base(int64_t p, int rows_per_atom)
 {
     return ((p >> 5) * (int64_t)rows_per_atom) * QNEP_TILE + (p & 31);
+}
+
+// The cell offset is decoded with shifts and added with one FMA per component (a table in shared memory cost 4-5 L1
+// wavefronts per neighbour in kernels that are bound by L1 wavefronts):  d += (d0, d1, d2) * (h0, h1, h2).
+__host__ __device__ __forceinline__ int qnep_image_bits(int d0, int d1, int d2)
+{
+    return (int)(((unsigned)(d0 & 3) << 30) | ((unsigned)(d1 & 3) << 28) | ((unsigned)(d2 & 3) << 26));
+}
+__device__ __forceinline__ void qnep_add_image_shift(int e, float h0, float h1, float h2, float& dx, float& dy, float& dz)
+{
+    dx = fmaf((float)(e >> 30), h0, dx);
+    dy = fmaf((float)((int)((unsigned)e << 2) >> 30), h1, dy);
+    dz = fmaf((float)((int)((unsigned)e << 4) >> 30), h2, dz);
 }
 
 constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (reading S9)
