@@ -119,6 +119,17 @@ struct ChebDeriv {
         for (int k = 2; k < NB; ++k) du = fmaf(a[k], kU[k], du);
         return fmaf(A, du, B * dt);
     }
+    // the same contraction with a_1..a_8 given as four register pairs (a_1, a_2) .. (a_7, a_8): packed FMAs
+    __device__ __forceinline__ float dot_pairs(float a0, const float2 (&ap)[4]) const
+    {
+        float2 dt = __fmul2_rn(ap[0], make_float2(Tp[1], Tp[2])), du = __fmul2_rn(ap[0], make_float2(1.f, kU[2]));
+#pragma unroll
+        for (int m = 1; m < 4; ++m) {
+            dt = __ffma2_rn(ap[m], make_float2(Tp[2 * m + 1], Tp[2 * m + 2]), dt);
+            du = __ffma2_rn(ap[m], make_float2(kU[2 * m + 1], kU[2 * m + 2]), du);
+        }
+        return fmaf(A, du.x + du.y, B * fmaf(a0, Tp[0], dt.x + dt.y));
+    }
 };
 
 // MUFU.RSQ without the denormal range fix-up of rsqrtf (arguments here are squared distances >= 1e-12)
@@ -415,9 +426,19 @@ __global__ void __launch_bounds__(ANG_BLOCK)
 k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
                const float* __restrict__ cA, float rcinv, float* __restrict__ D, float* __restrict__ Aout)
 {
+    // g_n = sum_k c_nk f_k = 1/2 fc [ (2 c_n0 + sum_{k>=1} c_nk) + sum_{k>=1} c_nk T_k ]: row (ti, tj, n) of the table holds the
+    // bracket's constant in slot 0 and c_n1..c_n8 behind it, so g_n is a dot product with (1, T_1..T_8) in packed FMAs and the
+    // basis functions f_k themselves are never formed.
     __shared__ __align__(16) float sh_c[T * T * NR * KP];
     __shared__ float4 sh_ring[ANG_DEPTH][ANG_BLOCK];
-    for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cA[i];
+    for (int i = threadIdx.x; i < T * T * NR; i += blockDim.x) {
+        const float* c = cA + i * KP;
+        float c0 = 2.f * c[0];
+#pragma unroll
+        for (int k = 1; k < NB; ++k) { c0 += c[k]; sh_c[i * KP + k] = c[k]; }
+        sh_c[i * KP] = c0;
+        sh_c[i * KP + 9] = 0.f; sh_c[i * KP + 10] = 0.f; sh_c[i * KP + 11] = 0.f;
+    }
     __syncthreads();
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
@@ -444,21 +465,25 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
         cp_async_commit();
         const float r2 = pr.x * pr.x + pr.y * pr.y + pr.z * pr.z;
         const float rinv = fast_rsqrt(r2), r = r2 * rinv;
-        float f[KP];
-        cheb_basis<true, false>(r, rcinv, f, nullptr);
-        f[9] = 0.f; f[10] = 0.f; f[11] = 0.f;
+        const float tt = r * rcinv;
+        const float hfc = 0.25f + 0.25f * __cosf(3.14159265358979f * tt);
+        const float tm1 = tt - 1.f;
+        const float xx = 2.f * tm1 * tm1 - 1.f, xx2 = xx + xx;
+        float Tk[NB];                                    // T_1 .. T_8 in Tk[1..8]
+        Tk[0] = 1.f; Tk[1] = xx;
+#pragma unroll
+        for (int k = 2; k < NB; ++k) Tk[k] = fmaf(xx2, Tk[k - 1], -Tk[k - 2]);
         const int tj = (unsigned)__float_as_int(pr.w) >> QNEP_NL_SHIFT;
         const float4* c4 = reinterpret_cast<const float4*>(sh_c + (ti * T + tj) * NR * KP);
         float2 g2[NR];
 #pragma unroll
         for (int a = 0; a < NR; ++a) {
-            // g_n = sum_k c_nk f_k over k pairs (rows are padded to 12 floats with zeros)
-            const float4 ca = c4[a * 3], cb = c4[a * 3 + 1], cc = c4[a * 3 + 2];
-            float2 v = __fmul2_rn(make_float2(ca.x, ca.y), make_float2(f[0], f[1]));
-            v = __ffma2_rn(make_float2(ca.z, ca.w), make_float2(f[2], f[3]), v);
-            v = __ffma2_rn(make_float2(cb.x, cb.y), make_float2(f[4], f[5]), v);
-            v = __ffma2_rn(make_float2(cb.z, cb.w), make_float2(f[6], f[7]), v);
-            const float g = fmaf(cc.x, f[8], v.x + v.y);
+            const float4 ca = c4[a * 3], cb = c4[a * 3 + 1], cc = c4[a * 3 + 2];      // (c0', c1, c2, c3) (c4..c7) (c8, 0, 0, 0)
+            float2 v = __fmul2_rn(make_float2(ca.x, ca.y), make_float2(Tk[0], Tk[1]));     // aligned pairs of the float4 rows
+            v = __ffma2_rn(make_float2(ca.z, ca.w), make_float2(Tk[2], Tk[3]), v);
+            v = __ffma2_rn(make_float2(cb.x, cb.y), make_float2(Tk[4], Tk[5]), v);
+            v = __ffma2_rn(make_float2(cb.z, cb.w), make_float2(Tk[6], Tk[7]), v);
+            const float g = hfc * fmaf(cc.x, Tk[8], v.x + v.y);
             g2[a] = make_float2(g, g);
         }
         float b[NLM];
@@ -499,8 +524,22 @@ __device__ __forceinline__ float tanh_f32(float z)
 }
 
 // Persistent blocks: the weights of all species are staged in shared memory once per block, then the block walks
-// chunks of 128 atoms.
-__global__ void __launch_bounds__(128)
+// chunks of 2 x 128 atoms.  A thread owns TWO atoms (p and p + 128 of the chunk) and keeps their descriptors and both
+// derivative vectors as register pairs (atom A, atom B): a weight read from shared memory serves both atoms, and every
+// update is one packed FMA (FFMA2) with the weight or the per-atom factor as the scalar operand -- half the issue
+// slots per atom of the scalar form, which was bound by issue slots (77 % busy, FMA pipe 63 %).  The two atoms of a
+// thread are of one species except where a chunk straddles a species boundary of the sorted order; there the hidden
+// layer is evaluated once per species with the other atom masked out.
+constexpr int NN_BLOCK = 128;
+#ifndef QNEP_NN_UNROLL
+#define QNEP_NN_UNROLL 2
+#endif
+constexpr int NN_UNROLL = QNEP_NN_UNROLL;
+
+#ifndef QNEP_NN_MINB
+#define QNEP_NN_MINB 2
+#endif
+__global__ void __launch_bounds__(NN_BLOCK, QNEP_NN_MINB)
 k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, float b1U, float b1q,
      const float4* __restrict__ xyzt, const float* __restrict__ D, float* __restrict__ Ui, float* __restrict__ qraw,
      float* __restrict__ FpU, float* __restrict__ FpQ, double* __restrict__ sums)
@@ -514,90 +553,71 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
     }
     __syncthreads();
     double accU = 0.0, accQ = 0.0;
-    for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < N; p += (int64_t)gridDim.x * blockDim.x) {
-        const int ti = __float_as_int(xyzt[p].w);
-        const float* w = sh_w + ti * nn_stride;
-        const float* b0 = w + H * W0P;
-        const float* w1U = b0 + H;
-        const float* w1q = w1U + H;
-#ifndef QNEP_NN_PACK
-#define QNEP_NN_PACK 0
-#endif
-#if QNEP_NN_PACK == 0
-        float x[W0P], dU[W0P], dQ[W0P];
-#pragma unroll
-        for (int v = 0; v < W0P; ++v) { x[v] = v < ND ? D[(int64_t)v * N + p] : 0.f; dU[v] = 0.f; dQ[v] = 0.f; }
-        float U = 0.f, q = 0.f;
-        for (int mu = 0; mu < H; ++mu) {
-            const float4* row = reinterpret_cast<const float4*>(w + mu * W0P);
-            float wr[W0P];
-#pragma unroll
-            for (int v4 = 0; v4 < W0P / 4; ++v4) {
-                const float4 t = row[v4];
-                wr[4 * v4] = t.x; wr[4 * v4 + 1] = t.y; wr[4 * v4 + 2] = t.z; wr[4 * v4 + 3] = t.w;
-            }
-            float z0 = -b0[mu], z1 = 0.f;
-#pragma unroll
-            for (int v = 0; v < ND; v += 2) { z0 = fmaf(wr[v], x[v], z0); if (v + 1 < ND) z1 = fmaf(wr[v + 1], x[v + 1], z1); }
-            const float hmu = tanh_f32(z0 + z1);
-            const float a = w1U[mu], b = w1q[mu];
-            U = fmaf(a, hmu, U);
-            q = fmaf(b, hmu, q);
-            const float dh = fmaf(-hmu, hmu, 1.f);
-            const float au = a * dh, bq = b * dh;
-#pragma unroll
-            for (int v = 0; v < ND; ++v) { dU[v] = fmaf(au, wr[v], dU[v]); dQ[v] = fmaf(bq, wr[v], dQ[v]); }
-        }
-        U -= b1U;
-        q -= b1q;
-        Ui[p] = U;
-        qraw[p] = q;
-#pragma unroll
-        for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + p] = dU[v]; FpQ[(int64_t)v * N + p] = dQ[v]; }
-#else
-        // experiment: the forward dot product scalar, the two backward updates packed (QNEP_NN_PACK = 1)
-        constexpr int NP = W0P / 2;
-        float2 x2[NP], dU2[NP], dQ2[NP];
-#pragma unroll
-        for (int i = 0; i < NP; ++i) {
-            x2[i] = make_float2(2 * i < ND ? D[(int64_t)(2 * i) * N + p] : 0.f, 2 * i + 1 < ND ? D[(int64_t)(2 * i + 1) * N + p] : 0.f);
-            dU2[i] = make_float2(0.f, 0.f);
-            dQ2[i] = make_float2(0.f, 0.f);
-        }
-        float U = 0.f, q = 0.f;
-        for (int mu = 0; mu < H; ++mu) {
-            const float4* row = reinterpret_cast<const float4*>(w + mu * W0P);
-            float2 wr[NP];
-#pragma unroll
-            for (int v4 = 0; v4 < W0P / 4; ++v4) {
-                const float4 t = row[v4];
-                wr[2 * v4] = make_float2(t.x, t.y); wr[2 * v4 + 1] = make_float2(t.z, t.w);
-            }
-            float z0 = -b0[mu], z1 = 0.f;
-#pragma unroll
-            for (int i = 0; i < (ND + 1) / 2; ++i) { z0 = fmaf(wr[i].x, x2[i].x, z0); if (2 * i + 1 < ND) z1 = fmaf(wr[i].y, x2[i].y, z1); }
-            const float hmu = tanh_f32(z0 + z1);
-            const float a = w1U[mu], b = w1q[mu];
-            U = fmaf(a, hmu, U);
-            q = fmaf(b, hmu, q);
-            const float dh = fmaf(-hmu, hmu, 1.f);
-            const float au = a * dh, bq = b * dh;
-            const float2 au2 = make_float2(au, au), bq2 = make_float2(bq, bq);
-#pragma unroll
-            for (int i = 0; i < (ND + 1) / 2; ++i) { dU2[i] = __ffma2_rn(au2, wr[i], dU2[i]); dQ2[i] = __ffma2_rn(bq2, wr[i], dQ2[i]); }
-        }
-        U -= b1U;
-        q -= b1q;
-        Ui[p] = U;
-        qraw[p] = q;
+    const int64_t nchunk = (N + 2 * NN_BLOCK - 1) / (2 * NN_BLOCK);
+    for (int64_t ch = blockIdx.x; ch < nchunk; ch += gridDim.x) {
+        const int64_t pA = ch * (2 * NN_BLOCK) + threadIdx.x, pB = pA + NN_BLOCK;
+        const bool okA = pA < N, okB = pB < N;
+        const int64_t qA = okA ? pA : N - 1, qB = okB ? pB : N - 1;
+        const int tA = __float_as_int(xyzt[qA].w), tB = __float_as_int(xyzt[qB].w);
+        float2 x[ND], dU[ND], dQ[ND];
 #pragma unroll
         for (int v = 0; v < ND; ++v) {
-            FpU[(int64_t)v * N + p] = (v & 1) ? dU2[v >> 1].y : dU2[v >> 1].x;
-            FpQ[(int64_t)v * N + p] = (v & 1) ? dQ2[v >> 1].y : dQ2[v >> 1].x;
+            x[v] = make_float2(D[(int64_t)v * N + qA], D[(int64_t)v * N + qB]);
+            dU[v] = make_float2(0.f, 0.f);
+            dQ[v] = make_float2(0.f, 0.f);
         }
-#endif
-        accU += (double)U;
-        accQ += (double)q;
+        float2 U = make_float2(0.f, 0.f), q = make_float2(0.f, 0.f);
+        const int npass = tA == tB ? 1 : 2;
+        for (int pass = 0; pass < npass; ++pass) {
+            const float* w = sh_w + (pass == 0 ? tA : tB) * nn_stride;
+            const float* b0 = w + H * W0P;
+            const float* w1U = b0 + H;
+            const float* w1q = w1U + H;
+            // which of the two atoms this pass serves (both when the species agree)
+            const float2 on = npass == 1 ? make_float2(1.f, 1.f) : (pass == 0 ? make_float2(1.f, 0.f) : make_float2(0.f, 1.f));
+#pragma unroll NN_UNROLL
+            for (int mu = 0; mu < H; ++mu) {
+                const float4* row = reinterpret_cast<const float4*>(w + mu * W0P);
+                float wr[W0P];
+#pragma unroll
+                for (int v4 = 0; v4 < W0P / 4; ++v4) {
+                    const float4 t = row[v4];
+                    wr[4 * v4] = t.x; wr[4 * v4 + 1] = t.y; wr[4 * v4 + 2] = t.z; wr[4 * v4 + 3] = t.w;
+                }
+                const float nb0 = -b0[mu];
+                float2 zc[4] = {make_float2(nb0, nb0), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};   // four chains
+#pragma unroll
+                for (int v = 0; v < ND; ++v) zc[v & 3] = __ffma2_rn(make_float2(wr[v], wr[v]), x[v], zc[v & 3]);
+                const float2 zs = __fadd2_rn(__fadd2_rn(zc[0], zc[1]), __fadd2_rn(zc[2], zc[3]));
+                const float2 h2 = make_float2(tanh_f32(zs.x), tanh_f32(zs.y));
+                const float a = w1U[mu], b = w1q[mu];
+                const float2 a2 = make_float2(a * on.x, a * on.y), b2 = make_float2(b * on.x, b * on.y);
+                U = __ffma2_rn(a2, h2, U);
+                q = __ffma2_rn(b2, h2, q);
+                const float2 dh = make_float2(fmaf(-h2.x, h2.x, 1.f), fmaf(-h2.y, h2.y, 1.f));
+                const float2 au = __fmul2_rn(a2, dh), bq = __fmul2_rn(b2, dh);
+#pragma unroll
+                for (int v = 0; v < ND; ++v) {
+                    const float2 wv = make_float2(wr[v], wr[v]);
+                    dU[v] = __ffma2_rn(au, wv, dU[v]);
+                    dQ[v] = __ffma2_rn(bq, wv, dQ[v]);
+                }
+            }
+        }
+        U.x -= b1U; U.y -= b1U;
+        q.x -= b1q; q.y -= b1q;
+        if (okA) {
+            Ui[pA] = U.x; qraw[pA] = q.x;
+#pragma unroll
+            for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + pA] = dU[v].x; FpQ[(int64_t)v * N + pA] = dQ[v].x; }
+            accU += (double)U.x; accQ += (double)q.x;
+        }
+        if (okB) {
+            Ui[pB] = U.y; qraw[pB] = q.y;
+#pragma unroll
+            for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + pB] = dU[v].y; FpQ[(int64_t)v * N + pB] = dQ[v].y; }
+            accU += (double)U.y; accQ += (double)q.y;
+        }
     }
     const double su = block_sum(accU, sh_red);
     const double sq = block_sum(accQ, sh_red);
@@ -1018,10 +1038,11 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                         // only s_ij + s_ji is needed: one contraction with P^{i,tj} + P^{j,ti}.  That holds for the TOTAL
                         // virial too: sum_i sum_j r_ij (x) rhat_ij s_ij runs over ordered pairs, and the terms (i, j) and
                         // (j, i) have the same dyad r_ij (x) rhat_ij, so every atom may book 1/2 (s_ij + s_ji) instead of s_ij.
-                        float Ps[NB];
-#pragma unroll
-                        for (int k = 0; k < NB; ++k) Ps[k] = Pi[k] + Pj[k];
-                        sij = 0.5f * cd.dot(Ps);
+                        const float2 Pp[4] = {__fadd2_rn(make_float2(Pi[1], Pi[2]), make_float2(a8[4], a8[5])),
+                                              __fadd2_rn(make_float2(Pi[3], Pi[4]), make_float2(a8[6], a8[7])),
+                                              __fadd2_rn(make_float2(Pi[5], Pi[6]), make_float2(b4.x, b4.y)),
+                                              __fadd2_rn(make_float2(Pi[7], Pi[8]), make_float2(b4.z, b4.w))};
+                        sij = 0.5f * cd.dot_pairs(Pi[0] + a8[3], Pp);
                         sji = sij;
                     }
                     const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
@@ -1159,12 +1180,12 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
     static bool attr_set = false;
     static int sms = 0;
     if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-    const int nb = (int)std::min<int64_t>((N + 127) / 128, (int64_t)sms * 4);      // persistent: 4 blocks of 128 threads per SM
+    const int nb = (int)std::min<int64_t>((N + 2 * NN_BLOCK - 1) / (2 * NN_BLOCK), (int64_t)sms * QNEP_NN_MINB);      // persistent: QNEP_NN_MINB blocks of 128 threads per SM
     if (!attr_set) {
         QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
-    k_nn<<<nb, 128, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
+    k_nn<<<nb, NN_BLOCK, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
                                h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
     const int nb2 = (int)((N + 255) / 256);
     k_neutralise<<<nb2, 256, 0, s>>>(N, h->d_qraw, h->d_sums, h->model.q_total, h->d_sidx, h->d_cm, h->d_q, h->d_qcm, charges_out);
