@@ -127,12 +127,13 @@ def electrostatics(pos, q, box, rc, mode, es, want_rho=False, want_atom_virial=F
     return dict(U=U, phi=phi, F=F, W=W.reshape(3, 3), rho=rho, W_atom=Wat)
 
 
-def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, debug=False, want_atom_virial=False):
-    """The whole force evaluation.  Returns a dict of fp64 arrays."""
+def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, debug=False, want_atom_virial=False, zbl=None):
+    """The whole force evaluation.  Returns a dict of fp64 arrays.  zbl = (r_inner, r_outer, Z per species) switches the
+    ZBL core on for this call (reading Z1)."""
     pos = _f64(pos)
     n = pos.shape[1]
     Dn = model.n_desc
-    energy = np.zeros(5)
+    energy = np.zeros(6)
     forces = np.zeros((3, n))
     virial = np.zeros(9)
     charges = np.zeros(n)
@@ -150,15 +151,44 @@ def compute(model, params, es, pos, types, box, use_bins=True, want_bec=False, d
         out["F_es"] = np.zeros((3, n))
         dbg = _Debug(*[_p(out[k]) for k in ("D", "U_i", "q_raw", "phi", "Fp", "rho", "F_es")])
     mm, ee = _model(model), _es(es)
-    rc_ = lib().orc_compute(C.byref(mm), _p(_f64(params)), C.byref(ee), C.c_int64(n), _p(pos),
+    set_zbl(zbl, model.n_types)
+    try:
+        rc_ = _call_compute(mm, params, ee, n, pos, types, box, use_bins, energy, forces, virial, charges, bec, dbg, wat)
+    finally:
+        set_zbl(None, model.n_types)
+    if rc_ != 0:
+        raise RuntimeError(f"orc_compute failed with code {rc_}")
+    out.update(energy=energy[0], energy_parts=dict(nep=energy[1], r=energy[2], k=energy[3], s=energy[4], zbl=energy[5]),
+               forces=forces, virial=virial.reshape(3, 3), charges=charges, bec=bec, virial_atom=wat)
+    return out
+
+
+def set_zbl(zbl, n_types):
+    f = lib().orc_set_zbl
+    f.restype = None
+    if zbl is None:
+        f(C.c_int(0), C.c_double(0.0), C.c_double(0.0), None, C.c_int(0))
+    else:
+        r1, r2, Z = zbl
+        Z = _f64(np.asarray(Z, dtype=np.float64))
+        assert len(Z) >= n_types
+        f(C.c_int(1), C.c_double(r1), C.c_double(r2), _p(Z), C.c_int(n_types))
+
+
+def zbl_pair(r, Zi, Zj, r1, r2):
+    """(U_ZBL(r), dU_ZBL/dr) of one pair (reading Z1)."""
+    u, du = C.c_double(0.0), C.c_double(0.0)
+    f = lib().orc_zbl_pair
+    f.restype = None
+    f(C.c_double(r), C.c_double(Zi), C.c_double(Zj), C.c_double(r1), C.c_double(r2), C.byref(u), C.byref(du))
+    return u.value, du.value
+
+
+def _call_compute(mm, params, ee, n, pos, types, box, use_bins, energy, forces, virial, charges, bec, dbg, wat):
+    return lib().orc_compute(C.byref(mm), _p(_f64(params)), C.byref(ee), C.c_int64(n), _p(pos),
                             _p(np.ascontiguousarray(types, dtype=np.int32)), _p(_f64(box)),
                             C.c_int(int(use_bins)), _p(energy), _p(forces), _p(virial), _p(charges), _p(bec),
                             C.byref(dbg) if dbg is not None else None, _p(wat))
-    if rc_ != 0:
-        raise RuntimeError(f"orc_compute failed with code {rc_}")
-    out.update(energy=energy[0], energy_parts=dict(nep=energy[1], r=energy[2], k=energy[3], s=energy[4]),
-               forces=forces, virial=virial.reshape(3, 3), charges=charges, bec=bec, virial_atom=wat)
-    return out
 
 
 def response(bec, efield=None, vel=None):
@@ -177,6 +207,8 @@ def response(bec, efield=None, vel=None):
 
 
 def compute_workload(w, **kw):
+    if getattr(w, "zbl", None) is not None and "zbl" not in kw:
+        kw["zbl"] = w.zbl
     return compute(w.model, w.params, w.es, w.pos, w.types, w.box, **kw)
 
 

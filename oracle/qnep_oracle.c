@@ -24,6 +24,8 @@
  *   BEC               :205-227 Eq. 24-28      reading S12
  *   field response    :229-237 Eq. 29-30      F^ext = E.Z, Pdot = sum_i Z_i v_i (orc_response)
  *   PPPM              :266-304 Eq. 34-38      readings G2 (Eq. 36), S10 (W, P = 5), S11 (FFT)
+ *   ZBL core          :39 (NEP4 -> NEP refs)  reading Z1: universal ZBL pair repulsion with a cosine switch (optional,
+ *                                             orc_set_zbl)
  *
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): NaCl Madelung constant,
  * Ewald vs brute-force image sum, alpha independence, U = 1/2 sum q phi + U^s,
@@ -33,7 +35,8 @@
  * alias-sum denominator vs brute force, BEC vs finite differences of q and of the cluster
  * polarization P = sum q~_i r_i (Eq. 26-28), Eq. 1 evaluated by hand (bias signs, per-type blocks),
  * Eq. 29-30 vs the point-charge limit (F = q E, Pdot = sum q v), the power identity, a case evaluated by
- * hand and finite differences of E.P and of P(t) (index order of Z).
+ * hand and finite differences of E.P and of P(t) (index order of Z); ZBL vs the bare-Coulomb limit r -> 0, the switch
+ * end points, finite-difference forces and finite-strain virials.
  * No function here is "parity unpinned".
  *
  * Units: Angstrom, eV, elementary charge.  K = 1/(4 pi eps0) (reading S9).
@@ -76,6 +79,19 @@ typedef struct {
     double *rho;     /* [Nx][Ny][Nz] PPPM charge mesh (z fastest)                   */
     double *F_es;    /* [3][N]       static electrostatic force only                */
 } orc_debug;
+
+void orc_zbl_pair(double r, double Zi, double Zj, double r1, double r2, double *u, double *du);
+/* optional ZBL core (reading Z1), switched on for the calls that follow by orc_set_zbl */
+#define ORC_MAX_TYPES 8
+static struct { int on; double r1, r2; double Z[ORC_MAX_TYPES]; } g_zbl = {0, 0.0, 0.0, {0}};
+
+void orc_set_zbl(int on, double r_inner, double r_outer, const double *Z, int n_types)
+{
+    g_zbl.on = on && r_outer > 0.0;
+    g_zbl.r1 = r_inner;
+    g_zbl.r2 = r_outer;
+    for (int t = 0; t < ORC_MAX_TYPES; ++t) g_zbl.Z[t] = (Z && t < n_types) ? Z[t] : 0.0;
+}
 
 /* ------------------------------------------------------------------------- */
 /* small helpers                                                              */
@@ -978,16 +994,28 @@ int orc_compute(const orc_model *m, const double *params, const orc_es *es, int6
     /* 8.-9. F_i = sum_j (F_ij - F_ji) + static terms (Eq. 11); W = sum_i sum_j r_ij (x) F_ji (Eq. 12) */
     for (int64_t i = 0; i < 3 * n; ++i) forces[i] = Fes[i];
     double Wt[9];
+    double Uzbl = 0.0;
     for (int a = 0; a < 9; ++a) Wt[a] = Wes[a];
     if (bec) for (int64_t i = 0; i < 9 * n; ++i) bec[i] = 0.0;
 #pragma omp parallel
     {
         double Wl[9] = {0};
+        double Uzl = 0.0;
 #pragma omp for schedule(dynamic, 16)
         for (int64_t i = 0; i < n; ++i) {
             int64_t b = nl.start[i], cnt = nl.start[i + 1] - nl.start[i];
             double *Fij = (double *)malloc(sizeof(double) * 3 * (cnt > 0 ? cnt : 1));
             partial_forces_of_atom(&P, types, &nl, i, Fp + i * Dn, Fij);
+            if (g_zbl.on) {
+                /* ZBL site energy U_i = 1/2 sum_j U_ZBL(r_ij): partial force 1/2 U'(r_ij) rhat_ij (reading Z1) */
+                for (int64_t p = 0; p < cnt; ++p) {
+                    double r = nl.d[4 * (b + p) + 3], u, du;
+                    if (r >= g_zbl.r2) continue;
+                    orc_zbl_pair(r, g_zbl.Z[types[i]], g_zbl.Z[types[nl.j[b + p]]], g_zbl.r1, g_zbl.r2, &u, &du);
+                    Uzl += 0.5 * u;
+                    for (int a = 0; a < 3; ++a) Fij[3 * p + a] += 0.5 * du * nl.d[4 * (b + p) + a] / r;
+                }
+            }
             for (int64_t p = 0; p < cnt; ++p) {
                 int64_t j = nl.j[b + p];
                 for (int a = 0; a < 3; ++a) {
@@ -1027,7 +1055,10 @@ int orc_compute(const orc_model *m, const double *params, const orc_es *es, int6
             free(Fij);
         }
 #pragma omp critical
-        for (int a = 0; a < 9; ++a) Wt[a] += Wl[a];
+        {
+            for (int a = 0; a < 9; ++a) Wt[a] += Wl[a];
+            Uzbl += Uzl;
+        }
     }
     if (bec)
         for (int64_t i = 0; i < n; ++i)
@@ -1040,11 +1071,45 @@ int orc_compute(const orc_model *m, const double *params, const orc_es *es, int6
     energy[2] = U3[0];
     energy[3] = U3[1];
     energy[4] = U3[2];
-    energy[0] = Unep + U3[0] + U3[1] + U3[2];
+    energy[5] = Uzbl;
+    energy[0] = Unep + U3[0] + U3[1] + U3[2] + Uzbl;
     for (int64_t i = 0; i < n; ++i) charges[i] = q[i];
     nlist_free(&nl);
     free(w); free(D); free(dU); free(dq); free(Ui); free(q); free(phi); free(Fes);
     return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* ZBL core repulsion (reading Z1; the paper defers to the NEP papers, :39)      */
+/* ------------------------------------------------------------------------- */
+/* U_ZBL(r) = K Z_i Z_j / r * phi(r / a) * f_sw(r),   a = 0.46850 / (Z_i^0.23 + Z_j^0.23) Angstrom,
+ * phi(x) = 0.18175 e^{-3.19980 x} + 0.50986 e^{-0.94229 x} + 0.28022 e^{-0.40290 x} + 0.02817 e^{-0.20162 x}
+ * (the universal screening function of Ziegler, Biersack and Littmark),
+ * f_sw = 1 for r < r_1, 1/2 [1 + cos(pi (r - r_1) / (r_2 - r_1))] for r_1 <= r < r_2, 0 beyond.
+ * The term enters as a site energy U_i^ZBL = 1/2 sum_j U_ZBL(r_ij), i.e. a partial force
+ * dU_i/dr_ij = 1/2 U'_ZBL(r_ij) rhat_ij that goes through Eq. 11 and Eq. 12 like the NEP ones. */
+void orc_zbl_pair(double r, double Zi, double Zj, double r1, double r2, double *u, double *du)
+{
+    static const double cphi[4] = {0.18175, 0.50986, 0.28022, 0.02817};
+    static const double dphi[4] = {3.19980, 0.94229, 0.40290, 0.20162};
+    *u = 0.0; *du = 0.0;
+    if (r >= r2) return;
+    double a = 0.46850 / (pow(Zi, 0.23) + pow(Zj, 0.23));
+    double x = r / a, phi = 0.0, dphidr = 0.0;
+    for (int k = 0; k < 4; ++k) {
+        double e = cphi[k] * exp(-dphi[k] * x);
+        phi += e;
+        dphidr -= dphi[k] / a * e;
+    }
+    double fsw = 1.0, dfsw = 0.0;
+    if (r >= r1) {
+        double t = ORC_PI * (r - r1) / (r2 - r1);
+        fsw = 0.5 * (1.0 + cos(t));
+        dfsw = -0.5 * sin(t) * ORC_PI / (r2 - r1);
+    }
+    double c = ORC_K_COULOMB * Zi * Zj / r;              /* bare Coulomb repulsion of the nuclei */
+    *u = c * phi * fsw;
+    *du = -c / r * phi * fsw + c * dphidr * fsw + c * phi * dfsw;
 }
 
 /* ------------------------------------------------------------------------- */

@@ -83,6 +83,7 @@ class Workload:
     params: np.ndarray        # float32 [n_params]
     es: EsDesc
     masses: np.ndarray = field(default=None)  # amu per type (MD only)
+    zbl: tuple = None         # optional ZBL core: (r_inner, r_outer, Z per species) (reading Z1)
     extra: dict = field(default_factory=dict)
 
     @property

@@ -753,3 +753,91 @@ def test_atom_virial_full_model_sums_to_total(oracle, mode, method):
     Wat = out["virial_atom"].reshape(3, 3, -1)
     assert np.abs(Wat.sum(axis=2) - out["virial"]).max() < 1e-11 * np.abs(out["virial"]).max()
     assert np.abs(Wat).max() > 1e-2
+
+
+# --------------------------------------------------- ZBL core (reading Z1)
+def test_zbl_pair_limits_and_switch(oracle):
+    """The screening function is normalised (phi(0) = 1), so U_ZBL -> K Z_i Z_j / r for r -> 0 (bare nuclei); the switch
+    leaves the function untouched below r_1, takes it to zero with zero slope at r_2, and dU/dr is the derivative of U."""
+    K = 14.3996454784
+    for (Zi, Zj) in ((8.0, 1.0), (56.0, 22.0)):
+        a = 0.46850 / (Zi ** 0.23 + Zj ** 0.23)
+        for r in (1e-6, 1e-5):
+            u, du = oracle.zbl_pair(r, Zi, Zj, 0.5, 1.0)
+            # first-order screening correction: phi(x) = 1 - (sum_k c_k d_k) x + O(x^2)
+            slope = 0.18175 * 3.19980 + 0.50986 * 0.94229 + 0.28022 * 0.40290 + 0.02817 * 0.20162
+            assert abs(u * r / (K * Zi * Zj) - (1.0 - slope * r / a)) < 3.0 * (r / a) ** 2 + 1e-12      # O(x^2) remainder
+        # below r_1 the switch is inactive: the value does not depend on (r_1, r_2)
+        assert oracle.zbl_pair(0.4, Zi, Zj, 0.5, 1.0) == oracle.zbl_pair(0.4, Zi, Zj, 0.45, 3.0)
+        # end of the switch: value and slope vanish, and nothing beyond
+        u2, du2 = oracle.zbl_pair(1.0 - 1e-9, Zi, Zj, 0.5, 1.0)
+        assert abs(u2) < 1e-12 * K * Zi * Zj and abs(du2) < 1e-6 * K * Zi * Zj
+        assert oracle.zbl_pair(1.0, Zi, Zj, 0.5, 1.0) == (0.0, 0.0)
+        # continuity of value and slope across r_1, and dU/dr against central differences inside the switch
+        ua, dua = oracle.zbl_pair(0.5 - 1e-9, Zi, Zj, 0.5, 1.0)
+        ub, dub = oracle.zbl_pair(0.5 + 1e-9, Zi, Zj, 0.5, 1.0)
+        assert abs(ua - ub) < 1e-6 * abs(ua) and abs(dua - dub) < 1e-6 * abs(dua)
+        for r in (0.3, 0.6, 0.9):
+            h = 1e-6
+            fd = (oracle.zbl_pair(r + h, Zi, Zj, 0.5, 1.0)[0] - oracle.zbl_pair(r - h, Zi, Zj, 0.5, 1.0)[0]) / (2 * h)
+            assert abs(fd - oracle.zbl_pair(r, Zi, Zj, 0.5, 1.0)[1]) < 1e-7 * abs(fd)
+        # repulsive and monotonically decreasing
+        us = [oracle.zbl_pair(r, Zi, Zj, 0.5, 1.0)[0] for r in np.linspace(0.05, 0.99, 40)]
+        assert all(x > y > 0 for x, y in zip(us, us[1:]))
+
+
+def test_zbl_dimer_energy_is_the_pair_function(oracle):
+    """Two atoms far from everything: the ZBL part of the energy is exactly U_ZBL(r) (1/2 per atom, one pair), the force is
+    -U'(r) along the bond, and the term vanishes when the pair is beyond r_2."""
+    w = I.config0(mode=2)
+    w.es = replace(w.es, method=0)
+    L = 40.0
+    box = np.diag([L, L, L]).ravel()
+    types = np.array([0, 1], dtype=np.int32)
+    zbl = (1.0, 2.0, (11.0, 17.0))
+    for r in (0.8, 1.5, 2.5):
+        pos = np.array([[5.0, 5.0 + r * 0.6], [7.0, 7.0 + r * 0.8], [9.0, 9.0]])
+        on = oracle.compute(w.model, w.params, w.es, pos, types, box, use_bins=False, zbl=zbl)
+        off = oracle.compute(w.model, w.params, w.es, pos, types, box, use_bins=False)
+        u, du = oracle.zbl_pair(r, 11.0, 17.0, 1.0, 2.0)
+        assert abs(on["energy_parts"]["zbl"] - u) < 1e-12 * max(1.0, abs(u))
+        assert abs((on["energy"] - off["energy"]) - u) < 1e-10 * max(1.0, abs(u))
+        dF = on["forces"] - off["forces"]
+        bond = np.array([0.6, 0.8, 0.0])
+        assert np.allclose(dF[:, 1], -du * bond, atol=1e-10 * max(1.0, abs(du)))
+        assert np.allclose(dF[:, 0], du * bond, atol=1e-10 * max(1.0, abs(du)))
+        if r > 2.0:
+            assert u == 0.0 and on["energy_parts"]["zbl"] == 0.0
+
+
+def test_zbl_forces_and_virial_in_the_full_model(oracle):
+    """With the ZBL term on (r_2 = 3.5 A on the 2.82 A lattice of config 0, so every nearest-neighbour pair is inside the
+    switch), forces are still -dE/dr, the virial is -dE/d(strain), and the per-atom virial sums to the total."""
+    w = _small_workload(2, 0.3)
+    zbl = (1.5, 3.5, (11.0, 17.0))
+    out = oracle.compute_workload(w, use_bins=False, zbl=zbl, want_atom_virial=True)
+    base = oracle.compute_workload(w, use_bins=False)
+    assert out["energy_parts"]["zbl"] > 1.0 and rel_rms(out["forces"], base["forces"]) > 1e-2
+    h = 1e-5
+    for (a, i) in ((0, 3), (2, 40)):
+        p1, p2 = w.pos.copy(), w.pos.copy()
+        p1[a, i] += h
+        p2[a, i] -= h
+        e1 = oracle.compute(w.model, w.params, w.es, p1, w.types, w.box, use_bins=False, zbl=zbl)["energy"]
+        e2 = oracle.compute(w.model, w.params, w.es, p2, w.types, w.box, use_bins=False, zbl=zbl)["energy"]
+        fd = -(e1 - e2) / (2 * h)
+        assert abs(fd - out["forces"][a, i]) < 2e-7 * max(1.0, abs(fd)), (fd, out["forces"][a, i])
+    for (a, b) in ((0, 0), (1, 2)):
+        eps = np.zeros((3, 3))
+        eps[a, b] = h
+        def energy(sign):
+            Fm = np.eye(3) + sign * eps
+            return oracle.compute(w.model, w.params, w.es, Fm @ w.pos, w.types,
+                                  (w.box.reshape(3, 3) @ Fm.T).ravel(), use_bins=False, zbl=zbl)["energy"]
+        fd = -(energy(1) - energy(-1)) / (2 * h)
+        assert abs(fd - out["virial"][a, b]) < 1e-6 * np.abs(out["virial"]).max(), (fd, out["virial"][a, b])
+    assert np.abs(out["forces"].sum(axis=1)).max() < 1e-9
+    assert np.allclose(out["virial_atom"].sum(axis=1).reshape(3, 3), out["virial"], atol=1e-9 * np.abs(out["virial"]).max())
+    # the switch-off state leaks nowhere: a later call without zbl is the plain model again
+    again = oracle.compute_workload(w, use_bins=False)
+    assert abs(again["energy"] - base["energy"]) < 1e-12 and again["energy_parts"]["zbl"] == 0.0
