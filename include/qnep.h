@@ -219,6 +219,19 @@ int qnep_set_md_graphs(qnep_handle *h, int32_t mode);
  */
 int qnep_set_pppm_kernels(qnep_handle *h, int32_t mode);
 
+/*
+ * Optional ZBL core repulsion (the paper defers to the NEP papers for it, PAPER.md :39; DESIGN.md
+ * reading Z1).  enabled != 0 adds to every pair closer than r_outer the universal Ziegler-Biersack-Littmark potential
+ *     U(r) = K Z_i Z_j / r * phi(r / a) * f_sw(r),   a = 0.46850 / (Z_i^0.23 + Z_j^0.23) Angstrom,
+ *     phi(x) = 0.18175 e^{-3.19980 x} + 0.50986 e^{-0.94229 x} + 0.28022 e^{-0.40290 x} + 0.02817 e^{-0.20162 x},
+ *     f_sw = 1 below r_inner, 1/2 [1 + cos(pi (r - r_inner) / (r_outer - r_inner))] up to r_outer, 0 beyond,
+ * as a site energy 1/2 sum_j U(r_ij) per atom: it enters energy, forces, virial and per-atom virial; charges and
+ * Born effective charges do not depend on it.  z_host [n_types] (HOST): atomic numbers, read during the call.
+ * The term is evaluated on the angular pair list, hence r_outer <= rc_a.  enabled == 0 switches it off (other arguments
+ * ignored).  Errors: INVALID_ARG (radii, atomic numbers), UNSUPPORTED (r_outer > rc_a).
+ */
+int qnep_set_zbl(qnep_handle *h, int32_t enabled, double r_inner, double r_outer, const double *z_host);
+
 /* Synchronise the stream of the last call and report its device-side error state (OK, NEIGHBOR_OVERFLOW, SKIN_VIOLATED, CUDA). */
 int qnep_check(qnep_handle *h);
 

@@ -230,15 +230,11 @@ int consume_flags(qnep_handle* h)
 __global__ void k_finalize(const double* __restrict__ sums, int mode, double* __restrict__ energy, double* __restrict__ virial)
 {
     if (threadIdx.x == 0 && energy) {
-        double e = sums[SUM_E_NEP] + sums[SUM_U_K];
+        double e = sums[SUM_E_NEP] + sums[SUM_U_K] + qnep_striped_sum(sums, 9);      // stripe slot 9: ZBL energy
         if (mode == 1) e += sums[SUM_U_R] + sums[SUM_U_S];
         energy[0] = e;
     }
-    if (threadIdx.x < 9 && virial) {
-        double w = sums[SUM_W0 + threadIdx.x];
-        for (int st = 0; st < QNEP_WSTRIPES; ++st) w += sums[SUM_COUNT + st * 9 + threadIdx.x];
-        virial[threadIdx.x] = w;
-    }
+    if (threadIdx.x < 9 && virial) virial[threadIdx.x] = sums[SUM_W0 + threadIdx.x] + qnep_striped_sum(sums, threadIdx.x);
 }
 
 // ---- debug / parity helpers -----------------------------------------------------------------------
@@ -262,7 +258,8 @@ __global__ void k_dbg_copy(int64_t n, const float* __restrict__ src, double* __r
 
 __global__ void k_dbg_energy(const double* __restrict__ sums, double* __restrict__ dst)
 {
-    dst[0] = sums[SUM_E_NEP]; dst[1] = sums[SUM_U_R]; dst[2] = sums[SUM_U_K]; dst[3] = sums[SUM_U_S];
+    dst[0] = sums[SUM_E_NEP] + qnep_striped_sum(sums, 9);      // short-ranged part: network site energies + ZBL core
+    dst[1] = sums[SUM_U_R]; dst[2] = sums[SUM_U_K]; dst[3] = sums[SUM_U_S];
 }
 
 // ---- velocity-Verlet kernels ----------------------------------------------------------------------
@@ -312,7 +309,7 @@ __global__ void k_vv_kick(int64_t N, double* __restrict__ vel, const double* __r
 
 __global__ void k_md_energy(const double* __restrict__ sums, int mode, double* __restrict__ out)
 {
-    double e = sums[SUM_E_NEP] + sums[SUM_U_K];
+    double e = sums[SUM_E_NEP] + sums[SUM_U_K] + qnep_striped_sum(sums, 9);
     if (mode == 1) e += sums[SUM_U_R] + sums[SUM_U_S];
     out[0] = e;
     out[1] = sums[SUM_KE];
@@ -673,6 +670,31 @@ int qnep_set_pppm_kernels(qnep_handle* h, int32_t mode)
     if (mode < 0 || mode > 2) { h->err = "qnep_set_pppm_kernels: mode must be 0, 1 or 2"; return QNEP_ERR_INVALID_ARG; }
     h->pppm_kernels = mode;
     h->ws_generation += 1;      // captured MD graphs hold the old kernels
+    return QNEP_OK;
+}
+
+int qnep_set_zbl(qnep_handle* h, int32_t enabled, double r_inner, double r_outer, const double* z_host)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    ZblParams z = {};
+    if (enabled) {
+        if (!z_host || !(r_inner >= 0.0) || !(r_outer > r_inner)) { h->err = "qnep_set_zbl: need 0 <= r_inner < r_outer and atomic numbers"; return QNEP_ERR_INVALID_ARG; }
+        if (r_outer > h->model.rc_a) { h->err = "qnep_set_zbl: r_outer beyond the angular cutoff (the core is evaluated on the angular pair list)"; return QNEP_ERR_UNSUPPORTED; }
+        const int T = h->model.n_types;
+        for (int t = 0; t < T; ++t)
+            if (!(z_host[t] > 0.0)) { h->err = "qnep_set_zbl: atomic numbers must be positive"; return QNEP_ERR_INVALID_ARG; }
+        z.on = 1;
+        z.r1 = (float)r_inner; z.r2 = (float)r_outer; z.r2sq = (float)(r_outer * r_outer);
+        z.sw = (float)(M_PI / (r_outer - r_inner));
+        for (int a = 0; a < T; ++a)
+            for (int b = 0; b < T; ++b) {
+                z.kzz[a][b] = (float)(QNEP_K_COULOMB * z_host[a] * z_host[b]);
+                z.ainv[a][b] = (float)((std::pow(z_host[a], 0.23) + std::pow(z_host[b], 0.23)) / 0.46850);
+            }
+    }
+    h->zbl = z;
+    h->ws_generation += 1;      // captured MD graphs hold the old kernel arguments
+    h->md_have_forces = false;
     return QNEP_OK;
 }
 

@@ -421,10 +421,11 @@ __device__ __forceinline__ void harmonics(float x, float y, float z, float* __re
 constexpr int ANG_BLOCK = 64, ANG_DEPTH = 8;
 constexpr int FA_KP2 = 10;     // float2 per row of the packed coefficient table of k_force_angular
 
-template <int T>
+template <int T, bool ZBL>
 __global__ void __launch_bounds__(ANG_BLOCK)
 k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
-               const float* __restrict__ cA, float rcinv, float* __restrict__ D, float* __restrict__ Aout)
+               const float* __restrict__ cA, float rcinv, float* __restrict__ D, float* __restrict__ Aout,
+               ZblParams zbl, double* __restrict__ sums)
 {
     // g_n = sum_k c_nk f_k = 1/2 fc [ (2 c_n0 + sum_{k>=1} c_nk) + sum_{k>=1} c_nk T_k ]: row (ti, tj, n) of the table holds the
     // bracket's constant in slot 0 and c_n1..c_n8 behind it, so g_n is a dot product with (1, T_1..T_8) in packed FMAs and the
@@ -440,9 +441,11 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
         sh_c[i * KP + 9] = 0.f; sh_c[i * KP + 10] = 0.f; sh_c[i * KP + 11] = 0.f;
     }
     __syncthreads();
-    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (p >= N) return;
+    const int64_t p0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = p0 < N;                                // threads beyond N stay for the warp sum of the ZBL energy
+    const int64_t p = live ? p0 : N - 1;
     const int ti = __float_as_int(xyzt[p].w);
+    float ezbl = 0.f;                                        // 1/2 sum_j U_ZBL(r_ij) of this atom (qnep_set_zbl)
     // accumulators as register pairs: the 120 updates A_nlm += g_n b_lm of a neighbour are 60 packed FMAs (FFMA2:
     // two FP32 FMAs per issued instruction; this kernel is bound by issue slots, not by latency)
     float2 A2[NR][NLM / 2];
@@ -450,7 +453,7 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
     for (int a = 0; a < NR; ++a)
 #pragma unroll
         for (int m = 0; m < NLM / 2; ++m) A2[a][m] = make_float2(0.f, 0.f);
-    const int n = nlvA[p];
+    const int n = live ? nlvA[p] : 0;
     const float4* rows = lvA + qnep_tiled_base(p, capLA);
     const int tid = threadIdx.x;
 #pragma unroll
@@ -465,6 +468,11 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
         cp_async_commit();
         const float r2 = pr.x * pr.x + pr.y * pr.y + pr.z * pr.z;
         const float rinv = fast_rsqrt(r2), r = r2 * rinv;
+        if (ZBL && r2 < zbl.r2sq) {
+            float u, du;
+            qnep_zbl_eval(zbl, ti, (int)((unsigned)__float_as_int(pr.w) >> QNEP_NL_SHIFT), r, rinv, u, du);
+            ezbl = fmaf(0.5f, u, ezbl);
+        }
         const float tt = r * rcinv;
         const float hfc = 0.25f + 0.25f * __cosf(3.14159265358979f * tt);
         const float tm1 = tt - 1.f;
@@ -493,6 +501,13 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
 #pragma unroll
             for (int m = 0; m < NLM / 2; ++m) A2[a][m] = __ffma2_rn(g2[a], make_float2(b[2 * m], b[2 * m + 1]), A2[a][m]);
     }
+    if (ZBL) {
+        double e = (double)ezbl;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+        if ((tid & 31) == 0 && e != 0.0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * QNEP_WSTRIDE + 9], e);
+    }
+    if (!live) return;
 #pragma unroll
     for (int a = 0; a < NR; ++a) {
         float d[4] = {0.f, 0.f, 0.f, 0.f};
@@ -646,7 +661,7 @@ __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const do
 // ------------------------------------------------------------------------------------------
 // ATOMV (with VIRIAL, not BEC): the pair term -r_ij (x) F_ij belongs to the per-atom virial of atom j (Eq. 12:
 // W_j = sum_i r_ji (x) F_ij) and is scattered to rows 3..11 of Facc.
-template <int T, bool BEC, bool VIRIAL, bool ATOMV = false>
+template <int T, bool BEC, bool VIRIAL, bool ATOMV = false, bool ZBL = false>
 #ifndef QNEP_FA_VIR_BLOCKS
 #define QNEP_FA_VIR_BLOCKS 4
 #endif
@@ -658,7 +673,7 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                 const float* __restrict__ cA, const float* __restrict__ cR, float rcinv, const float* __restrict__ FpU,
                 const float* __restrict__ FpQ, const float* __restrict__ phi, float sqrt_eps, const float* __restrict__ Ain,
                 float* __restrict__ Fp, float* __restrict__ recA, float4* __restrict__ recB, float* __restrict__ Facc,
-                double* __restrict__ sums)
+                double* __restrict__ sums, ZblParams zbl)
 {
     // Packed angular coefficient table for the loop below: row (ti, tj, n) holds ten float2,
     //   [0] = (2 c_0 + sum_{k>=1} c_k, 0)  and  [k] = (c_k, k c_k), k = 1..8   ([9] is padding),
@@ -882,7 +897,13 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                 vz2 = __ffma2_rn(G_, make_float2(cx, cy), vz2);
             }
 #undef QNEP_HPAIR
-            const float s0 = s02.x + s02.y;
+            float s0 = s02.x + s02.y;
+            if (!BEC && ZBL && r2 < zbl.r2sq) {
+                // ZBL site energy 1/2 sum_j U(r_ij): partial force 1/2 U'(r_ij) rhat_ij, booked like the NEP ones (reading Z1)
+                float u, du;
+                qnep_zbl_eval(zbl, ti, (int)((unsigned)jw >> QNEP_NL_SHIFT), r, rinv, u, du);
+                s0 = fmaf(0.5f, du, s0);
+            }
             const float vx = vxs + (vx2.x + vx2.y), vy = vys + (vy2.x + vy2.y), vz = vz2.x + vz2.y;
             const float uv = x * vx + y * vy + z * vz;
             const float fx = s0 * x + (vx - uv * x) * rinv;
@@ -921,7 +942,7 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
 #pragma unroll
         for (int a = 0; a < 9; ++a) {
             const double w = block_sum((double)W[a], sh_red);
-            if (threadIdx.x == 0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * 9 + a], -w);
+            if (threadIdx.x == 0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * QNEP_WSTRIDE + a], -w);
         }
     }
 }
@@ -1103,7 +1124,7 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
 #pragma unroll
         for (int a = 0; a < 9; ++a) {
             const double w = block_sum((double)W[a], sh_red);
-            if (threadIdx.x == 0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * 9 + a], -w);
+            if (threadIdx.x == 0) atomicAdd(&sums[SUM_COUNT + (blockIdx.x % QNEP_WSTRIPES) * QNEP_WSTRIDE + a], -w);
         }
     }
 }
@@ -1166,7 +1187,8 @@ int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s)
     const float rcinv = (float)(1.0 / h->model.rc_a);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        k_desc_angular<T><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A);
+        if (h->zbl.on) k_desc_angular<T, true><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A, h->zbl, h->d_sums);
+        else k_desc_angular<T, false><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A, h->zbl, h->d_sums);
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -1202,15 +1224,14 @@ int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, bool atomv,
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_Facc, 0, sizeof(float) * (bec ? 9 : (atomv ? 12 : 3)) * N, s));
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-#define QNEP_FA(B, V) k_force_angular<T, B, V><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv, \
-                                                                         h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf, \
-                                                                         h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums)
-        if (bec) QNEP_FA(true, false);
-        else if (atomv) k_force_angular<T, false, true, true><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv,
-                                                                                       h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf,
-                                                                                       h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums);
-        else if (virial) QNEP_FA(false, true);
-        else QNEP_FA(false, false);
+#define QNEP_FA(B, V, A, Z) k_force_angular<T, B, V, A, Z><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv, \
+                                                                                     h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf, \
+                                                                                     h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums, h->zbl)
+        const bool zb = h->zbl.on != 0;
+        if (bec) QNEP_FA(true, false, false, false);                 // the Born effective charges do not see the ZBL core
+        else if (atomv) { if (zb) QNEP_FA(false, true, true, true); else QNEP_FA(false, true, true, false); }
+        else if (virial) { if (zb) QNEP_FA(false, true, false, true); else QNEP_FA(false, true, false, false); }
+        else { if (zb) QNEP_FA(false, false, false, true); else QNEP_FA(false, false, false, false); }
 #undef QNEP_FA
     });
     h->launches += 1;

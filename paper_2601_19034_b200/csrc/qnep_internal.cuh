@@ -60,7 +60,41 @@ enum { SUM_E_NEP = 0, SUM_Q, SUM_PHI, SUM_U_R, SUM_U_K, SUM_U_S, SUM_W0 /* 9 ent
 // are spread over QNEP_WSTRIPES copies behind the named slots (stripe = block index mod QNEP_WSTRIPES); k_finalize adds
 // the stripes to SUM_W0.
 #define QNEP_WSTRIPES 64
-#define QNEP_SUM_ALLOC (SUM_COUNT + QNEP_WSTRIPES * 9)
+#define QNEP_WSTRIDE 10              // per stripe: nine virial components, then the ZBL energy (one add per warp of k_desc_angular)
+#define QNEP_SUM_ALLOC (SUM_COUNT + QNEP_WSTRIPES * QNEP_WSTRIDE)
+__device__ __forceinline__ double qnep_striped_sum(const double* sums, int slot)
+{
+    double v = 0.0;
+    for (int st = 0; st < QNEP_WSTRIPES; ++st) v += sums[SUM_COUNT + st * QNEP_WSTRIDE + slot];
+    return v;
+}
+
+// Optional ZBL core (include/qnep.h qnep_set_zbl; reading Z1), passed to the angular kernels by value:
+//   U(r) = kzz / r * phi(r * ainv) * f_sw(r),  phi = sum_k c_k exp(-d_k x),  f_sw the cosine switch r1 .. r2
+struct ZblParams {
+    int on;
+    float r1, r2, r2sq, sw;              // sw = pi / (r2 - r1)
+    float kzz[QNEP_MAX_TYPES][QNEP_MAX_TYPES];   // K Z_i Z_j
+    float ainv[QNEP_MAX_TYPES][QNEP_MAX_TYPES];  // (Z_i^0.23 + Z_j^0.23) / 0.46850
+};
+__device__ __forceinline__ void qnep_zbl_eval(const ZblParams& z, int ti, int tj, float r, float rinv, float& u, float& du)
+{
+    const float a = z.ainv[ti][tj], x = r * a;
+    const float e0 = 0.18175f * __expf(-3.19980f * x), e1 = 0.50986f * __expf(-0.94229f * x);
+    const float e2 = 0.28022f * __expf(-0.40290f * x), e3 = 0.02817f * __expf(-0.20162f * x);
+    const float phi = (e0 + e1) + (e2 + e3);
+    const float dphi = -a * (3.19980f * e0 + 0.94229f * e1 + 0.40290f * e2 + 0.20162f * e3);
+    float fsw = 1.f, dfsw = 0.f;
+    if (r >= z.r1) {
+        float sn, cs;
+        __sincosf(z.sw * (r - z.r1), &sn, &cs);
+        fsw = 0.5f + 0.5f * cs;
+        dfsw = -0.5f * z.sw * sn;
+    }
+    const float c = z.kzz[ti][tj] * rinv;
+    u = c * phi * fsw;
+    du = c * (fsw * (dphi - phi * rinv) + phi * dfsw);
+}
 // device-side int flags
 // overflow flags hold the largest count seen when a list exceeded its capacity (0 otherwise)
 enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_BAD_TYPE /* a species index outside 0..T-1 */, FLAG_COUNT = 8 };
@@ -170,6 +204,7 @@ struct qnep_handle {
     uint32_t md_want = 0;            // extra outputs of the evaluations inside qnep_md_run (qnep_md_set_outputs)
     double* md_virial = nullptr;
     double* md_charges = nullptr;
+    ZblParams zbl = {};              // optional ZBL core (qnep_set_zbl)
 
     // Ewald
     int nk = 0;
@@ -230,7 +265,7 @@ int qnep_launch_prep(qnep_handle* h, const double* pos, bool at_build, cudaStrea
 int qnep_launch_list_stats(qnep_handle* h, double out[6], cudaStream_t s);
 // descriptor.cu
 int qnep_launch_pairs(qnep_handle* h, cudaStream_t s);
-int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s);
+int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s);       // adds the ZBL energy when the core is on
 int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s);
 int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, bool atomv, cudaStream_t s);
 int qnep_launch_force_radial(qnep_handle* h, bool bec, bool virial, double* out, double* atomv_out, cudaStream_t s);

@@ -274,6 +274,54 @@ def test_atom_virial_parity(torch, oracle, case):
     assert_parity(w, again, ref, f"plain call after the atom virial call, {case}")
 
 
+# ---------------------------------------------------------------- ZBL core (reading Z1)
+@pytest.mark.parametrize("case", ["config0_lattice", "config1_water_bonds", "config2_garnet"])
+def test_zbl_parity(torch, oracle, case):
+    """qnep_set_zbl against the oracle's ZBL term: energy, forces, virial, per-atom virial; charges and the Born effective
+    charges do not change; switching it off restores the plain model; r_outer beyond the angular cutoff is refused."""
+    if case == "config0_lattice":
+        w = I.config0(mode=1)
+        w.zbl = (1.5, 3.5, (11.0, 17.0))          # every nearest-neighbour pair (2.82 A) sits inside the switch
+        bins = False
+    elif case == "config1_water_bonds":
+        w = I.config1()
+        w.zbl = (0.5, 1.0, (8.0, 1.0))            # the O-H bonds (0.96 A) are inside the switch
+        bins = True
+    else:
+        w = I.config2()
+        w.zbl = (1.0, 2.0, (3.0, 57.0, 40.0, 8.0))   # four species, closest pairs at 1.6 A
+        bins = True
+    ref = oracle.compute_workload(w, use_bins=bins, want_atom_virial=True, want_bec=True)
+    plain = oracle.compute_workload(replace(w, zbl=None), use_bins=bins)
+    assert ref["energy_parts"]["zbl"] > 1e-3 * w.n_atoms and rel_rms(ref["forces"], plain["forces"]) > 1e-3
+    h = Q.from_workload(w)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    try:
+        out = h.compute_atom_virial(pos, types, w.box)
+    except Q.QnepError as err:
+        if err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
+            raise
+        out = h.compute_atom_virial(pos, types, w.box)
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    assert_parity(w, res, ref, f"ZBL, {case}")
+    assert rel_rms(res["virial_atom"], ref["virial_atom"]) <= 1e-4
+    _, full = gpu_eval(torch, w, handle=h, want=Q.WANT_ALL | Q.WANT_BEC)
+    assert_parity(w, full, ref, f"ZBL, plain call, {case}")
+    assert rel_rms(full["bec"], ref["bec"]) <= 1e-4
+    parts = h.debug_copy(Q.DBG_ENERGY_PARTS, (4,)).cpu().numpy()
+    assert abs(parts[0] - (ref["energy_parts"]["nep"] + ref["energy_parts"]["zbl"])) <= TOL_E_PER_ATOM * w.n_atoms
+    h.set_zbl(None)
+    _, off = gpu_eval(torch, w, handle=h)
+    assert_parity(w, off, plain, f"ZBL off again, {case}")
+    with pytest.raises(Q.QnepError) as exc:
+        h.set_zbl((1.0, w.model.rc_a + 0.5, w.zbl[2]))
+    assert exc.value.code == Q.QNEP_ERR_UNSUPPORTED
+    with pytest.raises(Q.QnepError) as exc:
+        h.set_zbl((2.0, 1.0, w.zbl[2]))
+    assert exc.value.code == Q.QNEP_ERR_INVALID_ARG
+
+
 # ---------------------------------------------------------------- neighbour policy, errors
 def test_skin_and_rebuild_identity(torch, oracle):
     """Lists built with a skin and reused after the atoms moved give the same result as a fresh build."""
