@@ -66,17 +66,18 @@ def whole_job_value(n_atoms, steps, world, ms_total):
 
 # ncu counters per launch on config 4 in the launch configuration timed here (all outputs), from the ncu --set full capture
 # summarised in profiles/r02_ncu_full.txt: DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) and EXECUTED FP32
-# flops (smsp__sass_thread_inst_executed_op_{fadd,fmul,ffma}_pred_on, FMA = 2).  Reported only for that workload; the
+# flops (predicated-on thread executions per SASS opcode from the source page: FFMA 2, packed FFMA2 4, FMUL / FADD / MUFU 1,
+# FMUL2 / FADD2 2; the op_ffma counter does not see the packed instructions).  Reported only for that workload; the
 # algorithmic work model above them is what the contract's `frac` uses, the executed figure is the north_star's evidence.
 NCU_COUNTERS_CONFIG4 = {
-    "k_pairs": {"dram_bytes": 1.68e9, "executed_flops": 5.695e9},
-    "k_desc_angular": {"dram_bytes": 0.975e9, "executed_flops": 9.423e9},
-    "k_nn": {"dram_bytes": 0.283e9, "executed_flops": 1.353e10},
-    "k_force_angular": {"dram_bytes": 1.43e9, "executed_flops": 2.552e10},
-    "k_force_radial": {"dram_bytes": 0.652e9, "executed_flops": 9.453e9},
+    "k_pairs": {"dram_bytes": 1.596e9, "executed_flops": 7.975e9},
+    "k_desc_angular": {"dram_bytes": 1.033e9, "executed_flops": 1.151e10},
+    "k_nn": {"dram_bytes": 0.283e9, "executed_flops": 1.392e10},
+    "k_force_angular": {"dram_bytes": 1.449e9, "executed_flops": 2.577e10},
+    "k_force_radial": {"dram_bytes": 0.676e9, "executed_flops": 1.349e10},
 }
 NCU_COUNTERS_SOURCE = "profiles/r02_ncu_full.txt"
-NCU_PPPM_DRAM_BYTES_CONFIG4 = 1.92e9        # spread + five FFT kernels + gather, same capture
+NCU_PPPM_DRAM_BYTES_CONFIG4 = 1.921e9       # spread + five FFT kernels + gather, same capture
 
 
 def load_peaks():
@@ -201,6 +202,8 @@ def main():
     ap.add_argument("--cpu-sample-side", type=int, default=70, help="molecules per side of the oracle's sample (70 = full config 4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--zbl", type=float, nargs=2, default=None, metavar=("R_INNER", "R_OUTER"),
+                    help="switch the ZBL core on (water: Z = 8, 1); off by default: BASELINE.json's config has none")
     ap.add_argument("--pppm-kernels", type=int, default=0, help="qnep_set_pppm_kernels: 0 automatic, 1 per-atom spread, 2 sweep spread")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -222,6 +225,9 @@ def main():
     K, Wm = max(args.steps, 1), max(args.warmup, 3)
 
     w = make_workload(args.config, args)
+    if args.zbl:
+        assert w.model.n_types == 2, "--zbl names the atomic numbers of the water-like configs only"
+        w.zbl = (args.zbl[0], args.zbl[1], (8.0, 1.0))
     n = w.n_atoms
     h = Q.from_workload(w)
     h.set_neighbor_policy(args.skin, args.rebuild_every)
@@ -440,7 +446,7 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "n_atoms": n, "species": w.model.n_types, "pppm_grid": list(w.es.grid),
                        "mode": w.model.mode, "n_neurons": w.model.n_neurons, "md": "velocity-Verlet via qnep_md_run" + (", steps replayed as CUDA graphs (stage times from plain launches)" if md_graphs else ""),
-                       "dt_fs": dt_fs, "skin_A": args.skin, "rebuild_every": args.rebuild_every,
+                       "dt_fs": dt_fs, "zbl": list(w.zbl[:2]) if w.zbl else None, "skin_A": args.skin, "rebuild_every": args.rebuild_every,
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2_policy": "inputs larger than L2 (neighbour lists + meshes >> 126 MB); no flush needed",
                        "mean_skin_list": stats["mean_list"], "mean_neighbours_radial": stats["mean_radial"],
