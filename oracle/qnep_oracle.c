@@ -764,11 +764,12 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
         U[1] = Uk;
         for (int a = 0; a < 9; ++a) W[a] += Wk[a];
     } else if (es->method == 2) {
-        /* PPPM: Eq. 34-38, orthorhombic cell, order 5 */
+        /* PPPM: Eq. 34-38, order 5, any cell (:104 "k from the reciprocal basis vectors"): the mesh lives in fractional
+         * coordinates, mesh point s = (s_0 a + s_1 b + s_2 c) / N, and k = 2 pi (n_0 b*_0 + n_1 b*_1 + n_2 b*_2) */
         if (es->order != 5) return -3;
-        if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) return -3;
         int N[3] = {es->grid[0], es->grid[1], es->grid[2]};
-        double L[3] = {box[0], box[4], box[8]};
+        double inv[9];
+        inv3(box, inv);          /* fractional coordinate f_b = sum_a r_a inv[3 a + b];  k_a = 2 pi sum_b n_b inv[3 a + b] */
         int64_t ng = (int64_t)N[0] * N[1] * N[2];
         double *rho = (double *)calloc(2 * ng, sizeof(double));   /* complex */
         double *fld = (double *)malloc(sizeof(double) * 2 * ng);
@@ -780,7 +781,7 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
             int i0[3];
             double wt[3][5];
             for (int a = 0; a < 3; ++a) {
-                double u = w[a * n + i] / L[a] * N[a];
+                double u = (w[i] * inv[a] + w[n + i] * inv[3 + a] + w[2 * n + i] * inv[6 + a]) * N[a];
                 i0[a] = (int)floor(u + 0.5);
                 orc_bspline5(u - i0[a], wt[a]);
             }
@@ -804,11 +805,11 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                 for (int64_t m2 = 0; m2 < N[2]; ++m2) {
                     int64_t s = (m0 * N[1] + m1) * N[2] + m2;
                     int64_t mm[3] = {m0, m1, m2};
-                    double k[3], num = 1.0, den = 1.0;
-                    for (int a = 0; a < 3; ++a) {
-                        int64_t na = mm[a] < N[a] / 2 ? mm[a] : mm[a] - N[a];   /* -N/2 <= n < N/2 (:285) */
-                        k[a] = 2.0 * ORC_PI * na / L[a];
-                        double x = ORC_PI * na / N[a];
+                    double k[3] = {0.0, 0.0, 0.0}, num = 1.0, den = 1.0;
+                    for (int b = 0; b < 3; ++b) {
+                        int64_t nb = mm[b] < N[b] / 2 ? mm[b] : mm[b] - N[b];   /* -N/2 <= n < N/2 (:285) */
+                        for (int a = 0; a < 3; ++a) k[a] += 2.0 * ORC_PI * nb * inv[3 * a + b];
+                        double x = ORC_PI * nb / N[b];
                         num *= pow(sinc(x), 5);
                         den *= orc_alias_denominator(sin(x));
                     }
@@ -835,9 +836,13 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                         if (comp == 0) { fld[2 * s] = re; fld[2 * s + 1] = im; }
                         else {
                             int a = comp - 1;
-                            int64_t ma = a == 0 ? m0 : (a == 1 ? m1 : m2);
-                            int64_t na = ma < N[a] / 2 ? ma : ma - N[a];
-                            double ka = (2 * na == -(int64_t)N[a]) ? 0.0 : 2.0 * ORC_PI * na / L[a]; /* S11 */
+                            int64_t mm[3] = {m0, m1, m2};
+                            double ka = 0.0;
+                            for (int b = 0; b < 3; ++b) {
+                                int64_t nb = mm[b] < N[b] / 2 ? mm[b] : mm[b] - N[b];
+                                if (2 * nb == -(int64_t)N[b]) nb = 0;          /* S11: the Nyquist index carries no gradient */
+                                ka += 2.0 * ORC_PI * nb * inv[3 * a + b];
+                            }
                             fld[2 * s] = -ka * im;      /* i k (re + i im) */
                             fld[2 * s + 1] = ka * re;
                         }
@@ -850,7 +855,7 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
             int i0[3];
             double wt[3][5];
             for (int a = 0; a < 3; ++a) {
-                double u = w[a * n + i] / L[a] * N[a];
+                double u = (w[i] * inv[a] + w[n + i] * inv[3 + a] + w[2 * n + i] * inv[6 + a]) * N[a];
                 i0[a] = (int)floor(u + 0.5);
                 orc_bspline5(u - i0[a], wt[a]);
             }
@@ -878,10 +883,10 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                         for (int64_t m2 = 0; m2 < N[2]; ++m2) {
                             int64_t s = (m0 * N[1] + m1) * N[2] + m2;
                             int64_t mm[3] = {m0, m1, m2};
-                            double k[3];
+                            double k[3] = {0.0, 0.0, 0.0};
                             for (int c = 0; c < 3; ++c) {
                                 int64_t nc = mm[c] < N[c] / 2 ? mm[c] : mm[c] - N[c];
-                                k[c] = 2.0 * ORC_PI * nc / L[c];
+                                for (int d = 0; d < 3; ++d) k[d] += 2.0 * ORC_PI * nc * inv[3 * d + c];
                             }
                             double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
                             double Bab = 0.0;
@@ -894,7 +899,7 @@ static int electrostatics(int64_t n, const double *w, const double *q, const dou
                     int i0[3];
                     double wt[3][5];
                     for (int c = 0; c < 3; ++c) {
-                        double u = w[c * n + i] / L[c] * N[c];
+                        double u = (w[i] * inv[c] + w[n + i] * inv[3 + c] + w[2 * n + i] * inv[6 + c]) * N[c];
                         i0[c] = (int)floor(u + 0.5);
                         orc_bspline5(u - i0[c], wt[c]);
                     }

@@ -317,6 +317,16 @@ def config4(mode: int = 2, n_side: int = 70, grid: int = 256) -> Workload:
                           key="config4")
 
 
+def triclinic_variant(w: Workload, tilt=((0.0, 0.0, 0.0), (0.18, 0.0, 0.0), (0.07, -0.12, 0.0))) -> Workload:
+    """The same fractional coordinates in a tilted cell: row b gets tilt[b][a] * L_a added along a (lower-triangular
+    tilts keep the cell volume).  Stands in for the non-orthogonal cells of PAPER.md :104."""
+    from dataclasses import replace
+    h = w.box.reshape(3, 3)
+    hp = h + np.asarray(tilt, dtype=np.float64) @ np.diag(np.diag(h))
+    frac = np.linalg.solve(h.T, w.pos)
+    return replace(w, pos=np.ascontiguousarray(hp.T @ frac), box=hp.ravel().copy(), name=w.name + "_triclinic")
+
+
 def maxwell_boltzmann(w: Workload, temperature: float = 300.0, seed: int | None = None) -> np.ndarray:
     """Velocities [3][N] in A / (natural time unit), natural unit = A*sqrt(amu/eV)."""
     kB = 8.617333262e-5  # eV/K

@@ -841,3 +841,80 @@ def test_zbl_forces_and_virial_in_the_full_model(oracle):
     # the switch-off state leaks nowhere: a later call without zbl is the plain model again
     again = oracle.compute_workload(w, use_bins=False)
     assert abs(again["energy"] - base["energy"]) < 1e-12 and again["energy_parts"]["zbl"] == 0.0
+
+
+# --------------------------------------------------- triclinic cells (PAPER.md :104)
+def test_sheared_description_of_the_same_crystal(oracle):
+    """A periodic crystal does not know which cell vectors describe it: the cubic box (a, b, c) and the sheared box
+    (a + b, b, c + a) span the same lattice, so the whole model (neighbours over images, descriptors, network, Ewald with the
+    |k| <= 2 pi alpha sphere of the paper, forces, virial, charges) must give the same numbers -- on a triclinic cell."""
+    w = I.config0(mode=1)
+    w.es = replace(w.es, alpha=0.6, ewald_nmax2=0)          # physical k sphere (:110): the same k set in both descriptions
+    a = oracle.compute_workload(w, use_bins=False, want_bec=True, want_atom_virial=True)
+    h = w.box.reshape(3, 3)
+    sheared = np.array([h[0] + h[1], h[1], h[2] + h[0]])
+    assert abs(np.linalg.det(sheared) - np.linalg.det(h)) < 1e-9
+    for use_bins in (False, True):
+        b = oracle.compute(w.model, w.params, w.es, w.pos, w.types, sheared.ravel(), use_bins=use_bins, want_bec=True,
+                           want_atom_virial=True)
+        assert abs(a["energy"] - b["energy"]) < 1e-9
+        assert np.abs(a["forces"] - b["forces"]).max() < 1e-9
+        assert np.abs(a["virial"] - b["virial"]).max() < 1e-8
+        assert np.abs(a["charges"] - b["charges"]).max() < 1e-12
+        assert np.abs(a["bec"] - b["bec"]).max() < 1e-9
+        assert np.abs(a["virial_atom"] - b["virial_atom"]).max() < 1e-8
+
+
+_triclinic = I.triclinic_variant
+
+
+def test_triclinic_forces_and_virial_are_energy_derivatives(oracle):
+    """Eq. 11-23 on a genuinely triclinic cell (Ewald): F = -dE/dr, W = -dE/d(strain), sum F = 0, W symmetric."""
+    w = _triclinic(_small_workload(2, 0.3))
+    hbox = w.box.reshape(3, 3)
+    assert abs(hbox[1, 0]) > 1.0 and abs(hbox[2, 1]) > 1.0
+    out = oracle.compute_workload(w, use_bins=False)
+    h = 1e-5
+    for (a, i) in ((0, 5), (1, 33), (2, 60)):
+        p1, p2 = w.pos.copy(), w.pos.copy()
+        p1[a, i] += h
+        p2[a, i] -= h
+        e1 = oracle.compute(w.model, w.params, w.es, p1, w.types, w.box, use_bins=False)["energy"]
+        e2 = oracle.compute(w.model, w.params, w.es, p2, w.types, w.box, use_bins=False)["energy"]
+        fd = -(e1 - e2) / (2 * h)
+        assert abs(fd - out["forces"][a, i]) < 2e-7 * max(1.0, abs(fd)), (fd, out["forces"][a, i])
+    for (a, b) in ((0, 0), (1, 1), (0, 2), (2, 1)):
+        eps = np.zeros((3, 3))
+        eps[a, b] = h
+        def energy(sign):
+            Fm = np.eye(3) + sign * eps
+            return oracle.compute(w.model, w.params, w.es, Fm @ w.pos, w.types,
+                                  (w.box.reshape(3, 3) @ Fm.T).ravel(), use_bins=False)["energy"]
+        fd = -(energy(1) - energy(-1)) / (2 * h)
+        assert abs(fd - out["virial"][a, b]) < 1e-6 * np.abs(out["virial"]).max(), (fd, out["virial"][a, b])
+    assert np.abs(out["forces"].sum(axis=1)).max() < 1e-10
+    assert np.allclose(out["virial"], out["virial"].T, atol=1e-9 * np.abs(out["virial"]).max())
+
+
+def test_triclinic_pppm_converges_to_ewald(oracle):
+    """Eq. 34-39 with the mesh in fractional coordinates and k from the reciprocal basis vectors (:104): on a triclinic cell the
+    PPPM energy, potential, forces, virial and per-atom virial converge to the Ewald sum as the mesh is refined."""
+    L = 16.0
+    pos, q = _random_charges(120, L, 9)
+    h = np.array([[L, 0.0, 0.0], [0.2 * L, L, 0.0], [0.1 * L, -0.15 * L, 0.9 * L]])
+    frac = pos / L
+    pos = h.T @ frac
+    box = h.ravel()
+    ew = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=1, alpha=0.3, ewald_nmax2=225), want_atom_virial=True)
+    errs = []
+    for g in (16, 32, 64):
+        pm = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=2, alpha=0.3, grid=(g, g, g)), want_atom_virial=(g == 64))
+        errs.append((rel_rms(pm["F"], ew["F"]), abs(pm["U"][1] - ew["U"][1]) / abs(ew["U"][1]),
+                     rel_rms(pm["phi"], ew["phi"]), np.abs(pm["W"] - ew["W"]).max() / np.abs(ew["W"]).max()))
+    assert errs[0][0] < 2e-3 and errs[1][0] < 2e-5 and errs[2][0] < 2e-7, errs
+    assert errs[0][0] > 10 * errs[1][0] > 100 * errs[2][0]
+    assert errs[2][1] < 1e-7 and errs[2][2] < 1e-6 and errs[2][3] < 1e-6, errs
+    assert rel_rms(pm["W_atom"], ew["W_atom"]) < 1e-5
+    # anisotropic mesh on the same cell
+    pm2 = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=2, alpha=0.3, grid=(64, 32, 32)))
+    assert rel_rms(pm2["F"], ew["F"]) < 3e-5
