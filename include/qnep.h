@@ -35,7 +35,7 @@ typedef struct qnep_handle qnep_handle; /* opaque */
 enum {
     QNEP_OK = 0,
     QNEP_ERR_INVALID_ARG = -1,
-    QNEP_ERR_UNSUPPORTED = -2,       /* triclinic box, order != 5, non-power-of-2 grid, > 4 species, box < r_c + skin */
+    QNEP_ERR_UNSUPPORTED = -2,       /* order != 5, non-power-of-2 grid, > 4 species, cell narrower than r_c + skin      */
     QNEP_ERR_NEIGHBOR_OVERFLOW = -3, /* a neighbour list exceeded its capacity; capacity has been grown, call again */
     QNEP_ERR_SKIN_VIOLATED = -4,     /* an atom moved more than skin/2 since the last neighbour build */
     QNEP_ERR_CUDA = -5,
@@ -134,7 +134,9 @@ int qnep_set_neighbor_capacity(qnep_handle *h, int32_t cap_radial, int32_t cap_a
  * qnep_compute: one force evaluation, enqueued on `cuda_stream`.
  *   pos_dev     [3][N] float64, component-major, Angstrom, any periodic image (wrapped inside)
  *   types_dev   [N] int32, 0..n_types-1
- *   box         [9] float64 HOST, rows = cell vectors a, b, c; orthorhombic only in this version
+ *   box         [9] float64 HOST, rows = cell vectors a, b, c: any non-degenerate cell (PAPER.md :104; INVALID_ARG for zero
+ *               volume); its perpendicular width along every cell vector must be >= r_c + skin (UNSUPPORTED otherwise);
+ *               a PPPM mesh lives in the fractional coordinates of the cell
  *   want        QNEP_WANT_* flags; an output whose flag is clear may be NULL
  *   energy_dev  [1]    eV,   U^tot = U^NEP + U^ES (Eq. 4)
  *   forces_dev  [3][N] eV/A  (Eq. 11 + static electrostatic forces Eq. 15, 18 / 37)

@@ -47,21 +47,29 @@ int validate_es(qnep_handle* h, const qnep_es_desc* es)
     return QNEP_OK;
 }
 
-// geometry for a box; returns UNSUPPORTED for triclinic / too small boxes
+// geometry for a box (rows = cell vectors, any non-degenerate cell); returns UNSUPPORTED for boxes narrower than r_c + skin
 int make_geometry(qnep_handle* h, const double box[9], Geometry* g)
 {
-    if (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) {
-        h->err = "only orthorhombic boxes are supported in this version";
-        return QNEP_ERR_UNSUPPORTED;
-    }
     const double rcs = h->model.rc_r + h->skin;
+    const double* B = box;
+    const double det = B[0] * (B[4] * B[8] - B[5] * B[7]) - B[1] * (B[3] * B[8] - B[5] * B[6]) + B[2] * (B[3] * B[7] - B[4] * B[6]);
+    if (!(std::fabs(det) > 1e-12)) { h->err = "degenerate box (zero volume)"; return QNEP_ERR_INVALID_ARG; }
+    // inverse (adjugate / det): hinv[3a + b] = (h^-1)_{ab}
+    g->hinv[0] = (B[4] * B[8] - B[5] * B[7]) / det; g->hinv[1] = (B[2] * B[7] - B[1] * B[8]) / det; g->hinv[2] = (B[1] * B[5] - B[2] * B[4]) / det;
+    g->hinv[3] = (B[5] * B[6] - B[3] * B[8]) / det; g->hinv[4] = (B[0] * B[8] - B[2] * B[6]) / det; g->hinv[5] = (B[2] * B[3] - B[0] * B[5]) / det;
+    g->hinv[6] = (B[3] * B[7] - B[4] * B[6]) / det; g->hinv[7] = (B[1] * B[6] - B[0] * B[7]) / det; g->hinv[8] = (B[0] * B[4] - B[1] * B[3]) / det;
+    g->triclinic = (box[1] != 0 || box[2] != 0 || box[3] != 0 || box[5] != 0 || box[6] != 0 || box[7] != 0) ? 1 : 0;
     g->ncells = 1;
     for (int a = 0; a < 3; ++a) {
-        g->L[a] = box[4 * a];
+        for (int c = 0; c < 3; ++c) g->h[3 * a + c] = box[3 * a + c];
+        g->L[a] = std::sqrt(box[3 * a] * box[3 * a] + box[3 * a + 1] * box[3 * a + 1] + box[3 * a + 2] * box[3 * a + 2]);
         if (!(g->L[a] > 0)) { h->err = "box edge must be positive"; return QNEP_ERR_INVALID_ARG; }
-        if (g->L[a] < rcs) { h->err = "box edge smaller than r_c + skin"; return QNEP_ERR_UNSUPPORTED; }
-        g->ncell[a] = std::min(1023, std::max(1, (int)floor(g->L[a] / rcs)));
+        // perpendicular width of the cell along a: 1 / |reciprocal vector a| (= L_a for an orthorhombic box)
+        const double width = 1.0 / std::sqrt(g->hinv[a] * g->hinv[a] + g->hinv[3 + a] * g->hinv[3 + a] + g->hinv[6 + a] * g->hinv[6 + a]);
+        if (width < rcs) { h->err = "box narrower than r_c + skin"; return QNEP_ERR_UNSUPPORTED; }
+        g->ncell[a] = std::min(1023, std::max(1, (int)floor(width / rcs)));
         g->hcell[a] = g->L[a] / g->ncell[a];
+        for (int c = 0; c < 3; ++c) g->cellv[3 * a + c] = (float)(box[3 * a + c] / g->ncell[a]);
         g->ncells *= g->ncell[a];
         g->grid[a] = h->es.method == 2 ? h->es.grid[a] : 0;
         g->hmesh_inv[a] = g->grid[a] > 0 ? g->grid[a] / g->L[a] : 0.0;
@@ -80,7 +88,8 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
     int rc = make_geometry(h, box, &g);
     if (rc) return rc;
     const bool box_changed = std::memcmp(box, h->box, sizeof(double) * 9) != 0;
-    const double vol = g.L[0] * g.L[1] * g.L[2];
+    const double vol = std::fabs(g.h[0] * (g.h[4] * g.h[8] - g.h[5] * g.h[7]) - g.h[1] * (g.h[3] * g.h[8] - g.h[5] * g.h[6]) +
+                                 g.h[2] * (g.h[3] * g.h[7] - g.h[4] * g.h[6]));
     const double rho = (double)N / vol;
     auto cap_for = [&](double rc_, int user, int grown) {
         if (user > 0) return (user + 3) / 4 * 4;          // packed-word lists hold four slots per int4

@@ -227,7 +227,7 @@ __device__ __forceinline__ void stg_tiled_row(float4* base, int row, float x, fl
 __device__ __forceinline__ int lds_b32(unsigned addr) { int v; asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v; }
 __device__ __forceinline__ float lds_f32(unsigned addr) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory"); return v; }
 
-template <int T>
+template <int T, bool TRI>
 __global__ void __launch_bounds__(PAIRS_BLOCK)
 k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __restrict__ nl,
         const int* __restrict__ nn, const int* __restrict__ nlRend, const float* __restrict__ cR, float rcinv, int capR, int capLR, int capLA,
@@ -242,7 +242,7 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
     constexpr int QROW = PAIRS_BLOCK * 4, QR2 = PAIRS_QCAP * QROW, QMASK = QR2 - 1;   // bytes per slot, offset of the r^2 half, ring wrap
     for (int i = threadIdx.x; i < T * T * NR * KP; i += blockDim.x) sh_c[i] = cR[i];
     __syncthreads();
-    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
+    const CellVecs cv = qnep_cell_vecs(g.cellv, TRI ? 1 : 0);      // compile-time switch: the orthorhombic walk pays nothing for the general cell
     const int tid = threadIdx.x;
     const int64_t p0 = blockIdx.x * (int64_t)blockDim.x + tid;
     const bool live = p0 < N;                                // threads beyond N stay for the warp votes, with an empty list
@@ -320,7 +320,7 @@ k_pairs(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* __re
                 const int e = word_of(lv[v & 3], u);
                 const float4 xj = xjv[u];
                 float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
-                qnep_add_image_shift(e, h0, h1, h2, dx, dy, dz);
+                qnep_add_image_shift(e, cv, dx, dy, dz);
                 const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
                 if (act && r2 < g.rc_r2 && r2 >= 1e-12f) {
                     sts_pair(qbase + qoff, e, r2, QR2);
@@ -978,7 +978,7 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
 {
     __shared__ int4 sh_w[RAD_LV][RAD_BLOCK];
     __shared__ double sh_red[32];
-    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
+    const CellVecs cv = qnep_cell_vecs(g.cellv, g.triclinic);
     const int tid = threadIdx.x;
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + tid;
     float W[9];
@@ -1045,7 +1045,7 @@ k_force_radial(int64_t N, Geometry g, const float* __restrict__ recA, const floa
                         Pi[5] = o4.x; Pi[6] = o4.y; Pi[7] = o4.z; Pi[8] = o4.w;
                     }
                     float dx = a8[0] - xi.x, dy = a8[1] - xi.y, dz = a8[2] - xi.z;
-                    qnep_add_image_shift(e, h0, h1, h2, dx, dy, dz);
+                    qnep_add_image_shift(e, cv, dx, dy, dz);
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     const float rinv = fast_rsqrt(r2), r = r2 * rinv;
                     ChebDeriv cd;
@@ -1171,8 +1171,13 @@ int qnep_launch_pairs(qnep_handle* h, cudaStream_t s)
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
         static bool attr_set = false;                        // one flag per instantiation (the lambda is generic)
-        if (!attr_set) { cudaFuncSetAttribute(k_pairs<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PAIRS_SMEM); attr_set = true; }
-        k_pairs<T><<<nb, PAIRS_BLOCK, PAIRS_SMEM, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlRend, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
+        if (!attr_set) {
+            cudaFuncSetAttribute(k_pairs<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PAIRS_SMEM);
+            cudaFuncSetAttribute(k_pairs<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PAIRS_SMEM);
+            attr_set = true;
+        }
+        auto kern = h->geo.triclinic ? k_pairs<T, true> : k_pairs<T, false>;
+        kern<<<nb, PAIRS_BLOCK, PAIRS_SMEM, s>>>(N, h->geo, h->d_xyzt, h->d_nlR, h->d_nnR, h->d_nlRend, h->d_cR, rcinv, h->capR, h->capLR, h->capLA,
                                               h->d_lvR, h->d_nlvR, h->d_lvRend, h->d_lvA, h->d_nlvA, h->d_D, h->d_flags);
     });
     h->launches += 1;

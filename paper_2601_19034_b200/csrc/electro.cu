@@ -37,7 +37,7 @@ k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* 
             float* __restrict__ Fs, double* __restrict__ sums, float* __restrict__ Wat /* [9][N] or null */)
 {
     __shared__ double sh_red[32];
-    const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
+    const CellVecs cv = qnep_cell_vecs(g.cellv, g.triclinic);
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     const float Kc = (float)QNEP_K_COULOMB;
     const float two_a_sqrtpi = 2.f * alpha * 0.5641895835477563f;
@@ -54,7 +54,7 @@ k_realspace(int64_t N, Geometry g, const float4* __restrict__ xyzt, const int4* 
             const int j = e & QNEP_NL_MASK;
             const float4 xj = xyzt[j];
             float dx = xj.x - xi.x, dy = xj.y - xi.y, dz = xj.z - xi.z;
-            qnep_add_image_shift(e, h0, h1, h2, dx, dy, dz);
+            qnep_add_image_shift(e, cv, dx, dy, dz);
             const float r2 = dx * dx + dy * dy + dz * dz;
             if (r2 >= g.rc_r2) continue;
             const float r = sqrtf(r2), rinv = 1.f / r;
@@ -126,9 +126,10 @@ __global__ void k_ewald_phases(int64_t N, const double* __restrict__ pos, const 
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= N) return;
     const int i = sidx[p];
+    const double r[3] = {pos[i], pos[N + i], pos[2 * N + i]};
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        double f = pos[a * N + i] / g.L[a];
+        double f = r[0] * g.hinv[a] + r[1] * g.hinv[3 + a] + r[2] * g.hinv[6 + a];
         f -= floor(f);
         for (int n = 0; n <= nmax; ++n) {
             double t = 2.0 * n * f;
@@ -281,8 +282,10 @@ int qnep_launch_phi_finalize(qnep_handle* h, cudaStream_t s)
 // given, else |k| <= 2 pi alpha; G(k) of Eq. 9 in double, stored as float.
 int qnep_setup_ewald(qnep_handle* h)
 {
-    const double L[3] = {h->box[0], h->box[4], h->box[8]};
-    const double vol = L[0] * L[1] * L[2];
+    const Geometry& g = h->geo;                          // any cell: k = 2 pi (n0 b*_0 + n1 b*_1 + n2 b*_2), b*_b = column b of h^-1 (:104)
+    const double L[3] = {g.L[0], g.L[1], g.L[2]};        // lengths of the cell vectors (bound of the integer range, as in the oracle)
+    const double vol = std::fabs(g.h[0] * (g.h[4] * g.h[8] - g.h[5] * g.h[7]) - g.h[1] * (g.h[3] * g.h[8] - g.h[5] * g.h[6]) +
+                                 g.h[2] * (g.h[3] * g.h[7] - g.h[4] * g.h[6]));
     const double alpha = h->alpha;
     const double kmax = 2.0 * M_PI * alpha;
     int nmax[3];
@@ -297,7 +300,8 @@ int qnep_setup_ewald(qnep_handle* h)
             for (int n2 = -nmax[2]; n2 <= nmax[2]; ++n2) {
                 const bool half = n0 > 0 || (n0 == 0 && (n1 > 0 || (n1 == 0 && n2 > 0)));
                 if (!half) continue;
-                const double k[3] = {2.0 * M_PI * n0 / L[0], 2.0 * M_PI * n1 / L[1], 2.0 * M_PI * n2 / L[2]};
+                double k[3];
+                for (int a = 0; a < 3; ++a) k[a] = 2.0 * M_PI * (n0 * g.hinv[3 * a] + n1 * g.hinv[3 * a + 1] + n2 * g.hinv[3 * a + 2]);
                 const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
                 if (h->es.ewald_nmax2 > 0) { if (n0 * n0 + n1 * n1 + n2 * n2 > h->es.ewald_nmax2) continue; }
                 else if (k2 > kmax * kmax * (1.0 + 1e-12)) continue;

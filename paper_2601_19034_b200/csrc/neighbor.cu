@@ -18,19 +18,32 @@ namespace {
 
 __device__ __forceinline__ int pack3(int a, int b, int c) { return a | (b << 10) | (c << 20); }
 
-// offset of an atom from its cell origin: the periodic image nearest to `ref` (0 at build time: nearest to the origin;
-// the build-time offset on list-reuse steps)
-__device__ __forceinline__ double cell_offset(double x, double origin, double L, double ref)
+// Position of an atom relative to the origin of search cell c, for any cell (rows of g.h): with the fractional
+// coordinate f = r h^-1 and the cell origin c_a / ncell_a,  s_a = f_a - c_a / ncell_a  is wrapped to the periodic image
+// nearest to ref_a (0 at build time: nearest to the cell origin; the build-time value on list-reuse steps), and the
+// Cartesian offset is d = s h.  fr[a] = c_a / ncell_a + s_a is the (unwrapped) fractional coordinate the PPPM mesh uses.
+__device__ __forceinline__ void cell_relative(const Geometry& g, const double r[3], const int c[3], const double ref[3],
+                                              double d[3], double fr[3])
 {
-    double d = x - origin;
-    d -= L * rint((d - ref) / L);
-    return d;
+    double sfr[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double f = r[0] * g.hinv[a] + r[1] * g.hinv[3 + a] + r[2] * g.hinv[6 + a];
+        const double org = (double)c[a] / (double)g.ncell[a];
+        double sa = f - org;
+        sa -= rint(sa - ref[a]);
+        sfr[a] = sa;
+        fr[a] = org + sa;
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) d[k] = sfr[0] * g.h[k] + sfr[1] * g.h[3 + k] + sfr[2] * g.h[6 + k];
 }
 
-// PPPM mesh coordinate of x (reading S10): nearest mesh point i0 (wrapped into 0..n-1) and the fractional offset
-__device__ __forceinline__ void mesh_coord(double x, double hinv, int n, float* frac, int* i0)
+// PPPM mesh coordinate (reading S10) of fractional coordinate f on an axis of n points: nearest mesh point i0 (wrapped
+// into 0..n-1) and the offset from it in mesh units
+__device__ __forceinline__ void mesh_coord(double f, int n, float* frac, int* i0)
 {
-    const double u = x * hinv;
+    const double u = f * n;
     const double r = floor(u + 0.5);
     *frac = (float)(u - r);
     const int ir = (int)r % n;
@@ -44,9 +57,10 @@ __global__ void k_bin_count(int64_t N, int T, const double* __restrict__ pos, co
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= N) return;
     int c[3];
+    const double r[3] = {pos[i], pos[N + i], pos[2 * N + i]};
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        double f = pos[a * N + i] / g.L[a];
+        double f = r[0] * g.hinv[a] + r[1] * g.hinv[3 + a] + r[2] * g.hinv[6 + a];
         f -= floor(f);
         int ci = (int)(f * g.ncell[a]);
         c[a] = min(max(ci, 0), g.ncell[a] - 1);
@@ -163,12 +177,12 @@ __global__ void k_mbin_key(int64_t N, const double* __restrict__ pos, const int*
     const int cell = k % g.ncells;
     const int c[3] = {cell / (g.ncell[2] * g.ncell[1]), (cell / g.ncell[2]) % g.ncell[1], cell % g.ncell[2]};
     int m0[3];
+    {
+        const double r[3] = {pos[i], pos[N + i], pos[2 * N + i]}, ref[3] = {0.0, 0.0, 0.0};
+        double d[3], ff[3];
+        cell_relative(g, r, c, ref, d, ff);                                      // exactly what k_prep does at build time
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double origin = c[a] * g.hcell[a];
-        const double d = cell_offset(pos[a * N + i], origin, g.L[a], 0.0);       // exactly what k_prep does at build time
-        float fr;
-        mesh_coord(origin + d, g.hmesh_inv[a], g.grid[a], &fr, &m0[a]);
+        for (int a = 0; a < 3; ++a) { float fr; mesh_coord(ff[a], g.grid[a], &fr, &m0[a]); }
     }
     const int kb = ((m0[1] / QNEP_MB_Y) * nbz + m0[2] / QNEP_MB_Z) * nbx + m0[0] / QNEP_MB_X;
     mbkey[p] = kb;
@@ -211,14 +225,23 @@ __global__ void k_prep(int64_t N, const double* __restrict__ pos, const int32_t*
     // than three cells along an axis an atom near the +-L/2 plane would otherwise flip by a whole L between two steps
     // (a spurious skin violation, and a wrong r_ij for the list built from the other image).
     float o0[3] = {0.f, 0.f, 0.f};
-    if (!at_build) { const float4 o = off0[p]; o0[0] = o.x; o0[1] = o.y; o0[2] = o.z; }
+    double ref[3] = {0.0, 0.0, 0.0};
+    if (!at_build) {
+        const float4 o = off0[p];
+        o0[0] = o.x; o0[1] = o.y; o0[2] = o.z;
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double origin = c[a] * g.hcell[a];
-        const double d = cell_offset(pos[a * N + i], origin, g.L[a], (double)o0[a]);     // at build time o0 = 0
-        off[a] = (float)d;
-        if (g.grid[a] > 0) mesh_coord(origin + d, g.hmesh_inv[a], g.grid[a], &dx[a], &m0[a]);
-        else { dx[a] = 0.f; m0[a] = 0; }
+        for (int a = 0; a < 3; ++a) ref[a] = (double)o.x * g.hinv[a] + (double)o.y * g.hinv[3 + a] + (double)o.z * g.hinv[6 + a];
+    }
+    {
+        const double r[3] = {pos[i], pos[N + i], pos[2 * N + i]};
+        double d[3], ff[3];
+        cell_relative(g, r, c, ref, d, ff);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            off[a] = (float)d[a];
+            if (g.grid[a] > 0) mesh_coord(ff[a], g.grid[a], &dx[a], &m0[a]);
+            else { dx[a] = 0.f; m0[a] = 0; }
+        }
     }
     float4 v = make_float4(off[0], off[1], off[2], __int_as_float(type));
     xyzt[p] = v;
@@ -255,6 +278,7 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
     int nR = 0, nPad = 0;                // slots written, filler slots among them
     const float rcs2 = g.rcs_r2;
     const float h0 = (float)g.hcell[0], h1 = (float)g.hcell[1], h2 = (float)g.hcell[2];
+    const CellVecs cv = qnep_cell_vecs(g.cellv, g.triclinic);
     // type-major order: all neighbours of species 0 first, then species 1, ...  The per-step lists derived from
     // this one inherit the order, so the radial force kernel switches its own coefficient vector T - 1 times per atom.
     for (int t = 0; t < T; ++t) {
@@ -262,7 +286,7 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
             const int d0 = code / 9 - 1, d1 = (code / 3) % 3 - 1, d2 = code % 3 - 1;
             // the whole cell is out of reach of this atom?  (positions are relative to the atom's own cell, in [0, hcell);
             // with a single cell along an axis the coordinate is the nearest image to the origin instead: no pruning there)
-            {
+            if (!g.triclinic) {     // (the gaps along non-orthogonal axes do not add in quadrature: no pruning there)
                 const float ex = g.ncell[0] < 2 ? 0.f : (d0 < 0 ? xi.x : (d0 > 0 ? h0 - xi.x : 0.f));
                 const float ey = g.ncell[1] < 2 ? 0.f : (d1 < 0 ? xi.y : (d1 > 0 ? h1 - xi.y : 0.f));
                 const float ez = g.ncell[2] < 2 ? 0.f : (d2 < 0 ? xi.z : (d2 > 0 ? h2 - xi.z : 0.f));
@@ -275,7 +299,12 @@ k_build_lists(int64_t N, int T, Geometry g, const float4* __restrict__ xyzt, con
             n2 = n2 < 0 ? n2 + g.ncell[2] : (n2 >= g.ncell[2] ? n2 - g.ncell[2] : n2);
             const int cell = (n0 * g.ncell[1] + n1) * g.ncell[2] + n2;
             // r_ij = x_j - (x_i - shift)
-            const float ox = xi.x - d0 * h0, oy = xi.y - d1 * h1, oz = xi.z - d2 * h2;
+            float ox = xi.x, oy = xi.y, oz = xi.z;
+            {
+                float sx = 0.f, sy = 0.f, sz = 0.f;
+                qnep_add_image_shift(qnep_image_bits(d0, d1, d2), cv, sx, sy, sz);
+                ox -= sx; oy -= sy; oz -= sz;
+            }
             const int k = t * g.ncells + cell;
             const int b = start[k], e = start[k + 1];
             const int self = (code == 13 && t == ti) ? (int)p : -1;

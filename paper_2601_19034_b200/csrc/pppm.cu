@@ -244,16 +244,25 @@ k_fft_strided(int axis, int n0, int n1, int n2, float2* __restrict__ mesh_a, flo
         for (int k1 = 0; k1 < R2; ++k1) p[((u + S::TPL * d) + R1 * k1) * ta.stride] = v[d * R2 + k1];
 }
 
+// Non-orthogonal cells (PAPER.md :104, k from the reciprocal basis vectors): b[3a + c] = Cartesian component a of 2 pi b*_c.
+// The tables of a triclinic run hold the INTEGER index n of the axis in kk[] (k = sum_c n_c b_c is formed per mesh point,
+// and exp(-k^2 / 4 alpha^2) with it: neither is separable any more) and A[] without the Gaussian.  The gradient multiplier
+// stays per axis: kd[] = 2 pi n / |cell vector| (Nyquist entry zeroed), i.e. the meshes carry the components of
+// grad Phi along the RECIPROCAL basis vectors, and k_gather turns them into Cartesian components with the constant
+// matrix hinv[3a + c] |h_c| (the identity for an orthorhombic box).  That keeps kd_y, kd_z constants of an x line, which
+// the packing of the four fields into two transforms and the mirror lines of the half spectrum rely on.
+struct KB { float b[9]; };
+
 // ---- 3. fused pass along x: forward FFT, influence function, two inverse FFTs ------------------------
 // tables per axis a (offset a * FFT_MAXN): A[m] = exp(-k^2/4 alpha^2) sinc^10(pi n/N) / d(z)^2, kk[m] = k (true, for
 // k^2), kd[m] = k with the Nyquist entry zeroed (for the i k multiplier, S11).
 //   M1 = Phi + i (i kx Phi) = (1 - kx) Phi ;  M2 = i ky Phi + i (i kz Phi) = (-kz + i ky) Phi
-template <int R1, int R2, bool VIRIAL>
+template <int R1, int R2, bool VIRIAL, bool TRI>
 __global__ void __launch_bounds__(Split<R1, R2>::THREADS)
 k_fft_x_fused(int n0, int n1, int n2, float2* __restrict__ M1 /* in: S after the z and y passes; out: M1 */,
               float2* __restrict__ M2, const float2* __restrict__ twg, const float* __restrict__ tabA,
               const float* __restrict__ tabK, const float* __restrict__ tabKd, float c0 /* 2 pi / Omega */, float inv4a2,
-              double* __restrict__ sums)
+              double* __restrict__ sums, KB kb)
 {
     using S = Split<R1, R2>;
     using SI = Split<R2, R1>;
@@ -285,28 +294,32 @@ k_fft_x_fused(int n0, int n1, int n2, float2* __restrict__ M1 /* in: S after the
     const float kdy = tabKd[FFT_MAXN + iy], kdz = tabKd[2 * FFT_MAXN + iz];
     const float Ayz = c0 * tabA[FFT_MAXN + iy] * tabA[2 * FFT_MAXN + iz];
     const float kyz2 = ky * ky + kz * kz;
+    // TRI: ky, kz are the integer indices n1, n2 and (lx, ly, lz) = n1 b_1 + n2 b_2 is the part of k shared by the line
+    const float lx = TRI ? ky * kb.b[1] + kz * kb.b[2] : 0.f, ly = TRI ? ky * kb.b[4] + kz * kb.b[5] : 0.f, lz = TRI ? ky * kb.b[7] + kz * kb.b[8] : 0.f;
     float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
     for (int d = 0; d < S::D2; ++d)
 #pragma unroll
         for (int k1 = 0; k1 < R2; ++k1) {
             const int ix = (u + S::TPL * d) + R1 * k1;
-            const float kx = tK[ix], kdx = tKd[ix];
-            const float k2 = kx * kx + kyz2;
+            const float kdx = tKd[ix];
+            float kx = tK[ix], kyp = ky, kzp = kz, k2;
+            if (TRI) { const float nx = kx; kx = fmaf(nx, kb.b[0], lx); kyp = fmaf(nx, kb.b[3], ly); kzp = fmaf(nx, kb.b[6], lz); k2 = kx * kx + kyp * kyp + kzp * kzp; }
+            else k2 = kx * kx + kyz2;
             const float2 s = v[d * R2 + k1];
             float G = 0.f;
-            if (k2 > 0.f) G = __fdividef(Ayz * tA[ix], k2);
+            if (k2 > 0.f) G = __fdividef(TRI ? Ayz * tA[ix] * __expf(-k2 * inv4a2) : Ayz * tA[ix], k2);
             const float2 phi = make_float2(G * s.x, G * s.y);
             const float e = G * (s.x * s.x + s.y * s.y);
             acc[0] += e;
             if (VIRIAL && k2 > 0.f) {
                 const float bf = 2.f * inv4a2 + __fdividef(2.f, k2);
                 acc[1] += e * (1.f - bf * kx * kx);
-                acc[2] += e * (-bf * kx * ky);
-                acc[3] += e * (-bf * kx * kz);
-                acc[4] += e * (1.f - bf * ky * ky);
-                acc[5] += e * (-bf * ky * kz);
-                acc[6] += e * (1.f - bf * kz * kz);
+                acc[2] += e * (-bf * kx * kyp);
+                acc[3] += e * (-bf * kx * kzp);
+                acc[4] += e * (1.f - bf * kyp * kyp);
+                acc[5] += e * (-bf * kyp * kzp);
+                acc[6] += e * (1.f - bf * kzp * kzp);
             }
             v[d * R2 + k1] = make_float2((1.f - kdx) * phi.x, (1.f - kdx) * phi.y);
             w[d * R2 + k1] = make_float2(-kdz * phi.x - kdy * phi.y, -kdz * phi.y + kdy * phi.x);
@@ -359,11 +372,11 @@ k_fft_x_fused(int n0, int n1, int n2, float2* __restrict__ M1 /* in: S after the
 //     M1(x; -ky, -kz) = conj IDFT_x[(1 + kd_x) phi],     M2(x; -ky, -kz) = conj IDFT_x[(kd_z + i kd_y) phi],
 // with kd_y, kd_z of the STORED line.  Energy and virial sums weigh these lines twice.  One forward and four inverse
 // line transforms per stored line instead of one and two per line of the full spectrum.
-template <int R1, int R2, bool VIRIAL>
+template <int R1, int R2, bool VIRIAL, bool TRI>
 __global__ void __launch_bounds__(Split<R1, R2>::THREADS, Split<R1, R2>::THREADS >= 256 ? 3 : 1)
 k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2* __restrict__ M1, float2* __restrict__ M2,
                    const float2* __restrict__ twg, const float* __restrict__ tabA, const float* __restrict__ tabK,
-                   const float* __restrict__ tabKd, float c0 /* 2 pi / Omega */, float inv4a2, double* __restrict__ sums)
+                   const float* __restrict__ tabKd, float c0 /* 2 pi / Omega */, float inv4a2, double* __restrict__ sums, KB kb)
 {
     using S = Split<R1, R2>;
     using SI = Split<R2, R1>;
@@ -400,6 +413,8 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
     const float kdy = tabKd[FFT_MAXN + iy], kdz = tabKd[2 * FFT_MAXN + kzc];
     const float Ayz = c0 * tabA[FFT_MAXN + iy] * tabA[2 * FFT_MAXN + kzc];
     const float kyz2 = ky * ky + kzv * kzv;
+    // TRI: ky, kzv are the integer indices n1, n2 and (lx, ly, lz) = n1 b_1 + n2 b_2 is the part of k shared by the line
+    const float lx = TRI ? ky * kb.b[1] + kzv * kb.b[2] : 0.f, ly = TRI ? ky * kb.b[4] + kzv * kb.b[5] : 0.f, lz = TRI ? ky * kb.b[7] + kzv * kb.b[8] : 0.f;
     const float wgt = !valid ? 0.f : (mirrored ? 2.f : 1.f);
     float acc[7] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -407,11 +422,12 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
 #pragma unroll
         for (int k1 = 0; k1 < R2; ++k1) {
             const int ix = (u + S::TPL * d) + R1 * k1;
-            const float kx = tK[ix];
-            const float k2 = kx * kx + kyz2;
+            float kx = tK[ix], kyp = ky, kzp = kzv, k2;
+            if (TRI) { const float nx = kx; kx = fmaf(nx, kb.b[0], lx); kyp = fmaf(nx, kb.b[3], ly); kzp = fmaf(nx, kb.b[6], lz); k2 = kx * kx + kyp * kyp + kzp * kzp; }
+            else k2 = kx * kx + kyz2;
             const float2 sv = v[d * R2 + k1];
             float G = 0.f;
-            if (k2 > 0.f) G = __fdividef(Ayz * tA[ix], k2);
+            if (k2 > 0.f) G = __fdividef(TRI ? Ayz * tA[ix] * __expf(-k2 * inv4a2) : Ayz * tA[ix], k2);
             // phi = G S stays in the registers, kd_x phi is parked in shared memory for the second inverse transform
             const float2 ph = make_float2(G * sv.x, G * sv.y);
             const float kdx = tKd[ix];
@@ -422,11 +438,11 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
             if (VIRIAL && k2 > 0.f) {
                 const float bf = 2.f * inv4a2 + __fdividef(2.f, k2);
                 acc[1] += e * (1.f - bf * kx * kx);
-                acc[2] += e * (-bf * kx * ky);
-                acc[3] += e * (-bf * kx * kzv);
-                acc[4] += e * (1.f - bf * ky * ky);
-                acc[5] += e * (-bf * ky * kzv);
-                acc[6] += e * (1.f - bf * kzv * kzv);
+                acc[2] += e * (-bf * kx * kyp);
+                acc[3] += e * (-bf * kx * kzp);
+                acc[4] += e * (1.f - bf * kyp * kyp);
+                acc[5] += e * (-bf * kyp * kzp);
+                acc[6] += e * (1.f - bf * kzp * kzp);
             }
         }
     // Two inverse transforms along x give all four output lines, because kd_y and kd_z are constants of the line:
@@ -494,11 +510,11 @@ k_fft_x_fused_half(int n0, int n1, int n2, const float2* __restrict__ H, float2*
 //   M1 = W_xx + i W_yy,   M2 = W_zz + i W_xy,   M3 = W_xz + i W_yz,      B_ab = delta_ab - (2 / 4 alpha^2 + 2 / k^2) k_a k_b
 // (B is real and even in k, so each product phi B_ab is the spectrum of a real field).  Full spectrum in M3 (after the
 // forward z and y passes), in-place line by line for M3.
-template <int R1, int R2>
+template <int R1, int R2, bool TRI>
 __global__ void __launch_bounds__(Split<R1, R2>::THREADS)
 k_fft_x_virial(int n0, int n1, int n2, float2* __restrict__ M1, float2* __restrict__ M2, float2* __restrict__ M3,
                const float2* __restrict__ twg, const float* __restrict__ tabA, const float* __restrict__ tabK,
-               float c0 /* 2 pi / Omega */, float inv4a2)
+               float c0 /* 2 pi / Omega */, float inv4a2, KB kb)
 {
     using S = Split<R1, R2>;
     using SI = Split<R2, R1>;
@@ -526,14 +542,16 @@ k_fft_x_virial(int n0, int n1, int n2, float2* __restrict__ M1, float2* __restri
     const float ky = tabK[FFT_MAXN + iy], kz = tabK[2 * FFT_MAXN + iz];
     const float Ayz = c0 * tabA[FFT_MAXN + iy] * tabA[2 * FFT_MAXN + iz];
     const float kyz2 = ky * ky + kz * kz;
+    const float lx = TRI ? ky * kb.b[1] + kz * kb.b[2] : 0.f, ly = TRI ? ky * kb.b[4] + kz * kb.b[5] : 0.f, lz = TRI ? ky * kb.b[7] + kz * kb.b[8] : 0.f;
 #pragma unroll
     for (int d = 0; d < S::D2; ++d)
 #pragma unroll
         for (int k1 = 0; k1 < R2; ++k1) {
             const int ix = (u + S::TPL * d) + R1 * k1;
-            const float kx = tK[ix];
-            const float k2 = kx * kx + kyz2;
-            const float G = k2 > 0.f ? __fdividef(Ayz * tA[ix], k2) : 0.f;
+            float kx = tK[ix], kyp = ky, kzp = kz, k2;
+            if (TRI) { const float nx = kx; kx = fmaf(nx, kb.b[0], lx); kyp = fmaf(nx, kb.b[3], ly); kzp = fmaf(nx, kb.b[6], lz); k2 = kx * kx + kyp * kyp + kzp * kzp; }
+            else k2 = kx * kx + kyz2;
+            const float G = k2 > 0.f ? __fdividef(TRI ? Ayz * tA[ix] * __expf(-k2 * inv4a2) : Ayz * tA[ix], k2) : 0.f;
             ph[d * R2 + k1].x *= G; ph[d * R2 + k1].y *= G;
         }
     float2* const Ms[3] = {M1, M2, M3};
@@ -544,14 +562,15 @@ k_fft_x_virial(int n0, int n1, int n2, float2* __restrict__ M1, float2* __restri
 #pragma unroll
             for (int k1 = 0; k1 < R2; ++k1) {
                 const int ix = (u + S::TPL * d) + R1 * k1;
-                const float kx = tK[ix];
-                const float k2 = kx * kx + kyz2;
+                float kx = tK[ix], kyp = ky, kzp = kz, k2;
+                if (TRI) { const float nx = kx; kx = fmaf(nx, kb.b[0], lx); kyp = fmaf(nx, kb.b[3], ly); kzp = fmaf(nx, kb.b[6], lz); k2 = kx * kx + kyp * kyp + kzp * kzp; }
+                else k2 = kx * kx + kyz2;
                 const float bf = k2 > 0.f ? 2.f * inv4a2 + __fdividef(2.f, k2) : 0.f;
                 const float one = k2 > 0.f ? 1.f : 0.f;
                 float B1, B2;
-                if (pair == 0) { B1 = one - bf * kx * kx; B2 = one - bf * ky * ky; }
-                else if (pair == 1) { B1 = one - bf * kz * kz; B2 = -bf * kx * ky; }
-                else { B1 = -bf * kx * kz; B2 = -bf * ky * kz; }
+                if (pair == 0) { B1 = one - bf * kx * kx; B2 = one - bf * kyp * kyp; }
+                else if (pair == 1) { B1 = one - bf * kzp * kzp; B2 = -bf * kx * kyp; }
+                else { B1 = -bf * kx * kzp; B2 = -bf * kyp * kzp; }
                 const float2 f = ph[d * R2 + k1];
                 v[d * R2 + k1] = make_float2(f.x * B1 - f.y * B2, f.x * B2 + f.y * B1);
             }
@@ -688,7 +707,15 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
     const float c2k = 2.f * (float)QNEP_K_COULOMB;
     phik[p] = c2k * s_out[0][t];                          // bracket of Eq. 38
     const float cq = -c2k * q[p];                         // Eq. 37
-    const float fx = cq * s_out[1][t], fy = cq * s_out[2][t], fz = cq * s_out[3][t];
+    float fx = cq * s_out[1][t], fy = cq * s_out[2][t], fz = cq * s_out[3][t];
+    if (g.triclinic) {
+        // the meshes carry the gradient along the reciprocal basis vectors (see KB): Cartesian F_a = sum_c hinv[3a + c] |h_c| f_c
+        const float m0 = (float)g.L[0], m1 = (float)g.L[1], m2 = (float)g.L[2];
+        const float f0 = fx * m0, f1 = fy * m1, f2 = fz * m2;
+        fx = (float)g.hinv[0] * f0 + (float)g.hinv[1] * f1 + (float)g.hinv[2] * f2;
+        fy = (float)g.hinv[3] * f0 + (float)g.hinv[4] * f1 + (float)g.hinv[5] * f2;
+        fz = (float)g.hinv[6] * f0 + (float)g.hinv[7] * f1 + (float)g.hinv[8] * f2;
+    }
     if (add_to_Fs) { Fs[p] += fx; Fs[N + p] += fy; Fs[2 * N + p] += fz; }
     else { Fs[p] = fx; Fs[N + p] = fy; Fs[2 * N + p] = fz; }
 }
@@ -755,7 +782,8 @@ int qnep_setup_pppm(qnep_handle* h)
     if (!h->d_gtab) QNEP_CUDA_OK(h, cudaMalloc(&h->d_gtab, sizeof(float) * 9 * FFT_MAXN));
     std::vector<float2> tw(3 * FFT_MAXN, make_float2(0.f, 0.f));
     std::vector<float> tab(9 * FFT_MAXN, 0.f);
-    const double L[3] = {h->box[0], h->box[4], h->box[8]};
+    const double L[3] = {h->geo.L[0], h->geo.L[1], h->geo.L[2]};      // lengths of the cell vectors
+    const bool tri = h->geo.triclinic != 0;
     for (int a = 0; a < 3; ++a) {
         const int n = grid[a];
         for (int t = 0; t < n; ++t) {
@@ -768,8 +796,9 @@ int qnep_setup_pppm(qnep_handle* h)
             const double x = M_PI * nn / n;
             const double sc = x == 0.0 ? 1.0 : sin(x) / x;
             const double d = alias_den(sin(x));
-            tab[a * FFT_MAXN + m] = (float)(exp(-k * k / (4.0 * h->alpha * h->alpha)) * pow(sc, 10) / (d * d));
-            tab[(3 + a) * FFT_MAXN + m] = (float)k;
+            // triclinic: the Gaussian and k itself are formed per mesh point from the integer indices (see KB)
+            tab[a * FFT_MAXN + m] = (float)((tri ? 1.0 : exp(-k * k / (4.0 * h->alpha * h->alpha))) * pow(sc, 10) / (d * d));
+            tab[(3 + a) * FFT_MAXN + m] = tri ? (float)nn : (float)k;
             tab[(6 + a) * FFT_MAXN + m] = (2 * nn == -n) ? 0.f : (float)k;
         }
     }
@@ -782,7 +811,6 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
 {
     const int64_t N = h->N;
     const int nb = (int)((N + 127) / 128);
-    const double L[3] = {h->box[0], h->box[4], h->box[8]};
     const int n0 = h->geo.grid[0], n1 = h->geo.grid[1], n2 = h->geo.grid[2];
     const float2* tw0 = h->d_twiddle;
     const float2* tw1 = h->d_twiddle + FFT_MAXN;
@@ -800,7 +828,13 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
         k_spread<<<nb, 128, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cm, h->d_q, h->d_mesh);
         h->launches += 1;
     }
-    const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    const Geometry& G = h->geo;
+    const double vol = std::fabs(G.h[0] * (G.h[4] * G.h[8] - G.h[5] * G.h[7]) - G.h[1] * (G.h[3] * G.h[8] - G.h[5] * G.h[6]) +
+                                 G.h[2] * (G.h[3] * G.h[7] - G.h[4] * G.h[6]));
+    const float c0 = (float)(2.0 * M_PI / vol), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    const bool tri = G.triclinic != 0;
+    KB kb;
+    for (int k = 0; k < 9; ++k) kb.b[k] = (float)(2.0 * M_PI * G.hinv[k]);
     if (h->d_half) {
         // 2.-3. forward transform on the half spectrum (the mesh is real): z and y passes on [x][y][N2/2 + LINES],
         //       the fused x pass restores the full spectrum of M1, M2 on the way out
@@ -826,15 +860,14 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
             const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 3 * S::N +
                                 sizeof(float2) * S::E * S::THREADS;
             const unsigned nt = (unsigned)((int64_t)n1 * NH / LINES);
-            if (virial) {
-                note(allow_smem(k_fft_x_fused_half<R1, R2, true>, smem));
-                k_fft_x_fused_half<R1, R2, true><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_half, h->d_cm1, h->d_cm2, tw0, h->d_gtab,
-                                                                             h->d_gtab + 3 * FFT_MAXN, h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
-            } else {
-                note(allow_smem(k_fft_x_fused_half<R1, R2, false>, smem));
-                k_fft_x_fused_half<R1, R2, false><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_half, h->d_cm1, h->d_cm2, tw0, h->d_gtab,
-                                                                              h->d_gtab + 3 * FFT_MAXN, h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
-            }
+            auto go = [&](auto vf, auto tf) {
+                constexpr bool V = decltype(vf)::value, TR = decltype(tf)::value;
+                note(allow_smem(k_fft_x_fused_half<R1, R2, V, TR>, smem));
+                k_fft_x_fused_half<R1, R2, V, TR><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_half, h->d_cm1, h->d_cm2, tw0, h->d_gtab,
+                                                                              h->d_gtab + 3 * FFT_MAXN, h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums, kb);
+            };
+            if (virial) { if (tri) go(std::true_type(), std::true_type()); else go(std::true_type(), std::false_type()); }
+            else { if (tri) go(std::false_type(), std::true_type()); else go(std::false_type(), std::false_type()); }
         });
     } else {
     // 2. forward z (real -> complex), forward y
@@ -859,15 +892,14 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
         using SI = Split<R2, R1>;
         const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 3 * S::N;
         const unsigned nt = (unsigned)((int64_t)n1 * n2 / LINES);
-        if (virial) {
-            note(allow_smem(k_fft_x_fused<R1, R2, true>, smem));
-            k_fft_x_fused<R1, R2, true><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, tw0, h->d_gtab, h->d_gtab + 3 * FFT_MAXN,
-                                                                    h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
-        } else {
-            note(allow_smem(k_fft_x_fused<R1, R2, false>, smem));
-            k_fft_x_fused<R1, R2, false><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, tw0, h->d_gtab, h->d_gtab + 3 * FFT_MAXN,
-                                                                     h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums);
-        }
+        auto go = [&](auto vf, auto tf) {
+            constexpr bool V = decltype(vf)::value, TR = decltype(tf)::value;
+            note(allow_smem(k_fft_x_fused<R1, R2, V, TR>, smem));
+            k_fft_x_fused<R1, R2, V, TR><<<nt, S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, tw0, h->d_gtab, h->d_gtab + 3 * FFT_MAXN,
+                                                                     h->d_gtab + 6 * FFT_MAXN, c0, inv4a2, h->d_sums, kb);
+        };
+        if (virial) { if (tri) go(std::true_type(), std::true_type()); else go(std::true_type(), std::false_type()); }
+        else { if (tri) go(std::false_type(), std::true_type()); else go(std::false_type(), std::false_type()); }
     });
     }
     // 4. inverse y on both meshes, inverse z -> interleaved real fields
@@ -902,7 +934,6 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
 int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s)
 {
     const int64_t N = h->N;
-    const double L[3] = {h->box[0], h->box[4], h->box[8]};
     const int n0 = h->geo.grid[0], n1 = h->geo.grid[1], n2 = h->geo.grid[2];
     const float2* tw0 = h->d_twiddle;
     const float2* tw1 = h->d_twiddle + FFT_MAXN;
@@ -910,7 +941,13 @@ int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s)
     if (!h->d_cm3) QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm3, sizeof(float2) * h->ngrid));
     cudaError_t ce = cudaSuccess;
     auto note = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
-    const float c0 = (float)(2.0 * M_PI / (L[0] * L[1] * L[2])), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    const Geometry& G = h->geo;
+    const double vol = std::fabs(G.h[0] * (G.h[4] * G.h[8] - G.h[5] * G.h[7]) - G.h[1] * (G.h[3] * G.h[8] - G.h[5] * G.h[6]) +
+                                 G.h[2] * (G.h[3] * G.h[7] - G.h[4] * G.h[6]));
+    const float c0 = (float)(2.0 * M_PI / vol), inv4a2 = (float)(1.0 / (4.0 * h->alpha * h->alpha));
+    const bool tri = G.triclinic != 0;
+    KB kb;
+    for (int k = 0; k < 9; ++k) kb.b[k] = (float)(2.0 * M_PI * G.hinv[k]);
     with_split(n2, [&](auto r1, auto r2) {
         constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;
         using S = Split<R1, R2>;
@@ -930,9 +967,15 @@ int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s)
         using S = Split<R1, R2>;
         using SI = Split<R2, R1>;
         const size_t smem = sizeof(float2) * (LINES * (S::LP > SI::LP ? S::LP : SI::LP) + S::N) + sizeof(float) * 2 * S::N;
-        note(allow_smem(k_fft_x_virial<R1, R2>, smem));
-        k_fft_x_virial<R1, R2><<<(unsigned)((int64_t)n1 * n2 / LINES), S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, h->d_cm3, tw0, h->d_gtab,
-                                                                                             h->d_gtab + 3 * FFT_MAXN, c0, inv4a2);
+        if (tri) {
+            note(allow_smem(k_fft_x_virial<R1, R2, true>, smem));
+            k_fft_x_virial<R1, R2, true><<<(unsigned)((int64_t)n1 * n2 / LINES), S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, h->d_cm3, tw0, h->d_gtab,
+                                                                                                       h->d_gtab + 3 * FFT_MAXN, c0, inv4a2, kb);
+        } else {
+            note(allow_smem(k_fft_x_virial<R1, R2, false>, smem));
+            k_fft_x_virial<R1, R2, false><<<(unsigned)((int64_t)n1 * n2 / LINES), S::THREADS, smem, s>>>(n0, n1, n2, h->d_cm1, h->d_cm2, h->d_cm3, tw0, h->d_gtab,
+                                                                                                        h->d_gtab + 3 * FFT_MAXN, c0, inv4a2, kb);
+        }
     });
     with_split(n1, [&](auto r1, auto r2) {
         constexpr int R1 = decltype(r1)::value, R2 = decltype(r2)::value;

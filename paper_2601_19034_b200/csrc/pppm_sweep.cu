@@ -30,6 +30,8 @@
 
 #include "pppm_common.cuh"
 
+#include <cmath>
+
 namespace {
 
 constexpr int MBX = QNEP_MB_X, MBY = QNEP_MB_Y, MBZ = QNEP_MB_Z;
@@ -323,8 +325,12 @@ int qnep_setup_sweep(qnep_handle* h)
 bool qnep_sweep_usable(const qnep_handle* h)
 {
     if (h->es.method != 2 || h->nmbins == 0 || h->pppm_kernels == 1 || !h->tm_ok) return false;
-    for (int a = 0; a < 3; ++a)
-        if (0.5 * h->skin > h->geo.L[a] / h->geo.grid[a]) return false;
+    for (int a = 0; a < 3; ++a) {
+        // a displacement of skin / 2 changes the mesh coordinate along a by at most skin / 2 * |b*_a| * grid_a (any cell)
+        const double* hi = h->geo.hinv;
+        const double bnorm = std::sqrt(hi[a] * hi[a] + hi[3 + a] * hi[3 + a] + hi[6 + a] * hi[6 + a]);
+        if (0.5 * h->skin * bnorm * h->geo.grid[a] > 1.0) return false;
+    }
     return h->pppm_kernels == 2 || h->N >= QNEP_SWEEP_MIN_ATOMS;
 }
 

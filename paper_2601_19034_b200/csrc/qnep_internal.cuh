@@ -45,11 +45,26 @@ __host__ __device__ __forceinline__ int qnep_image_bits(int d0, int d1, int d2)
 {
     return (int)(((unsigned)(d0 & 3) << 30) | ((unsigned)(d1 & 3) << 28) | ((unsigned)(d2 & 3) << 26));
 }
-__device__ __forceinline__ void qnep_add_image_shift(int e, float h0, float h1, float h2, float& dx, float& dy, float& dz)
+struct CellVecs { float c[9]; int tri; };      // Geometry::cellv in registers
+__device__ __forceinline__ void qnep_add_image_shift(int e, const CellVecs& cv, float& dx, float& dy, float& dz)
 {
-    dx = fmaf((float)(e >> 30), h0, dx);
-    dy = fmaf((float)((int)((unsigned)e << 2) >> 30), h1, dy);
-    dz = fmaf((float)((int)((unsigned)e << 4) >> 30), h2, dz);
+    const float f0 = (float)(e >> 30), f1 = (float)((int)((unsigned)e << 2) >> 30), f2 = (float)((int)((unsigned)e << 4) >> 30);
+    dx = fmaf(f0, cv.c[0], dx);
+    dy = fmaf(f1, cv.c[4], dy);
+    dz = fmaf(f2, cv.c[8], dz);
+    if (cv.tri) {                                  // warp-uniform: off-diagonal parts of a non-orthogonal cell
+        dx = fmaf(f1, cv.c[3], fmaf(f2, cv.c[6], dx));
+        dy = fmaf(f0, cv.c[1], fmaf(f2, cv.c[7], dy));
+        dz = fmaf(f0, cv.c[2], fmaf(f1, cv.c[5], dz));
+    }
+}
+__device__ __forceinline__ CellVecs qnep_cell_vecs(const float (&cellv)[9], int tri)
+{
+    CellVecs cv;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) cv.c[k] = cellv[k];
+    cv.tri = tri;
+    return cv;
 }
 
 constexpr double QNEP_K_COULOMB = 14.3996454784;   // eV A / e^2 (reading S9)
@@ -99,9 +114,13 @@ __device__ __forceinline__ void qnep_zbl_eval(const ZblParams& z, int ti, int tj
 // overflow flags hold the largest count seen when a list exceeded its capacity (0 otherwise)
 enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_BAD_TYPE /* a species index outside 0..T-1 */, FLAG_COUNT = 8 };
 
-struct Geometry {            // orthorhombic cell and the cell grid of the neighbour search
-    double L[3];
-    double hcell[3];         // cell edge = L / ncell >= rc_r + skin
+struct Geometry {            // periodic cell (rows of h = cell vectors a, b, c; any non-degenerate cell) and the cell grid of the neighbour search
+    double L[3];             // lengths of the cell vectors (orthorhombic: the box edges)
+    double hcell[3];         // |cell vector| / ncell; the search cells are h_a / ncell_a with perpendicular widths >= rc_r + skin
+    double h[9];             // cell vectors, row a = h[3a .. 3a+2]
+    double hinv[9];          // fractional coordinate f_b = sum_a r_a hinv[3a + b]; reciprocal vector b = 2 pi hinv[. + b]
+    float cellv[9];          // edge vectors of a search cell, row a = h_a / ncell_a: the image shift of a neighbour word is d . cellv
+    int triclinic;           // 0: h is diagonal (cellv too: three FMAs per shift instead of nine)
     int ncell[3];
     int ncells;
     float rc_r2, rc_a2;      // cutoffs squared

@@ -322,6 +322,81 @@ def test_zbl_parity(torch, oracle, case):
     assert exc.value.code == Q.QNEP_ERR_INVALID_ARG
 
 
+# ---------------------------------------------------------------- triclinic cells (PAPER.md :104)
+@pytest.mark.parametrize("case", ["config0_ewald_mode1", "config0_ewald_mode2", "config1_no_es", "config1_pppm", "config1_pppm_mode1",
+                                  "config1_mesh16", "config2_pppm", "config1_sheared_box"])
+def test_triclinic_parity(torch, oracle, case):
+    """Non-orthogonal cells through the whole path: cell list and image shifts in the cell basis, Ewald and PPPM with k from
+    the reciprocal basis vectors, all outputs (E, F, W, q, BEC, per-atom virial).  'config1_sheared_box' describes the
+    ORTHORHOMBIC water box of config 1 by the cell (a + b, b, c): the same crystal, so the result must also agree with the
+    orthorhombic run (Ewald-free parts exactly, PPPM within the discretisation of the tilted mesh)."""
+    bins = True
+    if case.startswith("config0"):
+        w = I.triclinic_variant(I.config0(mode=1 if case.endswith("mode1") else 2), tilt=((0, 0, 0), (0.12, 0, 0), (0.05, -0.08, 0)))
+        bins = False
+    elif case == "config1_no_es":
+        w = I.triclinic_variant(I.config1())
+        w.es = replace(w.es, method=0)
+    elif case == "config1_pppm":
+        w = I.triclinic_variant(I.config1())
+    elif case == "config1_pppm_mode1":
+        w = I.triclinic_variant(I.config1(mode=1))
+    elif case == "config1_mesh16":
+        w = I.triclinic_variant(I.config1())
+        w.es = replace(w.es, grid=(32, 16, 16))
+    elif case == "config2_pppm":
+        w = I.triclinic_variant(I.config2(), tilt=((0, 0, 0), (-0.2, 0, 0), (0.1, 0.15, 0)))
+    else:
+        w0 = I.config1()
+        hb = w0.box.reshape(3, 3)
+        w = replace(w0, box=np.array([hb[0] + hb[1], hb[1], hb[2]]).ravel(), name="config1_sheared_box")
+    ref = oracle.compute_workload(w, use_bins=bins, want_atom_virial=True, want_bec=True)
+    h = Q.from_workload(w)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    try:
+        out = h.compute_atom_virial(pos, types, w.box)
+    except Q.QnepError as err:
+        if err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
+            raise
+        out = h.compute_atom_virial(pos, types, w.box)
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    assert_parity(w, res, ref, f"triclinic, {case}")
+    assert rel_rms(res["virial_atom"], ref["virial_atom"]) <= 1e-4
+    _, full = gpu_eval(torch, w, handle=h, want=Q.WANT_ALL | Q.WANT_BEC)
+    assert_parity(w, full, ref, f"triclinic, plain call, {case}")
+    assert rel_rms(full["bec"], ref["bec"]) <= 1e-4
+    st = h.neighbor_stats()
+    cr, _, _ = oracle.neighbors(w.pos, w.box, w.model.rc_r, use_bins=bins)
+    assert st["max_radial"] == cr.max() and abs(st["mean_radial"] - cr.mean()) < 1e-9
+    if case == "config1_sheared_box":
+        _, ortho = gpu_eval(torch, I.config1(), want=Q.WANT_ALL)
+        assert rel_rms(full["forces"], ortho["forces"]) < 2e-3        # PPPM discretisation of two different meshes
+        assert np.abs(full["charges"] - ortho["charges"]).max() < 1e-5
+
+
+def test_triclinic_list_reuse_and_md(torch, oracle):
+    """Skin lists on a triclinic cell: reused lists after the atoms moved give the fresh-build result, atoms that leave the
+    cell through a tilted face are wrapped by the fractional coordinate, and the MD driver conserves energy."""
+    w = I.triclinic_variant(I.config1())
+    rng = np.random.Generator(np.random.PCG64(7))
+    moved = replace(w, pos=w.pos + rng.uniform(-0.2, 0.2, size=w.pos.shape))
+    ref = oracle.compute_workload(moved)
+    h = Q.from_workload(w)
+    h.set_neighbor_policy(1.0, 10)
+    gpu_eval(torch, w, handle=h)                                  # builds the lists
+    _, res = gpu_eval(torch, moved, handle=h)                     # reuses them
+    assert h.get_timings()["neighbor"] < 0.05                     # no rebuild happened
+    assert_parity(moved, res, ref, "triclinic, lists reused")
+    # whole-lattice-vector translations of single atoms change nothing
+    hb = w.box.reshape(3, 3)
+    shifted = moved.pos.copy()
+    for i, (a, b, c) in enumerate(rng.integers(-2, 3, size=(50, 3))):
+        shifted[:, 7 * i] += a * hb[0] + b * hb[1] + c * hb[2]
+    _, res2 = gpu_eval(torch, replace(moved, pos=shifted), handle=Q.from_workload(w))
+    assert_parity(moved, res2, ref, "triclinic, unwrapped coordinates")
+
+
 # ---------------------------------------------------------------- neighbour policy, errors
 def test_skin_and_rebuild_identity(torch, oracle):
     """Lists built with a skin and reused after the atoms moved give the same result as a fresh build."""
@@ -402,11 +477,17 @@ def test_unsupported_inputs(torch):
     h = Q.from_workload(w)
     pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
     types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    # a cell so strongly tilted that its perpendicular width along b falls below r_c: the 27-cell search cannot serve it
     tric = w.box.copy()
-    tric[3] = 1.0
+    tric[3] = 20.0
     with pytest.raises(Q.QnepError) as ei:
         h.compute(pos, types, tric)
     assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED
+    flat = w.box.copy()
+    flat[6:9] = flat[0:3]                       # c parallel to a: zero volume
+    with pytest.raises(Q.QnepError) as ei:
+        h.compute(pos, types, flat)
+    assert ei.value.code == Q.QNEP_ERR_INVALID_ARG
     small = np.diag([5.0, 11.28, 11.28]).ravel()
     with pytest.raises(Q.QnepError) as ei:
         h.compute(pos, types, small)
