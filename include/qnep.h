@@ -215,7 +215,8 @@ int qnep_set_md_graphs(qnep_handle *h, int32_t mode);
 
 /*
  * Choice of the PPPM charge-assignment kernel (Eq. 35).  mode 0 (default): the shared-memory sweep kernel
- * when n_atoms >= 20000 and skin / 2 <= mesh spacing, else one thread per atom; 1: always one thread per atom;
+ * when n_atoms >= 20000, the mesh has at least 1024 (y, z) columns of 8 x 8 points (256 x 256) and skin / 2 <= mesh
+ * spacing, else one thread per atom; 1: always one thread per atom;
  * 2: the sweep kernel whenever skin / 2 <= mesh spacing (small systems too: used by the parity tests).  Both give the
  * same mesh up to the order of fp32 additions.  Errors: INVALID_ARG.
  */

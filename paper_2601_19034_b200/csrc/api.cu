@@ -176,6 +176,15 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         }
         for (int a = 0; a < 3; ++a) h->nmb[a] = nmb[a];
     }
+    {
+        // scratch of the multi-block scan: 2 (chunks + 1) ints for the longer of the two key arrays (2048 keys per chunk)
+        const size_t need = 2 * ((size_t)std::max(nkeys, h->nmbins) / 2048 + 2);
+        if (need > h->scantmp_len) {
+            if ((rc = dev_alloc(h, &h->d_scantmp, need))) return rc;
+            h->scantmp_len = need;
+            h->ws_generation += 1;
+        }
+    }
     const bool geo_changed = box_changed || std::memcmp(&g, &h->geo, sizeof(Geometry)) != 0;
     h->geo = g;
     std::memcpy(h->box, box, sizeof(double) * 9);
@@ -457,6 +466,13 @@ int enqueue_pipeline(qnep_handle* h, bool rebuild, bool timed, int64_t N, const 
     if ((rc = qnep_launch_desc_angular(h, s))) return rc;
     QNEP_STAGE(4);
     if ((rc = qnep_launch_nn(h, (want & QNEP_WANT_CHARGES) ? charges : nullptr, s))) return rc;
+    if (h->early_q_host && (want & QNEP_WANT_CHARGES)) {
+        // qnep_compute_host: the charges are final here (Eq. 33); their device-to-host copy overlaps the rest of the evaluation
+        QNEP_CUDA_OK(h, cudaEventRecord(h->ev_q_ready, s));
+        QNEP_CUDA_OK(h, cudaStreamWaitEvent(h->copy_stream, h->ev_q_ready, 0));
+        QNEP_CUDA_OK(h, cudaMemcpyAsync(h->early_q_host, h->early_q_dev, sizeof(double) * N, cudaMemcpyDeviceToHost, h->copy_stream));
+        QNEP_CUDA_OK(h, cudaEventRecord(h->ev_q_copied, h->copy_stream));
+    }
     QNEP_STAGE(5);
     if (h->es.method != 0 && h->model.mode == 1) { if ((rc = qnep_launch_realspace(h, atomv, s))) return rc; }
     QNEP_STAGE(6);
@@ -737,12 +753,22 @@ int qnep_compute_host(qnep_handle* h, int64_t n_atoms, const double* pos_host, c
     double* d_z = d_q + n;
     QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, s));
     QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_htypes, types_host, sizeof(int32_t) * n, cudaMemcpyHostToDevice, s));
+    const bool early_q = (want & QNEP_WANT_CHARGES) != 0;
+    if (early_q) {
+        if (!h->copy_stream) {
+            QNEP_CUDA_OK(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+            QNEP_CUDA_OK(h, cudaEventCreateWithFlags(&h->ev_q_ready, cudaEventDisableTiming));
+            QNEP_CUDA_OK(h, cudaEventCreateWithFlags(&h->ev_q_copied, cudaEventDisableTiming));
+        }
+        h->early_q_host = charges_host; h->early_q_dev = d_q;
+    }
     rc = qnep_compute(h, n_atoms, h->d_hpos, h->d_htypes, box, want, d_e, d_f, d_w, d_q, d_z, s);
+    h->early_q_host = nullptr; h->early_q_dev = nullptr;
     if (rc) return rc;
     if (want & QNEP_WANT_ENERGY) QNEP_CUDA_OK(h, cudaMemcpyAsync(energy_host, d_e, sizeof(double), cudaMemcpyDeviceToHost, s));
     if (want & QNEP_WANT_FORCES) QNEP_CUDA_OK(h, cudaMemcpyAsync(forces_host, d_f, sizeof(double) * 3 * n, cudaMemcpyDeviceToHost, s));
     if (want & QNEP_WANT_VIRIAL) QNEP_CUDA_OK(h, cudaMemcpyAsync(virial_host, d_w, sizeof(double) * 9, cudaMemcpyDeviceToHost, s));
-    if (want & QNEP_WANT_CHARGES) QNEP_CUDA_OK(h, cudaMemcpyAsync(charges_host, d_q, sizeof(double) * n, cudaMemcpyDeviceToHost, s));
+    if (early_q) QNEP_CUDA_OK(h, cudaStreamWaitEvent(s, h->ev_q_copied, 0));      // the copy was enqueued inside the pipeline
     if (want & QNEP_WANT_BEC) QNEP_CUDA_OK(h, cudaMemcpyAsync(bec_host, d_z, sizeof(double) * 9 * n, cudaMemcpyDeviceToHost, s));
     return qnep_check(h);
 }
@@ -959,9 +985,10 @@ void qnep_destroy(qnep_handle* h)
     if (!h) return;
     drop_md_graphs(h);
     if (h->md_stream) cudaStreamDestroy(h->md_stream);
+    if (h->copy_stream) { cudaStreamDestroy(h->copy_stream); cudaEventDestroy(h->ev_q_ready); cudaEventDestroy(h->ev_q_copied); }
     if (h->md_fence) cudaEventDestroy(h->md_fence);
     free_workspace(h);
-    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_ctot, h->d_cstart, h->d_mbcnt, h->d_mbstart, h->d_mbfill, h->d_sums, h->d_flags, h->d_kvec,
+    void* ptrs[] = {h->d_params, h->d_cR, h->d_cA, h->d_nn, h->d_cnt, h->d_start, h->d_fill, h->d_scantmp, h->d_ctot, h->d_cstart, h->d_mbcnt, h->d_mbstart, h->d_mbfill, h->d_sums, h->d_flags, h->d_kvec,
                     h->d_kint, h->d_ephase, h->d_S, h->d_mesh, h->d_half, h->d_cm1, h->d_cm2, h->d_cm3, h->d_Wat, h->d_field, h->d_gtab, h->d_twiddle, h->d_hpos,
                     h->d_htypes, h->d_hout};
     for (void* p : ptrs) if (p) cudaFree(p);

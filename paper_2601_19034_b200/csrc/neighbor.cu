@@ -111,6 +111,58 @@ __global__ void k_exclusive_scan(int n, const int* __restrict__ in, int* __restr
     if (threadIdx.x == 0) out[n] = carry;
 }
 
+// Exclusive scan over many blocks (key counts grow with the volume: T x ncells): every block scans SCAN_CHUNK elements in
+// place and reports its total, the totals are scanned by the single-block kernel above, a third pass adds the offsets.
+constexpr int SCAN_CHUNK = 2048;      // two elements per thread of a 1024-thread block
+
+__global__ void __launch_bounds__(1024)
+k_scan_chunks(int n, const int* __restrict__ in, int* __restrict__ out, int* __restrict__ totals)
+{
+    __shared__ int warp_sums[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int i0 = blockIdx.x * SCAN_CHUNK + 2 * threadIdx.x;
+    const int a = i0 < n ? in[i0] : 0, b = i0 + 1 < n ? in[i0 + 1] : 0;
+    int x = a + b;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_sums[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        int w = warp_sums[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, w, o);
+            if (lane >= o) w += y;
+        }
+        warp_sums[lane] = w;
+    }
+    __syncthreads();
+    const int excl = (wid > 0 ? warp_sums[wid - 1] : 0) + x - (a + b);
+    if (i0 < n) out[i0] = excl;
+    if (i0 + 1 < n) out[i0 + 1] = excl + a;
+    if (threadIdx.x == 1023) totals[blockIdx.x] = excl + a + b;
+}
+
+__global__ void k_scan_add(int n, int* __restrict__ out, const int* __restrict__ offsets, int nchunks)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] += offsets[i / SCAN_CHUNK];
+    if (i == n) out[n] = offsets[nchunks];        // grand total behind the last element
+}
+
+// out[0 .. n] = exclusive scan of in[0 .. n-1] (out[n] = total); tmp holds 2 (nchunks + 1) ints
+static void exclusive_scan(int n, const int* in, int* out, int* tmp, cudaStream_t s)
+{
+    if (n <= 4 * SCAN_CHUNK) { k_exclusive_scan<<<1, 1024, 0, s>>>(n, in, out); return; }
+    const int nchunks = (n + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    k_scan_chunks<<<nchunks, 1024, 0, s>>>(n, in, out, tmp);
+    k_exclusive_scan<<<1, 1024, 0, s>>>(nchunks, tmp, tmp + nchunks + 1);
+    k_scan_add<<<(n + 1 + 255) / 256, 256, 0, s>>>(n, out, tmp + nchunks + 1, nchunks);
+}
+
 __global__ void k_scatter(int64_t N, const int* __restrict__ key, const int* __restrict__ start,
                           int* __restrict__ fill, int* __restrict__ tmpidx)
 {
@@ -372,7 +424,7 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_cnt, 0, sizeof(int) * (h->nkeys + 1), s));
     QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_fill, 0, sizeof(int) * h->nkeys, s));
     k_bin_count<<<nb, 256, 0, s>>>(N, h->model.n_types, pos, types, h->geo, h->d_key, h->d_cnt, h->d_flags);
-    k_exclusive_scan<<<1, 1024, 0, s>>>(h->nkeys, h->d_cnt, h->d_start);
+    exclusive_scan(h->nkeys, h->d_cnt, h->d_start, h->d_scantmp, s);
     k_scatter<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_fill, h->d_tmpidx);
     k_rank<<<nb, 256, 0, s>>>(N, h->d_key, h->d_start, h->d_tmpidx, h->d_sidx);
     if (h->nmbins > 0) {
@@ -380,7 +432,7 @@ int qnep_launch_build(qnep_handle* h, const double* pos, const int32_t* types, c
         QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mbcnt, 0, sizeof(int) * (h->nmbins + 1), s));
         QNEP_CUDA_OK(h, cudaMemsetAsync(h->d_mbfill, 0, sizeof(int) * h->nmbins, s));
         k_mbin_key<<<nb, 256, 0, s>>>(N, pos, h->d_sidx, h->d_key, h->geo, h->nmb[0], h->nmb[2], h->d_mbkey, h->d_mbcnt);
-        k_exclusive_scan<<<1, 1024, 0, s>>>(h->nmbins, h->d_mbcnt, h->d_mbstart);
+        exclusive_scan(h->nmbins, h->d_mbcnt, h->d_mbstart, h->d_scantmp, s);
         k_scatter<<<nb, 256, 0, s>>>(N, h->d_mbkey, h->d_mbstart, h->d_mbfill, h->d_tmpidx);
         k_rank<<<nb, 256, 0, s>>>(N, h->d_mbkey, h->d_mbstart, h->d_tmpidx, h->d_cmi);
         k_invert_perm<<<nb, 256, 0, s>>>(N, h->d_cmi, h->d_cm);

@@ -331,7 +331,10 @@ bool qnep_sweep_usable(const qnep_handle* h)
         const double bnorm = std::sqrt(hi[a] * hi[a] + hi[3 + a] * hi[3 + a] + hi[6 + a] * hi[6 + a]);
         if (0.5 * h->skin * bnorm * h->geo.grid[a] > 1.0) return false;
     }
-    return h->pppm_kernels == 2 || h->N >= QNEP_SWEEP_MIN_ATOMS;
+    // automatic: the kernel runs one warp per column segment, so it needs thousands of columns to fill the GPU (1024 x 4
+    // at 256^3: 0.19 ms against 0.23 ms; at 128^3 and 64^3 the per-atom kernel is faster: 0.22 / 0.29 ms and 0.05 / 0.17 ms
+    // per reciprocal stage on configs 3 and 2)
+    return h->pppm_kernels == 2 || (h->N >= QNEP_SWEEP_MIN_ATOMS && h->nmb[1] * h->nmb[2] >= 1024);
 }
 
 int qnep_launch_spread_sweep(qnep_handle* h, cudaStream_t s)

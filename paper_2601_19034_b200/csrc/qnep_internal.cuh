@@ -166,6 +166,8 @@ struct qnep_handle {
     int* d_cnt = nullptr;            // [nkeys + 1]
     int* d_start = nullptr;          // [nkeys + 1]
     int* d_fill = nullptr;           // [nkeys]
+    int* d_scantmp = nullptr;        // chunk totals and their scan of the multi-block exclusive scan
+    size_t scantmp_len = 0;
     int* d_tmpidx = nullptr;         // [N]
     int* d_sidx = nullptr;           // [N] sorted -> original
     int* d_ctot = nullptr;           // [ncells + 1] atoms per cell (all species)
@@ -254,7 +256,9 @@ struct qnep_handle {
     cudaEvent_t md_fence = nullptr;
     uint64_t ws_generation = 0;            // bumped whenever workspace pointers, capacities or the geometry change
 
-    // host staging (qnep_compute_host)
+    // host staging (qnep_compute_host); the charges go back on a second stream while the PPPM and force kernels run
+    cudaStream_t copy_stream = nullptr; cudaEvent_t ev_q_ready = nullptr, ev_q_copied = nullptr;
+    double* early_q_host = nullptr; const double* early_q_dev = nullptr;
     double* d_hpos = nullptr; int32_t* d_htypes = nullptr; double* d_hout = nullptr; int64_t hostN = 0;
 
     // timing
