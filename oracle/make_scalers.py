@@ -25,6 +25,10 @@ def main():
         "config3": lambda: I.config3(n_cells=8, grid=32),
         # config 4's parameters on a 10^3-molecule box of the same construction
         "config4": lambda: I.config4(n_side=10, grid=32),
+        # configs 0-2 with NEP4's 4- and 5-body terms switched on (35 descriptors)
+        "config0_45body": lambda: I.with_higher_body_terms(I.config0(), "config0_45body"),
+        "config1_45body": lambda: I.with_higher_body_terms(I.config1(), "config1_45body"),
+        "config2_45body": lambda: I.with_higher_body_terms(I.config2(), "config2_45body"),
     }
     for key, make in samples.items():
         w = make()

@@ -41,7 +41,7 @@ class _Model(C.Structure):
     _fields_ = [("n_types", C.c_int32), ("n_max_r", C.c_int32), ("n_max_a", C.c_int32), ("l_max", C.c_int32),
                 ("basis_r", C.c_int32), ("basis_a", C.c_int32), ("n_neurons", C.c_int32),
                 ("rc_r", C.c_double), ("rc_a", C.c_double), ("mode", C.c_int32),
-                ("sqrt_eps_inf", C.c_double), ("q_total", C.c_double)]
+                ("sqrt_eps_inf", C.c_double), ("q_total", C.c_double), ("l_max_4b", C.c_int32), ("l_max_5b", C.c_int32)]
 
 
 class _Es(C.Structure):
@@ -71,7 +71,7 @@ def _p(a):
 
 def _model(m) -> _Model:
     return _Model(m.n_types, m.n_max_r, m.n_max_a, m.l_max, m.basis_r, m.basis_a, m.n_neurons,
-                  m.rc_r, m.rc_a, m.mode, m.sqrt_eps_inf, m.q_total)
+                  m.rc_r, m.rc_a, m.mode, m.sqrt_eps_inf, m.q_total, getattr(m, "l_max_4b", 0), getattr(m, "l_max_5b", 0))
 
 
 def _es(e) -> _Es:

@@ -24,6 +24,7 @@
  *   BEC               :205-227 Eq. 24-28      reading S12
  *   field response    :229-237 Eq. 29-30      F^ext = E.Z, Pdot = sum_i Z_i v_i (orc_response)
  *   PPPM              :266-304 Eq. 34-38      readings G2 (Eq. 36), S10 (W, P = 5), S11 (FFT)
+ *   4-/5-body terms   :39 (NEP4 -> NEP refs)  reading Z2: cubic invariant of the l = 2 moments, square of the l = 1 invariant
  *   ZBL core          :39 (NEP4 -> NEP refs)  reading Z1: universal ZBL pair repulsion with a cosine switch (optional,
  *                                             orc_set_zbl)
  *
@@ -59,6 +60,7 @@ typedef struct {
     double rc_r, rc_a;
     int32_t mode;              /* 1: U^r+U^k+U^s (Eq. 3); 2: U^k only (Eq. 5) */
     double sqrt_eps_inf, q_total;
+    int32_t l_max_4b, l_max_5b; /* NEP4 higher-body angular terms (reading Z2): 2 / 1 to switch them on, 0 = off */
 } orc_model;
 
 typedef struct {
@@ -403,7 +405,7 @@ static void split_params(const orc_model *m, const double *p, orc_params *P)
     P->m = m;
     P->nR = m->n_max_r + 1;
     P->nA = m->n_max_a + 1;
-    P->D = P->nR + P->nA * m->l_max;
+    P->D = P->nR + P->nA * m->l_max + (m->l_max_4b == 2 ? P->nA : 0) + (m->l_max_5b == 1 ? P->nA : 0);
     P->H = m->n_neurons;
     P->cR = p;
     P->cA = P->cR + (size_t)T * T * P->nR * (m->basis_r + 1);
@@ -456,6 +458,33 @@ static void descriptor_of_atom(const orc_params *P, const int32_t *types, const 
                 for (int l = 1; l <= m->l_max; ++l)
                     D[P->nR + n * m->l_max + (l - 1)] += ga[j * P->nA + n] * ga[k * P->nA + n] * Pl[l];
         }
+    /* Higher-body terms of NEP4 (reading Z2), per radial channel n, appended after the 3-body block:
+     *   4-body: q_n = tr(T_n^3),  T_n = sum_j g_n(r_ij) (rhat_ij rhat_ij^T - 1/3)   (the cubic invariant of the l = 2 moments;
+     *           as a sum over neighbour triples: g_j g_k g_l [c_jk c_kl c_lj - (c_jk^2 + c_kl^2 + c_lj^2)/3 + 2/9])
+     *   5-body: q_n = (w_n . w_n)^2,  w_n = sum_j g_n(r_ij) rhat_ij                (the l = 1 invariant squared;
+     *           as a sum over neighbour quadruples: g_j g_k g_l g_m c_jk c_lm)                                        */
+    int o4 = P->nR + P->nA * m->l_max, o5 = o4 + (m->l_max_4b == 2 ? P->nA : 0);
+    for (int n = 0; n < P->nA; ++n) {
+        double T[3][3] = {{0}}, w[3] = {0, 0, 0};
+        for (int64_t j = 0; j < na; ++j) {
+            double gj = ga[j * P->nA + n];
+            for (int a = 0; a < 3; ++a) {
+                w[a] += gj * u[3 * j + a];
+                for (int c = 0; c < 3; ++c) T[a][c] += gj * (u[3 * j + a] * u[3 * j + c] - (a == c ? 1.0 / 3.0 : 0.0));
+            }
+        }
+        if (m->l_max_4b == 2) {
+            double t3 = 0.0;
+            for (int a = 0; a < 3; ++a)
+                for (int c = 0; c < 3; ++c)
+                    for (int d = 0; d < 3; ++d) t3 += T[a][c] * T[c][d] * T[d][a];
+            D[o4 + n] = t3;
+        }
+        if (m->l_max_5b == 1) {
+            double w2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+            D[o5 + n] = w2 * w2;
+        }
+    }
     free(ga);
     free(u);
 }
@@ -517,6 +546,42 @@ static void partial_forces_of_atom(const orc_params *P, const int32_t *types, co
                 }
         }
         for (int a = 0; a < 3; ++a) Fij[idx[j] * 3 + a] += F[a];
+    }
+    /* higher-body terms (reading Z2): with S = T^2,
+     *   d tr(T^3)/dr_ij = 3 [ g' rhat (rhat.S.rhat - tr S / 3) + (g / r) 2 (S rhat - rhat (rhat.S.rhat)) ]
+     *   d (w.w)^2/dr_ij = 4 (w.w) [ g' rhat (w.rhat) + (g / r) (w - rhat (w.rhat)) ]                        */
+    int o4 = P->nR + P->nA * m->l_max, o5 = o4 + (m->l_max_4b == 2 ? P->nA : 0);
+    for (int n = 0; n < P->nA && (m->l_max_4b == 2 || m->l_max_5b == 1); ++n) {
+        double T[3][3] = {{0}}, w[3] = {0, 0, 0}, S[3][3] = {{0}};
+        for (int64_t j = 0; j < na; ++j) {
+            double gj = ga[j * P->nA + n];
+            for (int a = 0; a < 3; ++a) {
+                w[a] += gj * u[3 * j + a];
+                for (int c = 0; c < 3; ++c) T[a][c] += gj * (u[3 * j + a] * u[3 * j + c] - (a == c ? 1.0 / 3.0 : 0.0));
+            }
+        }
+        for (int a = 0; a < 3; ++a)
+            for (int c = 0; c < 3; ++c)
+                for (int d = 0; d < 3; ++d) S[a][c] += T[a][d] * T[d][c];
+        double trS = S[0][0] + S[1][1] + S[2][2], w2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+        for (int64_t j = 0; j < na; ++j) {
+            const double *uj = u + 3 * j;
+            double gj = ga[j * P->nA + n], dgj = dga[j * P->nA + n];
+            double Su[3], uSu = 0.0, wu = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                Su[a] = S[a][0] * uj[0] + S[a][1] * uj[1] + S[a][2] * uj[2];
+                wu += w[a] * uj[a];
+            }
+            for (int a = 0; a < 3; ++a) uSu += uj[a] * Su[a];
+            for (int a = 0; a < 3; ++a) {
+                double f = 0.0;
+                if (m->l_max_4b == 2)
+                    f += Fp[o4 + n] * 3.0 * (dgj * uj[a] * (uSu - trS / 3.0) + gj / ra[j] * 2.0 * (Su[a] - uj[a] * uSu));
+                if (m->l_max_5b == 1)
+                    f += Fp[o5 + n] * 4.0 * w2 * (dgj * uj[a] * wu + gj / ra[j] * (w[a] - uj[a] * wu));
+                Fij[idx[j] * 3 + a] += f;
+            }
+        }
     }
     free(ga); free(dga); free(u); free(ra); free(idx);
 }

@@ -52,10 +52,13 @@ class ModelDesc:
     mode: int = 2             # 1: U^r+U^k+U^s (Eq. 3); 2: U^k only (Eq. 5)
     sqrt_eps_inf: float = 1.5  # S15
     q_total: float = 0.0
+    l_max_4b: int = 0         # 2: NEP4 4-body terms on (one descriptor per angular radial channel; reading Z2)
+    l_max_5b: int = 0         # 1: NEP4 5-body terms on
 
     @property
     def n_desc(self) -> int:
-        return (self.n_max_r + 1) + (self.n_max_a + 1) * self.l_max
+        return ((self.n_max_r + 1) + (self.n_max_a + 1) * self.l_max
+                + ((self.n_max_a + 1) if self.l_max_4b == 2 else 0) + ((self.n_max_a + 1) if self.l_max_5b == 1 else 0))
 
     def n_params(self) -> int:
         T, H, D = self.n_types, self.n_neurons, self.n_desc
@@ -315,6 +318,15 @@ def config4(mode: int = 2, n_side: int = 70, grid: int = 256) -> Workload:
     """Million-atom water-like box: 70^3 H2O = 1,029,000 atoms, PPPM 256^3 (configs[4])."""
     return water_workload(n_side, grid, BASE_SEED + 4, f"config4_water{3 * n_side ** 3}_pppm{grid}", mode,
                           key="config4")
+
+
+def with_higher_body_terms(w: Workload, key: str) -> Workload:
+    """The same structure with NEP4's 4- and 5-body angular terms switched on (10 more descriptors): new random parameters
+    of the larger network (seed of the config + 5000), scaler from scalers.json[key]."""
+    from dataclasses import replace
+    m = replace(w.model, l_max_4b=2, l_max_5b=1)
+    seed = BASE_SEED + 6000 + sum(ord(c) for c in key)
+    return replace(w, model=m, params=random_params(m, seed, load_scaler(key, m.n_desc)), name=w.name + "_45body")
 
 
 def triclinic_variant(w: Workload, tilt=((0.0, 0.0, 0.0), (0.18, 0.0, 0.0), (0.07, -0.12, 0.0))) -> Workload:

@@ -918,3 +918,109 @@ def test_triclinic_pppm_converges_to_ewald(oracle):
     # anisotropic mesh on the same cell
     pm2 = oracle.electrostatics(pos, q, box, 6.0, 2, I.EsDesc(method=2, alpha=0.3, grid=(64, 32, 32)))
     assert rel_rms(pm2["F"], ew["F"]) < 3e-5
+
+
+# --------------------------------------------------- NEP4 4-/5-body terms (reading Z2)
+def test_higher_body_descriptors_vs_neighbour_sums(oracle):
+    """The 4-body term is a sum over neighbour TRIPLES and the 5-body term a sum over QUADRUPLES of products of the radial
+    functions with rotational invariants of the directions (numpy's Chebyshev series, brute-force loops over the neighbours):
+        q4_n = sum_jkl g_j g_k g_l [c_jk c_kl c_lj - (c_jk^2 + c_kl^2 + c_lj^2)/3 + 2/9],   q5_n = sum_jklm g_j g_k g_l g_m c_jk c_lm;
+    and q4 is the Wigner-3j contraction of the l = 2 moments (complex spherical harmonics from scipy) up to ONE constant."""
+    from numpy.polynomial import chebyshev as Ch
+    try:
+        from scipy.special import sph_harm_y
+        Y = lambda l, m, theta, phi: sph_harm_y(l, m, theta, phi)
+    except ImportError:
+        from scipy.special import sph_harm
+        Y = lambda l, m, theta, phi: sph_harm(m, l, phi, theta)
+    w = I.with_higher_body_terms(I.config0(), "config0_45body")
+    m = w.model
+    assert m.n_desc == 35
+    p = w.params.astype(np.float64)
+    off = I.param_offsets(m)
+    nR, nA, Kb = m.n_max_r + 1, m.n_max_a + 1, m.basis_r + 1
+    cA = p[off["c_a"]:off["scaler"]].reshape(2, 2, nA, Kb)
+    D = oracle.descriptors(m, p, w.pos, w.types, w.box)
+    # the first 25 descriptors are those of the plain model with the same coefficients
+    w0 = I.config0()
+    D0 = oracle.descriptors(w0.model, np.concatenate([p[:off["scaler"]], np.ones(25), np.zeros(w0.model.n_params() - off["scaler"] - 25)]),
+                            w.pos, w.types, w.box)
+    assert np.allclose(D[:, :25], D0, rtol=1e-13, atol=1e-13)
+    counts, jj, dd = oracle.neighbors(w.pos, w.box, m.rc_r, cap=48)
+
+    def g(c, r, rc):
+        x = 2 * (r / rc - 1) ** 2 - 1
+        fc = 0.5 * (1 + np.cos(np.pi * r / rc))
+        return 0.5 * (Ch.chebval(x, c) + c.sum()) * fc
+
+    # Wigner 3j symbols (2 2 2; m1 m2 m3) by the Racah formula
+    from math import factorial as f
+
+    def w3j(j1, j2, j3, m1, m2, m3):
+        if m1 + m2 + m3 != 0:
+            return 0.0
+        tri = f(j1 + j2 - j3) * f(j1 - j2 + j3) * f(-j1 + j2 + j3) / f(j1 + j2 + j3 + 1)
+        pre = np.sqrt(tri * f(j1 + m1) * f(j1 - m1) * f(j2 + m2) * f(j2 - m2) * f(j3 + m3) * f(j3 - m3))
+        tot = 0.0
+        for k in range(0, 20):
+            den = [k, j1 + j2 - j3 - k, j1 - m1 - k, j2 + m2 - k, j3 - j2 + m1 + k, j3 - j1 - m2 + k]
+            if min(den) < 0:
+                continue
+            tot += (-1) ** k / np.prod([float(f(x)) for x in den])
+        return (-1) ** (j1 - j2 - m3) * pre * tot
+
+    ratios = []
+    for i in (0, 13, 40):
+        ti = w.types[i]
+        ang = [(jj[i, s], dd[i, s]) for s in range(counts[i]) if dd[i, s][3] < m.rc_a]
+        u = np.array([d[:3] / d[3] for _, d in ang])
+        c = u @ u.T
+        for n in range(nA):
+            gv = np.array([g(cA[ti, w.types[j], n], d[3], m.rc_a) for j, d in ang])
+            q4 = np.einsum("j,k,l,jk,kl,lj->", gv, gv, gv, c, c, c) - np.einsum("j,k,l,jk->", gv, gv, gv, c ** 2) + 2.0 / 9.0 * gv.sum() ** 3
+            q5 = np.einsum("j,k,jk->", gv, gv, c) ** 2
+            assert abs(D[i, 25 + n] - q4) < 1e-10 * max(1.0, abs(q4)), (i, n, D[i, 25 + n], q4)
+            assert abs(D[i, 30 + n] - q5) < 1e-10 * max(1.0, abs(q5)), (i, n, D[i, 30 + n], q5)
+            A2 = {mm: sum(gj * Y(2, mm, np.arccos(uj[2]), np.arctan2(uj[1], uj[0])) for gj, uj in zip(gv, u)) for mm in range(-2, 3)}
+            inv3j = sum(w3j(2, 2, 2, a, b, -a - b) * A2[a] * A2[b] * A2[-a - b] for a in range(-2, 3) for b in range(-2, 3) if abs(a + b) <= 2)
+            assert abs(inv3j.imag) < 1e-10 * max(1.0, abs(inv3j.real))
+            if abs(q4) > 1e-6:
+                ratios.append(inv3j.real / q4)
+    assert len(ratios) >= 8 and np.ptp(ratios) < 1e-9 * abs(np.mean(ratios)), ratios     # one constant for all environments
+
+
+def test_higher_body_terms_invariance_and_derivatives(oracle):
+    """With the 4-/5-body terms on: rotation and translation invariance of energy and charges, F = -dE/dr and
+    W = -dE/d(strain) by central differences, BEC sum rule, and the new descriptors do move the result."""
+    w = I.with_higher_body_terms(_small_workload(2, 0.3), "config0_45body")
+    out = oracle.compute_workload(w, use_bins=False, want_bec=True, want_atom_virial=True)
+    h = 1e-5
+    for (a, i) in ((0, 2), (1, 30), (2, 61)):
+        p1, p2 = w.pos.copy(), w.pos.copy()
+        p1[a, i] += h
+        p2[a, i] -= h
+        e1 = oracle.compute(w.model, w.params, w.es, p1, w.types, w.box, use_bins=False)["energy"]
+        e2 = oracle.compute(w.model, w.params, w.es, p2, w.types, w.box, use_bins=False)["energy"]
+        fd = -(e1 - e2) / (2 * h)
+        assert abs(fd - out["forces"][a, i]) < 2e-7 * max(1.0, abs(fd)), (fd, out["forces"][a, i])
+    for (a, b) in ((0, 0), (1, 2)):
+        eps = np.zeros((3, 3))
+        eps[a, b] = h
+        def energy(sign):
+            Fm = np.eye(3) + sign * eps
+            return oracle.compute(w.model, w.params, w.es, Fm @ w.pos, w.types,
+                                  (w.box.reshape(3, 3) @ Fm.T).ravel(), use_bins=False)["energy"]
+        fd = -(energy(1) - energy(-1)) / (2 * h)
+        assert abs(fd - out["virial"][a, b]) < 1e-6 * np.abs(out["virial"]).max(), (fd, out["virial"][a, b])
+    assert np.abs(out["forces"].sum(axis=1)).max() < 1e-10
+    assert np.allclose(out["virial_atom"].sum(axis=1).reshape(3, 3), out["virial"], atol=1e-9 * np.abs(out["virial"]).max())
+    # a rotation that maps the cubic box onto itself (x -> y -> z -> x): energy and charges unchanged, forces rotate
+    rot = np.array([[0.0, 0.0, 1.0], [1.0, 0.0, 0.0], [0.0, 1.0, 0.0]])
+    r = oracle.compute(w.model, w.params, w.es, rot @ w.pos, w.types, w.box, use_bins=False)
+    assert abs(r["energy"] - out["energy"]) < 1e-10 and np.abs(r["charges"] - out["charges"]).max() < 1e-12
+    assert np.abs(r["forces"] - rot @ out["forces"]).max() < 1e-10
+    # the extra descriptors carry weight: zeroing their scaler changes the energy
+    off = I.param_offsets(w.model)
+    p0 = w.params.copy()
+    p0[off["scaler"] + 25:off["scaler"] + 35] = 0.0
+    assert abs(oracle.compute(w.model, p0, w.es, w.pos, w.types, w.box, use_bins=False)["energy"] - out["energy"]) > 1e-4
