@@ -59,6 +59,12 @@ typedef struct {
     int32_t mode;         /* 1: U^ES = U^r + U^k + U^s (Eq. 3); 2: U^ES = U^k (Eq. 5)                        */
     double sqrt_eps_inf;  /* Eq. 24, used only by the Born effective charges                                 */
     double q_total;       /* target total charge Q of Eq. 33                                                 */
+    /* NEP4's higher-body angular terms (PAPER.md :39 defers to the NEP papers; reading Z2), one descriptor per
+     * angular radial channel n each, appended behind the 3-body block: 4-body q_n = tr(T_n^3) with the l = 2 moment tensor
+     * T_n = sum_j g_n(r_ij) (rhat rhat^T - 1/3), 5-body q_n = (w_n . w_n)^2 with w_n = sum_j g_n(r_ij) rhat.
+     * THIS VERSION accepts (l_max_4b, l_max_5b) = (0, 0) [off] or (2, 1) [both on]; anything else: UNSUPPORTED.            */
+    int32_t l_max_4b;
+    int32_t l_max_5b;
 } qnep_model_desc;
 
 /* Reciprocal-space method -- the Ewald / PPPM selector (PAPER.md II.B.2 and II.F). */
@@ -107,7 +113,8 @@ enum {
  *   params_host [n_params] float32, order:
  *     c_R[ti][tj][n][k], c_A[ti][tj][n][k], s[n_desc],
  *     then per type: w0[H][n_desc], b0[H], w1U[H], w1q[H]; then b1U, b1q.
- *   n_desc = (n_max_r + 1) + (n_max_a + 1) * l_max.  The vector is copied.
+ *   n_desc = (n_max_r + 1) + (n_max_a + 1) * l_max  [+ 2 (n_max_a + 1) with the 4-/5-body terms: 4-body block, then 5-body
+ *   block].  The vector is copied.
  * Errors: INVALID_ARG (null pointer, wrong n_params, rc_a > rc_r), UNSUPPORTED, CUDA, OOM.
  */
 int qnep_create(const qnep_model_desc *model, const float *params_host, size_t n_params,

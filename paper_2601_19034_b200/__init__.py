@@ -45,7 +45,7 @@ class qnep_model_desc(C.Structure):
     _fields_ = [("n_types", C.c_int32), ("n_max_r", C.c_int32), ("n_max_a", C.c_int32), ("l_max", C.c_int32),
                 ("basis_r", C.c_int32), ("basis_a", C.c_int32), ("n_neurons", C.c_int32),
                 ("rc_r", C.c_double), ("rc_a", C.c_double), ("mode", C.c_int32),
-                ("sqrt_eps_inf", C.c_double), ("q_total", C.c_double)]
+                ("sqrt_eps_inf", C.c_double), ("q_total", C.c_double), ("l_max_4b", C.c_int32), ("l_max_5b", C.c_int32)]
 
 
 class qnep_es_desc(C.Structure):
@@ -126,7 +126,7 @@ def load_library():
 
 def _model_struct(m) -> qnep_model_desc:
     return qnep_model_desc(m.n_types, m.n_max_r, m.n_max_a, m.l_max, m.basis_r, m.basis_a, m.n_neurons,
-                           m.rc_r, m.rc_a, m.mode, m.sqrt_eps_inf, m.q_total)
+                           m.rc_r, m.rc_a, m.mode, m.sqrt_eps_inf, m.q_total, getattr(m, "l_max_4b", 0), getattr(m, "l_max_5b", 0))
 
 
 def _es_struct(e) -> qnep_es_desc:

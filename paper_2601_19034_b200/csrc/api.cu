@@ -126,14 +126,14 @@ int ensure_workspace(qnep_handle* h, int64_t N, const double box[9])
         if ((rc = dev_alloc(h, &h->d_nlvR, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_lvA, npad * capLA))) return rc;
         if ((rc = dev_alloc(h, &h->d_nlvA, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_D, n * QNEP_NDESC))) return rc;
+        if ((rc = dev_alloc(h, &h->d_D, n * h->ND))) return rc;
         if ((rc = dev_alloc(h, &h->d_A, n * QNEP_NRAD * QNEP_NLM))) return rc;
         if ((rc = dev_alloc(h, &h->d_Ui, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_qraw, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_q, n))) return rc;
-        if ((rc = dev_alloc(h, &h->d_FpU, n * QNEP_NDESC))) return rc;
-        if ((rc = dev_alloc(h, &h->d_FpQ, n * QNEP_NDESC))) return rc;
-        if ((rc = dev_alloc(h, &h->d_Fp, n * QNEP_NDESC))) return rc;
+        if ((rc = dev_alloc(h, &h->d_FpU, n * h->ND))) return rc;
+        if ((rc = dev_alloc(h, &h->d_FpQ, n * h->ND))) return rc;
+        if ((rc = dev_alloc(h, &h->d_Fp, n * h->ND))) return rc;
         if ((rc = dev_alloc(h, &h->d_recA, n * T * 8))) return rc;
         if ((rc = dev_alloc(h, &h->d_recB, n * T))) return rc;
         if ((rc = dev_alloc(h, &h->d_lvRend, n * T))) return rc;
@@ -385,7 +385,7 @@ void drop_md_graphs(qnep_handle* h)
 int upload_model(qnep_handle* h)
 {
     const qnep_model_desc& m = h->model;
-    const int T = m.n_types, H = m.n_neurons, D = QNEP_NDESC;
+    const int T = m.n_types, H = m.n_neurons, D = h->ND;
     const float* p = h->h_params.data();
     const size_t ncoef = (size_t)T * T * QNEP_NRAD * QNEP_NB;
     const float* cR = p;
@@ -403,7 +403,8 @@ int upload_model(qnep_handle* h)
                 pA[((size_t)tt * QNEP_NRAD + n) * QNEP_KPAD + k] = cA[((size_t)tt * QNEP_NRAD + n) * QNEP_NB + k];
             }
     // NN per type: w0 * scaler in rows padded to 28, then b0, w1U, w1q
-    const int W0P = 28;
+    const int W0P = (D + 3) / 4 * 4;
+    h->w0p = W0P;
     h->nn_stride = H * W0P + 3 * H;
     h->nn_stride = (h->nn_stride + 3) / 4 * 4;
     std::vector<float> pn((size_t)T * h->nn_stride, 0.f);
@@ -562,7 +563,12 @@ int qnep_create(const qnep_model_desc* model, const float* params_host, size_t n
         h->err = "this version supports n_types <= 4, n_max = 4, l_max = 4, basis = 8, n_neurons <= 256";
         return fail(QNEP_ERR_UNSUPPORTED);
     }
-    const int T = m.n_types, H = m.n_neurons, D = QNEP_NDESC;
+    if (!((m.l_max_4b == 0 && m.l_max_5b == 0) || (m.l_max_4b == 2 && m.l_max_5b == 1))) {
+        h->err = "this version takes the 4-/5-body terms both off (0, 0) or both on (l_max_4b = 2, l_max_5b = 1)";
+        return fail(QNEP_ERR_UNSUPPORTED);
+    }
+    h->ND = m.l_max_4b == 2 ? QNEP_NDESC_HB : QNEP_NDESC;
+    const int T = m.n_types, H = m.n_neurons, D = h->ND;
     const size_t expect = 2 * (size_t)T * T * QNEP_NRAD * QNEP_NB + D + (size_t)T * (H * D + 3 * H) + 2;
     if (n_params != expect) { h->err = "n_params does not match the model description"; return fail(QNEP_ERR_INVALID_ARG); }
     int rc = validate_es(h, es);
@@ -956,16 +962,16 @@ int qnep_debug_copy(qnep_handle* h, int32_t which, double* dst, int64_t n)
     const int nb = (int)((N + 255) / 256);
     auto need = [&](int64_t cnt) { if (n < cnt) { h->err = "debug buffer too small"; return false; } return true; };
     switch (which) {
-        case QNEP_DBG_DESCRIPTORS: if (!need(N * QNEP_NDESC)) return QNEP_ERR_INVALID_ARG;
-            k_dbg_rows<<<nb, 256, 0, s>>>(N, QNEP_NDESC, h->d_D, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_DESCRIPTORS: if (!need(N * h->ND)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, h->ND, h->d_D, h->d_sidx, 1, dst); break;
         case QNEP_DBG_SITE_ENERGY: if (!need(N)) return QNEP_ERR_INVALID_ARG;
             k_dbg_rows<<<nb, 256, 0, s>>>(N, 1, h->d_Ui, h->d_sidx, 1, dst); break;
         case QNEP_DBG_Q_RAW: if (!need(N)) return QNEP_ERR_INVALID_ARG;
             k_dbg_rows<<<nb, 256, 0, s>>>(N, 1, h->d_qraw, h->d_sidx, 1, dst); break;
         case QNEP_DBG_PHI: if (!need(N)) return QNEP_ERR_INVALID_ARG;
             k_dbg_rows<<<nb, 256, 0, s>>>(N, 1, h->d_phi, h->d_sidx, 1, dst); break;
-        case QNEP_DBG_FP: if (!need(N * QNEP_NDESC)) return QNEP_ERR_INVALID_ARG;
-            k_dbg_rows<<<nb, 256, 0, s>>>(N, QNEP_NDESC, h->d_Fp, h->d_sidx, 1, dst); break;
+        case QNEP_DBG_FP: if (!need(N * h->ND)) return QNEP_ERR_INVALID_ARG;
+            k_dbg_rows<<<nb, 256, 0, s>>>(N, h->ND, h->d_Fp, h->d_sidx, 1, dst); break;
         case QNEP_DBG_F_STATIC: if (!need(3 * N)) return QNEP_ERR_INVALID_ARG;
             k_dbg_rows<<<nb, 256, 0, s>>>(N, 3, h->d_Fs, h->d_sidx, 0, dst); break;
         case QNEP_DBG_MESH_RHO:

@@ -421,11 +421,28 @@ __device__ __forceinline__ void harmonics(float x, float y, float z, float* __re
 constexpr int ANG_BLOCK = 64, ANG_DEPTH = 8;
 constexpr int FA_KP2 = 10;     // float2 per row of the packed coefficient table of k_force_angular
 
+// NEP4's higher-body terms of one radial channel (reading Z2) from the real-harmonic sums A_lm, lm = 0..7
+// (b_0..2 = z, x, y; b_3..7 = 3z^2 - 1, xz, yz, x^2 - y^2, 2xy): the l = 1 vector w = sum_j g rhat and the traceless l = 2
+// tensor T = sum_j g (rhat rhat^T - 1/3), stored as (xx, yy, zz, xy, xz, yz); S = T^2.
+__device__ __forceinline__ void hb_moments(const float (&A)[8], float (&Tn)[6], float (&Sn)[6], float& w2)
+{
+    w2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
+    const float zz = A[3] * (1.f / 3.f);
+    Tn[0] = 0.5f * (A[6] - zz); Tn[1] = 0.5f * (-A[6] - zz); Tn[2] = zz;
+    Tn[3] = 0.5f * A[7]; Tn[4] = A[4]; Tn[5] = A[5];
+    Sn[0] = Tn[0] * Tn[0] + Tn[3] * Tn[3] + Tn[4] * Tn[4];
+    Sn[1] = Tn[3] * Tn[3] + Tn[1] * Tn[1] + Tn[5] * Tn[5];
+    Sn[2] = Tn[4] * Tn[4] + Tn[5] * Tn[5] + Tn[2] * Tn[2];
+    Sn[3] = Tn[0] * Tn[3] + Tn[3] * Tn[1] + Tn[4] * Tn[5];
+    Sn[4] = Tn[0] * Tn[4] + Tn[3] * Tn[5] + Tn[4] * Tn[2];
+    Sn[5] = Tn[3] * Tn[4] + Tn[1] * Tn[5] + Tn[5] * Tn[2];
+}
+
 template <int T, bool ZBL>
 __global__ void __launch_bounds__(ANG_BLOCK)
 k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restrict__ lvA, int capLA, const int* __restrict__ nlvA,
                const float* __restrict__ cA, float rcinv, float* __restrict__ D, float* __restrict__ Aout,
-               ZblParams zbl, double* __restrict__ sums)
+               ZblParams zbl, double* __restrict__ sums, int hb /* 4-/5-body terms on: rows 25..34 of D */)
 {
     // g_n = sum_k c_nk f_k = 1/2 fc [ (2 c_n0 + sum_{k>=1} c_nk) + sum_{k>=1} c_nk T_k ]: row (ti, tj, n) of the table holds the
     // bracket's constant in slot 0 and c_n1..c_n8 behind it, so g_n is a dot product with (1, T_1..T_8) in packed FMAs and the
@@ -519,6 +536,15 @@ k_desc_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __restr
         }
 #pragma unroll
         for (int l = 0; l < 4; ++l) D[(int64_t)(NR + a * 4 + l) * N + p] = d[l];
+        if (hb) {
+            float A8[8], Tn[6], Sn[6], w2;
+#pragma unroll
+            for (int lm = 0; lm < 8; ++lm) A8[lm] = (lm & 1) ? A2[a][lm >> 1].y : A2[a][lm >> 1].x;
+            hb_moments(A8, Tn, Sn, w2);
+            // 4-body: tr(T^3) = sum_ab S_ab T_ab;  5-body: (w.w)^2
+            D[(int64_t)(ND + a) * N + p] = Sn[0] * Tn[0] + Sn[1] * Tn[1] + Sn[2] * Tn[2] + 2.f * (Sn[3] * Tn[3] + Sn[4] * Tn[4] + Sn[5] * Tn[5]);
+            D[(int64_t)(ND + NR + a) * N + p] = w2 * w2;
+        }
     }
 }
 
@@ -639,6 +665,68 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
     if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
 }
 
+// One atom per thread, scalar FMAs: the form used when the 4-/5-body terms are on (35 descriptors; two atoms per thread
+// would need 3 x 35 register pairs).
+template <int NDT>
+__global__ void __launch_bounds__(128)
+k_nn1(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, float b1U, float b1q,
+      const float4* __restrict__ xyzt, const float* __restrict__ D, float* __restrict__ Ui, float* __restrict__ qraw,
+      float* __restrict__ FpU, float* __restrict__ FpQ, double* __restrict__ sums)
+{
+    constexpr int WP = (NDT + 3) / 4 * 4;
+    extern __shared__ __align__(16) float sh_w[];
+    __shared__ double sh_red[32];
+    {
+        const float4* src = reinterpret_cast<const float4*>(nnw);
+        float4* dst = reinterpret_cast<float4*>(sh_w);
+        for (int i = threadIdx.x; i < T * nn_stride / 4; i += blockDim.x) dst[i] = src[i];
+    }
+    __syncthreads();
+    double accU = 0.0, accQ = 0.0;
+    for (int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; p < N; p += (int64_t)gridDim.x * blockDim.x) {
+        const int ti = __float_as_int(xyzt[p].w);
+        const float* w = sh_w + ti * nn_stride;
+        const float* b0 = w + H * WP;
+        const float* w1U = b0 + H;
+        const float* w1q = w1U + H;
+        float x[WP], dU[WP], dQ[WP];
+#pragma unroll
+        for (int v = 0; v < WP; ++v) { x[v] = v < NDT ? D[(int64_t)v * N + p] : 0.f; dU[v] = 0.f; dQ[v] = 0.f; }
+        float U = 0.f, q = 0.f;
+        for (int mu = 0; mu < H; ++mu) {
+            const float4* row = reinterpret_cast<const float4*>(w + mu * WP);
+            float wr[WP];
+#pragma unroll
+            for (int v4 = 0; v4 < WP / 4; ++v4) {
+                const float4 t = row[v4];
+                wr[4 * v4] = t.x; wr[4 * v4 + 1] = t.y; wr[4 * v4 + 2] = t.z; wr[4 * v4 + 3] = t.w;
+            }
+            float z0 = -b0[mu], z1 = 0.f;
+#pragma unroll
+            for (int v = 0; v < NDT; v += 2) { z0 = fmaf(wr[v], x[v], z0); if (v + 1 < NDT) z1 = fmaf(wr[v + 1], x[v + 1], z1); }
+            const float hmu = tanh_f32(z0 + z1);
+            const float a = w1U[mu], b = w1q[mu];
+            U = fmaf(a, hmu, U);
+            q = fmaf(b, hmu, q);
+            const float dh = fmaf(-hmu, hmu, 1.f);
+            const float au = a * dh, bq = b * dh;
+#pragma unroll
+            for (int v = 0; v < NDT; ++v) { dU[v] = fmaf(au, wr[v], dU[v]); dQ[v] = fmaf(bq, wr[v], dQ[v]); }
+        }
+        U -= b1U;
+        q -= b1q;
+        Ui[p] = U;
+        qraw[p] = q;
+#pragma unroll
+        for (int v = 0; v < NDT; ++v) { FpU[(int64_t)v * N + p] = dU[v]; FpQ[(int64_t)v * N + p] = dQ[v]; }
+        accU += (double)U;
+        accQ += (double)q;
+    }
+    const double su = block_sum(accU, sh_red);
+    const double sq = block_sum(accQ, sh_red);
+    if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
+}
+
 // a5: Eq. 33 (reading G3): q_i = q_i^raw + (Q - sum_j q_j^raw) / N
 __global__ void k_neutralise(int64_t N, const float* __restrict__ qraw, const double* __restrict__ sums, double Qtot,
                              const int* __restrict__ sidx, const int* __restrict__ cm, float* __restrict__ q,
@@ -673,7 +761,7 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                 const float* __restrict__ cA, const float* __restrict__ cR, float rcinv, const float* __restrict__ FpU,
                 const float* __restrict__ FpQ, const float* __restrict__ phi, float sqrt_eps, const float* __restrict__ Ain,
                 float* __restrict__ Fp, float* __restrict__ recA, float4* __restrict__ recB, float* __restrict__ Facc,
-                double* __restrict__ sums, ZblParams zbl)
+                double* __restrict__ sums, ZblParams zbl, int hb /* 4-/5-body terms on */)
 {
     // Packed angular coefficient table for the loop below: row (ti, tj, n) holds ten float2,
     //   [0] = (2 c_0 + sum_{k>=1} c_k, 0)  and  [k] = (c_k, k c_k), k = 1..8   ([9] is padding),
@@ -750,12 +838,29 @@ k_force_angular(int64_t N, const float4* __restrict__ xyzt, const float4* __rest
                 Fp[v * N + p] = val;
                 fpl[l] = 2.f * val;
             }
+            // higher-body terms (reading Z2): dE/dA_lm for lm = 0..7 from q5 = (w.w)^2 and q4 = tr(T^3), S = T^2:
+            //   d q5 / d A_{0,1,2} = 4 (w.w) A;   d q4 / d A_3..7 = S_zz - (S_xx + S_yy)/2, 6 S_xz, 6 S_yz, 3/2 (S_xx - S_yy), 3 S_xy
+            float extra[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            if (hb) {
+                const int64_t v4 = ND + a, v5 = ND + NR + a;
+                const float f4 = cu * FpU[v4 * N + p] + cq * FpQ[v4 * N + p], f5 = cu * FpU[v5 * N + p] + cq * FpQ[v5 * N + p];
+                Fp[v4 * N + p] = f4; Fp[v5 * N + p] = f5;
+                float A8[8], Tn[6], Sn[6], w2;
+#pragma unroll
+                for (int lm = 0; lm < 8; ++lm) A8[lm] = Ain[(int64_t)(a * NLM + lm) * N + p];
+                hb_moments(A8, Tn, Sn, w2);
+                const float c5 = 4.f * w2 * f5;
+                extra[0] = c5 * A8[0]; extra[1] = c5 * A8[1]; extra[2] = c5 * A8[2];
+                extra[3] = f4 * (Sn[2] - 0.5f * (Sn[0] + Sn[1]));
+                extra[4] = 6.f * f4 * Sn[4]; extra[5] = 6.f * f4 * Sn[5];
+                extra[6] = 1.5f * f4 * (Sn[0] - Sn[1]); extra[7] = 3.f * f4 * Sn[3];
+            }
 #pragma unroll
             for (int m = 0; m < NLM / 2; ++m) {
                 constexpr int pa[NLM / 2] = {0, 8, 1, 6, 13, 22, 4, 9, 11, 16, 18, 20};
                 constexpr int pb[NLM / 2] = {3, 15, 2, 7, 14, 23, 5, 10, 12, 17, 19, 21};
-                Q2[a][m] = make_float2(c_Clm[pa[m]] * fpl[l_of_lm(pa[m])] * Ain[(int64_t)(a * NLM + pa[m]) * N + p],
-                                       c_Clm[pb[m]] * fpl[l_of_lm(pb[m])] * Ain[(int64_t)(a * NLM + pb[m]) * N + p]);
+                Q2[a][m] = make_float2(c_Clm[pa[m]] * fpl[l_of_lm(pa[m])] * Ain[(int64_t)(a * NLM + pa[m]) * N + p] + (pa[m] < 8 ? extra[pa[m]] : 0.f),
+                                       c_Clm[pb[m]] * fpl[l_of_lm(pb[m])] * Ain[(int64_t)(a * NLM + pb[m]) * N + p] + (pb[m] < 8 ? extra[pb[m]] : 0.f));
             }
         }
         float Fx = 0.f, Fy = 0.f, Fz = 0.f;
@@ -1192,8 +1297,8 @@ int qnep_launch_desc_angular(qnep_handle* h, cudaStream_t s)
     const float rcinv = (float)(1.0 / h->model.rc_a);
     dispatch_T(h->model.n_types, [&](auto t) {
         constexpr int T = decltype(t)::value;
-        if (h->zbl.on) k_desc_angular<T, true><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A, h->zbl, h->d_sums);
-        else k_desc_angular<T, false><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A, h->zbl, h->d_sums);
+        if (h->zbl.on) k_desc_angular<T, true><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A, h->zbl, h->d_sums, h->ND == QNEP_NDESC_HB ? 1 : 0);
+        else k_desc_angular<T, false><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, rcinv, h->d_D, h->d_A, h->zbl, h->d_sums, h->ND == QNEP_NDESC_HB ? 1 : 0);
     });
     h->launches += 1;
     QNEP_CUDA_OK(h, cudaGetLastError());
@@ -1212,8 +1317,16 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
         QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
-    k_nn<<<nb, NN_BLOCK, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
-                               h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
+    if (h->ND == QNEP_NDESC) {
+        k_nn<<<nb, NN_BLOCK, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
+                                        h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
+    } else {
+        static bool attr1 = false;
+        if (!attr1) { QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn1<QNEP_NDESC_HB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr1 = true; }
+        const int nb1 = (int)std::min<int64_t>((N + 127) / 128, (int64_t)sms * 3);
+        k_nn1<QNEP_NDESC_HB><<<nb1, 128, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
+                                                    h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
+    }
     const int nb2 = (int)((N + 255) / 256);
     k_neutralise<<<nb2, 256, 0, s>>>(N, h->d_qraw, h->d_sums, h->model.q_total, h->d_sidx, h->d_cm, h->d_q, h->d_qcm, charges_out);
     h->launches += 2;
@@ -1231,7 +1344,7 @@ int qnep_launch_force_angular(qnep_handle* h, bool bec, bool virial, bool atomv,
         constexpr int T = decltype(t)::value;
 #define QNEP_FA(B, V, A, Z) k_force_angular<T, B, V, A, Z><<<nb, ANG_BLOCK, 0, s>>>(N, h->d_xyzt, h->d_lvA, h->capLA, h->d_nlvA, h->d_cA, h->d_cR, rcinv, \
                                                                                      h->d_FpU, h->d_FpQ, h->d_phi, (float)h->model.sqrt_eps_inf, \
-                                                                                     h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums, h->zbl)
+                                                                                     h->d_A, h->d_Fp, h->d_recA, h->d_recB, h->d_Facc, h->d_sums, h->zbl, h->ND == QNEP_NDESC_HB ? 1 : 0)
         const bool zb = h->zbl.on != 0;
         if (bec) QNEP_FA(true, false, false, false);                 // the Born effective charges do not see the ZBL core
         else if (atomv) { if (zb) QNEP_FA(false, true, true, true); else QNEP_FA(false, true, true, false); }

@@ -17,7 +17,8 @@
 #define QNEP_KPAD 12                // Chebyshev coefficient rows padded from 9 to 12 floats (3 x float4)
 #define QNEP_NB 9                   // basis functions k = 0..8 (basis_r = basis_a = 8 in this version)
 #define QNEP_NRAD 5                 // n = 0..4
-#define QNEP_NDESC 25
+#define QNEP_NDESC 25               // radial + 3-body angular descriptors
+#define QNEP_NDESC_HB 35            // with NEP4's 4- and 5-body terms (rows 25..29 and 30..34)
 #define QNEP_GRAPH_MAX_ATOMS 100000   // above this the step is not launch-bound and keeps its per-stage events
 // PPPM mesh bins of the sweep kernel (pppm_sweep.cu): bin edge in mesh points along x, y, z
 #define QNEP_MB_X 4
@@ -144,6 +145,8 @@ struct qnep_handle {
     float* d_cA = nullptr;           // [T*T][5][KPAD]
     float* d_nn = nullptr;           // per type: w0[H][28] (scaler folded in? no: raw), b0[H], w1U[H], w1q[H]
     int nn_stride = 0;               // floats per type in d_nn
+    int ND = QNEP_NDESC;             // descriptors per atom: 25, or 35 with the 4-/5-body terms
+    int w0p = 28;                    // padded row length of w0 in d_nn (ND rounded up to a multiple of 4)
     float b1U = 0.f, b1q = 0.f;
     std::vector<float> h_params;
 

@@ -30,9 +30,10 @@ def test_header_symbols_are_exported(lib):
 
 def test_struct_layout_matches_header():
     # the ctypes mirrors must have the C layout (8-byte aligned doubles)
-    assert C.sizeof(Q.qnep_model_desc) == 72
+    assert C.sizeof(Q.qnep_model_desc) == 80          # 72 bytes of round 1 + l_max_4b, l_max_5b
     assert C.sizeof(Q.qnep_es_desc) == 40
     assert Q.qnep_model_desc.rc_r.offset == 32 and Q.qnep_model_desc.sqrt_eps_inf.offset == 56
+    assert Q.qnep_model_desc.l_max_4b.offset == 72 and Q.qnep_model_desc.l_max_5b.offset == 76
     assert Q.qnep_es_desc.alpha.offset == 8 and Q.qnep_es_desc.grid.offset == 20
 
 

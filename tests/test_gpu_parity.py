@@ -322,6 +322,54 @@ def test_zbl_parity(torch, oracle, case):
     assert exc.value.code == Q.QNEP_ERR_INVALID_ARG
 
 
+# ---------------------------------------------------------------- NEP4 4-/5-body terms (reading Z2)
+@pytest.mark.parametrize("case", ["config0_ewald_mode1", "config1_pppm", "config2_pppm", "config1_triclinic_zbl"])
+def test_higher_body_terms_parity(torch, oracle, case):
+    """Models with the 4-/5-body angular terms on (35 descriptors): stage parity of the descriptors (the ten new rows
+    separately), site energies, Fp; all outputs incl. BEC and per-atom virial; the last case combines them with a
+    triclinic cell and the ZBL core.  Models that ask for only one of the two terms are refused."""
+    bins = True
+    if case == "config0_ewald_mode1":
+        w = I.with_higher_body_terms(I.config0(mode=1), "config0_45body")
+        bins = False
+    elif case == "config1_pppm":
+        w = I.with_higher_body_terms(I.config1(), "config1_45body")
+    elif case == "config2_pppm":
+        w = I.with_higher_body_terms(I.config2(), "config2_45body")
+    else:
+        w = I.triclinic_variant(I.with_higher_body_terms(I.config1(), "config1_45body"))
+        w.zbl = (0.5, 1.0, (8.0, 1.0))
+    assert w.model.n_desc == 35
+    ref = oracle.compute_workload(w, use_bins=bins, debug=True, want_atom_virial=True, want_bec=True)
+    h = Q.from_workload(w)
+    pos = torch.tensor(w.pos, dtype=torch.float64, device="cuda")
+    types = torch.tensor(w.types, dtype=torch.int32, device="cuda")
+    try:
+        out = h.compute_atom_virial(pos, types, w.box)
+    except Q.QnepError as err:
+        if err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
+            raise
+        out = h.compute_atom_virial(pos, types, w.box)
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    assert_parity(w, res, ref, f"4-/5-body, {case}")
+    assert rel_rms(res["virial_atom"], ref["virial_atom"]) <= 1e-4
+    n, D = w.n_atoms, 35
+    Dg = h.debug_copy(Q.DBG_DESCRIPTORS, (n, D)).cpu().numpy()
+    for lo, hi in ((0, 25), (25, 30), (30, 35)):
+        assert np.abs(Dg[:, lo:hi] - ref["D"][:, lo:hi]).max() <= 3e-5 * np.abs(ref["D"][:, lo:hi]).max(), (lo, hi)
+    assert np.abs(ref["D"][:, 25:30]).max() > 1e-3 and np.abs(ref["D"][:, 30:35]).max() > 1e-3
+    assert np.abs(h.debug_copy(Q.DBG_SITE_ENERGY, (n,)).cpu().numpy() - ref["U_i"]).max() < 1e-5
+    assert rel_rms(h.debug_copy(Q.DBG_FP, (n, D)).cpu().numpy(), ref["Fp"]) < 1e-4
+    _, full = gpu_eval(torch, w, handle=h, want=Q.WANT_ALL | Q.WANT_BEC)
+    assert_parity(w, full, ref, f"4-/5-body, plain call, {case}")
+    assert rel_rms(full["bec"], ref["bec"]) <= 1e-4
+    if case == "config1_pppm":
+        from dataclasses import replace as rep
+        with pytest.raises(Q.QnepError) as exc:
+            Q.QNEP(rep(w.model, l_max_5b=0), I.random_params(rep(w.model, l_max_5b=0), 3), w.es)
+        assert exc.value.code == Q.QNEP_ERR_UNSUPPORTED
+
+
 # ---------------------------------------------------------------- triclinic cells (PAPER.md :104; SURVEY 8(f) row 3)
 @pytest.mark.parametrize("case", ["config0_ewald_mode1", "config0_ewald_mode2", "config1_no_es", "config1_pppm", "config1_pppm_mode1",
                                   "config1_mesh16", "config2_pppm", "config1_sheared_box"])
