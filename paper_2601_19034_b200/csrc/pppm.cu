@@ -218,8 +218,14 @@ k_fft_z_fwd_half(const float* __restrict__ rho, float2* __restrict__ out, const 
 }
 
 // ---- in-place pass along a strided axis (y): grid.y selects the mesh --------------------------------
+#ifndef QNEP_FFT_STRIDED_MINB
+#define QNEP_FFT_STRIDED_MINB 3       // three blocks of 256 threads per SM: 0.855 -> 0.812 ms per reciprocal stage (1, 2, 4, 5 are slower)
+#endif
+#ifndef QNEP_FFT_ZF_MINB
+#define QNEP_FFT_ZF_MINB 3
+#endif
 template <int R1, int R2, int SIGN>
-__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS, Split<R1, R2>::THREADS >= 256 ? QNEP_FFT_STRIDED_MINB : 1)
 k_fft_strided(int axis, int n0, int n1, int n2, float2* __restrict__ mesh_a, float2* __restrict__ mesh_b,
               const float2* __restrict__ twg)
 {
@@ -586,7 +592,7 @@ k_fft_x_virial(int n0, int n1, int n2, float2* __restrict__ M1, float2* __restri
 
 // ---- last inverse pass along z: M1, M2 -> interleaved real fields (Phi, E_x, E_y, E_z) -------------------
 template <int R1, int R2>
-__global__ void __launch_bounds__(Split<R1, R2>::THREADS)
+__global__ void __launch_bounds__(Split<R1, R2>::THREADS, Split<R1, R2>::THREADS >= 256 ? QNEP_FFT_ZF_MINB : 1)
 k_fft_z_fields(const float2* __restrict__ M1, const float2* __restrict__ M2, float4* __restrict__ field,
                const float2* __restrict__ twg)
 {
