@@ -230,6 +230,16 @@ int qnep_set_md_graphs(qnep_handle *h, int32_t mode);
 int qnep_set_pppm_kernels(qnep_handle *h, int32_t mode);
 
 /*
+ * Kernel of the batched network contraction (the one stage where the north_star allows tensor cores).
+ * mode 0 (default): packed FP32 FMAs, two atoms per thread.  mode 1: warp-level tensor-core MMA (m16n8k8 TF32) with the
+ * 3xTF32 split (three products per term), which keeps FP32-level accuracy: site energies agree with mode 0 to ~1e-6 eV and
+ * the stated tolerances hold (tests/test_gpu_parity.py::test_nn_tensor_core_kernel).  Measured on config 4: 0.338 ms against
+ * 0.310 ms for mode 0 (the legacy mma.sync path peaks at 277 TFLOP/s TF32 on B200 and the split triples the products), so
+ * FP32 stays the default.  Errors: INVALID_ARG, UNSUPPORTED (mode 1 with the 4-/5-body terms on).
+ */
+int qnep_set_nn_kernel(qnep_handle *h, int32_t mode);
+
+/*
  * Optional ZBL core repulsion (the paper defers to the NEP papers for it, PAPER.md :39; DESIGN.md
  * reading Z1).  enabled != 0 adds to every pair closer than r_outer the universal Ziegler-Biersack-Littmark potential
  *     U(r) = K Z_i Z_j / r * phi(r / a) * f_sw(r),   a = 0.46850 / (Z_i^0.23 + Z_j^0.23) Angstrom,

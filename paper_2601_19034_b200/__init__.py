@@ -37,7 +37,7 @@ DBG_DESCRIPTORS, DBG_SITE_ENERGY, DBG_Q_RAW, DBG_PHI, DBG_FP, DBG_MESH_RHO, DBG_
 ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_policy", "qnep_set_neighbor_capacity",
                "qnep_compute", "qnep_compute_atom_virial", "qnep_compute_host", "qnep_md_run", "qnep_md_set_outputs", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
-               "qnep_fma_peak", "qnep_set_zbl",
+               "qnep_fma_peak", "qnep_set_zbl", "qnep_set_nn_kernel",
                "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
 
 
@@ -110,6 +110,8 @@ def load_library():
     lib.qnep_response.argtypes = [vp, i64, vp, C.POINTER(dbl), vp, vp, vp, vp]
     lib.qnep_neighbor_stats.restype = C.c_int
     lib.qnep_neighbor_stats.argtypes = [vp, C.POINTER(dbl)]
+    lib.qnep_set_nn_kernel.restype = C.c_int
+    lib.qnep_set_nn_kernel.argtypes = [vp, i32]
     lib.qnep_set_zbl.restype = C.c_int
     lib.qnep_set_zbl.argtypes = [vp, i32, dbl, dbl, C.POINTER(dbl)]
     lib.qnep_fma_peak.restype = C.c_int
@@ -316,6 +318,10 @@ class QNEP:
     def set_pppm_kernels(self, mode: int):
         """0 automatic, 1 one thread per atom, 2 shared-memory sweep kernel: PPPM charge assignment."""
         self._ok(self._lib.qnep_set_pppm_kernels(self._h, int(mode)))
+
+    def set_nn_kernel(self, mode: int):
+        """0: packed FP32 FMAs (default); 1: tensor cores (mma.sync TF32, 3xTF32 split)."""
+        self._ok(self._lib.qnep_set_nn_kernel(self._h, int(mode)))
 
     def set_zbl(self, zbl):
         """zbl = (r_inner, r_outer, Z per species) switches the ZBL core on, None switches it off."""

@@ -704,6 +704,17 @@ int qnep_set_pppm_kernels(qnep_handle* h, int32_t mode)
     return QNEP_OK;
 }
 
+int qnep_set_nn_kernel(qnep_handle* h, int32_t mode)
+{
+    if (!h) return QNEP_ERR_INVALID_ARG;
+    if (mode != 0 && mode != 1) { h->err = "qnep_set_nn_kernel: mode must be 0 (FP32 FMA) or 1 (tensor cores)"; return QNEP_ERR_INVALID_ARG; }
+    if (mode == 1 && h->ND != QNEP_NDESC) { h->err = "qnep_set_nn_kernel: the tensor-core kernel takes the 25-descriptor model only"; return QNEP_ERR_UNSUPPORTED; }
+    h->nn_tensor = mode;
+    h->ws_generation += 1;      // captured MD graphs hold the old kernel
+    h->md_have_forces = false;
+    return QNEP_OK;
+}
+
 int qnep_set_zbl(qnep_handle* h, int32_t enabled, double r_inner, double r_outer, const double* z_host)
 {
     if (!h) return QNEP_ERR_INVALID_ARG;

@@ -665,6 +665,192 @@ k_nn(int64_t N, int T, int H, int nn_stride, const float* __restrict__ nnw, floa
     if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
 }
 
+// ------------------------------------------------------------------------------------------
+// a4 on the tensor cores (the one stage where the north_star allows them): the batched contraction
+//   Z[atoms x H] = X[atoms x 25] W0^T,   dU/dD[atoms x 25] = (w1U (1 - h^2))[atoms x H] W0,   dq/dD likewise
+// as warp-level mma.sync m16n8k8 TF32 with the 3xTF32 split (x = hi + lo, three products per term: the error of a product is
+// ~2^-21 relative, the level of the FP32 form, so the 1e-5 eV/atom energy tolerance holds -- measured in the parity tests).
+// A warp owns 32 atoms (two m16 tiles).  Per block of eight neurons: 24 mma give z, the activation and the two output
+// sums run on the accumulator fragment, and that fragment IS the A operand of the backward products for these eight
+// neurons (accumulator element (row, col 2t / 2t+1) = A element (row, k = t / t+4) once the neurons of the block are
+// taken in the order 0 2 4 6 1 3 5 7, which the B operand read from shared memory follows): no data movement.
+// Weights are split into hi / lo once per block, rows padded to 36 floats (conflict-free fragment reads).
+// ------------------------------------------------------------------------------------------
+constexpr int NNM_LD = 36;            // padded row of the split weight tables
+constexpr int NNM_K = 32;             // descriptors padded to four k-steps of eight
+
+__device__ __forceinline__ unsigned tf32_hi(float x) { unsigned r; asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x)); return r; }
+__device__ __forceinline__ void tf32_split(float x, unsigned& hi, unsigned& lo)
+{
+    hi = tf32_hi(x);
+    lo = tf32_hi(x - __uint_as_float(hi));
+}
+__device__ __forceinline__ void mma_tf32(float (&c)[4], const unsigned (&a)[4], unsigned b0, unsigned b1)
+{
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+__global__ void __launch_bounds__(128, 2)      // 242 registers; 1, 3 and 4 blocks per SM are slower (0.44 / 0.39 / 0.45 ms)
+k_nn_mma(int64_t N, int T, int H, int HP /* H rounded up to 8 */, int nn_stride, const float* __restrict__ nnw, float b1U, float b1q,
+         const float4* __restrict__ xyzt, const float* __restrict__ D, float* __restrict__ Ui, float* __restrict__ qraw,
+         float* __restrict__ FpU, float* __restrict__ FpQ, double* __restrict__ sums)
+{
+    extern __shared__ __align__(16) float sh_nn[];
+    // per type: Wh[HP][NNM_LD], Wl[HP][NNM_LD], b0[HP], w1U[HP], w1q[HP]
+    const int tstride = 2 * HP * NNM_LD + 3 * HP;
+    __shared__ double sh_red[32];
+    for (int i = threadIdx.x; i < T * tstride; i += blockDim.x) sh_nn[i] = 0.f;
+    __syncthreads();
+    for (int t = 0; t < T; ++t) {
+        const float* w = nnw + (size_t)t * nn_stride;            // w0s[H][W0P], b0[H], w1U[H], w1q[H]
+        float* dst = sh_nn + t * tstride;
+        for (int i = threadIdx.x; i < H * ND; i += blockDim.x) {
+            const int mu = i / ND, v = i - mu * ND;
+            unsigned hi, lo;
+            tf32_split(w[mu * W0P + v], hi, lo);
+            dst[mu * NNM_LD + v] = __uint_as_float(hi);
+            dst[HP * NNM_LD + mu * NNM_LD + v] = __uint_as_float(lo);
+        }
+        for (int i = threadIdx.x; i < 3 * H; i += blockDim.x) dst[2 * HP * NNM_LD + (i / H) * HP + (i % H)] = w[H * W0P + i];
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int g = lane >> 2, t4 = lane & 3;
+    double accU = 0.0, accQ = 0.0;
+    const int64_t nwtile = (N + 31) / 32;
+    for (int64_t wt = (int64_t)blockIdx.x * 4 + wib; wt < nwtile; wt += (int64_t)gridDim.x * 4) {
+        const int64_t a0 = wt * 32;
+        // rows of this lane: r = 0..3 -> atom a0 + g + 8 r  (m-tile r / 2, fragment row g + 8 (r & 1))
+        int64_t atom[4];
+        int typ[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            atom[r] = min(a0 + g + 8 * r, N - 1);
+            typ[r] = __float_as_int(xyzt[atom[r]].w);
+        }
+        // X fragments, split: xa[m][ks][4]
+        unsigned xh[2][4][4], xl[2][4][4];
+#pragma unroll
+        for (int m = 0; m < 2; ++m)
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int v = 8 * ks + t4 + 4 * (e >> 1);
+                    const float x = v < ND ? D[(int64_t)v * N + atom[2 * m + (e & 1)]] : 0.f;
+                    tf32_split(x, xh[m][ks][e], xl[m][ks][e]);
+                }
+        // which species does the warp hold?  (one, except at a species boundary of the sorted order)
+        unsigned present = 0;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) present |= 1u << typ[r];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) present |= __shfl_xor_sync(0xffffffffu, present, o);
+        for (int ty = 0; ty < T; ++ty) {
+            if (!((present >> ty) & 1u)) continue;
+            const float* Wh = sh_nn + ty * tstride;
+            const float* Wl = Wh + HP * NNM_LD;
+            const float* b0 = Wl + HP * NNM_LD;
+            const float* w1U = b0 + HP;
+            const float* w1q = w1U + HP;
+            float dU[2][4][4], dQ[2][4][4], U[4] = {0.f, 0.f, 0.f, 0.f}, q[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int m = 0; m < 2; ++m)
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) { dU[m][nt][e] = 0.f; dQ[m][nt][e] = 0.f; }
+            for (int j = 0; j < HP / 8; ++j) {
+                // forward: z[m] = X W0^T for neurons 8 j .. 8 j + 7 (B element (k, n) = w0[8 j + n][k])
+                // (three accumulators per tile: the mma latency is ~30 cycles and only two warps share a scheduler)
+                float z[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+                float zb[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, zc[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+                for (int ks = 0; ks < 4; ++ks) {
+                    const int o0 = (8 * j + g) * NNM_LD + 8 * ks + t4;
+                    const unsigned bh0 = __float_as_uint(Wh[o0]), bh1 = __float_as_uint(Wh[o0 + 4]);
+                    const unsigned bl0 = __float_as_uint(Wl[o0]), bl1 = __float_as_uint(Wl[o0 + 4]);
+#pragma unroll
+                    for (int m = 0; m < 2; ++m) {
+                        mma_tf32(zb[m], xl[m][ks], bh0, bh1);
+                        mma_tf32(zc[m], xh[m][ks], bl0, bl1);
+                        mma_tf32(z[m], xh[m][ks], bh0, bh1);
+                    }
+                }
+#pragma unroll
+                for (int m = 0; m < 2; ++m)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) z[m][e] += zb[m][e] + zc[m][e];
+                // activation on the accumulator fragment: element e of tile m = (row g + 8 (e >> 1), neuron 8 j + 2 t4 + (e & 1))
+                unsigned auh[2][4], aul[2][4], bqh[2][4], bql[2][4];
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const int mu = 8 * j + 2 * t4 + c;
+                    const float bb = b0[mu], aU = w1U[mu], aQ = w1q[mu];
+#pragma unroll
+                    for (int m = 0; m < 2; ++m)
+#pragma unroll
+                        for (int rr = 0; rr < 2; ++rr) {
+                            const float hmu = tanh_f32(z[m][2 * rr + c] - bb);
+                            U[2 * m + rr] = fmaf(aU, hmu, U[2 * m + rr]);
+                            q[2 * m + rr] = fmaf(aQ, hmu, q[2 * m + rr]);
+                            const float dh = fmaf(-hmu, hmu, 1.f);
+                            // A fragment of the backward product: (row g + 8 rr, k = t4 + 4 c)  ->  register rr + 2 c
+                            tf32_split(aU * dh, auh[m][rr + 2 * c], aul[m][rr + 2 * c]);
+                            tf32_split(aQ * dh, bqh[m][rr + 2 * c], bql[m][rr + 2 * c]);
+                        }
+                }
+                // backward: dU += AU W0, dQ += BQ W0 over these eight neurons (B element (k, n) = w0[8 j + pi(k)][8 nt + n],
+                // pi(k) = 2 k for k < 4, 2 (k - 4) + 1 else: the order the accumulator fragment holds them in)
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) {
+                    const int o0 = (8 * j + 2 * t4) * NNM_LD + 8 * nt + g;
+                    const unsigned bh0 = __float_as_uint(Wh[o0]), bh1 = __float_as_uint(Wh[o0 + NNM_LD]);
+                    const unsigned bl0 = __float_as_uint(Wl[o0]), bl1 = __float_as_uint(Wl[o0 + NNM_LD]);
+#pragma unroll
+                    for (int m = 0; m < 2; ++m) {
+                        mma_tf32(dU[m][nt], aul[m], bh0, bh1);
+                        mma_tf32(dU[m][nt], auh[m], bl0, bl1);
+                        mma_tf32(dU[m][nt], auh[m], bh0, bh1);
+                        mma_tf32(dQ[m][nt], bql[m], bh0, bh1);
+                        mma_tf32(dQ[m][nt], bqh[m], bl0, bl1);
+                        mma_tf32(dQ[m][nt], bqh[m], bh0, bh1);
+                    }
+                }
+            }
+            // the two output sums: a lane holds two of the eight neurons of every block, the quad holds all
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                U[r] += __shfl_xor_sync(0xffffffffu, U[r], 1); U[r] += __shfl_xor_sync(0xffffffffu, U[r], 2);
+                q[r] += __shfl_xor_sync(0xffffffffu, q[r], 1); q[r] += __shfl_xor_sync(0xffffffffu, q[r], 2);
+            }
+            // outputs of the rows of this species: accumulator element (row r, descriptor 8 nt + 2 t4 + c)
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int64_t p = a0 + g + 8 * r;
+                if (p < N && typ[r] == ty) {
+                    const float Uv = U[r] - b1U, qv = q[r] - b1q;
+                    if (t4 == 0) { Ui[p] = Uv; qraw[p] = qv; accU += (double)Uv; accQ += (double)qv; }
+#pragma unroll
+                    for (int nt = 0; nt < 4; ++nt)
+#pragma unroll
+                        for (int c = 0; c < 2; ++c) {
+                            const int v = 8 * nt + 2 * t4 + c;
+                            if (v < ND) {
+                                FpU[(int64_t)v * N + p] = dU[r >> 1][nt][2 * (r & 1) + c];
+                                FpQ[(int64_t)v * N + p] = dQ[r >> 1][nt][2 * (r & 1) + c];
+                            }
+                        }
+                }
+            }
+        }
+    }
+    const double su = block_sum(accU, sh_red);
+    const double sq = block_sum(accQ, sh_red);
+    if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
+}
+
 // One atom per thread, scalar FMAs: the form used when the 4-/5-body terms are on (35 descriptors; two atoms per thread
 // would need 3 x 35 register pairs).
 template <int NDT>
@@ -1318,7 +1504,15 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
         QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
-    if (h->ND == QNEP_NDESC) {
+    if (h->ND == QNEP_NDESC && h->nn_tensor) {
+        const int HP = (h->model.n_neurons + 7) / 8 * 8;
+        const size_t smem_t = sizeof(float) * (size_t)h->model.n_types * (2 * HP * NNM_LD + 3 * HP);
+        static bool attr_t = false;
+        if (!attr_t) { QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn_mma, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr_t = true; }
+        const int nbt = (int)std::min<int64_t>((N + 127) / 128, (int64_t)sms * 2);
+        k_nn_mma<<<nbt, 128, smem_t, s>>>(N, h->model.n_types, h->model.n_neurons, HP, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
+                                          h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
+    } else if (h->ND == QNEP_NDESC) {
         k_nn<<<nb, NN_BLOCK, smem, s>>>(N, h->model.n_types, h->model.n_neurons, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_xyzt,
                                         h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums);
     } else {

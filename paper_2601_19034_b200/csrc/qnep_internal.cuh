@@ -145,6 +145,7 @@ struct qnep_handle {
     float* d_cA = nullptr;           // [T*T][5][KPAD]
     float* d_nn = nullptr;           // per type: w0[H][28] (scaler folded in? no: raw), b0[H], w1U[H], w1q[H]
     int nn_stride = 0;               // floats per type in d_nn
+    int nn_tensor = 0;               // qnep_set_nn_kernel: 1 = k_nn_mma (tensor cores, 3xTF32) instead of the packed FP32 kernel
     int ND = QNEP_NDESC;             // descriptors per atom: 25, or 35 with the 4-/5-body terms
     int w0p = 28;                    // padded row length of w0 in d_nn (ND rounded up to a multiple of 4)
     float b1U = 0.f, b1q = 0.f;
