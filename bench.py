@@ -204,6 +204,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--zbl", type=float, nargs=2, default=None, metavar=("R_INNER", "R_OUTER"),
                     help="switch the ZBL core on (water: Z = 8, 1); off by default: BASELINE.json's config has none")
+    ap.add_argument("--nn-kernel", type=int, default=-1, help="qnep_set_nn_kernel: 0 packed FP32, 1 mma.sync 3xTF32, 2 tcgen05 3xTF32 (-1: the library's default)")
     ap.add_argument("--pppm-kernels", type=int, default=0, help="qnep_set_pppm_kernels: 0 automatic, 1 per-atom spread, 2 sweep spread")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -232,6 +233,8 @@ def main():
     h = Q.from_workload(w)
     h.set_neighbor_policy(args.skin, args.rebuild_every)
     h.set_pppm_kernels(args.pppm_kernels)
+    if args.nn_kernel >= 0:
+        h.set_nn_kernel(args.nn_kernel)
     masses = w.masses if w.masses is not None else np.ones(w.model.n_types)
     pos0 = torch.tensor(w.pos, dtype=torch.float64, device=dev)
     types = torch.tensor(w.types, dtype=torch.int32, device=dev)
@@ -405,6 +408,8 @@ def main():
     h2 = Q.from_workload(w)
     h2.set_neighbor_policy(args.skin, n_frames)      # the frames repeat after n_frames calls: rebuild there
     h2.set_pppm_kernels(args.pppm_kernels)
+    if args.nn_kernel >= 0:
+        h2.set_nn_kernel(args.nn_kernel)
 
     def e2e_step(k):
         h2.compute_host_raw(n, frames[k % n_frames].data_ptr(), ht.data_ptr(), box9, want, he.data_ptr(), hf.data_ptr(),

@@ -207,9 +207,13 @@ int consume_flags(qnep_handle* h)
     const int* f = h->h_flags;
     // the device flags are sticky (a rebuild inside qnep_md_run must not erase a violation seen earlier in the
     // run): they are cleared here, on the error path only, once the host has read them
-    if (f[FLAG_MAX_NR] || f[FLAG_MAX_LR] || f[FLAG_MAX_LA] || f[FLAG_SKIN] || f[FLAG_BAD_TYPE]) {
+    if (f[FLAG_MAX_NR] || f[FLAG_MAX_LR] || f[FLAG_MAX_LA] || f[FLAG_SKIN] || f[FLAG_BAD_TYPE] || f[FLAG_TENSOR_TIMEOUT]) {
         cudaMemsetAsync(h->d_flags, 0, sizeof(int) * FLAG_COUNT, h->last_stream);
         cudaStreamSynchronize(h->last_stream);
+    }
+    if (f[FLAG_TENSOR_TIMEOUT]) {
+        h->err = "k_nn_umma: a tensor-core operation did not complete";
+        return QNEP_ERR_CUDA;
     }
     if (f[FLAG_BAD_TYPE]) {
         h->err = "types_dev holds a species index outside 0..n_types-1";
@@ -707,8 +711,9 @@ int qnep_set_pppm_kernels(qnep_handle* h, int32_t mode)
 int qnep_set_nn_kernel(qnep_handle* h, int32_t mode)
 {
     if (!h) return QNEP_ERR_INVALID_ARG;
-    if (mode != 0 && mode != 1) { h->err = "qnep_set_nn_kernel: mode must be 0 (FP32 FMA) or 1 (tensor cores)"; return QNEP_ERR_INVALID_ARG; }
-    if (mode == 1 && h->ND != QNEP_NDESC) { h->err = "qnep_set_nn_kernel: the tensor-core kernel takes the 25-descriptor model only"; return QNEP_ERR_UNSUPPORTED; }
+    if (mode < 0 || mode > 2) { h->err = "qnep_set_nn_kernel: mode must be 0 (FP32 FMA), 1 (mma.sync) or 2 (tcgen05)"; return QNEP_ERR_INVALID_ARG; }
+    if (mode == 2 && h->model.n_neurons > 128) { h->err = "qnep_set_nn_kernel: the tcgen05 kernel takes at most 128 hidden neurons"; return QNEP_ERR_UNSUPPORTED; }
+    if (mode != 0 && h->ND != QNEP_NDESC) { h->err = "qnep_set_nn_kernel: the tensor-core kernel takes the 25-descriptor model only"; return QNEP_ERR_UNSUPPORTED; }
     h->nn_tensor = mode;
     h->ws_generation += 1;      // captured MD graphs hold the old kernel
     h->md_have_forces = false;

@@ -851,6 +851,243 @@ k_nn_mma(int64_t N, int T, int H, int HP /* H rounded up to 8 */, int nn_stride,
     if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
 }
 
+// ------------------------------------------------------------------------------------------
+// a4 on the 5th-generation tensor cores: tcgen05.mma kind::tf32 with accumulators AND the A operands in tensor memory.
+// A block of 128 threads owns 128 atoms of ONE species (tiles are cut per species range of the sorted order); thread r is
+// row r of every matrix, i.e. TMEM lane r:
+//   1. x (25 descriptors, padded to 32) is split into TF32 hi / lo and written to TMEM columns with tcgen05.st;
+//   2. one thread issues Z = X W0^T as 3 x 4 MMAs (M = 128, N = HP neurons, K = 8; A from TMEM, B = the split weights in
+//      shared memory, K-major canonical layout without swizzle), commits to an mbarrier;
+//   3. per chunk of 16 neurons every thread reads its 16 z values (tcgen05.ld), applies the activation, adds to its U and q,
+//      splits a (1 - h^2) for both outputs into hi / lo and stores them to TMEM as the A operand of the backward products
+//      dU/dD += AU W0, dq/dD += BQ W0 (N = 32 descriptors, K = 16), issued by one thread;
+//   4. dU/dD, dq/dD come back with tcgen05.ld, one row per thread, and go to FpU / FpQ with coalesced stores.
+// 3xTF32 keeps FP32-level accuracy (see k_nn_mma).  TMEM columns: Z [0, HP), operand staging [128, 192), dU [192, 224),
+// dQ [224, 256): 256 columns per block, two blocks per SM.
+// ------------------------------------------------------------------------------------------
+constexpr int UM_COL_A = 128, UM_COL_DU = 192, UM_COL_DQ = 224, UM_COLS = 256;
+
+__device__ __forceinline__ uint64_t umma_smem_desc(unsigned smem_addr, unsigned lbo_bytes, unsigned sbo_bytes)
+{
+    // start address, leading-dimension byte offset, stride byte offset (each >> 4), version 1 (Blackwell), no swizzle
+    return (uint64_t)((smem_addr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) | (1ull << 46);
+}
+__device__ __forceinline__ void umma_tf32_ts(unsigned tmem_d, unsigned tmem_a, uint64_t desc_b, unsigned idesc, unsigned accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}\n"
+                 ::"r"(tmem_d), "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(unsigned taddr, const unsigned (&v)[16])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+                   "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(unsigned taddr, float (&v)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]), "=f"(v[8]),
+                   "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15]) : "r"(taddr) : "memory");
+}
+// wait for the mbarrier phase; a bounded spin so that a faulting MMA cannot hang the device (flag -> QNEP_ERR_CUDA)
+__device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity)
+{
+    for (int spin = 0; spin < (1 << 24); ++spin) {
+        unsigned ok;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return true;
+    }
+    return false;
+}
+
+__global__ void __launch_bounds__(128, 2)
+k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_stride, const float* __restrict__ nnw, float b1U, float b1q,
+          const int* __restrict__ start /* [T * ncells + 1] first sorted index of every (species, cell) bucket */, int ncells,
+          const float* __restrict__ D, float* __restrict__ Ui, float* __restrict__ qraw,
+          float* __restrict__ FpU, float* __restrict__ FpQ, double* __restrict__ sums, int* __restrict__ flags)
+{
+    extern __shared__ __align__(128) unsigned char sh_um[];
+    // forward B (rows = neurons, K = 32 descriptors): [8 chunks][HP][4] hi, then lo; backward B (rows = 32 descriptors, K = HP
+    // neurons): [HP / 4 chunks][32][4] hi, then lo; then b0, w1U, w1q [HP]
+    float* Wf_h = reinterpret_cast<float*>(sh_um);
+    float* Wf_l = Wf_h + 32 * HP;
+    float* Wb_h = Wf_l + 32 * HP;
+    float* Wb_l = Wb_h + 32 * HP;
+    float* b0 = Wb_l + 32 * HP;
+    float* w1U = b0 + HP;
+    float* w1q = w1U + HP;
+    __shared__ __align__(8) unsigned long long sh_bar;
+    __shared__ unsigned sh_tmem;
+    __shared__ double sh_red[32];
+    __shared__ int sh_ts[QNEP_MAX_TYPES + 1];
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const unsigned bar = (unsigned)__cvta_generic_to_shared(&sh_bar);
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&sh_tmem)), "n"(UM_COLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+        asm volatile("fence.mbarrier_init.release.cluster;");
+        for (int t = 0; t <= T; ++t) sh_ts[t] = t < T ? start[t * ncells] : (int)N;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const unsigned tbase = sh_tmem + ((unsigned)(32 * warp) << 16);       // this warp's lanes
+    const unsigned tbase0 = sh_tmem;
+    const unsigned idesc_f = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(HP >> 3) << 17) | (8u << 24);    // F32 accum, TF32 x TF32, N = HP, M = 128
+    const unsigned idesc_b = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(32 >> 3) << 17) | (8u << 24);    // N = 32
+    const unsigned wf_h = (unsigned)__cvta_generic_to_shared(Wf_h), wf_l = (unsigned)__cvta_generic_to_shared(Wf_l);
+    const unsigned wb_h = (unsigned)__cvta_generic_to_shared(Wb_h), wb_l = (unsigned)__cvta_generic_to_shared(Wb_l);
+    // tiles: species t has ceil(n_t / 128) tiles
+    int ntile_t[QNEP_MAX_TYPES], ntiles = 0;
+    for (int t = 0; t < T; ++t) { ntile_t[t] = (sh_ts[t + 1] - sh_ts[t] + 127) / 128; ntiles += ntile_t[t]; }
+    unsigned phase = 0;
+    int loaded_type = -1;
+    bool ok = true;
+    double accU = 0.0, accQ = 0.0;
+    for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+        int ty = 0, rel = tile;
+        while (rel >= ntile_t[ty]) { rel -= ntile_t[ty]; ++ty; }
+        const int64_t row0 = sh_ts[ty] + (int64_t)rel * 128;
+        const int64_t p = row0 + tid;
+        const bool live = p < sh_ts[ty + 1];
+        if (ty != loaded_type) {
+            // (the previous tile's MMAs have completed: every tile ends with a wait on the barrier)
+            const float* w = nnw + (size_t)ty * nn_stride;
+            for (int i = tid; i < 32 * HP; i += blockDim.x) {
+                const int mu = i / 32, v = i - mu * 32;
+                const float x = (mu < H && v < ND) ? w[mu * W0P + v] : 0.f;
+                unsigned hi, lo;
+                tf32_split(x, hi, lo);
+                const int of = (v >> 2) * HP * 4 + mu * 4 + (v & 3);         // forward B: row mu, k = v
+                const int ob = (mu >> 2) * 32 * 4 + v * 4 + (mu & 3);        // backward B: row v, k = mu
+                Wf_h[of] = __uint_as_float(hi); Wf_l[of] = __uint_as_float(lo);
+                Wb_h[ob] = __uint_as_float(hi); Wb_l[ob] = __uint_as_float(lo);
+            }
+            for (int i = tid; i < HP; i += blockDim.x) {
+                b0[i] = i < H ? w[H * W0P + i] : 0.f;
+                w1U[i] = i < H ? w[H * W0P + H + i] : 0.f;
+                w1q[i] = i < H ? w[H * W0P + 2 * H + i] : 0.f;
+            }
+            loaded_type = ty;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy writes -> visible to the tensor core
+        }
+        // 1. X hi / lo to TMEM columns UM_COL_A .. +32 and +32 .. +64
+        {
+            unsigned xh[32], xl[32];
+#pragma unroll
+            for (int v = 0; v < 32; ++v) {
+                const float x = (live && v < ND) ? D[(int64_t)v * N + p] : 0.f;
+                tf32_split(x, xh[v], xl[v]);
+            }
+            tmem_st16(tbase + UM_COL_A, reinterpret_cast<const unsigned (&)[16]>(xh[0]));
+            tmem_st16(tbase + UM_COL_A + 16, reinterpret_cast<const unsigned (&)[16]>(xh[16]));
+            tmem_st16(tbase + UM_COL_A + 32, reinterpret_cast<const unsigned (&)[16]>(xl[0]));
+            tmem_st16(tbase + UM_COL_A + 48, reinterpret_cast<const unsigned (&)[16]>(xl[16]));
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        // 2. forward products
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                const uint64_t dh = umma_smem_desc(wf_h + 2 * ks * HP * 16, HP * 16, 128), dl = umma_smem_desc(wf_l + 2 * ks * HP * 16, HP * 16, 128);
+                umma_tf32_ts(tbase0, tbase0 + UM_COL_A + 32 + 8 * ks, dh, idesc_f, ks > 0);      // x_lo w_hi
+                umma_tf32_ts(tbase0, tbase0 + UM_COL_A + 8 * ks, dl, idesc_f, 1);                // x_hi w_lo
+                umma_tf32_ts(tbase0, tbase0 + UM_COL_A + 8 * ks, dh, idesc_f, 1);                // x_hi w_hi
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+        }
+        ok = mbar_wait(bar, phase);
+        phase ^= 1;
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        // 3. activation per chunk of 16 neurons, backward products
+        float U = 0.f, q = 0.f;
+        for (int c = 0; c < HP / 16 && ok; ++c) {
+            float z[16];
+            tmem_ld16(tbase + 16 * c, z);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            unsigned auh[16], aul[16], bqh[16], bql[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const int mu = 16 * c + k;
+                const float hmu = tanh_f32(z[k] - b0[mu]);
+                const float aU = w1U[mu], aQ = w1q[mu];
+                U = fmaf(aU, hmu, U);
+                q = fmaf(aQ, hmu, q);
+                const float dh = fmaf(-hmu, hmu, 1.f);
+                tf32_split(aU * dh, auh[k], aul[k]);
+                tf32_split(aQ * dh, bqh[k], bql[k]);
+            }
+            if (c > 0) {
+                // the staging columns are free once the products of the previous chunk have completed; the activation above ran
+                // while they were in flight
+                ok = mbar_wait(bar, phase);
+                phase ^= 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            }
+            tmem_st16(tbase + UM_COL_A, auh);
+            tmem_st16(tbase + UM_COL_A + 16, aul);
+            tmem_st16(tbase + UM_COL_A + 32, bqh);
+            tmem_st16(tbase + UM_COL_A + 48, bql);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncthreads();
+            if (tid == 0) {
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                for (int k2 = 0; k2 < 2; ++k2) {
+                    const int kk = 2 * c + k2;                                                   // k-step of eight neurons
+                    const uint64_t dh = umma_smem_desc(wb_h + 2 * kk * 512, 512, 128), dl = umma_smem_desc(wb_l + 2 * kk * 512, 512, 128);
+                    const unsigned acc = (c > 0 || k2 > 0) ? 1u : 0u;
+                    umma_tf32_ts(tbase0 + UM_COL_DU, tbase0 + UM_COL_A + 16 + 8 * k2, dh, idesc_b, acc);   // au_lo w_hi
+                    umma_tf32_ts(tbase0 + UM_COL_DU, tbase0 + UM_COL_A + 8 * k2, dl, idesc_b, 1);          // au_hi w_lo
+                    umma_tf32_ts(tbase0 + UM_COL_DU, tbase0 + UM_COL_A + 8 * k2, dh, idesc_b, 1);          // au_hi w_hi
+                    umma_tf32_ts(tbase0 + UM_COL_DQ, tbase0 + UM_COL_A + 48 + 8 * k2, dh, idesc_b, acc);
+                    umma_tf32_ts(tbase0 + UM_COL_DQ, tbase0 + UM_COL_A + 32 + 8 * k2, dl, idesc_b, 1);
+                    umma_tf32_ts(tbase0 + UM_COL_DQ, tbase0 + UM_COL_A + 32 + 8 * k2, dh, idesc_b, 1);
+                }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+            }
+        }
+        ok = ok && mbar_wait(bar, phase);          // the products of the last chunk: dU, dQ are complete
+        phase ^= 1;
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        // 4. outputs
+        if (ok) {
+            float du[32], dq[32];
+            tmem_ld16(tbase + UM_COL_DU, reinterpret_cast<float (&)[16]>(du[0]));
+            tmem_ld16(tbase + UM_COL_DU + 16, reinterpret_cast<float (&)[16]>(du[16]));
+            tmem_ld16(tbase + UM_COL_DQ, reinterpret_cast<float (&)[16]>(dq[0]));
+            tmem_ld16(tbase + UM_COL_DQ + 16, reinterpret_cast<float (&)[16]>(dq[16]));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (live) {
+                const float Uv = U - b1U, qv = q - b1q;
+                Ui[p] = Uv; qraw[p] = qv;
+                accU += (double)Uv; accQ += (double)qv;
+#pragma unroll
+                for (int v = 0; v < ND; ++v) { FpU[(int64_t)v * N + p] = du[v]; FpQ[(int64_t)v * N + p] = dq[v]; }
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();                               // all TMEM reads of this tile are done before the next tile overwrites
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    }
+    if (!ok) atomicOr(&flags[FLAG_TENSOR_TIMEOUT], 1);
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(sh_tmem), "n"(UM_COLS));
+    const double su = block_sum(accU, sh_red);
+    const double sq = block_sum(accQ, sh_red);
+    if (threadIdx.x == 0) { atomicAdd(&sums[SUM_E_NEP], su); atomicAdd(&sums[SUM_Q], sq); }
+}
+
 // One atom per thread, scalar FMAs: the form used when the 4-/5-body terms are on (35 descriptors; two atoms per thread
 // would need 3 x 35 register pairs).
 template <int NDT>
@@ -1504,7 +1741,15 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
         QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_set = true;
     }
-    if (h->ND == QNEP_NDESC && h->nn_tensor) {
+    if (h->ND == QNEP_NDESC && h->nn_tensor == 2) {
+        const int HP = (h->model.n_neurons + 15) / 16 * 16;
+        const size_t smem_u = sizeof(float) * (size_t)(4 * 32 * HP + 3 * HP);
+        static bool attr_u = false;
+        if (!attr_u) { QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)); attr_u = true; }
+        const int nbu = (int)std::min<int64_t>((N + 127) / 128 + h->model.n_types, (int64_t)sms * 2);
+        k_nn_umma<<<nbu, 128, smem_u, s>>>(N, h->model.n_types, h->model.n_neurons, HP, h->nn_stride, h->d_nn, h->b1U, h->b1q, h->d_start,
+                                           h->geo.ncells, h->d_D, h->d_Ui, h->d_qraw, h->d_FpU, h->d_FpQ, h->d_sums, h->d_flags);
+    } else if (h->ND == QNEP_NDESC && h->nn_tensor == 1) {
         const int HP = (h->model.n_neurons + 7) / 8 * 8;
         const size_t smem_t = sizeof(float) * (size_t)h->model.n_types * (2 * HP * NNM_LD + 3 * HP);
         static bool attr_t = false;

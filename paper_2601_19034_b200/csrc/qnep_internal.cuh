@@ -113,7 +113,7 @@ __device__ __forceinline__ void qnep_zbl_eval(const ZblParams& z, int ti, int tj
 }
 // device-side int flags
 // overflow flags hold the largest count seen when a list exceeded its capacity (0 otherwise)
-enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_BAD_TYPE /* a species index outside 0..T-1 */, FLAG_COUNT = 8 };
+enum { FLAG_MAX_NR = 0 /* skin list */, FLAG_MAX_LR /* live radial */, FLAG_MAX_LA /* live angular */, FLAG_SKIN, FLAG_BAD_TYPE /* a species index outside 0..T-1 */, FLAG_TENSOR_TIMEOUT /* k_nn_umma: an MMA never completed */, FLAG_COUNT = 8 };
 
 struct Geometry {            // periodic cell (rows of h = cell vectors a, b, c; any non-degenerate cell) and the cell grid of the neighbour search
     double L[3];             // lengths of the cell vectors (orthorhombic: the box edges)
@@ -145,7 +145,7 @@ struct qnep_handle {
     float* d_cA = nullptr;           // [T*T][5][KPAD]
     float* d_nn = nullptr;           // per type: w0[H][28] (scaler folded in? no: raw), b0[H], w1U[H], w1q[H]
     int nn_stride = 0;               // floats per type in d_nn
-    int nn_tensor = 0;               // qnep_set_nn_kernel: 1 = k_nn_mma (tensor cores, 3xTF32) instead of the packed FP32 kernel
+    int nn_tensor = 0;               // qnep_set_nn_kernel: 0 packed FP32 kernel, 1 = k_nn_mma (mma.sync 3xTF32), 2 = k_nn_umma (tcgen05 3xTF32)
     int ND = QNEP_NDESC;             // descriptors per atom: 25, or 35 with the 4-/5-body terms
     int w0p = 28;                    // padded row length of w0 in d_nn (ND rounded up to a multiple of 4)
     float b1U = 0.f, b1q = 0.f;

@@ -323,9 +323,10 @@ def test_zbl_parity(torch, oracle, case):
 
 
 # ---------------------------------------------------------------- network contraction on the tensor cores (row a4)
+@pytest.mark.parametrize("mode", [2, 1])
 @pytest.mark.parametrize("case", ["config0", "config1", "config2", "config3_ragged"])
-def test_nn_tensor_core_kernel(torch, oracle, case):
-    """qnep_set_nn_kernel(1): the mma.sync 3xTF32 kernel against the oracle at the tolerances of the FP32 kernel (stage
+def test_nn_tensor_core_kernel(torch, oracle, case, mode):
+    """qnep_set_nn_kernel(2 / 1): the tcgen05 / mma.sync 3xTF32 kernels against the oracle at the tolerances of the FP32 kernel (stage
     parity of U_i, q_raw, Fp and all outputs), and against the FP32 kernel itself.  config0 has H = 30 (padded to 32),
     config2 four species (warps that straddle a species boundary), config3_ragged an atom count that is no multiple of 32."""
     bins = True
@@ -344,13 +345,13 @@ def test_nn_tensor_core_kernel(torch, oracle, case):
     _, fp32 = gpu_eval(torch, w, handle=h)
     n, D = w.n_atoms, w.model.n_desc
     U32 = h.debug_copy(Q.DBG_SITE_ENERGY, (n,)).cpu().numpy()
-    h.set_nn_kernel(1)
+    h.set_nn_kernel(mode)
     _, res = gpu_eval(torch, w, handle=h)
-    assert_parity(w, res, ref, f"tensor-core network kernel, {case}")
+    assert_parity(w, res, ref, f"tensor-core network kernel {mode}, {case}")
     Ut = h.debug_copy(Q.DBG_SITE_ENERGY, (n,)).cpu().numpy()
     assert np.abs(Ut - ref["U_i"]).max() < 1e-5 and np.abs(h.debug_copy(Q.DBG_Q_RAW, (n,)).cpu().numpy() - ref["q_raw"]).max() < 1e-5
     assert rel_rms(h.debug_copy(Q.DBG_FP, (n, D)).cpu().numpy(), ref["Fp"]) < 1e-4
-    print(f"[nn tensor {case}] max |U_i(3xTF32) - U_i(FP32)| = {np.abs(Ut - U32).max():.2e} eV, vs oracle {np.abs(Ut - ref['U_i']).max():.2e} / {np.abs(U32 - ref['U_i']).max():.2e}")
+    print(f"[nn tensor mode {mode} {case}] max |U_i(3xTF32) - U_i(FP32)| = {np.abs(Ut - U32).max():.2e} eV, vs oracle {np.abs(Ut - ref['U_i']).max():.2e} / {np.abs(U32 - ref['U_i']).max():.2e}")
     assert np.abs(Ut - U32).max() < 5e-6
     assert rel_rms(res["forces"], fp32["forces"]) < 2e-5
     h.set_nn_kernel(0)
