@@ -231,11 +231,14 @@ int qnep_set_pppm_kernels(qnep_handle *h, int32_t mode);
 
 /*
  * Kernel of the batched network contraction (the one stage where the north_star allows tensor cores).
- * mode 0 (default): packed FP32 FMAs, two atoms per thread.  mode 1: warp-level tensor-core MMA (m16n8k8 TF32) with the
- * 3xTF32 split (three products per term), which keeps FP32-level accuracy: site energies agree with mode 0 to ~1e-6 eV and
- * the stated tolerances hold (tests/test_gpu_parity.py::test_nn_tensor_core_kernel).  Measured on config 4: 0.338 ms against
- * 0.310 ms for mode 0 (the legacy mma.sync path peaks at 277 TFLOP/s TF32 on B200 and the split triples the products), so
- * FP32 stays the default.  Errors: INVALID_ARG, UNSUPPORTED (mode 1 with the 4-/5-body terms on).
+ *   mode 2 (default for the 25-descriptor model with n_neurons <= 128): 5th-generation tensor cores, tcgen05.mma kind::tf32
+ *           with accumulators and A operands in tensor memory and the 3xTF32 split (three products per term), which keeps
+ *           FP32-level accuracy: site energies agree with mode 0 to ~3e-7 eV and the stated tolerances hold
+ *           (tests/test_gpu_parity.py::test_nn_tensor_core_kernel).  0.219 ms on config 4.
+ *   mode 1: warp-level mma.sync m16n8k8 TF32, same split (0.338 ms: the legacy path peaks at 277 TFLOP/s TF32 on B200).
+ *   mode 0: packed FP32 FMAs, two atoms per thread (0.310 ms); the default when the 4-/5-body terms are on (one atom per
+ *           thread, scalar) or n_neurons > 128.
+ * Errors: INVALID_ARG, UNSUPPORTED (modes 1, 2 with the 4-/5-body terms on; mode 2 with n_neurons > 128).
  */
 int qnep_set_nn_kernel(qnep_handle *h, int32_t mode);
 

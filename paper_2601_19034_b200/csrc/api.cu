@@ -572,6 +572,7 @@ int qnep_create(const qnep_model_desc* model, const float* params_host, size_t n
         return fail(QNEP_ERR_UNSUPPORTED);
     }
     h->ND = m.l_max_4b == 2 ? QNEP_NDESC_HB : QNEP_NDESC;
+    h->nn_tensor = (h->ND == QNEP_NDESC && m.n_neurons <= 128) ? 2 : 0;      // tcgen05 kernel where it applies (qnep_set_nn_kernel)
     const int T = m.n_types, H = m.n_neurons, D = h->ND;
     const size_t expect = 2 * (size_t)T * T * QNEP_NRAD * QNEP_NB + D + (size_t)T * (H * D + 3 * H) + 2;
     if (n_params != expect) { h->err = "n_params does not match the model description"; return fail(QNEP_ERR_INVALID_ARG); }

@@ -891,6 +891,13 @@ __device__ __forceinline__ void tmem_ld16(unsigned taddr, float (&v)[16])
                  : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]), "=f"(v[8]),
                    "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15]) : "r"(taddr) : "memory");
 }
+// split for operands formed on the fly: hi = x with the 13 low mantissa bits cleared (what the tensor core reads of a TF32
+// container anyway), lo = x - hi exactly; the hardware truncates lo to TF32 itself (error 2^-20 of x).  Two instructions.
+__device__ __forceinline__ void tf32_split_trunc(float x, unsigned& hi, unsigned& lo)
+{
+    hi = __float_as_uint(x) & 0xffffe000u;
+    lo = __float_as_uint(x - __uint_as_float(hi));
+}
 // wait for the mbarrier phase; a bounded spin so that a faulting MMA cannot hang the device (flag -> QNEP_ERR_CUDA)
 __device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity)
 {
@@ -916,9 +923,7 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
     float* Wf_l = Wf_h + 32 * HP;
     float* Wb_h = Wf_l + 32 * HP;
     float* Wb_l = Wb_h + 32 * HP;
-    float* b0 = Wb_l + 32 * HP;
-    float* w1U = b0 + HP;
-    float* w1q = w1U + HP;
+    float4* nc = reinterpret_cast<float4*>(Wb_l + 32 * HP);      // per neuron (b0, w1U, w1q, 0)
     __shared__ __align__(8) unsigned long long sh_bar;
     __shared__ unsigned sh_tmem;
     __shared__ double sh_red[32];
@@ -950,10 +955,26 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
     int loaded_type = -1;
     bool ok = true;
     double accU = 0.0, accQ = 0.0;
-    for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
-        int ty = 0, rel = tile;
+    // descriptors of a tile are requested one tile ahead (they were 8 % of the stalls when loaded at the point of use)
+    float xn[ND];
+    auto tile_row = [&](int tile, int& ty) -> int64_t {
+        int rel = tile;
+        ty = 0;
         while (rel >= ntile_t[ty]) { rel -= ntile_t[ty]; ++ty; }
-        const int64_t row0 = sh_ts[ty] + (int64_t)rel * 128;
+        return sh_ts[ty] + (int64_t)rel * 128;
+    };
+    auto request = [&](int tile) {
+        if (tile >= ntiles) return;
+        int ty;
+        const int64_t pp = tile_row(tile, ty) + tid;
+        const bool lv = pp < sh_ts[ty + 1];
+#pragma unroll
+        for (int v = 0; v < ND; ++v) xn[v] = lv ? D[(int64_t)v * N + pp] : 0.f;
+    };
+    request(blockIdx.x);
+    for (int tile = blockIdx.x; tile < ntiles && ok; tile += gridDim.x) {
+        int ty;
+        const int64_t row0 = tile_row(tile, ty);
         const int64_t p = row0 + tid;
         const bool live = p < sh_ts[ty + 1];
         if (ty != loaded_type) {
@@ -969,11 +990,8 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
                 Wf_h[of] = __uint_as_float(hi); Wf_l[of] = __uint_as_float(lo);
                 Wb_h[ob] = __uint_as_float(hi); Wb_l[ob] = __uint_as_float(lo);
             }
-            for (int i = tid; i < HP; i += blockDim.x) {
-                b0[i] = i < H ? w[H * W0P + i] : 0.f;
-                w1U[i] = i < H ? w[H * W0P + H + i] : 0.f;
-                w1q[i] = i < H ? w[H * W0P + 2 * H + i] : 0.f;
-            }
+            for (int i = tid; i < HP; i += blockDim.x)
+                nc[i] = i < H ? make_float4(w[H * W0P + i], w[H * W0P + H + i], w[H * W0P + 2 * H + i], 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
             loaded_type = ty;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy writes -> visible to the tensor core
         }
@@ -981,10 +999,8 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
         {
             unsigned xh[32], xl[32];
 #pragma unroll
-            for (int v = 0; v < 32; ++v) {
-                const float x = (live && v < ND) ? D[(int64_t)v * N + p] : 0.f;
-                tf32_split(x, xh[v], xl[v]);
-            }
+            for (int v = 0; v < 32; ++v) tf32_split_trunc(v < ND ? xn[v] : 0.f, xh[v], xl[v]);
+            request(tile + gridDim.x);
             tmem_st16(tbase + UM_COL_A, reinterpret_cast<const unsigned (&)[16]>(xh[0]));
             tmem_st16(tbase + UM_COL_A + 16, reinterpret_cast<const unsigned (&)[16]>(xh[16]));
             tmem_st16(tbase + UM_COL_A + 32, reinterpret_cast<const unsigned (&)[16]>(xl[0]));
@@ -1018,13 +1034,14 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
 #pragma unroll
             for (int k = 0; k < 16; ++k) {
                 const int mu = 16 * c + k;
-                const float hmu = tanh_f32(z[k] - b0[mu]);
-                const float aU = w1U[mu], aQ = w1q[mu];
+                const float4 cn = nc[mu];
+                const float hmu = tanh_f32(z[k] - cn.x);
+                const float aU = cn.y, aQ = cn.z;
                 U = fmaf(aU, hmu, U);
                 q = fmaf(aQ, hmu, q);
                 const float dh = fmaf(-hmu, hmu, 1.f);
-                tf32_split(aU * dh, auh[k], aul[k]);
-                tf32_split(aQ * dh, bqh[k], bql[k]);
+                tf32_split_trunc(aU * dh, auh[k], aul[k]);
+                tf32_split_trunc(aQ * dh, bqh[k], bql[k]);
             }
             if (c > 0) {
                 // the staging columns are free once the products of the previous chunk have completed; the activation above ran
@@ -1039,7 +1056,10 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
             tmem_st16(tbase + UM_COL_A + 48, bql);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncthreads();
+            // the issuing warp waits for the staging stores of all four warps; the other warps only announce theirs and go on
+            // to the activation of the next chunk
+            if (warp == 0) asm volatile("bar.sync 1, 128;" ::: "memory");
+            else asm volatile("bar.arrive 1, 128;" ::: "memory");
             if (tid == 0) {
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
@@ -1743,7 +1763,7 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
     }
     if (h->ND == QNEP_NDESC && h->nn_tensor == 2) {
         const int HP = (h->model.n_neurons + 15) / 16 * 16;
-        const size_t smem_u = sizeof(float) * (size_t)(4 * 32 * HP + 3 * HP);
+        const size_t smem_u = sizeof(float) * (size_t)(4 * 32 * HP + 4 * HP);
         static bool attr_u = false;
         if (!attr_u) { QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)); attr_u = true; }
         const int nbu = (int)std::min<int64_t>((N + 127) / 128 + h->model.n_types, (int64_t)sms * 2);

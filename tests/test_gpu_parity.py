@@ -342,6 +342,7 @@ def test_nn_tensor_core_kernel(torch, oracle, case, mode):
         w = replace(w0, pos=np.ascontiguousarray(w0.pos[:, :keep]), types=w0.types[:keep].copy(), name="config3_ragged")
     ref = oracle.compute_workload(w, use_bins=bins, debug=True)
     h = Q.from_workload(w)
+    h.set_nn_kernel(0)
     _, fp32 = gpu_eval(torch, w, handle=h)
     n, D = w.n_atoms, w.model.n_desc
     U32 = h.debug_copy(Q.DBG_SITE_ENERGY, (n,)).cpu().numpy()
