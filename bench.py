@@ -333,6 +333,7 @@ def main():
     kernels = {   # stage time (the kernel is bracketed alone, or with O(N) helpers), algorithmic flops per launch
         "k_pairs": (per_eval["desc_radial"], FLOPS_RAD_FWD_PER_NEIGHBOUR * live_r * n),
         "k_desc_angular": (per_eval["desc_angular"], FLOPS_ANG_FWD_PER_NEIGHBOUR * live_a * n),
+        # k_nn_umma by default: the contraction runs on the tensor cores (3xTF32), still counted by the FP32 work model
         "k_nn": (per_eval["nn"], (FLOPS_NN_FWD_H80 + FLOPS_NN_BWD_H80) * (H / 80.0) * n),
         "k_force_angular": (per_eval["force_angular"], FLOPS_ANG_BWD_PER_NEIGHBOUR * live_a * n),
         "k_force_radial": (per_eval["force_radial"], FLOPS_RAD_BWD_PER_NEIGHBOUR * live_r * n),
@@ -451,6 +452,7 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "n_atoms": n, "species": w.model.n_types, "pppm_grid": list(w.es.grid),
                        "mode": w.model.mode, "n_neurons": w.model.n_neurons, "md": "velocity-Verlet via qnep_md_run" + (", steps replayed as CUDA graphs (stage times from plain launches)" if md_graphs else ""),
+                       "nn_kernel": {-1: "library default (tcgen05 3xTF32)", 0: "packed FP32", 1: "mma.sync 3xTF32", 2: "tcgen05 3xTF32"}[args.nn_kernel],
                        "dt_fs": dt_fs, "zbl": list(w.zbl[:2]) if w.zbl else None, "skin_A": args.skin, "rebuild_every": args.rebuild_every,
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2_policy": "inputs larger than L2 (neighbour lists + meshes >> 126 MB); no flush needed",
