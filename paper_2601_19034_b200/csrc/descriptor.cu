@@ -901,7 +901,7 @@ __device__ __forceinline__ void tf32_split_trunc(float x, unsigned& hi, unsigned
 // wait for the mbarrier phase; a bounded spin so that a faulting MMA cannot hang the device (flag -> QNEP_ERR_CUDA)
 __device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity)
 {
-    for (int spin = 0; spin < (1 << 24); ++spin) {
+    for (int spin = 0; spin < (1 << 20); ++spin) {
         unsigned ok;
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
@@ -919,23 +919,27 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
     extern __shared__ __align__(128) unsigned char sh_um[];
     // forward B (rows = neurons, K = 32 descriptors): [8 chunks][HP][4] hi, then lo; backward B (rows = 32 descriptors, K = HP
     // neurons): [HP / 4 chunks][32][4] hi, then lo; then b0, w1U, w1q [HP]
+    // (backward: both outputs share the factor 1 - h^2, so the A operand is dh alone and the output weights are folded into two
+    //  B tables, WU = w1U_mu w0[mu][v] and WQ = w1q_mu w0[mu][v]: one split and one staging store per neuron instead of two)
     float* Wf_h = reinterpret_cast<float*>(sh_um);
     float* Wf_l = Wf_h + 32 * HP;
-    float* Wb_h = Wf_l + 32 * HP;
-    float* Wb_l = Wb_h + 32 * HP;
-    float4* nc = reinterpret_cast<float4*>(Wb_l + 32 * HP);      // per neuron (b0, w1U, w1q, 0)
-    __shared__ __align__(8) unsigned long long sh_bar;
+    // backward B: ONE table of 64 rows (rows 0..31: WU of descriptor v, rows 32..63: WQ), [HP / 4 chunks][64][4], so that
+    // dU/dD and dq/dD are the 64 columns of one accumulator and one MMA (N = 64) serves both
+    float* WB_h = Wf_l + 32 * HP;
+    float* WB_l = WB_h + 64 * HP;
+    float4* nc = reinterpret_cast<float4*>(WB_l + 64 * HP);      // per neuron (b0, w1U, w1q, 0)
+    __shared__ __align__(8) unsigned long long sh_bar[3];     // [0] forward products, [1], [2] backward products of even / odd chunks
     __shared__ unsigned sh_tmem;
     __shared__ double sh_red[32];
     __shared__ int sh_ts[QNEP_MAX_TYPES + 1];
     const int tid = threadIdx.x, warp = tid >> 5;
-    const unsigned bar = (unsigned)__cvta_generic_to_shared(&sh_bar);
+    const unsigned bar = (unsigned)__cvta_generic_to_shared(&sh_bar[0]);     // a waiter may lag ONE phase behind a barrier: one barrier per buffer
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&sh_tmem)), "n"(UM_COLS));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+        for (int i = 0; i < 3; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar + 8 * i));
         asm volatile("fence.mbarrier_init.release.cluster;");
         for (int t = 0; t <= T; ++t) sh_ts[t] = t < T ? start[t * ncells] : (int)N;
     }
@@ -945,13 +949,13 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
     const unsigned tbase = sh_tmem + ((unsigned)(32 * warp) << 16);       // this warp's lanes
     const unsigned tbase0 = sh_tmem;
     const unsigned idesc_f = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(HP >> 3) << 17) | (8u << 24);    // F32 accum, TF32 x TF32, N = HP, M = 128
-    const unsigned idesc_b = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(32 >> 3) << 17) | (8u << 24);    // N = 32
+    const unsigned idesc_b = (1u << 4) | (2u << 7) | (2u << 10) | ((unsigned)(64 >> 3) << 17) | (8u << 24);    // N = 64
     const unsigned wf_h = (unsigned)__cvta_generic_to_shared(Wf_h), wf_l = (unsigned)__cvta_generic_to_shared(Wf_l);
-    const unsigned wb_h = (unsigned)__cvta_generic_to_shared(Wb_h), wb_l = (unsigned)__cvta_generic_to_shared(Wb_l);
+    const unsigned wb_h = (unsigned)__cvta_generic_to_shared(WB_h), wb_l = (unsigned)__cvta_generic_to_shared(WB_l);
     // tiles: species t has ceil(n_t / 128) tiles
     int ntile_t[QNEP_MAX_TYPES], ntiles = 0;
     for (int t = 0; t < T; ++t) { ntile_t[t] = (sh_ts[t + 1] - sh_ts[t] + 127) / 128; ntiles += ntile_t[t]; }
-    unsigned phase = 0;
+    unsigned phase = 0, phc[2] = {0, 0};
     int loaded_type = -1;
     bool ok = true;
     double accU = 0.0, accQ = 0.0;
@@ -983,12 +987,16 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
             for (int i = tid; i < 32 * HP; i += blockDim.x) {
                 const int mu = i / 32, v = i - mu * 32;
                 const float x = (mu < H && v < ND) ? w[mu * W0P + v] : 0.f;
+                const float aU = mu < H ? w[H * W0P + H + mu] : 0.f, aQ = mu < H ? w[H * W0P + 2 * H + mu] : 0.f;
                 unsigned hi, lo;
                 tf32_split(x, hi, lo);
                 const int of = (v >> 2) * HP * 4 + mu * 4 + (v & 3);         // forward B: row mu, k = v
-                const int ob = (mu >> 2) * 32 * 4 + v * 4 + (mu & 3);        // backward B: row v, k = mu
+                const int ob = (mu >> 2) * 64 * 4 + v * 4 + (mu & 3);        // backward B: row v (WU) / 32 + v (WQ), k = mu
                 Wf_h[of] = __uint_as_float(hi); Wf_l[of] = __uint_as_float(lo);
-                Wb_h[ob] = __uint_as_float(hi); Wb_l[ob] = __uint_as_float(lo);
+                tf32_split(aU * x, hi, lo);
+                WB_h[ob] = __uint_as_float(hi); WB_l[ob] = __uint_as_float(lo);
+                tf32_split(aQ * x, hi, lo);
+                WB_h[ob + 32 * 4] = __uint_as_float(hi); WB_l[ob + 32 * 4] = __uint_as_float(lo);
             }
             for (int i = tid; i < HP; i += blockDim.x)
                 nc[i] = i < H ? make_float4(w[H * W0P + i], w[H * W0P + H + i], w[H * W0P + 2 * H + i], 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -1030,55 +1038,56 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
             float z[16];
             tmem_ld16(tbase + 16 * c, z);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            unsigned auh[16], aul[16], bqh[16], bql[16];
+            unsigned dhh[16], dhl[16];
 #pragma unroll
             for (int k = 0; k < 16; ++k) {
                 const int mu = 16 * c + k;
                 const float4 cn = nc[mu];
                 const float hmu = tanh_f32(z[k] - cn.x);
-                const float aU = cn.y, aQ = cn.z;
-                U = fmaf(aU, hmu, U);
-                q = fmaf(aQ, hmu, q);
-                const float dh = fmaf(-hmu, hmu, 1.f);
-                tf32_split_trunc(aU * dh, auh[k], aul[k]);
-                tf32_split_trunc(aQ * dh, bqh[k], bql[k]);
+                U = fmaf(cn.y, hmu, U);
+                q = fmaf(cn.z, hmu, q);
+                tf32_split_trunc(fmaf(-hmu, hmu, 1.f), dhh[k], dhl[k]);
             }
-            if (c > 0) {
-                // the staging columns are free once the products of the previous chunk have completed; the activation above ran
-                // while they were in flight
-                ok = mbar_wait(bar, phase);
-                phase ^= 1;
+            // two staging buffers of 32 columns (chunk parity): buffer c & 1 is free once the products of chunk c - 2 have
+            // completed, so the activation runs up to two chunks ahead of the tensor core
+            if (c > 1) {
+                ok = mbar_wait(bar + 8 + 8 * (c & 1), phc[c & 1]);
+                phc[c & 1] ^= 1;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             }
-            tmem_st16(tbase + UM_COL_A, auh);
-            tmem_st16(tbase + UM_COL_A + 16, aul);
-            tmem_st16(tbase + UM_COL_A + 32, bqh);
-            tmem_st16(tbase + UM_COL_A + 48, bql);
+            const unsigned stg = UM_COL_A + 32 * (c & 1);
+            tmem_st16(tbase + stg, dhh);
+            tmem_st16(tbase + stg + 16, dhl);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             // the issuing warp waits for the staging stores of all four warps; the other warps only announce theirs and go on
             // to the activation of the next chunk
-            if (warp == 0) asm volatile("bar.sync 1, 128;" ::: "memory");
-            else asm volatile("bar.arrive 1, 128;" ::: "memory");
+            // (two named barriers by chunk parity: the other warps may be one chunk ahead of the issuing warp)
+            if (warp == 0) asm volatile("bar.sync %0, 128;" ::"r"(1 + (c & 1)) : "memory");
+            else asm volatile("bar.arrive %0, 128;" ::"r"(1 + (c & 1)) : "memory");
             if (tid == 0) {
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
                 for (int k2 = 0; k2 < 2; ++k2) {
                     const int kk = 2 * c + k2;                                                   // k-step of eight neurons
-                    const uint64_t dh = umma_smem_desc(wb_h + 2 * kk * 512, 512, 128), dl = umma_smem_desc(wb_l + 2 * kk * 512, 512, 128);
+                    const uint64_t bh = umma_smem_desc(wb_h + 2 * kk * 1024, 1024, 128), bl = umma_smem_desc(wb_l + 2 * kk * 1024, 1024, 128);
                     const unsigned acc = (c > 0 || k2 > 0) ? 1u : 0u;
-                    umma_tf32_ts(tbase0 + UM_COL_DU, tbase0 + UM_COL_A + 16 + 8 * k2, dh, idesc_b, acc);   // au_lo w_hi
-                    umma_tf32_ts(tbase0 + UM_COL_DU, tbase0 + UM_COL_A + 8 * k2, dl, idesc_b, 1);          // au_hi w_lo
-                    umma_tf32_ts(tbase0 + UM_COL_DU, tbase0 + UM_COL_A + 8 * k2, dh, idesc_b, 1);          // au_hi w_hi
-                    umma_tf32_ts(tbase0 + UM_COL_DQ, tbase0 + UM_COL_A + 48 + 8 * k2, dh, idesc_b, acc);
-                    umma_tf32_ts(tbase0 + UM_COL_DQ, tbase0 + UM_COL_A + 32 + 8 * k2, dl, idesc_b, 1);
-                    umma_tf32_ts(tbase0 + UM_COL_DQ, tbase0 + UM_COL_A + 32 + 8 * k2, dh, idesc_b, 1);
+                    const unsigned a_hi = tbase0 + stg + 8 * k2, a_lo = tbase0 + stg + 16 + 8 * k2;
+                    umma_tf32_ts(tbase0 + UM_COL_DU, a_lo, bh, idesc_b, acc);      // dh_lo W_hi   (columns: dU/dD, then dq/dD)
+                    umma_tf32_ts(tbase0 + UM_COL_DU, a_hi, bl, idesc_b, 1);        // dh_hi W_lo
+                    umma_tf32_ts(tbase0 + UM_COL_DU, a_hi, bh, idesc_b, 1);        // dh_hi W_hi
                 }
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar + 8 + 8 * (c & 1)) : "memory");
             }
         }
-        ok = ok && mbar_wait(bar, phase);          // the products of the last chunk: dU, dQ are complete
-        phase ^= 1;
+        // the commits not yet waited for: those of the last two chunks (one if there is a single chunk); after them dU, dQ are complete
+        {
+            const int nch = HP / 16;
+            for (int c = max(nch - 2, 0); c < nch; ++c) {
+                ok = ok && mbar_wait(bar + 8 + 8 * (c & 1), phc[c & 1]);
+                phc[c & 1] ^= 1;
+            }
+        }
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         // 4. outputs
         if (ok) {
@@ -1763,7 +1772,7 @@ int qnep_launch_nn(qnep_handle* h, double* charges_out, cudaStream_t s)
     }
     if (h->ND == QNEP_NDESC && h->nn_tensor == 2) {
         const int HP = (h->model.n_neurons + 15) / 16 * 16;
-        const size_t smem_u = sizeof(float) * (size_t)(4 * 32 * HP + 4 * HP);
+        const size_t smem_u = sizeof(float) * (size_t)(6 * 32 * HP + 4 * HP);
         static bool attr_u = false;
         if (!attr_u) { QNEP_CUDA_OK(h, cudaFuncSetAttribute(k_nn_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)); attr_u = true; }
         const int nbu = (int)std::min<int64_t>((N + 127) / 128 + h->model.n_types, (int64_t)sms * 2);
