@@ -70,14 +70,16 @@ def whole_job_value(n_atoms, steps, world, ms_total):
 # FMUL2 / FADD2 2; the op_ffma counter does not see the packed instructions).  Reported only for that workload; the
 # algorithmic work model above them is what the contract's `frac` uses, the executed figure is the north_star's evidence.
 NCU_COUNTERS_CONFIG4 = {
-    "k_pairs": {"dram_bytes": 1.596e9, "executed_flops": 7.975e9},
-    "k_desc_angular": {"dram_bytes": 1.033e9, "executed_flops": 1.151e10},
-    "k_nn": {"dram_bytes": 0.283e9, "executed_flops": 1.392e10},
-    "k_force_angular": {"dram_bytes": 1.449e9, "executed_flops": 2.577e10},
-    "k_force_radial": {"dram_bytes": 0.676e9, "executed_flops": 1.349e10},
+    "k_pairs": {"dram_bytes": 1.594e9, "executed_flops": 7.975e9},
+    "k_desc_angular": {"dram_bytes": 1.032e9, "executed_flops": 1.151e10},
+    # k_nn_umma: the contraction runs on the tensor cores (42 tcgen05.mma per 128-atom tile, 3xTF32: 4.74e10 tensor flops per
+    # launch, not counted here); executed_flops is its FP32 part (activation, splits)
+    "k_nn": {"dram_bytes": 0.264e9, "executed_flops": 1.188e9, "tensor_flops": 4.74e10},
+    "k_force_angular": {"dram_bytes": 1.449e9, "executed_flops": 2.590e10},
+    "k_force_radial": {"dram_bytes": 0.677e9, "executed_flops": 1.349e10},
 }
 NCU_COUNTERS_SOURCE = "profiles/r02_ncu_full.txt"
-NCU_PPPM_DRAM_BYTES_CONFIG4 = 1.921e9       # spread + five FFT kernels + gather, same capture
+NCU_PPPM_DRAM_BYTES_CONFIG4 = 1.914e9       # spread + five FFT kernels + gather, same capture
 
 
 def load_peaks():
@@ -366,6 +368,7 @@ def main():
                                    "frac": frac_of_peak(v[1], v[0]), "frac_model": frac_of_peak(v[1], v[0]),
                                    "executed_flops_per_launch": ctr[k]["executed_flops"] if ctr else None,
                                    "executed_frac": frac_of_peak(ctr[k]["executed_flops"], v[0]) if ctr else None,
+                                   "tensor_flops_per_launch": ctr[k].get("tensor_flops") if ctr else None,
                                    "dram_bytes_per_launch": ctr[k]["dram_bytes"] if ctr else None}
                                for k, v in kernels.items()},
                 "all_fp32_stages": {"ms": fp32_ms, "algorithmic_flops": fp32_flops,
