@@ -436,7 +436,8 @@ def main():
     t_e2e = time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e, dist, dev)
     e2e = {"value": whole_job_value(n, Ke, world, t_e2e * 1e3), "unit": "atom-steps/s", "steps": Ke,
-           "h2d_bytes_per_step": int(frames[0].numel() * 8 + ht.numel() * 4),
+           # positions every call; the species travel only with the calls that rebuild the neighbour list (one in n_frames)
+           "h2d_bytes_per_step": int(frames[0].numel() * 8 + ht.numel() * 4 // n_frames),
            "d2h_bytes_per_step": int(hf.numel() * 8 + hq.numel() * 8 + 9 * 8 + 8),
            "outputs": "energy, forces, virial, charges",
            "api": "qnep_compute_host (pinned host buffers, a different frame per call; neighbour rebuild every %d calls)" % n_frames}

@@ -175,9 +175,10 @@ int qnep_compute_atom_virial(qnep_handle *h, int64_t n_atoms, const double *pos_
                              double *virial_dev, double *charges_dev, double *atom_virial_dev, void *cuda_stream);
 
 /*
- * qnep_compute_host: the same evaluation with HOST buffers: copies positions and types to the device,
- * runs qnep_compute, copies the requested outputs back and synchronises the stream; device-side errors
- * of THIS call are reported.  Layouts as above.
+ * qnep_compute_host: the same evaluation with HOST buffers: copies positions (and, on calls that may rebuild the
+ * neighbour list, the species: between builds the species of the last build apply, as in qnep_compute) to the device,
+ * runs qnep_compute, copies the requested outputs back (the charges on a second stream while the evaluation goes on)
+ * and synchronises the stream; device-side errors of THIS call are reported.  Layouts as above.
  */
 int qnep_compute_host(qnep_handle *h, int64_t n_atoms, const double *pos_host, const int32_t *types_host,
                       const double box[9], uint32_t want, double *energy_host, double *forces_host,

@@ -763,7 +763,8 @@ int qnep_compute_host(qnep_handle* h, int64_t n_atoms, const double* pos_host, c
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t n = (size_t)n_atoms;
-    if (h->hostN != n_atoms) {
+    const bool fresh = h->hostN != n_atoms;
+    if (fresh) {
         if ((rc = dev_alloc(h, &h->d_hpos, 3 * n))) return rc;
         if ((rc = dev_alloc(h, &h->d_htypes, n))) return rc;
         if ((rc = dev_alloc(h, &h->d_hout, 1 + 3 * n + 9 + n + 9 * n))) return rc;
@@ -775,7 +776,12 @@ int qnep_compute_host(qnep_handle* h, int64_t n_atoms, const double* pos_host, c
     double* d_q = d_w + 9;
     double* d_z = d_q + n;
     QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_hpos, pos_host, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, s));
-    QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_htypes, types_host, sizeof(int32_t) * n, cudaMemcpyHostToDevice, s));
+    // The species are read by the neighbour build only (between builds they sit in the sorted coordinate array), so they travel
+    // only with the calls that can rebuild: same predicate as plan_pipeline / ensure_workspace, erring on the side of copying.
+    const bool may_rebuild = fresh || h->force_rebuild || h->rebuild_every <= 1 || h->calls_since_build < 0 ||
+                             h->calls_since_build >= h->rebuild_every || h->N != n_atoms || h->flags_pending ||
+                             std::memcmp(box, h->box, sizeof(double) * 9) != 0;
+    if (may_rebuild) QNEP_CUDA_OK(h, cudaMemcpyAsync(h->d_htypes, types_host, sizeof(int32_t) * n, cudaMemcpyHostToDevice, s));
     const bool early_q = (want & QNEP_WANT_CHARGES) != 0;
     if (early_q) {
         if (!h->copy_stream) {
