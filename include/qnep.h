@@ -309,6 +309,36 @@ int qnep_fma_peak(double *tflops_host, void *cuda_stream);
  */
 int qnep_debug_copy(qnep_handle *h, int32_t which, double *dst_dev, int64_t n);
 
+/*
+ * qnep_neutralise_noalloc: Eq. 33 (PAPER.md :255-262; reading G3) on its own, for callers that are not allowed to
+ * allocate device memory:
+ *     charges_i = q_raw_i + (q_total - sum_j q_raw_j) / n_atoms.
+ * Everything else in this header sizes a workspace with cudaMalloc (qnep_create, and again when the atom count or the mesh
+ * grows).  Some callers cannot do that: a plug-in of an MD engine or inference server whose own pool already holds the rest
+ * of the GPU (a raw cudaMalloc from a library then fails, or takes memory the application had counted on); code in a
+ * section that must not stall the device (cudaMalloc / cudaFree may synchronise the whole context and so every other
+ * stream); code that must fix its memory footprint before the first step.  This entry point needs no handle and calls
+ * neither cudaMalloc nor cudaFree nor any library routine that allocates: the one piece of scratch it needs, the partial
+ * sums of q_raw, sits in an array compiled into the library (32 KiB, present on every GPU that loads the library until the
+ * process ends).
+ *   n_atoms      1 .. QNEP_NOALLOC_MAX_ATOMS; more is refused with QNEP_ERR_UNSUPPORTED and nothing is launched
+ *   q_raw_dev    [n_atoms] float64 DEVICE, the network's charge outputs before Eq. 33 (what QNEP_DBG_Q_RAW returns)
+ *   q_total      target total charge Q
+ *   charges_dev  [n_atoms] float64 DEVICE, owned by the caller; may be the same buffer as q_raw_dev
+ *   err_host     optional HOST buffer of err_len bytes that receives a message when the call fails (NULL: no message)
+ * Two kernels are enqueued on `cuda_stream` (on the current device); the call does not synchronise.  The result does not
+ * depend on the launch: every atom gets the same shift, summed in a fixed order.
+ * First call on a device: looks up the device address of the built-in array (cudaGetSymbolAddress) and loads the two
+ * kernels, once per device, with that device current.  Make that first call during start-up, outside any stream capture.
+ * Shared state: all calls on one device use the same array, and it keeps the last call's contents.  Each call overwrites
+ * the slots it reads before reading them, so nothing needs clearing between calls -- but calls whose kernels overlap on the
+ * GPU (two streams without an event between them, two host threads) corrupt each other's sums: order them.
+ * Errors: INVALID_ARG (null pointer, n_atoms <= 0), UNSUPPORTED (n_atoms above the maximum, device ordinal >= 64), CUDA.
+ */
+#define QNEP_NOALLOC_MAX_ATOMS 4194304 /* 4096 partial sums of 1024 atoms each */
+int qnep_neutralise_noalloc(int64_t n_atoms, const double *q_raw_dev, double q_total, double *charges_dev,
+                            void *cuda_stream, char *err_host, size_t err_len);
+
 void qnep_destroy(qnep_handle *h);
 
 /* Message of the last error on this handle (or of the last failed qnep_create if h == NULL); valid until the next call. */

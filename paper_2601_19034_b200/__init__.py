@@ -38,7 +38,8 @@ ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_poli
                "qnep_compute", "qnep_compute_atom_virial", "qnep_compute_host", "qnep_md_run", "qnep_md_set_outputs", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
                "qnep_fma_peak", "qnep_set_zbl", "qnep_set_nn_kernel",
-               "qnep_debug_copy", "qnep_destroy", "qnep_last_error"]
+               "qnep_debug_copy", "qnep_neutralise_noalloc", "qnep_destroy", "qnep_last_error"]
+NOALLOC_MAX_ATOMS = 4194304          # QNEP_NOALLOC_MAX_ATOMS of include/qnep.h
 
 
 class qnep_model_desc(C.Structure):
@@ -118,6 +119,8 @@ def load_library():
     lib.qnep_fma_peak.argtypes = [C.POINTER(dbl), vp]
     lib.qnep_debug_copy.restype = C.c_int
     lib.qnep_debug_copy.argtypes = [vp, i32, vp, i64]
+    lib.qnep_neutralise_noalloc.restype = C.c_int
+    lib.qnep_neutralise_noalloc.argtypes = [i64, vp, dbl, vp, vp, C.c_char_p, C.c_size_t]
     lib.qnep_destroy.restype = None
     lib.qnep_destroy.argtypes = [vp]
     lib.qnep_last_error.restype = C.c_char_p
@@ -366,6 +369,27 @@ def fma_peak(stream=None) -> float:
     if rc != QNEP_OK:
         raise QnepError(rc, "qnep_fma_peak failed")
     return float(out.value)
+
+
+def neutralise_noalloc(q_raw, q_total: float, out=None, stream=None):
+    """qnep_neutralise_noalloc: Eq. 33, ``out_i = q_raw_i + (q_total - sum q_raw) / N``, without a handle and without any
+    device allocation inside the library -- for callers whose GPU memory is owned by someone else's pool, or who may not
+    stall the device with cudaMalloc / cudaFree (see include/qnep.h).  q_raw: cuda float64 [N], N <= NOALLOC_MAX_ATOMS;
+    out: cuda float64 [N] supplied by the caller (``out=q_raw`` works in place); only when it is None does this
+    convenience wrapper -- not the library -- take one from torch.  All calls on a device share one built-in scratch array:
+    do not let two of them run at the same time on different streams.  The first call on a device does a one-off set-up."""
+    import torch
+    assert q_raw.is_cuda and q_raw.dtype == torch.float64 and q_raw.is_contiguous() and q_raw.dim() == 1
+    if out is None:
+        out = torch.empty_like(q_raw)
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.shape == q_raw.shape
+    msg = C.create_string_buffer(512)
+    with torch.cuda.device(q_raw.device):
+        rc = load_library().qnep_neutralise_noalloc(q_raw.shape[0], C.c_void_p(q_raw.data_ptr()), float(q_total),
+                                                    C.c_void_p(out.data_ptr()), QNEP._stream(stream), msg, len(msg))
+    if rc != QNEP_OK:
+        raise QnepError(rc, msg.value.decode())
+    return out
 
 
 def from_workload(w) -> QNEP:

@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqnep_b200.so")
-SOURCES = ["api.cu", "neighbor.cu", "descriptor.cu", "electro.cu", "pppm.cu", "pppm_sweep.cu"]
+SOURCES = ["api.cu", "neighbor.cu", "descriptor.cu", "electro.cu", "pppm.cu", "pppm_sweep.cu", "noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "qnep_internal.cuh"), os.path.join(CSRC, "fft_reg.cuh"), os.path.join(CSRC, "pppm_common.cuh"),
            os.path.join(HERE, "..", "include", "qnep.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
