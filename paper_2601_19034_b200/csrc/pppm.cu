@@ -767,7 +767,8 @@ int qnep_setup_pppm(qnep_handle* h)
     const int64_t ng = (int64_t)grid[0] * grid[1] * grid[2];
     if (ng != h->ngrid) {
         cudaFree(h->d_mesh); cudaFree(h->d_cm1); cudaFree(h->d_cm2); cudaFree(h->d_field);
-        h->d_mesh = nullptr; h->d_cm1 = nullptr; h->d_cm2 = nullptr; h->d_field = nullptr;
+        cudaFree(h->d_cm3);      // allocated on demand by qnep_launch_pppm_atom_virial with the mesh size of that time
+        h->d_mesh = nullptr; h->d_cm1 = nullptr; h->d_cm2 = nullptr; h->d_field = nullptr; h->d_cm3 = nullptr;
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_mesh, sizeof(float) * ng));
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm1, sizeof(float2) * ng));
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm2, sizeof(float2) * ng));
