@@ -65,21 +65,42 @@ def whole_job_value(n_atoms, steps, world, ms_total):
 
 
 # ncu counters per launch on config 4 in the launch configuration timed here (all outputs), from the ncu --set full capture
-# summarised in profiles/r02_ncu_full.txt: DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) and EXECUTED FP32
-# flops (predicated-on thread executions per SASS opcode from the source page: FFMA 2, packed FFMA2 4, FMUL / FADD / MUFU 1,
-# FMUL2 / FADD2 2; the op_ffma counter does not see the packed instructions).  Reported only for that workload; the
-# algorithmic work model above them is what the contract's `frac` uses, the executed figure is the north_star's evidence.
-NCU_COUNTERS_CONFIG4 = {
-    "k_pairs": {"dram_bytes": 1.594e9, "executed_flops": 7.975e9},
-    "k_desc_angular": {"dram_bytes": 1.032e9, "executed_flops": 1.151e10},
-    # k_nn_umma: the contraction runs on the tensor cores (42 tcgen05.mma per 128-atom tile, 3xTF32: 4.74e10 tensor flops per
-    # launch, not counted here); executed_flops is its FP32 part (activation, splits)
-    "k_nn": {"dram_bytes": 0.264e9, "executed_flops": 1.188e9, "tensor_flops": 4.74e10},
-    "k_force_angular": {"dram_bytes": 1.449e9, "executed_flops": 2.590e10},
-    "k_force_radial": {"dram_bytes": 0.677e9, "executed_flops": 1.349e10},
+# summarised in NCU_COUNTERS["source"]: DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) and EXECUTED FP32 flops
+# (predicated-on thread executions per SASS opcode from the source page: FFMA 2, packed FFMA2 4, FMUL / FADD / MUFU 1,
+# FMUL2 / FADD2 2; the op_ffma counter does not see the packed instructions).  Reported only for that workload.  They are the
+# north_star's evidence ("ncu-counted achieved FP32 FLOP/s"), so `roofline.frac` is the EXECUTED fraction whenever they apply;
+# the frozen algorithmic work model above stays beside it as `frac_model`.  The capture belongs to one state of the kernel
+# sources: "csrc_sha256" is the digest of csrc/ at capture time (csrc_digest() below), and the JSON line says
+# "counters_stale": true when the sources have changed since (re-capture, then update both).
+NCU_COUNTERS = {
+    "source": "profiles/r02_ncu_full.txt",
+    "captured_at_commit": "3cd59cc",
+    "csrc_sha256": None,
+    "kernels": {
+        "k_pairs": {"dram_bytes": 1.594e9, "executed_flops": 7.975e9},
+        "k_desc_angular": {"dram_bytes": 1.032e9, "executed_flops": 1.151e10},
+        # k_nn_umma: the contraction runs on the tensor cores (42 tcgen05.mma per 128-atom tile, 3xTF32: 4.74e10 tensor flops
+        # per launch); executed_flops is its FP32 part (activation, splits)
+        "k_nn": {"dram_bytes": 0.264e9, "executed_flops": 1.188e9, "tensor_flops": 4.74e10},
+        "k_force_angular": {"dram_bytes": 1.449e9, "executed_flops": 2.590e10},
+        "k_force_radial": {"dram_bytes": 0.677e9, "executed_flops": 1.349e10},
+    },
+    "pppm_dram_bytes": 1.914e9,          # spread + five FFT kernels + gather, same capture
 }
-NCU_COUNTERS_SOURCE = "profiles/r02_ncu_full.txt"
-NCU_PPPM_DRAM_BYTES_CONFIG4 = 1.914e9       # spread + five FFT kernels + gather, same capture
+TF32_OVER_BF16_NOMINAL = 0.5             # dense tensor peak of kind::tf32 relative to bf16 (B200_PROFILING.md nominal ratio)
+
+
+def csrc_digest() -> str:
+    """sha256 over the CUDA sources of the library, in name order: the state of the kernels the ncu counters belong to."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2601_19034_b200", "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()
 
 
 def load_peaks():
@@ -87,8 +108,9 @@ def load_peaks():
     if os.path.exists(path):
         with open(path) as f:
             p = json.load(f)
-        return dict(hbm_gbs=float(p["hbm_gbs"]), source="measured (MEASURED_PEAKS.json)")
-    return dict(hbm_gbs=6650.0, source="fallback (B200_PROFILING.md)")
+        return dict(hbm_gbs=float(p["hbm_gbs"]), bf16_tflops=float(p.get("bf16_tflops_sustained", p.get("bf16_tflops", 1400.0))),
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1400.0, source="fallback (B200_PROFILING.md)")
 
 
 def make_workload(cfg: int, args):
@@ -208,6 +230,9 @@ def main():
                     help="switch the ZBL core on (water: Z = 8, 1); off by default: BASELINE.json's config has none")
     ap.add_argument("--nn-kernel", type=int, default=-1, help="qnep_set_nn_kernel: 0 packed FP32, 1 mma.sync 3xTF32, 2 tcgen05 3xTF32 (-1: the library's default)")
     ap.add_argument("--pppm-kernels", type=int, default=0, help="qnep_set_pppm_kernels: 0 automatic, 1 per-atom spread, 2 sweep spread")
+    ap.add_argument("--optional-legs", action="store_true",
+                    help="also time the optional terms of SURVEY 8(f) on this workload (per-atom virial, ZBL core, triclinic cell, "
+                         "NEP4 4-/5-body terms): untimed by default, reported under \"optional_legs\"")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -342,41 +367,68 @@ def main():
     }
     dom = max(kernels, key=lambda k: kernels[k][0])
     dom_ms, dom_flops = kernels[dom]
-    fp32_ms = sum(v[0] for v in kernels.values())
-    fp32_flops = sum(v[1] for v in kernels.values())
-    achieved = dom_flops / (dom_ms * 1e-3) / 1e12 if dom_ms > 0 else 0.0
-    full4 = args.config == 4 and not args.n_side       # the workload the ncu counters were taken on
-    ctr = NCU_COUNTERS_CONFIG4 if full4 else {}
+    # the workload and kernel selection the ncu counters were taken on
+    full4 = args.config == 4 and not args.n_side and args.nn_kernel in (-1, 2) and not args.zbl
+    ctr = NCU_COUNTERS["kernels"] if full4 else {}
+    digest = csrc_digest()
+    peaks = load_peaks()
+    nn_on_tensor = args.nn_kernel != 0                 # library default (-1) and modes 1, 2: the contraction is not FP32 work
+    fp32_kernels = [k for k in kernels if not (k == "k_nn" and nn_on_tensor)]
 
     def frac_of_peak(flops, ms):
         return flops / (ms * 1e-3) / 1e12 / FP32_PEAK_NOMINAL_TFLOPS if ms > 0 else 0.0
 
-    exe_flops = sum(c["executed_flops"] for c in ctr.values()) if ctr else None
+    def tflops(flops, ms):
+        return flops / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+
+    fp32_ms = sum(kernels[k][0] for k in fp32_kernels)
+    fp32_flops = sum(kernels[k][1] for k in fp32_kernels)
+    exe_flops = sum(ctr[k]["executed_flops"] for k in fp32_kernels) if ctr else None
+    achieved_model = tflops(dom_flops, dom_ms)
+    achieved = tflops(ctr[dom]["executed_flops"], dom_ms) if ctr else achieved_model
+    tf32_peak = peaks["bf16_tflops"] * TF32_OVER_BF16_NOMINAL
+    nn_ms = kernels["k_nn"][0]
+    nn_tensor = None
+    if nn_on_tensor and ctr:
+        nn_tensor = {"kernel": "k_nn_umma (tcgen05 kind::tf32, 3xTF32)" if args.nn_kernel in (-1, 2) else "k_nn_mma (mma.sync TF32, 3xTF32)",
+                     "bound": "tensor", "ms": nn_ms, "tensor_flops_per_launch": ctr["k_nn"]["tensor_flops"],
+                     "achieved": tflops(ctr["k_nn"]["tensor_flops"], nn_ms), "unit": "TFLOP/s", "peak": tf32_peak,
+                     "peak_source": "%s bf16 sustained x %.1f (nominal TF32 : bf16 ratio)" % (peaks["source"], TF32_OVER_BF16_NOMINAL),
+                     "frac": tflops(ctr["k_nn"]["tensor_flops"], nn_ms) / tf32_peak,
+                     "note": "three TF32 products per term (3xTF32) are counted as executed; latency-bound at 128-atom tiles, "
+                             "not part of the FP32 aggregate"}
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
-                "frac_is": "frac_model: algorithmic flops of the frozen work model / live time / nominal peak; "
-                           "executed_frac (ncu-counted FP32 flops / live time / nominal peak) is the north_star's evidence",
-                "frac_model": achieved / FP32_PEAK_NOMINAL_TFLOPS,
+                "frac_is": ("executed: ncu-counted FP32 flops per launch / live launch time / nominal peak (the north_star's "
+                            "evidence); frac_model beside it is the frozen algorithmic work model of SURVEY 8(d)") if ctr else
+                           "frac_model: algorithmic flops of the frozen work model / live time / nominal peak (no ncu counters "
+                           "for this workload)",
+                "achieved_model": achieved_model, "frac_model": achieved_model / FP32_PEAK_NOMINAL_TFLOPS,
                 "executed_flops_per_launch": ctr[dom]["executed_flops"] if ctr else None,
                 "executed_frac": frac_of_peak(ctr[dom]["executed_flops"], dom_ms) if ctr else None,
                 "traffic": ctr[dom]["dram_bytes"] if ctr else None,
-                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, " + NCU_COUNTERS_SOURCE,
+                "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, " + NCU_COUNTERS["source"],
+                "counters_source": NCU_COUNTERS["source"], "counters_commit": NCU_COUNTERS["captured_at_commit"],
+                "counters_stale": bool(ctr) and NCU_COUNTERS["csrc_sha256"] != digest, "csrc_sha256": digest,
                 "peak_source": "nominal FP32 FMA: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "fma_loop_measured_tflops": fma_measured, "frac_of_measured_fma_loop": achieved / fma_measured if fma_measured else None,
                 "ms_per_launch": dom_ms, "algorithmic_flops_per_launch": dom_flops,
-                "per_kernel": {k: {"ms": v[0], "tflops": v[1] / (v[0] * 1e-3) / 1e12 if v[0] > 0 else 0.0,
-                                   "frac": frac_of_peak(v[1], v[0]), "frac_model": frac_of_peak(v[1], v[0]),
+                "per_kernel": {k: {"ms": v[0], "tflops_model": tflops(v[1], v[0]),
+                                   "frac": frac_of_peak(ctr[k]["executed_flops"], v[0]) if ctr else frac_of_peak(v[1], v[0]),
+                                   "frac_model": frac_of_peak(v[1], v[0]),
                                    "executed_flops_per_launch": ctr[k]["executed_flops"] if ctr else None,
                                    "executed_frac": frac_of_peak(ctr[k]["executed_flops"], v[0]) if ctr else None,
                                    "tensor_flops_per_launch": ctr[k].get("tensor_flops") if ctr else None,
+                                   "in_fp32_aggregate": k in fp32_kernels,
                                    "dram_bytes_per_launch": ctr[k]["dram_bytes"] if ctr else None}
                                for k, v in kernels.items()},
-                "all_fp32_stages": {"ms": fp32_ms, "algorithmic_flops": fp32_flops,
-                                    "tflops": fp32_flops / (fp32_ms * 1e-3) / 1e12,
-                                    "frac": frac_of_peak(fp32_flops, fp32_ms), "frac_model": frac_of_peak(fp32_flops, fp32_ms),
+                "all_fp32_stages": {"kernels": fp32_kernels, "ms": fp32_ms, "algorithmic_flops": fp32_flops,
+                                    "tflops_model": tflops(fp32_flops, fp32_ms),
+                                    "frac": frac_of_peak(exe_flops, fp32_ms) if exe_flops else frac_of_peak(fp32_flops, fp32_ms),
+                                    "frac_model": frac_of_peak(fp32_flops, fp32_ms),
                                     "executed_flops": exe_flops,
-                                    "executed_frac": frac_of_peak(exe_flops, fp32_ms) if exe_flops else None}}
-    peaks = load_peaks()
+                                    "executed_frac": frac_of_peak(exe_flops, fp32_ms) if exe_flops else None},
+                "nn_tensor": nn_tensor}
     mesh_bytes = float(np.prod(w.es.grid)) * 8.0
     fft_bytes = 3 * 3 * 2 * mesh_bytes - float(np.prod(w.es.grid)) * 4.0   # 3 transforms x 3 passes x (read + write)
     pppm = {"stage": "reciprocal (spread + 3 FFTs + influence + gather)", "bound": "hbm", "ms": per_eval["reciprocal"],
@@ -386,10 +438,11 @@ def main():
     pppm["frac"] = pppm["achieved"] / pppm["peak"]
     pppm["frac_is"] = "frac_model: the survey's 3-pass byte model (2.4 GB at 256^3) / live stage time / measured copy peak"
     pppm["frac_model"] = pppm["frac"]
-    pppm["dram_bytes_measured"] = NCU_PPPM_DRAM_BYTES_CONFIG4 if full4 else None
-    pppm["frac_measured_bytes"] = (NCU_PPPM_DRAM_BYTES_CONFIG4 / (pppm["ms"] * 1e-3) / 1e9 / pppm["peak"]
+    pppm["dram_bytes_measured"] = NCU_COUNTERS["pppm_dram_bytes"] if full4 else None
+    pppm["frac_measured_bytes"] = (NCU_COUNTERS["pppm_dram_bytes"] / (pppm["ms"] * 1e-3) / 1e9 / pppm["peak"]
                                    if (full4 and pppm["ms"] > 0) else None)
-    pppm["traffic_source"] = "ncu dram__bytes_read.sum + dram__bytes_write.sum over the stage's kernels, " + NCU_COUNTERS_SOURCE
+    pppm["traffic"] = pppm["dram_bytes_measured"]
+    pppm["traffic_source"] = "ncu dram__bytes_read.sum + dram__bytes_write.sum over the stage's kernels, " + NCU_COUNTERS["source"]
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----------
     # Every call gets its own positions: the start structure displaced along the initial velocities (0.5 fs per call), so
@@ -449,6 +502,13 @@ def main():
         v, dt, cores, sample, _ = time_oracle(args.cpu_sample_side, 1, 0, workload=w if same else None)
         cpu = {"value": v, "unit": "atom-steps/s", "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
 
+    extra_legs = None
+    if args.optional_legs and rank == 0:
+        h.destroy(); h2.destroy()
+        del vir_t, chg_t
+        torch.cuda.empty_cache()
+        extra_legs = optional_legs(Q, torch, w, args, dev)
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": "atom-steps/s", "n_gpus": world, "steps": K, "warmup": Wm,
@@ -470,9 +530,62 @@ def main():
             "md_sanity": md_sanity,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
+        if extra_legs is not None:
+            line["optional_legs"] = extra_legs
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def optional_legs(Q, torch, w, args, dev, evals=20, warm=5):
+    """ms per evaluation (CUDA events around `evals` qnep_compute calls at fixed positions, lists rebuilt every
+    args.rebuild_every calls, all four outputs) of the workload as it is and with each optional term of SURVEY 8(f):
+    per-atom virial (qnep_compute_atom_virial), ZBL core, the same fractional coordinates in a tilted cell, NEP4's 4-/5-body
+    descriptors (35-descriptor model on the scalar network kernel).  One handle at a time."""
+    from dataclasses import replace
+
+    def leg(wl, atom_virial=False):
+        h = Q.from_workload(wl)
+        h.set_neighbor_policy(args.skin, args.rebuild_every)
+        h.set_pppm_kernels(args.pppm_kernels)
+        pos = torch.tensor(wl.pos, dtype=torch.float64, device=dev)
+        types = torch.tensor(wl.types, dtype=torch.int32, device=dev)
+        out = {}
+
+        def one():
+            if atom_virial:
+                h.compute_atom_virial(pos, types, wl.box)
+            else:
+                h.compute(pos, types, wl.box, want=Q.WANT_ALL, out=out, check=False)
+
+        for k in range(warm + 1):
+            try:
+                one()
+                h.check()
+            except Q.QnepError as err:
+                if err.code != Q.QNEP_ERR_NEIGHBOR_OVERFLOW:
+                    raise
+        h.set_neighbor_policy(args.skin, args.rebuild_every)          # the timed calls start with a rebuild
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for k in range(evals):
+            one()
+        b.record()
+        torch.cuda.synchronize()
+        h.check()
+        h.destroy()
+        return a.elapsed_time(b) / evals
+
+    legs = {"as_configured": leg(w), "atom_virial": leg(w, atom_virial=True), "triclinic_cell": leg(I.triclinic_variant(w))}
+    if w.model.n_types == 2:
+        legs["zbl_core"] = leg(replace(w, zbl=(0.35, 0.7, (8.0, 1.0))))
+    key = {2: "config1_45body", 4: "config2_45body"}.get(w.model.n_types)
+    if key:
+        legs["higher_body_terms"] = leg(I.with_higher_body_terms(w, key))
+    return {"ms_per_eval": legs, "evals": evals, "unit": "ms",
+            "note": "qnep_compute at fixed positions, all four outputs, neighbour rebuild every %d calls; atom_virial through "
+                    "qnep_compute_atom_virial (synchronises per call)" % args.rebuild_every}
 
 
 def replace_masses(w, masses):

@@ -1,12 +1,17 @@
 /*
  * qnep.h -- C ABI of the B200-native qNEP force evaluation (arXiv 2601.19034).
  *
- * One call, qnep_compute(), evaluates for given positions, species and a periodic box
- * the total energy (Eq. 4), forces (Eq. 11), total virial (Eq. 12 + Eq. 22),
- * the neutralised partial charges (Eq. 1 second output node, Eq. 33) and, on request,
- * the per-ion Born effective charge tensor (Eq. 28).  Every step runs in hand-written
- * CUDA kernels for sm_100a inside this library; there is no CPU fallback, no cuFFT and
- * no other library on the path.
+ * One call, qnep_compute(), evaluates for given positions, species and a periodic cell of any
+ * shape (orthorhombic or triclinic, PAPER.md :104) the total energy (Eq. 4), forces (Eq. 11),
+ * total virial (Eq. 12 + Eq. 22), the neutralised partial charges (Eq. 1 second output node,
+ * Eq. 33) and, on request, the per-ion Born effective charge tensor (Eq. 28).  Beside it:
+ * qnep_compute_atom_virial (per-atom virial, Eq. 12 / 20 / 39), qnep_compute_host (host buffers),
+ * qnep_md_run (velocity-Verlet driver, optionally with virial and charges every step),
+ * qnep_response (Eq. 29-30), qnep_set_zbl (optional ZBL core), NEP4's 4-/5-body descriptors
+ * (qnep_model_desc.l_max_4b / l_max_5b), the Ewald / PPPM selector, and
+ * qnep_neutralise_noalloc (Eq. 33 for callers that may not allocate device memory).  Every step
+ * runs in hand-written CUDA kernels for sm_100a inside this library; there is no CPU fallback,
+ * no cuFFT and no other library on the path.
  *
  * Conventions
  *   - every function returns QNEP_OK (0) or a negative QNEP_ERR_* code; no C++ exception
@@ -31,6 +36,16 @@ extern "C" {
 #endif
 
 typedef struct qnep_handle qnep_handle; /* opaque */
+
+/*
+ * Version of this boundary: raised whenever a struct below changes size or layout or an entry point changes its signature
+ * (1: round-1 header; 2: qnep_model_desc grew by l_max_4b, l_max_5b; 3: qnep_neutralise_noalloc, qnep_abi_version).  The structs
+ * carry no size field, so a caller built against another header would hand qnep_create a struct of the wrong size: compare
+ * qnep_abi_version() (what the loaded library was built with) with QNEP_ABI_VERSION (what the caller was compiled with)
+ * once after loading.  Needs no device.
+ */
+#define QNEP_ABI_VERSION 3
+int qnep_abi_version(void);
 
 enum {
     QNEP_OK = 0,
@@ -239,7 +254,8 @@ int qnep_set_pppm_kernels(qnep_handle *h, int32_t mode);
  *   mode 1: warp-level mma.sync m16n8k8 TF32, same split (0.338 ms: the legacy path peaks at 277 TFLOP/s TF32 on B200).
  *   mode 0: packed FP32 FMAs, two atoms per thread (0.310 ms); the default when the 4-/5-body terms are on (one atom per
  *           thread, scalar) or n_neurons > 128.
- * Errors: INVALID_ARG, UNSUPPORTED (modes 1, 2 with the 4-/5-body terms on; mode 2 with n_neurons > 128).
+ * Errors: INVALID_ARG, UNSUPPORTED (modes 1, 2 with the 4-/5-body terms on; mode 2 with n_neurons > 128; mode 1 when the weight
+ *         tables of all species, n_types x (2 x 36 + 3) x n_neurons floats, exceed 200 KB of shared memory).
  */
 int qnep_set_nn_kernel(qnep_handle *h, int32_t mode);
 

@@ -38,7 +38,8 @@ ABI_SYMBOLS = ["qnep_create", "qnep_set_electrostatics", "qnep_set_neighbor_poli
                "qnep_compute", "qnep_compute_atom_virial", "qnep_compute_host", "qnep_md_run", "qnep_md_set_outputs", "qnep_md_reset", "qnep_set_md_graphs", "qnep_set_pppm_kernels", "qnep_check", "qnep_get_timings",
                "qnep_profile_reset", "qnep_profile_sum", "qnep_kernel_launches", "qnep_response", "qnep_neighbor_stats",
                "qnep_fma_peak", "qnep_set_zbl", "qnep_set_nn_kernel",
-               "qnep_debug_copy", "qnep_neutralise_noalloc", "qnep_destroy", "qnep_last_error"]
+               "qnep_debug_copy", "qnep_neutralise_noalloc", "qnep_abi_version", "qnep_destroy", "qnep_last_error"]
+ABI_VERSION = 3                      # QNEP_ABI_VERSION of the include/qnep.h these ctypes mirrors were written against
 NOALLOC_MAX_ATOMS = 4194304          # QNEP_NOALLOC_MAX_ATOMS of include/qnep.h
 
 
@@ -72,6 +73,11 @@ def load_library():
         raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2601_19034_b200.build` "
                           "(there is no CPU fallback)")
     lib = C.CDLL(LIB_PATH)
+    lib.qnep_abi_version.restype = C.c_int
+    lib.qnep_abi_version.argtypes = []
+    if lib.qnep_abi_version() != ABI_VERSION:
+        raise ImportError(f"{LIB_PATH} was built from a header of ABI version {lib.qnep_abi_version()}, this binding mirrors "
+                          f"version {ABI_VERSION}: rebuild with `python -m paper_2601_19034_b200.build --force`")
     vp, i64, i32, u32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_uint32, C.c_double
     lib.qnep_create.restype = C.c_int
     lib.qnep_create.argtypes = [C.POINTER(qnep_model_desc), vp, C.c_size_t, C.POINTER(qnep_es_desc), C.POINTER(vp)]
@@ -323,7 +329,9 @@ class QNEP:
         self._ok(self._lib.qnep_set_pppm_kernels(self._h, int(mode)))
 
     def set_nn_kernel(self, mode: int):
-        """0: packed FP32 FMAs (default); 1: tensor cores (mma.sync TF32, 3xTF32 split)."""
+        """2 (default for the 25-descriptor model with n_neurons <= 128): tcgen05 tensor cores, 3xTF32 split; 1: mma.sync
+        TF32, same split; 0: packed FP32 FMAs (the default otherwise).  UNSUPPORTED: modes 1, 2 with the 4-/5-body terms on,
+        mode 2 with n_neurons > 128, mode 1 when n_types x n_neurons needs more than 200 KB of shared memory."""
         self._ok(self._lib.qnep_set_nn_kernel(self._h, int(mode)))
 
     def set_zbl(self, zbl):

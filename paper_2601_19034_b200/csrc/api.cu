@@ -714,6 +714,14 @@ int qnep_set_nn_kernel(qnep_handle* h, int32_t mode)
     if (!h) return QNEP_ERR_INVALID_ARG;
     if (mode < 0 || mode > 2) { h->err = "qnep_set_nn_kernel: mode must be 0 (FP32 FMA), 1 (mma.sync) or 2 (tcgen05)"; return QNEP_ERR_INVALID_ARG; }
     if (mode == 2 && h->model.n_neurons > 128) { h->err = "qnep_set_nn_kernel: the tcgen05 kernel takes at most 128 hidden neurons"; return QNEP_ERR_UNSUPPORTED; }
+    if (mode == 1) {
+        // k_nn_mma keeps the split weight tables of all species in shared memory: T (2 HP 36 + 3 HP) floats, opt-in limit 200 KB
+        const size_t HP = (size_t)(h->model.n_neurons + 7) / 8 * 8;
+        if (sizeof(float) * (size_t)h->model.n_types * (2 * HP * 36 + 3 * HP) > 200 * 1024) {
+            h->err = "qnep_set_nn_kernel: the mma.sync kernel's weight tables (n_types x n_neurons) exceed 200 KB of shared memory";
+            return QNEP_ERR_UNSUPPORTED;
+        }
+    }
     if (mode != 0 && h->ND != QNEP_NDESC) { h->err = "qnep_set_nn_kernel: the tensor-core kernel takes the 25-descriptor model only"; return QNEP_ERR_UNSUPPORTED; }
     h->nn_tensor = mode;
     h->ws_generation += 1;      // captured MD graphs hold the old kernel
@@ -962,6 +970,8 @@ int qnep_response(qnep_handle* h, int64_t n_atoms, const double* bec_dev, const 
 }
 
 int64_t qnep_kernel_launches(const qnep_handle* h) { return h ? h->launches : 0; }
+
+int qnep_abi_version(void) { return QNEP_ABI_VERSION; }
 
 int qnep_neighbor_stats(qnep_handle* h, double out[6])
 {

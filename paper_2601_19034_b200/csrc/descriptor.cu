@@ -175,7 +175,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // a2: one walk over the skin list: the exact lists of this step and the radial descriptors
 //   live radial entry : the skin-list word (sorted index | cell offset of the image << 26), type-major like the skin list
 //                       (warp-tiled int4 layout); lvRend[t][p] = end of the species-t segment
-//   live angular pair : (dx, dy, dz, bits(sorted index | type << 27))
+//   live angular pair : (dx, dy, dz, bits(sorted index | type << 26: QNEP_NL_SHIFT; index limit 2^26))
 // The kernel is bound by L1 wavefronts (gathers of 16 bytes from ~15 lines per warp instruction, the queue and the
 // shift table in shared memory) and by issue slots, so both phases are kept to the instructions they need:
 //   phase 1, per SKIN entry (all lanes busy): list word -> position gather -> distance test; accepted entries are
@@ -1034,7 +1034,9 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         // 3. activation per chunk of 16 neurons, backward products
         float U = 0.f, q = 0.f;
-        for (int c = 0; c < HP / 16 && ok; ++c) {
+        // (after a timed-out wait the chunk loop still runs to its end: every warp keeps its named-barrier arrivals, so a
+        // thread that saw the time-out and one that did not cannot strand each other; the later waits return at once)
+        for (int c = 0; c < HP / 16; ++c) {
             float z[16];
             tmem_ld16(tbase + 16 * c, z);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -1051,7 +1053,7 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
             // two staging buffers of 32 columns (chunk parity): buffer c & 1 is free once the products of chunk c - 2 have
             // completed, so the activation runs up to two chunks ahead of the tensor core
             if (c > 1) {
-                ok = mbar_wait(bar + 8 + 8 * (c & 1), phc[c & 1]);
+                ok = ok && mbar_wait(bar + 8 + 8 * (c & 1), phc[c & 1]);
                 phc[c & 1] ^= 1;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             }
@@ -1106,7 +1108,8 @@ k_nn_umma(int64_t N, int T, int H, int HP /* H rounded up to 16 */, int nn_strid
             }
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();                               // all TMEM reads of this tile are done before the next tile overwrites
+        ok = __syncthreads_and(ok);                    // all TMEM reads of this tile are done before the next tile overwrites;
+                                                       // the whole block leaves the tile loop together after a time-out
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }
     if (!ok) atomicOr(&flags[FLAG_TENSOR_TIMEOUT], 1);

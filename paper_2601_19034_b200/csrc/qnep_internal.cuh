@@ -200,7 +200,7 @@ struct qnep_handle {
     int4* d_lvR = nullptr;           // warp-tiled [capLR / 4] int4 per atom: live radial list of this step (r < rc_r)
     int* d_nlvR = nullptr;           // [N]
     int* d_lvRend = nullptr;         // [T][N] end of the species-t segment of the (type-major) live radial list
-    float4* d_lvA = nullptr;         // warp-tiled [capLA] float4 per atom: live angular pairs (dx, dy, dz, bits(j | tj << 27))
+    float4* d_lvA = nullptr;         // warp-tiled [capLA] float4 per atom: live angular pairs (dx, dy, dz, bits(j | tj << 26))
     int* d_nlvA = nullptr;           // [N]
     float* d_D = nullptr;            // [25][N]
     float* d_A = nullptr;            // [5*24][N]

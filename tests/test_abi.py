@@ -28,6 +28,12 @@ def test_header_symbols_are_exported(lib):
         assert hasattr(lib, name), name
 
 
+def test_abi_version_matches_header(lib):
+    header = open(os.path.join(ROOT, "include", "qnep.h")).read()
+    (v,) = re.findall(r"#define QNEP_ABI_VERSION (\d+)", header)
+    assert int(v) == Q.ABI_VERSION == lib.qnep_abi_version()
+
+
 def test_struct_layout_matches_header():
     # the ctypes mirrors must have the C layout (8-byte aligned doubles)
     assert C.sizeof(Q.qnep_model_desc) == 80          # 72 bytes of round 1 + l_max_4b, l_max_5b

@@ -613,6 +613,18 @@ def test_unsupported_inputs(torch):
     with pytest.raises(Q.QnepError) as ei:
         h.compute(pos, types, small)
     assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED
+    h.destroy()
+    # the mma.sync network kernel keeps the weight tables of all species in shared memory: 4 species x 200 neurons do not
+    # fit its 200 KB and the selector must say so (it used to surface as a failed launch); 2 x 200 fit and must still be right
+    wide = I.ModelDesc(n_types=4, n_neurons=200, mode=w.model.mode)
+    hw = Q.QNEP(wide, I.random_params(wide, 5), w.es)
+    with pytest.raises(Q.QnepError) as ei:
+        hw.set_nn_kernel(1)
+    assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED and "shared memory" in str(ei.value)
+    with pytest.raises(Q.QnepError) as ei:
+        hw.set_nn_kernel(2)                       # tcgen05 kernel: at most 128 neurons
+    assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED
+    hw.destroy()
 
 
 def test_host_buffer_entry_point(torch, oracle):
