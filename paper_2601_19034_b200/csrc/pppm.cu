@@ -590,11 +590,23 @@ k_fft_x_virial(int n0, int n1, int n2, float2* __restrict__ M1, float2* __restri
     }
 }
 
+// Layout of the (Phi, E) mesh read by k_gather.  QNEP_FIELD_BRICKS = 0: [x][y][z] rows; a 5-point z run of float4 (80 B)
+// straddles a 128-byte line half the time, 37.5 line visits per 5^3 stencil.  QNEP_FIELD_BRICKS = 1: 2 x 2 x 2 bricks of
+// float4, one brick = one 128-byte line, point (x, y, z) at 8 * brick + (x & 1, y & 1, z & 1): five consecutive points of an
+// axis always fall into three bricks, so a stencil visits 27 lines, each read whole by the eight lanes of an atom's group.
+#ifndef QNEP_FIELD_BRICKS
+#define QNEP_FIELD_BRICKS 0
+#endif
+__device__ __forceinline__ int field_brick_index(int x, int y, int z, int n1, int n2)
+{
+    return (((((x >> 1) * (n1 >> 1) + (y >> 1)) * (n2 >> 1)) + (z >> 1)) << 3) | ((x & 1) << 2) | ((y & 1) << 1) | (z & 1);
+}
+
 // ---- last inverse pass along z: M1, M2 -> interleaved real fields (Phi, E_x, E_y, E_z) -------------------
 template <int R1, int R2>
 __global__ void __launch_bounds__(Split<R1, R2>::THREADS, Split<R1, R2>::THREADS >= 256 ? QNEP_FFT_ZF_MINB : 1)
 k_fft_z_fields(const float2* __restrict__ M1, const float2* __restrict__ M2, float4* __restrict__ field,
-               const float2* __restrict__ twg)
+               const float2* __restrict__ twg, int n1)
 {
     using S = Split<R1, R2>;
     extern __shared__ __align__(16) float2 smem[];
@@ -618,7 +630,12 @@ k_fft_z_fields(const float2* __restrict__ M1, const float2* __restrict__ M2, flo
 #pragma unroll
         for (int k1 = 0; k1 < R2; ++k1) {
             const float2 a = v[d * R2 + k1], c = w[d * R2 + k1];
+#if QNEP_FIELD_BRICKS
+            const int line = blockIdx.x * LINES + b, x = line / n1, y = line - x * n1, z = (u + S::TPL * d) + R1 * k1;
+            field[field_brick_index(x, y, z, n1, S::N)] = make_float4(a.x, a.y, c.x, c.y);
+#else
             field[base + (u + S::TPL * d) + R1 * k1] = make_float4(a.x, a.y, c.x, c.y);
+#endif
         }
 }
 
@@ -643,6 +660,9 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
     __shared__ float s_w[3][5][GATHER_BLOCK];
     __shared__ int s_i[3][5][GATHER_BLOCK];       // x: index * n1 * n2, y: index * n2, z: index
     __shared__ float s_out[4][GATHER_BLOCK];
+#if QNEP_FIELD_BRICKS
+    __shared__ int s_first[3][GATHER_BLOCK];      // wrapped index of the first stencil point per axis
+#endif
     const int t = threadIdx.x;
     const int64_t p0 = blockIdx.x * (int64_t)GATHER_BLOCK;
     {
@@ -659,6 +679,9 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
             s_i[1][i][t] = idx[1][i] * g.grid[2];
             s_i[2][i][t] = idx[2][i];
         }
+#if QNEP_FIELD_BRICKS
+        s_first[0][t] = idx[0][0]; s_first[1][t] = idx[1][0]; s_first[2][t] = idx[2][0];
+#endif
     }
     __syncthreads();
     const int c = t & (GATHER_GROUP - 1), grp = t / GATHER_GROUP;
@@ -667,7 +690,45 @@ k_gather(int64_t N, Geometry g, const float4* __restrict__ mfrac, const int* __r
     for (int it = 0; it < GATHER_GROUP; ++it) {
         const int al = it * NGRP + grp;
         float ph = 0.f, ex = 0.f, ey = 0.f, ez = 0.f;
+#if QNEP_FIELD_BRICKS
+        {
+            // lane c owns corner (dx, dy, dz) of every brick: stencil slot o = 2 k + d - parity along each axis (weight 0 outside 0..4)
+            const int dl[3] = {(c >> 2) & 1, (c >> 1) & 1, c & 1};
+            const int hb[3] = {g.grid[0] >> 1, g.grid[1] >> 1, g.grid[2] >> 1};
+            float wl[3][3];
+            int bo[3][3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const int i0 = s_first[a][al], par = i0 & 1, b0 = i0 >> 1;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int o = 2 * k + dl[a] - par;
+                    wl[a][k] = (o >= 0 && o < 5) ? s_w[a][min(max(o, 0), 4)][al] : 0.f;
+                    int bk = b0 + k;
+                    bk = bk >= hb[a] ? bk - hb[a] : bk;
+                    bo[a][k] = a == 0 ? bk * hb[1] * hb[2] : (a == 1 ? bk * hb[2] : bk);
+                }
+            }
+            const float4* fc = field + c;
+#pragma unroll
+            for (int kx = 0; kx < 3; ++kx)
+#pragma unroll
+                for (int ky = 0; ky < 3; ++ky) {
+                    const float wxy = wl[0][kx] * wl[1][ky];
+                    const int oxy = bo[0][kx] + bo[1][ky];
+#pragma unroll
+                    for (int kz = 0; kz < 3; ++kz) {
+                        const float w = wxy * wl[2][kz];
+                        const float4 f = fc[(oxy + bo[2][kz]) << 3];
+                        ph = fmaf(w, f.x, ph); ex = fmaf(w, f.y, ex);
+                        ey = fmaf(w, f.z, ey); ez = fmaf(w, f.w, ez);
+                    }
+                }
+        }
+        if (false) {
+#else
         if (c < 5) {
+#endif
             const int zc = s_i[2][cc][al];
             float wy[5];
             int oy[5];
@@ -768,7 +829,7 @@ int qnep_setup_pppm(qnep_handle* h)
     if (ng != h->ngrid) {
         cudaFree(h->d_mesh); cudaFree(h->d_cm1); cudaFree(h->d_cm2); cudaFree(h->d_field);
         cudaFree(h->d_cm3);      // allocated on demand by qnep_launch_pppm_atom_virial with the mesh size of that time
-        h->d_mesh = nullptr; h->d_cm1 = nullptr; h->d_cm2 = nullptr; h->d_field = nullptr; h->d_cm3 = nullptr;
+        h->d_mesh = nullptr; h->d_cm1 = nullptr; h->d_cm2 = nullptr; h->d_field = nullptr; h->d_cm3 = nullptr; h->cm3_ngrid = 0;
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_mesh, sizeof(float) * ng));
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm1, sizeof(float2) * ng));
         QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm2, sizeof(float2) * ng));
@@ -922,7 +983,7 @@ int qnep_launch_pppm(qnep_handle* h, bool virial, cudaStream_t s)
         using S = Split<R1, R2>;
         const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
         note(allow_smem(k_fft_z_fields<R1, R2>, smem));
-        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm1, h->d_cm2, h->d_field, tw2);
+        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm1, h->d_cm2, h->d_field, tw2, n1);
     });
     // 5. gather
     const int nbg = (int)((N + GATHER_BLOCK - 1) / GATHER_BLOCK);
@@ -945,7 +1006,11 @@ int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s)
     const float2* tw0 = h->d_twiddle;
     const float2* tw1 = h->d_twiddle + FFT_MAXN;
     const float2* tw2 = h->d_twiddle + 2 * FFT_MAXN;
-    if (!h->d_cm3) QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm3, sizeof(float2) * h->ngrid));
+    if (!h->d_cm3 || h->cm3_ngrid != h->ngrid) {         // first use, or the mesh changed size since (qnep_set_electrostatics)
+        cudaFree(h->d_cm3); h->d_cm3 = nullptr; h->cm3_ngrid = 0;
+        QNEP_CUDA_OK(h, cudaMalloc(&h->d_cm3, sizeof(float2) * h->ngrid));
+        h->cm3_ngrid = h->ngrid;
+    }
     cudaError_t ce = cudaSuccess;
     auto note = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
     const Geometry& G = h->geo;
@@ -1001,9 +1066,9 @@ int qnep_launch_pppm_atom_virial(qnep_handle* h, cudaStream_t s)
         using S = Split<R1, R2>;
         const size_t smem = sizeof(float2) * (LINES * S::LP + S::N);
         note(allow_smem(k_fft_z_fields<R1, R2>, smem));
-        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm1, h->d_cm2, h->d_field, tw2);
+        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm1, h->d_cm2, h->d_field, tw2, n1);
         k_gather<true><<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, 0, nullptr, nullptr, r1, h->d_Wat);
-        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm3, h->d_cm3, h->d_field, tw2);
+        k_fft_z_fields<R1, R2><<<(unsigned)((int64_t)n0 * n1 / LINES), S::THREADS, smem, s>>>(h->d_cm3, h->d_cm3, h->d_field, tw2, n1);
         k_gather<true><<<nbg, GATHER_BLOCK, 0, s>>>(N, h->geo, h->d_mfrac, h->d_mi0, h->d_cmi, h->d_q, h->d_field, 0, nullptr, nullptr, r2, h->d_Wat);
     });
     h->launches += 9;

@@ -246,6 +246,7 @@ struct qnep_handle {
     float2* d_cm1 = nullptr;         // complex meshes
     float2* d_cm2 = nullptr;
     float2* d_cm3 = nullptr;         // third complex mesh: per-atom virial pass only (allocated on first use)
+    int64_t cm3_ngrid = 0;           // mesh points d_cm3 was allocated for (checked against ngrid before every use)
     float4* d_field = nullptr;       // [Nx][Ny][Nz] (Phi, E_x, E_y, E_z)
     float* d_gtab = nullptr;         // 1-D influence tables: per axis N entries of (A_alpha) then k_alpha
     float2* d_twiddle = nullptr;     // per axis twiddles

@@ -78,6 +78,26 @@ def test_noalloc_matches_existing_path_on_calls_in_a_row(lib):
     assert torch.equal(outs[0], outs[2])                        # the same input gives the same bits, whatever ran in between
 
 
+@pytest.mark.gpu
+def test_noalloc_at_its_maximum_size_and_ragged_tails(lib):
+    """Exactly QNEP_NOALLOC_MAX_ATOMS atoms (all 4096 partial sums in use), then sizes around the 1024-atom block and the
+    256-thread edges, against the definition of Eq. 33 evaluated with torch in fp64 on the same device."""
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    gen = torch.Generator(device="cuda").manual_seed(20260119034)
+    for n in (Q.NOALLOC_MAX_ATOMS, 1, 255, 256, 257, 1023, 1024, 1025, 4097, Q.NOALLOC_MAX_ATOMS - 1):
+        q_raw = torch.randn(n, dtype=torch.float64, device="cuda", generator=gen) * 0.4
+        q_total = -1.0 if n % 2 else 2.0
+        got = Q.neutralise_noalloc(q_raw, q_total)
+        want = q_raw + (q_total - q_raw.sum()) / n
+        d = float((got - want).abs().max())
+        assert d <= 1e-12, (n, d)                                   # both in fp64; only the order of the sum differs
+        assert abs(float(got.sum()) - q_total) <= 1e-9
+    with pytest.raises(Q.QnepError) as ei:                          # one atom more than the built-in array serves
+        Q.neutralise_noalloc(torch.zeros(Q.NOALLOC_MAX_ATOMS + 1, dtype=torch.float64, device="cuda"), 0.0)
+    assert ei.value.code == Q.QNEP_ERR_UNSUPPORTED and "QNEP_NOALLOC_MAX_ATOMS" in str(ei.value)
+
+
 def test_noalloc_rejects_bad_sizes_before_touching_the_gpu(lib):
     # the argument checks come before any CUDA call, so this runs without a device; the pointers are never dereferenced
     msg = C.create_string_buffer(512)
