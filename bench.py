@@ -74,18 +74,18 @@ def whole_job_value(n_atoms, steps, world, ms_total):
 # "counters_stale": true when the sources have changed since (re-capture, then update both).
 NCU_COUNTERS = {
     "source": "profiles/r03_ncu_full.txt",
-    "captured_at_commit": "0e22918",
-    "csrc_sha256": "d47cd76d95f9a5a5ed1dba87aa5239e2df54bb6074764d00a6444d09078c9d05",
+    "captured_at_commit": "5825272",
+    "csrc_sha256": "f53fb14d5da0a24d1288e2b1c662d037407f3b4180d42560ee695bb416a014cc",
     "kernels": {
-        "k_pairs": {"dram_bytes": 1.594e9, "executed_flops": 7.975e9},
+        "k_pairs": {"dram_bytes": 1.596e9, "executed_flops": 7.975e9},
         "k_desc_angular": {"dram_bytes": 1.032e9, "executed_flops": 1.151e10},
         # k_nn_umma: the contraction runs on the tensor cores (42 tcgen05.mma per 128-atom tile, 3xTF32: 4.74e10 tensor flops
         # per launch); executed_flops is its FP32 part (activation, splits)
         "k_nn": {"dram_bytes": 0.2644e9, "executed_flops": 1.188e9, "tensor_flops": 4.74e10},
         "k_force_angular": {"dram_bytes": 1.451e9, "executed_flops": 2.590e10},
-        "k_force_radial": {"dram_bytes": 0.6777e9, "executed_flops": 1.349e10},
+        "k_force_radial": {"dram_bytes": 0.6782e9, "executed_flops": 1.349e10},
     },
-    "pppm_dram_bytes": 1.916e9,          # spread + five FFT kernels + gather, same capture
+    "pppm_dram_bytes": 1.915e9,          # spread + five FFT kernels + gather, same capture
 }
 TF32_OVER_BF16_NOMINAL = 0.5             # dense tensor peak of kind::tf32 relative to bf16 (B200_PROFILING.md nominal ratio)
 
